@@ -1,0 +1,561 @@
+// pixreco_api.cu — the C-ABI boundary of include/pixreco.h: handle, event slots, acquire/produce.
+//
+// pr_acquire is the body of the paper's acquire() with a ScopedContext around it (PAPER.md
+// L76, L94, L100): set the device, take buffers from the caching pool (L88-90), enqueue copies
+// and kernels on the event's own stream (L82-86), record the completion event and queue the
+// completion callback (L94) — and return.  pr_produce is produce(): it only reads what the
+// callback / event already made visible.  No blocking CUDA call appears in either (L31 fn.1).
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pixreco.h"
+#include "kernels.cuh"
+#include "pool.hpp"
+
+using namespace pixreco;
+
+namespace {
+enum SlotState { kIdle = 0, kInFlight = 1, kDone = 2 };
+constexpr uint32_t kMaxBatch = 4096;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+}  // namespace
+
+struct pr_handle {
+  pr_config cfg{};
+  Geom geom{};
+  float *dGain = nullptr, *dPed = nullptr;
+  CachingPool *devPool = nullptr, *hostPool = nullptr;
+  int smCount = 0, clusterBlocksPerSM = 1;
+  size_t clusterSmem = 0;
+  std::mutex mu;
+  std::vector<pr_event*> slots;
+  std::atomic<uint64_t> evAcquired{0}, evProduced{0}, words{0}, digis{0}, clusters{0}, launches{0}, memcpys{0}, callbacks{0};
+  std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
+  std::atomic<int> sticky{0};
+  std::string lastCuda;
+};
+
+struct SubEvent {            // host-side record of one event of the slot's batch
+  pr_input in{};
+  uint32_t cap = 0;
+  EvDesc desc{};
+  // pinned mirrors (nullptr unless wanted)
+  pr_output hostViews{};
+};
+
+struct pr_event {
+  pr_handle* h = nullptr;
+  int state = kIdle;
+  cudaEvent_t done = nullptr;
+  cudaStream_t stream = nullptr;
+  uint32_t n = 0;
+  std::vector<SubEvent> sub;
+  // per-acquire pool blocks
+  void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr; void* itemTab = nullptr;
+  // persistent per-slot blocks (grown on demand)
+  void* ctl = nullptr; size_t ctlBytes = 0;
+  HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
+  int status = PR_OK;        // filled when completion is observed
+  pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
+};
+
+namespace {
+
+int cuda_fail(pr_handle* h, cudaError_t e, const char* what) {
+  if (h) {
+    std::lock_guard<std::mutex> g(h->mu);
+    h->lastCuda = std::string(what) + ": " + cudaGetErrorString(e);
+    h->sticky.store(1);
+  }
+  cudaGetLastError();
+  return PR_ERR_CUDA;
+}
+#define PR_CUDA(h, call)                                   \
+  do {                                                     \
+    cudaError_t e__ = (call);                              \
+    if (e__ != cudaSuccess) return cuda_fail((h), e__, #call); \
+  } while (0)
+
+// Carves arrays out of one slab; first pass (base == nullptr) only measures.
+struct Carver {
+  char* base; size_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <typename T> T* take(size_t count) {
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += align_up(count * sizeof(T), 256);
+    return p;
+  }
+};
+
+// Device slab of one sub-event.  `stage`: room for the H2D copy of the inputs.
+void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, uint32_t** stageWords, uint16_t** stageAdc) {
+  if (stage) { *stageWords = c.take<uint32_t>(cap); *stageAdc = c.take<uint16_t>(cap); }
+  d.module = c.take<u16>(cap); d.row = c.take<u16>(cap); d.col = c.take<u16>(cap); d.adcOut = c.take<u16>(cap);
+  d.wordIdx = c.take<u32>(cap); d.charge = c.take<float>(cap); d.label = c.take<u32>(cap); d.clus = c.take<int32_t>(cap);
+  d.errWord = c.take<u32>(cap); d.errIdx = c.take<u32>(cap);
+  d.modDigiStart = c.take<u32>(M + 4); d.modClusStart = c.take<u32>(M + 4);
+  d.clLabel = c.take<u32>(cap); d.clSize = c.take<u32>(cap); d.clModule = c.take<u16>(cap);
+  d.clCharge = c.take<float>(cap); d.clRow = c.take<float>(cap); d.clCol = c.take<float>(cap);
+  d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
+  d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
+  d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap);
+}
+
+void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M) {
+  if (want & PR_WANT_DIGIS) {
+    o.h_module = c.take<uint16_t>(cap); o.h_row = c.take<uint16_t>(cap); o.h_col = c.take<uint16_t>(cap);
+    o.h_adc = c.take<uint16_t>(cap); o.h_word_idx = c.take<uint32_t>(cap); o.h_mod_digi_start = c.take<uint32_t>(M + 4);
+  }
+  if (want & PR_WANT_CHARGE) o.h_charge = c.take<float>(cap);
+  if (want & PR_WANT_LABELS) { o.h_label = c.take<uint32_t>(cap); o.h_clus = c.take<int32_t>(cap); }
+  if (want & PR_WANT_CLUSTERS) {
+    o.h_cl_label = c.take<uint32_t>(cap); o.h_cl_size = c.take<uint32_t>(cap); o.h_cl_module = c.take<uint16_t>(cap);
+    o.h_cl_charge = c.take<float>(cap); o.h_cl_row = c.take<float>(cap); o.h_cl_col = c.take<float>(cap);
+    o.h_mod_clus_start = c.take<uint32_t>(M + 4);
+  }
+  if (want & PR_WANT_ERRORS) { o.h_err_word = c.take<uint32_t>(cap); o.h_err_idx = c.take<uint32_t>(cap); }
+}
+
+int status_to_code(uint32_t bits) {
+  if (bits & PR_STATUS_INPUT_ORDER) return PR_ERR_INPUT_ORDER;
+  if (bits & PR_STATUS_CAPACITY) return PR_ERR_CAPACITY;
+  return PR_OK;
+}
+
+// Runs on a CUDA-internal thread: translate device status into the code for done().
+void CUDART_CB trampoline(void* p) {
+  pr_event* ev = static_cast<pr_event*>(p);
+  int worst = PR_OK;
+  for (uint32_t k = 0; k < ev->n; ++k) {
+    int c = status_to_code(ev->hostCounters[k].status);
+    if (c < worst) worst = c;
+  }
+  ev->h->callbacks.fetch_add(1);
+  if (ev->doneFn) ev->doneFn(ev->doneUser, worst);
+}
+
+void release_blocks(pr_event* ev, bool completed) {
+  pr_handle* h = ev->h;
+  if (ev->devSlab) { h->devPool->free(ev->devSlab, ev->stream, completed); ev->devSlab = nullptr; }
+  if (ev->descDev) { h->devPool->free(ev->descDev, ev->stream, completed); ev->descDev = nullptr; }
+  if (ev->hostSlab) { h->hostPool->free(ev->hostSlab, ev->stream, completed); ev->hostSlab = nullptr; }
+  if (ev->descStage) { h->hostPool->free(ev->descStage, ev->stream, completed); ev->descStage = nullptr; }
+  if (ev->itemTab) { h->hostPool->free(ev->itemTab, ev->stream, completed); ev->itemTab = nullptr; }
+}
+
+int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
+  if (!ev || !ins || n == 0 || n > kMaxBatch) return PR_ERR_INVALID_ARG;
+  pr_handle* h = ev->h;
+  if (h->sticky.load()) return PR_ERR_CUDA;
+  if (ev->state != kIdle) return PR_ERR_BAD_STATE;
+  const uint32_t M = h->cfg.n_modules, kind = ins[0].mem_kind, want = ins[0].want;
+  if (kind != PR_MEM_HOST_PINNED && kind != PR_MEM_DEVICE) return PR_ERR_INVALID_ARG;
+  if (want & ~0x1Fu) return PR_ERR_INVALID_ARG;
+  PR_CUDA(h, cudaSetDevice(h->cfg.device));
+  for (uint32_t k = 0; k < n; ++k) {
+    const pr_input& in = ins[k];
+    if (in.mem_kind != kind || in.want != want) return PR_ERR_INVALID_ARG;
+    if (in.n_words && (!in.words || !in.adc)) return PR_ERR_INVALID_ARG;
+    if (in.n_words > 0xFFFFFFF0u - kTileWords) return PR_ERR_INVALID_ARG;
+    if (in.n_words) {
+      if (kind == PR_MEM_DEVICE && (((uintptr_t)in.words | (uintptr_t)in.adc) & 15u)) return PR_ERR_INVALID_ARG;
+      cudaPointerAttributes pa{}, pb{};
+      if (cudaPointerGetAttributes(&pa, in.words) != cudaSuccess || cudaPointerGetAttributes(&pb, in.adc) != cudaSuccess) {
+        cudaGetLastError();
+        return PR_ERR_INVALID_ARG;
+      }
+      const cudaMemoryType need = kind == PR_MEM_DEVICE ? cudaMemoryTypeDevice : cudaMemoryTypeHost;
+      if (pa.type != need || pb.type != need) return PR_ERR_INVALID_ARG;   // pageable host memory would make the copy synchronous
+    }
+  }
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  const bool stage = kind == PR_MEM_HOST_PINNED;
+
+  // ---- layout
+  ev->sub.assign(n, SubEvent());
+  size_t devBytes = 0, hostBytes = 0;
+  uint32_t totalTiles = 0;
+  for (uint32_t k = 0; k < n; ++k) {
+    SubEvent& s = ev->sub[k];
+    s.in = ins[k];
+    s.cap = (uint32_t)align_up(s.in.n_words ? s.in.n_words : 1, 8);
+    Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
+    carve_device(cd, tmp, s.cap, M, stage, &sw, &sa);
+    devBytes += cd.off;
+    if (want) { Carver ch(nullptr); pr_output o{}; carve_host(ch, o, want, s.cap, M); hostBytes += ch.off; }
+    s.desc.tileBase = totalTiles;
+    s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
+    totalTiles += s.desc.nTiles;
+  }
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * M * n + (size_t)8 * totalTiles;
+
+  // ---- buffers from the pools (steady state: cache hits only)
+  if (ev->ctlBytes < ctlNeed) {
+    if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
+    ev->ctl = h->devPool->alloc(ctlNeed, stream);
+    ev->ctlBytes = ev->ctl ? (size_t)bin_bytes_for(ctlNeed) : 0;
+    if (!ev->ctl) return PR_ERR_OOM;
+  }
+  if (ev->hostCountersCap < n) {
+    if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
+    ev->hostCounters = (HostCounters*)h->hostPool->alloc(sizeof(HostCounters) * n, stream);
+    ev->hostCountersCap = ev->hostCounters ? n : 0;
+    if (!ev->hostCounters) return PR_ERR_OOM;
+  }
+  ev->stream = stream;
+  ev->devSlab = h->devPool->alloc(devBytes, stream);
+  if (!ev->devSlab) return PR_ERR_OOM;
+  if (want) {
+    ev->hostSlab = h->hostPool->alloc(hostBytes, stream);
+    ev->itemTab = h->hostPool->alloc(sizeof(ExportItem) * 18 * n, stream);   // export table (mapped pinned)
+    if (!ev->hostSlab || !ev->itemTab) { release_blocks(ev, true); return PR_ERR_OOM; }
+  }
+  if (n > 1) {
+    ev->descStage = h->hostPool->alloc(sizeof(EvDesc) * n, stream);
+    ev->descDev = h->devPool->alloc(sizeof(EvDesc) * n, stream);
+    if (!ev->descStage || !ev->descDev) { release_blocks(ev, true); return PR_ERR_OOM; }
+  }
+
+  // ---- carve
+  char* ctl = (char*)ev->ctl;
+  LaunchCtl* lc = (LaunchCtl*)ctl;
+  DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
+  u64* modState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
+  u64* tileState = modState + (size_t)M * n;
+  Carver cd(ev->devSlab), ch(ev->hostSlab);
+  std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
+  for (uint32_t k = 0; k < n; ++k) {
+    SubEvent& s = ev->sub[k];
+    EvDesc& d = s.desc;
+    carve_device(cd, d, s.cap, M, stage, &stW[k], &stA[k]);
+    d.words = stage ? stW[k] : s.in.words;
+    d.adc = stage ? stA[k] : s.in.adc;
+    d.nWords = s.in.n_words; d.cap = s.cap;
+    d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
+    d.modState = modState + (size_t)M * k; d.tileState = tileState + d.tileBase;
+    s.hostViews = pr_output{};
+    if (want) carve_host(ch, s.hostViews, want, s.cap, M);
+    ev->hostCounters[k] = HostCounters{};
+  }
+
+  // ---- enqueue (all asynchronous, one stream: P:L82)
+  uint64_t nMemcpy = 0, nLaunch = 0;
+  PR_CUDA(h, cudaMemsetAsync(ev->ctl, 0, ctlNeed, stream));
+  if (stage)
+    for (uint32_t k = 0; k < n; ++k) {
+      const SubEvent& s = ev->sub[k];
+      if (!s.in.n_words) continue;
+      PR_CUDA(h, cudaMemcpyAsync(stW[k], s.in.words, (size_t)s.in.n_words * 4, cudaMemcpyHostToDevice, stream));
+      PR_CUDA(h, cudaMemcpyAsync(stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
+      nMemcpy += 2;
+    }
+  const uint32_t totalModules = M * n;
+  uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
+  if (clusterGrid > totalModules) clusterGrid = totalModules;
+  if (n == 1) {
+    const EvDesc& d = ev->sub[0].desc;
+    k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, 1, lc, h->geom);
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
+  } else {
+    EvDesc* st = (EvDesc*)ev->descStage;
+    for (uint32_t k = 0; k < n; ++k) st[k] = ev->sub[k].desc;
+    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, sizeof(EvDesc) * n, cudaMemcpyHostToDevice, stream));
+    ++nMemcpy;
+    const EvDesc* dd = (const EvDesc*)ev->descDev;
+    k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+  }
+  nLaunch += 2;
+  PR_CUDA(h, cudaGetLastError());
+  if (want) {
+    // exact-size mirrors: the item table lives at the head of the pinned slab's tail (mapped memory)
+    std::vector<ExportItem> items;
+    for (uint32_t k = 0; k < n; ++k) {
+      const EvDesc& d = ev->sub[k].desc; const pr_output& o = ev->sub[k].hostViews;
+      auto add = [&](const void* src, const void* dst, uint32_t eb, uint32_t sel, uint32_t fixed) {
+        if (dst) items.push_back(ExportItem{src, const_cast<void*>(dst), eb, sel, fixed, k});
+      };
+      add(d.module, o.h_module, 2, 0, 0); add(d.row, o.h_row, 2, 0, 0); add(d.col, o.h_col, 2, 0, 0);
+      add(d.adcOut, o.h_adc, 2, 0, 0); add(d.wordIdx, o.h_word_idx, 4, 0, 0);
+      add(d.modDigiStart, o.h_mod_digi_start, 4, 3, M + 1);
+      add(d.charge, o.h_charge, 4, 0, 0); add(d.label, o.h_label, 4, 0, 0); add(d.clus, o.h_clus, 4, 0, 0);
+      add(d.clLabel, o.h_cl_label, 4, 2, 0); add(d.clSize, o.h_cl_size, 4, 2, 0); add(d.clModule, o.h_cl_module, 2, 2, 0);
+      add(d.clCharge, o.h_cl_charge, 4, 2, 0); add(d.clRow, o.h_cl_row, 4, 2, 0); add(d.clCol, o.h_cl_col, 4, 2, 0);
+      add(d.modClusStart, o.h_mod_clus_start, 4, 3, M + 1);
+      add(d.errWord, o.h_err_word, 4, 1, 0); add(d.errIdx, o.h_err_idx, 4, 1, 0);
+    }
+    void* itab = ev->itemTab;                      // read zero-copy by the kernel; freed at release
+    memcpy(itab, items.data(), items.size() * sizeof(ExportItem));
+    size_t maxBytes = 0;
+    for (uint32_t k = 0; k < n; ++k) maxBytes = maxBytes > (size_t)ev->sub[k].cap * 4 ? maxBytes : (size_t)ev->sub[k].cap * 4;
+    uint32_t gx = (uint32_t)((maxBytes / 16 + 255) / 256);
+    if (gx < 1) gx = 1;
+    if (gx > 64) gx = 64;
+    uint32_t gy = (uint32_t)items.size();
+    if (gy > 2048) gy = 2048;
+    k_export<<<dim3(gx, gy), 256, 0, stream>>>((const ExportItem*)itab, (uint32_t)items.size(), counters);
+    ++nLaunch;
+    PR_CUDA(h, cudaGetLastError());
+  }
+  PR_CUDA(h, cudaEventRecord(ev->done, stream));
+  ev->n = n;
+  ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
+  ev->status = PR_OK;
+  ev->state = kInFlight;
+  if (ev->doneFn) PR_CUDA(h, cudaLaunchHostFunc(stream, trampoline, ev));
+
+  h->evAcquired.fetch_add(n); h->launches.fetch_add(nLaunch); h->memcpys.fetch_add(nMemcpy);
+  uint64_t w = 0;
+  for (uint32_t k = 0; k < n; ++k) w += ins[k].n_words;
+  h->words.fetch_add(w);
+  uint32_t f = h->inFlight.fetch_add(1) + 1, mx = h->maxInFlight.load();
+  while (f > mx && !h->maxInFlight.compare_exchange_weak(mx, f)) {}
+  return PR_OK;
+}
+
+// Non-blocking completion check; moves kInFlight -> kDone.
+int poll(pr_event* ev) {
+  if (ev->state == kDone) return PR_OK;
+  if (ev->state != kInFlight) return PR_ERR_BAD_STATE;
+  cudaError_t r = cudaEventQuery(ev->done);
+  if (r == cudaErrorNotReady) { cudaGetLastError(); return PR_NOT_READY; }
+  if (r != cudaSuccess) return cuda_fail(ev->h, r, "cudaEventQuery");
+  int worst = PR_OK; uint64_t dg = 0, cl = 0;
+  for (uint32_t k = 0; k < ev->n; ++k) {
+    const HostCounters& c = ev->hostCounters[k];
+    int code = status_to_code(c.status);
+    if (code < worst) worst = code;
+    dg += c.nDigis; cl += c.nClusters;
+  }
+  ev->status = worst;
+  ev->state = kDone;
+  ev->h->inFlight.fetch_sub(1);
+  ev->h->evProduced.fetch_add(ev->n); ev->h->digis.fetch_add(dg); ev->h->clusters.fetch_add(cl);
+  return PR_OK;
+}
+
+void fill_output(pr_event* ev, uint32_t k, pr_output* out) {
+  const SubEvent& s = ev->sub[k];
+  const EvDesc& d = s.desc;
+  const HostCounters& c = ev->hostCounters[k];
+  *out = s.hostViews;
+  out->event_id = s.in.event_id;
+  out->n_words = c.nWords; out->n_digis = c.nDigis; out->n_errors = c.nErrors; out->n_kept_digis = c.nKept;
+  out->n_clusters_all = c.nClustersAll; out->n_clusters = c.nClusters; out->status_bits = c.status;
+  out->n_modules = ev->h->cfg.n_modules;
+  out->d_module = d.module; out->d_row = d.row; out->d_col = d.col; out->d_adc = d.adcOut; out->d_word_idx = d.wordIdx;
+  out->d_charge = d.charge; out->d_label = d.label; out->d_clus = d.clus;
+  out->d_mod_digi_start = d.modDigiStart; out->d_mod_clus_start = d.modClusStart;
+  out->d_cl_label = d.clLabel; out->d_cl_size = d.clSize; out->d_cl_module = d.clModule;
+  out->d_cl_charge = d.clCharge; out->d_cl_row = d.clRow; out->d_cl_col = d.clCol;
+  out->d_err_word = d.errWord; out->d_err_idx = d.errIdx;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pr_abi_version(void) { return PR_ABI_VERSION; }
+
+const char* pr_strerror(int code) {
+  switch (code) {
+    case PR_OK: return "ok";
+    case PR_NOT_READY: return "not ready";
+    case PR_ERR_INVALID_ARG: return "invalid argument";
+    case PR_ERR_BAD_STATE: return "bad state for this call";
+    case PR_ERR_CAPACITY: return "internal capacity exceeded";
+    case PR_ERR_INPUT_ORDER: return "input words not grouped by non-decreasing module";
+    case PR_ERR_BAD_CALIB: return "bad calibration table or threshold";
+    case PR_ERR_OOM: return "out of memory";
+    case PR_ERR_CUDA: return "CUDA error (see pr_last_cuda_error)";
+    default: return "unknown code";
+  }
+}
+
+const char* pr_last_cuda_error(pr_handle* h) {
+  if (!h) return "";
+  std::lock_guard<std::mutex> g(h->mu);
+  return h->lastCuda.c_str();
+}
+
+int pr_create(const pr_config* cfg, pr_handle** out) {
+  if (!out) return PR_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!cfg || cfg->struct_size != sizeof(pr_config)) return PR_ERR_INVALID_ARG;
+  if (cfg->n_modules < 1 || cfg->n_modules > 2048 || cfg->n_rows < 1 || cfg->n_rows > 256 || cfg->n_cols < 1 ||
+      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || cfg->flags)
+    return PR_ERR_INVALID_ARG;
+  // A9/A21: ranges that make the 2^-14 fixed-point sums exact and overflow-free
+  if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||
+      !std::isfinite(cfg->cluster_threshold_e) || !(std::fabs(cfg->cluster_threshold_e) < 1e12f))
+    return PR_ERR_BAD_CALIB;
+  for (uint32_t m = 0; m < cfg->n_modules; ++m) {
+    const float g = cfg->gain[m], p = cfg->pedestal[m];
+    if (!std::isfinite(g) || !(g > 0.0f) || !(g < 128.0f) || !std::isfinite(p) || !(std::fabs(p) < 65536.0f)) return PR_ERR_BAD_CALIB;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return PR_ERR_CUDA; }
+  if (cfg->device < 0 || cfg->device >= ndev) return PR_ERR_INVALID_ARG;
+
+  pr_handle* h = new (std::nothrow) pr_handle();
+  if (!h) return PR_ERR_OOM;
+  h->cfg = *cfg;
+  h->cfg.gain = h->cfg.pedestal = nullptr;
+  auto fail = [&](int code) { pr_destroy(h); return code; };
+  if (cudaSetDevice(cfg->device) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
+  cudaDeviceProp prop{};
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
+  h->smCount = prop.multiProcessorCount;
+  const size_t tb = (size_t)cfg->n_modules * sizeof(float);
+  if (cudaMalloc(&h->dGain, tb) != cudaSuccess || cudaMalloc(&h->dPed, tb) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_OOM); }
+  if (cudaMemcpy(h->dGain, cfg->gain, tb, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(h->dPed, cfg->pedestal, tb, cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
+  Geom& g = h->geom;
+  g.M = cfg->n_modules; g.R = cfg->n_rows; g.C = cfg->n_cols;
+  g.stride = (g.C + 2 + 31) / 32;
+  g.bitmapWords = (g.R + 2) * g.stride + 1;
+  g.pixThr = cfg->pixel_threshold_e;
+  g.clusThrFixed = (i64)llrint((double)cfg->cluster_threshold_e * 16384.0);
+  g.gain = h->dGain; g.ped = h->dPed;
+  h->clusterSmem = cluster_smem_bytes(g.bitmapWords);
+  if (cudaFuncSetAttribute(k_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_cluster<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess) {
+    cudaGetLastError(); return fail(PR_ERR_CUDA);
+  }
+  int bps = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_cluster<true>, kClusterThreads, h->clusterSmem) != cudaSuccess) { cudaGetLastError(); bps = 1; }
+  h->clusterBlocksPerSM = bps < 1 ? 1 : bps;
+  h->devPool = new CachingPool(make_device_backend(cfg->device), cfg->max_cached_bytes_device);
+  h->hostPool = new CachingPool(make_pinned_backend(cfg->device), cfg->max_cached_bytes_host);
+
+  // Pre-warm: run the allocation pattern of `max_events_in_flight` events of `max_words_hint`
+  // words once, so the first real events hit the cache (the paper amortises API cost).
+  if (cfg->max_words_hint && cfg->max_events_in_flight) {
+    const uint32_t cap = (uint32_t)align_up(cfg->max_words_hint, 8);
+    Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
+    carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
+    const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * g.M + (size_t)8 * tiles;
+    std::vector<void*> a, b, c;
+    for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
+      a.push_back(h->devPool->alloc(cd.off, nullptr));
+      b.push_back(h->devPool->alloc(ctlNeed, nullptr));
+      c.push_back(h->hostPool->alloc(sizeof(HostCounters), nullptr));
+    }
+    for (void* p : a) if (p) h->devPool->free(p, nullptr, true);
+    for (void* p : b) if (p) h->devPool->free(p, nullptr, true);
+    for (void* p : c) if (p) h->hostPool->free(p, nullptr, true);
+  }
+  *out = h;
+  return PR_OK;
+}
+
+int pr_destroy(pr_handle* h) {
+  if (!h) return PR_ERR_INVALID_ARG;
+  cudaSetDevice(h->cfg.device);
+  cudaDeviceSynchronize();                       // job end: allowed to block
+  std::vector<pr_event*> slots;
+  { std::lock_guard<std::mutex> g(h->mu); slots.swap(h->slots); }
+  for (pr_event* ev : slots) {
+    release_blocks(ev, true);
+    if (ev->ctl) h->devPool->free(ev->ctl, nullptr, true);
+    if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
+    if (ev->done) cudaEventDestroy(ev->done);
+    delete ev;
+  }
+  delete h->devPool; delete h->hostPool;
+  if (h->dGain) cudaFree(h->dGain);
+  if (h->dPed) cudaFree(h->dPed);
+  cudaGetLastError();
+  delete h;
+  return PR_OK;
+}
+
+int pr_event_create(pr_handle* h, pr_event** out) {
+  if (!h || !out) return PR_ERR_INVALID_ARG;
+  *out = nullptr;
+  PR_CUDA(h, cudaSetDevice(h->cfg.device));
+  pr_event* ev = new (std::nothrow) pr_event();
+  if (!ev) return PR_ERR_OOM;
+  ev->h = h;
+  cudaError_t e = cudaEventCreateWithFlags(&ev->done, cudaEventDisableTiming);
+  if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
+  { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
+  *out = ev;
+  return PR_OK;
+}
+
+int pr_event_destroy(pr_event* ev) {
+  if (!ev) return PR_ERR_INVALID_ARG;
+  pr_handle* h = ev->h;
+  if (ev->state == kInFlight && poll(ev) != PR_OK) return PR_ERR_BAD_STATE;
+  release_blocks(ev, true);
+  if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
+  if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
+  if (ev->done) cudaEventDestroy(ev->done);
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    for (size_t i = 0; i < h->slots.size(); ++i)
+      if (h->slots[i] == ev) { h->slots.erase(h->slots.begin() + i); break; }
+  }
+  delete ev;
+  return PR_OK;
+}
+
+int pr_acquire(pr_event* ev, const pr_input* in, void* cuda_stream) { return acquire_impl(ev, in, 1, cuda_stream); }
+int pr_acquire_batch(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) { return acquire_impl(ev, ins, n, cuda_stream); }
+
+int pr_query(pr_event* ev) {
+  if (!ev) return PR_ERR_INVALID_ARG;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  return poll(ev);
+}
+
+int pr_produce_batch(pr_event* ev, pr_output* outs, uint32_t n) {
+  if (!ev || !outs) return PR_ERR_INVALID_ARG;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  int r = poll(ev);
+  if (r != PR_OK) return r;
+  if (n != ev->n) return PR_ERR_INVALID_ARG;
+  for (uint32_t k = 0; k < n; ++k) fill_output(ev, k, outs + k);
+  return ev->status;
+}
+int pr_produce(pr_event* ev, pr_output* out) { return pr_produce_batch(ev, out, 1); }
+
+int pr_release(pr_event* ev) {
+  if (!ev) return PR_ERR_INVALID_ARG;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  int r = poll(ev);
+  if (r != PR_OK) return r;
+  release_blocks(ev, true);                      // completion observed: reusable by any stream at once
+  ev->state = kIdle;
+  ev->n = 0;
+  return PR_OK;
+}
+
+void* pr_event_cuda_event(pr_event* ev) { return ev ? (void*)ev->done : nullptr; }
+
+void* pr_host_alloc(pr_handle* h, size_t bytes) { return h ? h->hostPool->alloc(bytes, nullptr) : nullptr; }
+int pr_host_free(pr_handle* h, void* p) { return h ? h->hostPool->free(p, nullptr, true) : PR_ERR_INVALID_ARG; }
+
+int pr_get_stats(pr_handle* h, pr_stats* out) {
+  if (!h || !out) return PR_ERR_INVALID_ARG;
+  memset(out, 0, sizeof *out);
+  out->events_acquired = h->evAcquired.load(); out->events_produced = h->evProduced.load();
+  out->words = h->words.load(); out->digis = h->digis.load(); out->clusters = h->clusters.load();
+  out->kernel_launches = h->launches.load(); out->memcpy_calls = h->memcpys.load(); out->callbacks_fired = h->callbacks.load();
+  out->events_in_flight = h->inFlight.load(); out->max_events_in_flight = h->maxInFlight.load();
+  h->devPool->stats(&out->device_pool); h->hostPool->stats(&out->host_pool);
+  return PR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,277 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the
+same seeded inputs.  Bit-exact for every integer/index output; cluster charge within 1e-5
+relative and centroids within 1e-4 pixel (BASELINE.json north_star; A14) — and in fact the exact
+fixed-point reduce makes those bit-exact too, which is asserted as well."""
+import time
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2004_04334_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def pr():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the product path has no CPU fallback")
+    from paper_2004_04334_b200 import pixreco
+    pixreco.lib()
+    return pixreco
+
+
+def to_dev(a):
+    """numpy u32/u16 -> CUDA tensor with the same bytes (16-byte aligned by the torch allocator)."""
+    if a.shape[0] == 0:
+        return torch.empty(0, dtype=torch.int32 if a.dtype == np.uint32 else torch.int16, device="cuda")
+    v = a.view(np.int32) if a.dtype == np.uint32 else a.view(np.int16)
+    return torch.from_numpy(v.copy()).cuda()
+
+
+def wait(slot, timeout=60.0):
+    t0 = time.time()
+    while slot.query() == 1:
+        if time.time() - t0 > timeout:
+            raise TimeoutError("event did not complete")
+        time.sleep(0.0002)
+
+
+INT_FIELDS = ["module", "row", "col", "adc", "word_idx", "err_word", "err_idx", "mod_digi_start", "label", "clus",
+              "cl_label", "cl_module", "cl_size", "mod_clus_start"]
+
+
+def compare(out, ref, getter, strict_float=True):
+    assert (out.n_words, out.n_digis, out.n_errors, out.n_kept_digis, out.n_clusters_all, out.n_clusters) == \
+        (ref.n_words, ref.n_digis, ref.n_errors, ref.n_kept_digis, ref.n_clusters_all, ref.n_clusters)
+    assert out.status_bits == 0
+    for f in INT_FIELDS:
+        got = getter(f)
+        if got is None:
+            continue
+        assert np.array_equal(got, getattr(ref, f)), f
+    q = getter("charge")
+    if q is not None:
+        assert np.array_equal(q.view(np.uint32), ref.charge.view(np.uint32)), "charge bits (A7: single fmaf)"
+    c = getter("cl_charge")
+    if c is not None:
+        assert np.all(np.abs(c - ref.cl_charge) <= 1e-5 * np.abs(ref.cl_charge))
+        assert np.all(np.abs(getter("cl_row") - ref.cl_row) <= 1e-4) and np.all(np.abs(getter("cl_col") - ref.cl_col) <= 1e-4)
+        if strict_float:
+            for f in ("cl_charge", "cl_row", "cl_col"):
+                assert np.array_equal(getter(f).view(np.uint32), getattr(ref, f).view(np.uint32)), f
+
+
+def run_device(pr, ev, cal, **kw):
+    """Device-resident input, device views copied back by the test."""
+    with pr.PixReco(cal.gain, cal.pedestal, ev.n_rows, ev.n_cols, cal.pixel_threshold_e, cal.cluster_threshold_e, **kw) as p:
+        slot = p.slot()
+        w, a = to_dev(ev.words), to_dev(ev.adc)
+        s = torch.cuda.Stream()
+        slot.acquire(w, a, stream=s)
+        wait(slot)
+        code, out = slot.produce()
+        assert code == 0
+        got = {f: out.to_numpy(f) for f in pr.VIEW_SPEC}
+        slot.release()
+        return out, got
+
+
+def oracle_of(ev, cal):
+    return oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal, cal.pixel_threshold_e,
+                      cal.cluster_threshold_e, ev.n_rows, ev.n_cols)
+
+
+@pytest.mark.parametrize("config,event,over", [
+    (0, 0, {}), (0, 1, {}), (1, 0, {}), (1, 7, {}), (3, 0, {}), (3, 5, {}),
+    (4, 0, dict(n_modules=24)),                      # ~6.7k digis per module: workspace tier
+    (4, 1, dict(n_modules=6, fill_pixels=1900)),     # shared-memory tier with long strips and merges
+])
+def test_chain_parity_on_workloads(pr, config, event, over):
+    ev = wl.make_event(config, event, **over)
+    cal = wl.make_calib(config, n_modules=ev.n_modules)
+    out, got = run_device(pr, ev, cal)
+    compare(out, oracle_of(ev, cal), lambda f: got[f])
+
+
+def test_host_input_with_all_mirrors_and_callback(pr):
+    ev = wl.make_event(1, 3)
+    cal = wl.make_calib(1)
+    ref = oracle_of(ev, cal)
+    fired = []
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        hw = p.host_array(ev.n_words, np.uint32)
+        ha = p.host_array(ev.n_words, np.uint16)
+        hw[:] = ev.words
+        ha[:] = ev.adc
+        slot = p.slot()
+        s = torch.cuda.Stream()
+        slot.acquire(hw, ha, stream=s, want=pr.PR_WANT_ALL, event_id=42, done=lambda user, status: fired.append(status))
+        wait(slot)
+        t0 = time.time()
+        while not fired and time.time() - t0 < 10:
+            time.sleep(0.001)
+        assert fired == [0]
+        code, out = slot.produce()
+        assert code == 0 and out.event_id == 42
+        compare(out, ref, lambda f: out.host(f))              # exact-size pinned mirrors
+        compare(out, ref, lambda f: out.to_numpy(f))          # and the device views
+        slot.release()
+        st = p.stats()
+        assert st["callbacks_fired"] == 1 and st["events_produced"] == 1 and st["digis"] == ref.n_digis
+        p.host_free(hw)
+        p.host_free(ha)
+
+
+def test_want_subset_gives_only_those_mirrors(pr):
+    ev = wl.make_event(0, 2)
+    cal = wl.make_calib(0)
+    ref = oracle_of(ev, cal)
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(ev.words), to_dev(ev.adc), want=pr.PR_WANT_CLUSTERS)
+        wait(slot)
+        _, out = slot.produce()
+        assert out.host("module") is None and out.host("label") is None and out.host("err_word") is None
+        for f in ("cl_label", "cl_size", "cl_module", "mod_clus_start"):
+            assert np.array_equal(out.host(f), getattr(ref, f))
+        assert np.array_equal(out.host("cl_charge").view(np.uint32), ref.cl_charge.view(np.uint32))
+        slot.release()
+
+
+def hand(pixels, M):
+    return wl.event_from_pixels(pixels, M)
+
+
+def test_edge_cases(pr):
+    cal = wl.flat_calib(4)
+    cases = {
+        "empty": hand([], 4),
+        "all_errors": hand([0x80000001, 0x80100002, 0xFFFFFFFF], 4),
+        "one": hand([(3, 159, 415, 255)], 4),
+        "low_bits_and_out_of_range": wl.Event(np.array([wl.encode_word(1, 2, 3, 7), wl.encode_word(4, 0, 0), wl.encode_word(1, 160, 0),
+                                                        wl.encode_word(1, 0, 416), wl.encode_word(1, 2, 4, 5)], np.uint32),
+                                              np.array([60, 60, 60, 60, 60], np.uint16), 4),
+        "duplicates": hand([(0, 5, 5, 50), (0, 9, 9, 50), (0, 5, 5, 30), (0, 5, 6, 20), (0, 5, 5, 99)], 4),
+        "subthreshold_bridge": hand([(0, 3, 3, 60), (0, 3, 4, 12), (0, 3, 5, 60)], 4),
+        "dropped_cluster": hand([(0, 3, 3, 13), (0, 3, 4, 13), (0, 9, 9, 60)], 4),
+        "no_wrap": hand([(0, 159, 7, 60), (0, 0, 7, 60), (1, 10, 415, 60), (1, 11, 0, 60), (1, 10, 0, 60)], 4),
+        "module_boundary": hand([(1, 3, 3, 60), (2, 3, 3, 60), (2, 4, 4, 60)], 4),
+        "ragged_9_words": hand([(0, 1, c, 60) for c in range(9)], 4),
+    }
+    # U shape / spiral with the minimum index at the far end; strip interleaved
+    arm1 = [(0, r, 10, 60) for r in range(60)]
+    bottom = [(0, 59, c, 60) for c in range(11, 50)]
+    arm2 = [(0, r, 50, 60) for r in range(59, -1, -1)]
+    cases["u_shape"] = hand([arm2[-1]] + arm1 + bottom + arm2[:-1], 4)
+    sp, r, c, dr, dc, seg = [], 80, 200, 0, 1, 2
+    for _ in range(40):
+        for _ in range(seg):
+            sp.append((1, r, c, 60)); r += dr; c += dc
+        dr, dc = dc, -dr
+        seg += 2
+    cases["spiral_reversed"] = hand(sp[::-1], 4)
+    cols = list(range(100, 200))
+    cases["strip"] = hand([(3, 80, c, 60) for c in cols[::2]] + [(3, 80, c, 60) for c in cols[1::2]], 4)
+    for name, ev in cases.items():
+        out, got = run_device(pr, ev, cal)
+        compare(out, oracle_of(ev, cal), lambda f: got[f])
+
+
+def test_full_and_checkerboard_and_lattice_module(pr):
+    """Maximum sizes: 66 560 digis in one module (one cluster), 33 280 (checkerboard, one cluster),
+    16 640 isolated pixels (as many clusters as digis: per-cluster workspace tier)."""
+    rr, cc = np.meshgrid(np.arange(160), np.arange(416), indexing="ij")
+    cal = wl.flat_calib(2)
+    for sel in (np.ones_like(rr, bool), (rr + cc) % 2 == 0, (rr % 2 == 0) & (cc % 2 == 0)):
+        w = ((1 << 20) | (rr[sel].astype(np.uint32) << 12) | (cc[sel].astype(np.uint32) << 3)).astype(np.uint32)
+        w = np.random.default_rng(1).permutation(w)
+        ev = wl.Event(w, np.full(w.shape[0], 60, np.uint16), 2)
+        out, got = run_device(pr, ev, cal)
+        compare(out, oracle_of(ev, cal), lambda f: got[f])
+
+
+def test_general_geometry_and_thresholds(pr):
+    """Largest field values (2048 modules of 256 x 512) and non-default thresholds."""
+    rng = np.random.default_rng(5)
+    n = 40000
+    mods = np.sort(rng.integers(0, 2048, n)).astype(np.uint32)
+    rows = rng.integers(0, 256, n).astype(np.uint32)
+    cols = rng.integers(200, 512, n).astype(np.uint32)
+    cols[: n // 2] = rng.integers(480, 512, n // 2)          # dense near the last column
+    rows[: n // 2] = rng.integers(250, 256, n // 2)
+    w = ((mods << 20) | (rows << 12) | (cols << 3)).astype(np.uint32)
+    ev = wl.Event(w, rng.integers(0, 4096, n).astype(np.uint16), 2048, 256, 512)
+    cal = wl.Calib(rng.uniform(1, 127, 2048).astype(np.float32), rng.normal(0, 3000, 2048).astype(np.float32), 600.0, 25000.0)
+    out, got = run_device(pr, ev, cal)
+    compare(out, oracle_of(ev, cal), lambda f: got[f])
+
+
+def test_input_order_violation_is_reported_not_silent(pr):
+    cal = wl.flat_calib(4)
+    ev = hand([(2, 1, 1, 60), (0, 1, 1, 60), 0x80000000 | (5 << 20), (2, 3, 3, 60)], 4)
+    fired = []
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(ev.words), to_dev(ev.adc), done=lambda u, s: fired.append(s))
+        wait(slot)
+        code, out = slot.produce(raise_on_error=False)
+        assert code == pr.PR_ERR_INPUT_ORDER and out.status_bits & 1
+        assert (out.n_digis, out.n_errors) == (3, 1)
+        t0 = time.time()
+        while not fired and time.time() - t0 < 10:
+            time.sleep(0.001)
+        assert fired == [pr.PR_ERR_INPUT_ORDER]
+        slot.release()
+        # the slot stays usable
+        good = wl.make_event(0, 0, n_modules=4)
+        slot.acquire(to_dev(good.words), to_dev(good.adc))
+        wait(slot)
+        code, out = slot.produce()
+        assert code == 0
+        ref = oracle.run(good.words, good.adc, 4, cal.gain, cal.pedestal)
+        assert out.n_clusters == ref.n_clusters and np.array_equal(out.to_numpy("label"), ref.label)
+        slot.release()
+    # violation across a tile boundary (words 2047 | 2048) in a large event
+    big = wl.make_event(1, 0)
+    w = big.words.copy()
+    valid = np.flatnonzero((w >> 31) == 0)
+    i, j = valid[valid < 2048][-1], valid[valid >= 2048][0]
+    w[i], w[j] = (w[i] & 0x800FFFFF) | (900 << 20), (w[j] & 0x800FFFFF) | (3 << 20)
+    bad = wl.Event(w, big.adc, big.n_modules)
+    calb = wl.make_calib(1)
+    with pr.PixReco(calb.gain, calb.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(bad.words), to_dev(bad.adc))
+        wait(slot)
+        code, out = slot.produce(raise_on_error=False)
+        assert code == pr.PR_ERR_INPUT_ORDER
+        assert not oracle.decode(bad.words, bad.adc, bad.n_modules)["sorted_ok"]
+        slot.release()
+
+
+def test_batch_matches_single_events(pr):
+    """pr_acquire_batch: 12 events of mixed sizes (incl. an empty one) in one chain of launches."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, e) for e in range(5)] + [wl.make_event(3, e) for e in range(3)]
+    evs += [wl.Event(np.zeros(0, np.uint32), np.zeros(0, np.uint16), 1856)]
+    evs += [wl.make_event(1, 9), wl.make_event(3, 9),
+            wl.event_from_pixels([(1855, 159, 415, 200)], 1856)]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        dev = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+        s = torch.cuda.Stream()
+        slot.acquire_batch(dev, stream=s, want=pr.PR_WANT_CLUSTERS)
+        wait(slot)
+        code, outs = slot.produce_batch(len(evs))
+        assert code == 0 and len(outs) == len(evs)
+        for k, (e, out) in enumerate(zip(evs, outs)):
+            assert out.event_id == k
+            ref = oracle_of(e, cal)
+            got = {f: out.to_numpy(f) for f in pr.VIEW_SPEC}
+            compare(out, ref, lambda f: got[f])
+            assert np.array_equal(out.host("cl_label"), ref.cl_label)
+        slot.release()
