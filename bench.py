@@ -1,0 +1,554 @@
+#!/usr/bin/env python
+"""bench.py — pixel local reconstruction throughput on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extra]
+
+Metric: events/s (plus Mdigis/s) on seeded synthetic events of the configs[1] shape (Run-3
+HLT-like, ~50k digis in 1856 modules).  One *step* = one pass of the whole hot path (unpack +
+calibrate + compact, cluster + reduce + numbering, counters to the host) over 64 such events.
+
+  value     device-resident inputs (R1): 64-event batches through pr_acquire_batch/pr_produce_batch,
+            `--slots` batches in flight on their own streams.
+  e2e       the same through the same public API with pinned HOST inputs and the cluster table
+            copied back (want = CLUSTERS): H2D and D2H inside the timed region (R2).
+  extra     configs[2] exactly as BASELINE.json words it (one pr_acquire per event, 8 streams in
+            flight), and HBM-sized launches for the unpack kernel roofline (configs[3] batch of
+            256 events, configs[4] single event).
+  roofline  dominant kernel of the step: algorithmic bytes per launch / CUDA-event duration of
+            that kernel on its own stream (PR_FLAG_KERNEL_TIMING pass over the same steps).
+  cpu_baseline  the oracle (oracle/, single thread, as it stands) on a bounded sample.
+
+Inputs rotate through a pool larger than the 126 MB L2.  N>1 (torchrun): each rank runs the same
+per-GPU workload on its own device (events are independent: no collective on the data path),
+time = max over ranks, value = all ranks' events / that time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+EVENTS_PER_STEP = 64
+POOL_EVENTS = 512            # 512 x ~0.30 MB = ~154 MB of distinct input > 126 MB L2
+STREAMS_IN_FLIGHT = 8        # configs[2]
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--slots", type=int, default=4, help="batches in flight (batch mode)")
+    ap.add_argument("--no-extra", action="store_true")
+    ap.add_argument("--pool-events", type=int, default=POOL_EVENTS)
+    ap.add_argument("--only", default=None, choices=["configs2", "configs3", "configs4"],
+                    help="run just this extra case and print its JSON (for ncu captures of HBM-sized launches)")
+    ap.add_argument("--reps", type=int, default=6, help="timed launches per extra case")
+    return ap.parse_args()
+
+
+def load_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------ workload
+def make_pool(wl, config, n_events, first_event=0):
+    return [wl.make_event(config, first_event + e) for e in range(n_events)]
+
+
+def algorithmic_bytes(W, D, E, N, M):
+    """per event."""
+    unpack = 6 * W + 16 * D + 8 * E + 4 * (M + 1)            # a1+a2 fused: read words+adc, write digi SoA+charge+errors
+    cluster = 16 * D + 24 * N + 8 * (M + 1)                  # a3+a4 fused: read row,col,charge; write label,clus; cluster SoA
+    chain = 6 * W + 24 * D + 24 * N + 8 * E + 8 * (M + 1) + 32
+    return unpack, cluster, chain
+
+
+# ------------------------------------------------------------------ reference arm (the oracle)
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    import oracle
+    from paper_2004_04334_b200 import workloads as wl
+    cal = wl.make_calib(1)
+    sample = 16                                              # events per step (bounded sample of the 64-event step)
+    pool = make_pool(wl, 1, sample * 4)
+    ws = oracle.Workspace(max(e.n_words for e in pool), cal.n_modules)
+
+    def step(s):
+        d = 0
+        for k in range(sample):
+            e = pool[(s * sample + k) % len(pool)]
+            oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
+                           cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
+            d += int(ws.counters[0])
+        return d
+    steps = min(args.steps, 400)
+    for s in range(min(args.warmup, 10)):
+        step(s)
+    t0 = time.perf_counter()
+    digis = sum(step(s) for s in range(steps))
+    dt = time.perf_counter() - t0
+    v = sample * steps / dt
+    line = {"impl": "reference", "metric": "pixel-reco events/s", "value": v, "unit": "events/s", "n_gpus": args.gpus,
+            "steps": steps, "warmup": min(args.warmup, 10), "ms_per_step": dt / steps * 1e3 * (EVENTS_PER_STEP / sample),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32 (exact int64 sums)",
+            "data": "synthetic", "mdigis_per_s": digis / dt / 1e6,
+            "config": {"workload": "configs[1] Run-3 HLT-like events, oracle on host cores", "events_per_step": EVENTS_PER_STEP,
+                       "sample": f"{sample} of the step's {EVENTS_PER_STEP} events per step"},
+            "cpu_baseline": {"value": v, "unit": "events/s", "cores": 1, "kind": "oracle",
+                             "sample": f"{sample * steps} events of the configs[1] shape, single thread"},
+            "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ our arm
+class Bench:
+    def __init__(self, torch, pr, wl, device, flags=0, M=None, cal=None):
+        self.torch, self.pr, self.wl, self.device = torch, pr, wl, device
+        self.cal = cal
+        self.p = pr.PixReco(cal.gain, cal.pedestal, device=device, flags=flags)
+        self.lib = pr.lib()
+
+    def close(self):
+        self.p.close()
+
+    # -- inputs
+    def upload(self, pool):
+        """Device-resident copies (one big buffer each, 256-byte aligned slices)."""
+        torch = self.torch
+        offs, tot = [], 0
+        for e in pool:
+            offs.append(tot)
+            tot += (e.n_words + 63) // 64 * 64
+        W = np.zeros(max(tot, 64), np.uint32); A = np.zeros(max(tot, 64), np.uint16)
+        for e, o in zip(pool, offs):
+            W[o:o + e.n_words] = e.words; A[o:o + e.n_words] = e.adc
+        dW = torch.from_numpy(W.view(np.int32)).to(f"cuda:{self.device}")
+        dA = torch.from_numpy(A.view(np.int16)).to(f"cuda:{self.device}")
+        self._keep_dev = (dW, dA)
+        return [(dW.data_ptr() + 4 * o, dA.data_ptr() + 2 * o, e.n_words) for e, o in zip(pool, offs)]
+
+    def pin(self, pool):
+        """Pinned host copies from the library's host pool."""
+        offs, tot = [], 0
+        for e in pool:
+            offs.append(tot)
+            tot += (e.n_words + 63) // 64 * 64
+        W = self.p.host_array(max(tot, 64), np.uint32); A = self.p.host_array(max(tot, 64), np.uint16)
+        for e, o in zip(pool, offs):
+            W[o:o + e.n_words] = e.words; A[o:o + e.n_words] = e.adc
+        self._keep_pin = (W, A)
+        return [(W.ctypes.data + 4 * o, A.ctypes.data + 2 * o, e.n_words) for e, o in zip(pool, offs)]
+
+    def inputs(self, ptrs, kind, want):
+        pr = self.pr
+        arr = (pr.pr_input * len(ptrs))()
+        for k, (w, a, n) in enumerate(ptrs):
+            arr[k] = pr.pr_input(w, a, n, kind, want, k, pr.pr_done_fn(), None)
+        return arr
+
+    @staticmethod
+    def at(pr, arr, k):
+        """POINTER(pr_input) to element k of a pr_input array."""
+        return ctypes.cast(ctypes.addressof(arr) + k * ctypes.sizeof(pr.pr_input), ctypes.POINTER(pr.pr_input))
+
+    # -- timed region helper: device time between a gate event and the join of all streams
+    def timed(self, streams, fn):
+        torch = self.torch
+        gate = torch.cuda.Stream(device=self.device)
+        start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(self.device)
+        t0 = time.perf_counter()
+        start.record(gate)
+        for s in streams:
+            s.wait_event(start)
+        fn()
+        for s in streams:
+            gate.wait_stream(s)
+        end.record(gate)
+        torch.cuda.synchronize(self.device)
+        wall = time.perf_counter() - t0
+        return start.elapsed_time(end) * 1e-3, wall
+
+    # -- batch mode: `slots` batches of 64 events in flight
+    def run_batches(self, inp, n_events_pool, steps, slots, streams, first_step=0):
+        lib, pr = self.lib, self.pr
+        outs = (pr.pr_output * EVENTS_PER_STEP)()
+        nb = n_events_pool // EVENTS_PER_STEP
+        busy = [False] * len(slots)
+        digis = clusters = 0
+
+        def finish(i):
+            nonlocal digis, clusters
+            while True:
+                r = lib.pr_produce_batch(slots[i].ptr, outs, EVENTS_PER_STEP)
+                if r != pr.PR_NOT_READY:
+                    break
+            if r != 0:
+                raise RuntimeError(f"pr_produce_batch -> {r}")
+            for k in range(EVENTS_PER_STEP):
+                digis += outs[k].n_digis; clusters += outs[k].n_clusters
+            lib.pr_release(slots[i].ptr)
+            busy[i] = False
+        for s in range(steps):
+            i = s % len(slots)
+            if busy[i]:
+                finish(i)
+            b = (first_step + s) % nb
+            r = lib.pr_acquire_batch(slots[i].ptr, self.at(pr, inp, b * EVENTS_PER_STEP), EVENTS_PER_STEP,
+                                     ctypes.c_void_p(streams[i].cuda_stream))
+            if r != 0:
+                raise RuntimeError(f"pr_acquire_batch -> {r}: {lib.pr_last_cuda_error(self.p.handle).decode()}")
+            busy[i] = True
+        for i in range(len(slots)):
+            if busy[i]:
+                finish(i)
+        return digis, clusters
+
+    # -- configs[2]: one pr_acquire per event, 8 slots/streams in flight (A25: slot = stream = e mod 8)
+    def run_streams(self, inp, n_events_pool, n_events, slots, streams, first=0):
+        lib, pr = self.lib, self.pr
+        out = pr.pr_output()
+        busy = [False] * len(slots)
+        digis = clusters = 0
+        ptrs = [self.at(pr, inp, k) for k in range(n_events_pool)]
+
+        def finish(i):
+            nonlocal digis, clusters
+            while True:
+                r = lib.pr_produce(slots[i].ptr, ctypes.byref(out))
+                if r != pr.PR_NOT_READY:
+                    break
+            if r != 0:
+                raise RuntimeError(f"pr_produce -> {r}")
+            digis += out.n_digis; clusters += out.n_clusters
+            lib.pr_release(slots[i].ptr)
+            busy[i] = False
+        for e in range(n_events):
+            i = e % len(slots)
+            if busy[i]:
+                finish(i)
+            k = (first + e) % n_events_pool
+            r = lib.pr_acquire(slots[i].ptr, ptrs[k], ctypes.c_void_p(streams[i].cuda_stream))
+            if r != 0:
+                raise RuntimeError(f"pr_acquire -> {r}: {lib.pr_last_cuda_error(self.p.handle).decode()}")
+            busy[i] = True
+        for i in range(len(slots)):
+            if busy[i]:
+                finish(i)
+        return digis, clusters
+
+
+def run_ours(args, rank, world):
+    import torch
+    from paper_2004_04334_b200 import pixreco as pr, workloads as wl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    peak, peak_src = load_peaks()
+    K, Wm = args.steps, max(args.warmup, 3)
+    cal = wl.make_calib(1)
+    M = cal.n_modules
+    n_pool = max(args.pool_events // EVENTS_PER_STEP, 1) * EVENTS_PER_STEP
+    pool = make_pool(wl, 1, n_pool, first_event=rank * n_pool)       # every rank its own events (weak scaling)
+    meanW = float(np.mean([e.n_words for e in pool]))
+
+    b = Bench(torch, pr, wl, local, cal=cal)
+    dev_ptrs = b.upload(pool)
+    pin_ptrs = b.pin(pool)
+    inp_dev = b.inputs(dev_ptrs, pr.PR_MEM_DEVICE, 0)
+    inp_host = b.inputs(pin_ptrs, pr.PR_MEM_HOST_PINNED, pr.PR_WANT_CLUSTERS)
+    nslots = max(1, args.slots)
+    slots = [b.p.slot() for _ in range(nslots)]
+    streams = [torch.cuda.Stream(device=local) for _ in range(nslots)]
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(local)
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---------------- R1: device-resident, batch mode (the headline `value`)
+    b.run_batches(inp_dev, n_pool, Wm, slots, streams)                 # warm-up (fills the pools)
+    st0 = b.p.stats()
+    barrier()
+    clk = ClockSampler(local)
+    res = {}
+
+    def r1():
+        res["dc"] = b.run_batches(inp_dev, n_pool, K, slots, streams, first_step=Wm)
+    t_dev, t_wall = b.timed(streams, r1)
+    barrier()
+    clocks = clk.stop()
+    st1 = b.p.stats()
+    t_dev = max_over_ranks(t_dev)
+    digis, clusters = res["dc"]
+    n_events = K * EVENTS_PER_STEP
+    value = world * n_events / t_dev
+    launches = st1["kernel_launches"] - st0["kernel_launches"]
+    new_mallocs = st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"]
+
+    # ---------------- R2: end to end, pinned host inputs + cluster table back (same API)
+    b.run_batches(inp_host, n_pool, Wm, slots, streams)
+    barrier()
+    t_e2e, _ = b.timed(streams, lambda: b.run_batches(inp_host, n_pool, K, slots, streams, first_step=Wm))
+    barrier()
+    t_e2e = max_over_ranks(t_e2e)
+    e2e_value = world * n_events / t_e2e
+    h2d = int(6 * meanW * EVENTS_PER_STEP)
+    meanN = clusters / n_events
+    d2h = int((22 * meanN + 4 * (M + 1) + 32) * EVENTS_PER_STEP)
+    b.close()
+
+    line = {"metric": "pixel-reco events/s", "value": value, "unit": "events/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": t_dev / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u32+f32 (exact int64 sums)", "data": "synthetic",
+            "mdigis_per_s": world * digis / t_dev / 1e6,
+            "config": {"workload": "configs[1] Run-3 HLT-like events (1856 modules, ~50k digis, ~8k clusters/event); "
+                                   "step = 64 events = one pr_acquire_batch/pr_produce_batch",
+                       "events_per_step": EVENTS_PER_STEP, "batches_in_flight": nslots, "mean_words_per_event": meanW,
+                       "l2_policy": f"inputs rotate through {n_pool} distinct events ({n_pool * meanW * 6 / 1e6:.0f} MB) > 126 MB L2",
+                       "residency": "R1 device-resident inputs, counters to mapped pinned host"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": t_e2e / K * 1e3, "what": "pinned host inputs, want=CLUSTERS, same batch API"},
+            "steady_state_cudaMalloc": int(new_mallocs), "wall_s": t_wall}
+
+    if rank == 0:
+        # ---------------- kernel timing pass for the roofline (same steps, PR_FLAG_KERNEL_TIMING)
+        bt = Bench(torch, pr, wl, local, flags=pr.PR_FLAG_KERNEL_TIMING, cal=cal)
+        dp = bt.upload(pool)
+        it = bt.inputs(dp, pr.PR_MEM_DEVICE, 0)
+        sl = [bt.p.slot() for _ in range(nslots)]
+        bt.run_batches(it, n_pool, Wm, sl, streams)
+        s0 = bt.p.stats()
+        dg, cl = bt.run_batches(it, n_pool, K, sl, streams, first_step=Wm)
+        torch.cuda.synchronize(local)
+        s1 = bt.p.stats()
+        nt = s1["timed_acquires"] - s0["timed_acquires"]
+        t_un = (s1["unpack_ms"] - s0["unpack_ms"]) / nt * 1e-3
+        t_cl = (s1["cluster_ms"] - s0["cluster_ms"]) / nt * 1e-3
+        Dm, Nm = dg / (K * EVENTS_PER_STEP), cl / (K * EVENTS_PER_STEP)
+        Em = meanW - Dm
+        bu, bc, bchain = algorithmic_bytes(meanW, Dm, Em, Nm, M)
+        kern = {"k_unpack": {"ms": t_un * 1e3, "bytes": bu * EVENTS_PER_STEP, "gbs": bu * EVENTS_PER_STEP / t_un / 1e9},
+                "k_cluster": {"ms": t_cl * 1e3, "bytes": bc * EVENTS_PER_STEP, "gbs": bc * EVENTS_PER_STEP / t_cl / 1e9}}
+        dom = "k_cluster" if t_cl >= t_un else "k_unpack"
+        line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                            "frac": kern[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                            "frac_of_8TBs_nominal": kern[dom]["gbs"] / 8000.0,
+                            "algorithmic_bytes_per_launch": kern[dom]["bytes"], "ms_per_launch": kern[dom]["ms"],
+                            "units_per_launch": f"{EVENTS_PER_STEP} events", "kernels": kern,
+                            "chain": {"bytes_per_event": bchain, "gbs": bchain * value / world / 1e9,
+                                      "frac": bchain * value / world / 1e9 / peak}}
+        bt.close()
+        extra = {}
+        if not args.no_extra:
+            extra = run_extra(torch, pr, wl, local, peak)
+        line["extra"] = extra
+        line["cpu_baseline"] = cpu_baseline(wl, pool, cal)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def cpu_baseline(wl, pool, cal, budget_s=12.0):
+    import oracle
+    ws = oracle.Workspace(max(e.n_words for e in pool), cal.n_modules)
+    n, t0 = 0, time.perf_counter()
+    while True:
+        e = pool[n % len(pool)]
+        oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
+                       cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
+        n += 1
+        dt = time.perf_counter() - t0
+        if dt > budget_s or n >= 4096:
+            break
+    return {"value": n / dt, "unit": "events/s", "cores": 1, "kind": "oracle",
+            "sample": f"{n} events of the configs[1] shape, {dt:.1f} s, single thread (host has {os.cpu_count()} cores)"}
+
+
+def run_extra(torch, pr, wl, local, peak, only=None, reps_hbm=6):
+    """configs[2] as worded (per-event streams), and HBM-sized launches for the unpack roofline."""
+    extra = {}
+    if only in (None, "configs2"):
+        extra.update(run_configs2(torch, pr, wl, local))
+    # ---- HBM-sized launches, kernel timing on
+    for name, config, n_ev, batch in (("configs[3] 256-event batch", 3, 256, True), ("configs[4] single event", 4, 2, False)):
+        if only is not None and only != f"configs{config}":
+            continue
+        extra[name] = run_hbm_case(torch, pr, wl, local, peak, config, n_ev, batch, reps_hbm)
+    return extra
+
+
+def run_configs2(torch, pr, wl, local):
+    extra = {}
+    # ---- configs[2]: 64 events, one pr_acquire each, 8 streams in flight
+    cal = wl.make_calib(1)
+    pool = make_pool(wl, 1, 256)
+    b = Bench(torch, pr, wl, local, cal=cal)
+    inp = b.inputs(b.upload(pool), pr.PR_MEM_DEVICE, 0)
+    slots = [b.p.slot() for _ in range(STREAMS_IN_FLIGHT)]
+    streams = [torch.cuda.Stream(device=local) for _ in range(STREAMS_IN_FLIGHT)]
+    b.run_streams(inp, len(pool), 256, slots, streams)
+    st0 = b.p.stats()
+    reps = 40
+    t, wall = b.timed(streams, lambda: [b.run_streams(inp, len(pool), 64, slots, streams, first=64 * r) for r in range(reps)])
+    st1 = b.p.stats()
+    extra["configs[2] per-event streams"] = {
+        "events_per_s": 64 * reps / t, "events": 64 * reps, "streams_in_flight": STREAMS_IN_FLIGHT,
+        "us_per_event": t / (64 * reps) * 1e6, "max_events_in_flight": st1["max_events_in_flight"],
+        "new_cudaMalloc_in_timed_region": st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"],
+        "note": "one pr_acquire/pr_produce/pr_release per event from one host thread (Python driver); launch-latency bound"}
+    b.close()
+    return extra
+
+
+def run_hbm_case(torch, pr, wl, local, peak, config, n_ev, batch, reps):
+    if True:
+        cal = wl.make_calib(config)
+        pool = make_pool(wl, config, n_ev)
+        bt = Bench(torch, pr, wl, local, flags=pr.PR_FLAG_KERNEL_TIMING, cal=cal)
+        ptrs = bt.upload(pool)
+        inp = bt.inputs(ptrs, pr.PR_MEM_DEVICE, 0)
+        slot = bt.p.slot()
+        s = torch.cuda.Stream(device=local)
+        lib = pr.lib()
+        tot = {"W": 0, "D": 0, "N": 0}
+        outs = (pr.pr_output * n_ev)()
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")
+        s0 = None
+        for r in range(reps + 2):
+            if r == 2:
+                torch.cuda.synchronize(local)
+                s0 = bt.p.stats()
+            flush.fill_(r)                                   # evict L2 between iterations
+            torch.cuda.synchronize(local)
+            if batch:
+                rc = lib.pr_acquire_batch(slot.ptr, inp, n_ev, ctypes.c_void_p(s.cuda_stream))
+                n_out = n_ev
+            else:
+                rc = lib.pr_acquire(slot.ptr, Bench.at(pr, inp, r % n_ev), ctypes.c_void_p(s.cuda_stream))
+                n_out = 1
+            assert rc == 0, rc
+            while lib.pr_produce_batch(slot.ptr, outs, n_out) == pr.PR_NOT_READY:
+                pass
+            if r >= 2:
+                for k in range(n_out):
+                    tot["W"] += outs[k].n_words; tot["D"] += outs[k].n_digis; tot["N"] += outs[k].n_clusters
+            lib.pr_release(slot.ptr)
+        s1 = bt.p.stats()
+        nt = s1["timed_acquires"] - s0["timed_acquires"]
+        t_un = (s1["unpack_ms"] - s0["unpack_ms"]) / nt * 1e-3
+        t_cl = (s1["cluster_ms"] - s0["cluster_ms"]) / nt * 1e-3
+        W, D, N = tot["W"] / nt, tot["D"] / nt, tot["N"] / nt
+        n_per = n_ev if batch else 1
+        bu, bc, bchain = algorithmic_bytes(W, D, W - D, N, cal.n_modules * n_per)
+        res = {"events_per_launch": n_per, "words_per_launch": W, "digis_per_launch": D, "clusters_per_launch": N,
+                       "k_unpack": {"ms": t_un * 1e3, "gbs": bu / t_un / 1e9, "frac_of_measured_peak": bu / t_un / 1e9 / peak,
+                                    "frac_of_8TBs": bu / t_un / 1e9 / 8000.0, "algorithmic_bytes": bu},
+                       "k_cluster": {"ms": t_cl * 1e3, "gbs": bc / t_cl / 1e9, "frac_of_measured_peak": bc / t_cl / 1e9 / peak,
+                                     "algorithmic_bytes": bc},
+                       "chain": {"events_per_s": n_per / (t_un + t_cl), "mdigis_per_s": D / (t_un + t_cl) / 1e6,
+                                 "gbs": bchain / (t_un + t_cl) / 1e9, "frac_of_measured_peak": bchain / (t_un + t_cl) / 1e9 / peak},
+                       "l2_policy": "256 MiB fill between iterations"}
+        bt.close()
+        del flush
+        return res
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", 0))
+    world = int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.only:
+        import torch
+        from paper_2004_04334_b200 import pixreco as pr, workloads as wl
+        peak, _ = load_peaks()
+        print(json.dumps(run_extra(torch, pr, wl, 0, peak, only=args.only, reps_hbm=args.reps)), flush=True)
+        return
+    run_ours(args, rank, world)
+
+
+if __name__ == "__main__":
+    main()

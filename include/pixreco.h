@@ -95,8 +95,13 @@ typedef struct {
   uint32_t max_words_hint;        /* pre-warm the pools for events of this many words (0 = none)  */
   uint32_t max_events_in_flight;  /* ... and this many concurrent events                          */
   uint64_t max_cached_bytes_device, max_cached_bytes_host;   /* pool caps, 0 = unlimited          */
-  uint32_t flags;                 /* reserved, 0                                                  */
+  uint32_t flags;                 /* PR_FLAG_* mask                                               */
 } pr_config;
+
+/* pr_config.flags */
+#define PR_FLAG_KERNEL_TIMING 0x1u /* record CUDA events around each kernel on its stream and sum the
+                                      per-kernel device times into pr_stats (measurement aid; adds
+                                      three cudaEventRecord per acquire)                            */
 
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
@@ -141,6 +146,9 @@ typedef struct {
   uint64_t kernel_launches, memcpy_calls, callbacks_fired;
   uint32_t events_in_flight, max_events_in_flight;
   pr_pool_stats device_pool, host_pool;
+  /* PR_FLAG_KERNEL_TIMING only: device time summed over `timed_acquires` completed acquires */
+  uint64_t timed_acquires;
+  double   unpack_ms, cluster_ms, export_ms;
 } pr_stats;
 
 /* ---- handle: job start / job end (may block and allocate) ---- */
@@ -177,6 +185,12 @@ int pr_release(pr_event* ev);
 /* The slot's completion cudaEvent_t (as void*) for cudaStreamWaitEvent on a consumer's stream
  * (P:L108), valid between pr_acquire and pr_release.                                             */
 void* pr_event_cuda_event(pr_event* ev);
+/* Consumer-side synchronisation of P:L106-108: if the slot's work has already completed
+ * (cudaEventQuery) return at once; otherwise make `consumer_stream` wait for it with
+ * cudaStreamWaitEvent.  Never blocks the host.  After it returns PR_OK, work queued on
+ * `consumer_stream` may read the slot's device buffers (addresses: a previous pr_produce of a same-
+ * sized event on this slot, or any pr_produce after completion).                                 */
+int pr_stream_wait_event(pr_event* ev, void* consumer_stream);
 
 /* ---- pinned host memory from the handle's host pool, for inputs ---- */
 void* pr_host_alloc(pr_handle* h, size_t bytes);     /* NULL on failure */

@@ -34,6 +34,8 @@ constexpr int kTileWords = kUnpackThreads * kWordsPerThread;   // 2048
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
+constexpr u32 kWindowLog2 = 9;
+constexpr u32 kWindow = 1u << kWindowLog2;       // a cluster work unit = 512 consecutive digi indices
 constexpr u32 kSmemDigis = 2048;      // modules with more digis use the global workspace tier
 constexpr u32 kSmemClusters = 512;    // likewise for per-cluster accumulators
 
@@ -66,6 +68,8 @@ struct EvDesc {
   u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
   DevCounters* counters; HostCounters* hostCounters;
   u64 *tileState, *modState;        // look-back states: [nTiles], [M]
+  u32* winInv;                      // [nWin]: M - (first module starting in the window), 0 = none
+  u32 winBase, nWin;                // this event's windows in the launch's flattened unit space
 };
 
 struct Geom {
@@ -160,14 +164,15 @@ __device__ __forceinline__ const EvDesc& pick_event_by_tile(const EvDesc& single
 // One CTA per tile of 2048 words, 8 consecutive words per thread (2 x LDG.128 words + 1 x LDG.128
 // adc).  Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
 template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads)
+__global__ void __launch_bounds__(kUnpackThreads, 4)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
          LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   __shared__ __align__(16) u32 sWord[kTileWords + 8];
   __shared__ __align__(16) u16 sAdc[kTileWords + 8];
   __shared__ __align__(16) u16 sOff[kTileWords + 8];
   __shared__ u32 sWsum[8], sWmax[8];
-  __shared__ u32 sTicket, sExclCnt, sExclMax;
+  __shared__ u32 sLbCnt[8], sLbMax[8];
+  __shared__ u32 sTicket;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) sTicket = atomicAdd(&lc->tileTicket, 1u);
@@ -222,21 +227,42 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   }
   const u32 r0 = wbase + incl - cnt;                 // tile-local rank of this thread's first digi
 
-  // ---- decoupled look-back for the event-global digi offset and running max(module)+1
-  if (warp == 0) {
+  // ---- decoupled look-back for the event-global digi offset and running max(module)+1.
+  // The whole CTA looks back: thread j reads the state of tile (t-1-j), so one round covers 256
+  // predecessors (with ~450 tiles in flight a 32-wide window needed ~14 serial L2 round trips).
+  u32 g0 = 0, carryMax1 = 0;
+  {
     u64* state = ev.tileState;
-    u32 ec = 0, em = 0;
     if (tile > 0) {
-      if (lane == 0) st_state(state + tile, pack_state(kStAgg, tileCnt, tileMax1));
-      lookback(state, 0, (int)tile, lane, &ec, &em);
+      if (tid == 0) st_state(state + tile, pack_state(kStAgg, tileCnt, tileMax1));
+      int look = (int)tile - 1;
+      for (;;) {
+        const int idx = look - tid;
+        u64 v = kStIncl;                               // virtual zero inclusive before the event start
+        if (idx >= 0) do { v = ld_state(state + idx); } while (st_status(v) == 0);
+        const u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v) == 2);
+        const int upto = inclMask ? (__ffs(inclMask) - 1) : 31;
+        const u32 cc = lane <= upto ? st_count(v) : 0, mm = lane <= upto ? st_max1(v) : 0;
+        const u32 wc = __reduce_add_sync(0xFFFFFFFFu, cc), wm = __reduce_max_sync(0xFFFFFFFFu, mm);
+        __syncthreads();                               // previous readers of sLb* are done
+        if (lane == 0) { sLbCnt[warp] = wc; sLbMax[warp] = wm | (inclMask ? 0x80000000u : 0u); }
+        __syncthreads();
+        bool found = false;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          if (!found) {
+            g0 += sLbCnt[k];
+            const u32 x = sLbMax[k];
+            carryMax1 = max(carryMax1, x & 0xFFFu);
+            found = (x >> 31) != 0;
+          }
+        }
+        if (found) break;
+        look -= kUnpackThreads;
+      }
     }
-    if (lane == 0) {
-      st_state(state + tile, pack_state(kStIncl, ec + tileCnt, max(em, tileMax1)));
-      sExclCnt = ec; sExclMax = em;
-    }
+    if (tid == 0) st_state(state + tile, pack_state(kStIncl, g0 + tileCnt, max(carryMax1, tileMax1)));
   }
-  __syncthreads();
-  const u32 g0 = sExclCnt, carryMax1 = sExclMax;
   const u32 ph = g0 & 7u;                            // smem phase = global 16-byte phase of u16 arrays
 
   // ---- compact into shared memory; errors straight to global (rare)
@@ -282,7 +308,10 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       if (j & 1) { modv[j >> 1] |= mod << 16; rowv[j >> 1] |= row << 16; colv[j >> 1] |= col << 16; }
       else { modv[j >> 1] = mod; rowv[j >> 1] = row; colv[j >> 1] = col; }
       if (in) {
-        if ((int)mod > prev) for (int m = prev + 1; m <= (int)mod; ++m) ev.modDigiStart[m] = gb + j;
+        if ((int)mod > prev) {
+          for (int m = prev + 1; m <= (int)mod; ++m) ev.modDigiStart[m] = gb + j;
+          atomicMax(ev.winInv + ((gb + j) >> kWindowLog2), g.M - (u32)(prev + 1));   // first module starting in this digi window
+        }
         if ((int)mod < prev) violation = 1;
         prev = (int)mod;
       }
@@ -317,19 +346,35 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   if (tile == ev.nTiles - 1) {
     const u32 D = g0 + tileCnt, mx1 = max(carryMax1, tileMax1);
     for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) ev.modDigiStart[m] = D;
+    if (tid == 0 && mx1 < g.M) atomicMax(ev.winInv + (D >> kWindowLog2), g.M - mx1);   // trailing empty modules start at D
     if (tid == 0) { ev.counters->nWords = W; ev.counters->nDigis = D; ev.counters->nErrors = W - D; }
   }
 }
 
 // ================================================================== k_cluster (a3 + a4)
-struct ClusterSmem {           // carved from dynamic shared memory by the kernel
-  u32 *bitmap, *prefix, *perm, *parent, *root, *size;
-  int32_t* knum;
-  u64 *S, *Sx, *Sy;
-};
+// Work unit = one "window" of kWindow consecutive digi indices of one event: the CTA owns every
+// module whose first digi index falls into the window (k_unpack leaves the first such module in
+// winInv[]).  Because a module with more than kWindow digis reaches past the window's end, only
+// the LAST module of a window can be that large; all others ("smalls") together hold fewer than
+// 2*kWindow = kRangeCap digis.  Units are independent, so no CTA waits on another CTA's progress
+// before it has published all of its own counts:
+//   sparse path  the smalls of the window are clustered at once: shared-memory hash
+//                (module,row,col) -> digi, min-index union-find over the backward neighbours,
+//                per-root member lists walked by the root's thread for the exact int64 sums.
+//                O(1) work per digi, ~9 block barriers per ~19 modules (Run-3-like occupancy).
+//   dense path   a module with more than kWindow digis: occupancy bitmap + popcount ranks,
+//                union-find and per-cluster atomics (shared-memory tiers, global workspace beyond).
+// Dense numbering of kept clusters: decoupled look-back over per-module states.
+constexpr u32 kRangeCap = 2 * kWindow;           // > digis of a window's smalls; local index fits 10 bits
+constexpr u32 kHashSlots = 2048;
+constexpr u32 kEmpty = 0xFFFFFFFFu;
+constexpr int kPerThread = kRangeCap / kClusterThreads;   // 4
+
 __host__ __device__ inline size_t cluster_smem_bytes(u32 bitmapWords) {
   size_t w = (bitmapWords + 3) & ~3u;
-  return (size_t)w * 4 * 2 + (size_t)kSmemDigis * 4 * 2 + (size_t)kSmemClusters * (4 + 4 + 4 + 8 * 3) + 64;
+  size_t dense = (size_t)w * 4 * 2 + (size_t)kSmemDigis * 4 * 2 + (size_t)kSmemClusters * (4 + 4 + 4 + 8 * 3);
+  size_t sparse = (size_t)kHashSlots * 4 * 2 + (size_t)kRangeCap * 4 * 5;
+  return (dense > sparse ? dense : sparse) + 64;
 }
 
 __device__ __forceinline__ u32 uf_find(const volatile u32* parent, u32 x) {
@@ -350,15 +395,213 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
   }
 }
 
-template <bool kSingle>
-__global__ void __launch_bounds__(kClusterThreads)
-k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
-          LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
-  extern __shared__ __align__(16) unsigned char smemRaw[];
-  __shared__ u32 sScan[8];
-  __shared__ u32 sTicket, sBase, sLast;
+// Open-addressing hash: tabKey[h] = module << 17 | row << 9 | col (28 bits), tabVal[h] = minimum
+// local digi index on that pixel (duplicates: owner = min index, A6).
+__device__ __forceinline__ u32 hash_slot(u32 key) { return (key * 0x9E3779B1u) >> 21; }
+__device__ __forceinline__ void hash_insert(u32* tabKey, u32* tabVal, u32 key, u32 idx) {
+  u32 h = hash_slot(key);
+  for (;;) {
+    const u32 old = atomicCAS(tabKey + h, kEmpty, key);
+    if (old == kEmpty || old == key) { atomicMin(tabVal + h, idx); return; }
+    h = (h + 1) & (kHashSlots - 1);
+  }
+}
+__device__ __forceinline__ u32 hash_find(const u32* tabKey, const u32* tabVal, u32 key) {
+  u32 h = hash_slot(key);
+  for (;;) {
+    const u32 v = tabKey[h];
+    if (v == kEmpty) return kInvalid;
+    if (v == key) return tabVal[h];
+    h = (h + 1) & (kHashSlots - 1);
+  }
+}
 
+struct ClusterShared {
+  u32 scan[8];
+  u32 cnt[2][kPerThread * 8];       // per (k, warp): kept roots / all roots
+  u32 kb[kPerThread * 8];           // per (k, warp): ballot of kept roots
+  u32 offs[kPerThread * 8 + 1];
+  u32 ticket, base, last, first;
+};
+
+// Number of kept roots with local index < b (b in [0, n]); valid after the scan of the sparse path.
+__device__ __forceinline__ u32 kept_prefix(const ClusterShared& sh, u32 b, u32 total) {
+  if (b >= kRangeCap) return total;
+  const u32 k = b / kClusterThreads, r = b % kClusterThreads, w = r >> 5, l = r & 31;
+  return sh.offs[k * 8 + w] + __popc(sh.kb[k * 8 + w] & ((1u << l) - 1u));
+}
+
+// ---- sparse path: modules [m0, m1) of event ev (m1 > m0), digis [s, s+n), n < kRangeCap.
+// Returns the number of kept clusters; *baseOut = dense number of its first kept cluster.
+__device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom& g, u32 m0, u32 m1, u32 s, u32 n,
+                                                    unsigned char* smemRaw, ClusterShared& sh, u32* baseOut) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  u32* tabKey = reinterpret_cast<u32*>(smemRaw);
+  u32* tabVal = tabKey + kHashSlots;
+  u32* key = tabVal + kHashSlots;
+  u32* parent = key + kRangeCap;
+  u32* head = parent + kRangeCap;
+  u32* next = head + kRangeCap;
+  float* qs = reinterpret_cast<float*>(next + kRangeCap);
+
+  // interior modules contribute through the range's last module: publish "aggregate 0" for them
+  for (u32 m = m0 + tid; m + 1 < m1; m += kClusterThreads) st_state(ev.modState + m, pack_state(kStAgg, 0, 0));
+  u32 total = 0, nAll = 0;
+  u32 kb[kPerThread];
+  float cq[kPerThread], cr[kPerThread], cc[kPerThread]; u32 csz[kPerThread]; u32 keptMask = 0;
+  if (n > 0) {
+    // A: init
+    for (u32 i = tid; i < kHashSlots; i += kClusterThreads) { tabKey[i] = kEmpty; tabVal[i] = kInvalid; }
+    __syncthreads();
+    // B: load, kept flag (A8), hash insert
+    u32 myKept = 0;
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      if (i < n) {
+        const float q = ev.charge[s + i];
+        const bool kept = q >= g.pixThr;
+        u32 kk = kInvalid;
+        if (kept) {
+          kk = (u32)ev.module[s + i] << 17 | (u32)ev.row[s + i] << 9 | (u32)ev.col[s + i];
+          hash_insert(tabKey, tabVal, kk, i);
+          ++myKept;
+        }
+        key[i] = kk; qs[i] = q; parent[i] = kept ? i : kInvalid; head[i] = kInvalid;
+      }
+    }
+    myKept = __reduce_add_sync(0xFFFFFFFFu, myKept);
+    if (lane == 0 && myKept) atomicAdd(&ev.counters->nKept, myKept);
+    __syncthreads();
+    // C: unions with backward neighbours: N ? {N} : { NE?, W ? {W} : NW? }; duplicates join their owner
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      if (i >= n) continue;
+      const u32 kk = key[i];
+      if (kk == kInvalid) continue;
+      const u32 owner = hash_find(tabKey, tabVal, kk);
+      if (owner != i) { uf_union(parent, i, owner); continue; }
+      const u32 row = (kk >> 9) & 0xFFu, col = kk & 0x1FFu;
+      u32 j = row ? hash_find(tabKey, tabVal, kk - 512u) : kInvalid;
+      if (j != kInvalid) { uf_union(parent, i, j); continue; }
+      if (row && col + 1 < g.C) { j = hash_find(tabKey, tabVal, kk - 511u); if (j != kInvalid) uf_union(parent, i, j); }
+      j = col ? hash_find(tabKey, tabVal, kk - 1u) : kInvalid;
+      if (j != kInvalid) uf_union(parent, i, j);
+      else if (row && col) { j = hash_find(tabKey, tabVal, kk - 513u); if (j != kInvalid) uf_union(parent, i, j); }
+    }
+    __syncthreads();
+    // D: flatten and push every kept digi on its root's member list
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      if (i >= n || parent[i] == kInvalid) continue;
+      const u32 rt = uf_find(parent, i);
+      if (rt != i) parent[i] = rt;
+      next[i] = atomicExch(head + rt, i);
+    }
+    __syncthreads();
+    // E: each root walks its list: exact fixed-point sums (A9), cluster threshold
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      const bool isRoot = i < n && parent[i] == i;
+      bool keptC = false;
+      csz[k] = 0; cq[k] = cr[k] = cc[k] = 0.f;
+      if (isRoot) {
+        u64 S = 0, Sx = 0, Sy = 0; u32 sz = 0;
+        for (u32 j = head[i]; j != kInvalid; j = next[j]) {
+          const u32 kj = key[j];
+          const u64 qf = (u64)__float2ll_rz(qs[j] * 16384.0f);
+          S += qf; Sx += qf * ((kj >> 9) & 0xFFu); Sy += qf * (kj & 0x1FFu); ++sz;
+        }
+        keptC = (i64)S >= g.clusThrFixed;
+        if (keptC) {
+          const double dS = __ll2double_rn((i64)S);
+          cq[k] = __double2float_rn(dS * (1.0 / 16384.0));
+          cr[k] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sx), dS));
+          cc[k] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sy), dS));
+          csz[k] = sz;
+        }
+      }
+      kb[k] = __ballot_sync(0xFFFFFFFFu, keptC);
+      const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
+      keptMask |= (u32)keptC << k;
+      if (lane == 0) { sh.cnt[0][k * 8 + warp] = __popc(kb[k]); sh.cnt[1][k * 8 + warp] = __popc(rb); sh.kb[k * 8 + warp] = kb[k]; }
+    }
+    __syncthreads();
+    if (warp == 0) {
+      const u32 c0 = sh.cnt[0][lane], c1 = sh.cnt[1][lane];
+      const u32 inc = warp_incl_scan(c0, lane);
+      const u32 t1 = __reduce_add_sync(0xFFFFFFFFu, c1);
+      sh.offs[lane] = inc - c0;
+      if (lane == 31) { sh.offs[32] = inc; sh.scan[0] = t1; }
+    }
+    __syncthreads();
+    total = sh.offs[32]; nAll = sh.scan[0];
+    // local number of every kept root goes to head[root] (lists are no longer needed)
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      if (i < n && parent[i] == i)
+        head[i] = (keptMask >> k & 1) ? sh.offs[k * 8 + warp] + __popc(kb[k] & ((1u << lane) - 1u)) : kInvalid;
+    }
+  }
+  // F: cross-module look-back through the range's last module
+  const u32 mLast = m1 - 1;
+  if (warp == 0) {
+    u32 ec = 0, em = 0;
+    if (mLast > 0) {
+      if (lane == 0) st_state(ev.modState + mLast, pack_state(kStAgg, total, 0));
+      if (m0 > 0) lookback(ev.modState, 0, (int)m0, lane, &ec, &em);
+    }
+    if (lane == 0) { st_state(ev.modState + mLast, pack_state(kStIncl, ec + total, 0)); sh.base = ec; }
+  }
+  __syncthreads();
+  const u32 base = sh.base;
+  // G: outputs
+  if (n > 0) {
+#pragma unroll
+    for (int k = 0; k < kPerThread; ++k) {
+      const u32 i = k * kClusterThreads + tid;
+      if (i >= n) continue;
+      const u32 p = parent[i];
+      u32 lab = kInvalid; int32_t cl = -1;
+      if (p != kInvalid) {
+        lab = s + p;
+        const u32 kn = head[p];
+        cl = kn == kInvalid ? -1 : (int32_t)(base + kn);
+      }
+      ev.label[s + i] = lab; ev.clus[s + i] = cl;
+      if (keptMask >> k & 1) {
+        const u32 o = base + head[i];
+        if (o < ev.cap) {
+          ev.clLabel[o] = s + i; ev.clModule[o] = (u16)(key[i] >> 17); ev.clSize[o] = csz[k];
+          ev.clCharge[o] = cq[k]; ev.clRow[o] = cr[k]; ev.clCol[o] = cc[k];
+        }
+      }
+    }
+  }
+  // modClusStart[m] = base + kept clusters rooted before the module's first digi
+  for (u32 m = m0 + tid; m < m1; m += kClusterThreads)
+    ev.modClusStart[m] = base + (n > 0 ? kept_prefix(sh, ev.modDigiStart[m] - s, total) : 0u);
+  if (tid == 0 && nAll) atomicAdd(&ev.counters->nClustersAll, nAll);
+  *baseOut = base;
+  return total;
+}
+
+// ---- dense path: one module m with digis [s, s+nn), in two halves so that the caller can publish
+// the module's count before it waits for anything (count) and write outputs later (output).
+// `deferred`: shared memory will be reused in between, so every array that must survive lives in
+// the global workspace tier.
+struct DenseCtx {
+  u32 *perm, *parent, *root, *csize; int32_t* knum; u64 *S, *Sx, *Sy;
+  u32 nAll, nKept;
+};
+
+__device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32 s, u32 nn, bool deferred,
+                                            unsigned char* smemRaw, ClusterShared& sh, DenseCtx& cx) {
+  const int tid = threadIdx.x, lane = tid & 31;
   const u32 bwPad = (g.bitmapWords + 3) & ~3u;
   u64* smS = reinterpret_cast<u64*>(smemRaw);
   u64* smSx = smS + kSmemClusters;
@@ -370,198 +613,244 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   u32* smRoot = smParent + kSmemDigis;
   u32* smSize = smRoot + kSmemClusters;
   int32_t* smKnum = reinterpret_cast<int32_t*>(smSize + kSmemClusters);
-
-  const u32 totalModules = nEv * g.M;
+  u32* sScan = sh.scan;
   const u32 stride = g.stride;
+
+  const bool digiInSmem = !deferred && nn <= kSmemDigis;
+  u32* perm = digiInSmem ? smPerm : ev.wsPerm + s;
+  u32* parent = digiInSmem ? smParent : ev.wsParent + s;
+  cx.perm = perm; cx.parent = parent;
+  cx.root = smRoot; cx.csize = smSize; cx.knum = smKnum; cx.S = smS; cx.Sx = smSx; cx.Sy = smSy;
+
+  // P0: clear the occupancy bitmap, init perm
+  for (u32 i = tid; i < g.bitmapWords; i += kClusterThreads) smBitmap[i] = 0;
+  for (u32 i = tid; i < nn; i += kClusterThreads) perm[i] = kInvalid;
+  __syncthreads();
+  // P1: kept flag (A8: q >= pixThr) and occupancy bits at padded coordinates (row+1, col+1)
+  u32 myKept = 0;
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    const float q = ev.charge[s + i];
+    const bool kept = q >= g.pixThr;
+    parent[i] = kept ? i : kInvalid;
+    if (kept) {
+      const u32 b = ev.col[s + i] + 1u, wd = (ev.row[s + i] + 1u) * stride + (b >> 5);
+      atomicOr(smBitmap + wd, 1u << (b & 31));
+      ++myKept;
+    }
+  }
+  myKept = __reduce_add_sync(0xFFFFFFFFu, myKept);
+  __syncthreads();
+  // P2: exclusive popcount prefix per bitmap word (contiguous chunk per thread)
+  {
+    const u32 per = (g.bitmapWords + kClusterThreads - 1) / kClusterThreads;
+    const u32 lo = min(tid * per, g.bitmapWords), hi = min(lo + per, g.bitmapWords);
+    u32 sum = 0;
+    for (u32 i = lo; i < hi; ++i) sum += __popc(smBitmap[i]);
+    u32 tot;
+    u32 run = block_excl_scan(sum, sScan, &tot);
+    for (u32 i = lo; i < hi; ++i) { smPrefix[i] = run; run += __popc(smBitmap[i]); }
+  }
+  if (lane == 0 && myKept) atomicAdd(&ev.counters->nKept, myKept);
+  __syncthreads();
+  // P3: owner of each occupied pixel = the minimum digi index on it (duplicates, A6)
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    if (parent[i] == kInvalid) continue;
+    const u32 b = ev.col[s + i] + 1u, wd = (ev.row[s + i] + 1u) * stride + (b >> 5);
+    const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
+    atomicMin(perm + r, i);
+  }
+  __syncthreads();
+  // P4: unions with the backward neighbours (W, NW, N, NE), decision tree:
+  //     N ? {N} : { NE?, W ? {W} : NW? }   — spans every 8-adjacency once all pixels did it.
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    if (parent[i] == kInvalid) continue;
+    const u32 prow = ev.row[s + i] + 1u, b = ev.col[s + i] + 1u;
+    const u32 wd = prow * stride + (b >> 5);
+    const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
+    const u32 owner = perm[r];
+    if (owner != i) { uf_union(parent, i, owner); continue; }
+    const u32 pos = b - 1u, w0 = pos >> 5, shf = pos & 31u;
+    const u32 rowAbove = (prow - 1u) * stride, rowSelf = prow * stride;
+    const u32 nb = __funnelshift_r(smBitmap[rowAbove + w0], smBitmap[rowAbove + w0 + 1], shf) & 7u;
+    const u32 cb = __funnelshift_r(smBitmap[rowSelf + w0], smBitmap[rowSelf + w0 + 1], shf) & 7u;
+    auto owner_at = [&](u32 rowBase, u32 bb) -> u32 {
+      const u32 ww = rowBase + (bb >> 5);
+      return perm[smPrefix[ww] + __popc(smBitmap[ww] & ((1u << (bb & 31)) - 1u))];
+    };
+    if (nb & 2u) {
+      uf_union(parent, i, owner_at(rowAbove, b));
+    } else {
+      if (nb & 4u) uf_union(parent, i, owner_at(rowAbove, b + 1u));
+      if (cb & 1u) uf_union(parent, i, owner_at(rowSelf, b - 1u));
+      else if (nb & 1u) uf_union(parent, i, owner_at(rowAbove, b - 1u));
+    }
+  }
+  __syncthreads();
+  // P5: flatten (roots are stable now)
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    if (parent[i] == kInvalid) continue;
+    const u32 rt = uf_find(parent, i);
+    if (rt != i) parent[i] = rt;
+  }
+  __syncthreads();
+  // P6: ordinal of every root in ascending index (= ascending label) order -> perm[root]
+  {
+    const u32 per = (nn + kClusterThreads - 1) / kClusterThreads;
+    const u32 lo = min(tid * per, nn), hi = min(lo + per, nn);
+    u32 c = 0;
+    for (u32 i = lo; i < hi; ++i) c += (parent[i] == i);
+    u32 run = block_excl_scan(c, sScan, &cx.nAll);
+    if (deferred || cx.nAll > kSmemClusters) {
+      cx.root = ev.wsRoot + s; cx.csize = ev.wsSize + s; cx.knum = ev.wsKnum + s;
+      cx.S = ev.wsS + s; cx.Sx = ev.wsSx + s; cx.Sy = ev.wsSy + s;
+    }
+    for (u32 i = lo; i < hi; ++i)
+      if (parent[i] == i) { perm[i] = run; cx.root[run] = i; ++run; }
+  }
+  // P7: zero the accumulators
+  for (u32 c = tid; c < cx.nAll; c += kClusterThreads) { cx.S[c] = 0; cx.Sx[c] = 0; cx.Sy[c] = 0; cx.csize[c] = 0; }
+  __syncthreads();
+  // P8: exact fixed-point sums (A9): qf = q * 2^14 is an integer for every kept digi
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    const u32 p = parent[i];
+    if (p == kInvalid) continue;
+    const u32 c = perm[p];
+    const u64 qf = (u64)__float2ll_rz(ev.charge[s + i] * 16384.0f);
+    atomicAdd(reinterpret_cast<unsigned long long*>(cx.S + c), (unsigned long long)qf);
+    atomicAdd(reinterpret_cast<unsigned long long*>(cx.Sx + c), (unsigned long long)(qf * ev.row[s + i]));
+    atomicAdd(reinterpret_cast<unsigned long long*>(cx.Sy + c), (unsigned long long)(qf * ev.col[s + i]));
+    atomicAdd(cx.csize + c, 1u);
+  }
+  __syncthreads();
+  // P9: cluster threshold (A8, A9) and local numbering of kept clusters
+  {
+    const u32 per = (cx.nAll + kClusterThreads - 1) / kClusterThreads;
+    const u32 lo = min(tid * per, cx.nAll), hi = min(lo + per, cx.nAll);
+    u32 c = 0;
+    for (u32 k = lo; k < hi; ++k) c += ((i64)cx.S[k] >= g.clusThrFixed);
+    u32 run = block_excl_scan(c, sScan, &cx.nKept);
+    for (u32 k = lo; k < hi; ++k) cx.knum[k] = ((i64)cx.S[k] >= g.clusThrFixed) ? (int32_t)run++ : -1;
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ void dense_output(const EvDesc& ev, u32 m, u32 s, u32 nn, u32 base, const DenseCtx& cx) {
+  const int tid = threadIdx.x;
+  for (u32 k = tid; k < cx.nAll; k += kClusterThreads) {
+    const int32_t kn = cx.knum[k];
+    if (kn < 0) continue;
+    const u32 o = base + (u32)kn;
+    if (o >= ev.cap) continue;                      // cannot happen (N <= D <= cap); stay in bounds
+    const double dS = __ll2double_rn((i64)cx.S[k]);
+    ev.clLabel[o] = s + cx.root[k];
+    ev.clModule[o] = (u16)m;
+    ev.clSize[o] = cx.csize[k];
+    ev.clCharge[o] = __double2float_rn(dS * (1.0 / 16384.0));
+    ev.clRow[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)cx.Sx[k]), dS));
+    ev.clCol[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)cx.Sy[k]), dS));
+  }
+  for (u32 i = tid; i < nn; i += kClusterThreads) {
+    const u32 p = cx.parent[i];
+    u32 lab = kInvalid; int32_t cl = -1;
+    if (p != kInvalid) {
+      lab = s + p;
+      const int32_t kn = cx.knum[cx.perm[p]];
+      cl = kn < 0 ? -1 : (int32_t)(base + (u32)kn);
+    }
+    ev.label[s + i] = lab;
+    ev.clus[s + i] = cl;
+  }
+  if (tid == 0) {
+    ev.modClusStart[m] = base;
+    if (cx.nAll) atomicAdd(&ev.counters->nClustersAll, cx.nAll);
+  }
+}
+
+template <bool kSingle>
+__device__ __forceinline__ const EvDesc& pick_event_by_window(const EvDesc& single, const EvDesc* batch, u32 nEv, u32 t) {
+  if (kSingle) return single;
+  u32 lo = 0, hi = nEv - 1;                          // last event with winBase <= t
+  while (lo < hi) {
+    u32 mid = (lo + hi + 1) >> 1;
+    if (batch[mid].winBase <= t) lo = mid; else hi = mid - 1;
+  }
+  return batch[lo];
+}
+
+template <bool kSingle>
+__global__ void __launch_bounds__(kClusterThreads)
+k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 totalWindows,
+          LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+  extern __shared__ __align__(16) unsigned char smemRaw[];
+  __shared__ ClusterShared sh;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
   for (;;) {
     __syncthreads();
-    if (tid == 0) sTicket = atomicAdd(&lc->modTicket, 1u);
+    if (tid == 0) sh.ticket = atomicAdd(&lc->modTicket, 1u);
     __syncthreads();
-    const u32 ticket = sTicket;
-    if (ticket >= totalModules) break;
-    const u32 e = kSingle ? 0u : ticket / g.M, m = kSingle ? ticket : ticket - e * g.M;
-    const EvDesc& ev = kSingle ? single : batch[e];
-    const u32 s = ev.modDigiStart[m], n = ev.modDigiStart[m + 1] - s;
-    const bool order_bad = (ev.counters->status & 1u) != 0;   // outputs undefined then; stay in bounds
-    const u32 nn = (order_bad || s + n > ev.cap || s > ev.cap) ? 0u : n;
-
-    u32 nKeptDigis = 0, nAll = 0, nKeptClusters = 0;
-    const bool digiInSmem = nn <= kSmemDigis;
-    u32* perm = digiInSmem ? smPerm : ev.wsPerm + s;
-    u32* parent = digiInSmem ? smParent : ev.wsParent + s;
-    bool clInSmem = true;
-    u32* root = smRoot; u32* csize = smSize; int32_t* knum = smKnum; u64 *S = smS, *Sx = smSx, *Sy = smSy;
-
-    if (nn > 0) {
-      // P0: clear the occupancy bitmap, init perm
-      for (u32 i = tid; i < g.bitmapWords; i += kClusterThreads) smBitmap[i] = 0;
-      for (u32 i = tid; i < nn; i += kClusterThreads) perm[i] = kInvalid;
-      __syncthreads();
-      // P1: kept flag (A8: q >= pixThr) and occupancy bits at padded coordinates (row+1, col+1)
-      u32 myKept = 0;
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        const float q = ev.charge[s + i];
-        const bool kept = q >= g.pixThr;
-        parent[i] = kept ? i : kInvalid;
-        if (kept) {
-          const u32 b = ev.col[s + i] + 1u, wd = (ev.row[s + i] + 1u) * stride + (b >> 5);
-          atomicOr(smBitmap + wd, 1u << (b & 31));
-          ++myKept;
+    const u32 ticket = sh.ticket;
+    if (ticket >= totalWindows) break;
+    const EvDesc& ev = pick_event_by_window<kSingle>(single, batch, nEv, ticket);
+    const u32 j = ticket - ev.winBase;
+    const u32 wi = ev.winInv[j];
+    // An event that violated the input contract (A5) has undefined modDigiStart: no per-digi work.
+    const bool bad = (ev.counters->status & 1u) != 0;
+    if (wi != 0 && !bad) {
+      const u32 first = g.M - wi, hi = (j + 1) << kWindowLog2;
+      // modules whose first digi lies in this window: [first, mEnd)
+      u32 mEnd = first;
+      for (;;) {
+        const u32 m = mEnd + tid;
+        const int c = __syncthreads_count(m < g.M && ev.modDigiStart[m] < hi);
+        mEnd += (u32)c;
+        if (c < kClusterThreads) break;
+      }
+      const u32 s = ev.modDigiStart[first];
+      const u32 sLastMod = ev.modDigiStart[mEnd - 1], sEnd = ev.modDigiStart[mEnd];
+      const bool bigLast = sEnd - sLastMod > kWindow;
+      const u32 smallEnd = bigLast ? mEnd - 1 : mEnd;
+      const bool haveSmall = smallEnd > first;
+      const bool sane = s <= sLastMod && sLastMod <= sEnd && sEnd <= ev.cap && (!haveSmall || ev.modDigiStart[smallEnd] - s < kRangeCap);
+      if (sane) {
+        DenseCtx cx;
+        const u32 mBig = mEnd - 1, nBig = sEnd - sLastMod;
+        if (bigLast) {
+          // count the big module FIRST and publish its aggregate, so nobody waits on this CTA
+          dense_count(ev, g, sLastMod, nBig, haveSmall, smemRaw, sh, cx);
+          if (tid == 0 && mBig > 0) st_state(ev.modState + mBig, pack_state(kStAgg, cx.nKept, 0));
         }
-      }
-      myKept = __reduce_add_sync(0xFFFFFFFFu, myKept);
-      __syncthreads();
-      // P2: exclusive popcount prefix per bitmap word (contiguous chunk per thread)
-      {
-        const u32 per = (g.bitmapWords + kClusterThreads - 1) / kClusterThreads;
-        const u32 lo = min(tid * per, g.bitmapWords), hi = min(lo + per, g.bitmapWords);
-        u32 sum = 0;
-        for (u32 i = lo; i < hi; ++i) sum += __popc(smBitmap[i]);
-        u32 tot;
-        u32 run = block_excl_scan(sum, sScan, &tot);
-        for (u32 i = lo; i < hi; ++i) { smPrefix[i] = run; run += __popc(smBitmap[i]); }
-      }
-      if (lane == 0 && myKept) atomicAdd(&ev.counters->nKept, myKept);
-      nKeptDigis = 1;   // (only used as "did work" marker below)
-      __syncthreads();
-      // P3: owner of each occupied pixel = the minimum digi index on it (duplicates, A6)
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        if (parent[i] == kInvalid) continue;
-        const u32 b = ev.col[s + i] + 1u, wd = (ev.row[s + i] + 1u) * stride + (b >> 5);
-        const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
-        atomicMin(perm + r, i);
-      }
-      __syncthreads();
-      // P4: unions with the backward neighbours (W, NW, N, NE), decision tree:
-      //     N ? {N} : { NE?, W ? {W} : NW? }   — spans every 8-adjacency once all pixels did it.
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        if (parent[i] == kInvalid) continue;
-        const u32 prow = ev.row[s + i] + 1u, b = ev.col[s + i] + 1u;
-        const u32 wd = prow * stride + (b >> 5);
-        const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
-        const u32 owner = perm[r];
-        if (owner != i) { uf_union(parent, i, owner); continue; }
-        const u32 pos = b - 1u, w0 = pos >> 5, sh = pos & 31u;
-        const u32 rowAbove = (prow - 1u) * stride, rowSelf = prow * stride;
-        const u32 nb = __funnelshift_r(smBitmap[rowAbove + w0], smBitmap[rowAbove + w0 + 1], sh) & 7u;
-        const u32 cb = __funnelshift_r(smBitmap[rowSelf + w0], smBitmap[rowSelf + w0 + 1], sh) & 7u;
-        // rank of a pixel at padded (rowBase, bit position bb)
-        auto owner_at = [&](u32 rowBase, u32 bb) -> u32 {
-          const u32 ww = rowBase + (bb >> 5);
-          return perm[smPrefix[ww] + __popc(smBitmap[ww] & ((1u << (bb & 31)) - 1u))];
-        };
-        if (nb & 2u) {
-          uf_union(parent, i, owner_at(rowAbove, b));
-        } else {
-          if (nb & 4u) uf_union(parent, i, owner_at(rowAbove, b + 1u));
-          if (cb & 1u) uf_union(parent, i, owner_at(rowSelf, b - 1u));
-          else if (nb & 1u) uf_union(parent, i, owner_at(rowAbove, b - 1u));
+        u32 base = 0, total = 0;
+        if (haveSmall) {
+          total = cluster_range_sparse(ev, g, first, smallEnd, s, ev.modDigiStart[smallEnd] - s, smemRaw, sh, &base);
+          base += total;
+        } else if (bigLast) {
+          if (warp == 0) {
+            u32 ec = 0, em = 0;
+            if (mBig > 0) lookback(ev.modState, 0, (int)mBig, lane, &ec, &em);
+            if (lane == 0) sh.base = ec;
+          }
+          __syncthreads();
+          base = sh.base;
         }
-      }
-      __syncthreads();
-      // P5: flatten (roots are stable now)
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        if (parent[i] == kInvalid) continue;
-        const u32 rt = uf_find(parent, i);
-        if (rt != i) parent[i] = rt;
-      }
-      __syncthreads();
-      // P6: ordinal of every root in ascending index (= ascending label) order -> perm[root]
-      {
-        const u32 per = (nn + kClusterThreads - 1) / kClusterThreads;
-        const u32 lo = min(tid * per, nn), hi = min(lo + per, nn);
-        u32 c = 0;
-        for (u32 i = lo; i < hi; ++i) c += (parent[i] == i);
-        u32 run = block_excl_scan(c, sScan, &nAll);
-        clInSmem = nAll <= kSmemClusters;
-        if (!clInSmem) {
-          root = ev.wsRoot + s; csize = ev.wsSize + s; knum = ev.wsKnum + s;
-          S = ev.wsS + s; Sx = ev.wsSx + s; Sy = ev.wsSy + s;
+        if (bigLast) {
+          if (tid == 0) st_state(ev.modState + mBig, pack_state(kStIncl, base + cx.nKept, 0));
+          dense_output(ev, mBig, sLastMod, nBig, base, cx);
+          base += cx.nKept;
         }
-        for (u32 i = lo; i < hi; ++i)
-          if (parent[i] == i) { perm[i] = run; root[run] = i; ++run; }
-      }
-      // P7: zero the accumulators
-      for (u32 c = tid; c < nAll; c += kClusterThreads) { S[c] = 0; Sx[c] = 0; Sy[c] = 0; csize[c] = 0; }
-      __syncthreads();
-      // P8: exact fixed-point sums (A9): qf = q * 2^14 is an integer for every kept digi
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        const u32 p = parent[i];
-        if (p == kInvalid) continue;
-        const u32 c = perm[p];
-        const u64 qf = (u64)__float2ll_rz(ev.charge[s + i] * 16384.0f);
-        atomicAdd(reinterpret_cast<unsigned long long*>(S + c), (unsigned long long)qf);
-        atomicAdd(reinterpret_cast<unsigned long long*>(Sx + c), (unsigned long long)(qf * ev.row[s + i]));
-        atomicAdd(reinterpret_cast<unsigned long long*>(Sy + c), (unsigned long long)(qf * ev.col[s + i]));
-        atomicAdd(csize + c, 1u);
-      }
-      __syncthreads();
-      // P9: cluster threshold (A8, A9) and local numbering of kept clusters
-      {
-        const u32 per = (nAll + kClusterThreads - 1) / kClusterThreads;
-        const u32 lo = min(tid * per, nAll), hi = min(lo + per, nAll);
-        u32 c = 0;
-        for (u32 k = lo; k < hi; ++k) c += ((i64)S[k] >= g.clusThrFixed);
-        u32 run = block_excl_scan(c, sScan, &nKeptClusters);
-        for (u32 k = lo; k < hi; ++k) knum[k] = ((i64)S[k] >= g.clusThrFixed) ? (int32_t)run++ : -1;
-      }
-    }
-    // P10: dense numbering across modules: decoupled look-back over the event's modules
-    if (warp == 0) {
-      u32 ec = 0, em = 0;
-      if (m > 0) {
-        if (lane == 0) st_state(ev.modState + m, pack_state(kStAgg, nKeptClusters, 0));
-        lookback(ev.modState, 0, (int)m, lane, &ec, &em);
-      }
-      if (lane == 0) {
-        st_state(ev.modState + m, pack_state(kStIncl, ec + nKeptClusters, 0));
-        sBase = ec;
+        if (mEnd == g.M && tid == 0) { ev.modClusStart[g.M] = base; ev.counters->nClusters = base; }
+      } else if (tid == 0) {
+        atomicOr(&ev.counters->status, 2u);            // PR_STATUS_CAPACITY: inconsistent module table
       }
     }
     __syncthreads();
-    const u32 base = sBase;
-    // P11: outputs
-    if (nn > 0) {
-      for (u32 k = tid; k < nAll; k += kClusterThreads) {
-        const int32_t kn = knum[k];
-        if (kn < 0) continue;
-        const u32 o = base + (u32)kn;
-        if (o >= ev.cap) continue;                      // cannot happen (N <= D <= cap); stay in bounds
-        const double dS = __ll2double_rn((i64)S[k]);
-        ev.clLabel[o] = s + root[k];
-        ev.clModule[o] = (u16)m;
-        ev.clSize[o] = csize[k];
-        ev.clCharge[o] = __double2float_rn(dS * (1.0 / 16384.0));
-        ev.clRow[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sx[k]), dS));
-        ev.clCol[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sy[k]), dS));
-      }
-      for (u32 i = tid; i < nn; i += kClusterThreads) {
-        const u32 p = parent[i];
-        u32 lab = kInvalid; int32_t cl = -1;
-        if (p != kInvalid) {
-          lab = s + p;
-          const int32_t kn = knum[perm[p]];
-          cl = kn < 0 ? -1 : (int32_t)(base + (u32)kn);
-        }
-        ev.label[s + i] = lab;
-        ev.clus[s + i] = cl;
-      }
-    } else if (order_bad) {
-      // undefined-but-initialised outputs for an event that violated the input contract
-      for (u32 i = tid; i < n && s + i < ev.cap; i += kClusterThreads) { ev.label[s + i] = kInvalid; ev.clus[s + i] = -1; }
-    }
     if (tid == 0) {
-      ev.modClusStart[m] = base;
-      if (nAll) atomicAdd(&ev.counters->nClustersAll, nAll);
-      if (m == g.M - 1) { ev.modClusStart[g.M] = base + nKeptClusters; ev.counters->nClusters = base + nKeptClusters; }
       __threadfence();
-      sLast = (atomicAdd(&lc->modDone, 1u) == totalModules - 1);
+      sh.last = (atomicAdd(&lc->modDone, 1u) == totalWindows - 1);
     }
-    (void)nKeptDigis;
     __syncthreads();
-    if (sLast) {
-      // the launch's last module: publish every event's counters to mapped pinned host memory
+    if (sh.last) {
+      // the launch's last unit: publish every event's counters to mapped pinned host memory
       __threadfence();
       for (u32 k = tid; k < nEv; k += kClusterThreads) {
         const EvDesc& d = kSingle ? single : batch[k];

@@ -41,6 +41,8 @@ struct pr_handle {
   std::atomic<uint64_t> evAcquired{0}, evProduced{0}, words{0}, digis{0}, clusters{0}, launches{0}, memcpys{0}, callbacks{0};
   std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
   std::atomic<int> sticky{0};
+  bool timing = false;
+  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msExport = 0;   // guarded by mu
   std::string lastCuda;
 };
 
@@ -66,6 +68,8 @@ struct pr_event {
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
   int status = PR_OK;        // filled when completion is observed
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
+  cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING
+  bool exported = false;
 };
 
 namespace {
@@ -183,7 +187,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // ---- layout
   ev->sub.assign(n, SubEvent());
   size_t devBytes = 0, hostBytes = 0;
-  uint32_t totalTiles = 0;
+  uint32_t totalTiles = 0, totalWindows = 0;
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     s.in = ins[k];
@@ -195,8 +199,12 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     s.desc.tileBase = totalTiles;
     s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
     totalTiles += s.desc.nTiles;
+    s.desc.winBase = totalWindows;
+    s.desc.nWin = (s.in.n_words >> kWindowLog2) + 1;
+    totalWindows += s.desc.nWin;
   }
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * M * n + (size_t)8 * totalTiles;
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * M * n + (size_t)8 * totalTiles +
+                         (size_t)4 * totalWindows;
 
   // ---- buffers from the pools (steady state: cache hits only)
   if (ev->ctlBytes < ctlNeed) {
@@ -231,6 +239,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
   u64* modState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
   u64* tileState = modState + (size_t)M * n;
+  u32* winInv = (u32*)(tileState + totalTiles);
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
   for (uint32_t k = 0; k < n; ++k) {
@@ -241,7 +250,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.adc = stage ? stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
-    d.modState = modState + (size_t)M * k; d.tileState = tileState + d.tileBase;
+    d.modState = modState + (size_t)M * k; d.tileState = tileState + d.tileBase; d.winInv = winInv + d.winBase;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
@@ -258,13 +267,14 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       PR_CUDA(h, cudaMemcpyAsync(stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
       nMemcpy += 2;
     }
-  const uint32_t totalModules = M * n;
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
-  if (clusterGrid > totalModules) clusterGrid = totalModules;
+  if (clusterGrid > totalWindows) clusterGrid = totalWindows;
+  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
     k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, 1, lc, h->geom);
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, totalWindows, lc, h->geom);
   } else {
     EvDesc* st = (EvDesc*)ev->descStage;
     for (uint32_t k = 0; k < n; ++k) st[k] = ev->sub[k].desc;
@@ -272,10 +282,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ++nMemcpy;
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, totalWindows, lc, h->geom);
   }
   nLaunch += 2;
   PR_CUDA(h, cudaGetLastError());
+  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+  ev->exported = want != 0;
   if (want) {
     // exact-size mirrors: the item table lives at the head of the pinned slab's tail (mapped memory)
     std::vector<ExportItem> items;
@@ -306,6 +319,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ++nLaunch;
     PR_CUDA(h, cudaGetLastError());
   }
+  if (h->timing && want) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
   PR_CUDA(h, cudaEventRecord(ev->done, stream));
   ev->n = n;
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
@@ -338,6 +352,14 @@ int poll(pr_event* ev) {
   }
   ev->status = worst;
   ev->state = kDone;
+  if (ev->h->timing) {
+    float a = 0, b = 0, c = 0;
+    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess) {
+      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[2], ev->tev[3]) != cudaSuccess) c = 0;
+      std::lock_guard<std::mutex> g(ev->h->mu);
+      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msExport += c;
+    } else cudaGetLastError();
+  }
   ev->h->inFlight.fetch_sub(1);
   ev->h->evProduced.fetch_add(ev->n); ev->h->digis.fetch_add(dg); ev->h->clusters.fetch_add(cl);
   return PR_OK;
@@ -392,7 +414,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   *out = nullptr;
   if (!cfg || cfg->struct_size != sizeof(pr_config)) return PR_ERR_INVALID_ARG;
   if (cfg->n_modules < 1 || cfg->n_modules > 2048 || cfg->n_rows < 1 || cfg->n_rows > 256 || cfg->n_cols < 1 ||
-      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || cfg->flags)
+      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~PR_FLAG_KERNEL_TIMING))
     return PR_ERR_INVALID_ARG;
   // A9/A21: ranges that make the 2^-14 fixed-point sums exact and overflow-free
   if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||
@@ -410,6 +432,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   if (!h) return PR_ERR_OOM;
   h->cfg = *cfg;
   h->cfg.gain = h->cfg.pedestal = nullptr;
+  h->timing = (cfg->flags & PR_FLAG_KERNEL_TIMING) != 0;
   auto fail = [&](int code) { pr_destroy(h); return code; };
   if (cudaSetDevice(cfg->device) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
   cudaDeviceProp prop{};
@@ -444,7 +467,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * g.M + (size_t)8 * tiles;
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * g.M + (size_t)8 * tiles + (size_t)4 * ((cap >> kWindowLog2) + 1);
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
@@ -470,6 +493,7 @@ int pr_destroy(pr_handle* h) {
     if (ev->ctl) h->devPool->free(ev->ctl, nullptr, true);
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
     if (ev->done) cudaEventDestroy(ev->done);
+    for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
@@ -489,6 +513,8 @@ int pr_event_create(pr_handle* h, pr_event** out) {
   ev->h = h;
   cudaError_t e = cudaEventCreateWithFlags(&ev->done, cudaEventDisableTiming);
   if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
+  if (h->timing)
+    for (int i = 0; i < 4; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
   { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
   *out = ev;
   return PR_OK;
@@ -502,6 +528,7 @@ int pr_event_destroy(pr_event* ev) {
   if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
   if (ev->done) cudaEventDestroy(ev->done);
+  for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
   {
     std::lock_guard<std::mutex> g(h->mu);
     for (size_t i = 0; i < h->slots.size(); ++i)
@@ -544,6 +571,19 @@ int pr_release(pr_event* ev) {
 
 void* pr_event_cuda_event(pr_event* ev) { return ev ? (void*)ev->done : nullptr; }
 
+int pr_stream_wait_event(pr_event* ev, void* consumer_stream) {
+  if (!ev) return PR_ERR_INVALID_ARG;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  if (ev->state == kDone) return PR_OK;
+  PR_CUDA(ev->h, cudaSetDevice(ev->h->cfg.device));
+  cudaError_t r = cudaEventQuery(ev->done);
+  if (r == cudaSuccess) return PR_OK;
+  if (r != cudaErrorNotReady) return cuda_fail(ev->h, r, "cudaEventQuery");
+  cudaGetLastError();
+  PR_CUDA(ev->h, cudaStreamWaitEvent((cudaStream_t)consumer_stream, ev->done, 0));
+  return PR_OK;
+}
+
 void* pr_host_alloc(pr_handle* h, size_t bytes) { return h ? h->hostPool->alloc(bytes, nullptr) : nullptr; }
 int pr_host_free(pr_handle* h, void* p) { return h ? h->hostPool->free(p, nullptr, true) : PR_ERR_INVALID_ARG; }
 
@@ -555,6 +595,10 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
   out->kernel_launches = h->launches.load(); out->memcpy_calls = h->memcpys.load(); out->callbacks_fired = h->callbacks.load();
   out->events_in_flight = h->inFlight.load(); out->max_events_in_flight = h->maxInFlight.load();
   h->devPool->stats(&out->device_pool); h->hostPool->stats(&out->host_pool);
+  {
+    std::lock_guard<std::mutex> g(h->mu);
+    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->export_ms = h->msExport;
+  }
   return PR_OK;
 }
 

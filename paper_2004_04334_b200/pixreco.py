@@ -28,6 +28,7 @@ PR_WANT_DIGIS, PR_WANT_CHARGE, PR_WANT_LABELS, PR_WANT_CLUSTERS, PR_WANT_ERRORS 
 PR_WANT_ALL = 31
 PR_POOL_DEVICE, PR_POOL_PINNED, PR_POOL_FAKE = 0, 1, 2
 PR_INVALID_LABEL = 0xFFFFFFFF
+PR_FLAG_KERNEL_TIMING = 1
 
 pr_done_fn = ctypes.CFUNCTYPE(None, c_void_p, c_int)
 
@@ -77,7 +78,8 @@ class pr_stats(ctypes.Structure):
     _fields_ = ([(n, c_uint64) for n in ("events_acquired", "events_produced", "words", "digis", "clusters",
                                          "kernel_launches", "memcpy_calls", "callbacks_fired")] +
                 [("events_in_flight", c_uint32), ("max_events_in_flight", c_uint32),
-                 ("device_pool", pr_pool_stats), ("host_pool", pr_pool_stats)])
+                 ("device_pool", pr_pool_stats), ("host_pool", pr_pool_stats), ("timed_acquires", c_uint64),
+                 ("unpack_ms", ctypes.c_double), ("cluster_ms", ctypes.c_double), ("export_ms", ctypes.c_double)])
 
 
 # every symbol include/pixreco.h declares: name -> (restype, argtypes)
@@ -93,6 +95,7 @@ SIGNATURES = {
     "pr_produce_batch": (c_int, [c_void_p, POINTER(pr_output), c_uint32]),
     "pr_release": (c_int, [c_void_p]),
     "pr_event_cuda_event": (c_void_p, [c_void_p]),
+    "pr_stream_wait_event": (c_int, [c_void_p, c_void_p]),
     "pr_host_alloc": (c_void_p, [c_void_p, c_size_t]),
     "pr_host_free": (c_int, [c_void_p, c_void_p]),
     "pr_get_stats": (c_int, [c_void_p, POINTER(pr_stats)]),
@@ -267,6 +270,11 @@ class EventSlot:
     def cuda_event(self) -> int:
         return lib().pr_event_cuda_event(self.ptr)
 
+    def stream_wait(self, consumer_stream) -> int:
+        """make ``consumer_stream`` wait for this slot's work unless already complete."""
+        s = getattr(consumer_stream, "cuda_stream", consumer_stream)
+        return _check(lib().pr_stream_wait_event(self.ptr, c_void_p(s)), "pr_stream_wait_event", self.owner.handle)
+
     def destroy(self):
         if self.ptr:
             _check(lib().pr_event_destroy(self.ptr), "pr_event_destroy", self.owner.handle)
@@ -277,14 +285,15 @@ class PixReco:
     """One ``pr_handle``: calibration tables + pools on one device."""
 
     def __init__(self, gain, pedestal, n_rows=160, n_cols=416, pixel_threshold_e=1000.0, cluster_threshold_e=4000.0,
-                 device=0, max_words_hint=0, max_events_in_flight=0, max_cached_bytes_device=0, max_cached_bytes_host=0):
+                 device=0, max_words_hint=0, max_events_in_flight=0, max_cached_bytes_device=0, max_cached_bytes_host=0,
+                 flags=0):
         gain = np.ascontiguousarray(gain, np.float32)
         pedestal = np.ascontiguousarray(pedestal, np.float32)
         if gain.shape != pedestal.shape or gain.ndim != 1:
             raise ValueError("gain/pedestal must be 1-D arrays of equal length")
         cfg = pr_config(ctypes.sizeof(pr_config), device, gain.shape[0], n_rows, n_cols, gain.ctypes.data,
                         pedestal.ctypes.data, pixel_threshold_e, cluster_threshold_e, max_words_hint,
-                        max_events_in_flight, max_cached_bytes_device, max_cached_bytes_host, 0)
+                        max_events_in_flight, max_cached_bytes_device, max_cached_bytes_host, flags)
         h = c_void_p()
         _check(lib().pr_create(ctypes.byref(cfg), ctypes.byref(h)), "pr_create")
         self.handle, self.device, self.n_modules = h, device, int(gain.shape[0])
@@ -319,8 +328,9 @@ class PixReco:
         _check(lib().pr_get_stats(self.handle, ctypes.byref(st)), "pr_get_stats", self.handle)
 
         def conv(s):
-            return {n: (conv(getattr(s, n)) if isinstance(getattr(s, n), ctypes.Structure) else int(getattr(s, n)))
-                    for n, _ in s._fields_}
+            return {n: (conv(getattr(s, n)) if isinstance(getattr(s, n), ctypes.Structure) else
+                        (float(getattr(s, n)) if t is ctypes.c_double else int(getattr(s, n))))
+                    for n, t in s._fields_}
         return conv(st)
 
     def close(self):

@@ -1,0 +1,231 @@
+"""GPU boundary behaviour: the acquire/produce contract of the paper, tested on the C ABI.
+
+  * acquire launches work and returns; the thread is free
+  * completion via callback on a non-framework thread, exactly once, carrying status (L35, L94)
+  * work in one stream is serial, different streams concurrent (L82, L86); results identical
+  * pool amortises runtime allocations: zero new cudaMalloc in steady state (L88-90)
+  * a consumer on another stream waits on the product's event (L108)
+  * transfers only when asked (L112)
+"""
+import ctypes
+import threading
+import time
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2004_04334_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def pr():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the product path has no CPU fallback")
+    from paper_2004_04334_b200 import pixreco
+    pixreco.lib()
+    return pixreco
+
+
+def to_dev(a):
+    v = a.view(np.int32) if a.dtype == np.uint32 else a.view(np.int16)
+    return torch.from_numpy(v.copy()).cuda()
+
+
+def wait(slot, timeout=60.0):
+    t0 = time.time()
+    while slot.query() == 1:
+        assert time.time() - t0 < timeout
+        time.sleep(0.0002)
+
+
+def test_acquire_returns_at_once_behind_a_long_queue(pr):
+    """A ~100 ms spin kernel sits in front on the same stream: pr_acquire must still return in
+    well under that, pr_query/pr_produce must say NOT_READY without waiting."""
+    ev, cal = wl.make_event(1, 0), wl.make_calib(1)
+    with pr.PixReco(cal.gain, cal.pedestal, max_words_hint=60000, max_events_in_flight=8) as p:
+        w, a = to_dev(ev.words), to_dev(ev.adc)
+        slots = [p.slot() for _ in range(8)]
+        streams = [torch.cuda.Stream() for _ in range(8)]
+        for sl, s in zip(slots, streams):          # warm every slot (ctl buffers, pool bins)
+            sl.acquire(w, a, stream=s); wait(sl); sl.produce(); sl.release()
+        torch.cuda.synchronize()
+        spin_cycles = int(0.1 * 1.5e9)
+        for s in streams:
+            with torch.cuda.stream(s):
+                torch.cuda._sleep(spin_cycles)
+        t0 = time.perf_counter()
+        for sl, s in zip(slots, streams):
+            sl.acquire(w, a, stream=s)
+        t_acq = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        states = [sl.query() for sl in slots]
+        codes = [sl.produce()[0] for sl in slots]
+        t_poll = time.perf_counter() - t0
+        assert states == [pr.PR_NOT_READY] * 8 and codes == [pr.PR_NOT_READY] * 8
+        assert t_acq < 0.02, f"8 acquires took {t_acq * 1e3:.2f} ms behind a 100 ms queue"
+        assert t_poll < 0.01
+        assert slots[0].release() == pr.PR_NOT_READY            # nothing is released while in flight
+        with pytest.raises(pr.PixRecoError):                    # acquire on a busy slot
+            slots[0].acquire(w, a, stream=streams[0])
+        for sl in slots:
+            wait(sl)
+            assert sl.produce()[0] == 0
+            sl.release()
+
+
+def test_callback_fires_once_on_another_thread_with_outputs_visible(pr):
+    ev, cal = wl.make_event(0, 0), wl.make_calib(0)
+    ref = oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal)
+    seen = []
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        holder = {}
+
+        def done(user, status):
+            # runs on a CUDA-internal thread: only record; outputs must already be visible
+            raw = pr.pr_output()
+            seen.append((threading.get_ident(), status))
+
+        for rep in range(5):
+            slot.acquire(to_dev(ev.words), to_dev(ev.adc), stream=torch.cuda.Stream(), want=pr.PR_WANT_CLUSTERS, done=done)
+            t0 = time.time()
+            while len(seen) <= rep:
+                assert time.time() - t0 < 20
+                time.sleep(0.0005)
+            code, out = slot.produce()             # after the callback: must be ready at once
+            assert code == 0 and out.n_clusters == ref.n_clusters
+            assert np.array_equal(out.host("cl_label"), ref.cl_label)
+            slot.release()
+        time.sleep(0.05)
+        assert len(seen) == 5 and all(s == 0 for _, s in seen)
+        assert all(t != threading.get_ident() for t, _ in seen)
+        assert p.stats()["callbacks_fired"] == 5
+        del holder
+
+
+def test_concurrent_streams_same_results_and_zero_steady_state_malloc(pr):
+    """configs[2] in small: 64 events, 8 in flight, slot = stream = e mod 8 (A25); every event's
+    counters and cluster labels equal the oracle's; no cudaMalloc/cudaHostAlloc after warm-up."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, e) for e in range(64)]
+    refs = [oracle.run(e.words, e.adc, e.n_modules, cal.gain, cal.pedestal) for e in evs]
+    dev = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slots = [p.slot() for _ in range(8)]
+        streams = [torch.cuda.Stream() for _ in range(8)]
+
+        def one_pass(check):
+            pending = {}
+            for e in range(64):
+                i = e % 8
+                if i in pending:
+                    wait(slots[i])
+                    code, out = slots[i].produce()
+                    check(pending.pop(i), code, out)
+                    slots[i].release()
+                slots[i].acquire(*dev[e], stream=streams[i], event_id=e)
+                pending[i] = e
+            for i, e in pending.items():
+                wait(slots[i])
+                code, out = slots[i].produce()
+                check(e, code, out)
+                slots[i].release()
+
+        def check(e, code, out):
+            r = refs[e]
+            assert code == 0 and out.event_id == e
+            assert (out.n_digis, out.n_errors, out.n_kept_digis, out.n_clusters_all, out.n_clusters) == \
+                (r.n_digis, r.n_errors, r.n_kept_digis, r.n_clusters_all, r.n_clusters)
+            assert np.array_equal(out.to_numpy("cl_label"), r.cl_label)
+            assert np.array_equal(out.to_numpy("label"), r.label)
+
+        one_pass(check)                             # warm-up fills the pools
+        s0 = p.stats()
+        for _ in range(3):
+            one_pass(lambda e, code, out: None if (code == 0 and out.n_clusters == refs[e].n_clusters) else pytest.fail("mismatch"))
+        s1 = p.stats()
+        assert s1["device_pool"]["backend_allocs"] == s0["device_pool"]["backend_allocs"]
+        assert s1["host_pool"]["backend_allocs"] == s0["host_pool"]["backend_allocs"]
+        assert s1["device_pool"]["backend_frees"] == 0
+        assert s1["max_events_in_flight"] == 8
+        assert s1["events_produced"] == 4 * 64
+
+
+def test_consumer_on_another_stream_waits_on_the_product_event(pr):
+    """cudaStreamWaitEvent(consumerStream, productEvent) instead of a host wait."""
+    ev, cal = wl.make_event(1, 1), wl.make_calib(1)
+    ref = oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal)
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        prod, cons = torch.cuda.Stream(), torch.cuda.Stream()
+        w, a = to_dev(ev.words), to_dev(ev.adc)
+        # learn the (stable) output addresses from a first run on this slot
+        slot.acquire(w, a, stream=prod); wait(slot)
+        _, out0 = slot.produce()
+        charge_ptr, n = out0.raw.d_charge, out0.n_digis
+        slot.release()
+        with torch.cuda.stream(prod):
+            torch.cuda._sleep(int(0.02 * 1.5e9))
+        slot.acquire(w, a, stream=prod)
+        assert slot.query() == pr.PR_NOT_READY
+        assert slot.stream_wait(cons) == 0                      # cudaStreamWaitEvent, no host wait
+        with torch.cuda.stream(cons):                           # consumer work queued BEFORE completion
+            class _Cai:
+                __cuda_array_interface__ = {"shape": (n,), "typestr": "<f4", "data": (charge_ptr, False), "version": 2, "strides": None}
+            early_total = torch.as_tensor(_Cai(), device="cuda").double().sum()
+        wait(slot)
+        _, out = slot.produce()
+        assert out.raw.d_charge == charge_ptr and out.n_digis == n      # same block reused (pool)
+        with torch.cuda.stream(cons):
+            total = out.device("charge").double().sum()
+        assert float(total.item()) == pytest.approx(float(ref.charge.astype(np.float64).sum()), rel=1e-12)
+        assert float(early_total.item()) == float(total.item())
+        assert slot.stream_wait(cons) == 0                      # complete: returns at once
+        slot.release()
+
+
+def test_transfers_only_when_asked(pr):
+    ev, cal = wl.make_event(0, 0), wl.make_calib(0)
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(ev.words), to_dev(ev.adc), want=0); wait(slot)
+        _, out = slot.produce()
+        assert all(out.host(f) is None for f in pr.VIEW_SPEC)
+        slot.release()
+        st = p.stats()
+        assert st["memcpy_calls"] == 0 and st["kernel_launches"] == 2       # device input, no mirrors: 2 kernels, no copies
+        slot.acquire(to_dev(ev.words), to_dev(ev.adc), want=pr.PR_WANT_ERRORS); wait(slot)
+        _, out = slot.produce()
+        assert out.host("err_idx") is not None and out.host("cl_label") is None
+        slot.release()
+        assert p.stats()["kernel_launches"] == 5                            # + export kernel
+
+
+def test_argument_and_state_errors(pr):
+    ev, cal = wl.make_event(0, 0), wl.make_calib(0)
+    lib = pr.lib()
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        out = pr.pr_output()
+        assert lib.pr_produce(slot.ptr, ctypes.byref(out)) == pr.PR_ERR_BAD_STATE      # produce before acquire
+        assert lib.pr_query(slot.ptr) == pr.PR_ERR_BAD_STATE
+        assert lib.pr_release(slot.ptr) == pr.PR_ERR_BAD_STATE
+        pageable_w, pageable_a = ev.words.copy(), ev.adc.copy()
+        inp = pr.pr_input(pageable_w.ctypes.data, pageable_a.ctypes.data, ev.n_words, pr.PR_MEM_HOST_PINNED, 0, 0, pr.pr_done_fn(), None)
+        assert lib.pr_acquire(slot.ptr, ctypes.byref(inp), None) == pr.PR_ERR_INVALID_ARG   # pageable host memory
+        w, a = to_dev(ev.words), to_dev(ev.adc)
+        inp = pr.pr_input(w.data_ptr() + 4, a.data_ptr(), ev.n_words - 1, pr.PR_MEM_DEVICE, 0, 0, pr.pr_done_fn(), None)
+        assert lib.pr_acquire(slot.ptr, ctypes.byref(inp), None) == pr.PR_ERR_INVALID_ARG   # misaligned device input
+        inp = pr.pr_input(w.data_ptr(), a.data_ptr(), ev.n_words, 7, 0, 0, pr.pr_done_fn(), None)
+        assert lib.pr_acquire(slot.ptr, ctypes.byref(inp), None) == pr.PR_ERR_INVALID_ARG
+        inp = pr.pr_input(w.data_ptr(), a.data_ptr(), ev.n_words, pr.PR_MEM_DEVICE, 0x100, 0, pr.pr_done_fn(), None)
+        assert lib.pr_acquire(slot.ptr, ctypes.byref(inp), None) == pr.PR_ERR_INVALID_ARG
+        # still usable, on the legacy default stream (NULL)
+        slot.acquire(w, a); wait(slot)
+        assert slot.produce()[0] == 0
+        slot.release()
+        slot.destroy()
