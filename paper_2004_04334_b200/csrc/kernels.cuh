@@ -67,7 +67,7 @@ struct EvDesc {
   // global workspace tier for large modules [cap] each
   u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
   DevCounters* counters; HostCounters* hostCounters;
-  u64 *tileState, *modState;        // look-back states: [nTiles], [M]
+  u64 *tileState, *winState;        // look-back states: [nTiles], [nWin]
   u32* winInv;                      // [nWin]: M - (first module starting in the window), 0 = none
   u32 winBase, nWin;                // this event's windows in the launch's flattened unit space
 };
@@ -148,6 +148,43 @@ __device__ __forceinline__ void lookback(const u64* state, int first, int self, 
   *cnt = c; *mx1 = m;
 }
 
+
+// CTA-wide decoupled look-back (blockDim = 256): thread j reads the state of unit (self-1-j), so
+// one round covers 256 predecessors.  With hundreds of units in flight, a 32-wide window needed
+// one serial L2 round trip per 32 predecessors and dominated the kernels.  Every thread returns
+// the combined (count, max1) of all predecessors in [0, self).  Contains __syncthreads.
+struct LbShared { u32 cnt[8], mx[8]; };
+__device__ __forceinline__ void lookback_cta(const u64* state, int self, LbShared& lb, u32* cnt, u32* mx1) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  u32 c = 0, m = 0;
+  int look = self - 1;
+  while (look >= 0) {                                  // block-uniform
+    const int idx = look - tid;
+    u64 v = kStIncl;                                   // virtual zero inclusive before unit 0
+    if (idx >= 0) do { v = ld_state(state + idx); } while (st_status(v) == 0);
+    const u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v) == 2);
+    const int upto = inclMask ? (__ffs(inclMask) - 1) : 31;
+    const u32 cc = lane <= upto ? st_count(v) : 0, mm = lane <= upto ? st_max1(v) : 0;
+    const u32 wc = __reduce_add_sync(0xFFFFFFFFu, cc), wm = __reduce_max_sync(0xFFFFFFFFu, mm);
+    __syncthreads();                                   // previous readers of lb are done
+    if (lane == 0) { lb.cnt[warp] = wc; lb.mx[warp] = wm | (inclMask ? 0x80000000u : 0u); }
+    __syncthreads();
+    bool found = false;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      if (!found) {
+        c += lb.cnt[k];
+        const u32 x = lb.mx[k];
+        m = max(m, x & 0xFFFu);
+        found = (x >> 31) != 0;
+      }
+    }
+    if (found) break;
+    look -= 256;
+  }
+  *cnt = c; *mx1 = m;
+}
+
 template <bool kSingle>
 __device__ __forceinline__ const EvDesc& pick_event_by_tile(const EvDesc& single, const EvDesc* batch, u32 nEv, u32 t, u32* e) {
   if (kSingle) { *e = 0; return single; }
@@ -171,7 +208,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   __shared__ __align__(16) u16 sAdc[kTileWords + 8];
   __shared__ __align__(16) u16 sOff[kTileWords + 8];
   __shared__ u32 sWsum[8], sWmax[8];
-  __shared__ u32 sLbCnt[8], sLbMax[8];
+  __shared__ LbShared sLb;
   __shared__ u32 sTicket;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -227,39 +264,13 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   }
   const u32 r0 = wbase + incl - cnt;                 // tile-local rank of this thread's first digi
 
-  // ---- decoupled look-back for the event-global digi offset and running max(module)+1.
-  // The whole CTA looks back: thread j reads the state of tile (t-1-j), so one round covers 256
-  // predecessors (with ~450 tiles in flight a 32-wide window needed ~14 serial L2 round trips).
+  // ---- decoupled look-back for the event-global digi offset and running max(module)+1
   u32 g0 = 0, carryMax1 = 0;
   {
     u64* state = ev.tileState;
     if (tile > 0) {
       if (tid == 0) st_state(state + tile, pack_state(kStAgg, tileCnt, tileMax1));
-      int look = (int)tile - 1;
-      for (;;) {
-        const int idx = look - tid;
-        u64 v = kStIncl;                               // virtual zero inclusive before the event start
-        if (idx >= 0) do { v = ld_state(state + idx); } while (st_status(v) == 0);
-        const u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v) == 2);
-        const int upto = inclMask ? (__ffs(inclMask) - 1) : 31;
-        const u32 cc = lane <= upto ? st_count(v) : 0, mm = lane <= upto ? st_max1(v) : 0;
-        const u32 wc = __reduce_add_sync(0xFFFFFFFFu, cc), wm = __reduce_max_sync(0xFFFFFFFFu, mm);
-        __syncthreads();                               // previous readers of sLb* are done
-        if (lane == 0) { sLbCnt[warp] = wc; sLbMax[warp] = wm | (inclMask ? 0x80000000u : 0u); }
-        __syncthreads();
-        bool found = false;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          if (!found) {
-            g0 += sLbCnt[k];
-            const u32 x = sLbMax[k];
-            carryMax1 = max(carryMax1, x & 0xFFFu);
-            found = (x >> 31) != 0;
-          }
-        }
-        if (found) break;
-        look -= kUnpackThreads;
-      }
+      lookback_cta(state, (int)tile, sLb, &g0, &carryMax1);
     }
     if (tid == 0) st_state(state + tile, pack_state(kStIncl, g0 + tileCnt, max(carryMax1, tileMax1)));
   }
@@ -422,6 +433,7 @@ struct ClusterShared {
   u32 kb[kPerThread * 8];           // per (k, warp): ballot of kept roots
   u32 offs[kPerThread * 8 + 1];
   u32 ticket, base, last, first;
+  LbShared lb;
 };
 
 // Number of kept roots with local index < b (b in [0, n]); valid after the scan of the sparse path.
@@ -431,9 +443,22 @@ __device__ __forceinline__ u32 kept_prefix(const ClusterShared& sh, u32 b, u32 t
   return sh.offs[k * 8 + w] + __popc(sh.kb[k * 8 + w] & ((1u << l) - 1u));
 }
 
-// ---- sparse path: modules [m0, m1) of event ev (m1 > m0), digis [s, s+n), n < kRangeCap.
+// Publish this unit's kept-cluster count, look back over the event's earlier windows, publish the
+// inclusive prefix.  Returns the dense number of the unit's first kept cluster (all threads).
+__device__ __forceinline__ u32 unit_lookback(const EvDesc& ev, u32 j, u32 total, ClusterShared& sh) {
+  u32 ec = 0, em = 0;
+  if (j > 0) {
+    if (threadIdx.x == 0) st_state(ev.winState + j, pack_state(kStAgg, total, 0));
+    lookback_cta(ev.winState, (int)j, sh.lb, &ec, &em);
+  }
+  if (threadIdx.x == 0) st_state(ev.winState + j, pack_state(kStIncl, ec + total, 0));
+  return ec;
+}
+
+// ---- sparse path: modules [m0, m1) of event ev (m1 > m0), digis [s, s+n), n < kRangeCap, all
+// starting in window j.  `extra` = kept clusters of the window's big module (numbered after these).
 // Returns the number of kept clusters; *baseOut = dense number of its first kept cluster.
-__device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom& g, u32 m0, u32 m1, u32 s, u32 n,
+__device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom& g, u32 j, u32 extra, u32 m0, u32 m1, u32 s, u32 n,
                                                     unsigned char* smemRaw, ClusterShared& sh, u32* baseOut) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   u32* tabKey = reinterpret_cast<u32*>(smemRaw);
@@ -444,8 +469,6 @@ __device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom
   u32* next = head + kRangeCap;
   float* qs = reinterpret_cast<float*>(next + kRangeCap);
 
-  // interior modules contribute through the range's last module: publish "aggregate 0" for them
-  for (u32 m = m0 + tid; m + 1 < m1; m += kClusterThreads) st_state(ev.modState + m, pack_state(kStAgg, 0, 0));
   u32 total = 0, nAll = 0;
   u32 kb[kPerThread];
   float cq[kPerThread], cr[kPerThread], cc[kPerThread]; u32 csz[kPerThread]; u32 keptMask = 0;
@@ -547,18 +570,10 @@ __device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom
         head[i] = (keptMask >> k & 1) ? sh.offs[k * 8 + warp] + __popc(kb[k] & ((1u << lane) - 1u)) : kInvalid;
     }
   }
-  // F: cross-module look-back through the range's last module
-  const u32 mLast = m1 - 1;
-  if (warp == 0) {
-    u32 ec = 0, em = 0;
-    if (mLast > 0) {
-      if (lane == 0) st_state(ev.modState + mLast, pack_state(kStAgg, total, 0));
-      if (m0 > 0) lookback(ev.modState, 0, (int)m0, lane, &ec, &em);
-    }
-    if (lane == 0) { st_state(ev.modState + mLast, pack_state(kStIncl, ec + total, 0)); sh.base = ec; }
-  }
+  // F: numbering base of this window through the cross-window look-back
   __syncthreads();
-  const u32 base = sh.base;
+  const u32 base = unit_lookback(ev, j, total + extra, sh);
+  __syncthreads();
   // G: outputs
   if (n > 0) {
 #pragma unroll
@@ -783,7 +798,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
           LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   extern __shared__ __align__(16) unsigned char smemRaw[];
   __shared__ ClusterShared sh;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x;
 
   for (;;) {
     __syncthreads();
@@ -815,33 +830,27 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       if (sane) {
         DenseCtx cx;
         const u32 mBig = mEnd - 1, nBig = sEnd - sLastMod;
-        if (bigLast) {
-          // count the big module FIRST and publish its aggregate, so nobody waits on this CTA
-          dense_count(ev, g, sLastMod, nBig, haveSmall, smemRaw, sh, cx);
-          if (tid == 0 && mBig > 0) st_state(ev.modState + mBig, pack_state(kStAgg, cx.nKept, 0));
-        }
-        u32 base = 0, total = 0;
+        if (bigLast) dense_count(ev, g, sLastMod, nBig, haveSmall, smemRaw, sh, cx);   // count first: nobody waits on us
+        const u32 nBigKept = bigLast ? cx.nKept : 0u;
+        u32 base = 0;
         if (haveSmall) {
-          total = cluster_range_sparse(ev, g, first, smallEnd, s, ev.modDigiStart[smallEnd] - s, smemRaw, sh, &base);
+          const u32 total = cluster_range_sparse(ev, g, j, nBigKept, first, smallEnd, s, ev.modDigiStart[smallEnd] - s, smemRaw, sh, &base);
           base += total;
-        } else if (bigLast) {
-          if (warp == 0) {
-            u32 ec = 0, em = 0;
-            if (mBig > 0) lookback(ev.modState, 0, (int)mBig, lane, &ec, &em);
-            if (lane == 0) sh.base = ec;
-          }
-          __syncthreads();
-          base = sh.base;
+        } else {
+          base = unit_lookback(ev, j, nBigKept, sh);
         }
         if (bigLast) {
-          if (tid == 0) st_state(ev.modState + mBig, pack_state(kStIncl, base + cx.nKept, 0));
           dense_output(ev, mBig, sLastMod, nBig, base, cx);
-          base += cx.nKept;
+          base += nBigKept;
         }
         if (mEnd == g.M && tid == 0) { ev.modClusStart[g.M] = base; ev.counters->nClusters = base; }
-      } else if (tid == 0) {
-        atomicOr(&ev.counters->status, 2u);            // PR_STATUS_CAPACITY: inconsistent module table
+      } else {
+        if (tid == 0) atomicOr(&ev.counters->status, 2u);   // PR_STATUS_CAPACITY: inconsistent module table
+        unit_lookback(ev, j, 0, sh);
       }
+    } else {
+      // empty window (or bad event): transparent to its successors, no look-back of its own
+      if (tid == 0) st_state(ev.winState + j, pack_state(j > 0 ? kStAgg : kStIncl, 0, 0));
     }
     __syncthreads();
     if (tid == 0) {

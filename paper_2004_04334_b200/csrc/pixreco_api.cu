@@ -203,8 +203,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     s.desc.nWin = (s.in.n_words >> kWindowLog2) + 1;
     totalWindows += s.desc.nWin;
   }
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * M * n + (size_t)8 * totalTiles +
-                         (size_t)4 * totalWindows;
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + (size_t)12 * totalWindows;
 
   // ---- buffers from the pools (steady state: cache hits only)
   if (ev->ctlBytes < ctlNeed) {
@@ -237,9 +236,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   char* ctl = (char*)ev->ctl;
   LaunchCtl* lc = (LaunchCtl*)ctl;
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
-  u64* modState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
-  u64* tileState = modState + (size_t)M * n;
-  u32* winInv = (u32*)(tileState + totalTiles);
+  u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
+  u64* winState = tileState + totalTiles;
+  u32* winInv = (u32*)(winState + totalWindows);
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
   for (uint32_t k = 0; k < n; ++k) {
@@ -250,7 +249,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.adc = stage ? stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
-    d.modState = modState + (size_t)M * k; d.tileState = tileState + d.tileBase; d.winInv = winInv + d.winBase;
+    d.tileState = tileState + d.tileBase; d.winState = winState + d.winBase; d.winInv = winInv + d.winBase;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
@@ -467,7 +466,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * g.M + (size_t)8 * tiles + (size_t)4 * ((cap >> kWindowLog2) + 1);
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + (size_t)12 * ((cap >> kWindowLog2) + 1);
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
