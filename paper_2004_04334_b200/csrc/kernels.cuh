@@ -2,9 +2,10 @@
 //
 //   k_unpack   a1+a2 fused: raw word decode, calibration, STABLE digi/error compaction with a
 //              single-pass decoupled look-back scan, modDigiStart, input-order check.
-//   k_cluster  a3+a4 fused: per-module 8-connected components (bitmap + rank lookup + min-index
-//              union-find in shared memory), exact int64 fixed-point cluster sums, cluster
-//              threshold, dense numbering through a cross-module decoupled look-back.
+//   k_cluster  a3+a4 fused: per-module 8-connected components (warp per module: hash look-up +
+//              label equivalence in shared memory; CTA per large module: bitmap + rank look-up +
+//              min-index union-find), exact cluster sums, cluster threshold, per-module numbering.
+//   k_finalize event-wide dense cluster numbering, cluster SoA, modClusStart, counters to the host.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
 //
 // Kernels are batch-capable: a launch processes nEv independent events described by EvDesc
@@ -34,8 +35,6 @@ constexpr int kTileWords = kUnpackThreads * kWordsPerThread;   // 2048
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
-constexpr u32 kWindowLog2 = 9;
-constexpr u32 kWindow = 1u << kWindowLog2;       // a cluster work unit = 512 consecutive digi indices
 constexpr u32 kSmemDigis = 2048;      // modules with more digis use the global workspace tier
 constexpr u32 kSmemClusters = 512;    // likewise for per-cluster accumulators
 
@@ -67,9 +66,10 @@ struct EvDesc {
   // global workspace tier for large modules [cap] each
   u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
   DevCounters* counters; HostCounters* hostCounters;
-  u64 *tileState, *winState;        // look-back states: [nTiles], [nWin]
-  u32* winInv;                      // [nWin]: M - (first module starting in the window), 0 = none
-  u32 winBase, nWin;                // this event's windows in the launch's flattened unit space
+  u64* tileState;                   // k_unpack look-back states [nTiles]
+  u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
+  // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
+  double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
 };
 
 struct Geom {
@@ -321,7 +321,6 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       if (in) {
         if ((int)mod > prev) {
           for (int m = prev + 1; m <= (int)mod; ++m) ev.modDigiStart[m] = gb + j;
-          atomicMax(ev.winInv + ((gb + j) >> kWindowLog2), g.M - (u32)(prev + 1));   // first module starting in this digi window
         }
         if ((int)mod < prev) violation = 1;
         prev = (int)mod;
@@ -357,35 +356,49 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   if (tile == ev.nTiles - 1) {
     const u32 D = g0 + tileCnt, mx1 = max(carryMax1, tileMax1);
     for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) ev.modDigiStart[m] = D;
-    if (tid == 0 && mx1 < g.M) atomicMax(ev.winInv + (D >> kWindowLog2), g.M - mx1);   // trailing empty modules start at D
     if (tid == 0) { ev.counters->nWords = W; ev.counters->nDigis = D; ev.counters->nErrors = W - D; }
   }
 }
 
 // ================================================================== k_cluster (a3 + a4)
-// Work unit = one "window" of kWindow consecutive digi indices of one event: the CTA owns every
-// module whose first digi index falls into the window (k_unpack leaves the first such module in
-// winInv[]).  Because a module with more than kWindow digis reaches past the window's end, only
-// the LAST module of a window can be that large; all others ("smalls") together hold fewer than
-// 2*kWindow = kRangeCap digis.  Units are independent, so no CTA waits on another CTA's progress
-// before it has published all of its own counts:
-//   sparse path  the smalls of the window are clustered at once: shared-memory hash
-//                (module,row,col) -> digi, min-index union-find over the backward neighbours,
-//                per-root member lists walked by the root's thread for the exact int64 sums.
-//                O(1) work per digi, ~9 block barriers per ~19 modules (Run-3-like occupancy).
-//   dense path   a module with more than kWindow digis: occupancy bitmap + popcount ranks,
-//                union-find and per-cluster atomics (shared-memory tiers, global workspace beyond).
-// Dense numbering of kept clusters: decoupled look-back over per-module states.
-constexpr u32 kRangeCap = 2 * kWindow;           // > digis of a window's smalls; local index fits 10 bits
-constexpr u32 kHashSlots = 2048;
+// Every module is an independent problem.  No unit of work waits for another one:
+//   warp path    a module with at most kWarpCap digis is clustered by ONE warp, with only
+//                __syncwarp between its phases: warp-private hash table (row,col) -> digi for the
+//                backward-neighbour look-ups (each found edge is recorded on both ends),
+//                label-equivalence rounds (min over neighbours, hook the old representative with
+//                atomicMin, pointer jumping) until stable, then per-cluster sums accumulated in
+//                shared memory as binary64 (exact: at most 256 terms below 2^43).  Warps take
+//                batches of kModBatch consecutive modules from a global ticket.
+//   dense path   a module with more than kWarpCap digis is clustered by a whole CTA: occupancy
+//                bitmap + popcount ranks, union-find and per-cluster atomics (shared-memory tiers,
+//                global workspace beyond).  Every CTA first scans its residue class of the
+//                launch's modules for such modules, then joins the warp path.
+// Both paths write label[] (final), clus[] = rank of the digi's cluster among the module's kept
+// clusters (or -1), the module's kept-cluster count, and stage the kept clusters' sums at index
+// (first digi of the module + rank).  k_finalize turns the ranks into the event-wide dense
+// numbering (ascending label order, A12) and writes the cluster SoA.
+constexpr u32 kWarpCap = 256;                    // warp path: modules with at most this many digis
+constexpr u32 kWarpTab = 2 * kWarpCap;           // hash slots per warp (load <= 1/4 up to 128 digis, <= 1/2 beyond)
+constexpr u32 kAccRoots = 96;                    // clusters accumulated per pass over a module
+constexpr u32 kModBatch = 8;                     // modules per warp ticket
 constexpr u32 kEmpty = 0xFFFFFFFFu;
-constexpr int kPerThread = kRangeCap / kClusterThreads;   // 4
+constexpr u32 kNoKey = 0xFFFFFFFFu;
+constexpr u32 kNoRank = 0xFFFFu;
 
-__host__ __device__ inline size_t cluster_smem_bytes(u32 bitmapWords) {
+struct WarpRegion {                 // 5 KB of shared memory per warp
+  u32 tab[kWarpTab];                // hash table; afterwards L[256] then the head of the accumulators
+  uint2 nb[kWarpCap];               // 8 neighbour digi indices, one byte each (self = none); afterwards accumulators
+  u32 key[kWarpCap];                // row << 9 | col of kept digis, kNoKey otherwise
+};
+static_assert(sizeof(u32) * (kWarpTab - kWarpCap) + sizeof(uint2) * kWarpCap >= kAccRoots * 28, "accumulators must fit");
+
+__host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords) {
   size_t w = (bitmapWords + 3) & ~3u;
-  size_t dense = (size_t)w * 4 * 2 + (size_t)kSmemDigis * 4 * 2 + (size_t)kSmemClusters * (4 + 4 + 4 + 8 * 3);
-  size_t sparse = (size_t)kHashSlots * 4 * 2 + (size_t)kRangeCap * 4 * 5;
-  return (dense > sparse ? dense : sparse) + 64;
+  return (size_t)w * 4 * 2 + (size_t)kSmemDigis * 4 * 2 + (size_t)kSmemClusters * (4 + 4 + 4 + 8 * 3);
+}
+__host__ __device__ inline size_t cluster_smem_bytes(u32 bitmapWords) {
+  size_t dense = dense_smem_bytes(bitmapWords), warp = sizeof(WarpRegion) * (kClusterThreads / 32);
+  return ((dense > warp ? dense : warp) + 15) & ~(size_t)15;
 }
 
 __device__ __forceinline__ u32 uf_find(const volatile u32* parent, u32 x) {
@@ -406,215 +419,209 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
   }
 }
 
-// Open-addressing hash: tabKey[h] = module << 17 | row << 9 | col (28 bits), tabVal[h] = minimum
-// local digi index on that pixel (duplicates: owner = min index, A6).
-__device__ __forceinline__ u32 hash_slot(u32 key) { return (key * 0x9E3779B1u) >> 21; }
-__device__ __forceinline__ void hash_insert(u32* tabKey, u32* tabVal, u32 key, u32 idx) {
-  u32 h = hash_slot(key);
-  for (;;) {
-    const u32 old = atomicCAS(tabKey + h, kEmpty, key);
-    if (old == kEmpty || old == key) { atomicMin(tabVal + h, idx); return; }
-    h = (h + 1) & (kHashSlots - 1);
-  }
-}
-__device__ __forceinline__ u32 hash_find(const u32* tabKey, const u32* tabVal, u32 key) {
-  u32 h = hash_slot(key);
-  for (;;) {
-    const u32 v = tabKey[h];
-    if (v == kEmpty) return kInvalid;
-    if (v == key) return tabVal[h];
-    h = (h + 1) & (kHashSlots - 1);
-  }
-}
-
 struct ClusterShared {
   u32 scan[8];
-  u32 cnt[2][kPerThread * 8];       // per (k, warp): kept roots / all roots
-  u32 kb[kPerThread * 8];           // per (k, warp): ballot of kept roots
-  u32 offs[kPerThread * 8 + 1];
-  u32 ticket, base, last, first;
-  LbShared lb;
+  u32 nBig, big[kClusterThreads];
 };
 
-// Number of kept roots with local index < b (b in [0, n]); valid after the scan of the sparse path.
-__device__ __forceinline__ u32 kept_prefix(const ClusterShared& sh, u32 b, u32 total) {
-  if (b >= kRangeCap) return total;
-  const u32 k = b / kClusterThreads, r = b % kClusterThreads, w = r >> 5, l = r & 31;
-  return sh.offs[k * 8 + w] + __popc(sh.kb[k * 8 + w] & ((1u << l) - 1u));
+__device__ __forceinline__ u32 wm_slot(u32 key, u32 shift) { return (key * 0x9E3779B1u) >> shift; }
+// First digi on pixel `key` (a module without duplicate pixels), kEmpty if none.
+__device__ __forceinline__ u32 wm_find(const u32* tab, u32 pmask, u32 shift, u32 key) {
+  u32 h = wm_slot(key, shift);
+  for (;;) {
+    const u32 v = tab[h];
+    if (v == kEmpty) return kEmpty;
+    if ((v >> 8) == key) return v & 0xFFu;
+    h = (h + 1) & pmask;
+  }
+}
+// Minimum digi index on pixel `key` (duplicate pixels present: owner = min index, A6).
+__device__ __forceinline__ u32 wm_find_min(const u32* tab, u32 pmask, u32 shift, u32 key) {
+  u32 h = wm_slot(key, shift), best = kEmpty;
+  for (;;) {
+    const u32 v = tab[h];
+    if (v == kEmpty) return best;
+    if ((v >> 8) == key) best = min(best, v & 0xFFu);
+    h = (h + 1) & pmask;
+  }
 }
 
-// Publish this unit's kept-cluster count, look back over the event's earlier windows, publish the
-// inclusive prefix.  Returns the dense number of the unit's first kept cluster (all threads).
-__device__ __forceinline__ u32 unit_lookback(const EvDesc& ev, u32 j, u32 total, ClusterShared& sh) {
-  u32 ec = 0, em = 0;
-  if (j > 0) {
-    if (threadIdx.x == 0) st_state(ev.winState + j, pack_state(kStAgg, total, 0));
-    lookback_cta(ev.winState, (int)j, sh.lb, &ec, &em);
+// ---- warp path: one module = digis [s, s+n), 0 < n <= kWarpCap, processed by the calling warp.
+// Returns (kept digis, clusters, kept clusters) in all lanes.
+__device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr,
+                                            u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
+  const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+  const u32 nPad = (n + 31u) & ~31u;
+  const u32 lg = min(32u - (u32)__clz((int)(max(4u * n, 128u) - 1u)), 9u);   // log2 table size: >= 4n up to 128 digis, 512 beyond
+  const u32 pmask = (1u << lg) - 1u, shift = 32u - lg;
+  u32* tab = wr.tab;
+  unsigned char* nbB = reinterpret_cast<unsigned char*>(wr.nb);
+
+  // A: clear the table
+  for (u32 i = lane * 4u; i <= pmask; i += 128u) *reinterpret_cast<uint4*>(tab + i) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
+  __syncwarp();
+  // B: load, kept flag (A8), insert; every digi starts with no neighbours (all bytes = self)
+  u32 nKept = 0; bool dup = false;
+  for (u32 i = lane; i < nPad; i += 32u) {
+    u32 key = kNoKey;
+    if (i < n && ev.charge[s + i] >= g.pixThr) key = (u32)ev.row[s + i] << 9 | (u32)ev.col[s + i];
+    wr.key[i] = key;
+    wr.nb[i] = make_uint2(i * 0x01010101u, i * 0x01010101u);
+    if (key != kNoKey) {
+      const u32 ent = key << 8 | i;
+      u32 h = wm_slot(key, shift);
+      for (;;) {
+        const u32 old = atomicCAS(tab + h, kEmpty, ent);
+        if (old == kEmpty) break;
+        if ((old >> 8) == key) dup = true;
+        h = (h + 1) & pmask;
+      }
+    }
+    nKept += __popc(__ballot_sync(0xFFFFFFFFu, key != kNoKey));
   }
-  if (threadIdx.x == 0) st_state(ev.winState + j, pack_state(kStIncl, ec + total, 0));
-  return ec;
+  dup = __any_sync(0xFFFFFFFFu, dup);
+  __syncwarp();
+  // C: backward neighbours W, NW, N, NE of every kept digi; an edge found is recorded on both
+  // ends (slot d of i, slot d+4 of the neighbour: one writer per slot).  A duplicate only follows
+  // its pixel's owner (A6).
+  for (u32 i = lane; i < nPad; i += 32u) {
+    const u32 key = wr.key[i];
+    if (key == kNoKey) continue;
+    const u32 row = key >> 9, col = key & 511u;
+    if (dup) {
+      const u32 owner = wm_find_min(tab, pmask, shift, key);
+      if (owner != i) { nbB[i * 8u] = (unsigned char)owner; continue; }
+    }
+    const bool up = row > 0, left = col > 0, right = col + 1 < g.C;
+#define WM_NB(cond, delta, d)                                                                      \
+    if (cond) {                                                                                    \
+      const u32 j = dup ? wm_find_min(tab, pmask, shift, key - (delta)) : wm_find(tab, pmask, shift, key - (delta)); \
+      if (j != kEmpty) { nbB[i * 8u + (d)] = (unsigned char)j; nbB[j * 8u + (d) + 4u] = (unsigned char)i; }          \
+    }
+    WM_NB(left, 1u, 0u)
+    WM_NB(up && left, 513u, 1u)
+    WM_NB(up, 512u, 2u)
+    WM_NB(up && right, 511u, 3u)
+#undef WM_NB
+  }
+  __syncwarp();
+  // D: label equivalence.  L[i] only decreases and always names a digi of i's component; a round
+  // takes the minimum over the neighbours, hooks the old representative under it, then flattens.
+  u32* L = tab;
+  for (u32 i = lane; i < nPad; i += 32u) L[i] = i;
+  __syncwarp();
+  for (;;) {
+    bool changed = false;
+    for (u32 i = lane; i < nPad; i += 32u) {
+      const uint2 nb = wr.nb[i];
+      const u32 li = L[i];
+      u32 m = li;
+      m = min(m, L[nb.x & 0xFFu]); m = min(m, L[(nb.x >> 8) & 0xFFu]); m = min(m, L[(nb.x >> 16) & 0xFFu]); m = min(m, L[nb.x >> 24]);
+      m = min(m, L[nb.y & 0xFFu]); m = min(m, L[(nb.y >> 8) & 0xFFu]); m = min(m, L[(nb.y >> 16) & 0xFFu]); m = min(m, L[nb.y >> 24]);
+      if (m < li) {
+        atomicMin(L + li, m);
+        if (li != i) atomicMin(L + i, m);
+        changed = true;
+      }
+    }
+    if (!__any_sync(0xFFFFFFFFu, changed)) break;
+    __syncwarp();
+    for (u32 i = lane; i < nPad; i += 32u) {
+      u32 l = L[i], p;
+      while ((p = L[l]) != l) l = p;
+      L[i] = l;
+    }
+    __syncwarp();
+  }
+  // E: rank of every root among the module's clusters (ascending index): L[root] |= rank << 8
+  u32 nR = 0;
+  for (u32 i = lane; i < nPad; i += 32u) {
+    const bool isRoot = wr.key[i] != kNoKey && L[i] == i;
+    const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
+    if (isRoot) L[i] = i | (nR + __popc(rb & lt)) << 8 | kNoRank << 16;
+    nR += __popc(rb);
+  }
+  __syncwarp();
+  // F: per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory, kAccRoots
+  // clusters per pass.  Lanes of one 32-digi chunk that share a cluster take turns, so every
+  // read-modify-write has one owner; then the roots apply the cluster threshold (A8), number the
+  // kept clusters and stage their sums.
+  double* acc = reinterpret_cast<double*>(tab + kWarpCap);
+  u32* cnt = reinterpret_cast<u32*>(acc + kAccRoots * 3u);
+  u32 nK = 0;
+  for (u32 p0 = 0; p0 < nR; p0 += kAccRoots) {
+    const u32 nAcc = min(nR - p0, kAccRoots);
+    for (u32 i = lane; i < nAcc * 3u; i += 32u) acc[i] = 0.0;
+    for (u32 i = lane; i < nAcc; i += 32u) cnt[i] = 0u;
+    __syncwarp();
+    for (u32 i = lane; i < nPad; i += 32u) {
+      const u32 key = wr.key[i];
+      u32 rk = 0; bool in = false;
+      u32 r = 256u + lane;
+      if (key != kNoKey) {
+        r = L[i] & 0xFFu;
+        rk = ((L[r] >> 8) & 0xFFu) - p0;
+        in = rk < nAcc;
+        if (!in) r = 256u + lane;
+      }
+      const u32 peers = __match_any_sync(0xFFFFFFFFu, r);
+      const u32 turn = __popc(peers & lt);
+      const u32 turns = __reduce_max_sync(0xFFFFFFFFu, in ? (u32)__popc(peers) : 0u);
+      double qf = 0.0, qx = 0.0, qy = 0.0;
+      if (in) {
+        qf = (double)(ev.charge[s + i] * 16384.0f);
+        qx = qf * (double)(key >> 9); qy = qf * (double)(key & 511u);
+      }
+      for (u32 t = 0; t < turns; ++t) {
+        if (in && turn == t) {
+          double* a = acc + rk * 3u;
+          a[0] += qf; a[1] += qx; a[2] += qy;
+          if (t == 0) cnt[rk] += (u32)__popc(peers);
+        }
+        __syncwarp();
+      }
+    }
+    for (u32 i = lane; i < nPad; i += 32u) {
+      const u32 w = wr.key[i] != kNoKey ? L[i] : 0u;
+      const u32 rk = ((w >> 8) & 0xFFu) - p0;
+      const bool mine = wr.key[i] != kNoKey && (w & 0xFFu) == i && rk < nAcc;
+      double S = 0.0;
+      if (mine) S = acc[rk * 3u];
+      const bool keptC = mine && __double2ll_rz(S) >= g.clusThrFixed;
+      const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
+      if (keptC) {
+        const u32 kr = nK + __popc(kb & lt), o = s + kr;
+        ev.stS[o] = S; ev.stSx[o] = acc[rk * 3u + 1u]; ev.stSy[o] = acc[rk * 3u + 2u];
+        ev.stLabel[o] = s + i; ev.stSize[o] = cnt[rk];
+        L[i] = (w & 0xFFFFu) | kr << 16;
+      }
+      nK += __popc(kb);
+    }
+    __syncwarp();
+  }
+  // G: per-digi outputs: label (final), cluster rank within the module
+  for (u32 i = lane; i < n; i += 32u) {
+    const bool kept = wr.key[i] != kNoKey;
+    u32 lab = kInvalid; int32_t cl = -1;
+    if (kept) {
+      const u32 r = L[i] & 0xFFu, kr = L[r] >> 16;
+      lab = s + r;
+      if (kr != kNoRank) cl = (int32_t)kr;
+    }
+    ev.label[s + i] = lab; ev.clus[s + i] = cl;
+  }
+  *nKeptDigis = nKept; *nRootsOut = nR; *nKeptClusters = nK;
 }
 
-// ---- sparse path: modules [m0, m1) of event ev (m1 > m0), digis [s, s+n), n < kRangeCap, all
-// starting in window j.  `extra` = kept clusters of the window's big module (numbered after these).
-// Returns the number of kept clusters; *baseOut = dense number of its first kept cluster.
-__device__ __forceinline__ u32 cluster_range_sparse(const EvDesc& ev, const Geom& g, u32 j, u32 extra, u32 m0, u32 m1, u32 s, u32 n,
-                                                    unsigned char* smemRaw, ClusterShared& sh, u32* baseOut) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  u32* tabKey = reinterpret_cast<u32*>(smemRaw);
-  u32* tabVal = tabKey + kHashSlots;
-  u32* key = tabVal + kHashSlots;
-  u32* parent = key + kRangeCap;
-  u32* head = parent + kRangeCap;
-  u32* next = head + kRangeCap;
-  float* qs = reinterpret_cast<float*>(next + kRangeCap);
-
-  u32 total = 0, nAll = 0;
-  u32 kb[kPerThread];
-  float cq[kPerThread], cr[kPerThread], cc[kPerThread]; u32 csz[kPerThread]; u32 keptMask = 0;
-  if (n > 0) {
-    // A: init
-    for (u32 i = tid; i < kHashSlots; i += kClusterThreads) { tabKey[i] = kEmpty; tabVal[i] = kInvalid; }
-    __syncthreads();
-    // B: load, kept flag (A8), hash insert
-    u32 myKept = 0;
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      if (i < n) {
-        const float q = ev.charge[s + i];
-        const bool kept = q >= g.pixThr;
-        u32 kk = kInvalid;
-        if (kept) {
-          kk = (u32)ev.module[s + i] << 17 | (u32)ev.row[s + i] << 9 | (u32)ev.col[s + i];
-          hash_insert(tabKey, tabVal, kk, i);
-          ++myKept;
-        }
-        key[i] = kk; qs[i] = q; parent[i] = kept ? i : kInvalid; head[i] = kInvalid;
-      }
-    }
-    myKept = __reduce_add_sync(0xFFFFFFFFu, myKept);
-    if (lane == 0 && myKept) atomicAdd(&ev.counters->nKept, myKept);
-    __syncthreads();
-    // C: unions with backward neighbours: N ? {N} : { NE?, W ? {W} : NW? }; duplicates join their owner
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      if (i >= n) continue;
-      const u32 kk = key[i];
-      if (kk == kInvalid) continue;
-      const u32 owner = hash_find(tabKey, tabVal, kk);
-      if (owner != i) { uf_union(parent, i, owner); continue; }
-      const u32 row = (kk >> 9) & 0xFFu, col = kk & 0x1FFu;
-      u32 j = row ? hash_find(tabKey, tabVal, kk - 512u) : kInvalid;
-      if (j != kInvalid) { uf_union(parent, i, j); continue; }
-      if (row && col + 1 < g.C) { j = hash_find(tabKey, tabVal, kk - 511u); if (j != kInvalid) uf_union(parent, i, j); }
-      j = col ? hash_find(tabKey, tabVal, kk - 1u) : kInvalid;
-      if (j != kInvalid) uf_union(parent, i, j);
-      else if (row && col) { j = hash_find(tabKey, tabVal, kk - 513u); if (j != kInvalid) uf_union(parent, i, j); }
-    }
-    __syncthreads();
-    // D: flatten and push every kept digi on its root's member list
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      if (i >= n || parent[i] == kInvalid) continue;
-      const u32 rt = uf_find(parent, i);
-      if (rt != i) parent[i] = rt;
-      next[i] = atomicExch(head + rt, i);
-    }
-    __syncthreads();
-    // E: each root walks its list: exact fixed-point sums (A9), cluster threshold
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      const bool isRoot = i < n && parent[i] == i;
-      bool keptC = false;
-      csz[k] = 0; cq[k] = cr[k] = cc[k] = 0.f;
-      if (isRoot) {
-        u64 S = 0, Sx = 0, Sy = 0; u32 sz = 0;
-        for (u32 j = head[i]; j != kInvalid; j = next[j]) {
-          const u32 kj = key[j];
-          const u64 qf = (u64)__float2ll_rz(qs[j] * 16384.0f);
-          S += qf; Sx += qf * ((kj >> 9) & 0xFFu); Sy += qf * (kj & 0x1FFu); ++sz;
-        }
-        keptC = (i64)S >= g.clusThrFixed;
-        if (keptC) {
-          const double dS = __ll2double_rn((i64)S);
-          cq[k] = __double2float_rn(dS * (1.0 / 16384.0));
-          cr[k] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sx), dS));
-          cc[k] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)Sy), dS));
-          csz[k] = sz;
-        }
-      }
-      kb[k] = __ballot_sync(0xFFFFFFFFu, keptC);
-      const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
-      keptMask |= (u32)keptC << k;
-      if (lane == 0) { sh.cnt[0][k * 8 + warp] = __popc(kb[k]); sh.cnt[1][k * 8 + warp] = __popc(rb); sh.kb[k * 8 + warp] = kb[k]; }
-    }
-    __syncthreads();
-    if (warp == 0) {
-      const u32 c0 = sh.cnt[0][lane], c1 = sh.cnt[1][lane];
-      const u32 inc = warp_incl_scan(c0, lane);
-      const u32 t1 = __reduce_add_sync(0xFFFFFFFFu, c1);
-      sh.offs[lane] = inc - c0;
-      if (lane == 31) { sh.offs[32] = inc; sh.scan[0] = t1; }
-    }
-    __syncthreads();
-    total = sh.offs[32]; nAll = sh.scan[0];
-    // local number of every kept root goes to head[root] (lists are no longer needed)
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      if (i < n && parent[i] == i)
-        head[i] = (keptMask >> k & 1) ? sh.offs[k * 8 + warp] + __popc(kb[k] & ((1u << lane) - 1u)) : kInvalid;
-    }
-  }
-  // F: numbering base of this window through the cross-window look-back
-  __syncthreads();
-  const u32 base = unit_lookback(ev, j, total + extra, sh);
-  __syncthreads();
-  // G: outputs
-  if (n > 0) {
-#pragma unroll
-    for (int k = 0; k < kPerThread; ++k) {
-      const u32 i = k * kClusterThreads + tid;
-      if (i >= n) continue;
-      const u32 p = parent[i];
-      u32 lab = kInvalid; int32_t cl = -1;
-      if (p != kInvalid) {
-        lab = s + p;
-        const u32 kn = head[p];
-        cl = kn == kInvalid ? -1 : (int32_t)(base + kn);
-      }
-      ev.label[s + i] = lab; ev.clus[s + i] = cl;
-      if (keptMask >> k & 1) {
-        const u32 o = base + head[i];
-        if (o < ev.cap) {
-          ev.clLabel[o] = s + i; ev.clModule[o] = (u16)(key[i] >> 17); ev.clSize[o] = csz[k];
-          ev.clCharge[o] = cq[k]; ev.clRow[o] = cr[k]; ev.clCol[o] = cc[k];
-        }
-      }
-    }
-  }
-  // modClusStart[m] = base + kept clusters rooted before the module's first digi
-  for (u32 m = m0 + tid; m < m1; m += kClusterThreads)
-    ev.modClusStart[m] = base + (n > 0 ? kept_prefix(sh, ev.modDigiStart[m] - s, total) : 0u);
-  if (tid == 0 && nAll) atomicAdd(&ev.counters->nClustersAll, nAll);
-  *baseOut = base;
-  return total;
-}
-
-// ---- dense path: one module m with digis [s, s+nn), in two halves so that the caller can publish
-// the module's count before it waits for anything (count) and write outputs later (output).
-// `deferred`: shared memory will be reused in between, so every array that must survive lives in
-// the global workspace tier.
+// ---- dense path: one module = digis [s, s+nn), nn > kWarpCap, processed by the whole CTA.
+// dense_count clusters and sums (shared-memory tiers, global workspace beyond); dense_stage writes
+// label[], clus[] = rank among the module's kept clusters, and stages the kept clusters' sums.
 struct DenseCtx {
   u32 *perm, *parent, *root, *csize; int32_t* knum; u64 *S, *Sx, *Sy;
   u32 nAll, nKept;
 };
 
-__device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32 s, u32 nn, bool deferred,
+__device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32 s, u32 nn,
                                             unsigned char* smemRaw, ClusterShared& sh, DenseCtx& cx) {
   const int tid = threadIdx.x, lane = tid & 31;
   const u32 bwPad = (g.bitmapWords + 3) & ~3u;
@@ -631,7 +638,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   u32* sScan = sh.scan;
   const u32 stride = g.stride;
 
-  const bool digiInSmem = !deferred && nn <= kSmemDigis;
+  const bool digiInSmem = nn <= kSmemDigis;
   u32* perm = digiInSmem ? smPerm : ev.wsPerm + s;
   u32* parent = digiInSmem ? smParent : ev.wsParent + s;
   cx.perm = perm; cx.parent = parent;
@@ -715,7 +722,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
     u32 c = 0;
     for (u32 i = lo; i < hi; ++i) c += (parent[i] == i);
     u32 run = block_excl_scan(c, sScan, &cx.nAll);
-    if (deferred || cx.nAll > kSmemClusters) {
+    if (cx.nAll > kSmemClusters) {
       cx.root = ev.wsRoot + s; cx.csize = ev.wsSize + s; cx.knum = ev.wsKnum + s;
       cx.S = ev.wsS + s; cx.Sx = ev.wsSx + s; cx.Sy = ev.wsSy + s;
     }
@@ -749,126 +756,171 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
 }
 
-__device__ __forceinline__ void dense_output(const EvDesc& ev, u32 m, u32 s, u32 nn, u32 base, const DenseCtx& cx) {
+__device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 nn, const DenseCtx& cx) {
   const int tid = threadIdx.x;
   for (u32 k = tid; k < cx.nAll; k += kClusterThreads) {
     const int32_t kn = cx.knum[k];
     if (kn < 0) continue;
-    const u32 o = base + (u32)kn;
-    if (o >= ev.cap) continue;                      // cannot happen (N <= D <= cap); stay in bounds
-    const double dS = __ll2double_rn((i64)cx.S[k]);
-    ev.clLabel[o] = s + cx.root[k];
-    ev.clModule[o] = (u16)m;
-    ev.clSize[o] = cx.csize[k];
-    ev.clCharge[o] = __double2float_rn(dS * (1.0 / 16384.0));
-    ev.clRow[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)cx.Sx[k]), dS));
-    ev.clCol[o] = __double2float_rn(__ddiv_rn(__ll2double_rn((i64)cx.Sy[k]), dS));
+    const u32 o = s + (u32)kn;                       // kn <= k < nn: inside the module's own range
+    ev.stS[o] = __ll2double_rn((i64)cx.S[k]); ev.stSx[o] = __ll2double_rn((i64)cx.Sx[k]); ev.stSy[o] = __ll2double_rn((i64)cx.Sy[k]);
+    ev.stLabel[o] = s + cx.root[k]; ev.stSize[o] = cx.csize[k];
   }
   for (u32 i = tid; i < nn; i += kClusterThreads) {
     const u32 p = cx.parent[i];
     u32 lab = kInvalid; int32_t cl = -1;
-    if (p != kInvalid) {
-      lab = s + p;
-      const int32_t kn = cx.knum[cx.perm[p]];
-      cl = kn < 0 ? -1 : (int32_t)(base + (u32)kn);
-    }
+    if (p != kInvalid) { lab = s + p; cl = cx.knum[cx.perm[p]]; }
     ev.label[s + i] = lab;
     ev.clus[s + i] = cl;
   }
   if (tid == 0) {
-    ev.modClusStart[m] = base;
+    ev.modCount[m] = cx.nKept;
     if (cx.nAll) atomicAdd(&ev.counters->nClustersAll, cx.nAll);
   }
 }
 
 template <bool kSingle>
-__device__ __forceinline__ const EvDesc& pick_event_by_window(const EvDesc& single, const EvDesc* batch, u32 nEv, u32 t) {
-  if (kSingle) return single;
-  u32 lo = 0, hi = nEv - 1;                          // last event with winBase <= t
-  while (lo < hi) {
-    u32 mid = (lo + hi + 1) >> 1;
-    if (batch[mid].winBase <= t) lo = mid; else hi = mid - 1;
-  }
-  return batch[lo];
-}
-
-template <bool kSingle>
-__global__ void __launch_bounds__(kClusterThreads)
-k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 totalWindows,
+__global__ void __launch_bounds__(kClusterThreads, 4)
+k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
           LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   extern __shared__ __align__(16) unsigned char smemRaw[];
   __shared__ ClusterShared sh;
-  const int tid = threadIdx.x;
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  const u32 M = g.M, total = nEv * M;
 
+  // ---- phase 1: dense path.  Module (e, m) has index e * M + m; CTA b looks at the indices
+  // congruent to b modulo the grid size (neighbouring hot modules go to different CTAs).
+  for (u32 base = 0; base < total; base += gridDim.x * kClusterThreads) {
+    const u32 gi = base + tid * gridDim.x + blockIdx.x;
+    bool big = false;
+    if (gi < total) {
+      const u32 e = gi / M, m = gi - e * M;
+      const EvDesc& ev = kSingle ? single : batch[e];
+      if (!(ev.counters->status & 1u)) {              // A5 violated: modDigiStart is undefined, no per-digi work
+        const u32 s = ev.modDigiStart[m], t = ev.modDigiStart[m + 1];
+        big = t >= s && t <= ev.cap && t - s > kWarpCap;
+      }
+    }
+    if (tid == 0) sh.nBig = 0;
+    __syncthreads();
+    if (big) sh.big[atomicAdd(&sh.nBig, 1u)] = gi;
+    __syncthreads();
+    const u32 nBig = sh.nBig;
+    for (u32 k = 0; k < nBig; ++k) {
+      const u32 gk = sh.big[k], e = gk / M, m = gk - e * M;
+      const EvDesc& ev = kSingle ? single : batch[e];
+      const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
+      DenseCtx cx;
+      dense_count(ev, g, s, nn, smemRaw, sh, cx);
+      dense_stage(ev, m, s, nn, cx);
+      __syncthreads();
+    }
+    __syncthreads();
+  }
+
+  // ---- phase 2: warp path.  A ticket is a batch of kModBatch consecutive modules of one event.
+  WarpRegion& wr = reinterpret_cast<WarpRegion*>(smemRaw)[warp];
+  const u32 bpe = (M + kModBatch - 1) / kModBatch, nTickets = nEv * bpe;
   for (;;) {
-    __syncthreads();
-    if (tid == 0) sh.ticket = atomicAdd(&lc->modTicket, 1u);
-    __syncthreads();
-    const u32 ticket = sh.ticket;
-    if (ticket >= totalWindows) break;
-    const EvDesc& ev = pick_event_by_window<kSingle>(single, batch, nEv, ticket);
-    const u32 j = ticket - ev.winBase;
-    const u32 wi = ev.winInv[j];
-    // An event that violated the input contract (A5) has undefined modDigiStart: no per-digi work.
-    const bool bad = (ev.counters->status & 1u) != 0;
-    if (wi != 0 && !bad) {
-      const u32 first = g.M - wi, hi = (j + 1) << kWindowLog2;
-      // modules whose first digi lies in this window: [first, mEnd)
-      u32 mEnd = first;
-      for (;;) {
-        const u32 m = mEnd + tid;
-        const int c = __syncthreads_count(m < g.M && ev.modDigiStart[m] < hi);
-        mEnd += (u32)c;
-        if (c < kClusterThreads) break;
-      }
-      const u32 s = ev.modDigiStart[first];
-      const u32 sLastMod = ev.modDigiStart[mEnd - 1], sEnd = ev.modDigiStart[mEnd];
-      const bool bigLast = sEnd - sLastMod > kWindow;
-      const u32 smallEnd = bigLast ? mEnd - 1 : mEnd;
-      const bool haveSmall = smallEnd > first;
-      const bool sane = s <= sLastMod && sLastMod <= sEnd && sEnd <= ev.cap && (!haveSmall || ev.modDigiStart[smallEnd] - s < kRangeCap);
-      if (sane) {
-        DenseCtx cx;
-        const u32 mBig = mEnd - 1, nBig = sEnd - sLastMod;
-        if (bigLast) dense_count(ev, g, sLastMod, nBig, haveSmall, smemRaw, sh, cx);   // count first: nobody waits on us
-        const u32 nBigKept = bigLast ? cx.nKept : 0u;
-        u32 base = 0;
-        if (haveSmall) {
-          const u32 total = cluster_range_sparse(ev, g, j, nBigKept, first, smallEnd, s, ev.modDigiStart[smallEnd] - s, smemRaw, sh, &base);
-          base += total;
-        } else {
-          base = unit_lookback(ev, j, nBigKept, sh);
-        }
-        if (bigLast) {
-          dense_output(ev, mBig, sLastMod, nBig, base, cx);
-          base += nBigKept;
-        }
-        if (mEnd == g.M && tid == 0) { ev.modClusStart[g.M] = base; ev.counters->nClusters = base; }
+    u32 t = 0;
+    if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
+    t = __shfl_sync(0xFFFFFFFFu, t, 0);
+    if (t >= nTickets) break;
+    const u32 e = t / bpe, m0 = (t - e * bpe) * kModBatch, nm = min(kModBatch, M - m0);
+    const EvDesc& ev = kSingle ? single : batch[e];
+    if (ev.counters->status & 1u) continue;
+    const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
+    u32 accK = 0, accA = 0;
+    for (u32 k = 0; k < nm; ++k) {
+      const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
+      u32 cnt = 0;
+      if (t1 < s || t1 > ev.cap) {
+        if (lane == 0) atomicOr(&ev.counters->status, 2u);   // PR_STATUS_CAPACITY: inconsistent module table
       } else {
-        if (tid == 0) atomicOr(&ev.counters->status, 2u);   // PR_STATUS_CAPACITY: inconsistent module table
-        unit_lookback(ev, j, 0, sh);
+        const u32 n = t1 - s;
+        if (n > kWarpCap) continue;                          // dense path wrote this module
+        if (n > 0) {
+          u32 nk, nr;
+          warp_module(ev, g, s, n, wr, &nk, &nr, &cnt);
+          accK += nk; accA += nr;
+        }
       }
-    } else {
-      // empty window (or bad event): transparent to its successors, no look-back of its own
-      if (tid == 0) st_state(ev.winState + j, pack_state(j > 0 ? kStAgg : kStIncl, 0, 0));
+      if (lane == 0) ev.modCount[m0 + k] = cnt;
+    }
+    if (lane == 0) {
+      if (accK) atomicAdd(&ev.counters->nKept, accK);
+      if (accA) atomicAdd(&ev.counters->nClustersAll, accA);
+    }
+  }
+}
+
+// ================================================================== k_finalize (numbering of a4)
+// One CTA per (event, group of kFinMods consecutive modules): the group's first dense cluster
+// number is the sum of the kept-cluster counts of all earlier modules (at most 2048 values), so
+// no CTA depends on another.  Turns clus[] ranks into event-wide cluster numbers, converts the
+// staged sums into the cluster SoA (A9: binary64 division, one rounding to binary32), writes
+// modClusStart[]; the launch's last CTA publishes all counters to mapped pinned host memory.
+constexpr u32 kFinMods = 32;
+template <bool kSingle>
+__global__ void __launch_bounds__(256)
+k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent,
+           LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+  __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8], sLast;
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
+  const u32 e = blockIdx.x / unitsPerEvent, u = blockIdx.x - e * unitsPerEvent;
+  const EvDesc& ev = kSingle ? single : batch[e];
+  const u32 m0 = u * kFinMods, m1 = min(m0 + kFinMods, M);
+  if (!(ev.counters->status & 1u)) {
+    u32 sum = 0, base;
+    for (u32 m = tid; m < m0; m += 256) sum += ev.modCount[m];
+    block_excl_scan(sum, sScan, &base);
+    if (warp == 0) {
+      const u32 c = m0 + lane < m1 ? ev.modCount[m0 + lane] : 0u;
+      const u32 incl = warp_incl_scan(c, lane);
+      sStart[lane] = base + incl - c;
+      if (lane == 31) sStart[32] = base + incl;
+      sDigi[lane] = ev.modDigiStart[min(m0 + lane, M)];
+      if (lane == 31) sDigi[32] = ev.modDigiStart[min(m0 + 32u, M)];
     }
     __syncthreads();
-    if (tid == 0) {
-      __threadfence();
-      sh.last = (atomicAdd(&lc->modDone, 1u) == totalWindows - 1);
-    }
-    __syncthreads();
-    if (sh.last) {
-      // the launch's last unit: publish every event's counters to mapped pinned host memory
-      __threadfence();
-      for (u32 k = tid; k < nEv; k += kClusterThreads) {
-        const EvDesc& d = kSingle ? single : batch[k];
-        const volatile DevCounters* c = d.counters;
-        HostCounters h;
-        h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
-        h.nClustersAll = c->nClustersAll; h.nClusters = c->nClusters; h.status = c->status; h.seq = 1;
-        *d.hostCounters = h;
+    for (u32 m = m0 + tid; m < m1; m += 256) ev.modClusStart[m] = sStart[m - m0];
+    if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
+    const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
+    if (d0 <= d1 && d1 <= ev.cap) {
+      for (u32 d = d0 + tid; d < d1; d += 256) {
+        const int32_t c = ev.clus[d];
+        if (c >= 0) ev.clus[d] = (int32_t)(sStart[min((u32)ev.module[d] - m0, kFinMods - 1)] + (u32)c);
       }
+      for (u32 o = sStart[0] + tid; o < sStart[32]; o += 256) {
+        u32 li = 0;
+#pragma unroll
+        for (u32 step = 16; step > 0; step >>= 1)
+          if (li + step < kFinMods + 1 && sStart[li + step] <= o) li += step;   // last module with start <= o and a cluster there
+        const u32 src = sDigi[li] + (o - sStart[li]);
+        if (o < ev.cap && src < ev.cap) {
+          const double S = ev.stS[src];
+          ev.clLabel[o] = ev.stLabel[src]; ev.clModule[o] = (u16)(m0 + li); ev.clSize[o] = ev.stSize[src];
+          ev.clCharge[o] = __double2float_rn(S * (1.0 / 16384.0));
+          ev.clRow[o] = __double2float_rn(__ddiv_rn(ev.stSx[src], S));
+          ev.clCol[o] = __double2float_rn(__ddiv_rn(ev.stSy[src], S));
+        }
+      }
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    sLast = (atomicAdd(&lc->modDone, 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (sLast) {
+    __threadfence();
+    for (u32 k = tid; k < nEv; k += 256) {
+      const EvDesc& d = kSingle ? single : batch[k];
+      const volatile DevCounters* c = d.counters;
+      HostCounters h;
+      h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
+      h.nClustersAll = c->nClustersAll; h.nClusters = c->nClusters; h.status = c->status; h.seq = 1;
+      *d.hostCounters = h;
     }
   }
 }

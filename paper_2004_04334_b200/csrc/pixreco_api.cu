@@ -42,7 +42,7 @@ struct pr_handle {
   std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
   std::atomic<int> sticky{0};
   bool timing = false;
-  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msExport = 0;   // guarded by mu
+  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msFinalize = 0, msExport = 0;   // guarded by mu
   std::string lastCuda;
 };
 
@@ -68,7 +68,7 @@ struct pr_event {
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
   int status = PR_OK;        // filled when completion is observed
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
-  cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING
+  cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, finalize, export
   bool exported = false;
 };
 
@@ -112,6 +112,9 @@ void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, ui
   d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
   d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
   d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap);
+  d.modCount = c.take<u32>(M + 4);
+  d.stS = c.take<double>(cap); d.stSx = c.take<double>(cap); d.stSy = c.take<double>(cap);
+  d.stLabel = c.take<u32>(cap); d.stSize = c.take<u32>(cap);
 }
 
 void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M) {
@@ -187,7 +190,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // ---- layout
   ev->sub.assign(n, SubEvent());
   size_t devBytes = 0, hostBytes = 0;
-  uint32_t totalTiles = 0, totalWindows = 0;
+  uint32_t totalTiles = 0;
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     s.in = ins[k];
@@ -199,11 +202,8 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     s.desc.tileBase = totalTiles;
     s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
     totalTiles += s.desc.nTiles;
-    s.desc.winBase = totalWindows;
-    s.desc.nWin = (s.in.n_words >> kWindowLog2) + 1;
-    totalWindows += s.desc.nWin;
   }
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + (size_t)12 * totalWindows;
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles;
 
   // ---- buffers from the pools (steady state: cache hits only)
   if (ev->ctlBytes < ctlNeed) {
@@ -237,8 +237,6 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   LaunchCtl* lc = (LaunchCtl*)ctl;
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
   u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
-  u64* winState = tileState + totalTiles;
-  u32* winInv = (u32*)(winState + totalWindows);
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
   for (uint32_t k = 0; k < n; ++k) {
@@ -249,7 +247,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.adc = stage ? stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
-    d.tileState = tileState + d.tileBase; d.winState = winState + d.winBase; d.winInv = winInv + d.winBase;
+    d.tileState = tileState + d.tileBase;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
@@ -266,14 +264,24 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       PR_CUDA(h, cudaMemcpyAsync(stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
       nMemcpy += 2;
     }
+  // k_cluster: persistent CTAs (dense scan + warp tickets).  A small launch gets one CTA per warp
+  // ticket or per possible dense module (a dense module has more than kWarpCap digis).
+  const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
+  uint64_t totalWords = 0;
+  for (uint32_t k = 0; k < n; ++k) totalWords += ins[k].n_words;
+  const uint64_t warpTickets = (uint64_t)n * ((M + kModBatch - 1) / kModBatch), maxDense = totalWords / (kWarpCap + 1);
+  const uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
-  if (clusterGrid > totalWindows) clusterGrid = totalWindows;
+  if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
+  if (clusterGrid < 1) clusterGrid = 1;
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
     k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, 1, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, totalWindows, lc, h->geom);
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
   } else {
     EvDesc* st = (EvDesc*)ev->descStage;
     for (uint32_t k = 0; k < n; ++k) st[k] = ev->sub[k].desc;
@@ -282,11 +290,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, totalWindows, lc, h->geom);
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
   }
-  nLaunch += 2;
+  nLaunch += 3;
   PR_CUDA(h, cudaGetLastError());
-  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
   ev->exported = want != 0;
   if (want) {
     // exact-size mirrors: the item table lives at the head of the pinned slab's tail (mapped memory)
@@ -318,7 +328,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ++nLaunch;
     PR_CUDA(h, cudaGetLastError());
   }
-  if (h->timing && want) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
+  if (h->timing && want) PR_CUDA(h, cudaEventRecord(ev->tev[4], stream));
   PR_CUDA(h, cudaEventRecord(ev->done, stream));
   ev->n = n;
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
@@ -352,11 +362,12 @@ int poll(pr_event* ev) {
   ev->status = worst;
   ev->state = kDone;
   if (ev->h->timing) {
-    float a = 0, b = 0, c = 0;
-    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess) {
-      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[2], ev->tev[3]) != cudaSuccess) c = 0;
+    float a = 0, b = 0, c = 0, f = 0;
+    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess &&
+        cudaEventElapsedTime(&f, ev->tev[2], ev->tev[3]) == cudaSuccess) {
+      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[3], ev->tev[4]) != cudaSuccess) c = 0;
       std::lock_guard<std::mutex> g(ev->h->mu);
-      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msExport += c;
+      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msFinalize += f; ev->h->msExport += c;
     } else cudaGetLastError();
   }
   ev->h->inFlight.fetch_sub(1);
@@ -466,7 +477,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + (size_t)12 * ((cap >> kWindowLog2) + 1);
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles;
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
@@ -492,7 +503,7 @@ int pr_destroy(pr_handle* h) {
     if (ev->ctl) h->devPool->free(ev->ctl, nullptr, true);
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
     if (ev->done) cudaEventDestroy(ev->done);
-    for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+    for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
@@ -513,7 +524,7 @@ int pr_event_create(pr_handle* h, pr_event** out) {
   cudaError_t e = cudaEventCreateWithFlags(&ev->done, cudaEventDisableTiming);
   if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
   if (h->timing)
-    for (int i = 0; i < 4; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
+    for (int i = 0; i < 5; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
   { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
   *out = ev;
   return PR_OK;
@@ -527,7 +538,7 @@ int pr_event_destroy(pr_event* ev) {
   if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
   if (ev->done) cudaEventDestroy(ev->done);
-  for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+  for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
   {
     std::lock_guard<std::mutex> g(h->mu);
     for (size_t i = 0; i < h->slots.size(); ++i)
@@ -596,7 +607,7 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
   h->devPool->stats(&out->device_pool); h->hostPool->stats(&out->host_pool);
   {
     std::lock_guard<std::mutex> g(h->mu);
-    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->export_ms = h->msExport;
+    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->finalize_ms = h->msFinalize; out->export_ms = h->msExport;
   }
   return PR_OK;
 }

@@ -275,3 +275,36 @@ def test_batch_matches_single_events(pr):
             compare(out, ref, lambda f: got[f])
             assert np.array_equal(out.host("cl_label"), ref.cl_label)
         slot.release()
+
+
+def _blob_module(rng, m, n, dup_frac=0.0, box=40):
+    """n digis of module m packed into a small box (many merges, long chains), random order,
+    ADC spanning both thresholds; optionally some duplicate pixels (A6)."""
+    r0, c0 = int(rng.integers(0, 160 - box)), int(rng.integers(0, 416 - box))
+    cells = rng.permutation(box * box)[: max(n - int(n * dup_frac), 1)]
+    pix = [(m, r0 + int(x) // box, c0 + int(x) % box) for x in cells]
+    while len(pix) < n:
+        pix.append(pix[int(rng.integers(0, len(pix)))])
+    order = rng.permutation(len(pix))
+    return [(*pix[k], int(rng.integers(5, 256))) for k in order]
+
+
+@pytest.mark.parametrize("sizes,dup", [
+    ([1, 2, 31, 32, 33, 63, 64, 65, 127, 128, 129, 255, 256, 257, 0, 0, 300, 300, 511, 512, 513, 5, 1024, 3], 0.0),
+    ([256] * 9 + [257] * 3 + [40] * 30, 0.0),
+    ([17, 100, 256, 250, 257, 600, 20, 20], 0.15),
+    ([3] * 700, 0.0),                                    # hundreds of modules per 512-digi window
+])
+def test_module_size_boundaries(pr, sizes, dup):
+    """Modules on both sides of every path boundary of k_cluster (warp path up to 256 digis, dense
+    path beyond, two dense modules in one window, windows with hundreds of tiny modules)."""
+    rng = np.random.default_rng(len(sizes) * 1000 + int(dup * 100))
+    M = len(sizes) + 3
+    pix = []
+    for m, n in enumerate(sizes):
+        if n:
+            pix += _blob_module(rng, m + 1, n, dup, box=12 if n <= 64 else 40)
+    ev = hand(pix, M)
+    cal = wl.Calib(rng.uniform(60, 100, M).astype(np.float32), rng.normal(0, 200, M).astype(np.float32), 1000.0, 4000.0)
+    out, got = run_device(pr, ev, cal)
+    compare(out, oracle_of(ev, cal), lambda f: got[f])
