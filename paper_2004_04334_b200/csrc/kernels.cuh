@@ -446,6 +446,99 @@ __device__ __forceinline__ u32 wm_find_min(const u32* tab, u32 pmask, u32 shift,
   }
 }
 
+// ---- warp path, one digi per lane: module = digis [s, s+n), 0 < n <= 32.  Everything lives in
+// registers: adjacency and reachability are 32-bit lane masks (Warshall closure with shuffles),
+// the cluster's minimum lane is its root, sums run along each cluster's lane list.
+__device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr,
+                                                  u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
+  const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+  constexpr u32 pmask = 127u, shift = 25u;          // 128 slots: load <= 1/4
+  u32* tab = wr.tab;
+  u32* fw = wr.tab + 128;                           // forward edges: lane mask per digi
+  *reinterpret_cast<uint4*>(tab + lane * 4u) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
+  fw[lane] = 0u;
+  __syncwarp();
+  float q = 0.f; u32 key = kNoKey;
+  if (lane < n) {
+    q = ev.charge[s + lane];
+    if (q >= g.pixThr) key = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
+  }
+  const bool kept = key != kNoKey;
+  bool dup = false;
+  if (kept) {
+    const u32 ent = key << 8 | lane;
+    u32 h = wm_slot(key, shift);
+    for (;;) {
+      const u32 old = atomicCAS(tab + h, kEmpty, ent);
+      if (old == kEmpty) break;
+      if ((old >> 8) == key) dup = true;
+      h = (h + 1) & pmask;
+    }
+  }
+  const u32 keptMask = __ballot_sync(0xFFFFFFFFu, kept);
+  dup = __any_sync(0xFFFFFFFFu, dup);
+  __syncwarp();
+  // backward neighbours W, NW, N, NE; each edge is recorded on both ends
+  u32 adj = 1u << lane;
+  if (kept) {
+    const u32 row = key >> 9, col = key & 511u;
+    u32 owner = lane;
+    if (dup) owner = wm_find_min(tab, pmask, shift, key);
+    if (owner != lane) {                              // a duplicate only joins its pixel's owner (A6)
+      adj |= 1u << owner; atomicOr(fw + owner, 1u << lane);
+    } else {
+      const bool up = row > 0, left = col > 0, right = col + 1 < g.C;
+#define WM_NB(cond, delta)                                                                          \
+      if (cond) {                                                                                   \
+        const u32 j = dup ? wm_find_min(tab, pmask, shift, key - (delta)) : wm_find(tab, pmask, shift, key - (delta)); \
+        if (j != kEmpty) { adj |= 1u << j; atomicOr(fw + j, 1u << lane); }                          \
+      }
+      WM_NB(left, 1u)
+      WM_NB(up && left, 513u)
+      WM_NB(up, 512u)
+      WM_NB(up && right, 511u)
+#undef WM_NB
+    }
+  }
+  __syncwarp();
+  u32 reach = adj | fw[lane];
+  // transitive closure (Warshall): after step j every lane that reaches j also reaches all of j's set
+  for (u32 j = 0; j < n; ++j) {
+    const u32 rj = __shfl_sync(0xFFFFFFFFu, reach, j);
+    if (reach & (1u << j)) reach |= rj;
+  }
+  const u32 root = (u32)__ffs((int)reach) - 1u;
+  const bool isRoot = kept && root == lane;
+  const u32 nR = (u32)__popc(__ballot_sync(0xFFFFFFFFu, isRoot));
+  // sums of qf = q * 2^14 (A9) in binary64 (exact: at most 32 terms below 2^43), suffix sums along the lane list
+  double qf = 0.0, qx = 0.0, qy = 0.0;
+  if (kept) { qf = (double)(q * 16384.0f); qx = qf * (double)(key >> 9); qy = qf * (double)(key & 511u); }
+  const u32 most = __reduce_max_sync(0xFFFFFFFFu, (u32)__popc(reach));
+  const u32 above = reach & (0xFFFFFFFEu << lane);
+  u32 nxt = above ? (u32)__ffs((int)above) - 1u : 32u;
+  for (u32 span = 1; span < most; span <<= 1) {
+    const u32 src = nxt & 31u;
+    const double a = __shfl_sync(0xFFFFFFFFu, qf, src), b = __shfl_sync(0xFFFFFFFFu, qx, src), c = __shfl_sync(0xFFFFFFFFu, qy, src);
+    const u32 nn = __shfl_sync(0xFFFFFFFFu, nxt, src);
+    if (nxt < 32u) { qf += a; qx += b; qy += c; nxt = nn; }
+  }
+  const bool keptC = isRoot && __double2ll_rz(qf) >= g.clusThrFixed;
+  const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
+  const u32 kr = (u32)__popc(kb & lt);
+  if (keptC) {
+    const u32 o = s + kr;
+    ev.stS[o] = qf; ev.stSx[o] = qx; ev.stSy[o] = qy;
+    ev.stLabel[o] = s + lane; ev.stSize[o] = (u32)__popc(reach);
+  }
+  const u32 krRoot = __shfl_sync(0xFFFFFFFFu, keptC ? kr : kNoRank, root);
+  if (lane < n) {
+    ev.label[s + lane] = kept ? s + root : kInvalid;
+    ev.clus[s + lane] = (kept && krRoot != kNoRank) ? (int32_t)krRoot : -1;
+  }
+  __syncwarp();
+  *nKeptDigis = (u32)__popc(keptMask); *nRootsOut = nR; *nKeptClusters = (u32)__popc(kb);
+}
+
 // ---- warp path: one module = digis [s, s+n), 0 < n <= kWarpCap, processed by the calling warp.
 // Returns (kept digis, clusters, kept clusters) in all lanes.
 __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr,
@@ -543,9 +636,9 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   }
   __syncwarp();
   // F: per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory, kAccRoots
-  // clusters per pass.  Lanes of one 32-digi chunk that share a cluster take turns, so every
-  // read-modify-write has one owner; then the roots apply the cluster threshold (A8), number the
-  // kept clusters and stage their sums.
+  // clusters per pass.  The lanes of one 32-digi chunk that share a cluster are reduced with
+  // shuffles, their first lane owns the read-modify-write; then the roots apply the cluster
+  // threshold (A8), number the kept clusters and stage their sums.
   double* acc = reinterpret_cast<double*>(tab + kWarpCap);
   u32* cnt = reinterpret_cast<u32*>(acc + kAccRoots * 3u);
   u32 nK = 0;
@@ -565,21 +658,27 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
         if (!in) r = 256u + lane;
       }
       const u32 peers = __match_any_sync(0xFFFFFFFFu, r);
-      const u32 turn = __popc(peers & lt);
-      const u32 turns = __reduce_max_sync(0xFFFFFFFFu, in ? (u32)__popc(peers) : 0u);
+      const u32 most = __reduce_max_sync(0xFFFFFFFFu, in ? (u32)__popc(peers) : 0u);
       double qf = 0.0, qx = 0.0, qy = 0.0;
       if (in) {
         qf = (double)(ev.charge[s + i] * 16384.0f);
         qx = qf * (double)(key >> 9); qy = qf * (double)(key & 511u);
       }
-      for (u32 t = 0; t < turns; ++t) {
-        if (in && turn == t) {
-          double* a = acc + rk * 3u;
-          a[0] += qf; a[1] += qx; a[2] += qy;
-          if (t == 0) cnt[rk] += (u32)__popc(peers);
-        }
-        __syncwarp();
+      // suffix sums along each cluster's lane list by pointer jumping: the first lane ends with the total
+      const u32 above = peers & (0xFFFFFFFEu << lane);
+      u32 nxt = above ? (u32)__ffs((int)above) - 1u : 32u;
+      for (u32 span = 1; span < most; span <<= 1) {
+        const u32 src = nxt & 31u;
+        const double a = __shfl_sync(0xFFFFFFFFu, qf, src), b = __shfl_sync(0xFFFFFFFFu, qx, src), c = __shfl_sync(0xFFFFFFFFu, qy, src);
+        const u32 nn = __shfl_sync(0xFFFFFFFFu, nxt, src);
+        if (nxt < 32u) { qf += a; qx += b; qy += c; nxt = nn; }
       }
+      if (in && (peers & lt) == 0u) {                 // one owner per cluster and chunk
+        double* a = acc + rk * 3u;
+        a[0] += qf; a[1] += qx; a[2] += qy;
+        cnt[rk] += (u32)__popc(peers);
+      }
+      __syncwarp();
     }
     for (u32 i = lane; i < nPad; i += 32u) {
       const u32 w = wr.key[i] != kNoKey ? L[i] : 0u;
@@ -840,7 +939,8 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         if (n > kWarpCap) continue;                          // dense path wrote this module
         if (n > 0) {
           u32 nk, nr;
-          warp_module(ev, g, s, n, wr, &nk, &nr, &cnt);
+          if (n <= 32u) warp_module_small(ev, g, s, n, wr, &nk, &nr, &cnt);
+          else warp_module(ev, g, s, n, wr, &nk, &nr, &cnt);
           accK += nk; accA += nr;
         }
       }
