@@ -30,8 +30,8 @@ constexpr u32 kInvalid = 0xFFFFFFFFu;
 
 // ---- unpack kernel geometry ----
 constexpr int kUnpackThreads = 256;
-constexpr int kWordsPerThread = 8;
-constexpr int kTileWords = kUnpackThreads * kWordsPerThread;   // 2048
+constexpr int kRowsPerWarp = 8;                                      // rows of 32 consecutive words per warp
+constexpr int kTileWords = kUnpackThreads * kRowsPerWarp;            // 2048
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
@@ -44,7 +44,7 @@ struct DevCounters {
 };
 // Per-launch control words (zeroed per acquire).
 struct LaunchCtl {
-  u32 tileTicket, modTicket, modDone, pad[13];
+  u32 modTicket, modDone, pad[14];
 };
 // What the host reads after completion (mapped pinned memory, written by the last block).
 struct HostCounters {
@@ -78,7 +78,7 @@ struct Geom {
   u32 bitmapWords;                  // (R+2)*stride + 1
   float pixThr;
   i64 clusThrFixed;                 // llrint(clusThr * 2^14)
-  const float *gain, *ped;          // device [M]
+  const float2* calib;              // device [M]: (gain, pedestal)
 };
 
 // ------------------------------------------------------------------ small helpers
@@ -125,30 +125,6 @@ __device__ __forceinline__ u32 block_excl_scan(u32 v, u32* sw, u32* total) {
   return base + incl - v;
 }
 
-// Decoupled look-back over states [first, self): returns the combined (count, max1) of all
-// predecessors.  Called by one full warp.
-__device__ __forceinline__ void lookback(const u64* state, int first, int self, int lane, u32* cnt, u32* mx1) {
-  u32 c = 0, m = 0;
-  int look = self - 1;
-  while (look >= first) {
-    int idx = look - lane;
-    u64 v;
-    bool real = idx >= first;
-    do {
-      v = real ? ld_state(state + idx) : kStIncl;    // virtual zero inclusive before the event start
-    } while (__any_sync(0xFFFFFFFFu, st_status(v) == 0));
-    u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v) == 2);
-    int upto = inclMask ? (__ffs(inclMask) - 1) : 31;
-    u32 cc = lane <= upto ? st_count(v) : 0, mm = lane <= upto ? st_max1(v) : 0;
-    c += __reduce_add_sync(0xFFFFFFFFu, cc);
-    m = max(m, __reduce_max_sync(0xFFFFFFFFu, mm));
-    if (inclMask) break;
-    look -= 32;
-  }
-  *cnt = c; *mx1 = m;
-}
-
-
 // CTA-wide decoupled look-back (blockDim = 256): thread j reads the state of unit (self-1-j), so
 // one round covers 256 predecessors.  With hundreds of units in flight, a 32-wide window needed
 // one serial L2 round trip per 32 predecessors and dominated the kernels.  Every thread returns
@@ -185,84 +161,72 @@ __device__ __forceinline__ void lookback_cta(const u64* state, int self, LbShare
   *cnt = c; *mx1 = m;
 }
 
-template <bool kSingle>
-__device__ __forceinline__ const EvDesc& pick_event_by_tile(const EvDesc& single, const EvDesc* batch, u32 nEv, u32 t, u32* e) {
-  if (kSingle) { *e = 0; return single; }
-  u32 lo = 0, hi = nEv - 1;                          // last event with tileBase <= t
-  while (lo < hi) {
-    u32 mid = (lo + hi + 1) >> 1;
-    if (batch[mid].tileBase <= t) lo = mid; else hi = mid - 1;
-  }
-  *e = lo;
-  return batch[lo];
-}
-
 // ================================================================== k_unpack (a1 + a2)
-// One CTA per tile of 2048 words, 8 consecutive words per thread (2 x LDG.128 words + 1 x LDG.128
-// adc).  Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
+// One CTA per tile of kTileWords words; warp w owns kRowsPerWarp rows of 32 consecutive words, lane l
+// of row j holds word (32 j + l): every load and every store instruction of a warp touches one
+// contiguous run.  Compaction is a warp ballot + popcount (no shared-memory staging): the digi's
+// place is  g0 (digis of earlier tiles, decoupled look-back) + digis of earlier warps + digis of
+// earlier rows + popc(ballot & lanes below).  Tiles are taken in blockIdx order (the look-back
+// relies on CTAs being scheduled in that order, like every single-pass scan does); in a batch the
+// tile -> event map is a table written by the host next to the descriptors.
+// Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
 template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads, 4)
-k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
-         LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
-  __shared__ __align__(16) u32 sWord[kTileWords + 8];
-  __shared__ __align__(16) u16 sAdc[kTileWords + 8];
-  __shared__ __align__(16) u16 sOff[kTileWords + 8];
+__global__ void __launch_bounds__(kUnpackThreads, 5)
+k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
+         const __grid_constant__ Geom g) {
   __shared__ u32 sWsum[8], sWmax[8];
   __shared__ LbShared sLb;
-  __shared__ u32 sTicket;
+  __shared__ __align__(16) EvDesc sEv;             // batch: the tile's descriptor (pointers stay out of registers)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) sTicket = atomicAdd(&lc->tileTicket, 1u);
-  __syncthreads();
-  const u32 t = sTicket;
-  u32 e;
-  const EvDesc& ev = pick_event_by_tile<kSingle>(single, batch, nEv, t, &e);
-  const u32 tile = t - ev.tileBase, W = ev.nWords;
-  const u32 i0 = tile * kTileWords + tid * kWordsPerThread;
+  const u32 lt = (1u << lane) - 1u;
+  if (!kSingle) {
+    const u32* src = reinterpret_cast<const u32*>(batch + tileEvent[blockIdx.x]);
+    if (tid < (int)(sizeof(EvDesc) / 4)) reinterpret_cast<u32*>(&sEv)[tid] = __ldg(src + tid);
+    __syncthreads();
+  }
+  const EvDesc& ev = kSingle ? single : sEv;
+  const u32 tile = blockIdx.x - ev.tileBase, W = ev.nWords;
+  const u32 i0 = tile * kTileWords + warp * (32u * kRowsPerWarp) + lane;   // this lane's word of row 0
 
-  // ---- load 8 words + 8 adc
-  u32 w[8]; u16 a[8];
-  if (i0 + 8 <= W) {
-    const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(ev.words + i0));
-    const uint4 w1 = __ldg(reinterpret_cast<const uint4*>(ev.words + i0) + 1);
-    const uint4 aa = __ldg(reinterpret_cast<const uint4*>(ev.adc + i0));
-    w[0] = w0.x; w[1] = w0.y; w[2] = w0.z; w[3] = w0.w; w[4] = w1.x; w[5] = w1.y; w[6] = w1.z; w[7] = w1.w;
-    a[0] = (u16)aa.x; a[1] = (u16)(aa.x >> 16); a[2] = (u16)aa.y; a[3] = (u16)(aa.y >> 16);
-    a[4] = (u16)aa.z; a[5] = (u16)(aa.z >> 16); a[6] = (u16)aa.w; a[7] = (u16)(aa.w >> 16);
-  } else {
+  // ---- load: kRowsPerWarp x (LDG.32 word + LDG.U16 adc), all in flight together
+  u32 w[kRowsPerWarp], a[kRowsPerWarp];
+  {
+    const u32* __restrict__ pw = ev.words + i0;
+    const u16* __restrict__ pa = ev.adc + i0;
+    if (i0 - lane + 32u * kRowsPerWarp <= W) {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const bool in = i0 + j < W;
-      w[j] = in ? __ldg(ev.words + i0 + j) : 0u;
-      a[j] = in ? __ldg(ev.adc + i0 + j) : (u16)0;
+      for (int j = 0; j < kRowsPerWarp; ++j) { w[j] = __ldcs(pw + 32 * j); a[j] = __ldcs(pa + 32 * j); }
+    } else {
+#pragma unroll
+      for (int j = 0; j < kRowsPerWarp; ++j) {
+        const bool in = i0 + 32u * j < W;
+        w[j] = in ? __ldcs(pw + 32 * j) : 0x80000000u;
+        a[j] = in ? __ldcs(pa + 32 * j) : 0u;
+      }
     }
   }
-  // ---- decode validity (A2, A3): digi iff !bit31 and module<M and row<R and col<C
-  u32 vmask = 0, inmask = 0, max1 = 0;
+  // ---- validity (A2, A3): digi iff !bit31 and module<M and row<R and col<C
+  u32 vmask = 0, cnt = 0, max1 = 0;
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
+  for (int j = 0; j < kRowsPerWarp; ++j) {
     const u32 x = w[j];
     const u32 mod = (x >> 20) & 0x7FFu, row = (x >> 12) & 0xFFu, col = (x >> 3) & 0x1FFu;
-    const bool in = i0 + j < W;
-    const bool ok = in && !(x >> 31) && mod < g.M && row < g.R && col < g.C;
-    inmask |= (u32)in << j;
-    vmask |= (u32)ok << j;
-    if (ok) max1 = max(max1, mod + 1);
+    const bool ok = (int)x >= 0 && mod < g.M && row < g.R && col < g.C && i0 + 32u * j < W;
+    cnt += __popc(__ballot_sync(0xFFFFFFFFu, ok));
+    if (ok) { max1 = max(max1, mod + 1u); vmask |= 1u << j; }
   }
-  const u32 cnt = __popc(vmask);
-  const u32 incl = warp_incl_scan(cnt, lane);
   const u32 wmax = __reduce_max_sync(0xFFFFFFFFu, max1);
-  if (lane == 31) { sWsum[warp] = incl; sWmax[warp] = wmax; }
+  if (lane == 0) { sWsum[warp] = cnt; sWmax[warp] = wmax; }
   __syncthreads();
-  u32 wbase = 0, tileCnt = 0, tileMax1 = 0;
+  u32 wbase = 0, tileCnt = 0, tileMax1 = 0, prev1 = 0;
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
-    const u32 s = sWsum[k];
-    if (k < warp) wbase += s;
+    const u32 s = sWsum[k], m = sWmax[k];
+    if (k < warp) { wbase += s; prev1 = max(prev1, m); }
     tileCnt += s;
-    tileMax1 = max(tileMax1, sWmax[k]);
+    tileMax1 = max(tileMax1, m);
   }
-  const u32 r0 = wbase + incl - cnt;                 // tile-local rank of this thread's first digi
 
   // ---- decoupled look-back for the event-global digi offset and running max(module)+1
   u32 g0 = 0, carryMax1 = 0;
@@ -274,81 +238,37 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     }
     if (tid == 0) st_state(state + tile, pack_state(kStIncl, g0 + tileCnt, max(carryMax1, tileMax1)));
   }
-  const u32 ph = g0 & 7u;                            // smem phase = global 16-byte phase of u16 arrays
 
-  // ---- compact into shared memory; errors straight to global (rare)
-  {
-    u32 p = ph + r0, before = g0 + r0;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      if (vmask >> j & 1) {
-        sWord[p] = w[j]; sAdc[p] = a[j]; sOff[p] = (u16)(tid * kWordsPerThread + j);
-        ++p; ++before;
-      } else if (inmask >> j & 1) {
-        const u32 i = i0 + j, ei = i - before;       // errors before i = i - digis before i
-        ev.errWord[ei] = w[j]; ev.errIdx[ei] = i;
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- write out: chunk c covers global digis [ga + 8c, ga + 8c + 8), ga = g0 & ~7
-  const u32 ga = g0 - ph, end = ph + tileCnt;
-  const u32 nChunks = (end + 7) >> 3;
-  const u32 wordBase = tile * kTileWords;
+  // ---- write: digis straight to their place (consecutive lanes -> consecutive addresses), errors
+  // to theirs (rare), module boundaries into modDigiStart, order check (A5).  prev1 = module + 1 of
+  // the digi before the current row (sorted input: the maximum so far), 0 if there is none.
+  u32 pos = g0 + wbase;
+  prev1 = max(prev1, carryMax1);
   u32 violation = 0;
-  for (u32 c = tid; c < nChunks; c += kUnpackThreads) {
-    const u32 sb = c << 3, gb = ga + sb;
-    const uint4 x0 = *reinterpret_cast<const uint4*>(sWord + sb);
-    const uint4 x1 = *reinterpret_cast<const uint4*>(sWord + sb + 4);
-    const uint4 av = *reinterpret_cast<const uint4*>(sAdc + sb);
-    const uint4 ov = *reinterpret_cast<const uint4*>(sOff + sb);
-    const u32 xs[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-    const u32 a2[4] = {av.x, av.y, av.z, av.w}, o2[4] = {ov.x, ov.y, ov.z, ov.w};
-    int prev = (sb > ph) ? (int)((sWord[sb - 1] >> 20) & 0x7FFu) : (int)carryMax1 - 1;
-    u32 modv[4], rowv[4], colv[4], widx[8]; float q[8];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const u32 s = sb + j;
-      const bool in = s >= ph && s < end;
-      const u32 x = xs[j];
-      const u32 mod = in ? (x >> 20) & 0x7FFu : 0u, row = (x >> 12) & 0xFFu, col = (x >> 3) & 0x1FFu;
-      const u32 ad = (a2[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu, off = (o2[j >> 1] >> ((j & 1) * 16)) & 0xFFFFu;
-      q[j] = __fmaf_rn((float)ad, __ldg(g.gain + mod), __ldg(g.ped + mod));     // A7: one rounding
-      widx[j] = wordBase + off;
-      if (j & 1) { modv[j >> 1] |= mod << 16; rowv[j >> 1] |= row << 16; colv[j >> 1] |= col << 16; }
-      else { modv[j >> 1] = mod; rowv[j >> 1] = row; colv[j >> 1] = col; }
-      if (in) {
-        if ((int)mod > prev) {
-          for (int m = prev + 1; m <= (int)mod; ++m) ev.modDigiStart[m] = gb + j;
-        }
-        if ((int)mod < prev) violation = 1;
-        prev = (int)mod;
-      }
+  for (int j = 0; j < kRowsPerWarp; ++j) {
+    const u32 b = __ballot_sync(0xFFFFFFFFu, vmask >> j & 1u), below = b & lt;
+    const u32 x = w[j];
+    const u32 mod = (x >> 20) & 0x7FFu;
+    const u32 p = pos + __popc(below);                 // digis before this word
+    const u32 i = i0 + 32u * j;
+    const u32 mprev = __shfl_sync(0xFFFFFFFFu, mod, (31 - __clz((int)below)) & 31);
+    const u32 mlast = __shfl_sync(0xFFFFFFFFu, mod, (31 - __clz((int)b)) & 31);
+    if (b >> lane & 1u) {
+      const u32 pm1 = below ? mprev + 1u : prev1;
+      const float2 gp = __ldg(g.calib + mod);
+      ev.module[p] = (u16)mod; ev.row[p] = (u16)((x >> 12) & 0xFFu); ev.col[p] = (u16)((x >> 3) & 0x1FFu);
+      ev.adcOut[p] = (u16)a[j]; ev.wordIdx[p] = i;
+      ev.charge[p] = __fmaf_rn((float)a[j], gp.x, gp.y);                       // A7: one rounding
+      if (mod + 1u > pm1) {
+        for (u32 m = pm1; m <= mod; ++m) ev.modDigiStart[m] = p;
+      } else if (mod + 1u < pm1) violation = 1;
+    } else if (i < W) {
+      const u32 ei = i - p;                            // errors before word i = i - digis before i
+      ev.errWord[ei] = x; ev.errIdx[ei] = i;
     }
-    if (sb >= ph && sb + 8 <= end) {
-      *reinterpret_cast<uint4*>(ev.module + gb) = make_uint4(modv[0], modv[1], modv[2], modv[3]);
-      *reinterpret_cast<uint4*>(ev.row + gb) = make_uint4(rowv[0], rowv[1], rowv[2], rowv[3]);
-      *reinterpret_cast<uint4*>(ev.col + gb) = make_uint4(colv[0], colv[1], colv[2], colv[3]);
-      *reinterpret_cast<uint4*>(ev.adcOut + gb) = av;
-      *reinterpret_cast<uint4*>(ev.wordIdx + gb) = make_uint4(widx[0], widx[1], widx[2], widx[3]);
-      *reinterpret_cast<uint4*>(ev.wordIdx + gb + 4) = make_uint4(widx[4], widx[5], widx[6], widx[7]);
-      *reinterpret_cast<float4*>(ev.charge + gb) = make_float4(q[0], q[1], q[2], q[3]);
-      *reinterpret_cast<float4*>(ev.charge + gb + 4) = make_float4(q[4], q[5], q[6], q[7]);
-    } else {
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const u32 s = sb + j;
-        if (s >= ph && s < end) {
-          ev.module[gb + j] = (u16)(modv[j >> 1] >> ((j & 1) * 16));
-          ev.row[gb + j] = (u16)(rowv[j >> 1] >> ((j & 1) * 16));
-          ev.col[gb + j] = (u16)(colv[j >> 1] >> ((j & 1) * 16));
-          ev.adcOut[gb + j] = (u16)(a2[j >> 1] >> ((j & 1) * 16));
-          ev.wordIdx[gb + j] = widx[j];
-          ev.charge[gb + j] = q[j];
-        }
-      }
-    }
+    if (b) prev1 = mlast + 1u;
+    pos += __popc(b);
   }
   if (violation) atomicOr(&ev.counters->status, 1u);  // PR_STATUS_INPUT_ORDER (A5)
 

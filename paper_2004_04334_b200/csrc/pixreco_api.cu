@@ -32,7 +32,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct pr_handle {
   pr_config cfg{};
   Geom geom{};
-  float *dGain = nullptr, *dPed = nullptr;
+  float2* dCalib = nullptr;
   CachingPool *devPool = nullptr, *hostPool = nullptr;
   int smCount = 0, clusterBlocksPerSM = 1;
   size_t clusterSmem = 0;
@@ -226,9 +226,10 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ev->itemTab = h->hostPool->alloc(sizeof(ExportItem) * 18 * n, stream);   // export table (mapped pinned)
     if (!ev->hostSlab || !ev->itemTab) { release_blocks(ev, true); return PR_ERR_OOM; }
   }
+  const size_t descBytes = sizeof(EvDesc) * n + sizeof(u16) * totalTiles;   // descriptors, then the tile -> event map
   if (n > 1) {
-    ev->descStage = h->hostPool->alloc(sizeof(EvDesc) * n, stream);
-    ev->descDev = h->devPool->alloc(sizeof(EvDesc) * n, stream);
+    ev->descStage = h->hostPool->alloc(descBytes, stream);
+    ev->descDev = h->devPool->alloc(descBytes, stream);
     if (!ev->descStage || !ev->descDev) { release_blocks(ev, true); return PR_ERR_OOM; }
   }
 
@@ -277,18 +278,22 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, 1, lc, h->geom);
+    k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, nullptr, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
   } else {
     EvDesc* st = (EvDesc*)ev->descStage;
-    for (uint32_t k = 0; k < n; ++k) st[k] = ev->sub[k].desc;
-    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, sizeof(EvDesc) * n, cudaMemcpyHostToDevice, stream));
+    u16* te = (u16*)(st + n);
+    for (uint32_t k = 0; k < n; ++k) {
+      st[k] = ev->sub[k].desc;
+      for (uint32_t t = 0; t < st[k].nTiles; ++t) te[st[k].tileBase + t] = (u16)k;
+    }
+    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, descBytes, cudaMemcpyHostToDevice, stream));
     ++nMemcpy;
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -448,17 +453,20 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   cudaDeviceProp prop{};
   if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
   h->smCount = prop.multiProcessorCount;
-  const size_t tb = (size_t)cfg->n_modules * sizeof(float);
-  if (cudaMalloc(&h->dGain, tb) != cudaSuccess || cudaMalloc(&h->dPed, tb) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_OOM); }
-  if (cudaMemcpy(h->dGain, cfg->gain, tb, cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemcpy(h->dPed, cfg->pedestal, tb, cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
+  {
+    std::vector<float2> cal(cfg->n_modules);
+    for (uint32_t m = 0; m < cfg->n_modules; ++m) cal[m] = make_float2(cfg->gain[m], cfg->pedestal[m]);
+    const size_t tb = cal.size() * sizeof(float2);
+    if (cudaMalloc(&h->dCalib, tb) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_OOM); }
+    if (cudaMemcpy(h->dCalib, cal.data(), tb, cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
+  }
   Geom& g = h->geom;
   g.M = cfg->n_modules; g.R = cfg->n_rows; g.C = cfg->n_cols;
   g.stride = (g.C + 2 + 31) / 32;
   g.bitmapWords = (g.R + 2) * g.stride + 1;
   g.pixThr = cfg->pixel_threshold_e;
   g.clusThrFixed = (i64)llrint((double)cfg->cluster_threshold_e * 16384.0);
-  g.gain = h->dGain; g.ped = h->dPed;
+  g.calib = h->dCalib;
   h->clusterSmem = cluster_smem_bytes(g.bitmapWords);
   if (cudaFuncSetAttribute(k_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess ||
       cudaFuncSetAttribute(k_cluster<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess) {
@@ -507,8 +515,7 @@ int pr_destroy(pr_handle* h) {
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
-  if (h->dGain) cudaFree(h->dGain);
-  if (h->dPed) cudaFree(h->dPed);
+  if (h->dCalib) cudaFree(h->dCalib);
   cudaGetLastError();
   delete h;
   return PR_OK;
