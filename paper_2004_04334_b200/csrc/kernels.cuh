@@ -17,6 +17,7 @@
 // Definitions of every quantity: DESIGN.md, readings A1-A14.  Shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 namespace pixreco {
@@ -30,8 +31,8 @@ constexpr u32 kInvalid = 0xFFFFFFFFu;
 
 // ---- unpack kernel geometry ----
 constexpr int kUnpackThreads = 256;
-constexpr int kRowsPerWarp = 8;                                      // rows of 32 consecutive words per warp
-constexpr int kTileWords = kUnpackThreads * kRowsPerWarp;            // 2048
+constexpr int kTileWords = 8 * kUnpackThreads;                       // 2048: each thread owns two runs of 4 consecutive words
+constexpr int kLookBack = 8;                                         // predecessor states per lane and look-back round (256 per round)
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
@@ -51,26 +52,31 @@ struct HostCounters {
   u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, seq;
 };
 
-// One event of a launch.
+// One event of a launch.  The first 128 bytes are all that k_unpack reads: in a batch, one warp-wide
+// load brings them into shared memory.
 struct EvDesc {
   const u32* words; const u16* adc;
   u32 nWords, tileBase, nTiles, cap;
-  // digi SoA [cap]
-  u16 *module, *row, *col, *adcOut; u32* wordIdx; float* charge; u32* label; int32_t* clus;
+  // digi SoA [cap] (first six written by k_unpack)
+  u16 *module, *row, *col, *adcOut; u32* wordIdx; float* charge;
   // error list [cap]
   u32 *errWord, *errIdx;
-  // [M+1]
-  u32 *modDigiStart, *modClusStart;
+  u32* modDigiStart;                // [M+1]
+  DevCounters* counters;
+  u64* tileState;                   // k_unpack look-back states [nTiles]
+  u64 unpackPad;                    // ---- 128 bytes up to here ----
+  u32* label; int32_t* clus;
+  u32* modClusStart;                // [M+1]
   // cluster SoA [cap]
   u32 *clLabel, *clSize; u16* clModule; float *clCharge, *clRow, *clCol;
   // global workspace tier for large modules [cap] each
   u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
-  DevCounters* counters; HostCounters* hostCounters;
-  u64* tileState;                   // k_unpack look-back states [nTiles]
+  HostCounters* hostCounters;
   u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
   // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
   double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
 };
+static_assert(offsetof(EvDesc, label) == 128, "k_unpack's part of the descriptor is one 128-byte line");
 
 struct Geom {
   u32 M, R, C;
@@ -125,158 +131,287 @@ __device__ __forceinline__ u32 block_excl_scan(u32 v, u32* sw, u32* total) {
   return base + incl - v;
 }
 
-// CTA-wide decoupled look-back (blockDim = 256): thread j reads the state of unit (self-1-j), so
-// one round covers 256 predecessors.  With hundreds of units in flight, a 32-wide window needed
-// one serial L2 round trip per 32 predecessors and dominated the kernels.  Every thread returns
-// the combined (count, max1) of all predecessors in [0, self).  Contains __syncthreads.
-struct LbShared { u32 cnt[8], mx[8]; };
-__device__ __forceinline__ void lookback_cta(const u64* state, int self, LbShared& lb, u32* cnt, u32* mx1) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// Decoupled look-back by ONE warp, split in two so that its latency hides behind other work:
+// lookback_issue puts the first round's state loads in flight (lane l reads kLookBack predecessors,
+// 32 * kLookBack tiles per round); lookback_resolve consumes them, spins on predecessors that had
+// not published yet, and goes further back if no inclusive state was among them.  Returns in all
+// lanes the combined (count, max module + 1) of all predecessors in [0, self).
+__device__ __forceinline__ void lookback_issue(const u64* state, int self, u32 lane, u64 (&v)[kLookBack]) {
+#pragma unroll
+  for (int k = 0; k < kLookBack; ++k) {
+    const int idx = self - 1 - 32 * k - (int)lane;
+    v[k] = idx >= 0 ? ld_state(state + idx) : kStIncl;     // virtual zero inclusive before tile 0
+  }
+}
+__device__ __forceinline__ void lookback_resolve(const u64* state, int self, u32 lane, u64 (&v)[kLookBack], u32* cnt, u32* mx1) {
   u32 c = 0, m = 0;
   int look = self - 1;
-  while (look >= 0) {                                  // block-uniform
-    const int idx = look - tid;
-    u64 v = kStIncl;                                   // virtual zero inclusive before unit 0
-    if (idx >= 0) do { v = ld_state(state + idx); } while (st_status(v) == 0);
-    const u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v) == 2);
-    const int upto = inclMask ? (__ffs(inclMask) - 1) : 31;
-    const u32 cc = lane <= upto ? st_count(v) : 0, mm = lane <= upto ? st_max1(v) : 0;
-    const u32 wc = __reduce_add_sync(0xFFFFFFFFu, cc), wm = __reduce_max_sync(0xFFFFFFFFu, mm);
-    __syncthreads();                                   // previous readers of lb are done
-    if (lane == 0) { lb.cnt[warp] = wc; lb.mx[warp] = wm | (inclMask ? 0x80000000u : 0u); }
-    __syncthreads();
+  for (;;) {                                               // warp-uniform
     bool found = false;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < kLookBack; ++k) {
       if (!found) {
-        c += lb.cnt[k];
-        const u32 x = lb.mx[k];
-        m = max(m, x & 0xFFFu);
-        found = (x >> 31) != 0;
+        const int idx = look - 32 * k - (int)lane;
+        while (st_status(v[k]) == 0) v[k] = ld_state(state + idx);   // predecessor has not published yet
+        const u32 inclMask = __ballot_sync(0xFFFFFFFFu, st_status(v[k]) == 2);
+        const u32 upto = inclMask ? (u32)__ffs((int)inclMask) - 1u : 31u;
+        c += __reduce_add_sync(0xFFFFFFFFu, lane <= upto ? st_count(v[k]) : 0u);
+        m = max(m, __reduce_max_sync(0xFFFFFFFFu, lane <= upto ? st_max1(v[k]) : 0u));
+        found = inclMask != 0u;
       }
     }
     if (found) break;
-    look -= 256;
+    look -= 32 * kLookBack;
+#pragma unroll
+    for (int k = 0; k < kLookBack; ++k) {
+      const int idx = look - 32 * k - (int)lane;
+      v[k] = idx >= 0 ? ld_state(state + idx) : kStIncl;
+    }
   }
   *cnt = c; *mx1 = m;
 }
 
 // ================================================================== k_unpack (a1 + a2)
-// One CTA per tile of kTileWords words; warp w owns kRowsPerWarp rows of 32 consecutive words, lane l
-// of row j holds word (32 j + l): every load and every store instruction of a warp touches one
-// contiguous run.  Compaction is a warp ballot + popcount (no shared-memory staging): the digi's
-// place is  g0 (digis of earlier tiles, decoupled look-back) + digis of earlier warps + digis of
-// earlier rows + popc(ballot & lanes below).  Tiles are taken in blockIdx order (the look-back
-// relies on CTAs being scheduled in that order, like every single-pass scan does); in a batch the
-// tile -> event map is a table written by the host next to the descriptors.
+// Persistent CTAs; CTA b takes tiles b, b + gridDim.x, ... of the launch (a tile = kTileWords
+// consecutive words of one event; the grid never exceeds what is co-resident).  Thread t owns words
+// [4t, 4t+4) and [1024 + 4t, 1024 + 4t + 4) of the tile: one LDG.128 + one LDG.64 per run.
+// The loop is software-pipelined over tiles so that no phase waits for another CTA:
+//   A(i)  decode + validity (A2, A3), packed warp scan of the two runs' counts, publish the tile
+//         aggregate, stage every word in shared memory (digis at their position in the tile,
+//         error words behind them), issue the loads of tile i+1, issue the look-back loads of tile i
+//   B(i-1) write the previous tile from shared memory: its event-global digi offset g0 is known by
+//         now; a quad of 4 consecutive digis aligned to the OUTPUT position becomes one 8- or
+//         16-byte store per array (module,row,col,adc u16; wordIdx u32; charge f32 = fmaf, A7);
+//         module boundaries (modDigiStart) and order violations (A5) come from comparing each
+//         digi with the one before it; error words (rare) are copied out behind
+//   R(i)  warp 0 resolves tile i's look-back (its loads flew during B) and publishes the
+//         inclusive state
+// The stage is kept in four planes (slot s lives at plane s & 3, index s >> 2), so that both the
+// scattered staging stores and the output-aligned quad reads are free of bank conflicts whatever
+// g0 mod 4 is.
 // Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
-template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads, 5)
-k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
-         const __grid_constant__ Geom g) {
-  __shared__ u32 sWsum[8], sWmax[8];
-  __shared__ LbShared sLb;
-  __shared__ __align__(16) EvDesc sEv;             // batch: the tile's descriptor (pointers stay out of registers)
+constexpr u32 kStagePlane = kTileWords / 4 + 4;
+__device__ __forceinline__ u32 stage_idx(u32 s) { return (s & 3u) * kStagePlane + (s >> 2); }
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const u32 lt = (1u << lane) - 1u;
-  if (!kSingle) {
-    const u32* src = reinterpret_cast<const u32*>(batch + tileEvent[blockIdx.x]);
-    if (tid < (int)(sizeof(EvDesc) / 4)) reinterpret_cast<u32*>(&sEv)[tid] = __ldg(src + tid);
-    __syncthreads();
+struct UnpackStage { u32 x[4 * kStagePlane], a[4 * kStagePlane]; };   // raw word; adc | (word offset in tile) << 16
+struct UnpackShared {
+  UnpackStage st[2];                // tile i is staged in st[i & 1]; slot = 4 + position
+  uint2 wagg[8];                    // per warp: packed counts of the two runs, max(module)+1
+  u32 g0, carry1;                   // look-back result of the tile just resolved
+  u32 desc[4][32];                  // batch: descriptors of the previous, this, the next tile and the one after
+};
+
+struct RawTile { uint4 xa, xb; uint2 aa, ab; };   // aa/ab: four u16 adc values each
+
+__device__ __forceinline__ void unpack_load(const u32* __restrict__ words, const u16* __restrict__ adc, u32 W, u32 tileInEv,
+                                            u32 tid, RawTile& r) {
+  const u32 T0 = tileInEv * (u32)kTileWords;
+  if (T0 + (u32)kTileWords <= W) {
+    r.xa = __ldcs(reinterpret_cast<const uint4*>(words + T0) + tid);
+    r.xb = __ldcs(reinterpret_cast<const uint4*>(words + T0 + kTileWords / 2) + tid);
+    r.aa = __ldcs(reinterpret_cast<const uint2*>(adc + T0) + tid);
+    r.ab = __ldcs(reinterpret_cast<const uint2*>(adc + T0 + kTileWords / 2) + tid);
+  } else {                                             // the event's ragged last tile: words beyond W read as invalid
+    u32 x[8], a[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const u32 i = T0 + (j < 4 ? 0u : (u32)kTileWords / 2) + 4u * tid + (u32)(j & 3);
+      const bool in = i < W;
+      x[j] = in ? __ldcs(words + i) : 0xFFFFFFFFu;
+      a[j] = in ? (u32)__ldcs(adc + i) : 0u;
+    }
+    r.xa = make_uint4(x[0], x[1], x[2], x[3]); r.xb = make_uint4(x[4], x[5], x[6], x[7]);
+    r.aa = make_uint2(a[0] | a[1] << 16, a[2] | a[3] << 16); r.ab = make_uint2(a[4] | a[5] << 16, a[6] | a[7] << 16);
   }
-  const EvDesc& ev = kSingle ? single : sEv;
-  const u32 tile = blockIdx.x - ev.tileBase, W = ev.nWords;
-  const u32 i0 = tile * kTileWords + warp * (32u * kRowsPerWarp) + lane;   // this lane's word of row 0
+}
 
-  // ---- load: kRowsPerWarp x (LDG.32 word + LDG.U16 adc), all in flight together
-  u32 w[kRowsPerWarp], a[kRowsPerWarp];
-  {
-    const u32* __restrict__ pw = ev.words + i0;
-    const u16* __restrict__ pa = ev.adc + i0;
-    if (i0 - lane + 32u * kRowsPerWarp <= W) {
+// B: write one staged tile.  n digis at event positions [g0, g0 + n); carry1 = module + 1 of the
+// digi before the tile (0 if none); the tile's in-range words are [wordBase, wordBase + inRange).
+__device__ __forceinline__ void unpack_write(const EvDesc& ev, const Geom& g, const UnpackStage& st, u32 tid, u32 tile, u32 n,
+                                             u32 tileMax1, u32 g0, u32 carry1) {
+  const u32 ph = g0 & 3u, base4 = g0 & ~3u, nQ = (ph + n + 3u) >> 2, wordBase = tile * (u32)kTileWords, W = ev.nWords;
+  const u32 fake = ((carry1 - 1u) & 0xFFFu) << 20;       // stands for "the digi before this tile"
+  u32 violation = 0;
+  for (u32 q = tid; q < nQ; q += kUnpackThreads) {
+    const u32 p0 = base4 + 4u * q, s0 = 4u * q + 4u - ph;  // output element p0 + j <- stage slot s0 + j
+    if (4u * q >= ph && 4u * q + 4u <= ph + n) {
+      u32 xs[5], as[4];
+      xs[0] = s0 == 4u ? fake : st.x[stage_idx(s0 - 1u)];
 #pragma unroll
-      for (int j = 0; j < kRowsPerWarp; ++j) { w[j] = __ldcs(pw + 32 * j); a[j] = __ldcs(pa + 32 * j); }
-    } else {
+      for (int j = 0; j < 4; ++j) { xs[j + 1] = st.x[stage_idx(s0 + (u32)j)]; as[j] = st.a[stage_idx(s0 + (u32)j)]; }
+      const u32 d = (xs[1] ^ xs[0]) | (xs[2] ^ xs[1]) | (xs[3] ^ xs[2]) | (xs[4] ^ xs[3]);
+      float4 ch;
+      if ((d >> 20) == 0u) {                             // one module, same as the digi before: the common case
+        const float2 gp = __ldg(g.calib + (xs[1] >> 20));
+        ch.x = __fmaf_rn((float)(as[0] & 0xFFFFu), gp.x, gp.y); ch.y = __fmaf_rn((float)(as[1] & 0xFFFFu), gp.x, gp.y);
+        ch.z = __fmaf_rn((float)(as[2] & 0xFFFFu), gp.x, gp.y); ch.w = __fmaf_rn((float)(as[3] & 0xFFFFu), gp.x, gp.y);
+      } else {
+        float c4[4];
 #pragma unroll
-      for (int j = 0; j < kRowsPerWarp; ++j) {
-        const bool in = i0 + 32u * j < W;
-        w[j] = in ? __ldcs(pw + 32 * j) : 0x80000000u;
-        a[j] = in ? __ldcs(pa + 32 * j) : 0u;
+        for (int j = 0; j < 4; ++j) {
+          const u32 mod = xs[j + 1] >> 20, prev1 = ((xs[j] >> 20) + 1u) & 0xFFFu;
+          const float2 gp = __ldg(g.calib + mod);
+          c4[j] = __fmaf_rn((float)(as[j] & 0xFFFFu), gp.x, gp.y);
+          if (mod + 1u > prev1) {
+            for (u32 m = prev1; m <= mod; ++m) ev.modDigiStart[m] = p0 + (u32)j;
+          } else if (mod + 1u < prev1) violation = 1;
+        }
+        ch = make_float4(c4[0], c4[1], c4[2], c4[3]);
+      }
+      *reinterpret_cast<uint2*>(ev.module + p0) = make_uint2((xs[1] >> 20) | (xs[2] >> 20) << 16, (xs[3] >> 20) | (xs[4] >> 20) << 16);
+      *reinterpret_cast<uint2*>(ev.row + p0) = make_uint2(((xs[1] >> 12) & 0xFFu) | ((xs[2] >> 12) & 0xFFu) << 16,
+                                                          ((xs[3] >> 12) & 0xFFu) | ((xs[4] >> 12) & 0xFFu) << 16);
+      *reinterpret_cast<uint2*>(ev.col + p0) = make_uint2(((xs[1] >> 3) & 0x1FFu) | ((xs[2] >> 3) & 0x1FFu) << 16,
+                                                          ((xs[3] >> 3) & 0x1FFu) | ((xs[4] >> 3) & 0x1FFu) << 16);
+      *reinterpret_cast<uint2*>(ev.adcOut + p0) = make_uint2(__byte_perm(as[0], as[1], 0x5410), __byte_perm(as[2], as[3], 0x5410));
+      *reinterpret_cast<uint4*>(ev.wordIdx + p0) = make_uint4(wordBase + (as[0] >> 16), wordBase + (as[1] >> 16),
+                                                              wordBase + (as[2] >> 16), wordBase + (as[3] >> 16));
+      *reinterpret_cast<float4*>(ev.charge + p0) = ch;
+    } else {                                              // the tile's first and last quad may be partial
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const u32 pos = 4u * q + (u32)j - ph;             // position in the tile (wraps below 0)
+        if (pos >= n) continue;
+        const u32 xx = st.x[stage_idx(pos + 4u)], aa = st.a[stage_idx(pos + 4u)];
+        const u32 xp = pos ? st.x[stage_idx(pos + 3u)] : fake;
+        const u32 mod = xx >> 20, prev1 = ((xp >> 20) + 1u) & 0xFFFu, p = p0 + (u32)j;
+        const float2 gp = __ldg(g.calib + mod);
+        ev.module[p] = (u16)mod; ev.row[p] = (u16)((xx >> 12) & 0xFFu); ev.col[p] = (u16)((xx >> 3) & 0x1FFu);
+        ev.adcOut[p] = (u16)(aa & 0xFFFFu); ev.wordIdx[p] = wordBase + (aa >> 16);
+        ev.charge[p] = __fmaf_rn((float)(aa & 0xFFFFu), gp.x, gp.y);
+        if (mod + 1u > prev1) {
+          for (u32 m = prev1; m <= mod; ++m) ev.modDigiStart[m] = p;
+        } else if (mod + 1u < prev1) violation = 1;
       }
     }
   }
-  // ---- validity (A2, A3): digi iff !bit31 and module<M and row<R and col<C
-  u32 vmask = 0, cnt = 0, max1 = 0;
-#pragma unroll
-  for (int j = 0; j < kRowsPerWarp; ++j) {
-    const u32 x = w[j];
-    const u32 mod = (x >> 20) & 0x7FFu, row = (x >> 12) & 0xFFu, col = (x >> 3) & 0x1FFu;
-    const bool ok = (int)x >= 0 && mod < g.M && row < g.R && col < g.C && i0 + 32u * j < W;
-    cnt += __popc(__ballot_sync(0xFFFFFFFFu, ok));
-    if (ok) { max1 = max(max1, mod + 1u); vmask |= 1u << j; }
-  }
-  const u32 wmax = __reduce_max_sync(0xFFFFFFFFu, max1);
-  if (lane == 0) { sWsum[warp] = cnt; sWmax[warp] = wmax; }
-  __syncthreads();
-  u32 wbase = 0, tileCnt = 0, tileMax1 = 0, prev1 = 0;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    const u32 s = sWsum[k], m = sWmax[k];
-    if (k < warp) { wbase += s; prev1 = max(prev1, m); }
-    tileCnt += s;
-    tileMax1 = max(tileMax1, m);
-  }
-
-  // ---- decoupled look-back for the event-global digi offset and running max(module)+1
-  u32 g0 = 0, carryMax1 = 0;
+  if (violation) atomicOr(&ev.counters->status, 1u);     // PR_STATUS_INPUT_ORDER (A5)
+  // ---- error words (A2-A4): staged behind the digis in word order; errors before the tile = words - digis before it
   {
-    u64* state = ev.tileState;
-    if (tile > 0) {
-      if (tid == 0) st_state(state + tile, pack_state(kStAgg, tileCnt, tileMax1));
-      lookback_cta(state, (int)tile, sLb, &g0, &carryMax1);
+    const u32 inRange = W > wordBase ? min(W - wordBase, (u32)kTileWords) : 0u, nErr = inRange - n, e0 = wordBase - g0;
+    for (u32 e = tid; e < nErr; e += kUnpackThreads) {
+      const u32 s = stage_idx(n + e + 4u);
+      ev.errWord[e0 + e] = st.x[s]; ev.errIdx[e0 + e] = wordBase + (st.a[s] >> 16);
     }
-    if (tid == 0) st_state(state + tile, pack_state(kStIncl, g0 + tileCnt, max(carryMax1, tileMax1)));
   }
-
-  // ---- write: digis straight to their place (consecutive lanes -> consecutive addresses), errors
-  // to theirs (rare), module boundaries into modDigiStart, order check (A5).  prev1 = module + 1 of
-  // the digi before the current row (sorted input: the maximum so far), 0 if there is none.
-  u32 pos = g0 + wbase;
-  prev1 = max(prev1, carryMax1);
-  u32 violation = 0;
-#pragma unroll
-  for (int j = 0; j < kRowsPerWarp; ++j) {
-    const u32 b = __ballot_sync(0xFFFFFFFFu, vmask >> j & 1u), below = b & lt;
-    const u32 x = w[j];
-    const u32 mod = (x >> 20) & 0x7FFu;
-    const u32 p = pos + __popc(below);                 // digis before this word
-    const u32 i = i0 + 32u * j;
-    const u32 mprev = __shfl_sync(0xFFFFFFFFu, mod, (31 - __clz((int)below)) & 31);
-    const u32 mlast = __shfl_sync(0xFFFFFFFFu, mod, (31 - __clz((int)b)) & 31);
-    if (b >> lane & 1u) {
-      const u32 pm1 = below ? mprev + 1u : prev1;
-      const float2 gp = __ldg(g.calib + mod);
-      ev.module[p] = (u16)mod; ev.row[p] = (u16)((x >> 12) & 0xFFu); ev.col[p] = (u16)((x >> 3) & 0x1FFu);
-      ev.adcOut[p] = (u16)a[j]; ev.wordIdx[p] = i;
-      ev.charge[p] = __fmaf_rn((float)a[j], gp.x, gp.y);                       // A7: one rounding
-      if (mod + 1u > pm1) {
-        for (u32 m = pm1; m <= mod; ++m) ev.modDigiStart[m] = p;
-      } else if (mod + 1u < pm1) violation = 1;
-    } else if (i < W) {
-      const u32 ei = i - p;                            // errors before word i = i - digis before i
-      ev.errWord[ei] = x; ev.errIdx[ei] = i;
-    }
-    if (b) prev1 = mlast + 1u;
-    pos += __popc(b);
-  }
-  if (violation) atomicOr(&ev.counters->status, 1u);  // PR_STATUS_INPUT_ORDER (A5)
-
   // ---- the event's last tile closes modDigiStart and the counters
-  if (tile == ev.nTiles - 1) {
-    const u32 D = g0 + tileCnt, mx1 = max(carryMax1, tileMax1);
+  if (tile == ev.nTiles - 1u) {
+    const u32 D = g0 + n, mx1 = max(carry1, tileMax1);
     for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) ev.modDigiStart[m] = D;
     if (tid == 0) { ev.counters->nWords = W; ev.counters->nDigis = D; ev.counters->nErrors = W - D; }
+  }
+}
+
+template <bool kSingle>
+__global__ void __launch_bounds__(kUnpackThreads, 4)
+k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
+         u32 totalTiles, const __grid_constant__ Geom g) {
+  __shared__ __align__(16) UnpackShared sh;
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, G = gridDim.x;
+  u32 t = blockIdx.x;
+  if (t >= totalTiles) return;
+  u32 prv = 3, cur = 0, nxt = 1, nn = 2, eNN = 0;      // descriptor ring (batch)
+  if (!kSingle) {
+    if (warp < 2) {
+      const u32 tt = min(t + warp * G, totalTiles - 1u);
+      sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[tt]) + lane);
+      if (warp == 1 && t + 2u * G < totalTiles) eNN = tileEvent[t + 2u * G];
+    }
+    __syncthreads();
+  }
+  RawTile raw;
+  {
+    const EvDesc& ev = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[0]);
+    unpack_load(ev.words, ev.adc, ev.nWords, t - ev.tileBase, tid, raw);
+  }
+  const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
+  bool haveA = true, haveB = false;
+  u32 pTile = 0, pN = 0, pMax1 = 0, pG0 = 0, pCarry1 = 0;          // the previous tile, for B
+
+  for (u32 it = 0;; ++it) {
+    const EvDesc& ev = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[cur]);
+    UnpackStage& st = sh.st[it & 1u];
+    u32 tile = 0, n = 0, tileMax1 = 0, dword = 0, eN3 = 0;
+    u32 x[8], ap[4], vmask = 0, packed = 0, incl = 0;
+    RawTile rawNext;
+    u64 lb[kLookBack];
+    if (haveA) {
+      tile = t - ev.tileBase;
+      // batch: descriptor of tile t + 2G and event of tile t + 3G, in flight until the end of the iteration
+      if (!kSingle && warp == 1) {
+        if (t + 2u * G < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(batch + eNN) + lane);
+        if (t + 3u * G < totalTiles) eN3 = tileEvent[t + 3u * G];
+      }
+      // ---- validity (A2, A3): digi iff module < M (bit 31 set makes it >= 2048), row < R, col < C
+      x[0] = raw.xa.x; x[1] = raw.xa.y; x[2] = raw.xa.z; x[3] = raw.xa.w; x[4] = raw.xb.x; x[5] = raw.xb.y; x[6] = raw.xb.z; x[7] = raw.xb.w;
+      ap[0] = raw.aa.x; ap[1] = raw.aa.y; ap[2] = raw.ab.x; ap[3] = raw.ab.y;
+      int mmax = -1;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const u32 mod = x[j] >> 20;
+        const bool ok = mod < limM && (x[j] & 0xFF000u) < limR && (x[j] & 0xFF8u) < limC;
+        if (ok) { vmask |= 1u << j; mmax = max(mmax, (int)mod); }
+      }
+      packed = (u32)__popc(vmask & 15u) | (u32)__popc(vmask >> 4) << 16;
+      incl = warp_incl_scan(packed, (int)lane);
+      const u32 wmax1 = __reduce_max_sync(0xFFFFFFFFu, (u32)(mmax + 1));
+      if (lane == 31) sh.wagg[warp] = make_uint2(incl, wmax1);
+    }
+    __syncthreads();                                                         // #1
+    if (haveA) {
+      u32 base = 0, tot = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const uint2 s = sh.wagg[k];
+        if (k < (int)warp) base += s.x;
+        tot += s.x;
+        tileMax1 = max(tileMax1, s.y);
+      }
+      const u32 tileA = tot & 0xFFFFu;
+      n = tileA + (tot >> 16);
+      u64* state = ev.tileState;
+      if (tid == 0) st_state(state + tile, pack_state(tile ? kStAgg : kStIncl, n, tileMax1));
+      // ---- the next tile's loads are issued now and consumed in the next iteration
+      if (t + G < totalTiles) {
+        const EvDesc& en = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[nxt]);
+        unpack_load(en.words, en.adc, en.nWords, t + G - en.tileBase, tid, rawNext);
+      }
+      if (warp == 0 && tile) lookback_issue(state, (int)tile, lane, lb);
+      // ---- stage: digi k of the tile at slot 4 + k, error word e of the tile at slot 4 + n + e
+      const u32 ex = base + incl - packed;
+      u32 posA = ex & 0xFFFFu, posB = tileA + (ex >> 16);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const u32 off = (j < 4 ? 0u : (u32)kTileWords / 2) + 4u * tid + (u32)(j & 3);
+        const u32 a16 = (j & 1) ? ap[j >> 1] >> 16 : ap[j >> 1] & 0xFFFFu;
+        u32& pos = j < 4 ? posA : posB;
+        u32 s;
+        if (vmask >> j & 1u) { s = 4u + pos; ++pos; }
+        else s = 4u + n + (off - pos);                    // words beyond W of a ragged tile land beyond the used slots
+        if (s < 4u + (u32)kTileWords) {
+          s = stage_idx(s);
+          st.x[s] = x[j]; st.a[s] = a16 | off << 16;
+        }
+      }
+    }
+    if (haveB) {
+      const EvDesc& ep = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[prv]);
+      unpack_write(ep, g, sh.st[(it & 1u) ^ 1u], tid, pTile, pN, pMax1, pG0, pCarry1);
+    }
+    if (haveA && warp == 0) {
+      u32 c = 0, m = 0;
+      if (tile) {
+        lookback_resolve(ev.tileState, (int)tile, lane, lb, &c, &m);
+        if (lane == 0) st_state(ev.tileState + tile, pack_state(kStIncl, c + n, max(m, tileMax1)));
+      }
+      if (lane == 0) { sh.g0 = c; sh.carry1 = m; }
+    }
+    __syncthreads();                                                         // #2
+    if (!haveA) break;
+    haveB = true; pTile = tile; pN = n; pMax1 = tileMax1; pG0 = sh.g0; pCarry1 = sh.carry1;
+    if (!kSingle && warp == 1) { sh.desc[nn][lane] = dword; eNN = eN3; }
+    t += G; haveA = t < totalTiles; raw = rawNext;
+    const u32 r = prv; prv = cur; cur = nxt; nxt = nn; nn = r;
   }
 }
 

@@ -34,7 +34,7 @@ struct pr_handle {
   Geom geom{};
   float2* dCalib = nullptr;
   CachingPool *devPool = nullptr, *hostPool = nullptr;
-  int smCount = 0, clusterBlocksPerSM = 1;
+  int smCount = 0, clusterBlocksPerSM = 1, unpackBlocksPerSM = 1;
   size_t clusterSmem = 0;
   std::mutex mu;
   std::vector<pr_event*> slots;
@@ -275,10 +275,14 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
   if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
   if (clusterGrid < 1) clusterGrid = 1;
+  // k_unpack: persistent CTAs striding over the tiles; never more than are co-resident (its look-back
+  // waits on earlier tiles, which must therefore be running or done)
+  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
+  if (unpackGrid > totalTiles) unpackGrid = totalTiles;
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<totalTiles, kUnpackThreads, 0, stream>>>(d, nullptr, nullptr, h->geom);
+    k_unpack<true><<<unpackGrid, kUnpackThreads, 0, stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -293,7 +297,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, descBytes, cudaMemcpyHostToDevice, stream));
     ++nMemcpy;
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<totalTiles, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), h->geom);
+    k_unpack<false><<<unpackGrid, kUnpackThreads, 0, stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -475,6 +479,9 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   int bps = 1;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_cluster<true>, kClusterThreads, h->clusterSmem) != cudaSuccess) { cudaGetLastError(); bps = 1; }
   h->clusterBlocksPerSM = bps < 1 ? 1 : bps;
+  int ups = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ups, k_unpack<false>, kUnpackThreads, 0) != cudaSuccess) { cudaGetLastError(); ups = 1; }
+  h->unpackBlocksPerSM = ups < 1 ? 1 : ups;
   h->devPool = new CachingPool(make_device_backend(cfg->device), cfg->max_cached_bytes_device);
   h->hostPool = new CachingPool(make_pinned_backend(cfg->device), cfg->max_cached_bytes_host);
 
