@@ -31,7 +31,7 @@ constexpr u32 kInvalid = 0xFFFFFFFFu;
 
 // ---- unpack kernel geometry ----
 constexpr int kUnpackThreads = 256;
-constexpr int kTileWords = 8 * kUnpackThreads;                       // 2048: each thread owns two runs of 4 consecutive words
+constexpr int kTileWords = 8 * kUnpackThreads;                       // 2048: warp w owns words [256w, 256w + 256), lane l word 32j + l of row j
 constexpr int kLookBack = 8;                                         // predecessor states per lane and look-back round (256 per round)
 
 // ---- cluster kernel geometry ----
@@ -173,246 +173,284 @@ __device__ __forceinline__ void lookback_resolve(const u64* state, int self, u32
 
 // ================================================================== k_unpack (a1 + a2)
 // Persistent CTAs; CTA b takes tiles b, b + gridDim.x, ... of the launch (a tile = kTileWords
-// consecutive words of one event; the grid never exceeds what is co-resident).  Thread t owns words
-// [4t, 4t+4) and [1024 + 4t, 1024 + 4t + 4) of the tile: one LDG.128 + one LDG.64 per run.
-// The loop is software-pipelined over tiles so that no phase waits for another CTA:
-//   A(i)  decode + validity (A2, A3), packed warp scan of the two runs' counts, publish the tile
-//         aggregate, stage every word in shared memory (digis at their position in the tile,
-//         error words behind them), issue the loads of tile i+1, issue the look-back loads of tile i
-//   B(i-1) write the previous tile from shared memory: its event-global digi offset g0 is known by
-//         now; a quad of 4 consecutive digis aligned to the OUTPUT position becomes one 8- or
-//         16-byte store per array (module,row,col,adc u16; wordIdx u32; charge f32 = fmaf, A7);
-//         module boundaries (modDigiStart) and order violations (A5) come from comparing each
-//         digi with the one before it; error words (rare) are copied out behind
-//   R(i)  warp 0 resolves tile i's look-back (its loads flew during B) and publishes the
-//         inclusive state
-// The stage is kept in four planes (slot s lives at plane s & 3, index s >> 2), so that both the
-// scattered staging stores and the output-aligned quad reads are free of bank conflicts whatever
-// g0 mod 4 is.
+// consecutive words of one event; the grid never exceeds what is co-resident, because the
+// look-back reads states published by CTAs that must be running).  "Local tile k" below is the
+// k-th tile of this CTA.  Per iteration i the CTA does, with two barriers:
+//   load    (end of iteration i)  one thread issues TMA bulk copies (cp.async.bulk, completion on an
+//           mbarrier) of tile i + kRawSlots into the ring slot tile i just vacated: raw words and
+//           ADC values reach shared memory without passing through registers
+//   count   tile i + kCountAhead: validity (A2, A3) of every word, one ballot per 32 words kept in
+//           shared memory, per-warp digi counts; the tile's aggregate (count, max module + 1) is
+//           PUBLISHED kCountAhead iterations before the tile is written, so when a successor looks
+//           back, the aggregate has long been there: no CTA waits for the progress of another one
+//   scatter tile i: its event-global digi offset g0 is known (look-back resolved in iteration
+//           i - 1).  Warp w owns words [256w, 256w + 256) of the tile, lane l word 32j + l of row j:
+//           position = g0 + warp prefix + row prefix + popc(ballot below lane).  The digi is stored
+//           in FINAL form (module,row,col,adc u16; wordIdx u32; charge f32 = fmaf, A7) into six
+//           shared-memory arrays at index 8 + (g0 & 7) + position, i.e. with the 16-byte phase of
+//           its global destination; error words (rare) go straight to global memory
+//   look-back (warp 0) for tile i + 1: loads issued before the scatter, resolved after it
+//   store   one thread issues six TMA bulk stores of the 16-byte-aligned middle of the staged
+//           arrays; sixteen lanes store the up-to-7 head and tail elements; all threads scan the
+//           staged module array for module boundaries (modDigiStart) and order violations (A5)
 // Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
-constexpr u32 kStagePlane = kTileWords / 4 + 4;
-__device__ __forceinline__ u32 stage_idx(u32 s) { return (s & 3u) * kStagePlane + (s >> 2); }
+constexpr int kRawSlots = 4;                      // raw tiles in the shared-memory ring
+constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
+constexpr int kDescRing = 8;                      // descriptor ring (batch), power of two >= kRawSlots + 2
+constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
+static_assert(kCountAhead >= 1 && kCountAhead <= kRawSlots - 2, "a raw tile needs a full iteration to arrive before it is counted");
+static_assert(kRawSlots + 2 <= kDescRing, "descriptor ring too small");
 
-struct UnpackStage { u32 x[4 * kStagePlane], a[4 * kStagePlane]; };   // raw word; adc | (word offset in tile) << 16
-struct UnpackShared {
-  UnpackStage st[2];                // tile i is staged in st[i & 1]; slot = 4 + position
-  uint2 wagg[8];                    // per warp: packed counts of the two runs, max(module)+1
-  u32 g0, carry1;                   // look-back result of the tile just resolved
-  u32 desc[4][32];                  // batch: descriptors of the previous, this, the next tile and the one after
+struct __align__(128) UnpackShared {
+  u32 words[kRawSlots][kTileWords];               // raw ring (TMA destination)
+  u16 adc[kRawSlots][kTileWords];
+  u16 sModule[kStageElems], sRow[kStageElems], sCol[kStageElems], sAdc[kStageElems];   // staging (TMA source)
+  u32 sWordIdx[kStageElems];
+  float sCharge[kStageElems];
+  u64 full[kRawSlots];                            // mbarriers: raw slot filled
+  u32 bal[kRawSlots][8][8];                       // [slot][warp][row] validity ballots
+  u32 wcnt[kRawSlots][8], wmax[kRawSlots][8];     // per warp: digis, max(module)+1
+  u32 g0[2], carry1[2];                           // look-back result of local tile k at [k & 1]
+  u32 desc[kDescRing][32];                        // batch: first 128 bytes of the tiles' event descriptors
 };
 
-struct RawTile { uint4 xa, xb; uint2 aa, ab; };   // aa/ab: four u16 adc values each
-
-__device__ __forceinline__ void unpack_load(const u32* __restrict__ words, const u16* __restrict__ adc, u32 W, u32 tileInEv,
-                                            u32 tid, RawTile& r) {
-  const u32 T0 = tileInEv * (u32)kTileWords;
-  if (T0 + (u32)kTileWords <= W) {
-    r.xa = __ldcs(reinterpret_cast<const uint4*>(words + T0) + tid);
-    r.xb = __ldcs(reinterpret_cast<const uint4*>(words + T0 + kTileWords / 2) + tid);
-    r.aa = __ldcs(reinterpret_cast<const uint2*>(adc + T0) + tid);
-    r.ab = __ldcs(reinterpret_cast<const uint2*>(adc + T0 + kTileWords / 2) + tid);
-  } else {                                             // the event's ragged last tile: words beyond W read as invalid
-    u32 x[8], a[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      const u32 i = T0 + (j < 4 ? 0u : (u32)kTileWords / 2) + 4u * tid + (u32)(j & 3);
-      const bool in = i < W;
-      x[j] = in ? __ldcs(words + i) : 0xFFFFFFFFu;
-      a[j] = in ? (u32)__ldcs(adc + i) : 0u;
-    }
-    r.xa = make_uint4(x[0], x[1], x[2], x[3]); r.xb = make_uint4(x[4], x[5], x[6], x[7]);
-    r.aa = make_uint2(a[0] | a[1] << 16, a[2] | a[3] << 16); r.ab = make_uint2(a[4] | a[5] << 16, a[6] | a[7] << 16);
-  }
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-
-// B: write one staged tile.  n digis at event positions [g0, g0 + n); carry1 = module + 1 of the
-// digi before the tile (0 if none); the tile's in-range words are [wordBase, wordBase + inRange).
-__device__ __forceinline__ void unpack_write(const EvDesc& ev, const Geom& g, const UnpackStage& st, u32 tid, u32 tile, u32 n,
-                                             u32 tileMax1, u32 g0, u32 carry1) {
-  const u32 ph = g0 & 3u, base4 = g0 & ~3u, nQ = (ph + n + 3u) >> 2, wordBase = tile * (u32)kTileWords, W = ev.nWords;
-  const u32 fake = ((carry1 - 1u) & 0xFFFu) << 20;       // stands for "the digi before this tile"
-  u32 violation = 0;
-  for (u32 q = tid; q < nQ; q += kUnpackThreads) {
-    const u32 p0 = base4 + 4u * q, s0 = 4u * q + 4u - ph;  // output element p0 + j <- stage slot s0 + j
-    if (4u * q >= ph && 4u * q + 4u <= ph + n) {
-      u32 xs[5], as[4];
-      xs[0] = s0 == 4u ? fake : st.x[stage_idx(s0 - 1u)];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { xs[j + 1] = st.x[stage_idx(s0 + (u32)j)]; as[j] = st.a[stage_idx(s0 + (u32)j)]; }
-      const u32 d = (xs[1] ^ xs[0]) | (xs[2] ^ xs[1]) | (xs[3] ^ xs[2]) | (xs[4] ^ xs[3]);
-      float4 ch;
-      if ((d >> 20) == 0u) {                             // one module, same as the digi before: the common case
-        const float2 gp = __ldg(g.calib + (xs[1] >> 20));
-        ch.x = __fmaf_rn((float)(as[0] & 0xFFFFu), gp.x, gp.y); ch.y = __fmaf_rn((float)(as[1] & 0xFFFFu), gp.x, gp.y);
-        ch.z = __fmaf_rn((float)(as[2] & 0xFFFFu), gp.x, gp.y); ch.w = __fmaf_rn((float)(as[3] & 0xFFFFu), gp.x, gp.y);
-      } else {
-        float c4[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const u32 mod = xs[j + 1] >> 20, prev1 = ((xs[j] >> 20) + 1u) & 0xFFFu;
-          const float2 gp = __ldg(g.calib + mod);
-          c4[j] = __fmaf_rn((float)(as[j] & 0xFFFFu), gp.x, gp.y);
-          if (mod + 1u > prev1) {
-            for (u32 m = prev1; m <= mod; ++m) ev.modDigiStart[m] = p0 + (u32)j;
-          } else if (mod + 1u < prev1) violation = 1;
-        }
-        ch = make_float4(c4[0], c4[1], c4[2], c4[3]);
-      }
-      *reinterpret_cast<uint2*>(ev.module + p0) = make_uint2((xs[1] >> 20) | (xs[2] >> 20) << 16, (xs[3] >> 20) | (xs[4] >> 20) << 16);
-      *reinterpret_cast<uint2*>(ev.row + p0) = make_uint2(((xs[1] >> 12) & 0xFFu) | ((xs[2] >> 12) & 0xFFu) << 16,
-                                                          ((xs[3] >> 12) & 0xFFu) | ((xs[4] >> 12) & 0xFFu) << 16);
-      *reinterpret_cast<uint2*>(ev.col + p0) = make_uint2(((xs[1] >> 3) & 0x1FFu) | ((xs[2] >> 3) & 0x1FFu) << 16,
-                                                          ((xs[3] >> 3) & 0x1FFu) | ((xs[4] >> 3) & 0x1FFu) << 16);
-      *reinterpret_cast<uint2*>(ev.adcOut + p0) = make_uint2(__byte_perm(as[0], as[1], 0x5410), __byte_perm(as[2], as[3], 0x5410));
-      *reinterpret_cast<uint4*>(ev.wordIdx + p0) = make_uint4(wordBase + (as[0] >> 16), wordBase + (as[1] >> 16),
-                                                              wordBase + (as[2] >> 16), wordBase + (as[3] >> 16));
-      *reinterpret_cast<float4*>(ev.charge + p0) = ch;
-    } else {                                              // the tile's first and last quad may be partial
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const u32 pos = 4u * q + (u32)j - ph;             // position in the tile (wraps below 0)
-        if (pos >= n) continue;
-        const u32 xx = st.x[stage_idx(pos + 4u)], aa = st.a[stage_idx(pos + 4u)];
-        const u32 xp = pos ? st.x[stage_idx(pos + 3u)] : fake;
-        const u32 mod = xx >> 20, prev1 = ((xp >> 20) + 1u) & 0xFFFu, p = p0 + (u32)j;
-        const float2 gp = __ldg(g.calib + mod);
-        ev.module[p] = (u16)mod; ev.row[p] = (u16)((xx >> 12) & 0xFFu); ev.col[p] = (u16)((xx >> 3) & 0x1FFu);
-        ev.adcOut[p] = (u16)(aa & 0xFFFFu); ev.wordIdx[p] = wordBase + (aa >> 16);
-        ev.charge[p] = __fmaf_rn((float)(aa & 0xFFFFu), gp.x, gp.y);
-        if (mod + 1u > prev1) {
-          for (u32 m = prev1; m <= mod; ++m) ev.modDigiStart[m] = p;
-        } else if (mod + 1u < prev1) violation = 1;
-      }
-    }
-  }
-  if (violation) atomicOr(&ev.counters->status, 1u);     // PR_STATUS_INPUT_ORDER (A5)
-  // ---- error words (A2-A4): staged behind the digis in word order; errors before the tile = words - digis before it
-  {
-    const u32 inRange = W > wordBase ? min(W - wordBase, (u32)kTileWords) : 0u, nErr = inRange - n, e0 = wordBase - g0;
-    for (u32 e = tid; e < nErr; e += kUnpackThreads) {
-      const u32 s = stage_idx(n + e + 4u);
-      ev.errWord[e0 + e] = st.x[s]; ev.errIdx[e0 + e] = wordBase + (st.a[s] >> 16);
-    }
-  }
-  // ---- the event's last tile closes modDigiStart and the counters
-  if (tile == ev.nTiles - 1u) {
-    const u32 D = g0 + n, mx1 = max(carry1, tileMax1);
-    for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) ev.modDigiStart[m] = D;
-    if (tid == 0) { ev.counters->nWords = W; ev.counters->nDigis = D; ev.counters->nErrors = W - D; }
-  }
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
+  u32 ok;
+  do {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void bulk_load(void* dstSmem, const void* srcGlobal, u32 bytes, u64* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dstSmem)), "l"(__cvta_generic_to_global(srcGlobal)), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dstGlobal, const void* srcSmem, u32 bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               ::"l"(__cvta_generic_to_global(dstGlobal)), "r"(smem_u32(srcSmem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads, 4)
+__global__ void __launch_bounds__(kUnpackThreads, 2)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
          u32 totalTiles, const __grid_constant__ Geom g) {
-  __shared__ __align__(16) UnpackShared sh;
-  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, G = gridDim.x;
-  u32 t = blockIdx.x;
-  if (t >= totalTiles) return;
-  u32 prv = 3, cur = 0, nxt = 1, nn = 2, eNN = 0;      // descriptor ring (batch)
-  if (!kSingle) {
-    if (warp < 2) {
-      const u32 tt = min(t + warp * G, totalTiles - 1u);
-      sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[tt]) + lane);
-      if (warp == 1 && t + 2u * G < totalTiles) eNN = tileEvent[t + 2u * G];
-    }
-    __syncthreads();
-  }
-  RawTile raw;
-  {
-    const EvDesc& ev = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[0]);
-    unpack_load(ev.words, ev.adc, ev.nWords, t - ev.tileBase, tid, raw);
-  }
+  extern __shared__ __align__(128) unsigned char unpackSmem[];
+  UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
+  const u32 first = blockIdx.x;
+  if (first >= totalTiles) return;
+  const int nLocal = (int)((totalTiles - first + G - 1u) / G);
   const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
-  bool haveA = true, haveB = false;
-  u32 pTile = 0, pN = 0, pMax1 = 0, pG0 = 0, pCarry1 = 0;          // the previous tile, for B
-
-  for (u32 it = 0;; ++it) {
-    const EvDesc& ev = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[cur]);
-    UnpackStage& st = sh.st[it & 1u];
-    u32 tile = 0, n = 0, tileMax1 = 0, dword = 0, eN3 = 0;
-    u32 x[8], ap[4], vmask = 0, packed = 0, incl = 0;
-    RawTile rawNext;
-    u64 lb[kLookBack];
-    if (haveA) {
-      tile = t - ev.tileBase;
-      // batch: descriptor of tile t + 2G and event of tile t + 3G, in flight until the end of the iteration
-      if (!kSingle && warp == 1) {
-        if (t + 2u * G < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(batch + eNN) + lane);
-        if (t + 3u * G < totalTiles) eN3 = tileEvent[t + 3u * G];
-      }
-      // ---- validity (A2, A3): digi iff module < M (bit 31 set makes it >= 2048), row < R, col < C
-      x[0] = raw.xa.x; x[1] = raw.xa.y; x[2] = raw.xa.z; x[3] = raw.xa.w; x[4] = raw.xb.x; x[5] = raw.xb.y; x[6] = raw.xb.z; x[7] = raw.xb.w;
-      ap[0] = raw.aa.x; ap[1] = raw.aa.y; ap[2] = raw.ab.x; ap[3] = raw.ab.y;
-      int mmax = -1;
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const u32 mod = x[j] >> 20;
-        const bool ok = mod < limM && (x[j] & 0xFF000u) < limR && (x[j] & 0xFF8u) < limC;
-        if (ok) { vmask |= 1u << j; mmax = max(mmax, (int)mod); }
-      }
-      packed = (u32)__popc(vmask & 15u) | (u32)__popc(vmask >> 4) << 16;
-      incl = warp_incl_scan(packed, (int)lane);
-      const u32 wmax1 = __reduce_max_sync(0xFFFFFFFFu, (u32)(mmax + 1));
-      if (lane == 31) sh.wagg[warp] = make_uint2(incl, wmax1);
+  auto desc_of = [&](int k) -> const EvDesc& {
+    return kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[k & (kDescRing - 1)]);
+  };
+  // ---- load of local tile k into its ring slot, by warp 0: TMA for the 16-byte multiple, lanes for the tail
+  auto issue_load = [&](int k) {
+    const EvDesc& e = desc_of(k);
+    const u32 T0 = (first + (u32)k * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+    const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)k % kRawSlots;
+    const u32 n4 = nIn & ~3u, n8 = nIn & ~7u;
+    if (lane == 0) {
+      mbar_expect_tx(&sh.full[slot], n4 * 4u + n8 * 2u);
+      if (n4) bulk_load(sh.words[slot], e.words + T0, n4 * 4u, &sh.full[slot]);
+      if (n8) bulk_load(sh.adc[slot], e.adc + T0, n8 * 2u, &sh.full[slot]);
     }
-    __syncthreads();                                                         // #1
-    if (haveA) {
-      u32 base = 0, tot = 0;
+    if (lane < nIn - n4) sh.words[slot][n4 + lane] = __ldcs(e.words + T0 + n4 + lane);
+    if (lane < nIn - n8) sh.adc[slot][n8 + lane] = __ldcs(e.adc + T0 + n8 + lane);
+  };
+
+  // ---- prologue: barriers, the first descriptors, the first loads
+  if (tid == 0) {
 #pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const uint2 s = sh.wagg[k];
-        if (k < (int)warp) base += s.x;
-        tot += s.x;
-        tileMax1 = max(tileMax1, s.y);
-      }
-      const u32 tileA = tot & 0xFFFFu;
-      n = tileA + (tot >> 16);
-      u64* state = ev.tileState;
-      if (tid == 0) st_state(state + tile, pack_state(tile ? kStAgg : kStIncl, n, tileMax1));
-      // ---- the next tile's loads are issued now and consumed in the next iteration
-      if (t + G < totalTiles) {
-        const EvDesc& en = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[nxt]);
-        unpack_load(en.words, en.adc, en.nWords, t + G - en.tileBase, tid, rawNext);
-      }
-      if (warp == 0 && tile) lookback_issue(state, (int)tile, lane, lb);
-      // ---- stage: digi k of the tile at slot 4 + k, error word e of the tile at slot 4 + n + e
-      const u32 ex = base + incl - packed;
-      u32 posA = ex & 0xFFFFu, posB = tileA + (ex >> 16);
+    for (int s = 0; s < kRawSlots; ++s) mbar_init(&sh.full[s], 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  u32 eNext = 0;                                               // batch, warp 1: event of local tile i + kRawSlots + 1
+  if (!kSingle) {
+    if ((int)warp <= kRawSlots && (int)warp < nLocal)
+      sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[first + warp * G]) + lane);
+    if (warp == 1 && kRawSlots + 1 < nLocal) eNext = tileEvent[first + (u32)(kRawSlots + 1) * G];
+  }
+  __syncthreads();
+  if (warp == 0)
+    for (int k = 0; k < kRawSlots && k < nLocal; ++k) issue_load(k);
+  __syncthreads();
+
+  for (int i = -kCountAhead; i < nLocal; ++i) {
+    // batch: descriptor of local tile i + kRawSlots + 1 in flight until the end of the iteration
+    u32 dword = 0, eN2 = 0;
+    const int kd = i + kRawSlots + 1;
+    if (!kSingle && warp == 1 && i >= 0) {
+      if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
+      if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
+    }
+    // ---- count: local tile i + kCountAhead
+    const int kc = i + kCountAhead;
+    if (kc < nLocal) {
+      const EvDesc& e = desc_of(kc);
+      const u32 T0 = (first + (u32)kc * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)kc % kRawSlots;
+      mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u);
+      const u32* wseg = sh.words[slot] + 256u * warp + lane;
+      u32 cnt = 0, mx = 0, myb = 0;
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        const u32 off = (j < 4 ? 0u : (u32)kTileWords / 2) + 4u * tid + (u32)(j & 3);
-        const u32 a16 = (j & 1) ? ap[j >> 1] >> 16 : ap[j >> 1] & 0xFFFFu;
-        u32& pos = j < 4 ? posA : posB;
-        u32 s;
-        if (vmask >> j & 1u) { s = 4u + pos; ++pos; }
-        else s = 4u + n + (off - pos);                    // words beyond W of a ragged tile land beyond the used slots
-        if (s < 4u + (u32)kTileWords) {
-          s = stage_idx(s);
-          st.x[s] = x[j]; st.a[s] = a16 | off << 16;
+        const u32 x = wseg[32 * j];
+        const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC && 256u * warp + 32u * j + lane < nIn;
+        const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
+        cnt += (u32)__popc(b);
+        if (ok) mx = max(mx, x);                               // a digi's word has bit 31 clear: max word = max module
+        if ((int)lane == j) myb = b;
+      }
+      if (lane < 8u) sh.bal[slot][warp][lane] = myb;
+      mx = __reduce_max_sync(0xFFFFFFFFu, mx);
+      if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
+    }
+    if (tid == 0 && i > 0) bulk_wait_read();                   // the staging arrays are free again
+    __syncthreads();                                                         // #1
+    // ---- warp 0: publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
+    const int kl = i + 1;
+    u32 tl = 0;
+    u64 lb[kLookBack];
+    if (warp == 0) {
+      if (kc < nLocal) {
+        const EvDesc& e = desc_of(kc);
+        const u32 tile = first + (u32)kc * G - e.tileBase, slot = (u32)kc % kRawSlots;
+        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+        const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
+        if (lane == 0) st_state(e.tileState + tile, pack_state(tile ? kStAgg : kStIncl, n, mx1));
+      }
+      if (kl >= 0 && kl < nLocal) {
+        const EvDesc& e = desc_of(kl);
+        tl = first + (u32)kl * G - e.tileBase;
+        if (tl) lookback_issue(e.tileState, (int)tl, lane, lb);
+      }
+    }
+    // ---- scatter: local tile i
+    if (i >= 0) {
+      const EvDesc& e = desc_of(i);
+      const u32 T0 = (first + (u32)i * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)i % kRawSlots;
+      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u;
+      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u;
+      const u32 wbase = __reduce_add_sync(0xFFFFFFFFu, lane < warp ? c8 : 0u);
+      const u32 myb = lane < 8u ? sh.bal[slot][warp][lane] : 0u;
+      const u32* wseg = sh.words[slot] + 256u * warp + lane;
+      const u16* aseg = sh.adc[slot] + 256u * warp + lane;
+      u32 ebase = 8u + ph + wbase;                             // staging element of the warp's next digi
+      const u32 wi0 = T0 + 256u * warp + lane;                 // event-local index of this lane's word of row 0
+      if (tid == 0) sh.sModule[8u + ph - 1u] = (u16)(sh.carry1[i & 1] - 1u);   // "the digi before the tile" (0xFFFF: none)
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const u32 b = __shfl_sync(0xFFFFFFFFu, myb, j);
+        const u32 x = wseg[32 * j], a = aseg[32 * j];
+        const u32 el = ebase + (u32)__popc(b & lt);
+        if (b >> lane & 1u) {
+          const u32 mod = x >> 20;
+          const float2 gp = __ldg(g.calib + mod);
+          sh.sModule[el] = (u16)mod; sh.sRow[el] = (u16)((x >> 12) & 0xFFu); sh.sCol[el] = (u16)((x >> 3) & 0x1FFu);
+          sh.sAdc[el] = (u16)a; sh.sWordIdx[el] = wi0 + 32u * j;
+          sh.sCharge[el] = __fmaf_rn((float)a, gp.x, gp.y);
+        } else if (256u * warp + 32u * j + lane < nIn) {
+          // error word (A2-A4): errors before it = words before it - digis before it
+          const u32 ei = (wi0 + 32u * j) - (g0 + (el - 8u - ph));
+          e.errWord[ei] = x; e.errIdx[ei] = wi0 + 32u * j;
+        }
+        ebase += (u32)__popc(b);
+      }
+    }
+    // ---- warp 0: resolve the look-back of tile i + 1 (its loads flew during the scatter)
+    if (warp == 0 && kl >= 0 && kl < nLocal) {
+      const EvDesc& e = desc_of(kl);
+      const u32 slot = (u32)kl % kRawSlots;
+      u32 c = 0, m = 0;
+      if (tl) {
+        lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m);
+        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+        const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
+        if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
+      }
+      if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
+    }
+    fence_async_smem();                                        // staged digis -> visible to the TMA store
+    __syncthreads();                                                         // #2
+    if (i >= 0) {
+      const EvDesc& e = desc_of(i);
+      const u32 tile = first + (u32)i * G - e.tileBase, slot = (u32)i % kRawSlots;
+      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
+      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
+      const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
+      const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
+      if (warp == 0) {
+        if (lane == 0) {
+          if (midHi > midLo) {
+            const u32 cnt = midHi - midLo, se = 8u + ph + (midLo - g0);
+            bulk_store(e.module + midLo, sh.sModule + se, cnt * 2u); bulk_store(e.row + midLo, sh.sRow + se, cnt * 2u);
+            bulk_store(e.col + midLo, sh.sCol + se, cnt * 2u); bulk_store(e.adcOut + midLo, sh.sAdc + se, cnt * 2u);
+            bulk_store(e.wordIdx + midLo, sh.sWordIdx + se, cnt * 4u); bulk_store(e.charge + midLo, sh.sCharge + se, cnt * 4u);
+          }
+          bulk_commit();
+        }
+        if (i + kRawSlots < nLocal) issue_load(i + kRawSlots);   // into the slot this tile vacated
+      } else if (warp == 1 && lane < 16u) {
+        // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
+        const u32 k = lane < 8u ? lane : n - 16u + lane;
+        const u32 p = g0 + k;
+        if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
+          const u32 se = 8u + ph + k;
+          e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
+          e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
         }
       }
-    }
-    if (haveB) {
-      const EvDesc& ep = kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[prv]);
-      unpack_write(ep, g, sh.st[(it & 1u) ^ 1u], tid, pTile, pN, pMax1, pG0, pCarry1);
-    }
-    if (haveA && warp == 0) {
-      u32 c = 0, m = 0;
-      if (tile) {
-        lookback_resolve(ev.tileState, (int)tile, lane, lb, &c, &m);
-        if (lane == 0) st_state(ev.tileState + tile, pack_state(kStIncl, c + n, max(m, tileMax1)));
+      // module boundaries (modDigiStart) and order violations (A5): digi at staging element idx vs the one before it
+      {
+        const u32 lo = 8u + ph, hi = lo + n;
+        u32 violation = 0;
+        for (u32 c = 1u + tid; 8u * c < hi; c += kUnpackThreads) {
+          const uint4 v = *reinterpret_cast<const uint4*>(sh.sModule + 8u * c);
+          const u32 prev = sh.sModule[8u * c - 1u];
+          const u32 rep = prev * 0x10001u;
+          if (((v.x ^ rep) | (v.y ^ rep) | (v.z ^ rep) | (v.w ^ rep)) == 0u) continue;   // eight digis of the module before them
+          const u32 w4[4] = {v.x, v.y, v.z, v.w};
+          u32 p = prev;
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const u32 m = (q & 1) ? w4[q >> 1] >> 16 : w4[q >> 1] & 0xFFFFu, idx = 8u * c + (u32)q;
+            if (idx >= lo && idx < hi && m != p) {
+              const u32 prev1 = (p + 1u) & 0xFFFFu;
+              if (m + 1u > prev1) {
+                for (u32 mm = prev1; mm <= m; ++mm) e.modDigiStart[mm] = g0 + (idx - lo);
+              } else violation = 1;
+            }
+            p = m;
+          }
+        }
+        if (violation) atomicOr(&e.counters->status, 1u);      // PR_STATUS_INPUT_ORDER (A5)
       }
-      if (lane == 0) { sh.g0 = c; sh.carry1 = m; }
+      // the event's last tile closes modDigiStart and the counters
+      if (tile == e.nTiles - 1u) {
+        const u32 D = g0 + n, mx1 = max(carry1, tileMax1), W = e.nWords;
+        for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) e.modDigiStart[m] = D;
+        if (tid == 0) { e.counters->nWords = W; e.counters->nDigis = D; e.counters->nErrors = W - D; }
+      }
     }
-    __syncthreads();                                                         // #2
-    if (!haveA) break;
-    haveB = true; pTile = tile; pN = n; pMax1 = tileMax1; pG0 = sh.g0; pCarry1 = sh.carry1;
-    if (!kSingle && warp == 1) { sh.desc[nn][lane] = dword; eNN = eN3; }
-    t += G; haveA = t < totalTiles; raw = rawNext;
-    const u32 r = prv; prv = cur; cur = nxt; nxt = nn; nn = r;
+    if (!kSingle && warp == 1 && i >= 0) {
+      if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
+      eNext = eN2;
+    }
   }
+  if (tid == 0) bulk_wait_all();
 }
 
 // ================================================================== k_cluster (a3 + a4)
