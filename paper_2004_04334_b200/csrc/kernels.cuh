@@ -194,6 +194,7 @@ __device__ __forceinline__ void lookback_resolve(const u64* state, int self, u32
 //           arrays; sixteen lanes store the up-to-7 head and tail elements; all threads scan the
 //           staged module array for module boundaries (modDigiStart) and order violations (A5)
 // Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
+constexpr int kUnpackCtasPerSM = 2;
 constexpr int kRawSlots = 4;                      // raw tiles in the shared-memory ring
 constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
 constexpr int kDescRing = 8;                      // descriptor ring (batch), power of two >= kRawSlots + 2
@@ -242,12 +243,13 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads, 2)
+__global__ void __launch_bounds__(kUnpackThreads + 32, kUnpackCtasPerSM)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
          u32 totalTiles, const __grid_constant__ Geom g) {
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
+  const bool ctl = warp == 8u;                               // warps 0..7 work on words; warp 8 publishes, looks back, drives the TMA
   const u32 first = blockIdx.x;
   if (first >= totalTiles) return;
   const int nLocal = (int)((totalTiles - first + G - 1u) / G);
@@ -255,7 +257,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   auto desc_of = [&](int k) -> const EvDesc& {
     return kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[k & (kDescRing - 1)]);
   };
-  // ---- load of local tile k into its ring slot, by warp 0: TMA for the 16-byte multiple, lanes for the tail
+  // ---- load of local tile k into its ring slot, by the control warp: TMA for the 16-byte multiple, lanes for the tail
   auto issue_load = [&](int k) {
     const EvDesc& e = desc_of(k);
     const u32 T0 = (first + (u32)k * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
@@ -276,28 +278,30 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     for (int s = 0; s < kRawSlots; ++s) mbar_init(&sh.full[s], 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  u32 eNext = 0;                                               // batch, warp 1: event of local tile i + kRawSlots + 1
+  u32 eNext = 0;                                               // batch, control warp: event of local tile i + kRawSlots + 1
   if (!kSingle) {
     if ((int)warp <= kRawSlots && (int)warp < nLocal)
       sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[first + warp * G]) + lane);
-    if (warp == 1 && kRawSlots + 1 < nLocal) eNext = tileEvent[first + (u32)(kRawSlots + 1) * G];
+    if (ctl && kRawSlots + 1 < nLocal) eNext = tileEvent[first + (u32)(kRawSlots + 1) * G];
   }
   __syncthreads();
-  if (warp == 0)
+  if (ctl)
     for (int k = 0; k < kRawSlots && k < nLocal; ++k) issue_load(k);
   __syncthreads();
 
   for (int i = -kCountAhead; i < nLocal; ++i) {
-    // batch: descriptor of local tile i + kRawSlots + 1 in flight until the end of the iteration
-    u32 dword = 0, eN2 = 0;
-    const int kd = i + kRawSlots + 1;
-    if (!kSingle && warp == 1 && i >= 0) {
-      if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
-      if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
-    }
-    // ---- count: local tile i + kCountAhead
-    const int kc = i + kCountAhead;
-    if (kc < nLocal) {
+    const int kc = i + kCountAhead, kl = i + 1, kd = i + kRawSlots + 1;
+    u32 dword = 0, eN2 = 0, tl = 0;
+    u64 lb[kLookBack];
+    if (ctl) {
+      // batch: descriptor of local tile i + kRawSlots + 1 in flight until the end of the iteration
+      if (!kSingle && i >= 0) {
+        if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
+        if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
+      }
+      if (lane == 0 && i > 0) bulk_wait_read();                // the staging arrays are free again
+    } else if (kc < nLocal) {
+      // ---- count: local tile i + kCountAhead
       const EvDesc& e = desc_of(kc);
       const u32 T0 = (first + (u32)kc * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
       const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)kc % kRawSlots;
@@ -317,13 +321,9 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       mx = __reduce_max_sync(0xFFFFFFFFu, mx);
       if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
     }
-    if (tid == 0 && i > 0) bulk_wait_read();                   // the staging arrays are free again
     __syncthreads();                                                         // #1
-    // ---- warp 0: publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
-    const int kl = i + 1;
-    u32 tl = 0;
-    u64 lb[kLookBack];
-    if (warp == 0) {
+    if (ctl) {
+      // ---- publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
       if (kc < nLocal) {
         const EvDesc& e = desc_of(kc);
         const u32 tile = first + (u32)kc * G - e.tileBase, slot = (u32)kc % kRawSlots;
@@ -336,9 +336,8 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         tl = first + (u32)kl * G - e.tileBase;
         if (tl) lookback_issue(e.tileState, (int)tl, lane, lb);
       }
-    }
-    // ---- scatter: local tile i
-    if (i >= 0) {
+    } else if (i >= 0) {
+      // ---- scatter: local tile i
       const EvDesc& e = desc_of(i);
       const u32 T0 = (first + (u32)i * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
       const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)i % kRawSlots;
@@ -350,7 +349,10 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       const u16* aseg = sh.adc[slot] + 256u * warp + lane;
       u32 ebase = 8u + ph + wbase;                             // staging element of the warp's next digi
       const u32 wi0 = T0 + 256u * warp + lane;                 // event-local index of this lane's word of row 0
-      if (tid == 0) sh.sModule[8u + ph - 1u] = (u16)(sh.carry1[i & 1] - 1u);   // "the digi before the tile" (0xFFFF: none)
+      if (tid == 0) {                                          // "the digi before the tile" for the order check (module 0 if none)
+        const u32 c1 = sh.carry1[i & 1];
+        sh.sModule[8u + ph - 1u] = (u16)(c1 ? c1 - 1u : 0u);
+      }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const u32 b = __shfl_sync(0xFFFFFFFFu, myb, j);
@@ -369,30 +371,15 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         }
         ebase += (u32)__popc(b);
       }
+      fence_async_smem();                                      // staged digis -> visible to the TMA store
     }
-    // ---- warp 0: resolve the look-back of tile i + 1 (its loads flew during the scatter)
-    if (warp == 0 && kl >= 0 && kl < nLocal) {
-      const EvDesc& e = desc_of(kl);
-      const u32 slot = (u32)kl % kRawSlots;
-      u32 c = 0, m = 0;
-      if (tl) {
-        lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m);
-        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
-        const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
-        if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
-      }
-      if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
-    }
-    fence_async_smem();                                        // staged digis -> visible to the TMA store
     __syncthreads();                                                         // #2
-    if (i >= 0) {
-      const EvDesc& e = desc_of(i);
-      const u32 tile = first + (u32)i * G - e.tileBase, slot = (u32)i % kRawSlots;
-      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
-      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
-      const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
-      const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
-      if (warp == 0) {
+    if (ctl) {
+      if (i >= 0) {
+        const EvDesc& e = desc_of(i);
+        const u32 slot = (u32)i % kRawSlots, g0 = sh.g0[i & 1], ph = g0 & 7u;
+        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+        const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
         if (lane == 0) {
           if (midHi > midLo) {
             const u32 cnt = midHi - midLo, se = 8u + ph + (midLo - g0);
@@ -403,40 +390,77 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
           bulk_commit();
         }
         if (i + kRawSlots < nLocal) issue_load(i + kRawSlots);   // into the slot this tile vacated
-      } else if (warp == 1 && lane < 16u) {
+      }
+      // ---- resolve the look-back of tile i + 1 (its loads flew during the scatter), publish its inclusive state
+      if (kl >= 0 && kl < nLocal) {
+        const EvDesc& e = desc_of(kl);
+        const u32 slot = (u32)kl % kRawSlots;
+        u32 c = 0, m = 0;
+        if (tl) {
+          lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m);
+          const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+          const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
+          if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
+        }
+        if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
+      }
+      if (!kSingle && i >= 0) {
+        if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
+        eNext = eN2;
+      }
+    } else if (i >= 0) {
+      const EvDesc& e = desc_of(i);
+      const u32 tile = first + (u32)i * G - e.tileBase, slot = (u32)i % kRawSlots;
+      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
+      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
+      const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
+      const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
+      const u32 lo = 8u + ph, hi = lo + n;
+      if (warp == 7u && lane < 16u) {
         // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
         const u32 k = lane < 8u ? lane : n - 16u + lane;
         const u32 p = g0 + k;
         if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
-          const u32 se = 8u + ph + k;
+          const u32 se = lo + k;
           e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
           e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
         }
       }
-      // module boundaries (modDigiStart) and order violations (A5): digi at staging element idx vs the one before it
+      // order check (A5): no digi's module is below that of the digi before it.  Eight digis per thread;
+      // per halfword, bit 15 of (m | 0x8000) - p stays set iff m >= p (modules are below 2^11).
       {
-        const u32 lo = 8u + ph, hi = lo + n;
-        u32 violation = 0;
+        u32 bad = 0;
         for (u32 c = 1u + tid; 8u * c < hi; c += kUnpackThreads) {
           const uint4 v = *reinterpret_cast<const uint4*>(sh.sModule + 8u * c);
           const u32 prev = sh.sModule[8u * c - 1u];
-          const u32 rep = prev * 0x10001u;
-          if (((v.x ^ rep) | (v.y ^ rep) | (v.z ^ rep) | (v.w ^ rep)) == 0u) continue;   // eight digis of the module before them
-          const u32 w4[4] = {v.x, v.y, v.z, v.w};
-          u32 p = prev;
+          if (8u * c >= lo && 8u * c + 8u <= hi) {
+            const u32 s0 = v.x << 16 | prev, s1 = __funnelshift_l(v.x, v.y, 16), s2 = __funnelshift_l(v.y, v.z, 16), s3 = __funnelshift_l(v.z, v.w, 16);
+            const u32 t = ((v.x | 0x80008000u) - s0) & ((v.y | 0x80008000u) - s1) & ((v.z | 0x80008000u) - s2) & ((v.w | 0x80008000u) - s3);
+            bad |= ~t & 0x80008000u;
+          } else {                                             // the tile's first and last chunk may be partial
+            const u32 w4[4] = {v.x, v.y, v.z, v.w};
+            u32 p = prev;
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            const u32 m = (q & 1) ? w4[q >> 1] >> 16 : w4[q >> 1] & 0xFFFFu, idx = 8u * c + (u32)q;
-            if (idx >= lo && idx < hi && m != p) {
-              const u32 prev1 = (p + 1u) & 0xFFFFu;
-              if (m + 1u > prev1) {
-                for (u32 mm = prev1; mm <= m; ++mm) e.modDigiStart[mm] = g0 + (idx - lo);
-              } else violation = 1;
+            for (int q = 0; q < 8; ++q) {
+              const u32 m = (q & 1) ? w4[q >> 1] >> 16 : w4[q >> 1] & 0xFFFFu, idx = 8u * c + (u32)q;
+              if (idx >= lo && idx < hi && m < p) bad = 1u;
+              p = m;
             }
-            p = m;
           }
         }
-        if (violation) atomicOr(&e.counters->status, 1u);      // PR_STATUS_INPUT_ORDER (A5)
+        if (bad) atomicOr(&e.counters->status, 1u);            // PR_STATUS_INPUT_ORDER
+      }
+      // modDigiStart[m] for the modules that begin in this tile (or are skipped by it): first staged digi
+      // with module >= m, by binary search (the staged modules ascend unless the order check fired)
+      if (n) {
+        const u32 mLast = sh.sModule[hi - 1u];
+        for (u32 m = carry1 + tid; m <= mLast; m += kUnpackThreads) {
+          u32 pos = 0;
+#pragma unroll
+          for (u32 step = (u32)kTileWords; step; step >>= 1)
+            if (pos + step <= n && sh.sModule[lo + pos + step - 1u] < m) pos += step;
+          e.modDigiStart[m] = g0 + pos;
+        }
       }
       // the event's last tile closes modDigiStart and the counters
       if (tile == e.nTiles - 1u) {
@@ -445,12 +469,8 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         if (tid == 0) { e.counters->nWords = W; e.counters->nDigis = D; e.counters->nErrors = W - D; }
       }
     }
-    if (!kSingle && warp == 1 && i >= 0) {
-      if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
-      eNext = eN2;
-    }
   }
-  if (tid == 0) bulk_wait_all();
+  if (ctl && lane == 0) bulk_wait_all();
 }
 
 // ================================================================== k_cluster (a3 + a4)
