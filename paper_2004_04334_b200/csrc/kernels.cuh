@@ -242,16 +242,28 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+#ifdef PIXRECO_TRACE
+__device__ unsigned long long g_trace[1024 * 32];
+#define TR_T(v) long long v; asm volatile("mov.u64 %0, %%clock64;" : "=l"(v) :: "memory")
+#define TR_ADD(slot, t0) do { long long t1_; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1_) :: "memory"); trAcc[slot] += (unsigned long long)(t1_ - (t0)); } while (0)
+#else
+#define TR_T(v)
+#define TR_ADD(slot, t0)
+#endif
 template <bool kSingle>
-__global__ void __launch_bounds__(kUnpackThreads + 32, kUnpackCtasPerSM)
+__global__ void __launch_bounds__(kUnpackThreads + 64, kUnpackCtasPerSM)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
          u32 totalTiles, const __grid_constant__ Geom g) {
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
-  const bool ctl = warp == 8u;                               // warps 0..7 work on words; warp 8 publishes, looks back, drives the TMA
+  const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA; warp 9 publishes and looks back
   const u32 first = blockIdx.x;
   if (first >= totalTiles) return;
+#ifdef PIXRECO_TRACE
+  unsigned long long trAcc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long trStart = clock64();
+#endif
   const int nLocal = (int)((totalTiles - first + G - 1u) / G);
   const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
   auto desc_of = [&](int k) -> const EvDesc& {
@@ -299,13 +311,13 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
         if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
       }
-      if (lane == 0 && i > 0) bulk_wait_read();                // the staging arrays are free again
-    } else if (kc < nLocal) {
+      { TR_T(t0); if (lane == 0 && i > 0) bulk_wait_read(); TR_ADD(0, t0); }   // the staging arrays are free again
+    } else if (!scn && kc < nLocal) {
       // ---- count: local tile i + kCountAhead
       const EvDesc& e = desc_of(kc);
       const u32 T0 = (first + (u32)kc * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
       const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)kc % kRawSlots;
-      mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u);
+      { TR_T(t0); mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u); if (warp == 0) TR_ADD(1, t0); }
       const u32* wseg = sh.words[slot] + 256u * warp + lane;
       u32 cnt = 0, mx = 0, myb = 0;
 #pragma unroll
@@ -321,8 +333,8 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       mx = __reduce_max_sync(0xFFFFFFFFu, mx);
       if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
     }
-    __syncthreads();                                                         // #1
-    if (ctl) {
+    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(2, t0); }                                                         // #1
+    if (scn) {
       // ---- publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
       if (kc < nLocal) {
         const EvDesc& e = desc_of(kc);
@@ -336,7 +348,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         tl = first + (u32)kl * G - e.tileBase;
         if (tl) lookback_issue(e.tileState, (int)tl, lane, lb);
       }
-    } else if (i >= 0) {
+    } else if (!ctl && i >= 0) {
       // ---- scatter: local tile i
       const EvDesc& e = desc_of(i);
       const u32 T0 = (first + (u32)i * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
@@ -373,7 +385,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       }
       fence_async_smem();                                      // staged digis -> visible to the TMA store
     }
-    __syncthreads();                                                         // #2
+    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(3, t0); }                                                         // #2
     if (ctl) {
       if (i >= 0) {
         const EvDesc& e = desc_of(i);
@@ -390,23 +402,33 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
           bulk_commit();
         }
         if (i + kRawSlots < nLocal) issue_load(i + kRawSlots);   // into the slot this tile vacated
+        if (lane < 16u) {
+          // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
+          const u32 lo = 8u + ph, k = lane < 8u ? lane : n - 16u + lane, p = g0 + k;
+          if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
+            const u32 se = lo + k;
+            e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
+            e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
+          }
+        }
       }
+      if (!kSingle && i >= 0) {
+        if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
+        eNext = eN2;
+      }
+    } else if (scn) {
       // ---- resolve the look-back of tile i + 1 (its loads flew during the scatter), publish its inclusive state
       if (kl >= 0 && kl < nLocal) {
         const EvDesc& e = desc_of(kl);
         const u32 slot = (u32)kl % kRawSlots;
         u32 c = 0, m = 0;
         if (tl) {
-          lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m);
+          { TR_T(t0); lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m); TR_ADD(6, t0); }
           const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
           const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
           if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
         }
         if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
-      }
-      if (!kSingle && i >= 0) {
-        if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
-        eNext = eN2;
       }
     } else if (i >= 0) {
       const EvDesc& e = desc_of(i);
@@ -414,18 +436,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
       const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
       const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
-      const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
       const u32 lo = 8u + ph, hi = lo + n;
-      if (warp == 7u && lane < 16u) {
-        // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
-        const u32 k = lane < 8u ? lane : n - 16u + lane;
-        const u32 p = g0 + k;
-        if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
-          const u32 se = lo + k;
-          e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
-          e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
-        }
-      }
       // order check (A5): no digi's module is below that of the digi before it.  Eight digis per thread;
       // per halfword, bit 15 of (m | 0x8000) - p stays set iff m >= p (modules are below 2^11).
       {
@@ -450,15 +461,34 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         }
         if (bad) atomicOr(&e.counters->status, 1u);            // PR_STATUS_INPUT_ORDER
       }
-      // modDigiStart[m] for the modules that begin in this tile (or are skipped by it): first staged digi
-      // with module >= m, by binary search (the staged modules ascend unless the order check fired)
+      // modDigiStart[m] for the modules that begin in this tile (or are skipped by it): the number of staged
+      // digis with module < m (the staged modules ascend unless the order check fired).  First the warp
+      // segments that lie entirely below m (wmax <= m), then a 4-ary search inside the first one that
+      // does not.  Module carry1 + 8 * lane + warp goes to this thread: every warp gets its share.
       if (n) {
         const u32 mLast = sh.sModule[hi - 1u];
-        for (u32 m = carry1 + tid; m <= mLast; m += kUnpackThreads) {
-          u32 pos = 0;
+        u32 sc[8], sm[8];
 #pragma unroll
-          for (u32 step = (u32)kTileWords; step; step >>= 1)
-            if (pos + step <= n && sh.sModule[lo + pos + step - 1u] < m) pos += step;
+        for (int w = 0; w < 8; ++w) { sc[w] = __shfl_sync(0xFFFFFFFFu, c8, w); sm[w] = __shfl_sync(0xFFFFFFFFu, m8, w); }
+        for (u32 m = carry1 + 8u * lane + warp; m <= mLast; m += kUnpackThreads) {
+          u32 pos = 0, len = 0;
+          bool open = true;
+#pragma unroll
+          for (int w = 0; w < 8; ++w) {
+            if (open && sm[w] <= m) pos += sc[w];
+            else if (open) { open = false; len = sc[w]; }
+          }
+          // invariant: digis [0, pos) are < m, digi pos + len (if inside the segment) is >= m
+          const u16* base = sh.sModule + lo;
+#pragma unroll
+          for (u32 q = 64u; q; q >>= 2) {                      // len <= 256: quarters of 64, 16, 4, 1
+            u32 adv = 0;
+#pragma unroll
+            for (u32 r = 1; r <= 3u; ++r)
+              if (r * q <= len && base[pos + r * q - 1u] < m) adv = r;
+            pos += adv * q;
+            len = min(len - adv * q, q);
+          }
           e.modDigiStart[m] = g0 + pos;
         }
       }
@@ -471,6 +501,15 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     }
   }
   if (ctl && lane == 0) bulk_wait_all();
+#ifdef PIXRECO_TRACE
+  if (lane == 0 && blockIdx.x < 1024) {
+    unsigned long long* o = g_trace + blockIdx.x * 32;
+    o[warp * 2] = trAcc[2]; o[warp * 2 + 1] = trAcc[3];
+    if (ctl) { o[20] = trAcc[0]; o[22] = (unsigned long long)(clock64() - trStart); }
+    if (scn) o[21] = trAcc[6];
+    if (warp == 0) o[23] = trAcc[1];
+  }
+#endif
 }
 
 // ================================================================== k_cluster (a3 + a4)

@@ -282,7 +282,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<unpackGrid, kUnpackThreads + 32, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
+    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -297,7 +297,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, descBytes, cudaMemcpyHostToDevice, stream));
     ++nMemcpy;
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<unpackGrid, kUnpackThreads + 32, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
+    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -484,7 +484,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     cudaGetLastError(); return fail(PR_ERR_CUDA);
   }
   int ups = 1;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ups, k_unpack<false>, kUnpackThreads + 32, sizeof(UnpackShared)) != cudaSuccess) { cudaGetLastError(); ups = 1; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ups, k_unpack<false>, kUnpackThreads + 64, sizeof(UnpackShared)) != cudaSuccess) { cudaGetLastError(); ups = 1; }
   h->unpackBlocksPerSM = ups < 1 ? 1 : ups;
   h->devPool = new CachingPool(make_device_backend(cfg->device), cfg->max_cached_bytes_device);
   h->hostPool = new CachingPool(make_pinned_backend(cfg->device), cfg->max_cached_bytes_host);
@@ -629,5 +629,13 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
   }
   return PR_OK;
 }
+
+#ifdef PIXRECO_TRACE
+int pr_debug_trace(unsigned long long* out, int n, int reset) {
+  if (out && cudaMemcpyFromSymbol(out, g_trace, sizeof(unsigned long long) * n) != cudaSuccess) return -1;
+  if (reset) { static unsigned long long z[1024 * 32]; cudaMemcpyToSymbol(g_trace, z, sizeof z); }
+  return 0;
+}
+#endif
 
 }  // extern "C"
