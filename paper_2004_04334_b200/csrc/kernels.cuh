@@ -73,6 +73,7 @@ struct EvDesc {
   u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
   HostCounters* hostCounters;
   u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
+  u32* grpCount;                    // [ceil(M / 32)] the same summed over groups of kFinMods modules (zeroed per acquire)
   // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
   double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
 };
@@ -1025,6 +1026,7 @@ __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 
   }
   if (tid == 0) {
     ev.modCount[m] = cx.nKept;
+    if (cx.nKept) atomicAdd(&ev.grpCount[m / 32u], cx.nKept);
     if (cx.nAll) atomicAdd(&ev.counters->nClustersAll, cx.nAll);
   }
 }
@@ -1080,7 +1082,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     const EvDesc& ev = kSingle ? single : batch[e];
     if (ev.counters->status & 1u) continue;
     const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
-    u32 accK = 0, accA = 0;
+    u32 accK = 0, accA = 0, accG = 0;
     for (u32 k = 0; k < nm; ++k) {
       const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
       u32 cnt = 0;
@@ -1097,7 +1099,9 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         }
       }
       if (lane == 0) ev.modCount[m0 + k] = cnt;
+      accG += cnt;
     }
+    if (lane == 0 && accG) atomicAdd(&ev.grpCount[m0 / 32u], accG);     // kModBatch divides 32: one group per ticket
     if (lane == 0) {
       if (accK) atomicAdd(&ev.counters->nKept, accK);
       if (accA) atomicAdd(&ev.counters->nClustersAll, accA);
@@ -1110,20 +1114,21 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
 // number is the sum of the kept-cluster counts of all earlier modules (at most 2048 values), so
 // no CTA depends on another.  Turns clus[] ranks into event-wide cluster numbers, converts the
 // staged sums into the cluster SoA (A9: binary64 division, one rounding to binary32), writes
-// modClusStart[]; the launch's last CTA publishes all counters to mapped pinned host memory.
+// modClusStart[]; the CTA of an event's last module group publishes that event's counters to mapped pinned host memory.
 constexpr u32 kFinMods = 32;
+static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
 template <bool kSingle>
 __global__ void __launch_bounds__(256)
 k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent,
            LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
-  __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8], sLast;
+  __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8];
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
   const u32 e = blockIdx.x / unitsPerEvent, u = blockIdx.x - e * unitsPerEvent;
   const EvDesc& ev = kSingle ? single : batch[e];
   const u32 m0 = u * kFinMods, m1 = min(m0 + kFinMods, M);
   if (!(ev.counters->status & 1u)) {
     u32 sum = 0, base;
-    for (u32 m = tid; m < m0; m += 256) sum += ev.modCount[m];
+    for (u32 k = tid; k < u; k += 256) sum += ev.grpCount[k];      // groups of kFinMods modules before this one
     block_excl_scan(sum, sScan, &base);
     if (warp == 0) {
       const u32 c = m0 + lane < m1 ? ev.modCount[m0 + lane] : 0u;
@@ -1138,9 +1143,17 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
     const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
     if (d0 <= d1 && d1 <= ev.cap) {
-      for (u32 d = d0 + tid; d < d1; d += 256) {
-        const int32_t c = ev.clus[d];
-        if (c >= 0) ev.clus[d] = (int32_t)(sStart[min((u32)ev.module[d] - m0, kFinMods - 1)] + (u32)c);
+      for (u32 dd = d0 + tid; dd < d1; dd += 4u * 256u) {     // four independent digis per thread and trip
+        int32_t c[4]; u32 md[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const u32 d = dd + 256u * k;
+          c[k] = d < d1 ? ev.clus[d] : -1;
+          md[k] = d < d1 ? (u32)ev.module[d] : m0;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (c[k] >= 0) ev.clus[dd + 256u * k] = (int32_t)(sStart[min(md[k] - m0, kFinMods - 1)] + (u32)c[k]);
       }
       for (u32 o = sStart[0] + tid; o < sStart[32]; o += 256) {
         u32 li = 0;
@@ -1158,22 +1171,15 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
       }
     }
   }
-  __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    sLast = (atomicAdd(&lc->modDone, 1u) == gridDim.x - 1);
-  }
-  __syncthreads();
-  if (sLast) {
-    __threadfence();
-    for (u32 k = tid; k < nEv; k += 256) {
-      const EvDesc& d = kSingle ? single : batch[k];
-      const volatile DevCounters* c = d.counters;
-      HostCounters h;
-      h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
-      h.nClustersAll = c->nClustersAll; h.nClusters = c->nClusters; h.status = c->status; h.seq = 1;
-      *d.hostCounters = h;
-    }
+  // The CTA of the event's last module group publishes the event's counters to mapped pinned host memory: all
+  // the others were final when this kernel started, nClusters is this CTA's own result.
+  if (m1 == M && tid == 0) {
+    const DevCounters* c = ev.counters;
+    const u32 status = c->status;
+    HostCounters h;
+    h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
+    h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[32]; h.status = status; h.seq = 1;
+    *ev.hostCounters = h;
   }
 }
 

@@ -203,7 +203,8 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
     totalTiles += s.desc.nTiles;
   }
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles;
+  const size_t grpPerEv = align_up((M + 31) / 32, 16);      // u32 per event
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + 4 * grpPerEv * n;
 
   // ---- buffers from the pools (steady state: cache hits only)
   if (ev->ctlBytes < ctlNeed) {
@@ -249,6 +250,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
     d.tileState = tileState + d.tileBase;
+    d.grpCount = (u32*)(tileState + totalTiles) + grpPerEv * k;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
@@ -496,7 +498,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles;
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + 4 * align_up((g.M + 31) / 32, 16);
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
