@@ -62,7 +62,7 @@ struct pr_event {
   uint32_t n = 0;
   std::vector<SubEvent> sub;
   // per-acquire pool blocks
-  void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr; void* itemTab = nullptr;
+  void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr;
   // persistent per-slot blocks (grown on demand)
   void* ctl = nullptr; size_t ctlBytes = 0;
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
@@ -156,7 +156,6 @@ void release_blocks(pr_event* ev, bool completed) {
   if (ev->descDev) { h->devPool->free(ev->descDev, ev->stream, completed); ev->descDev = nullptr; }
   if (ev->hostSlab) { h->hostPool->free(ev->hostSlab, ev->stream, completed); ev->hostSlab = nullptr; }
   if (ev->descStage) { h->hostPool->free(ev->descStage, ev->stream, completed); ev->descStage = nullptr; }
-  if (ev->itemTab) { h->hostPool->free(ev->itemTab, ev->stream, completed); ev->itemTab = nullptr; }
 }
 
 int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
@@ -187,16 +186,34 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const bool stage = kind == PR_MEM_HOST_PINNED;
 
+  // ---- host inputs of a batch that form one nearly dense span per array (a DAQ buffer, the bench's pool) are staged
+  // by ONE copy per array, each event keeping its offset inside the span; otherwise one copy per event and array
+  uintptr_t wLo = ~(uintptr_t)0, wHi = 0, aLo = ~(uintptr_t)0, aHi = 0;
+  bool merged = false;
+  if (stage && n > 1) {
+    size_t wSum = 0, aSum = 0;
+    for (uint32_t k = 0; k < n; ++k) {
+      if (!ins[k].n_words) continue;
+      const uintptr_t w = (uintptr_t)ins[k].words, a = (uintptr_t)ins[k].adc;
+      wLo = w < wLo ? w : wLo; wHi = w + 4 * (size_t)ins[k].n_words > wHi ? w + 4 * (size_t)ins[k].n_words : wHi;
+      aLo = a < aLo ? a : aLo; aHi = a + 2 * (size_t)ins[k].n_words > aHi ? a + 2 * (size_t)ins[k].n_words : aHi;
+      wSum += 4 * (size_t)ins[k].n_words; aSum += 2 * (size_t)ins[k].n_words;
+    }
+    merged = wSum > 0 && wHi - wLo <= wSum + wSum / 4 + 4096 && aHi - aLo <= aSum + aSum / 4 + 4096;
+    for (uint32_t k = 0; merged && k < n; ++k)
+      if (ins[k].n_words && ((((uintptr_t)ins[k].words - wLo) | ((uintptr_t)ins[k].adc - aLo)) & 15u)) merged = false;   // TMA wants 16-byte alignment
+  }
+
   // ---- layout
   ev->sub.assign(n, SubEvent());
-  size_t devBytes = 0, hostBytes = 0;
+  size_t devBytes = merged ? align_up(wHi - wLo, 256) + align_up(aHi - aLo, 256) : 0, hostBytes = 0;
   uint32_t totalTiles = 0;
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     s.in = ins[k];
     s.cap = (uint32_t)align_up(s.in.n_words ? s.in.n_words : 1, 8);
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
-    carve_device(cd, tmp, s.cap, M, stage, &sw, &sa);
+    carve_device(cd, tmp, s.cap, M, stage && !merged, &sw, &sa);
     devBytes += cd.off;
     if (want) { Carver ch(nullptr); pr_output o{}; carve_host(ch, o, want, s.cap, M); hostBytes += ch.off; }
     s.desc.tileBase = totalTiles;
@@ -224,11 +241,12 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (!ev->devSlab) return PR_ERR_OOM;
   if (want) {
     ev->hostSlab = h->hostPool->alloc(hostBytes, stream);
-    ev->itemTab = h->hostPool->alloc(sizeof(ExportItem) * 18 * n, stream);   // export table (mapped pinned)
-    if (!ev->hostSlab || !ev->itemTab) { release_blocks(ev, true); return PR_ERR_OOM; }
+    if (!ev->hostSlab) { release_blocks(ev, true); return PR_ERR_OOM; }
   }
-  const size_t descBytes = sizeof(EvDesc) * n + sizeof(u16) * totalTiles;   // descriptors, then the tile -> event map
-  if (n > 1) {
+  // one block, one H2D copy: event descriptors and the tile -> event map (batches), then the export table (mirrors)
+  const size_t descPart = n > 1 ? align_up(sizeof(EvDesc) * n + sizeof(u16) * totalTiles, 16) : 0;
+  const size_t descBytes = descPart + (want ? sizeof(ExportItem) * 18 * n : 0);
+  if (descBytes) {
     ev->descStage = h->hostPool->alloc(descBytes, stream);
     ev->descDev = h->devPool->alloc(descBytes, stream);
     if (!ev->descStage || !ev->descDev) { release_blocks(ev, true); return PR_ERR_OOM; }
@@ -241,10 +259,15 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
+  char *spanW = nullptr, *spanA = nullptr;
+  if (merged) { spanW = cd.take<char>(wHi - wLo); spanA = cd.take<char>(aHi - aLo); }
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     EvDesc& d = s.desc;
-    carve_device(cd, d, s.cap, M, stage, &stW[k], &stA[k]);
+    carve_device(cd, d, s.cap, M, stage && !merged, &stW[k], &stA[k]);
+    if (merged && s.in.n_words) {
+      stW[k] = (uint32_t*)(spanW + ((uintptr_t)s.in.words - wLo)); stA[k] = (uint16_t*)(spanA + ((uintptr_t)s.in.adc - aLo));
+    }
     d.words = stage ? stW[k] : s.in.words;
     d.adc = stage ? stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
@@ -259,7 +282,11 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // ---- enqueue (all asynchronous, one stream: P:L82)
   uint64_t nMemcpy = 0, nLaunch = 0;
   PR_CUDA(h, cudaMemsetAsync(ev->ctl, 0, ctlNeed, stream));
-  if (stage)
+  if (merged) {
+    PR_CUDA(h, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
+    PR_CUDA(h, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
+    nMemcpy += 2;
+  } else if (stage)
     for (uint32_t k = 0; k < n; ++k) {
       const SubEvent& s = ev->sub[k];
       if (!s.in.n_words) continue;
@@ -281,37 +308,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // waits on earlier tiles, which must therefore be running or done)
   uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
   if (unpackGrid > totalTiles) unpackGrid = totalTiles;
-  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
-  if (n == 1) {
-    const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
-  } else {
-    EvDesc* st = (EvDesc*)ev->descStage;
-    u16* te = (u16*)(st + n);
-    for (uint32_t k = 0; k < n; ++k) {
-      st[k] = ev->sub[k].desc;
-      for (uint32_t t = 0; t < st[k].nTiles; ++t) te[st[k].tileBase + t] = (u16)k;
-    }
-    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st, descBytes, cudaMemcpyHostToDevice, stream));
-    ++nMemcpy;
-    const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
-  }
-  nLaunch += 3;
-  PR_CUDA(h, cudaGetLastError());
-  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
-  ev->exported = want != 0;
+  // descriptor block: [EvDesc x n][tile -> event map] for batches, then the export table (exact-size mirrors)
+  std::vector<ExportItem> items;
   if (want) {
-    // exact-size mirrors: the item table lives at the head of the pinned slab's tail (mapped memory)
-    std::vector<ExportItem> items;
     for (uint32_t k = 0; k < n; ++k) {
       const EvDesc& d = ev->sub[k].desc; const pr_output& o = ev->sub[k].hostViews;
       auto add = [&](const void* src, const void* dst, uint32_t eb, uint32_t sel, uint32_t fixed) {
@@ -326,16 +325,51 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       add(d.modClusStart, o.h_mod_clus_start, 4, 3, M + 1);
       add(d.errWord, o.h_err_word, 4, 1, 0); add(d.errIdx, o.h_err_idx, 4, 1, 0);
     }
-    void* itab = ev->itemTab;                      // read zero-copy by the kernel; freed at release
-    memcpy(itab, items.data(), items.size() * sizeof(ExportItem));
+  }
+  if (descBytes) {
+    char* st8 = (char*)ev->descStage;
+    if (n > 1) {
+      EvDesc* st = (EvDesc*)st8;
+      u16* te = (u16*)(st + n);
+      for (uint32_t k = 0; k < n; ++k) {
+        st[k] = ev->sub[k].desc;
+        for (uint32_t t = 0; t < st[k].nTiles; ++t) te[st[k].tileBase + t] = (u16)k;
+      }
+    }
+    if (!items.empty()) memcpy(st8 + descPart, items.data(), items.size() * sizeof(ExportItem));
+    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st8, descPart + items.size() * sizeof(ExportItem), cudaMemcpyHostToDevice, stream));
+    ++nMemcpy;
+  }
+  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
+  if (n == 1) {
+    const EvDesc& d = ev->sub[0].desc;
+    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
+  } else {
+    const EvDesc* dd = (const EvDesc*)ev->descDev;
+    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
+  }
+  nLaunch += 3;
+  PR_CUDA(h, cudaGetLastError());
+  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
+  ev->exported = want != 0;
+  if (want && !items.empty()) {
+    const ExportItem* itab = (const ExportItem*)((const char*)ev->descDev + descPart);   // device-resident export table
     size_t maxBytes = 0;
     for (uint32_t k = 0; k < n; ++k) maxBytes = maxBytes > (size_t)ev->sub[k].cap * 4 ? maxBytes : (size_t)ev->sub[k].cap * 4;
-    uint32_t gx = (uint32_t)((maxBytes / 16 + 255) / 256);
+    uint32_t gx = (uint32_t)((maxBytes / 16 + 1023) / 1024);       // grid-stride copy: about four 16-byte vectors per thread
     if (gx < 1) gx = 1;
     if (gx > 64) gx = 64;
     uint32_t gy = (uint32_t)items.size();
     if (gy > 2048) gy = 2048;
-    k_export<<<dim3(gx, gy), 256, 0, stream>>>((const ExportItem*)itab, (uint32_t)items.size(), counters);
+    k_export<<<dim3(gx, gy), 256, 0, stream>>>(itab, (uint32_t)items.size(), counters);
     ++nLaunch;
     PR_CUDA(h, cudaGetLastError());
   }
