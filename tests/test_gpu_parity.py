@@ -277,6 +277,49 @@ def test_batch_matches_single_events(pr):
         slot.release()
 
 
+@pytest.mark.parametrize("layout", ["one_span", "separate", "misaligned_span"])
+def test_host_input_batch_staging_paths(pr, layout):
+    """Pinned host inputs of a batch: one dense span (staged by one copy per array), separately allocated
+    buffers and a span whose events are not 16-byte aligned relative to each other (one copy per event)."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, 20 + e) for e in range(4)] + [wl.Event(np.zeros(0, np.uint32), np.zeros(0, np.uint16), 1856)]
+    evs += [wl.make_event(3, 21), wl.event_from_pixels([(7, 3, 5, 90), (7, 3, 6, 120)], 1856)]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        if layout == "separate":
+            bufs = []
+            for e in evs:
+                hw, ha = p.host_array(max(e.n_words, 1), np.uint32), p.host_array(max(e.n_words, 1), np.uint16)
+                hw[:e.n_words], ha[:e.n_words] = e.words, e.adc
+                bufs.append((hw[:e.n_words], ha[:e.n_words]))
+        else:
+            step = 8 if layout == "one_span" else 3               # element alignment of each event inside the pool
+            offs, tot = [], 0
+            for e in evs:
+                offs.append(tot)
+                tot += (e.n_words + step - 1) // step * step + (0 if layout == "one_span" else 1)
+            W, A = p.host_array(tot + 8, np.uint32), p.host_array(tot + 8, np.uint16)
+            bufs = []
+            for e, o in zip(evs, offs):
+                W[o:o + e.n_words], A[o:o + e.n_words] = e.words, e.adc
+                bufs.append((W[o:o + e.n_words], A[o:o + e.n_words]))
+        slot = p.slot()
+        st0 = p.stats()
+        slot.acquire_batch(bufs, stream=torch.cuda.Stream(), want=pr.PR_WANT_ALL)
+        wait(slot)
+        code, outs = slot.produce_batch(len(evs))
+        assert code == 0
+        copies = p.stats()["memcpy_calls"] - st0["memcpy_calls"]
+        n_nonempty = sum(1 for e in evs if e.n_words)
+        if layout == "separate":                                   # pool blocks may or may not happen to be adjacent
+            assert copies in (3, 2 * n_nonempty + 1)
+        else:
+            assert copies == (3 if layout == "one_span" else 2 * n_nonempty + 1)     # + the descriptor/export-table block
+        for e, out in zip(evs, outs):
+            ref = oracle_of(e, cal)
+            compare(out, ref, lambda f: out.host(f))
+        slot.release()
+
+
 def _blob_module(rng, m, n, dup_frac=0.0, box=40):
     """n digis of module m packed into a small box (many merges, long chains), random order,
     ADC spanning both thresholds; optionally some duplicate pixels (A6)."""
