@@ -276,6 +276,7 @@ class Bench:
         out = pr.pr_output()
         busy = [False] * len(slots)
         digis = clusters = 0
+        self.spans = []
         ptrs = [self.at(pr, inp, k) for k in range(n_events_pool)]
 
         def finish(i):
@@ -287,6 +288,7 @@ class Bench:
             if r != 0:
                 raise RuntimeError(f"pr_produce -> {r}")
             digis += out.n_digis; clusters += out.n_clusters
+            self.spans.append((out.t_start_ns, out.t_end_ns))
             lib.pr_release(slots[i].ptr)
             busy[i] = False
         for e in range(n_events):
@@ -476,7 +478,12 @@ def run_configs2(torch, pr, wl, local):
     reps = 40
     t, wall = b.timed(streams, lambda: [b.run_streams(inp, len(pool), 64, slots, streams, first=64 * r) for r in range(reps)])
     st1 = b.p.stats()
+    sp = sorted(b.spans)                             # device %globaltimer intervals of the last pass's events
+    busy_ns = sum(t1 - t0 for t0, t1 in sp)
+    wall_ns = max(t1 for _, t1 in sp) - min(t0 for t0, _ in sp)
     extra["configs[2] per-event streams"] = {
+        "mean_events_in_flight_on_device": busy_ns / max(wall_ns, 1),
+        "consecutive_events_overlapping": sum(1 for a, c in zip(sp, sp[1:]) if c[0] < a[1]) / max(len(sp) - 1, 1),
         "events_per_s": 64 * reps / t, "events": 64 * reps, "streams_in_flight": STREAMS_IN_FLIGHT,
         "us_per_event": t / (64 * reps) * 1e6, "max_events_in_flight": st1["max_events_in_flight"],
         "new_cudaMalloc_in_timed_region": st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"],

@@ -44,7 +44,7 @@
 extern "C" {
 #endif
 
-#define PR_ABI_VERSION 1
+#define PR_ABI_VERSION 2
 
 /* ---- return codes (int).  Negative = error.  pr_strerror() names them. ---- */
 #define PR_OK               0
@@ -120,6 +120,9 @@ typedef struct {                  /* one event's input, filled by the caller bef
 typedef struct {
   uint64_t event_id;
   uint32_t n_words, n_digis, n_errors, n_kept_digis, n_clusters_all, n_clusters, status_bits, n_modules;
+  uint64_t t_start_ns, t_end_ns;  /* device %globaltimer when the first kernel of the acquire started and when this
+                                     event's counters were published: kernels of events on different streams may
+                                     overlap; the intervals show whether they did                         */
   const uint16_t *d_module, *d_row, *d_col, *d_adc; const uint32_t* d_word_idx;
   const float* d_charge; const uint32_t* d_label; const int32_t* d_clus;
   const uint32_t *d_mod_digi_start, *d_mod_clus_start;

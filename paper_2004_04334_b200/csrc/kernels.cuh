@@ -45,12 +45,20 @@ struct DevCounters {
 };
 // Per-launch control words (zeroed per acquire).
 struct LaunchCtl {
-  u32 modTicket, modDone, pad[14];
+  u32 modTicket, modDone;
+  u64 tStart;                       // %globaltimer at the start of the acquire's first kernel
+  u32 pad[12];
 };
 // What the host reads after completion (mapped pinned memory, written by the last block).
 struct HostCounters {
   u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, seq;
+  u64 tStart, tEnd;                 // %globaltimer: first kernel of the acquire started, this event's counters published
 };
+__device__ __forceinline__ u64 global_timer() {
+  u64 t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 
 // One event of a launch.  The first 128 bytes are all that k_unpack reads: in a batch, one warp-wide
 // load brings them into shared memory.
@@ -254,13 +262,14 @@ __device__ unsigned long long g_trace[1024 * 32];
 template <bool kSingle>
 __global__ void __launch_bounds__(kUnpackThreads + 64, kUnpackCtasPerSM)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
-         u32 totalTiles, const __grid_constant__ Geom g) {
+         u32 totalTiles, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
   const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA; warp 9 publishes and looks back
   const u32 first = blockIdx.x;
   if (first >= totalTiles) return;
+  if (first == 0 && tid == 0) lc->tStart = global_timer();
 #ifdef PIXRECO_TRACE
   unsigned long long trAcc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   const long long trStart = clock64();
@@ -1179,6 +1188,7 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     HostCounters h;
     h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
     h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[32]; h.status = status; h.seq = 1;
+    h.tStart = lc->tStart; h.tEnd = global_timer();
     *ev.hostCounters = h;
   }
 }

@@ -343,14 +343,14 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
   if (n == 1) {
     const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, h->geom);
+    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, h->geom);
+    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
@@ -429,6 +429,7 @@ void fill_output(pr_event* ev, uint32_t k, pr_output* out) {
   out->n_words = c.nWords; out->n_digis = c.nDigis; out->n_errors = c.nErrors; out->n_kept_digis = c.nKept;
   out->n_clusters_all = c.nClustersAll; out->n_clusters = c.nClusters; out->status_bits = c.status;
   out->n_modules = ev->h->cfg.n_modules;
+  out->t_start_ns = c.tStart; out->t_end_ns = c.tEnd;
   out->d_module = d.module; out->d_row = d.row; out->d_col = d.col; out->d_adc = d.adcOut; out->d_word_idx = d.wordIdx;
   out->d_charge = d.charge; out->d_label = d.label; out->d_clus = d.clus;
   out->d_mod_digi_start = d.modDigiStart; out->d_mod_clus_start = d.modClusStart;

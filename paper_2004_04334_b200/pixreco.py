@@ -66,6 +66,7 @@ class pr_output(ctypes.Structure):
     _fields_ = ([("event_id", c_uint64)] +
                 [(n, c_uint32) for n in ("n_words", "n_digis", "n_errors", "n_kept_digis", "n_clusters_all",
                                          "n_clusters", "status_bits", "n_modules")] +
+                [("t_start_ns", c_uint64), ("t_end_ns", c_uint64)] +
                 [("d_" + n, c_void_p) for n in _VIEWS] + [("h_" + n, c_void_p) for n in _VIEWS])
 
 
@@ -160,7 +161,7 @@ class Output:
 
     def __init__(self, raw: pr_output, device: int):
         self.raw, self._device = raw, device
-        for n, _ in pr_output._fields_[:9]:
+        for n, _ in pr_output._fields_[:11]:                  # event_id, eight counters, t_start_ns, t_end_ns
             setattr(self, n, int(getattr(raw, n)))
 
     def _len(self, name):

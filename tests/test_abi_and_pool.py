@@ -20,7 +20,7 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pr.lib()
     for name in declared:
         assert getattr(lib, name) is not None
-    assert lib.pr_abi_version() == 1
+    assert lib.pr_abi_version() == 2
     assert lib.pr_strerror(pr.PR_ERR_INPUT_ORDER).decode().startswith("input words")
 
 
@@ -28,7 +28,7 @@ def test_struct_layouts_match_the_header():
     # sizes the C side checks (struct_size) or relies on
     assert ctypes.sizeof(pr.pr_config) == 72
     assert ctypes.sizeof(pr.pr_input) == 56
-    assert ctypes.sizeof(pr.pr_output) == 8 + 8 * 4 + 36 * 8
+    assert ctypes.sizeof(pr.pr_output) == 8 + 8 * 4 + 2 * 8 + 36 * 8       # event_id, counters, two device time stamps, 36 views
     assert ctypes.sizeof(pr.pr_pool_stats) == 64
 
 

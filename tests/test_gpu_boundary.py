@@ -145,9 +145,22 @@ def test_concurrent_streams_same_results_and_zero_steady_state_malloc(pr):
 
         one_pass(check)                             # warm-up fills the pools
         s0 = p.stats()
+        spans = []                                  # (event, device ns when its first kernel started / its counters were out)
+
+        def light(e, code, out):
+            if not (code == 0 and out.n_clusters == refs[e].n_clusters):
+                pytest.fail("mismatch")
+            assert out.t_end_ns > out.t_start_ns > 0
+            spans.append((e, out.t_start_ns, out.t_end_ns))
         for _ in range(3):
-            one_pass(lambda e, code, out: None if (code == 0 and out.n_clusters == refs[e].n_clusters) else pytest.fail("mismatch"))
+            one_pass(light)
         s1 = p.stats()
+        # P:L86 "work in different streams may run concurrently": the device intervals of events on different
+        # streams overlap (each event alone is far too small to fill the GPU)
+        spans.sort(key=lambda x: x[1])
+        overlapping = sum(1 for a, b in zip(spans, spans[1:]) if b[1] < a[2])
+        assert overlapping >= len(spans) // 4, f"only {overlapping} of {len(spans)} consecutive events overlapped on the device"
+
         assert s1["device_pool"]["backend_allocs"] == s0["device_pool"]["backend_allocs"]
         assert s1["host_pool"]["backend_allocs"] == s0["host_pool"]["backend_allocs"]
         assert s1["device_pool"]["backend_frees"] == 0
