@@ -611,7 +611,7 @@ __device__ __forceinline__ u32 wm_find_min(const u32* tab, u32 pmask, u32 shift,
 // ---- warp path, one digi per lane: module = digis [s, s+n), 0 < n <= 32.  Everything lives in
 // registers: adjacency and reachability are 32-bit lane masks (Warshall closure with shuffles),
 // the cluster's minimum lane is its root, sums run along each cluster's lane list.
-__device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr,
+__device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr, float q0, u32 rc0,
                                                   u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   constexpr u32 pmask = 127u, shift = 25u;          // 128 slots: load <= 1/4
@@ -620,11 +620,9 @@ __device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& 
   *reinterpret_cast<uint4*>(tab + lane * 4u) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
   fw[lane] = 0u;
   __syncwarp();
-  float q = 0.f; u32 key = kNoKey;
-  if (lane < n) {
-    q = ev.charge[s + lane];
-    if (q >= g.pixThr) key = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
-  }
+  // (q0, rc0): charge and row << 9 | col of digi s + lane, loaded by the caller while the previous module was processed
+  const float q = lane < n ? q0 : 0.f;
+  const u32 key = (lane < n && q >= g.pixThr) ? rc0 : kNoKey;                  // A8
   const bool kept = key != kNoKey;
   bool dup = false;
   if (kept) {
@@ -703,7 +701,7 @@ __device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& 
 
 // ---- warp path: one module = digis [s, s+n), 0 < n <= kWarpCap, processed by the calling warp.
 // Returns (kept digis, clusters, kept clusters) in all lanes.
-__device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr,
+__device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr, float q0, u32 rc0,
                                             u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   const u32 nPad = (n + 31u) & ~31u;
@@ -716,10 +714,14 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   for (u32 i = lane * 4u; i <= pmask; i += 128u) *reinterpret_cast<uint4*>(tab + i) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
   __syncwarp();
   // B: load, kept flag (A8), insert; every digi starts with no neighbours (all bytes = self)
+  // The loads run one chunk ahead (the first chunk came with the call): charge, row and col together.
   u32 nKept = 0; bool dup = false;
+  float qc = q0; u32 rcc = rc0;
   for (u32 i = lane; i < nPad; i += 32u) {
-    u32 key = kNoKey;
-    if (i < n && ev.charge[s + i] >= g.pixThr) key = (u32)ev.row[s + i] << 9 | (u32)ev.col[s + i];
+    float qn = 0.f; u32 rcn = 0;
+    if (i + 32u < n) { qn = ev.charge[s + i + 32u]; rcn = (u32)ev.row[s + i + 32u] << 9 | (u32)ev.col[s + i + 32u]; }
+    const u32 key = (i < n && qc >= g.pixThr) ? rcc : kNoKey;                  // A8
+    qc = qn; rcc = rcn;
     wr.key[i] = key;
     wr.nb[i] = make_uint2(i * 0x01010101u, i * 0x01010101u);
     if (key != kNoKey) {
@@ -1092,8 +1094,20 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     if (ev.counters->status & 1u) continue;
     const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
     u32 accK = 0, accA = 0, accG = 0;
+    // first chunk (digi s + lane) of a module is loaded while the module before it is processed
+    auto preload = [&](u32 k, float* q, u32* rc) {
+      const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
+      *q = 0.f; *rc = 0u;
+      if (t1 >= s && t1 <= ev.cap && t1 - s <= kWarpCap && lane < t1 - s) {
+        *q = ev.charge[s + lane]; *rc = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
+      }
+    };
+    float qNext; u32 rcNext;
+    preload(0, &qNext, &rcNext);
     for (u32 k = 0; k < nm; ++k) {
       const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
+      const float q0 = qNext; const u32 rc0 = rcNext;
+      if (k + 1u < nm) preload(k + 1u, &qNext, &rcNext);
       u32 cnt = 0;
       if (t1 < s || t1 > ev.cap) {
         if (lane == 0) atomicOr(&ev.counters->status, 2u);   // PR_STATUS_CAPACITY: inconsistent module table
@@ -1102,8 +1116,8 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         if (n > kWarpCap) continue;                          // dense path wrote this module
         if (n > 0) {
           u32 nk, nr;
-          if (n <= 32u) warp_module_small(ev, g, s, n, wr, &nk, &nr, &cnt);
-          else warp_module(ev, g, s, n, wr, &nk, &nr, &cnt);
+          if (n <= 32u) warp_module_small(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
+          else warp_module(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
           accK += nk; accA += nr;
         }
       }
