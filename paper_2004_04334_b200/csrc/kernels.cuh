@@ -608,71 +608,42 @@ __device__ __forceinline__ u32 wm_find_min(const u32* tab, u32 pmask, u32 shift,
   }
 }
 
-// ---- warp path, one digi per lane: module = digis [s, s+n), 0 < n <= 32.  Everything lives in
-// registers: adjacency and reachability are 32-bit lane masks (Warshall closure with shuffles),
-// the cluster's minimum lane is its root, sums run along each cluster's lane list.
-__device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr, float q0, u32 rc0,
-                                                  u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
+// ---- warp path, one digi per lane: a PACK of consecutive modules with at most 32 digis together, digis
+// [s, s+n).  Everything lives in registers: lane i learns its neighbours by comparing its (module, row,
+// col) with every other lane's (n shuffles, no table; two digis on one pixel are simply adjacent, A6),
+// adjacency and reachability are 32-bit lane masks (Warshall closure with shuffles), a cluster's
+// minimum lane is its root, sums run along each cluster's lane list.  mIdx/mStart: the lane's module
+// (index within the pack) and that module's first digi.  Returns the ballots of kept digis, of roots
+// and of roots of kept clusters.
+__device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s, u32 n, float q0, u32 rc0, u32 mIdx, u32 mStart,
+                                          u32* keptDigis, u32* roots, u32* keptRoots) {
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
-  constexpr u32 pmask = 127u, shift = 25u;          // 128 slots: load <= 1/4
-  u32* tab = wr.tab;
-  u32* fw = wr.tab + 128;                           // forward edges: lane mask per digi
-  *reinterpret_cast<uint4*>(tab + lane * 4u) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-  fw[lane] = 0u;
-  __syncwarp();
-  // (q0, rc0): charge and row << 9 | col of digi s + lane, loaded by the caller while the previous module was processed
   const float q = lane < n ? q0 : 0.f;
-  const u32 key = (lane < n && q >= g.pixThr) ? rc0 : kNoKey;                  // A8
-  const bool kept = key != kNoKey;
-  bool dup = false;
-  if (kept) {
-    const u32 ent = key << 8 | lane;
-    u32 h = wm_slot(key, shift);
-    for (;;) {
-      const u32 old = atomicCAS(tab + h, kEmpty, ent);
-      if (old == kEmpty) break;
-      if ((old >> 8) == key) dup = true;
-      h = (h + 1) & pmask;
-    }
+  const bool kept = lane < n && q >= g.pixThr;                                  // A8
+  // K = col | row << 10 | module << 19 with a guard bit above col and row: K_i - K_j + (1 | 1 << 10) has both
+  // fields in {0, 1, 2} and nothing else set iff same module, |d row| <= 1 and |d col| <= 1.  A digi that is
+  // not kept gets a module of its own.
+  const u32 K = kept ? ((rc0 & 511u) | (rc0 >> 9) << 10 | mIdx << 19) : (0x1000u + lane) << 19;
+  const u32 Kb = K + 0x401u;
+  u32 adj = 0;
+#pragma unroll 4
+  for (u32 j = 0; j < n; ++j) {
+    const u32 t = Kb - __shfl_sync(0xFFFFFFFFu, K, j);
+    const u32 bad = (t & ~0xC03u) | (t & (t >> 1) & 0x401u);
+    adj |= (bad == 0u ? 1u : 0u) << j;
   }
-  const u32 keptMask = __ballot_sync(0xFFFFFFFFu, kept);
-  dup = __any_sync(0xFFFFFFFFu, dup);
-  __syncwarp();
-  // backward neighbours W, NW, N, NE; each edge is recorded on both ends
-  u32 adj = 1u << lane;
-  if (kept) {
-    const u32 row = key >> 9, col = key & 511u;
-    u32 owner = lane;
-    if (dup) owner = wm_find_min(tab, pmask, shift, key);
-    if (owner != lane) {                              // a duplicate only joins its pixel's owner (A6)
-      adj |= 1u << owner; atomicOr(fw + owner, 1u << lane);
-    } else {
-      const bool up = row > 0, left = col > 0, right = col + 1 < g.C;
-#define WM_NB(cond, delta)                                                                          \
-      if (cond) {                                                                                   \
-        const u32 j = dup ? wm_find_min(tab, pmask, shift, key - (delta)) : wm_find(tab, pmask, shift, key - (delta)); \
-        if (j != kEmpty) { adj |= 1u << j; atomicOr(fw + j, 1u << lane); }                          \
-      }
-      WM_NB(left, 1u)
-      WM_NB(up && left, 513u)
-      WM_NB(up, 512u)
-      WM_NB(up && right, 511u)
-#undef WM_NB
-    }
-  }
-  __syncwarp();
-  u32 reach = adj | fw[lane];
+  adj |= 1u << lane;
   // transitive closure (Warshall): after step j every lane that reaches j also reaches all of j's set
+  u32 reach = adj;
   for (u32 j = 0; j < n; ++j) {
     const u32 rj = __shfl_sync(0xFFFFFFFFu, reach, j);
     if (reach & (1u << j)) reach |= rj;
   }
   const u32 root = (u32)__ffs((int)reach) - 1u;
   const bool isRoot = kept && root == lane;
-  const u32 nR = (u32)__popc(__ballot_sync(0xFFFFFFFFu, isRoot));
   // sums of qf = q * 2^14 (A9) in binary64 (exact: at most 32 terms below 2^43), suffix sums along the lane list
   double qf = 0.0, qx = 0.0, qy = 0.0;
-  if (kept) { qf = (double)(q * 16384.0f); qx = qf * (double)(key >> 9); qy = qf * (double)(key & 511u); }
+  if (kept) { qf = (double)(q * 16384.0f); qx = qf * (double)(rc0 >> 9); qy = qf * (double)(rc0 & 511u); }
   const u32 most = __reduce_max_sync(0xFFFFFFFFu, (u32)__popc(reach));
   const u32 above = reach & (0xFFFFFFFEu << lane);
   u32 nxt = above ? (u32)__ffs((int)above) - 1u : 32u;
@@ -684,9 +655,9 @@ __device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& 
   }
   const bool keptC = isRoot && __double2ll_rz(qf) >= g.clusThrFixed;
   const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
-  const u32 kr = (u32)__popc(kb & lt);
+  const u32 kr = (u32)__popc(kb & lt & ~((1u << (mStart - s)) - 1u));           // rank among the module's kept clusters
   if (keptC) {
-    const u32 o = s + kr;
+    const u32 o = mStart + kr;
     ev.stS[o] = qf; ev.stSx[o] = qx; ev.stSy[o] = qy;
     ev.stLabel[o] = s + lane; ev.stSize[o] = (u32)__popc(reach);
   }
@@ -695,8 +666,7 @@ __device__ __forceinline__ void warp_module_small(const EvDesc& ev, const Geom& 
     ev.label[s + lane] = kept ? s + root : kInvalid;
     ev.clus[s + lane] = (kept && krRoot != kNoRank) ? (int32_t)krRoot : -1;
   }
-  __syncwarp();
-  *nKeptDigis = (u32)__popc(keptMask); *nRootsOut = nR; *nKeptClusters = (u32)__popc(kb);
+  *keptDigis = __ballot_sync(0xFFFFFFFFu, kept); *roots = __ballot_sync(0xFFFFFFFFu, isRoot); *keptRoots = kb;
 }
 
 // ---- warp path: one module = digis [s, s+n), 0 < n <= kWarpCap, processed by the calling warp.
@@ -1094,35 +1064,59 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     if (ev.counters->status & 1u) continue;
     const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
     u32 accK = 0, accA = 0, accG = 0;
-    // first chunk (digi s + lane) of a module is loaded while the module before it is processed
-    auto preload = [&](u32 k, float* q, u32* rc) {
-      const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
+    // The ticket's digis are contiguous.  The next unit's first chunk (32 digis) is loaded while the current unit
+    // (a pack of small modules, or one module of 33..kWarpCap digis) is processed.
+    const u32 sEnd = min(__shfl_sync(0xFFFFFFFFu, st, nm), ev.cap);
+    auto preload = [&](u32 s, float* q, u32* rc) {
       *q = 0.f; *rc = 0u;
-      if (t1 >= s && t1 <= ev.cap && t1 - s <= kWarpCap && lane < t1 - s) {
-        *q = ev.charge[s + lane]; *rc = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
-      }
+      if (s + lane < sEnd) { *q = ev.charge[s + lane]; *rc = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane]; }
     };
     float qNext; u32 rcNext;
-    preload(0, &qNext, &rcNext);
-    for (u32 k = 0; k < nm; ++k) {
+    preload(__shfl_sync(0xFFFFFFFFu, st, 0), &qNext, &rcNext);
+    for (u32 k = 0; k < nm;) {
       const u32 s = __shfl_sync(0xFFFFFFFFu, st, k), t1 = __shfl_sync(0xFFFFFFFFu, st, k + 1);
+      if (t1 < s || t1 > ev.cap) {                           // inconsistent module table
+        if (lane == 0) { atomicOr(&ev.counters->status, 2u); ev.modCount[m0 + k] = 0u; }   // PR_STATUS_CAPACITY
+        preload(t1 <= ev.cap ? t1 : sEnd, &qNext, &rcNext);
+        ++k;
+        continue;
+      }
       const float q0 = qNext; const u32 rc0 = rcNext;
-      if (k + 1u < nm) preload(k + 1u, &qNext, &rcNext);
-      u32 cnt = 0;
-      if (t1 < s || t1 > ev.cap) {
-        if (lane == 0) atomicOr(&ev.counters->status, 2u);   // PR_STATUS_CAPACITY: inconsistent module table
-      } else {
+      if (t1 - s > 32u) {                                    // one module of its own
         const u32 n = t1 - s;
-        if (n > kWarpCap) continue;                          // dense path wrote this module
-        if (n > 0) {
-          u32 nk, nr;
-          if (n <= 32u) warp_module_small(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
-          else warp_module(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
-          accK += nk; accA += nr;
+        preload(t1, &qNext, &rcNext);
+        if (n <= kWarpCap) {                                 // else: the dense path wrote this module
+          u32 nk, nr, cnt;
+          warp_module(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
+          accK += nk; accA += nr; accG += cnt;
+          if (lane == 0) ev.modCount[m0 + k] = cnt;
+        }
+        ++k;
+        continue;
+      }
+      // pack: modules k .. k2-1, consecutive, consistent, at most 32 digis together
+      u32 k2 = k + 1u, e2 = t1, mIdx = 0, mStart = s;
+      while (k2 < nm) {
+        const u32 en = __shfl_sync(0xFFFFFFFFu, st, k2 + 1u);
+        if (en < e2 || en > ev.cap || en - s > 32u) break;
+        if (e2 - s <= lane) { mIdx = k2 - k; mStart = e2; }   // module k2 starts at e2
+        e2 = en; ++k2;
+      }
+      preload(e2, &qNext, &rcNext);
+      const u32 n = e2 - s;
+      u32 kd = 0, rb = 0, kb = 0;
+      if (n) warp_pack(ev, g, s, n, q0, rc0, mIdx, mStart, &kd, &rb, &kb);
+      accK += (u32)__popc(kd); accA += (u32)__popc(rb); accG += (u32)__popc(kb);
+      // kept clusters per module of the pack: lane j - k writes module j's
+      {
+        const u32 j = k + lane;
+        const u32 lo = __shfl_sync(0xFFFFFFFFu, st, min(j, nm)) - s, hi = __shfl_sync(0xFFFFFFFFu, st, min(j + 1u, nm)) - s;
+        if (j < k2) {
+          const u32 mask = (hi >= 32u ? 0xFFFFFFFFu : (1u << hi) - 1u) & ~(lo >= 32u ? 0xFFFFFFFFu : (1u << lo) - 1u);
+          ev.modCount[m0 + j] = (u32)__popc(kb & mask);
         }
       }
-      if (lane == 0) ev.modCount[m0 + k] = cnt;
-      accG += cnt;
+      k = k2;
     }
     if (lane == 0 && accG) atomicAdd(&ev.grpCount[m0 / 32u], accG);     // kModBatch divides 32: one group per ticket
     if (lane == 0) {
