@@ -47,7 +47,7 @@ STREAMS_IN_FLIGHT = 8        # configs[2]
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--slots", type=int, default=4, help="batches in flight (batch mode)")
@@ -57,6 +57,16 @@ def parse():
                     help="run just this extra case and print its JSON (for ncu captures of HBM-sized launches)")
     ap.add_argument("--reps", type=int, default=6, help="timed launches per extra case")
     return ap.parse_args()
+
+
+def load_traffic(kernel):
+    """DRAM bytes per launch of `kernel` (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+    ncu --set full capture of this bench's step (profiles/traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f)["kernels"][kernel]["dram_bytes_per_launch"]
+    except Exception:
+        return None
 
 
 def load_peaks():
@@ -77,7 +87,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
@@ -417,7 +427,7 @@ def run_ours(args, rank, world):
                                "gbs": (8 * Dm + 56 * Nm + 4 * (M + 1)) * EVENTS_PER_STEP / t_fi / 1e9}}
         dom = max(kern, key=lambda k: kern[k]["ms"])
         line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                            "frac": kern[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                            "frac": kern[dom]["gbs"] / peak, "traffic": load_traffic(dom), "peak_source": peak_src,
                             "frac_of_8TBs_nominal": kern[dom]["gbs"] / 8000.0,
                             "algorithmic_bytes_per_launch": kern[dom]["bytes"], "ms_per_launch": kern[dom]["ms"],
                             "units_per_launch": f"{EVENTS_PER_STEP} events", "kernels": kern,

@@ -161,6 +161,12 @@ def test_edge_cases(pr):
         "no_wrap": hand([(0, 159, 7, 60), (0, 0, 7, 60), (1, 10, 415, 60), (1, 11, 0, 60), (1, 10, 0, 60)], 4),
         "module_boundary": hand([(1, 3, 3, 60), (2, 3, 3, 60), (2, 4, 4, 60)], 4),
         "ragged_9_words": hand([(0, 1, c, 60) for c in range(9)], 4),
+        # several small modules clustered in one register pass: same pixels in neighbouring modules stay apart,
+        # an empty module in between, duplicates, a module boundary right next to a sub-threshold digi
+        "pack_same_pixels": hand([(0, 10, 10, 60), (0, 10, 11, 60), (1, 10, 10, 60), (1, 10, 11, 60), (1, 11, 12, 60),
+                                  (3, 10, 10, 60), (3, 9, 9, 12), (3, 10, 10, 70), (3, 11, 11, 20)], 4),
+        "pack_exactly_32": hand([(0, 5, c, 60) for c in range(16)] + [(1, 5, c, 60) for c in range(0, 32, 2)], 4),
+        "pack_33": hand([(0, 5, c, 60) for c in range(16)] + [(1, 5, c, 60) for c in range(17)], 4),
     }
     # U shape / spiral with the minimum index at the far end; strip interleaved
     arm1 = [(0, r, 10, 60) for r in range(60)]
