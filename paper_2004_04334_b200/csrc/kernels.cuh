@@ -734,8 +734,21 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   __syncwarp();
   // D: label equivalence.  L[i] only decreases and always names a digi of i's component; a round
   // takes the minimum over the neighbours, hooks the old representative under it, then flattens.
+  // The first round needs no look-ups: with L = identity the minimum over the neighbours is the minimum
+  // neighbour index.
   u32* L = tab;
-  for (u32 i = lane; i < nPad; i += 32u) L[i] = i;
+  for (u32 i = lane; i < nPad; i += 32u) {
+    const uint2 nb = wr.nb[i];
+    u32 v = __vminu4(nb.x, nb.y);
+    v = __vminu4(v, v >> 16); v = __vminu4(v, v >> 8);
+    L[i] = min(i, v & 0xFFu);
+  }
+  __syncwarp();
+  for (u32 i = lane; i < nPad; i += 32u) {
+    u32 l = L[i], p;
+    while ((p = L[l]) != l) l = p;
+    L[i] = l;
+  }
   __syncwarp();
   for (;;) {
     bool changed = false;
