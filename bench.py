@@ -280,6 +280,53 @@ class Bench:
                 finish(i)
         return digis, clusters
 
+    # -- the same with the host copy as a stage of its own (pr_transfer): acquire with want = 0, produce,
+    #    then transfer the cluster table (device gather + one exact-size DMA copy), produce again
+    def run_batches_transfer(self, inp, n_events_pool, steps, slots, streams, want, first_step=0):
+        lib, pr = self.lib, self.pr
+        outs = (pr.pr_output * EVENTS_PER_STEP)()
+        nb = n_events_pool // EVENTS_PER_STEP
+        stage = [0] * len(slots)                      # 0 idle, 1 acquire in flight, 2 transfer in flight
+        clusters = 0
+
+        def advance(i, block):
+            """Moves slot i forward; returns True when it is idle again."""
+            nonlocal clusters
+            while stage[i]:
+                r = lib.pr_produce_batch(slots[i].ptr, outs, EVENTS_PER_STEP)
+                if r == pr.PR_NOT_READY:
+                    if not block:
+                        return False
+                    continue
+                if r != 0:
+                    raise RuntimeError(f"pr_produce_batch -> {r}")
+                if stage[i] == 1:
+                    r = lib.pr_transfer(slots[i].ptr, want, ctypes.c_void_p(streams[i].cuda_stream), pr.pr_done_fn(), None)
+                    if r != 0:
+                        raise RuntimeError(f"pr_transfer -> {r}")
+                    stage[i] = 2
+                else:
+                    for k in range(EVENTS_PER_STEP):
+                        clusters += outs[k].n_clusters
+                    lib.pr_release(slots[i].ptr)
+                    stage[i] = 0
+            return True
+        for s in range(steps):
+            i = s % len(slots)
+            for j in range(len(slots)):               # keep the other slots' stages moving
+                if j != i:
+                    advance(j, False)
+            advance(i, True)
+            b = (first_step + s) % nb
+            r = lib.pr_acquire_batch(slots[i].ptr, self.at(pr, inp, b * EVENTS_PER_STEP), EVENTS_PER_STEP,
+                                     ctypes.c_void_p(streams[i].cuda_stream))
+            if r != 0:
+                raise RuntimeError(f"pr_acquire_batch -> {r}")
+            stage[i] = 1
+        for i in range(len(slots)):
+            advance(i, True)
+        return clusters
+
     # -- configs[2]: one pr_acquire per event, 8 slots/streams in flight (A25: slot = stream = e mod 8)
     def run_streams(self, inp, n_events_pool, n_events, slots, streams, first=0):
         lib, pr = self.lib, self.pr
@@ -383,6 +430,14 @@ def run_ours(args, rank, world):
     barrier()
     t_e2e = max_over_ranks(t_e2e)
     e2e_value = world * n_events / t_e2e
+    # ---------------- R2': the same with the host copy as a stage of its own (pr_transfer)
+    inp_host0 = b.inputs(pin_ptrs, pr.PR_MEM_HOST_PINNED, 0)
+    b.run_batches_transfer(inp_host0, n_pool, Wm, slots, streams, pr.PR_WANT_CLUSTERS)
+    barrier()
+    t_tr, _ = b.timed(streams, lambda: b.run_batches_transfer(inp_host0, n_pool, min(K, 400), slots, streams, pr.PR_WANT_CLUSTERS, first_step=Wm))
+    barrier()
+    t_tr = max_over_ranks(t_tr)
+    e2e_transfer = world * min(K, 400) * EVENTS_PER_STEP / t_tr
     h2d = int(6 * meanW * EVENTS_PER_STEP)
     meanN = clusters / n_events
     d2h = int((22 * meanN + 4 * (M + 1) + 32) * EVENTS_PER_STEP)
@@ -399,7 +454,9 @@ def run_ours(args, rank, world):
                        "residency": "R1 device-resident inputs, counters to mapped pinned host"},
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": t_e2e / K * 1e3, "what": "pinned host inputs, want=CLUSTERS, same batch API"},
+                    "ms_per_step": t_e2e / K * 1e3, "what": "pinned host inputs, want=CLUSTERS, same batch API",
+                    "with_transfer_stage": {"value": e2e_transfer, "unit": "events/s",
+                                            "what": "want=0, then pr_transfer(CLUSTERS) after produce: device gather + one exact-size DMA copy per batch (P:L112)"}},
             "steady_state_cudaMalloc": int(new_mallocs), "wall_s": t_wall}
 
     if rank == 0:

@@ -185,6 +185,15 @@ int pr_produce_batch(pr_event* ev, pr_output* outs, uint32_t n);   /* outs[n]; w
 /* Return the slot's buffers to the pools; invalidates pr_output views.  PR_NOT_READY if the work
  * has not completed yet (nothing is released then).                                              */
 int pr_release(pr_event* ev);
+/* Transfer on demand as a stage of its own (the copy to the host is a module of its own, run
+ * only if something consumes it, and it learns about completion like any External Worker).  After a
+ * pr_produce that returned PR_OK, enqueue exact-size DMA copies (cudaMemcpyAsync, sizes taken from the
+ * event's counters) of the outputs in `want` that have no host mirror yet, on `cuda_stream` (any stream
+ * of the device: the slot's work is complete), and return at once.  The slot is in flight again:
+ * pr_query / pr_produce (/ `done`, may be NULL) as after pr_acquire; the next PR_OK pr_produce also fills
+ * the h_* views of what was requested here.  PR_ERR_BAD_STATE unless the slot is complete and not
+ * released; PR_ERR_INVALID_ARG for unknown bits; an event with a device-detected error transfers nothing. */
+int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done, void* user);
 /* The slot's completion cudaEvent_t (as void*) for cudaStreamWaitEvent on a consumer's stream
  * (P:L108), valid between pr_acquire and pr_release.                                             */
 void* pr_event_cuda_event(pr_event* ev);

@@ -70,6 +70,8 @@ struct pr_event {
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
   cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, finalize, export
   bool exported = false;
+  bool transferStage = false;  // the work in flight is a pr_transfer: completion does not count the events again
+  std::vector<void*> extraHost, extraDev;  // pinned / device blocks of pr_transfer stages, returned at release
 };
 
 namespace {
@@ -156,6 +158,9 @@ void release_blocks(pr_event* ev, bool completed) {
   if (ev->descDev) { h->devPool->free(ev->descDev, ev->stream, completed); ev->descDev = nullptr; }
   if (ev->hostSlab) { h->hostPool->free(ev->hostSlab, ev->stream, completed); ev->hostSlab = nullptr; }
   if (ev->descStage) { h->hostPool->free(ev->descStage, ev->stream, completed); ev->descStage = nullptr; }
+  for (void* p : ev->extraHost) h->hostPool->free(p, ev->stream, completed);
+  for (void* p : ev->extraDev) h->devPool->free(p, ev->stream, completed);
+  ev->extraHost.clear(); ev->extraDev.clear();
 }
 
 int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
@@ -379,6 +384,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
   ev->status = PR_OK;
   ev->state = kInFlight;
+  ev->transferStage = false;
   if (ev->doneFn) PR_CUDA(h, cudaLaunchHostFunc(stream, trampoline, ev));
 
   h->evAcquired.fetch_add(n); h->launches.fetch_add(nLaunch); h->memcpys.fetch_add(nMemcpy);
@@ -406,6 +412,7 @@ int poll(pr_event* ev) {
   }
   ev->status = worst;
   ev->state = kDone;
+  if (ev->transferStage) { ev->transferStage = false; ev->h->inFlight.fetch_sub(1); return PR_OK; }
   if (ev->h->timing) {
     float a = 0, b = 0, c = 0, f = 0;
     if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess &&
@@ -631,6 +638,93 @@ int pr_release(pr_event* ev) {
   release_blocks(ev, true);                      // completion observed: reusable by any stream at once
   ev->state = kIdle;
   ev->n = 0;
+  return PR_OK;
+}
+
+int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done, void* user) {
+  if (!ev || (want & ~0x1Fu)) return PR_ERR_INVALID_ARG;
+  pr_handle* h = ev->h;
+  if (h->sticky.load()) return PR_ERR_CUDA;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  if (ev->state == kInFlight && poll(ev) != PR_OK) return PR_ERR_BAD_STATE;
+  PR_CUDA(h, cudaSetDevice(h->cfg.device));
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  const uint32_t M = h->cfg.n_modules;
+  struct Copy { const void* src; const void** view; size_t bytes; };
+  std::vector<Copy> copies;
+  size_t total = 0;
+  for (uint32_t k = 0; k < ev->n; ++k) {
+    SubEvent& s = ev->sub[k];
+    const HostCounters& c = ev->hostCounters[k];
+    if (status_to_code(c.status) != PR_OK) continue;           // outputs undefined: nothing to copy
+    const EvDesc& d = s.desc; pr_output& o = s.hostViews;
+    auto add = [&](const void* src, const void** view, size_t count, size_t eb) {
+      if (*view) return;                                        // already mirrored
+      copies.push_back(Copy{src, view, count * eb});
+      total += align_up(count * eb ? count * eb : 1, 256);
+    };
+    const size_t D = c.nDigis, E = c.nErrors, N = c.nClusters;
+    if (want & PR_WANT_DIGIS) {
+      add(d.module, (const void**)&o.h_module, D, 2); add(d.row, (const void**)&o.h_row, D, 2); add(d.col, (const void**)&o.h_col, D, 2);
+      add(d.adcOut, (const void**)&o.h_adc, D, 2); add(d.wordIdx, (const void**)&o.h_word_idx, D, 4);
+      add(d.modDigiStart, (const void**)&o.h_mod_digi_start, M + 1, 4);
+    }
+    if (want & PR_WANT_CHARGE) add(d.charge, (const void**)&o.h_charge, D, 4);
+    if (want & PR_WANT_LABELS) { add(d.label, (const void**)&o.h_label, D, 4); add(d.clus, (const void**)&o.h_clus, D, 4); }
+    if (want & PR_WANT_CLUSTERS) {
+      add(d.clLabel, (const void**)&o.h_cl_label, N, 4); add(d.clSize, (const void**)&o.h_cl_size, N, 4);
+      add(d.clModule, (const void**)&o.h_cl_module, N, 2); add(d.clCharge, (const void**)&o.h_cl_charge, N, 4);
+      add(d.clRow, (const void**)&o.h_cl_row, N, 4); add(d.clCol, (const void**)&o.h_cl_col, N, 4);
+      add(d.modClusStart, (const void**)&o.h_mod_clus_start, M + 1, 4);
+    }
+    if (want & PR_WANT_ERRORS) { add(d.errWord, (const void**)&o.h_err_word, E, 4); add(d.errIdx, (const void**)&o.h_err_idx, E, 4); }
+  }
+  char* slab = nullptr;
+  if (total) {
+    slab = (char*)h->hostPool->alloc(total, stream);
+    if (!slab) return PR_ERR_OOM;
+    ev->extraHost.push_back(slab);
+  }
+  size_t off = 0; uint64_t nMemcpy = 0, nLaunch = 0;
+  if (copies.size() <= 4) {
+    for (const Copy& c : copies) {
+      *c.view = slab + off;
+      if (c.bytes) { PR_CUDA(h, cudaMemcpyAsync(slab + off, c.src, c.bytes, cudaMemcpyDeviceToHost, stream)); ++nMemcpy; }
+      off += align_up(c.bytes ? c.bytes : 1, 256);
+    }
+  } else {
+    // many arrays (a batch): gather them on the device into one block laid out like the host slab, then ONE DMA copy.
+    // The gather table goes up with one small copy; the sizes are exact because the counters are already on the host.
+    const size_t tabBytes = align_up(sizeof(ExportItem) * copies.size(), 256);
+    char* dstage = (char*)h->devPool->alloc(total + tabBytes, stream);
+    ExportItem* htab = (ExportItem*)h->hostPool->alloc(tabBytes, stream);
+    if (dstage) ev->extraDev.push_back(dstage);
+    if (htab) ev->extraHost.push_back(htab);
+    if (!dstage || !htab) return PR_ERR_OOM;
+    uint32_t nItems = 0;
+    for (const Copy& c : copies) {
+      *c.view = slab + off;
+      if (c.bytes) htab[nItems++] = ExportItem{c.src, dstage + tabBytes + off, 1u, 3u, (uint32_t)c.bytes, 0u};
+      off += align_up(c.bytes ? c.bytes : 1, 256);
+    }
+    if (nItems) {
+      PR_CUDA(h, cudaMemcpyAsync(dstage, htab, sizeof(ExportItem) * nItems, cudaMemcpyHostToDevice, stream));
+      k_export<<<dim3(4, nItems < 2048u ? nItems : 2048u), 256, 0, stream>>>((const ExportItem*)dstage, nItems, (const DevCounters*)ev->ctl);
+      PR_CUDA(h, cudaGetLastError());
+      PR_CUDA(h, cudaMemcpyAsync(slab, dstage + tabBytes, total, cudaMemcpyDeviceToHost, stream));
+      nMemcpy += 2; nLaunch += 1;
+    }
+  }
+  h->launches.fetch_add(nLaunch);
+  PR_CUDA(h, cudaEventRecord(ev->done, stream));
+  ev->stream = stream;
+  ev->doneFn = done; ev->doneUser = user;
+  ev->state = kInFlight;
+  ev->transferStage = true;
+  if (done) PR_CUDA(h, cudaLaunchHostFunc(stream, trampoline, ev));
+  h->memcpys.fetch_add(nMemcpy);
+  uint32_t f = h->inFlight.fetch_add(1) + 1, mx = h->maxInFlight.load();
+  while (f > mx && !h->maxInFlight.compare_exchange_weak(mx, f)) {}
   return PR_OK;
 }
 

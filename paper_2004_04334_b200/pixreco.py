@@ -104,6 +104,7 @@ SIGNATURES = {
     "pr_strerror": (c_char_p, [c_int]),
     "pr_last_cuda_error": (c_char_p, [c_void_p]),
     "pr_abi_version": (c_int, []),
+    "pr_transfer": (c_int, [c_void_p, c_uint32, c_void_p, pr_done_fn, c_void_p]),
     "pr_pool_create": (c_int, [c_int, c_int, c_uint64, POINTER(c_void_p)]),
     "pr_pool_alloc": (c_void_p, [c_void_p, c_size_t, c_void_p]),
     "pr_pool_free": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -239,6 +240,14 @@ class EventSlot:
         self._keep = keep
         s = getattr(stream, "cuda_stream", stream)
         return _check(lib().pr_acquire_batch(self.ptr, arr, len(events), c_void_p(s)), "pr_acquire_batch", self.owner.handle)
+
+    def transfer(self, want, stream=0, done=None) -> int:
+        """Transfer on demand: after a PR_OK produce, copy the outputs in ``want`` to pinned host memory
+        with exact-size DMA copies on ``stream``; the slot is in flight again until query/produce say PR_OK."""
+        cb = pr_done_fn(done) if done is not None else pr_done_fn()
+        self._keep_transfer = cb
+        s = getattr(stream, "cuda_stream", stream)
+        return _check(lib().pr_transfer(self.ptr, want, c_void_p(s), cb, None), "pr_transfer", self.owner.handle)
 
     def query(self) -> int:
         return _check(lib().pr_query(self.ptr), "pr_query", self.owner.handle)

@@ -42,6 +42,15 @@ def wait(slot, timeout=60.0):
         time.sleep(0.0002)
 
 
+def lib_code(fn):
+    """The pr_* code of a binding call that raises PixRecoError."""
+    from paper_2004_04334_b200 import pixreco
+    try:
+        return fn()
+    except pixreco.PixRecoError as e:
+        return e.code
+
+
 def test_acquire_returns_at_once_behind_a_long_queue(pr):
     """A ~100 ms spin kernel sits in front on the same stream: pr_acquire must still return in
     well under that, pr_query/pr_produce must say NOT_READY without waiting."""
@@ -216,6 +225,58 @@ def test_transfers_only_when_asked(pr):
         assert out.host("err_idx") is not None and out.host("cl_label") is None
         slot.release()
         assert p.stats()["kernel_launches"] == 7                            # + export kernel
+
+
+def test_transfer_on_demand_is_a_stage_of_its_own(pr):
+    """the copy to the host runs only when a consumer turns up, as an External-Worker stage of
+    its own: pr_transfer after pr_produce, exact-size DMA copies, completion by query or callback."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, 40), wl.make_event(1, 41), wl.Event(np.zeros(0, np.uint32), np.zeros(0, np.uint16), 1856)]
+    refs = [oracle.run(e.words, e.adc, e.n_modules, cal.gain, cal.pedestal) for e in evs]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        assert lib_code(lambda: slot.transfer(pr.PR_WANT_CLUSTERS)) == pr.PR_ERR_BAD_STATE          # nothing acquired
+        slot.acquire_batch([(to_dev(e.words), to_dev(e.adc)) for e in evs], stream=torch.cuda.Stream(), want=pr.PR_WANT_ERRORS)
+        wait(slot)
+        code, outs = slot.produce_batch(len(evs))
+        assert code == 0 and all(o.host("cl_label") is None and o.host("err_idx") is not None for o in outs)
+        m0 = p.stats()["memcpy_calls"]
+        fired = []
+        consumer = torch.cuda.Stream()                                    # a consumer's stream, not the producer's
+        slot.transfer(pr.PR_WANT_CLUSTERS | pr.PR_WANT_LABELS | pr.PR_WANT_ERRORS, stream=consumer, done=lambda u, st: fired.append(st))
+        wait(slot)
+        code, outs = slot.produce_batch(len(evs))
+        assert code == 0
+        # 19 arrays (clusters: 6 + mod_clus_start, labels: 2, per non-empty event; errors were mirrored already): more
+        # than four, so they are gathered on the device and leave with ONE copy (+ one for the gather table)
+        assert p.stats()["memcpy_calls"] - m0 == 2
+        for o, r in zip(outs, refs):
+            assert np.array_equal(o.host("cl_label"), r.cl_label) and np.array_equal(o.host("cl_size"), r.cl_size)
+            assert np.array_equal(o.host("cl_module"), r.cl_module) and np.array_equal(o.host("mod_clus_start"), r.mod_clus_start)
+            assert np.array_equal(o.host("cl_charge").view(np.uint32), r.cl_charge.view(np.uint32))
+            assert np.array_equal(o.host("cl_row").view(np.uint32), r.cl_row.view(np.uint32))
+            assert np.array_equal(o.host("cl_col").view(np.uint32), r.cl_col.view(np.uint32))
+            assert np.array_equal(o.host("label"), r.label) and np.array_equal(o.host("clus"), r.clus)
+            assert np.array_equal(o.host("err_idx"), r.err_idx) and o.host("charge") is None
+        t0 = time.time()
+        while not fired and time.time() - t0 < 10:
+            time.sleep(0.001)
+        assert fired == [0]
+        st = p.stats()
+        assert st["events_produced"] == len(evs) and st["events_in_flight"] == 0     # the stage does not count the events again
+        slot.release()
+        assert lib_code(lambda: slot.transfer(pr.PR_WANT_DIGIS)) == pr.PR_ERR_BAD_STATE             # released
+        # a single event and few arrays: plain exact-size copies, no kernel
+        slot.acquire(to_dev(evs[0].words), to_dev(evs[0].adc), want=0); wait(slot)
+        assert slot.produce()[0] == 0
+        s0 = p.stats()
+        slot.transfer(pr.PR_WANT_CHARGE | pr.PR_WANT_ERRORS); wait(slot)
+        code, out = slot.produce()
+        s1 = p.stats()
+        assert code == 0 and s1["memcpy_calls"] - s0["memcpy_calls"] == 3 and s1["kernel_launches"] == s0["kernel_launches"]
+        assert np.array_equal(out.host("charge").view(np.uint32), refs[0].charge.view(np.uint32))
+        assert np.array_equal(out.host("err_word"), refs[0].err_word) and np.array_equal(out.host("err_idx"), refs[0].err_idx)
+        slot.release()
 
 
 def test_argument_and_state_errors(pr):
