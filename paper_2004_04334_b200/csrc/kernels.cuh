@@ -1,10 +1,12 @@
 // kernels.cuh — sm_100a device code of the hot path (BASELINE.json north_star subsystem (2)).
 //
 //   k_unpack   a1+a2 fused: raw word decode, calibration, STABLE digi/error compaction with a
-//              single-pass decoupled look-back scan, modDigiStart, input-order check.
-//   k_cluster  a3+a4 fused: per-module 8-connected components (warp per module: hash look-up +
-//              label equivalence in shared memory; CTA per large module: bitmap + rank look-up +
-//              min-index union-find), exact cluster sums, cluster threshold, per-module numbering.
+//              single-pass decoupled look-back scan, modDigiStart, input-order check; TMA bulk
+//              loads into a shared-memory ring, staged SoA output written by TMA bulk stores.
+//   k_cluster  a3+a4 fused: per-module 8-connected components (one warp per pack of small modules:
+//              all in registers; per module of 33..256 digis: hash look-up + label equivalence in
+//              shared memory; CTA per large module: bitmap + rank look-up + min-index union-find),
+//              exact cluster sums, cluster threshold, per-module numbering.
 //   k_finalize event-wide dense cluster numbering, cluster SoA, modClusStart, counters to the host.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
 //
@@ -524,8 +526,9 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
 
 // ================================================================== k_cluster (a3 + a4)
 // Every module is an independent problem.  No unit of work waits for another one:
-//   warp path    a module with at most kWarpCap digis is clustered by ONE warp, with only
-//                __syncwarp between its phases: warp-private hash table (row,col) -> digi for the
+//   warp path    consecutive modules with at most 32 digis together are clustered in one pass by ONE
+//                warp, in registers (warp_pack).  A module of 33..kWarpCap digis is clustered by ONE warp with
+//                only __syncwarp between its phases: warp-private hash table (row,col) -> digi for the
 //                backward-neighbour look-ups (each found edge is recorded on both ends),
 //                label-equivalence rounds (min over neighbours, hook the old representative with
 //                atomicMin, pointer jumping) until stable, then per-cluster sums accumulated in
