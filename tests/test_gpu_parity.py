@@ -283,6 +283,30 @@ def test_batch_matches_single_events(pr):
         slot.release()
 
 
+@pytest.mark.parametrize("config,n_events", [(1, 64), (3, 48), (4, 1)])
+def test_full_size_launches_as_bench_times_them(pr, config, n_events):
+    """The launch configurations bench.py times, at BASELINE.json's full sizes: the 64-event configs[1] batch, a
+    configs[3] batch (48 of the 256 events: every event is compared in full), one whole configs[4] event
+    (12.4 M digis, dense path with the global workspace tier).  Every output array against the oracle."""
+    cal = wl.make_calib(config)
+    evs = [wl.make_event(config, 100 + e) for e in range(n_events)]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        dev = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+        if n_events > 1:
+            slot.acquire_batch(dev, stream=torch.cuda.Stream())
+        else:
+            slot.acquire(*dev[0], stream=torch.cuda.Stream())
+        wait(slot, timeout=300.0)
+        code, outs = slot.produce_batch(n_events)
+        assert code == 0
+        for e, out in zip(evs, outs):
+            ref = oracle_of(e, cal)
+            got = {f: out.to_numpy(f) for f in pr.VIEW_SPEC}
+            compare(out, ref, lambda f: got[f])
+        slot.release()
+
+
 @pytest.mark.parametrize("layout", ["one_span", "separate", "misaligned_span"])
 def test_host_input_batch_staging_paths(pr, layout):
     """Pinned host inputs of a batch: one dense span (staged by one copy per array), separately allocated
