@@ -69,6 +69,19 @@ def load_traffic(kernel):
         return None
 
 
+def load_issue(kernel, ms, sm_mhz, n_sm=148):
+    """Context for a kernel that is not HBM-bound: warp-instructions per launch (same ncu capture as `traffic`)
+    over the measured duration, against 4 schedulers x 1 warp-instruction per cycle per SM at the sampled clock."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            wi = json.load(f)["kernels"][kernel]["warp_inst_per_launch"]
+        peak = n_sm * 4 * (sm_mhz or 1965.0) * 1e6
+        return {"warp_inst_per_launch": wi, "achieved_per_s": wi / (ms * 1e-3), "peak_per_s": peak,
+                "frac": wi / (ms * 1e-3) / peak, "note": "instruction issue, not an algorithmic roofline"}
+    except Exception:
+        return None
+
+
 def load_peaks():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -488,6 +501,7 @@ def run_ours(args, rank, world):
                             "frac_of_8TBs_nominal": kern[dom]["gbs"] / 8000.0,
                             "algorithmic_bytes_per_launch": kern[dom]["bytes"], "ms_per_launch": kern[dom]["ms"],
                             "units_per_launch": f"{EVENTS_PER_STEP} events", "kernels": kern,
+                            "issue_slots": load_issue(dom, kern[dom]["ms"], clocks.get("sm_mhz")),
                             "chain": {"bytes_per_event": bchain, "gbs": bchain * value / world / 1e9,
                                       "frac": bchain * value / world / 1e9 / peak}}
         bt.close()
