@@ -40,6 +40,8 @@ constexpr int kLookBack = 8;                                         // predeces
 constexpr int kClusterThreads = 256;
 constexpr u32 kSmemDigis = 2048;      // modules with more digis use the global workspace tier
 constexpr u32 kSmemClusters = 512;    // likewise for per-cluster accumulators
+constexpr u32 kDenseDigis = 8192;     // the same tiers of k_dense (two CTAs per SM with their own, larger shared memory)
+constexpr u32 kDenseClusters = 512;
 
 // Per-event device counters (lives in the slot's control block, zeroed per acquire).
 struct DevCounters {
@@ -49,7 +51,8 @@ struct DevCounters {
 struct LaunchCtl {
   u32 modTicket, modDone;
   u64 tStart;                       // %globaltimer at the start of the acquire's first kernel
-  u32 pad[12];
+  u32 nBig, bigTicket;              // modules handed from k_cluster to k_dense, next one to take
+  u32 pad[10];
 };
 // What the host reads after completion (mapped pinned memory, written by the last block).
 struct HostCounters {
@@ -557,16 +560,29 @@ struct WarpRegion {                 // 5 KB of shared memory per warp
 };
 static_assert(sizeof(u32) * (kWarpTab - kWarpCap) + sizeof(uint2) * kWarpCap >= kAccRoots * 28, "accumulators must fit");
 
-__host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords) {
+__host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords, u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
   size_t w = (bitmapWords + 3) & ~3u;
-  return (size_t)w * 4 * 2 + (size_t)kSmemDigis * 4 * 2 + (size_t)kSmemClusters * (4 + 4 + 4 + 8 * 3);
+  return (size_t)w * 4 * 2 + (size_t)capDigis * 4 * 2 + (size_t)capClusters * (4 + 4 + 4 + 8 * 3);
 }
 __host__ __device__ inline size_t cluster_smem_bytes(u32 bitmapWords) {
   size_t dense = dense_smem_bytes(bitmapWords), warp = sizeof(WarpRegion) * (kClusterThreads / 32);
   return ((dense > warp ? dense : warp) + 15) & ~(size_t)15;
 }
 
-__device__ __forceinline__ u32 uf_find(const volatile u32* parent, u32 x) {
+// Root of x, halving the path on the way (a node's parent only ever moves to another ancestor in its set, so
+// concurrent finds and hooks stay consistent).  Only while unions are running: see uf_root.
+__device__ __forceinline__ u32 uf_find(volatile u32* parent, u32 x) {
+  u32 p = parent[x];
+  while (p != x) {
+    const u32 gp = parent[p];
+    if (gp != p) parent[x] = gp;
+    x = p; p = gp;
+  }
+  return x;
+}
+// Root of x without touching the forest: for the flattening pass, where a late halving store could
+// overwrite another thread's final root.
+__device__ __forceinline__ u32 uf_root(const volatile u32* parent, u32 x) {
   u32 p;
   while ((p = parent[x]) != x) x = p;
   return x;
@@ -871,23 +887,24 @@ struct DenseCtx {
 };
 
 __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32 s, u32 nn,
-                                            unsigned char* smemRaw, ClusterShared& sh, DenseCtx& cx) {
+                                            unsigned char* smemRaw, ClusterShared& sh, DenseCtx& cx,
+                                            u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
   const int tid = threadIdx.x, lane = tid & 31;
   const u32 bwPad = (g.bitmapWords + 3) & ~3u;
   u64* smS = reinterpret_cast<u64*>(smemRaw);
-  u64* smSx = smS + kSmemClusters;
-  u64* smSy = smSx + kSmemClusters;
-  u32* smBitmap = reinterpret_cast<u32*>(smSy + kSmemClusters);
+  u64* smSx = smS + capClusters;
+  u64* smSy = smSx + capClusters;
+  u32* smBitmap = reinterpret_cast<u32*>(smSy + capClusters);
   u32* smPrefix = smBitmap + bwPad;
   u32* smPerm = smPrefix + bwPad;
-  u32* smParent = smPerm + kSmemDigis;
-  u32* smRoot = smParent + kSmemDigis;
-  u32* smSize = smRoot + kSmemClusters;
-  int32_t* smKnum = reinterpret_cast<int32_t*>(smSize + kSmemClusters);
+  u32* smParent = smPerm + capDigis;
+  u32* smRoot = smParent + capDigis;
+  u32* smSize = smRoot + capClusters;
+  int32_t* smKnum = reinterpret_cast<int32_t*>(smSize + capClusters);
   u32* sScan = sh.scan;
   const u32 stride = g.stride;
 
-  const bool digiInSmem = nn <= kSmemDigis;
+  const bool digiInSmem = nn <= capDigis;
   u32* perm = digiInSmem ? smPerm : ev.wsPerm + s;
   u32* parent = digiInSmem ? smParent : ev.wsParent + s;
   cx.perm = perm; cx.parent = parent;
@@ -960,7 +977,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   // P5: flatten (roots are stable now)
   for (u32 i = tid; i < nn; i += kClusterThreads) {
     if (parent[i] == kInvalid) continue;
-    const u32 rt = uf_find(parent, i);
+    const u32 rt = uf_root(parent, i);
     if (rt != i) parent[i] = rt;
   }
   __syncthreads();
@@ -971,7 +988,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
     u32 c = 0;
     for (u32 i = lo; i < hi; ++i) c += (parent[i] == i);
     u32 run = block_excl_scan(c, sScan, &cx.nAll);
-    if (cx.nAll > kSmemClusters) {
+    if (cx.nAll > capClusters) {
       cx.root = ev.wsRoot + s; cx.csize = ev.wsSize + s; cx.knum = ev.wsKnum + s;
       cx.S = ev.wsS + s; cx.Sx = ev.wsSx + s; cx.Sy = ev.wsSy + s;
     }
@@ -1031,7 +1048,7 @@ __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 
 template <bool kSingle>
 __global__ void __launch_bounds__(kClusterThreads, 4)
 k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
-          LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+          LaunchCtl* __restrict__ lc, u32* __restrict__ bigList, const __grid_constant__ Geom g) {
   extern __shared__ __align__(16) unsigned char smemRaw[];
   __shared__ ClusterShared sh;
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -1049,6 +1066,10 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         const u32 s = ev.modDigiStart[m], t = ev.modDigiStart[m + 1];
         big = t >= s && t <= ev.cap && t - s > kWarpCap;
       }
+    }
+    if (bigList) {                                      // a launch full of large modules: k_dense takes them (larger tiers)
+      if (big) bigList[atomicAdd(&lc->nBig, 1u)] = gi;
+      continue;
     }
     if (tid == 0) sh.nBig = 0;
     __syncthreads();
@@ -1139,6 +1160,33 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       if (accK) atomicAdd(&ev.counters->nKept, accK);
       if (accA) atomicAdd(&ev.counters->nClustersAll, accA);
     }
+  }
+}
+
+// ================================================================== k_dense (a3 + a4 for launches full of large modules)
+// The dense path of k_cluster as a kernel of its own, for launches whose modules are large on average
+// (BASELINE.json configs[4]: 6.7k digis per module): two CTAs per SM with 8192 digis / 512 clusters
+// per module in shared memory instead of 2048 / 512, so the union-find of such a module never leaves
+// the SM.  k_cluster only collects the large modules in that case (bigList); CTAs take them by ticket.
+template <bool kSingle>
+__global__ void __launch_bounds__(kClusterThreads, 2)
+k_dense(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, LaunchCtl* __restrict__ lc,
+        const u32* __restrict__ bigList, const __grid_constant__ Geom g) {
+  extern __shared__ __align__(16) unsigned char smemRaw[];
+  __shared__ ClusterShared sh;
+  const u32 M = g.M, nBig = lc->nBig;
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) sh.nBig = atomicAdd(&lc->bigTicket, 1u);
+    __syncthreads();
+    const u32 t = sh.nBig;
+    if (t >= nBig) break;
+    const u32 gk = bigList[t], e = gk / M, m = gk - e * M;
+    const EvDesc& ev = kSingle ? single : batch[e];
+    const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
+    DenseCtx cx;
+    dense_count(ev, g, s, nn, smemRaw, sh, cx, kDenseDigis, kDenseClusters);
+    dense_stage(ev, m, s, nn, cx);
   }
 }
 

@@ -35,7 +35,8 @@ struct pr_handle {
   float2* dCalib = nullptr;
   CachingPool *devPool = nullptr, *hostPool = nullptr;
   int smCount = 0, clusterBlocksPerSM = 1, unpackBlocksPerSM = 1;
-  size_t clusterSmem = 0;
+  size_t clusterSmem = 0, denseSmem = 0;
+  int denseBlocksPerSM = 1;
   std::mutex mu;
   std::vector<pr_event*> slots;
   std::atomic<uint64_t> evAcquired{0}, evProduced{0}, words{0}, digis{0}, clusters{0}, launches{0}, memcpys{0}, callbacks{0};
@@ -226,7 +227,12 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     totalTiles += s.desc.nTiles;
   }
   const size_t grpPerEv = align_up((M + 31) / 32, 16);      // u32 per event
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + 4 * grpPerEv * n;
+  uint64_t totalWords = 0;
+  for (uint32_t k = 0; k < n; ++k) totalWords += ins[k].n_words;
+  // launches whose modules are large on average (configs[4]) hand their large modules to k_dense
+  const bool denseKernel = totalWords > (uint64_t)kWarpCap * M * n;
+  const size_t bigCap = denseKernel ? (size_t)(totalWords / (kWarpCap + 1) + 2) : 0;
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + 4 * grpPerEv * n + 4 * bigCap;
 
   // ---- buffers from the pools (steady state: cache hits only)
   if (ev->ctlBytes < ctlNeed) {
@@ -262,6 +268,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   LaunchCtl* lc = (LaunchCtl*)ctl;
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
   u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
+  u32* bigList = denseKernel ? (u32*)(tileState + totalTiles) + grpPerEv * n : nullptr;
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
   char *spanW = nullptr, *spanA = nullptr;
@@ -302,13 +309,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // k_cluster: persistent CTAs (dense scan + warp tickets).  A small launch gets one CTA per warp
   // ticket or per possible dense module (a dense module has more than kWarpCap digis).
   const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
-  uint64_t totalWords = 0;
-  for (uint32_t k = 0; k < n; ++k) totalWords += ins[k].n_words;
   const uint64_t warpTickets = (uint64_t)n * ((M + kModBatch - 1) / kModBatch), maxDense = totalWords / (kWarpCap + 1);
   const uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
   if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
   if (clusterGrid < 1) clusterGrid = 1;
+  uint32_t denseGrid = (uint32_t)(h->smCount * h->denseBlocksPerSM);
+  if (denseGrid > bigCap) denseGrid = bigCap ? (uint32_t)bigCap : 1u;
   // k_unpack: persistent CTAs striding over the tiles; never more than are co-resident (its look-back
   // waits on earlier tiles, which must therefore be running or done)
   uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
@@ -350,18 +357,20 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     const EvDesc& d = ev->sub[0].desc;
     k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, h->geom);
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, h->geom);
+    if (denseKernel) k_dense<true><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, h->geom);
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, h->geom);
+    if (denseKernel) k_dense<false><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
   }
-  nLaunch += 3;
+  nLaunch += denseKernel ? 4 : 3;
   PR_CUDA(h, cudaGetLastError());
   if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
   ev->exported = want != 0;
@@ -520,6 +529,14 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
       cudaFuncSetAttribute(k_cluster<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess) {
     cudaGetLastError(); return fail(PR_ERR_CUDA);
   }
+  h->denseSmem = dense_smem_bytes(g.bitmapWords, kDenseDigis, kDenseClusters);
+  if (cudaFuncSetAttribute(k_dense<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->denseSmem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_dense<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->denseSmem) != cudaSuccess) {
+    cudaGetLastError(); return fail(PR_ERR_CUDA);
+  }
+  int dps = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&dps, k_dense<true>, kClusterThreads, h->denseSmem) != cudaSuccess) { cudaGetLastError(); dps = 1; }
+  h->denseBlocksPerSM = dps < 1 ? 1 : dps;
   int bps = 1;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_cluster<true>, kClusterThreads, h->clusterSmem) != cudaSuccess) { cudaGetLastError(); bps = 1; }
   h->clusterBlocksPerSM = bps < 1 ? 1 : bps;
