@@ -7,6 +7,8 @@
 //              all in registers; per module of 33..256 digis: hash look-up + label equivalence in
 //              shared memory; CTA per large module: bitmap + rank look-up + min-index union-find),
 //              exact cluster sums, cluster threshold, per-module numbering.
+//   k_dense    the large-module path of k_cluster as a kernel of its own (larger shared-memory tiers), used
+//              by launches whose modules are large on average.
 //   k_finalize event-wide dense cluster numbering, cluster SoA, modClusStart, counters to the host.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
 //

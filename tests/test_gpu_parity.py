@@ -367,6 +367,7 @@ def _blob_module(rng, m, n, dup_frac=0.0, box=40):
     ([256] * 9 + [257] * 3 + [40] * 30, 0.0),
     ([17, 100, 256, 250, 257, 600, 20, 20], 0.15),
     ([3] * 700, 0.0),                                    # hundreds of modules per 512-digi window
+    ([3000, 5, 40, 300, 9000, 0, 700, 33, 8192, 8193], 0.1),   # large on average: the large ones go to k_dense (both of its tiers)
 ])
 def test_module_size_boundaries(pr, sizes, dup):
     """Modules on both sides of every path boundary of k_cluster (warp path up to 256 digis, dense
