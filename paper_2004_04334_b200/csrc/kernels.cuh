@@ -550,7 +550,8 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
 constexpr u32 kWarpCap = 256;                    // warp path: modules with at most this many digis
 constexpr u32 kWarpTab = 2 * kWarpCap;           // hash slots per warp (load <= 1/4 up to 128 digis, <= 1/2 beyond)
 constexpr u32 kAccRoots = 96;                    // clusters accumulated per pass over a module
-constexpr u32 kModBatch = 4;                     // modules per warp ticket (small tickets: a short tail; 8 was 6 % slower, 16 17 %)
+constexpr u32 kModBatch = 4;                     // most modules per warp ticket (small tickets: a short tail; 8 was 6 % slower, 16 17 %);
+                                                 // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
 constexpr u32 kEmpty = 0xFFFFFFFFu;
 constexpr u32 kNoKey = 0xFFFFFFFFu;
 constexpr u32 kNoRank = 0xFFFFu;
@@ -1050,7 +1051,7 @@ __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 
 template <bool kSingle>
 __global__ void __launch_bounds__(kClusterThreads, 4)
 k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv,
-          LaunchCtl* __restrict__ lc, u32* __restrict__ bigList, const __grid_constant__ Geom g) {
+          LaunchCtl* __restrict__ lc, u32* __restrict__ bigList, u32 modBatch, const __grid_constant__ Geom g) {
   extern __shared__ __align__(16) unsigned char smemRaw[];
   __shared__ ClusterShared sh;
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -1090,15 +1091,15 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     __syncthreads();
   }
 
-  // ---- phase 2: warp path.  A ticket is a batch of kModBatch consecutive modules of one event.
+  // ---- phase 2: warp path.  A ticket is a batch of modBatch (1, 2 or 4) consecutive modules of one event.
   WarpRegion& wr = reinterpret_cast<WarpRegion*>(smemRaw)[warp];
-  const u32 bpe = (M + kModBatch - 1) / kModBatch, nTickets = nEv * bpe;
+  const u32 bpe = (M + modBatch - 1) / modBatch, nTickets = nEv * bpe;
   for (;;) {
     u32 t = 0;
     if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
     t = __shfl_sync(0xFFFFFFFFu, t, 0);
     if (t >= nTickets) break;
-    const u32 e = t / bpe, m0 = (t - e * bpe) * kModBatch, nm = min(kModBatch, M - m0);
+    const u32 e = t / bpe, m0 = (t - e * bpe) * modBatch, nm = min(modBatch, M - m0);
     const EvDesc& ev = kSingle ? single : batch[e];
     if (ev.counters->status & 1u) continue;
     const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
@@ -1157,7 +1158,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       }
       k = k2;
     }
-    if (lane == 0 && accG) atomicAdd(&ev.grpCount[m0 / 32u], accG);     // kModBatch divides 32: one group per ticket
+    if (lane == 0 && accG) atomicAdd(&ev.grpCount[m0 / 32u], accG);     // modBatch divides 32: one group per ticket
     if (lane == 0) {
       if (accK) atomicAdd(&ev.counters->nKept, accK);
       if (accA) atomicAdd(&ev.counters->nClustersAll, accA);

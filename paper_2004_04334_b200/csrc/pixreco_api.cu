@@ -309,7 +309,10 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // k_cluster: persistent CTAs (dense scan + warp tickets).  A small launch gets one CTA per warp
   // ticket or per possible dense module (a dense module has more than kWarpCap digis).
   const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
-  const uint64_t warpTickets = (uint64_t)n * ((M + kModBatch - 1) / kModBatch), maxDense = totalWords / (kWarpCap + 1);
+  // tickets of 4 modules when there are plenty, of 2 or 1 when the launch is small (a single event): every warp gets work
+  const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
+  const uint32_t modBatch = (uint64_t)n * M >= 4 * warpsResident ? kModBatch : (uint64_t)n * M >= 2 * warpsResident ? 2u : 1u;
+  const uint64_t warpTickets = ((uint64_t)n * ((M + modBatch - 1) / modBatch) + 7) / 8, maxDense = totalWords / (kWarpCap + 1);
   const uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
   if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
@@ -357,7 +360,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     const EvDesc& d = ev->sub[0].desc;
     k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, h->geom);
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<true><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
@@ -365,7 +368,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, h->geom);
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<false><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
