@@ -1203,11 +1203,13 @@ constexpr u32 kFinMods = 32;
 static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
 template <bool kSingle>
 __global__ void __launch_bounds__(256)
-k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent,
+k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent, u32 splits,
            LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8];
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
-  const u32 e = blockIdx.x / unitsPerEvent, u = blockIdx.x - e * unitsPerEvent;
+  // `splits` CTAs share one (event, group) when events are huge: slice sp of the group's digis and clusters
+  const u32 unit = blockIdx.x / splits, sp = blockIdx.x - unit * splits;
+  const u32 e = unit / unitsPerEvent, u = unit - e * unitsPerEvent;
   const EvDesc& ev = kSingle ? single : batch[e];
   const u32 m0 = u * kFinMods, m1 = min(m0 + kFinMods, M);
   if (!(ev.counters->status & 1u)) {
@@ -1223,11 +1225,13 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
       if (lane == 31) sDigi[32] = ev.modDigiStart[min(m0 + 32u, M)];
     }
     __syncthreads();
-    for (u32 m = m0 + tid; m < m1; m += 256) ev.modClusStart[m] = sStart[m - m0];
-    if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
+    if (sp == 0) {
+      for (u32 m = m0 + tid; m < m1; m += 256) ev.modClusStart[m] = sStart[m - m0];
+      if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
+    }
     const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
     if (d0 <= d1 && d1 <= ev.cap) {
-      for (u32 dd = d0 + tid; dd < d1; dd += 4u * 256u) {     // four independent digis per thread and trip
+      for (u32 dd = d0 + sp * 1024u + tid; dd < d1; dd += splits * 1024u) {     // four independent digis per thread and trip
         int32_t c[4]; u32 md[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -1239,7 +1243,7 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
         for (int k = 0; k < 4; ++k)
           if (c[k] >= 0) ev.clus[dd + 256u * k] = (int32_t)(sStart[min(md[k] - m0, kFinMods - 1)] + (u32)c[k]);
       }
-      for (u32 o = sStart[0] + tid; o < sStart[32]; o += 256) {
+      for (u32 o = sStart[0] + sp * 256u + tid; o < sStart[32]; o += splits * 256u) {
         u32 li = 0;
 #pragma unroll
         for (u32 step = 16; step > 0; step >>= 1)
@@ -1257,7 +1261,7 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
   }
   // The CTA of the event's last module group publishes the event's counters to mapped pinned host memory: all
   // the others were final when this kernel started, nClusters is this CTA's own result.
-  if (m1 == M && tid == 0) {
+  if (m1 == M && sp == 0 && tid == 0) {
     const DevCounters* c = ev.counters;
     const u32 status = c->status;
     HostCounters h;

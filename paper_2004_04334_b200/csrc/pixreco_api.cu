@@ -317,6 +317,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
   if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
   if (clusterGrid < 1) clusterGrid = 1;
+  // k_finalize: one CTA per (event, 32 modules); huge events get several CTAs per group (about 8k words each)
+  uint32_t finSplits = (uint32_t)(totalWords / ((uint64_t)n * unitsPerEvent * 8192) + 1);
+  if (finSplits > 64) finSplits = 64;
   uint32_t denseGrid = (uint32_t)(h->smCount * h->denseBlocksPerSM);
   if (denseGrid > bigCap) denseGrid = bigCap ? (uint32_t)bigCap : 1u;
   // k_unpack: persistent CTAs striding over the tiles; never more than are co-resident (its look-back
@@ -363,7 +366,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<true><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<true><<<unitsPerEvent, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, lc, h->geom);
+    k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, lc, h->geom);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
@@ -371,7 +374,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<false><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<false><<<n * unitsPerEvent, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, lc, h->geom);
+    k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, finSplits, lc, h->geom);
   }
   nLaunch += denseKernel ? 4 : 3;
   PR_CUDA(h, cudaGetLastError());
