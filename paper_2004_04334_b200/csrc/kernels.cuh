@@ -128,8 +128,9 @@ __device__ __forceinline__ u32 warp_incl_scan(u32 v, int lane) {
   return v;
 }
 
-// Block-wide exclusive scan of one value per thread (blockDim = 256); returns exclusive prefix,
-// *total = block sum.  `sw` is 8 words of shared scratch.  Contains two __syncthreads.
+// Block-wide exclusive scan of one value per thread (blockDim = 32 * kWarps); returns exclusive prefix,
+// *total = block sum.  `sw` is kWarps words of shared scratch.  Contains two __syncthreads.
+template <int kWarps = 8>
 __device__ __forceinline__ u32 block_excl_scan(u32 v, u32* sw, u32* total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   u32 incl = warp_incl_scan(v, lane);
@@ -138,7 +139,7 @@ __device__ __forceinline__ u32 block_excl_scan(u32 v, u32* sw, u32* total) {
   __syncthreads();
   u32 base = 0, tot = 0;
 #pragma unroll
-  for (int w = 0; w < 8; ++w) {
+  for (int w = 0; w < kWarps; ++w) {
     u32 s = sw[w];
     if (w < warp) base += s;
     tot += s;
@@ -604,7 +605,7 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
 }
 
 struct ClusterShared {
-  u32 scan[8];
+  u32 scan[16];
   u32 nBig, big[kClusterThreads];
 };
 
@@ -889,6 +890,7 @@ struct DenseCtx {
   u32 nAll, nKept;
 };
 
+template <u32 kT = kClusterThreads>
 __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32 s, u32 nn,
                                             unsigned char* smemRaw, ClusterShared& sh, DenseCtx& cx,
                                             u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
@@ -914,12 +916,12 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   cx.root = smRoot; cx.csize = smSize; cx.knum = smKnum; cx.S = smS; cx.Sx = smSx; cx.Sy = smSy;
 
   // P0: clear the occupancy bitmap, init perm
-  for (u32 i = tid; i < g.bitmapWords; i += kClusterThreads) smBitmap[i] = 0;
-  for (u32 i = tid; i < nn; i += kClusterThreads) perm[i] = kInvalid;
+  for (u32 i = tid; i < g.bitmapWords; i += kT) smBitmap[i] = 0;
+  for (u32 i = tid; i < nn; i += kT) perm[i] = kInvalid;
   __syncthreads();
   // P1: kept flag (A8: q >= pixThr) and occupancy bits at padded coordinates (row+1, col+1)
   u32 myKept = 0;
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     const float q = ev.charge[s + i];
     const bool kept = q >= g.pixThr;
     parent[i] = kept ? i : kInvalid;
@@ -933,18 +935,18 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
   // P2: exclusive popcount prefix per bitmap word (contiguous chunk per thread)
   {
-    const u32 per = (g.bitmapWords + kClusterThreads - 1) / kClusterThreads;
+    const u32 per = (g.bitmapWords + kT - 1) / kT;
     const u32 lo = min(tid * per, g.bitmapWords), hi = min(lo + per, g.bitmapWords);
     u32 sum = 0;
     for (u32 i = lo; i < hi; ++i) sum += __popc(smBitmap[i]);
     u32 tot;
-    u32 run = block_excl_scan(sum, sScan, &tot);
+    u32 run = block_excl_scan<kT / 32>(sum, sScan, &tot);
     for (u32 i = lo; i < hi; ++i) { smPrefix[i] = run; run += __popc(smBitmap[i]); }
   }
   if (lane == 0 && myKept) atomicAdd(&ev.counters->nKept, myKept);
   __syncthreads();
   // P3: owner of each occupied pixel = the minimum digi index on it (duplicates, A6)
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     if (parent[i] == kInvalid) continue;
     const u32 b = ev.col[s + i] + 1u, wd = (ev.row[s + i] + 1u) * stride + (b >> 5);
     const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
@@ -953,7 +955,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
   // P4: unions with the backward neighbours (W, NW, N, NE), decision tree:
   //     N ? {N} : { NE?, W ? {W} : NW? }   — spans every 8-adjacency once all pixels did it.
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     if (parent[i] == kInvalid) continue;
     const u32 prow = ev.row[s + i] + 1u, b = ev.col[s + i] + 1u;
     const u32 wd = prow * stride + (b >> 5);
@@ -978,7 +980,7 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   }
   __syncthreads();
   // P5: flatten (roots are stable now)
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     if (parent[i] == kInvalid) continue;
     const u32 rt = uf_root(parent, i);
     if (rt != i) parent[i] = rt;
@@ -986,11 +988,11 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
   // P6: ordinal of every root in ascending index (= ascending label) order -> perm[root]
   {
-    const u32 per = (nn + kClusterThreads - 1) / kClusterThreads;
+    const u32 per = (nn + kT - 1) / kT;
     const u32 lo = min(tid * per, nn), hi = min(lo + per, nn);
     u32 c = 0;
     for (u32 i = lo; i < hi; ++i) c += (parent[i] == i);
-    u32 run = block_excl_scan(c, sScan, &cx.nAll);
+    u32 run = block_excl_scan<kT / 32>(c, sScan, &cx.nAll);
     if (cx.nAll > capClusters) {
       cx.root = ev.wsRoot + s; cx.csize = ev.wsSize + s; cx.knum = ev.wsKnum + s;
       cx.S = ev.wsS + s; cx.Sx = ev.wsSx + s; cx.Sy = ev.wsSy + s;
@@ -999,10 +1001,10 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
       if (parent[i] == i) { perm[i] = run; cx.root[run] = i; ++run; }
   }
   // P7: zero the accumulators
-  for (u32 c = tid; c < cx.nAll; c += kClusterThreads) { cx.S[c] = 0; cx.Sx[c] = 0; cx.Sy[c] = 0; cx.csize[c] = 0; }
+  for (u32 c = tid; c < cx.nAll; c += kT) { cx.S[c] = 0; cx.Sx[c] = 0; cx.Sy[c] = 0; cx.csize[c] = 0; }
   __syncthreads();
   // P8: exact fixed-point sums (A9): qf = q * 2^14 is an integer for every kept digi
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     const u32 p = parent[i];
     if (p == kInvalid) continue;
     const u32 c = perm[p];
@@ -1015,26 +1017,27 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
   // P9: cluster threshold (A8, A9) and local numbering of kept clusters
   {
-    const u32 per = (cx.nAll + kClusterThreads - 1) / kClusterThreads;
+    const u32 per = (cx.nAll + kT - 1) / kT;
     const u32 lo = min(tid * per, cx.nAll), hi = min(lo + per, cx.nAll);
     u32 c = 0;
     for (u32 k = lo; k < hi; ++k) c += ((i64)cx.S[k] >= g.clusThrFixed);
-    u32 run = block_excl_scan(c, sScan, &cx.nKept);
+    u32 run = block_excl_scan<kT / 32>(c, sScan, &cx.nKept);
     for (u32 k = lo; k < hi; ++k) cx.knum[k] = ((i64)cx.S[k] >= g.clusThrFixed) ? (int32_t)run++ : -1;
   }
   __syncthreads();
 }
 
+template <u32 kT = kClusterThreads>
 __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 nn, const DenseCtx& cx) {
   const int tid = threadIdx.x;
-  for (u32 k = tid; k < cx.nAll; k += kClusterThreads) {
+  for (u32 k = tid; k < cx.nAll; k += kT) {
     const int32_t kn = cx.knum[k];
     if (kn < 0) continue;
     const u32 o = s + (u32)kn;                       // kn <= k < nn: inside the module's own range
     ev.stS[o] = __ll2double_rn((i64)cx.S[k]); ev.stSx[o] = __ll2double_rn((i64)cx.Sx[k]); ev.stSy[o] = __ll2double_rn((i64)cx.Sy[k]);
     ev.stLabel[o] = s + cx.root[k]; ev.stSize[o] = cx.csize[k];
   }
-  for (u32 i = tid; i < nn; i += kClusterThreads) {
+  for (u32 i = tid; i < nn; i += kT) {
     const u32 p = cx.parent[i];
     u32 lab = kInvalid; int32_t cl = -1;
     if (p != kInvalid) { lab = s + p; cl = cx.knum[cx.perm[p]]; }
@@ -1171,8 +1174,9 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
 // (BASELINE.json configs[4]: 6.7k digis per module): two CTAs per SM with 8192 digis / 512 clusters
 // per module in shared memory instead of 2048 / 512, so the union-find of such a module never leaves
 // the SM.  k_cluster only collects the large modules in that case (bigList); CTAs take them by ticket.
+constexpr u32 kDenseThreads = 512;
 template <bool kSingle>
-__global__ void __launch_bounds__(kClusterThreads, 2)
+__global__ void __launch_bounds__(kDenseThreads, 2)
 k_dense(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, LaunchCtl* __restrict__ lc,
         const u32* __restrict__ bigList, const __grid_constant__ Geom g) {
   extern __shared__ __align__(16) unsigned char smemRaw[];
@@ -1188,8 +1192,8 @@ k_dense(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch,
     const EvDesc& ev = kSingle ? single : batch[e];
     const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
     DenseCtx cx;
-    dense_count(ev, g, s, nn, smemRaw, sh, cx, kDenseDigis, kDenseClusters);
-    dense_stage(ev, m, s, nn, cx);
+    dense_count<kDenseThreads>(ev, g, s, nn, smemRaw, sh, cx, kDenseDigis, kDenseClusters);
+    dense_stage<kDenseThreads>(ev, m, s, nn, cx);
   }
 }
 

@@ -364,7 +364,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
-    if (denseKernel) k_dense<true><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
+    if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, lc, h->geom);
   } else {
@@ -372,7 +372,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, modBatch, h->geom);
-    if (denseKernel) k_dense<false><<<denseGrid, kClusterThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
+    if (denseKernel) k_dense<false><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
     if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
     k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, finSplits, lc, h->geom);
   }
@@ -541,7 +541,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     cudaGetLastError(); return fail(PR_ERR_CUDA);
   }
   int dps = 1;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&dps, k_dense<true>, kClusterThreads, h->denseSmem) != cudaSuccess) { cudaGetLastError(); dps = 1; }
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&dps, k_dense<true>, kDenseThreads, h->denseSmem) != cudaSuccess) { cudaGetLastError(); dps = 1; }
   h->denseBlocksPerSM = dps < 1 ? 1 : dps;
   int bps = 1;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_cluster<true>, kClusterThreads, h->clusterSmem) != cudaSuccess) { cudaGetLastError(); bps = 1; }
