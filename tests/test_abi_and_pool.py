@@ -62,6 +62,23 @@ def test_create_rejects_bad_arguments_without_a_device():
     assert not h.value
 
 
+def test_null_slots_are_rejected_without_a_device():
+    """Every slot-level entry point checks its handle before touching CUDA."""
+    lib = pr.lib()
+    out = pr.pr_output()
+    inp = pr.pr_input(None, None, 0, pr.PR_MEM_DEVICE, 0, 0, pr.pr_done_fn(), None)
+    assert lib.pr_acquire(None, ctypes.byref(inp), None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_acquire_batch(None, ctypes.byref(inp), 1, None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_query(None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_produce(None, ctypes.byref(out)) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_release(None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_transfer(None, pr.PR_WANT_CLUSTERS, None, pr.pr_done_fn(), None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_stream_wait_event(None, None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_event_destroy(None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_destroy(None) == pr.PR_ERR_INVALID_ARG
+    assert not lib.pr_event_cuda_event(None)
+
+
 # ------------------------------------------------------------------ allocator on the fake backend
 class Pool:
     def __init__(self, max_cached=0):
