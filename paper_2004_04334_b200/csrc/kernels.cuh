@@ -1096,13 +1096,20 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
 
   // ---- phase 2: warp path.  A ticket is a batch of modBatch (1, 2 or 4) consecutive modules of one event.
   WarpRegion& wr = reinterpret_cast<WarpRegion*>(smemRaw)[warp];
-  const u32 bpe = (M + modBatch - 1) / modBatch, nTickets = nEv * bpe;
+  // Tickets shrink towards the end of a large launch (modBatch 4): the first nEvA events are handed out four
+  // modules at a time, the next nEvB events two at a time, the rest one by one, so that the last tickets are short.
+  const u32 bpe = (M + modBatch - 1) / modBatch, bpeB = (M + 1u) / 2u;
+  const u32 nEvA = modBatch == 4u ? nEv - nEv / 4u : nEv, nEvB = modBatch == 4u ? (nEv - nEvA + 1u) / 2u : 0u;
+  const u32 tA = nEvA * bpe, tB = tA + nEvB * bpeB, nTickets = tB + (nEv - nEvA - nEvB) * M;
   for (;;) {
     u32 t = 0;
     if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
     t = __shfl_sync(0xFFFFFFFFu, t, 0);
     if (t >= nTickets) break;
-    const u32 e = t / bpe, m0 = (t - e * bpe) * modBatch, nm = min(modBatch, M - m0);
+    u32 e, m0, nm;
+    if (t < tA) { e = t / bpe; m0 = (t - e * bpe) * modBatch; nm = min(modBatch, M - m0); }
+    else if (t < tB) { const u32 u = t - tA; e = u / bpeB; m0 = (u - e * bpeB) * 2u; nm = min(2u, M - m0); e += nEvA; }
+    else { const u32 u = t - tB; e = u / M; m0 = u - e * M; nm = 1u; e += nEvA + nEvB; }
     const EvDesc& ev = kSingle ? single : batch[e];
     if (ev.counters->status & 1u) continue;
     const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
