@@ -480,24 +480,16 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         if (bad) atomicOr(&e.counters->status, 1u);            // PR_STATUS_INPUT_ORDER
       }
       // modDigiStart[m] for the modules that begin in this tile (or are skipped by it): the number of staged
-      // digis with module < m (the staged modules ascend unless the order check fired).  First the warp
-      // segments that lie entirely below m (wmax <= m), then a 4-ary search inside the first one that
-      // does not.  Module carry1 + 8 * lane + warp goes to this thread: every warp gets its share.
+      // digis with module < m (the staged modules ascend unless the order check fired).  Warp w resolves the
+      // modules that are new in its own 256-word segment, [max module + 1 before it, max module + 1 in it), by a
+      // 4-ary search inside the segment: every warp gets its share.
       if (n) {
-        const u32 mLast = sh.sModule[hi - 1u];
-        u32 sc[8], sm[8];
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { sc[w] = __shfl_sync(0xFFFFFFFFu, c8, w); sm[w] = __shfl_sync(0xFFFFFFFFu, m8, w); }
-        for (u32 m = carry1 + 8u * lane + warp; m <= mLast; m += kUnpackThreads) {
-          u32 pos = 0, len = 0;
-          bool open = true;
-#pragma unroll
-          for (int w = 0; w < 8; ++w) {
-            if (open && sm[w] <= m) pos += sc[w];
-            else if (open) { open = false; len = sc[w]; }
-          }
-          // invariant: digis [0, pos) are < m, digi pos + len (if inside the segment) is >= m
-          const u16* base = sh.sModule + lo;
+        const u32 prev1 = max(carry1, __reduce_max_sync(0xFFFFFFFFu, lane < warp ? m8 : 0u));
+        const u32 wbase = __reduce_add_sync(0xFFFFFFFFu, lane < warp ? c8 : 0u);
+        const u32 cntW = __shfl_sync(0xFFFFFFFFu, c8, warp), mx1W = __shfl_sync(0xFFFFFFFFu, m8, warp);
+        const u16* base = sh.sModule + lo + wbase;
+        for (u32 m = prev1 + lane; m < mx1W; m += 32u) {
+          u32 pos = 0, len = cntW;                             // digis [0, pos) of the segment are < m; the answer is < pos + len
 #pragma unroll
           for (u32 q = 64u; q; q >>= 2) {                      // len <= 256: quarters of 64, 16, 4, 1
             u32 adv = 0;
@@ -507,7 +499,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
             pos += adv * q;
             len = min(len - adv * q, q);
           }
-          e.modDigiStart[m] = g0 + pos;
+          e.modDigiStart[m] = g0 + wbase + pos;
         }
       }
       // the event's last tile closes modDigiStart and the counters
