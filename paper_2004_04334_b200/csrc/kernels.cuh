@@ -338,14 +338,27 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       { TR_T(t0); mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u); if (warp == 0) TR_ADD(1, t0); }
       const u32* wseg = sh.words[slot] + 256u * warp + lane;
       u32 cnt = 0, mx = 0, myb = 0;
+      const u32 inWarp = nIn > 256u * warp ? nIn - 256u * warp : 0u;      // words of this warp's segment that exist
+      if (inWarp >= 256u) {                                    // the common case: no range test per word
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        const u32 x = wseg[32 * j];
-        const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC && 256u * warp + 32u * j + lane < nIn;
-        const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
-        cnt += (u32)__popc(b);
-        if (ok) mx = max(mx, x);                               // a digi's word has bit 31 clear: max word = max module
-        if ((int)lane == j) myb = b;
+        for (int j = 0; j < 8; ++j) {
+          const u32 x = wseg[32 * j];
+          const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC;
+          const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
+          cnt += (u32)__popc(b);
+          if (ok) mx = max(mx, x);                             // a digi's word has bit 31 clear: max word = max module
+          if ((int)lane == j) myb = b;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const u32 x = wseg[32 * j];
+          const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC && 32u * j + lane < inWarp;
+          const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
+          cnt += (u32)__popc(b);
+          if (ok) mx = max(mx, x);
+          if ((int)lane == j) myb = b;
+        }
       }
       if (lane < 8u) sh.bal[slot][warp][lane] = myb;
       mx = __reduce_max_sync(0xFFFFFFFFu, mx);
