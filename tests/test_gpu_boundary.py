@@ -52,7 +52,7 @@ def lib_code(fn):
 
 
 def test_acquire_returns_at_once_behind_a_long_queue(pr):
-    """A ~100 ms spin kernel sits in front on the same stream: pr_acquire must still return in
+    """A ~300 ms spin kernel sits in front on the same stream: pr_acquire must still return in
     well under that, pr_query/pr_produce must say NOT_READY without waiting."""
     ev, cal = wl.make_event(1, 0), wl.make_calib(1)
     with pr.PixReco(cal.gain, cal.pedestal, max_words_hint=60000, max_events_in_flight=8) as p:
@@ -62,7 +62,7 @@ def test_acquire_returns_at_once_behind_a_long_queue(pr):
         for sl, s in zip(slots, streams):          # warm every slot (ctl buffers, pool bins)
             sl.acquire(w, a, stream=s); wait(sl); sl.produce(); sl.release()
         torch.cuda.synchronize()
-        spin_cycles = int(0.1 * 1.5e9)
+        spin_cycles = int(0.3 * 2.0e9)                # ~300 ms at the B200's 1.97 GHz
         for s in streams:
             with torch.cuda.stream(s):
                 torch.cuda._sleep(spin_cycles)
@@ -75,8 +75,9 @@ def test_acquire_returns_at_once_behind_a_long_queue(pr):
         codes = [sl.produce()[0] for sl in slots]
         t_poll = time.perf_counter() - t0
         assert states == [pr.PR_NOT_READY] * 8 and codes == [pr.PR_NOT_READY] * 8
-        assert t_acq < 0.02, f"8 acquires took {t_acq * 1e3:.2f} ms behind a 100 ms queue"
-        assert t_poll < 0.01
+        # typically 0.2 ms and 0.05 ms; the slack is for a cold box (first process after boot)
+        assert t_acq < 0.05, f"8 acquires took {t_acq * 1e3:.2f} ms behind a 300 ms queue"
+        assert t_poll < 0.05
         assert slots[0].release() == pr.PR_NOT_READY            # nothing is released while in flight
         with pytest.raises(pr.PixRecoError):                    # acquire on a busy slot
             slots[0].acquire(w, a, stream=streams[0])
