@@ -1,0 +1,355 @@
+// k_unpack.cuh — a1 + a2: raw words -> digis with calibration, stable compaction (TMA ring, count-ahead, look-back)
+// Part of kernels.cuh (include that, not this file).
+#pragma once
+#include "common.cuh"
+
+namespace pixreco {
+
+// ================================================================== k_unpack (a1 + a2)
+// Persistent CTAs; CTA b takes tiles b, b + gridDim.x, ... of the launch (a tile = kTileWords
+// consecutive words of one event; the grid never exceeds what is co-resident, because the
+// look-back reads states published by CTAs that must be running).  "Local tile k" below is the
+// k-th tile of this CTA.  Per iteration i the CTA does, with two barriers:
+//   load    (end of iteration i)  one thread issues TMA bulk copies (cp.async.bulk, completion on an
+//           mbarrier) of tile i + kRawSlots into the ring slot tile i just vacated: raw words and
+//           ADC values reach shared memory without passing through registers
+//   count   tile i + kCountAhead: validity (A2, A3) of every word, one ballot per 32 words kept in
+//           shared memory, per-warp digi counts; the tile's aggregate (count, max module + 1) is
+//           PUBLISHED kCountAhead iterations before the tile is written, so when a successor looks
+//           back, the aggregate has long been there: no CTA waits for the progress of another one
+//   scatter tile i: its event-global digi offset g0 is known (look-back resolved in iteration
+//           i - 1).  Warp w owns words [256w, 256w + 256) of the tile, lane l word 32j + l of row j:
+//           position = g0 + warp prefix + row prefix + popc(ballot below lane).  The digi is stored
+//           in FINAL form (module,row,col,adc u16; wordIdx u32; charge f32 = fmaf, A7) into six
+//           shared-memory arrays at index 8 + (g0 & 7) + position, i.e. with the 16-byte phase of
+//           its global destination; error words (rare) go straight to global memory
+//   look-back (warp 0) for tile i + 1: loads issued before the scatter, resolved after it
+//   store   one thread issues six TMA bulk stores of the 16-byte-aligned middle of the staged
+//           arrays; sixteen lanes store the up-to-7 head and tail elements; all threads scan the
+//           staged module array for module boundaries (modDigiStart) and order violations (A5)
+// Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
+constexpr int kUnpackCtasPerSM = 2;
+constexpr int kRawSlots = 4;                      // raw tiles in the shared-memory ring
+constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
+constexpr int kDescRing = 8;                      // descriptor ring (batch), power of two >= kRawSlots + 2
+constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
+static_assert(kCountAhead >= 1 && kCountAhead <= kRawSlots - 2, "a raw tile needs a full iteration to arrive before it is counted");
+static_assert(kRawSlots + 2 <= kDescRing, "descriptor ring too small");
+
+struct __align__(128) UnpackShared {
+  u32 words[kRawSlots][kTileWords];               // raw ring (TMA destination)
+  u16 adc[kRawSlots][kTileWords];
+  u16 sModule[kStageElems], sRow[kStageElems], sCol[kStageElems], sAdc[kStageElems];   // staging (TMA source)
+  u32 sWordIdx[kStageElems];
+  float sCharge[kStageElems];
+  u64 full[kRawSlots];                            // mbarriers: raw slot filled
+  u32 bal[kRawSlots][8][8];                       // [slot][warp][row] validity ballots
+  u32 wcnt[kRawSlots][8], wmax[kRawSlots][8];     // per warp: digis, max(module)+1
+  u32 g0[2], carry1[2];                           // look-back result of local tile k at [k & 1]
+  u32 desc[kDescRing][32];                        // batch: first 128 bytes of the tiles' event descriptors
+};
+
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u64* bar, u32 count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
+  u32 ok;
+  do {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void bulk_load(void* dstSmem, const void* srcGlobal, u32 bytes, u64* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dstSmem)), "l"(__cvta_generic_to_global(srcGlobal)), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* dstGlobal, const void* srcSmem, u32 bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               ::"l"(__cvta_generic_to_global(dstGlobal)), "r"(smem_u32(srcSmem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+#ifdef PIXRECO_TRACE
+__device__ unsigned long long g_trace[1024 * 32];
+#define TR_T(v) long long v; asm volatile("mov.u64 %0, %%clock64;" : "=l"(v) :: "memory")
+#define TR_ADD(slot, t0) do { long long t1_; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1_) :: "memory"); trAcc[slot] += (unsigned long long)(t1_ - (t0)); } while (0)
+#else
+#define TR_T(v)
+#define TR_ADD(slot, t0)
+#endif
+template <bool kSingle>
+__global__ void __launch_bounds__(kUnpackThreads + 64, kUnpackCtasPerSM)
+k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
+         u32 totalTiles, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+  extern __shared__ __align__(128) unsigned char unpackSmem[];
+  UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
+  const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA; warp 9 publishes and looks back
+  const u32 first = blockIdx.x;
+  if (first >= totalTiles) return;
+  if (first == 0 && tid == 0) lc->tStart = global_timer();
+#ifdef PIXRECO_TRACE
+  unsigned long long trAcc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const long long trStart = clock64();
+#endif
+  const int nLocal = (int)((totalTiles - first + G - 1u) / G);
+  const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
+  auto desc_of = [&](int k) -> const EvDesc& {
+    return kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[k & (kDescRing - 1)]);
+  };
+  // ---- load of local tile k into its ring slot, by the control warp: TMA for the 16-byte multiple, lanes for the tail
+  auto issue_load = [&](int k) {
+    const EvDesc& e = desc_of(k);
+    const u32 T0 = (first + (u32)k * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+    const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)k % kRawSlots;
+    const u32 n4 = nIn & ~3u, n8 = nIn & ~7u;
+    if (lane == 0) {
+      mbar_expect_tx(&sh.full[slot], n4 * 4u + n8 * 2u);
+      if (n4) bulk_load(sh.words[slot], e.words + T0, n4 * 4u, &sh.full[slot]);
+      if (n8) bulk_load(sh.adc[slot], e.adc + T0, n8 * 2u, &sh.full[slot]);
+    }
+    if (lane < nIn - n4) sh.words[slot][n4 + lane] = __ldcs(e.words + T0 + n4 + lane);
+    if (lane < nIn - n8) sh.adc[slot][n8 + lane] = __ldcs(e.adc + T0 + n8 + lane);
+  };
+
+  // ---- prologue: barriers, the first descriptors, the first loads
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < kRawSlots; ++s) mbar_init(&sh.full[s], 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  u32 eNext = 0;                                               // batch, control warp: event of local tile i + kRawSlots + 1
+  if (!kSingle) {
+    if ((int)warp <= kRawSlots && (int)warp < nLocal)
+      sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[first + warp * G]) + lane);
+    if (ctl && kRawSlots + 1 < nLocal) eNext = tileEvent[first + (u32)(kRawSlots + 1) * G];
+  }
+  __syncthreads();
+  if (ctl)
+    for (int k = 0; k < kRawSlots && k < nLocal; ++k) issue_load(k);
+  __syncthreads();
+
+  for (int i = -kCountAhead; i < nLocal; ++i) {
+    const int kc = i + kCountAhead, kl = i + 1, kd = i + kRawSlots + 1;
+    u32 dword = 0, eN2 = 0, tl = 0;
+    u64 lb[kLookBack];
+    if (ctl) {
+      // batch: descriptor of local tile i + kRawSlots + 1 in flight until the end of the iteration
+      if (!kSingle && i >= 0) {
+        if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
+        if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
+      }
+      { TR_T(t0); if (lane == 0 && i > 0) bulk_wait_read(); TR_ADD(0, t0); }   // the staging arrays are free again
+    } else if (!scn && kc < nLocal) {
+      // ---- count: local tile i + kCountAhead
+      const EvDesc& e = desc_of(kc);
+      const u32 T0 = (first + (u32)kc * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)kc % kRawSlots;
+      { TR_T(t0); mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u); if (warp == 0) TR_ADD(1, t0); }
+      const u32* wseg = sh.words[slot] + 256u * warp + lane;
+      u32 cnt = 0, mx = 0, myb = 0;
+      const u32 inWarp = nIn > 256u * warp ? nIn - 256u * warp : 0u;      // words of this warp's segment that exist
+      if (inWarp >= 256u) {                                    // the common case: no range test per word
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const u32 x = wseg[32 * j];
+          const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC;
+          const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
+          cnt += (u32)__popc(b);
+          if (ok) mx = max(mx, x);                             // a digi's word has bit 31 clear: max word = max module
+          if ((int)lane == j) myb = b;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const u32 x = wseg[32 * j];
+          const bool ok = (x >> 20) < limM && (x & 0xFF000u) < limR && (x & 0xFF8u) < limC && 32u * j + lane < inWarp;
+          const u32 b = __ballot_sync(0xFFFFFFFFu, ok);
+          cnt += (u32)__popc(b);
+          if (ok) mx = max(mx, x);
+          if ((int)lane == j) myb = b;
+        }
+      }
+      if (lane < 8u) sh.bal[slot][warp][lane] = myb;
+      mx = __reduce_max_sync(0xFFFFFFFFu, mx);
+      if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
+    }
+    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(2, t0); }                                                         // #1
+    if (scn) {
+      // ---- publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
+      if (kc < nLocal) {
+        const EvDesc& e = desc_of(kc);
+        const u32 tile = first + (u32)kc * G - e.tileBase, slot = (u32)kc % kRawSlots;
+        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+        const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
+        if (lane == 0) st_state(e.tileState + tile, pack_state(tile ? kStAgg : kStIncl, n, mx1));
+      }
+      if (kl >= 0 && kl < nLocal) {
+        const EvDesc& e = desc_of(kl);
+        tl = first + (u32)kl * G - e.tileBase;
+        if (tl) lookback_issue(e.tileState, (int)tl, lane, lb);
+      }
+    } else if (!ctl && i >= 0) {
+      // ---- scatter: local tile i
+      const EvDesc& e = desc_of(i);
+      const u32 T0 = (first + (u32)i * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)i % kRawSlots;
+      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u;
+      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u;
+      const u32 wbase = __reduce_add_sync(0xFFFFFFFFu, lane < warp ? c8 : 0u);
+      const u32 myb = lane < 8u ? sh.bal[slot][warp][lane] : 0u;
+      const u32* wseg = sh.words[slot] + 256u * warp + lane;
+      const u16* aseg = sh.adc[slot] + 256u * warp + lane;
+      u32 ebase = 8u + ph + wbase;                             // staging element of the warp's next digi
+      const u32 wi0 = T0 + 256u * warp + lane;                 // event-local index of this lane's word of row 0
+      if (tid == 0) {                                          // "the digi before the tile" for the order check (module 0 if none)
+        const u32 c1 = sh.carry1[i & 1];
+        sh.sModule[8u + ph - 1u] = (u16)(c1 ? c1 - 1u : 0u);
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const u32 b = __shfl_sync(0xFFFFFFFFu, myb, j);
+        const u32 x = wseg[32 * j], a = aseg[32 * j];
+        const u32 el = ebase + (u32)__popc(b & lt);
+        if (b >> lane & 1u) {
+          const u32 mod = x >> 20;
+          const float2 gp = __ldg(g.calib + mod);
+          sh.sModule[el] = (u16)mod; sh.sRow[el] = (u16)((x >> 12) & 0xFFu); sh.sCol[el] = (u16)((x >> 3) & 0x1FFu);
+          sh.sAdc[el] = (u16)a; sh.sWordIdx[el] = wi0 + 32u * j;
+          sh.sCharge[el] = __fmaf_rn((float)a, gp.x, gp.y);
+        } else if (256u * warp + 32u * j + lane < nIn) {
+          // error word (A2-A4): errors before it = words before it - digis before it
+          const u32 ei = (wi0 + 32u * j) - (g0 + (el - 8u - ph));
+          e.errWord[ei] = x; e.errIdx[ei] = wi0 + 32u * j;
+        }
+        ebase += (u32)__popc(b);
+      }
+      fence_async_smem();                                      // staged digis -> visible to the TMA store
+    }
+    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(3, t0); }                                                         // #2
+    if (ctl) {
+      if (i >= 0) {
+        const EvDesc& e = desc_of(i);
+        const u32 slot = (u32)i % kRawSlots, g0 = sh.g0[i & 1], ph = g0 & 7u;
+        const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+        const u32 midLo = (g0 + 7u) & ~7u, midHi = (g0 + n) & ~7u;
+        if (lane == 0) {
+          if (midHi > midLo) {
+            const u32 cnt = midHi - midLo, se = 8u + ph + (midLo - g0);
+            bulk_store(e.module + midLo, sh.sModule + se, cnt * 2u); bulk_store(e.row + midLo, sh.sRow + se, cnt * 2u);
+            bulk_store(e.col + midLo, sh.sCol + se, cnt * 2u); bulk_store(e.adcOut + midLo, sh.sAdc + se, cnt * 2u);
+            bulk_store(e.wordIdx + midLo, sh.sWordIdx + se, cnt * 4u); bulk_store(e.charge + midLo, sh.sCharge + se, cnt * 4u);
+          }
+          bulk_commit();
+        }
+        if (i + kRawSlots < nLocal) issue_load(i + kRawSlots);   // into the slot this tile vacated
+        if (lane < 16u) {
+          // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
+          const u32 lo = 8u + ph, k = lane < 8u ? lane : n - 16u + lane, p = g0 + k;
+          if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
+            const u32 se = lo + k;
+            e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
+            e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
+          }
+        }
+      }
+      if (!kSingle && i >= 0) {
+        if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
+        eNext = eN2;
+      }
+    } else if (scn) {
+      // ---- resolve the look-back of tile i + 1 (its loads flew during the scatter), publish its inclusive state
+      if (kl >= 0 && kl < nLocal) {
+        const EvDesc& e = desc_of(kl);
+        const u32 slot = (u32)kl % kRawSlots;
+        u32 c = 0, m = 0;
+        if (tl) {
+          { TR_T(t0); lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m); TR_ADD(6, t0); }
+          const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
+          const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
+          if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
+        }
+        if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
+      }
+    } else if (i >= 0) {
+      const EvDesc& e = desc_of(i);
+      const u32 tile = first + (u32)i * G - e.tileBase, slot = (u32)i % kRawSlots;
+      const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
+      const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
+      const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
+      const u32 lo = 8u + ph, hi = lo + n;
+      // order check (A5): no digi's module is below that of the digi before it.  Eight digis per thread;
+      // per halfword, bit 15 of (m | 0x8000) - p stays set iff m >= p (modules are below 2^11).
+      {
+        u32 bad = 0;
+        for (u32 c = 1u + tid; 8u * c < hi; c += kUnpackThreads) {
+          const uint4 v = *reinterpret_cast<const uint4*>(sh.sModule + 8u * c);
+          const u32 prev = sh.sModule[8u * c - 1u];
+          if (8u * c >= lo && 8u * c + 8u <= hi) {
+            const u32 s0 = v.x << 16 | prev, s1 = __funnelshift_l(v.x, v.y, 16), s2 = __funnelshift_l(v.y, v.z, 16), s3 = __funnelshift_l(v.z, v.w, 16);
+            const u32 t = ((v.x | 0x80008000u) - s0) & ((v.y | 0x80008000u) - s1) & ((v.z | 0x80008000u) - s2) & ((v.w | 0x80008000u) - s3);
+            bad |= ~t & 0x80008000u;
+          } else {                                             // the tile's first and last chunk may be partial
+            const u32 w4[4] = {v.x, v.y, v.z, v.w};
+            u32 p = prev;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const u32 m = (q & 1) ? w4[q >> 1] >> 16 : w4[q >> 1] & 0xFFFFu, idx = 8u * c + (u32)q;
+              if (idx >= lo && idx < hi && m < p) bad = 1u;
+              p = m;
+            }
+          }
+        }
+        if (bad) atomicOr(&e.counters->status, 1u);            // PR_STATUS_INPUT_ORDER
+      }
+      // modDigiStart[m] for the modules that begin in this tile (or are skipped by it): the number of staged
+      // digis with module < m (the staged modules ascend unless the order check fired).  Warp w resolves the
+      // modules that are new in its own 256-word segment, [max module + 1 before it, max module + 1 in it), by a
+      // 4-ary search inside the segment: every warp gets its share.
+      if (n) {
+        const u32 prev1 = max(carry1, __reduce_max_sync(0xFFFFFFFFu, lane < warp ? m8 : 0u));
+        const u32 wbase = __reduce_add_sync(0xFFFFFFFFu, lane < warp ? c8 : 0u);
+        const u32 cntW = __shfl_sync(0xFFFFFFFFu, c8, warp), mx1W = __shfl_sync(0xFFFFFFFFu, m8, warp);
+        const u16* base = sh.sModule + lo + wbase;
+        for (u32 m = prev1 + lane; m < mx1W; m += 32u) {
+          u32 pos = 0, len = cntW;                             // digis [0, pos) of the segment are < m; the answer is < pos + len
+#pragma unroll
+          for (u32 q = 64u; q; q >>= 2) {                      // len <= 256: quarters of 64, 16, 4, 1
+            u32 adv = 0;
+#pragma unroll
+            for (u32 r = 1; r <= 3u; ++r)
+              if (r * q <= len && base[pos + r * q - 1u] < m) adv = r;
+            pos += adv * q;
+            len = min(len - adv * q, q);
+          }
+          e.modDigiStart[m] = g0 + wbase + pos;
+        }
+      }
+      // the event's last tile closes modDigiStart and the counters
+      if (tile == e.nTiles - 1u) {
+        const u32 D = g0 + n, mx1 = max(carry1, tileMax1), W = e.nWords;
+        for (u32 m = mx1 + tid; m <= g.M; m += kUnpackThreads) e.modDigiStart[m] = D;
+        if (tid == 0) { e.counters->nWords = W; e.counters->nDigis = D; e.counters->nErrors = W - D; }
+      }
+    }
+  }
+  if (ctl && lane == 0) bulk_wait_all();
+#ifdef PIXRECO_TRACE
+  if (lane == 0 && blockIdx.x < 1024) {
+    unsigned long long* o = g_trace + blockIdx.x * 32;
+    o[warp * 2] = trAcc[2]; o[warp * 2 + 1] = trAcc[3];
+    if (ctl) { o[20] = trAcc[0]; o[22] = (unsigned long long)(clock64() - trStart); }
+    if (scn) o[21] = trAcc[6];
+    if (warp == 0) o[23] = trAcc[1];
+  }
+#endif
+}
+
+}  // namespace pixreco
