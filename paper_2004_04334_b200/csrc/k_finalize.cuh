@@ -44,16 +44,23 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
     if (d0 <= d1 && d1 <= ev.cap) {
       for (u32 dd = d0 + sp * 1024u + tid; dd < d1; dd += splits * 1024u) {     // four independent digis per thread and trip
-        int32_t c[4]; u32 md[4];
+        int32_t c[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           const u32 d = dd + 256u * k;
           c[k] = d < d1 ? ev.clus[d] : -1;
-          md[k] = d < d1 ? (u32)ev.module[d] : m0;
         }
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (c[k] >= 0) ev.clus[dd + 256u * k] = (int32_t)(sStart[min(md[k] - m0, kFinMods - 1)] + (u32)c[k]);
+        for (int k = 0; k < 4; ++k) {
+          if (c[k] < 0) continue;
+          // the digi's module within the group: the last one that starts at or before the digi (no read of module[])
+          const u32 d = dd + 256u * k;
+          u32 li = 0;
+#pragma unroll
+          for (u32 step = 16; step > 0; step >>= 1)
+            if (li + step < m1 - m0 && sDigi[li + step] <= d) li += step;
+          ev.clus[d] = (int32_t)(sStart[li] + (u32)c[k]);
+        }
       }
       for (u32 o = sStart[0] + sp * 256u + tid; o < sStart[32]; o += splits * 256u) {
         u32 li = 0;
