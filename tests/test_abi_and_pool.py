@@ -62,6 +62,27 @@ def test_create_rejects_bad_arguments_without_a_device():
     assert not h.value
 
 
+def test_sources_keep_the_papers_rules():
+    """PAPER.md L31 fn. 1 and L82-88 as static checks on the sources: the blocking CUDA calls appear only in
+    pr_create / pr_destroy (job start / job end), and device code neither asserts, traps nor prints."""
+    csrc = os.path.join(ROOT, "paper_2004_04334_b200", "csrc")
+    api = open(os.path.join(csrc, "pixreco_api.cu")).read()
+    blocking = re.compile(r"\bcuda(DeviceSynchronize|StreamSynchronize|EventSynchronize|Memcpy|Memset|Malloc|Free|HostAlloc|FreeHost)\s*\(")
+    # split the file into top-level functions by their opening line
+    funcs = re.split(r"\n(?=(?:int|void\*?|const char\*|uint64_t)\s+pr_[a-z_]+\s*\()", api)
+    for f in funcs:
+        m = re.match(r"(?:int|void\*?|const char\*|uint64_t)\s+(pr_[a-z_]+)", f)
+        name = m.group(1) if m else "<helpers>"
+        hits = set(x.group(0).rstrip("( ") for x in blocking.finditer(f))
+        if name in ("pr_create", "pr_destroy"):
+            continue
+        assert not hits, (name, hits)
+    for fn in os.listdir(csrc):
+        if fn.endswith(".cuh"):
+            code = re.sub(r"//.*", "", open(os.path.join(csrc, fn)).read())
+            assert not re.search(r"(?<![_a-z])assert\s*\(|__trap\s*\(|\bprintf\s*\(", code), fn
+
+
 def test_null_slots_are_rejected_without_a_device():
     """Every slot-level entry point checks its handle before touching CUDA."""
     lib = pr.lib()
