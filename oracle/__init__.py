@@ -20,6 +20,7 @@ from dataclasses import dataclass
 import numpy as np
 
 INVALID = 0xFFFFFFFF
+PITCH_ROW_UM, PITCH_COL_UM = 100.0, 150.0      # A26: local x runs along the row index, local y along the col index
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pixreco_oracle.c")
@@ -43,7 +44,7 @@ def _load():
     global _lib
     if _lib is None:
         _lib = ctypes.CDLL(build())
-        for name in ("po_decode", "po_calibrate", "po_cluster", "po_reduce", "po_run", "po_check_exact_sums"):
+        for name in ("po_decode", "po_calibrate", "po_cluster", "po_reduce", "po_hits", "po_run", "po_check_exact_sums"):
             getattr(_lib, name).restype = ctypes.c_int
         _lib.po_decode.restype = None
         _lib.po_calibrate.restype = None
@@ -87,6 +88,13 @@ class Result:
     cl_col: np.ndarray      # f32 [N]
     clus: np.ndarray        # i32 [D]
     mod_clus_start: np.ndarray  # u32 [M+1]
+    ht_x: np.ndarray        # f32 [N] local x (um), hit k belongs to cluster k
+    ht_y: np.ndarray        # f32 [N]
+    ht_xerr: np.ndarray     # f32 [N]
+    ht_yerr: np.ndarray     # f32 [N]
+    ht_rows: np.ndarray     # u32 [N] minRow | maxRow << 16
+    ht_cols: np.ndarray     # u32 [N] minCol | maxCol << 16
+    ht_flags: np.ndarray    # u16 [N] bit0 touches a row border, bit1 a col border
 
 
 def decode(words, adc, n_modules, n_rows=160, n_cols=416):
@@ -165,6 +173,26 @@ def reduce(label, charge, module, row, col, cluster_threshold_e, n_modules):
                 n_clusters_all=nall.value, n_clusters=N)
 
 
+def hits(clus, charge, row, col, n_clusters, n_rows=160, n_cols=416, pitch_row_um=PITCH_ROW_UM, pitch_col_um=PITCH_COL_UM):
+    """O5.  Returns dict(ht_x, ht_y, ht_xerr, ht_yerr, ht_rows, ht_cols, ht_flags) for the kept clusters 0..N-1."""
+    clus = np.ascontiguousarray(clus, np.int32)
+    charge = np.ascontiguousarray(charge, np.float32)
+    row = np.ascontiguousarray(row, np.uint16)
+    col = np.ascontiguousarray(col, np.uint16)
+    D, N = clus.shape[0], int(n_clusters)
+    cap = max(N, 1)
+    x, y, xe, ye = (np.zeros(cap, np.float32) for _ in range(4))
+    rows, cols = np.zeros(cap, np.uint32), np.zeros(cap, np.uint32)
+    flags = np.zeros(cap, np.uint16)
+    rc = _load().po_hits(_u32(D), _u32(N), _u32(n_rows), _u32(n_cols), _p(clus), _p(charge), _p(row), _p(col),
+                         ctypes.c_double(pitch_row_um), ctypes.c_double(pitch_col_um),
+                         _p(x), _p(y), _p(xe), _p(ye), _p(rows), _p(cols), _p(flags))
+    if rc != 0:
+        raise MemoryError("po_hits")
+    return dict(ht_x=x[:N], ht_y=y[:N], ht_xerr=xe[:N], ht_yerr=ye[:N], ht_rows=rows[:N], ht_cols=cols[:N],
+                ht_flags=flags[:N])
+
+
 class Workspace:
     """Caller-owned output arrays of capacity W for :func:`run` (so timing excludes numpy allocs)."""
 
@@ -174,6 +202,9 @@ class Workspace:
         self.u16 = [np.zeros(cap, np.uint16) for _ in range(5)]   # module,row,col,adc,cl_module
         self.u32 = [np.zeros(cap, np.uint32) for _ in range(6)]   # word_idx,err_word,err_idx,label,cl_label,cl_size
         self.f32 = [np.zeros(cap, np.float32) for _ in range(4)]  # charge,cl_charge,cl_row,cl_col
+        self.hit_f32 = [np.zeros(cap, np.float32) for _ in range(4)]   # ht_x,ht_y,ht_xerr,ht_yerr
+        self.hit_u32 = [np.zeros(cap, np.uint32) for _ in range(2)]    # ht_rows,ht_cols
+        self.hit_flags = np.zeros(cap, np.uint16)
         self.kept = np.zeros(cap, np.uint8)
         self.clus = np.zeros(cap, np.int32)
         self.mds = np.zeros(n_modules + 1, np.uint32)
@@ -181,21 +212,25 @@ class Workspace:
         self.counters = np.zeros(8, np.uint32)
 
 
-def run_raw(words, adc, n_modules, n_rows, n_cols, gain, pedestal, pix_thr, clus_thr, ws: Workspace) -> int:
-    """The whole chain O1..O4 into ``ws`` (no trimming, no copies).  Returns po_run's rc."""
+def run_raw(words, adc, n_modules, n_rows, n_cols, gain, pedestal, pix_thr, clus_thr, ws: Workspace,
+            pitch_row_um=PITCH_ROW_UM, pitch_col_um=PITCH_COL_UM) -> int:
+    """The whole chain O1..O5 into ``ws`` (no trimming, no copies).  Returns po_run's rc."""
     mod, row, col, a, clm = ws.u16
     widx, ew, ei, label, cll, cls = ws.u32
     q, clq, clr, clc = ws.f32
+    hx, hy, hxe, hye = ws.hit_f32
+    hr, hc = ws.hit_u32
     return _load().po_run(_p(words), _p(adc), _u32(words.shape[0]), _u32(n_modules), _u32(n_rows), _u32(n_cols),
                           _p(gain), _p(pedestal), ctypes.c_float(pix_thr), ctypes.c_float(clus_thr),
                           _p(mod), _p(row), _p(col), _p(a), _p(widx), _p(ew), _p(ei), _p(ws.mds),
                           _p(q), _p(ws.kept), _p(label), _p(cll), _p(clm), _p(cls), _p(clq), _p(clr), _p(clc),
-                          _p(ws.clus), _p(ws.mcs), _p(ws.counters))
+                          _p(ws.clus), _p(ws.mcs), ctypes.c_double(pitch_row_um), ctypes.c_double(pitch_col_um),
+                          _p(hx), _p(hy), _p(hxe), _p(hye), _p(hr), _p(hc), _p(ws.hit_flags), _p(ws.counters))
 
 
 def run(words, adc, n_modules, gain, pedestal, pixel_threshold_e=1000.0, cluster_threshold_e=4000.0,
-        n_rows=160, n_cols=416) -> Result:
-    """The whole chain O1..O4 on one event."""
+        n_rows=160, n_cols=416, pitch_row_um=PITCH_ROW_UM, pitch_col_um=PITCH_COL_UM) -> Result:
+    """The whole chain O1..O5 on one event."""
     words = np.ascontiguousarray(words, np.uint32)
     adc = np.ascontiguousarray(adc, np.uint16)
     gain = np.ascontiguousarray(gain, np.float32)
@@ -203,7 +238,7 @@ def run(words, adc, n_modules, gain, pedestal, pixel_threshold_e=1000.0, cluster
     assert gain.shape[0] == n_modules and pedestal.shape[0] == n_modules and adc.shape == words.shape
     ws = Workspace(words.shape[0], n_modules)
     rc = run_raw(words, adc, n_modules, n_rows, n_cols, gain, pedestal, pixel_threshold_e,
-                 cluster_threshold_e, ws)
+                 cluster_threshold_e, ws, pitch_row_um, pitch_col_um)
     if rc == -2:
         raise ArithmeticError("a kept charge is not a multiple of 2^-14 (pixel threshold < 512?)")
     if rc != 0:
@@ -212,13 +247,16 @@ def run(words, adc, n_modules, gain, pedestal, pixel_threshold_e=1000.0, cluster
     mod, row, col, a, clm = ws.u16
     widx, ew, ei, label, cll, cls = ws.u32
     q, clq, clr, clc = ws.f32
+    hx, hy, hxe, hye = ws.hit_f32
+    hr, hc = ws.hit_u32
     return Result(words.shape[0], D, E, nk, nall, N, bool(ok), mod[:D], row[:D], col[:D], a[:D], widx[:D],
                   ew[:E], ei[:E], ws.mds, q[:D], ws.kept[:D], label[:D], cll[:N], clm[:N], cls[:N], clq[:N],
-                  clr[:N], clc[:N], ws.clus[:D], ws.mcs)
+                  clr[:N], clc[:N], ws.clus[:D], ws.mcs, hx[:N], hy[:N], hxe[:N], hye[:N], hr[:N], hc[:N],
+                  ws.hit_flags[:N])
 
 
 def check_exact_sums(label, charge, col) -> int:
-    """O5 (A9): 0 if the exact-sum claims hold for this event; O(D x clusters), small events only."""
+    """O6 (A9): 0 if the exact-sum claims hold for this event; O(D x clusters), small events only."""
     label = np.ascontiguousarray(label, np.uint32)
     charge = np.ascontiguousarray(charge, np.float32)
     col = np.ascontiguousarray(col, np.uint16)

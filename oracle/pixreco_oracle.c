@@ -4,7 +4,7 @@
  * raw-word decode with stable digi/error compaction -> per-module ADC-to-charge calibration with
  * pixel threshold -> per-module 8-connected connected components with canonical label = minimum
  * digi index -> exact cluster charge sums, charge-weighted centroids, cluster threshold and dense
- * numbering.
+ * numbering -> hits (bounding box, local position, error estimate) of the kept clusters.
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * build, load or call anything in oracle/.  It shares no code, header, table or helper with the
@@ -21,7 +21,8 @@
  * round trip, closed-form calibration values and the float64 single-rounding identity, exhaustive
  * 4x4 occupancy patterns against an O(n^2) transitive closure, scipy.ndimage.label /
  * sum_labels / center_of_mass, networkx components for duplicate pixels, special shapes,
- * permutation invariance, worked reduce example.  Against the PAPER there is nothing to pin:
+ * permutation invariance, worked reduce example; for hits: worked values, closed forms (single
+ * pixel, strips, centred and translated clusters), numpy min/max and scipy.ndimage.center_of_mass.  Against the PAPER there is nothing to pin:
  * it prints no value for this path ("parity unpinned" with respect to the paper).
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fPIC -shared pixreco_oracle.c -lm
@@ -194,8 +195,68 @@ int po_reduce(uint32_t D, uint32_t M,
   return rc;
 }
 
-/* ---- the whole chain, in order O1..O4 (what bench.py's cpu_baseline times) ----
+/* ---- O5 hits (the step after clustering in the paper's Fig. 1: raw -> clusters
+ * -> hits).  The paper defines no hit arithmetic (L118); readings A26-A30 of
+ * DESIGN.md fix it.  For every KEPT cluster k (dense number of O4), over its member digis
+ * {d : clus[d] == k} (duplicates included, A6):
+ *   bounding box   minRow, maxRow, minCol, maxCol                                        (A28)
+ *   exact sums     S, Sx, Sy as in O4 (int64, scale 2^14)                                (A9)
+ *   local position x = ((double)Sx/(double)S + 0.5 - R/2) * pitch_row   [um]  (row index -> local x)
+ *                  y = ((double)Sy/(double)S + 0.5 - C/2) * pitch_col   [um]  (col index -> local y)
+ *                  pixel centres sit at index + 0.5, origin at the module centre, uniform pitch, no
+ *                  big-pixel correction (A13, A26); binary64 operations in exactly this order
+ *                  (divide, add 0.5, subtract R/2, multiply), each rounded to nearest, then ONE
+ *                  cast to binary32 (A27)
+ *   edge flags     bit0: minRow == 0 or maxRow == R-1;  bit1: minCol == 0 or maxCol == C-1   (A29)
+ *   error estimate per coordinate, span = max - min + 1, c = 1/sqrt(12) (binary64 literal):
+ *                  touching that border: pitch*c*span; else span == 1: pitch*c; else pitch*c*0.5
+ *                  evaluated as (pitch*c)*factor in binary64, cast to binary32               (A30)
+ * ht_rows = minRow | maxRow << 16, ht_cols = minCol | maxCol << 16.  Returns 0, -1 on allocation failure. */
+int po_hits(uint32_t D, uint32_t N, uint32_t R, uint32_t C,
+            const int32_t *clus, const float *charge, const uint16_t *d_row, const uint16_t *d_col,
+            double pitch_row_um, double pitch_col_um,
+            float *ht_x, float *ht_y, float *ht_xerr, float *ht_yerr,
+            uint32_t *ht_rows, uint32_t *ht_cols, uint16_t *ht_flags) {
+  const double inv_sqrt12 = 0.28867513459481287;   /* 1/sqrt(12) rounded to binary64 */
+  size_t n = N ? N : 1;
+  int64_t *S = (int64_t *)calloc(n, sizeof(int64_t)), *Sx = (int64_t *)calloc(n, sizeof(int64_t)), *Sy = (int64_t *)calloc(n, sizeof(int64_t));
+  uint32_t *rmin = (uint32_t *)malloc(n * sizeof(uint32_t)), *rmax = (uint32_t *)malloc(n * sizeof(uint32_t));
+  uint32_t *cmin = (uint32_t *)malloc(n * sizeof(uint32_t)), *cmax = (uint32_t *)malloc(n * sizeof(uint32_t));
+  if (!S || !Sx || !Sy || !rmin || !rmax || !cmin || !cmax) { free(S); free(Sx); free(Sy); free(rmin); free(rmax); free(cmin); free(cmax); return -1; }
+  for (uint32_t k = 0; k < N; ++k) { rmin[k] = 0xFFFFFFFFu; cmin[k] = 0xFFFFFFFFu; rmax[k] = 0; cmax[k] = 0; }
+  for (uint32_t d = 0; d < D; ++d) {
+    if (clus[d] < 0) continue;
+    uint32_t k = (uint32_t)clus[d];
+    int64_t qf = (int64_t)(charge[d] * 16384.0f);
+    S[k] += qf; Sx[k] += qf * (int64_t)d_row[d]; Sy[k] += qf * (int64_t)d_col[d];
+    if (d_row[d] < rmin[k]) rmin[k] = d_row[d];
+    if (d_row[d] > rmax[k]) rmax[k] = d_row[d];
+    if (d_col[d] < cmin[k]) cmin[k] = d_col[d];
+    if (d_col[d] > cmax[k]) cmax[k] = d_col[d];
+  }
+  for (uint32_t k = 0; k < N; ++k) {
+    double x = (double)Sx[k] / (double)S[k];
+    x = x + 0.5; x = x - 0.5 * (double)R; x = x * pitch_row_um;
+    double y = (double)Sy[k] / (double)S[k];
+    y = y + 0.5; y = y - 0.5 * (double)C; y = y * pitch_col_um;
+    ht_x[k] = (float)x; ht_y[k] = (float)y;
+    uint32_t span_r = rmax[k] - rmin[k] + 1, span_c = cmax[k] - cmin[k] + 1;
+    int edge_r = (rmin[k] == 0 || rmax[k] == R - 1), edge_c = (cmin[k] == 0 || cmax[k] == C - 1);
+    double fr = edge_r ? (double)span_r : (span_r == 1 ? 1.0 : 0.5);
+    double fc = edge_c ? (double)span_c : (span_c == 1 ? 1.0 : 0.5);
+    double er = pitch_row_um * inv_sqrt12; er = er * fr;
+    double ec = pitch_col_um * inv_sqrt12; ec = ec * fc;
+    ht_xerr[k] = (float)er; ht_yerr[k] = (float)ec;
+    ht_rows[k] = rmin[k] | (rmax[k] << 16); ht_cols[k] = cmin[k] | (cmax[k] << 16);
+    ht_flags[k] = (uint16_t)((edge_r ? 1 : 0) | (edge_c ? 2 : 0));
+  }
+  free(S); free(Sx); free(Sy); free(rmin); free(rmax); free(cmin); free(cmax);
+  return 0;
+}
+
+/* ---- the whole chain, in order O1..O5 (what bench.py's cpu_baseline times) ----
  * All output arrays have capacity W (mod_* arrays M+1) and are owned by the caller.
+ * Hit arrays have capacity W too.
  * counters[0..6] = n_digis, n_errors, n_kept_digis, n_clusters_all, n_clusters, sorted_ok, rc.   */
 int po_run(const uint32_t *words, const uint16_t *adc, uint32_t W,
            uint32_t M, uint32_t R, uint32_t C,
@@ -205,7 +266,10 @@ int po_run(const uint32_t *words, const uint16_t *adc, uint32_t W,
            float *charge, uint8_t *kept, uint32_t *label,
            uint32_t *cl_label, uint16_t *cl_module, uint32_t *cl_size,
            float *cl_charge, float *cl_row, float *cl_col,
-           int32_t *clus, uint32_t *mod_clus_start, uint32_t *counters) {
+           int32_t *clus, uint32_t *mod_clus_start,
+           double pitch_row_um, double pitch_col_um,
+           float *ht_x, float *ht_y, float *ht_xerr, float *ht_yerr,
+           uint32_t *ht_rows, uint32_t *ht_cols, uint16_t *ht_flags, uint32_t *counters) {
   uint32_t D, E, ok, nk, nall, N;
   po_decode(words, adc, W, M, R, C, d_module, d_row, d_col, d_adc, d_word_idx, e_word, e_idx,
             mod_digi_start, &D, &E, &ok);
@@ -215,12 +279,14 @@ int po_run(const uint32_t *words, const uint16_t *adc, uint32_t W,
     rc = po_reduce(D, M, label, charge, d_module, d_row, d_col, clus_thr, cl_label, cl_module, cl_size,
                    cl_charge, cl_row, cl_col, clus, mod_clus_start, &nall, &N);
   else { nall = 0; N = 0; }
+  if (rc == 0 && po_hits(D, N, R, C, clus, charge, d_row, d_col, pitch_row_um, pitch_col_um, ht_x, ht_y, ht_xerr, ht_yerr,
+                         ht_rows, ht_cols, ht_flags) != 0) rc = -1;
   counters[0] = D; counters[1] = E; counters[2] = nk; counters[3] = nall; counters[4] = N;
   counters[5] = ok; counters[6] = (uint32_t)rc;
   return rc;
 }
 
-/* ---- O5 exact-sum self-check (A9), paranoid mode, never timed.  Verifies for one event's
+/* ---- O6 exact-sum self-check (A9), paranoid mode, never timed.  Verifies for one event's
  * decoded/calibrated/labelled data that (a) q*2^14 is integral for every kept digi, (b) int64
  * sums equal an __int128 accumulation, (c) where the sums stay below 2^53 a plain binary64 sum
  * in index order and in reversed order both equal S*2^-14.  Returns 0 if all hold, else the
