@@ -27,6 +27,9 @@
  *   a4 reduce   per cluster exact int64 fixed-point (2^-14 e) sums -> size, charge, charge-
  *               weighted (row,col) centroid; kept iff charge >= cluster thr; kept clusters
  *               numbered in ascending label order (A9, A12, A13)
+ *   hits        the step after clustering in the paper's Fig. 1: one hit per kept cluster —
+ *               bounding box, local position from the exact sums (pixel centre = index + 0.5, origin
+ *               at the module centre, times the pitch), border flags, error estimate (A26-A30)
  *
  * Threading: any host thread may use different pr_event objects concurrently; one pr_event is
  * used by one thread at a time.  Every entry point sets the CUDA device of its handle.
@@ -44,7 +47,7 @@
 extern "C" {
 #endif
 
-#define PR_ABI_VERSION 2
+#define PR_ABI_VERSION 3
 
 /* ---- return codes (int).  Negative = error.  pr_strerror() names them. ---- */
 #define PR_OK               0
@@ -69,6 +72,8 @@ extern "C" {
 #define PR_WANT_LABELS   0x04u  /* label, clus */
 #define PR_WANT_CLUSTERS 0x08u  /* cluster SoA, mod_clus_start */
 #define PR_WANT_ERRORS   0x10u
+#define PR_WANT_HITS     0x20u  /* hit SoA (one hit per kept cluster: local position, errors, bounding box, edge flags) */
+#define PR_WANT_ALL      0x3Fu
 
 /* pr_output.status_bits (device-detected conditions) */
 #define PR_STATUS_INPUT_ORDER 0x1u
@@ -96,12 +101,14 @@ typedef struct {
   uint32_t max_events_in_flight;  /* ... and this many concurrent events                          */
   uint64_t max_cached_bytes_device, max_cached_bytes_host;   /* pool caps, 0 = unlimited          */
   uint32_t flags;                 /* PR_FLAG_* mask                                               */
+  float    pitch_row_um, pitch_col_um;   /* pixel pitch along the row index (local x) and the col index (local y) in um for
+                                     the hits (A26); 0 = the defaults 100 and 150                  */
 } pr_config;
 
 /* pr_config.flags */
 #define PR_FLAG_KERNEL_TIMING 0x1u /* record CUDA events around each kernel on its stream and sum the
                                       per-kernel device times into pr_stats (measurement aid; adds
-                                      four cudaEventRecord per acquire)                            */
+                                      three cudaEventRecord per acquire)                           */
 
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
@@ -115,7 +122,7 @@ typedef struct {                  /* one event's input, filled by the caller bef
 
 /* Views into library-owned buffers; valid from a PR_OK pr_produce until pr_release(ev).
  * d_* are device pointers (always set); h_* are pinned-host mirrors (NULL unless in `want`).
- * Lengths: digi arrays n_digis; err arrays n_errors; cluster arrays n_clusters;
+ * Lengths: digi arrays n_digis; err arrays n_errors; cluster and hit arrays n_clusters;
  * mod_*_start n_modules+1.                                                                        */
 typedef struct {
   uint64_t event_id;
@@ -129,12 +136,18 @@ typedef struct {
   const uint32_t *d_cl_label, *d_cl_size; const uint16_t* d_cl_module;
   const float *d_cl_charge, *d_cl_row, *d_cl_col;
   const uint32_t *d_err_word, *d_err_idx;
+  const float *d_ht_x, *d_ht_y, *d_ht_xerr, *d_ht_yerr;   /* [n_clusters] um; hit k belongs to cluster k (A26, A27, A30) */
+  const uint32_t *d_ht_rows, *d_ht_cols;                  /* minRow | maxRow << 16, minCol | maxCol << 16 (A28)          */
+  const uint16_t* d_ht_flags;                             /* bit 0: touches row 0 or R-1, bit 1: col 0 or C-1 (A29)      */
   const uint16_t *h_module, *h_row, *h_col, *h_adc; const uint32_t* h_word_idx;
   const float* h_charge; const uint32_t* h_label; const int32_t* h_clus;
   const uint32_t *h_mod_digi_start, *h_mod_clus_start;
   const uint32_t *h_cl_label, *h_cl_size; const uint16_t* h_cl_module;
   const float *h_cl_charge, *h_cl_row, *h_cl_col;
   const uint32_t *h_err_word, *h_err_idx;
+  const float *h_ht_x, *h_ht_y, *h_ht_xerr, *h_ht_yerr;
+  const uint32_t *h_ht_rows, *h_ht_cols;
+  const uint16_t* h_ht_flags;
 } pr_output;
 
 typedef struct {
@@ -151,7 +164,7 @@ typedef struct {
   pr_pool_stats device_pool, host_pool;
   /* PR_FLAG_KERNEL_TIMING only: device time summed over `timed_acquires` completed acquires */
   uint64_t timed_acquires;
-  double   unpack_ms, cluster_ms, finalize_ms, export_ms;
+  double   unpack_ms, cluster_ms, export_ms;
 } pr_stats;
 
 /* ---- handle: job start / job end (may block and allocate) ---- */
@@ -183,8 +196,13 @@ int pr_query(pr_event* ev);
 int pr_produce(pr_event* ev, pr_output* out);
 int pr_produce_batch(pr_event* ev, pr_output* outs, uint32_t n);   /* outs[n]; worst status returned */
 /* Return the slot's buffers to the pools; invalidates pr_output views.  PR_NOT_READY if the work
- * has not completed yet (nothing is released then).                                              */
+ * has not completed yet, or its completion callback has not returned yet (nothing is released then).
+ * The caller must have seen its own consumers of the d_* views complete (or use pr_release_on).  */
 int pr_release(pr_event* ev);
+/* The same when a consumer kernel queued on `consumer_stream` may still be reading the d_* views:
+ * the buffers go back to the pool tagged with that stream and an event recorded on it now, so another stream
+ * reuses them only after the consumer's work has completed (queried, never waited on).            */
+int pr_release_on(pr_event* ev, void* consumer_stream);
 /* Transfer on demand as a stage of its own (the copy to the host is a module of its own, run
  * only if something consumes it, and it learns about completion like any External Worker).  After a
  * pr_produce that returned PR_OK, enqueue exact-size DMA copies (cudaMemcpyAsync, sizes taken from the

@@ -1,0 +1,39 @@
+/* pixreco_driver.h — a multi-threaded C++ client of the C ABI (pixreco.h) for the paper's own usage pattern:
+ * one pr_acquire per event on the event's own stream, issued from several host threads at once, completion by
+ * polling, never a blocking wait (TBB tasks on many threads; BASELINE.json
+ * configs[2]; SURVEY 8(d) "issuing host threads in {1, 2, 4}").  It uses nothing but pixreco.h: it is a caller of
+ * the library, not part of the hot path.  Built as libpixreco_driver.so next to libpixreco.so.
+ */
+#ifndef PIXRECO_DRIVER_H
+#define PIXRECO_DRIVER_H
+
+#include <stdint.h>
+
+#include "pixreco.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  double   wall_s;                 /* first pr_acquire to last pr_produce, over all threads (A24)                  */
+  double   acquire_us_median, acquire_us_mean, acquire_us_p99;   /* host time inside pr_acquire, per call           */
+  uint64_t events, digis, clusters;
+  uint64_t produce_polls;          /* pr_produce calls that answered PR_NOT_READY                                  */
+  int32_t  status;                 /* PR_OK or the first error any thread saw                                      */
+  uint32_t threads;
+} prd_result;
+
+/* Run `n_events` events: event e takes input pool[(first + e) % n_pool], slot e % n_slots and stream e % n_slots
+ * (A25); a slot is acquired again only after its previous event was produced and released.  Thread t of `n_threads`
+ * drives the slots s with s % n_threads == t.  t_start_ns / t_end_ns (may be NULL, else [n_events]) receive the
+ * device time stamps of every event (pr_output.t_start_ns / t_end_ns).  `want` and `mem_kind` come with the inputs.
+ * Returns res->status.                                                                                            */
+int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slots,
+                    const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
+                    uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIXRECO_DRIVER_H */

@@ -10,7 +10,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libpixreco.so")
 SOURCES = ["pixreco_api.cu", "pool.cpp"]
-DEPS = SOURCES + ["kernels.cuh", "common.cuh", "k_unpack.cuh", "k_cluster.cuh", "k_finalize.cuh", "pool.hpp"]
+DEPS = SOURCES + ["kernels.cuh", "common.cuh", "k_unpack.cuh", "k_cluster.cuh", "k_export.cuh", "pool.hpp"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -38,3 +38,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB
+
+
+# The multi-threaded C++ client of the C ABI (include/pixreco_driver.h): host-only, links against libpixreco.so.
+DRIVER_LIB = os.path.join(_HERE, "libpixreco_driver.so")
+DRIVER_SRC = os.path.join(CSRC, "stream_driver.cpp")
+
+
+def build_driver(force: bool = False) -> str:
+    build()
+    deps = [DRIVER_SRC, os.path.join(INCLUDE, "pixreco_driver.h"), os.path.join(INCLUDE, "pixreco.h")]
+    if force or not os.path.exists(DRIVER_LIB) or any(os.path.getmtime(d) > os.path.getmtime(DRIVER_LIB) for d in deps):
+        tmp = DRIVER_LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-I", INCLUDE, "-o", tmp, DRIVER_SRC,
+                               "-L", _HERE, "-l:libpixreco.so", "-Wl,-rpath,$ORIGIN"])
+        os.replace(tmp, DRIVER_LIB)
+    return DRIVER_LIB

@@ -21,23 +21,26 @@ constexpr int kLookBack = 8;                                         // predeces
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
-constexpr u32 kSmemDigis = 2048;      // modules with more digis use the global workspace tier
-constexpr u32 kSmemClusters = 512;    // likewise for per-cluster accumulators
-constexpr u32 kDenseDigis = 8192;     // the same tiers of k_dense (two CTAs per SM with their own, larger shared memory)
-constexpr u32 kDenseClusters = 512;
+constexpr u32 kUnitCap = 2047;        // digis of one unit (consecutive modules of one event) on the fast path: 11-bit local index
+constexpr u32 kMaxGroup = 16;         // modules per unit at most (4-bit module index inside the hash key)
+constexpr u32 kDenseDigis = 8192;     // shared-memory tiers of k_dense (one module per CTA); beyond: global workspace
+constexpr u32 kDenseClusters = 384;
+constexpr u32 kAccWords = 14;         // u32 accumulators / record words per cluster (see k_cluster.cuh)
+constexpr u32 kMaxModuleDigis = (1u << 17) - 1u;   // A9: the exact sums are overflow-free up to 2^17 digis per module; more -> PR_STATUS_CAPACITY
 
-// Per-event device counters (lives in the slot's control block, zeroed per acquire).
+// Per-event device counters.  They live in the slot's control block, which is ALL ZERO between acquires: whoever
+// uses a word last puts the zero back (no per-acquire memset).
 struct DevCounters {
-  u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, pad;
+  u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, unitsDone;
 };
-// Per-launch control words (zeroed per acquire).
+// Per-launch control words (all zero between acquires).
 struct LaunchCtl {
-  u32 modTicket, modDone;
+  u32 tileTicket, unpackExited;     // k_unpack: next tile of the launch, CTAs that have left
+  u32 unitTicket, clusterExited;    // k_cluster / k_dense: next unit, CTAs that have left
   u64 tStart;                       // %globaltimer at the start of the acquire's first kernel
-  u32 nBig, bigTicket;              // modules handed from k_cluster to k_dense, next one to take
   u32 pad[10];
 };
-// What the host reads after completion (mapped pinned memory, written by the last block).
+// What the host reads after completion (mapped pinned memory, written by the CTA that finishes the event).
 struct HostCounters {
   u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, seq;
   u64 tStart, tEnd;                 // %globaltimer: first kernel of the acquire started, this event's counters published
@@ -65,13 +68,15 @@ struct EvDesc {
   u32* modClusStart;                // [M+1]
   // cluster SoA [cap]
   u32 *clLabel, *clSize; u16* clModule; float *clCharge, *clRow, *clCol;
-  // global workspace tier for large modules [cap] each
-  u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy;
+  // hit SoA [cap], hit k belongs to cluster k (A26-A30)
+  float *htX, *htY, *htXerr, *htYerr; u32 *htRows, *htCols; u16* htFlags;
+  // global workspace tier of the dense path [cap] each (modules beyond the shared-memory tiers)
+  u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum;
+  u32* wsAcc;                       // [kAccWords * cap] per-cluster accumulators
+  u32* stage;                       // [kAccWords * cap] finished cluster records of units that could not be written in place
   HostCounters* hostCounters;
-  u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
-  u32* grpCount;                    // [ceil(M / 32)] the same summed over groups of kFinMods modules (zeroed per acquire)
-  // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
-  double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
+  DevCounters* result;              // device copy of the event's final counters (per acquire; k_export reads its sizes there)
+  u32* grpAgg;                      // [nGroups] kept clusters of each unit | ready bit (numbering look-back)
 };
 static_assert(offsetof(EvDesc, label) == 128, "k_unpack's part of the descriptor is one 128-byte line");
 
@@ -81,6 +86,7 @@ struct Geom {
   u32 bitmapWords;                  // (R+2)*stride + 1
   float pixThr;
   i64 clusThrFixed;                 // llrint(clusThr * 2^14)
+  double pitchRow, pitchCol;        // um per row index (local x) / col index (local y), A26
   const float2* calib;              // device [M]: (gain, pedestal)
 };
 

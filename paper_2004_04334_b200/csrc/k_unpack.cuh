@@ -6,10 +6,15 @@
 namespace pixreco {
 
 // ================================================================== k_unpack (a1 + a2)
-// Persistent CTAs; CTA b takes tiles b, b + gridDim.x, ... of the launch (a tile = kTileWords
-// consecutive words of one event; the grid never exceeds what is co-resident, because the
-// look-back reads states published by CTAs that must be running).  "Local tile k" below is the
-// k-th tile of this CTA.  Per iteration i the CTA does, with two barriers:
+// Persistent CTAs; a tile = kTileWords consecutive words of one event.  Tiles are handed out by an ATOMIC TICKET
+// (LaunchCtl::tileTicket) in launch order, drawn by the control warp six tiles ahead of the scatter: a tile is only
+// ever owned by a CTA that is running, and a CTA works through its tiles in ascending order, so the look-back (which
+// reads states published by the owners of earlier tiles) makes progress whatever the order or the moment in which the
+// hardware starts the CTAs — also beside other kernels that fill part of the GPU.  `pro` (1..7) bounds the tiles a CTA
+// holds at a time (7 = a full pipeline): small launches spread one tile per CTA (the pipeline then runs with bubbles), large ones keep the
+// pipeline full.  "Local tile k" below is the k-th slot of this CTA's pipeline (a tile, a bubble, or the end mark).
+// The last CTA to leave puts the zeros back into the ticket and the look-back states (the control block is all zero
+// between acquires: no per-acquire memset).  Per iteration i the CTA does, with two barriers:
 //   load    (end of iteration i)  one thread issues TMA bulk copies (cp.async.bulk, completion on an
 //           mbarrier) of tile i + kRawSlots into the ring slot tile i just vacated: raw words and
 //           ADC values reach shared memory without passing through registers
@@ -31,10 +36,12 @@ namespace pixreco {
 constexpr int kUnpackCtasPerSM = 2;
 constexpr int kRawSlots = 4;                      // raw tiles in the shared-memory ring
 constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
-constexpr int kDescRing = 8;                      // descriptor ring (batch), power of two >= kRawSlots + 2
+constexpr int kDescRing = 8;                      // descriptor / tile-index ring, power of two >= kRawSlots + 4
+constexpr int kDrawAhead = 6;                     // a ticket drawn in iteration i becomes local tile i + kDrawAhead
+constexpr u32 kTileSkip = 0xFFFFFFFEu, kTileEnd = 0xFFFFFFFFu;   // pipeline slot without a tile: a bubble / no more tiles
 constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
 static_assert(kCountAhead >= 1 && kCountAhead <= kRawSlots - 2, "a raw tile needs a full iteration to arrive before it is counted");
-static_assert(kRawSlots + 2 <= kDescRing, "descriptor ring too small");
+static_assert(kRawSlots + 4 <= kDescRing && kDrawAhead == kRawSlots + 2, "rings too small for the draw-ahead");
 
 struct __align__(128) UnpackShared {
   u32 words[kRawSlots][kTileWords];               // raw ring (TMA destination)
@@ -47,6 +54,8 @@ struct __align__(128) UnpackShared {
   u32 wcnt[kRawSlots][8], wmax[kRawSlots][8];     // per warp: digis, max(module)+1
   u32 g0[2], carry1[2];                           // look-back result of local tile k at [k & 1]
   u32 desc[kDescRing][32];                        // batch: first 128 bytes of the tiles' event descriptors
+  u32 tile[kDescRing];                            // tile index (ticket) of local tile k at [k & 7], or kTileSkip / kTileEnd
+  u32 last;                                       // this CTA is the last one to leave
 };
 
 __device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
@@ -76,39 +85,30 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-#ifdef PIXRECO_TRACE
-__device__ unsigned long long g_trace[1024 * 32];
-#define TR_T(v) long long v; asm volatile("mov.u64 %0, %%clock64;" : "=l"(v) :: "memory")
-#define TR_ADD(slot, t0) do { long long t1_; asm volatile("mov.u64 %0, %%clock64;" : "=l"(t1_) :: "memory"); trAcc[slot] += (unsigned long long)(t1_ - (t0)); } while (0)
-#else
-#define TR_T(v)
-#define TR_ADD(slot, t0)
-#endif
 template <bool kSingle>
 __global__ void __launch_bounds__(kUnpackThreads + 64, kUnpackCtasPerSM)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
-         u32 totalTiles, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+         u32 totalTiles, u32 pro, LaunchCtl* __restrict__ lc, u64* __restrict__ tileStateAll, const __grid_constant__ Geom g) {
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
-  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u, G = gridDim.x;
-  const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA; warp 9 publishes and looks back
-  const u32 first = blockIdx.x;
-  if (first >= totalTiles) return;
-  if (first == 0 && tid == 0) lc->tStart = global_timer();
-#ifdef PIXRECO_TRACE
-  unsigned long long trAcc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  const long long trStart = clock64();
-#endif
-  const int nLocal = (int)((totalTiles - first + G - 1u) / G);
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u;
+  const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA and draws the tickets; warp 9 publishes and looks back
   const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
   auto desc_of = [&](int k) -> const EvDesc& {
     return kSingle ? single : *reinterpret_cast<const EvDesc*>(sh.desc[k & (kDescRing - 1)]);
   };
-  // ---- load of local tile k into its ring slot, by the control warp: TMA for the 16-byte multiple, lanes for the tail
+  auto tile_of = [&](int k) -> u32 { return sh.tile[k & (kDescRing - 1)]; };   // < totalTiles iff local tile k is a tile
+  // ---- load of local tile k into its ring slot, by the control warp: TMA for the 16-byte multiple, lanes for the tail.
+  // A slot without a tile still completes its barrier phase (0 bytes), so phase parity follows the local index.
   auto issue_load = [&](int k) {
+    const u32 t = tile_of(k), slot = (u32)k % kRawSlots;
+    if (t >= totalTiles) {
+      if (lane == 0) mbar_expect_tx(&sh.full[slot], 0u);
+      return;
+    }
     const EvDesc& e = desc_of(k);
-    const u32 T0 = (first + (u32)k * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
-    const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)k % kRawSlots;
+    const u32 T0 = (t - e.tileBase) * (u32)kTileWords, W = e.nWords;
+    const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u;
     const u32 n4 = nIn & ~3u, n8 = nIn & ~7u;
     if (lane == 0) {
       mbar_expect_tx(&sh.full[slot], n4 * 4u + n8 * 2u);
@@ -119,40 +119,51 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     if (lane < nIn - n8) sh.adc[slot][n8 + lane] = __ldcs(e.adc + T0 + n8 + lane);
   };
 
-  // ---- prologue: barriers, the first descriptors, the first loads
+  // ---- prologue: barriers, the first block of tickets (local tiles 0 .. kDrawAhead - 1), their descriptors and loads
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kRawSlots; ++s) mbar_init(&sh.full[s], 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const u32 blk = min(pro, (u32)kDrawAhead);               // the first block of consecutive tiles: one atomic
+    const u32 t0 = atomicAdd(&lc->tileTicket, blk);
+    if (t0 == 0u) lc->tStart = global_timer();
+#pragma unroll
+    for (u32 j = 0; j < (u32)kDescRing; ++j)
+      sh.tile[j] = j < blk ? (t0 + j < totalTiles ? t0 + j : kTileEnd) : (j < (u32)kDrawAhead && t0 + blk <= totalTiles ? kTileSkip : kTileEnd);
+    sh.last = 0u;
   }
-  u32 eNext = 0;                                               // batch, control warp: event of local tile i + kRawSlots + 1
-  if (!kSingle) {
-    if ((int)warp <= kRawSlots && (int)warp < nLocal)
-      sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[first + warp * G]) + lane);
-    if (ctl && kRawSlots + 1 < nLocal) eNext = tileEvent[first + (u32)(kRawSlots + 1) * G];
+  __syncthreads();
+  if (!kSingle && (int)warp < kDrawAhead && tile_of((int)warp) < totalTiles)
+    sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[tile_of((int)warp)]) + lane);
+  // control warp: tiles in flight, whether a draw came back empty, the ticket drawn in the previous iteration and its event
+  u32 inflight = 0, tktP = kTileSkip, eP = 0;
+  bool ended = false;
+  if (ctl) {
+    for (int j = 0; j < kDrawAhead; ++j) { inflight += tile_of(j) < totalTiles ? 1u : 0u; ended = ended || tile_of(j) == kTileEnd; }
   }
   __syncthreads();
   if (ctl)
-    for (int k = 0; k < kRawSlots && k < nLocal; ++k) issue_load(k);
+    for (int k = 0; k < kRawSlots; ++k) issue_load(k);
   __syncthreads();
 
-  for (int i = -kCountAhead; i < nLocal; ++i) {
-    const int kc = i + kCountAhead, kl = i + 1, kd = i + kRawSlots + 1;
-    u32 dword = 0, eN2 = 0, tl = 0;
+  for (int i = -kCountAhead;; ++i) {
+    const int kc = i + kCountAhead, kl = i + 1, kd = i + kDrawAhead - 1;
+    const u32 ti = i >= 0 ? tile_of(i) : kTileSkip;            // this iteration's tile to scatter and store
+    if (ti == kTileEnd) break;
+    const bool vi = ti < totalTiles, vc = tile_of(kc) < totalTiles, vl = tile_of(kl) < totalTiles;
+    u32 dword = 0, tkt = kTileSkip, tl = 0;
     u64 lb[kLookBack];
     if (ctl) {
-      // batch: descriptor of local tile i + kRawSlots + 1 in flight until the end of the iteration
-      if (!kSingle && i >= 0) {
-        if (kd < nLocal) dword = __ldg(reinterpret_cast<const u32*>(batch + eNext) + lane);
-        if (kd + 1 < nLocal) eN2 = tileEvent[first + (u32)(kd + 1) * G];
-      }
-      { TR_T(t0); if (lane == 0 && i > 0) bulk_wait_read(); TR_ADD(0, t0); }   // the staging arrays are free again
-    } else if (!scn && kc < nLocal) {
+      // a new ticket (it becomes local tile i + kDrawAhead); the descriptor of the one drawn an iteration ago
+      if (i >= 0 && !ended && inflight < pro && lane == 0) tkt = atomicAdd(&lc->tileTicket, 1u);
+      if (!kSingle && tktP < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(batch + eP) + lane);
+      if (lane == 0 && i > 0) bulk_wait_read();               // the staging arrays are free again
+    } else if (!scn && vc) {
       // ---- count: local tile i + kCountAhead
       const EvDesc& e = desc_of(kc);
-      const u32 T0 = (first + (u32)kc * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 T0 = (tile_of(kc) - e.tileBase) * (u32)kTileWords, W = e.nWords;
       const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)kc % kRawSlots;
-      { TR_T(t0); mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u); if (warp == 0) TR_ADD(1, t0); }
+      mbar_wait(&sh.full[slot], ((u32)kc / kRawSlots) & 1u);
       const u32* wseg = sh.words[slot] + 256u * warp + lane;
       u32 cnt = 0, mx = 0, myb = 0;
       const u32 inWarp = nIn > 256u * warp ? nIn - 256u * warp : 0u;      // words of this warp's segment that exist
@@ -181,25 +192,25 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       mx = __reduce_max_sync(0xFFFFFFFFu, mx);
       if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
     }
-    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(2, t0); }                                                         // #1
+    __syncthreads();                                                                                           // #1
     if (scn) {
       // ---- publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
-      if (kc < nLocal) {
+      if (vc) {
         const EvDesc& e = desc_of(kc);
-        const u32 tile = first + (u32)kc * G - e.tileBase, slot = (u32)kc % kRawSlots;
+        const u32 tile = tile_of(kc) - e.tileBase, slot = (u32)kc % kRawSlots;
         const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
         const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
         if (lane == 0) st_state(e.tileState + tile, pack_state(tile ? kStAgg : kStIncl, n, mx1));
       }
-      if (kl >= 0 && kl < nLocal) {
+      if (kl >= 0 && vl) {
         const EvDesc& e = desc_of(kl);
-        tl = first + (u32)kl * G - e.tileBase;
+        tl = tile_of(kl) - e.tileBase;
         if (tl) lookback_issue(e.tileState, (int)tl, lane, lb);
       }
-    } else if (!ctl && i >= 0) {
+    } else if (!ctl && vi) {
       // ---- scatter: local tile i
       const EvDesc& e = desc_of(i);
-      const u32 T0 = (first + (u32)i * G - e.tileBase) * (u32)kTileWords, W = e.nWords;
+      const u32 T0 = (ti - e.tileBase) * (u32)kTileWords, W = e.nWords;
       const u32 nIn = W > T0 ? min(W - T0, (u32)kTileWords) : 0u, slot = (u32)i % kRawSlots;
       const u32 g0 = sh.g0[i & 1], ph = g0 & 7u;
       const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u;
@@ -233,9 +244,9 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       }
       fence_async_smem();                                      // staged digis -> visible to the TMA store
     }
-    { TR_T(t0); __syncthreads(); { volatile u32* vp = sh.g0; u32 dummy = vp[0]; asm volatile("" :: "r"(dummy) : "memory"); } TR_ADD(3, t0); }                                                         // #2
+    __syncthreads();                                                                                           // #2
     if (ctl) {
-      if (i >= 0) {
+      if (vi) {
         const EvDesc& e = desc_of(i);
         const u32 slot = (u32)i % kRawSlots, g0 = sh.g0[i & 1], ph = g0 & 7u;
         const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
@@ -249,7 +260,6 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
           }
           bulk_commit();
         }
-        if (i + kRawSlots < nLocal) issue_load(i + kRawSlots);   // into the slot this tile vacated
         if (lane < 16u) {
           // head (k < 8) and tail (k >= n - 8) digis outside the 16-byte-aligned middle
           const u32 lo = 8u + ph, k = lane < 8u ? lane : n - 16u + lane, p = g0 + k;
@@ -259,28 +269,39 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
             e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
           }
         }
+        --inflight;
       }
-      if (!kSingle && i >= 0) {
-        if (kd < nLocal) sh.desc[kd & (kDescRing - 1)][lane] = dword;
-        eNext = eN2;
+      if (i >= 0) issue_load(i + kRawSlots);                   // into the slot this tile vacated (its ring entry was written an iteration ago)
+      if (i >= 1) {
+        // ring entry of local tile i + kDrawAhead - 1: the ticket drawn in the previous iteration
+        if (!kSingle && tktP < totalTiles) sh.desc[kd & (kDescRing - 1)][lane] = dword;
+        if (lane == 0) sh.tile[kd & (kDescRing - 1)] = tktP < totalTiles ? tktP : (ended ? kTileEnd : kTileSkip);
       }
+      if (i >= 0) {
+        // this iteration's draw: its event now, its descriptor in the next iteration
+        tkt = __shfl_sync(0xFFFFFFFFu, tkt, 0);
+        if (tkt < totalTiles) { ++inflight; if (!kSingle) eP = tileEvent[tkt]; }
+        else if (tkt != kTileSkip) ended = true;               // the launch has no more tiles
+        tktP = tkt;
+      }
+      __syncwarp();
     } else if (scn) {
       // ---- resolve the look-back of tile i + 1 (its loads flew during the scatter), publish its inclusive state
-      if (kl >= 0 && kl < nLocal) {
+      if (kl >= 0 && vl) {
         const EvDesc& e = desc_of(kl);
         const u32 slot = (u32)kl % kRawSlots;
         u32 c = 0, m = 0;
         if (tl) {
-          { TR_T(t0); lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m); TR_ADD(6, t0); }
+          lookback_resolve(e.tileState, (int)tl, lane, lb, &c, &m);
           const u32 n = __reduce_add_sync(0xFFFFFFFFu, lane < 8u ? sh.wcnt[slot][lane] : 0u);
           const u32 mx1 = __reduce_max_sync(0xFFFFFFFFu, lane < 8u ? sh.wmax[slot][lane] : 0u);
           if (lane == 0) st_state(e.tileState + tl, pack_state(kStIncl, c + n, max(m, mx1)));
         }
         if (lane == 0) { sh.g0[kl & 1] = c; sh.carry1[kl & 1] = m; }
       }
-    } else if (i >= 0) {
+    } else if (vi) {
       const EvDesc& e = desc_of(i);
-      const u32 tile = first + (u32)i * G - e.tileBase, slot = (u32)i % kRawSlots;
+      const u32 tile = ti - e.tileBase, slot = (u32)i % kRawSlots;
       const u32 g0 = sh.g0[i & 1], ph = g0 & 7u, carry1 = sh.carry1[i & 1];
       const u32 c8 = lane < 8u ? sh.wcnt[slot][lane] : 0u, m8 = lane < 8u ? sh.wmax[slot][lane] : 0u;
       const u32 n = __reduce_add_sync(0xFFFFFFFFu, c8), tileMax1 = __reduce_max_sync(0xFFFFFFFFu, m8);
@@ -341,15 +362,18 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     }
   }
   if (ctl && lane == 0) bulk_wait_all();
-#ifdef PIXRECO_TRACE
-  if (lane == 0 && blockIdx.x < 1024) {
-    unsigned long long* o = g_trace + blockIdx.x * 32;
-    o[warp * 2] = trAcc[2]; o[warp * 2 + 1] = trAcc[3];
-    if (ctl) { o[20] = trAcc[0]; o[22] = (unsigned long long)(clock64() - trStart); }
-    if (scn) o[21] = trAcc[6];
-    if (warp == 0) o[23] = trAcc[1];
+  // ---- the last CTA to leave puts the zeros back: look-back states and ticket words
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    sh.last = atomicAdd(&lc->unpackExited, 1u) == gridDim.x - 1u ? 1u : 0u;
   }
-#endif
+  __syncthreads();
+  if (sh.last) {
+    __threadfence();
+    for (u32 t = tid; t < totalTiles; t += kUnpackThreads + 64) tileStateAll[t] = 0ull;
+    if (tid == 0) { lc->tileTicket = 0u; lc->unpackExited = 0u; }
+  }
 }
 
 }  // namespace pixreco

@@ -2,14 +2,14 @@
 //
 //   k_unpack   a1+a2 fused: raw word decode, calibration, STABLE digi/error compaction with a
 //              single-pass decoupled look-back scan, modDigiStart, input-order check; TMA bulk
-//              loads into a shared-memory ring, staged SoA output written by TMA bulk stores.
-//   k_cluster  a3+a4 fused: per-module 8-connected components (one warp per pack of small modules:
-//              all in registers; per module of 33..256 digis: hash look-up + label equivalence in
-//              shared memory; CTA per large module: bitmap + rank look-up + min-index union-find),
-//              exact cluster sums, cluster threshold, per-module numbering.
-//   k_dense    the large-module path of k_cluster as a kernel of its own (larger shared-memory tiers), used
-//              by launches whose modules are large on average.
-//   k_finalize event-wide dense cluster numbering, cluster SoA, modClusStart, counters to the host.
+//              loads into a shared-memory ring, staged SoA output written by TMA bulk stores; tiles
+//              handed out by an atomic ticket.
+//   k_cluster  a3+a4+hits fused, one CTA per unit of consecutive modules, one thread per digi:
+//              shared-memory hash + min-index union-find, exact cluster sums by 32-bit limb
+//              reductions, cluster threshold, EVENT-WIDE numbering by a look-back over the units,
+//              cluster and hit tables, counters to the host.  One pass, nothing re-read.
+//   k_dense    the same for launches whose modules are large on average: one module per CTA,
+//              occupancy bitmap + popcount ranks + union-find, larger shared-memory tiers.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
 //
 // Kernels are batch-capable: a launch processes nEv independent events described by EvDesc
@@ -23,4 +23,4 @@
 #include "common.cuh"
 #include "k_unpack.cuh"
 #include "k_cluster.cuh"
-#include "k_finalize.cuh"
+#include "k_export.cuh"

@@ -25,6 +25,7 @@ using namespace pixreco;
 namespace {
 enum SlotState { kIdle = 0, kInFlight = 1, kDone = 2 };
 constexpr uint32_t kMaxBatch = 4096;
+constexpr uint32_t kMaxExportItems = 25;      // arrays of one event that can get a host mirror
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 }  // namespace
@@ -43,7 +44,7 @@ struct pr_handle {
   std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
   std::atomic<int> sticky{0};
   bool timing = false;
-  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msFinalize = 0, msExport = 0;   // guarded by mu
+  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msExport = 0;   // guarded by mu
   std::string lastCuda;
 };
 
@@ -61,18 +62,23 @@ struct pr_event {
   cudaEvent_t done = nullptr;
   cudaStream_t stream = nullptr;
   uint32_t n = 0;
-  std::vector<SubEvent> sub;
+  std::vector<SubEvent> sub;                 // grows only: no heap traffic in steady state
+  std::vector<uint32_t*> stW; std::vector<uint16_t*> stA; std::vector<ExportItem> items;   // per-acquire scratch, kept
   // per-acquire pool blocks
   void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr;
-  // persistent per-slot blocks (grown on demand)
+  // persistent per-slot blocks (grown on demand).  The control block is ALL ZERO between acquires: the kernels put the
+  // zeros back themselves, so it is cleared only when it is (re)allocated.
   void* ctl = nullptr; size_t ctlBytes = 0;
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
   int status = PR_OK;        // filled when completion is observed
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
-  cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, finalize, export
+  std::atomic<int> cbPending{0};             // a completion callback is queued and has not returned yet
+  cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, export
   bool exported = false;
   bool transferStage = false;  // the work in flight is a pr_transfer: completion does not count the events again
   std::vector<void*> extraHost, extraDev;  // pinned / device blocks of pr_transfer stages, returned at release
+  // last validated input pointers (their memory kind is not asked again)
+  const void *lastWords = nullptr, *lastAdc = nullptr; uint32_t lastKind = 0;
 };
 
 namespace {
@@ -112,12 +118,12 @@ void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, ui
   d.modDigiStart = c.take<u32>(M + 4); d.modClusStart = c.take<u32>(M + 4);
   d.clLabel = c.take<u32>(cap); d.clSize = c.take<u32>(cap); d.clModule = c.take<u16>(cap);
   d.clCharge = c.take<float>(cap); d.clRow = c.take<float>(cap); d.clCol = c.take<float>(cap);
-  d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
-  d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
-  d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap);
-  d.modCount = c.take<u32>(M + 4);
-  d.stS = c.take<double>(cap); d.stSx = c.take<double>(cap); d.stSy = c.take<double>(cap);
-  d.stLabel = c.take<u32>(cap); d.stSize = c.take<u32>(cap);
+  d.htX = c.take<float>(cap); d.htY = c.take<float>(cap); d.htXerr = c.take<float>(cap); d.htYerr = c.take<float>(cap);
+  d.htRows = c.take<u32>(cap); d.htCols = c.take<u32>(cap); d.htFlags = c.take<u16>(cap);
+  d.result = c.take<DevCounters>(1);
+  // touched only by units beyond the shared-memory caps
+  d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap); d.wsKnum = c.take<int32_t>(cap);
+  d.wsAcc = c.take<u32>((size_t)cap * kAccWords); d.stage = c.take<u32>((size_t)cap * kAccWords);
 }
 
 void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M) {
@@ -133,6 +139,10 @@ void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M
     o.h_mod_clus_start = c.take<uint32_t>(M + 4);
   }
   if (want & PR_WANT_ERRORS) { o.h_err_word = c.take<uint32_t>(cap); o.h_err_idx = c.take<uint32_t>(cap); }
+  if (want & PR_WANT_HITS) {
+    o.h_ht_x = c.take<float>(cap); o.h_ht_y = c.take<float>(cap); o.h_ht_xerr = c.take<float>(cap); o.h_ht_yerr = c.take<float>(cap);
+    o.h_ht_rows = c.take<uint32_t>(cap); o.h_ht_cols = c.take<uint32_t>(cap); o.h_ht_flags = c.take<uint16_t>(cap);
+  }
 }
 
 int status_to_code(uint32_t bits) {
@@ -151,6 +161,7 @@ void CUDART_CB trampoline(void* p) {
   }
   ev->h->callbacks.fetch_add(1);
   if (ev->doneFn) ev->doneFn(ev->doneUser, worst);
+  ev->cbPending.store(0, std::memory_order_release);   // only now may the slot be released, re-armed or destroyed
 }
 
 void release_blocks(pr_event* ev, bool completed) {
@@ -164,6 +175,54 @@ void release_blocks(pr_event* ev, bool completed) {
   ev->extraHost.clear(); ev->extraDev.clear();
 }
 
+// Whether [p, p + bytes) is memory of the kind the caller declared.  Pointers inside a live block of the handle's own
+// pinned pool (pr_host_alloc) and the pointers validated by the slot's previous acquire need no CUDA call.
+bool kind_ok(pr_event* ev, const void* words, const void* adc, uint32_t kind) {
+  if (ev->lastKind == kind && ev->lastWords == words && ev->lastAdc == adc) return true;
+  pr_handle* h = ev->h;
+  bool ok;
+  uintptr_t base; size_t bytes;
+  if (kind == PR_MEM_HOST_PINNED && h->hostPool->find_live(words, &base, &bytes) && h->hostPool->find_live(adc, &base, &bytes)) ok = true;
+  else {
+    cudaPointerAttributes pa{}, pb{};
+    if (cudaPointerGetAttributes(&pa, words) != cudaSuccess || cudaPointerGetAttributes(&pb, adc) != cudaSuccess) {
+      cudaGetLastError();
+      return false;
+    }
+    const cudaMemoryType need = kind == PR_MEM_DEVICE ? cudaMemoryTypeDevice : cudaMemoryTypeHost;
+    ok = pa.type == need && pb.type == need;     // pageable host memory would make the copy synchronous
+  }
+  if (ok) { ev->lastWords = words; ev->lastAdc = adc; ev->lastKind = kind; }
+  return ok;
+}
+
+// Something failed after work was queued: the slot goes back to idle, its blocks return to the pool tagged with the
+// stream (reused elsewhere only after what was queued has run), the control block is dropped (its zeros are not
+// guaranteed any more).  The handle is sticky-failed by PR_CUDA already.
+int fail_after_enqueue(pr_event* ev, int code) {
+  pr_handle* h = ev->h;
+  release_blocks(ev, false);
+  if (ev->ctl) { h->devPool->free(ev->ctl, ev->stream, false); ev->ctl = nullptr; ev->ctlBytes = 0; }
+  ev->state = kIdle; ev->n = 0;
+  return code;
+}
+#define PR_CUDA_Q(ev, call)                                 \
+  do {                                                      \
+    cudaError_t e__ = (call);                               \
+    if (e__ != cudaSuccess) return fail_after_enqueue((ev), cuda_fail((ev)->h, e__, #call)); \
+  } while (0)
+
+// Modules per unit of k_cluster: a power of two <= kMaxGroup with a few hundred digis per unit, and enough units to
+// fill the GPU when the launch allows it.
+uint32_t pick_group(pr_handle* h, uint64_t totalWords, uint32_t n, uint32_t M) {
+  const double perModule = (double)totalWords / ((double)n * M) + 1e-9;
+  uint32_t G = kMaxGroup;
+  while (G > 1 && perModule * G > 448.0) G >>= 1;
+  const uint64_t resident = (uint64_t)h->smCount * h->clusterBlocksPerSM;
+  while (G > 2 && (uint64_t)n * ((M + G - 1) / G) < resident / 2) G >>= 1;
+  return G;
+}
+
 int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
   if (!ev || !ins || n == 0 || n > kMaxBatch) return PR_ERR_INVALID_ARG;
   pr_handle* h = ev->h;
@@ -171,7 +230,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (ev->state != kIdle) return PR_ERR_BAD_STATE;
   const uint32_t M = h->cfg.n_modules, kind = ins[0].mem_kind, want = ins[0].want;
   if (kind != PR_MEM_HOST_PINNED && kind != PR_MEM_DEVICE) return PR_ERR_INVALID_ARG;
-  if (want & ~0x1Fu) return PR_ERR_INVALID_ARG;
+  if (want & ~PR_WANT_ALL) return PR_ERR_INVALID_ARG;
   PR_CUDA(h, cudaSetDevice(h->cfg.device));
   for (uint32_t k = 0; k < n; ++k) {
     const pr_input& in = ins[k];
@@ -180,20 +239,15 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     if (in.n_words > 0xFFFFFFF0u - kTileWords) return PR_ERR_INVALID_ARG;
     if (in.n_words) {
       if (kind == PR_MEM_DEVICE && (((uintptr_t)in.words | (uintptr_t)in.adc) & 15u)) return PR_ERR_INVALID_ARG;
-      cudaPointerAttributes pa{}, pb{};
-      if (cudaPointerGetAttributes(&pa, in.words) != cudaSuccess || cudaPointerGetAttributes(&pb, in.adc) != cudaSuccess) {
-        cudaGetLastError();
-        return PR_ERR_INVALID_ARG;
-      }
-      const cudaMemoryType need = kind == PR_MEM_DEVICE ? cudaMemoryTypeDevice : cudaMemoryTypeHost;
-      if (pa.type != need || pb.type != need) return PR_ERR_INVALID_ARG;   // pageable host memory would make the copy synchronous
+      if (!kind_ok(ev, in.words, in.adc, kind)) return PR_ERR_INVALID_ARG;
     }
   }
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const bool stage = kind == PR_MEM_HOST_PINNED;
 
-  // ---- host inputs of a batch that form one nearly dense span per array (a DAQ buffer, the bench's pool) are staged
-  // by ONE copy per array, each event keeping its offset inside the span; otherwise one copy per event and array
+  // ---- host inputs of a batch that lie in ONE pinned block of the handle's pool and form a nearly dense span per array (a
+  // DAQ buffer from pr_host_alloc, the bench's pool) are staged by ONE copy per array, each event keeping its offset
+  // inside the span; anything else gets one copy per event and array (the gaps of a span were never handed to the library)
   uintptr_t wLo = ~(uintptr_t)0, wHi = 0, aLo = ~(uintptr_t)0, aHi = 0;
   bool merged = false;
   if (stage && n > 1) {
@@ -206,14 +260,20 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       wSum += 4 * (size_t)ins[k].n_words; aSum += 2 * (size_t)ins[k].n_words;
     }
     merged = wSum > 0 && wHi - wLo <= wSum + wSum / 4 + 4096 && aHi - aLo <= aSum + aSum / 4 + 4096;
+    if (merged) {
+      uintptr_t bw, ba; size_t sw, sa;
+      merged = h->hostPool->find_live((const void*)wLo, &bw, &sw) && wHi <= bw + sw &&
+               h->hostPool->find_live((const void*)aLo, &ba, &sa) && aHi <= ba + sa;
+    }
     for (uint32_t k = 0; merged && k < n; ++k)
       if (ins[k].n_words && ((((uintptr_t)ins[k].words - wLo) | ((uintptr_t)ins[k].adc - aLo)) & 15u)) merged = false;   // TMA wants 16-byte alignment
   }
 
   // ---- layout
-  ev->sub.assign(n, SubEvent());
+  if (ev->sub.size() < n) { ev->sub.resize(n); ev->stW.resize(n); ev->stA.resize(n); }
   size_t devBytes = merged ? align_up(wHi - wLo, 256) + align_up(aHi - aLo, 256) : 0, hostBytes = 0;
   uint32_t totalTiles = 0;
+  uint64_t totalWords = 0;
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     s.in = ins[k];
@@ -222,24 +282,26 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     carve_device(cd, tmp, s.cap, M, stage && !merged, &sw, &sa);
     devBytes += cd.off;
     if (want) { Carver ch(nullptr); pr_output o{}; carve_host(ch, o, want, s.cap, M); hostBytes += ch.off; }
+    s.desc = EvDesc{};
     s.desc.tileBase = totalTiles;
     s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
     totalTiles += s.desc.nTiles;
+    totalWords += s.in.n_words;
   }
-  const size_t grpPerEv = align_up((M + 31) / 32, 16);      // u32 per event
-  uint64_t totalWords = 0;
-  for (uint32_t k = 0; k < n; ++k) totalWords += ins[k].n_words;
-  // launches whose modules are large on average (configs[4]) hand their large modules to k_dense
-  const bool denseKernel = totalWords > (uint64_t)kWarpCap * M * n;
-  const size_t bigCap = denseKernel ? (size_t)(totalWords / (kWarpCap + 1) + 2) : 0;
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + 4 * grpPerEv * n + 4 * bigCap;
+  // launches whose modules are large on average (configs[4]) go to k_dense: one module per unit
+  const bool denseKernel = totalWords > (uint64_t)256 * M * n;
+  const uint32_t G = denseKernel ? 1u : pick_group(h, totalWords, n, M);
+  const uint32_t nGroups = (M + G - 1) / G;
+  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + (size_t)4 * nGroups * n;
 
   // ---- buffers from the pools (steady state: cache hits only)
+  bool ctlFresh = false;
   if (ev->ctlBytes < ctlNeed) {
     if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
     ev->ctl = h->devPool->alloc(ctlNeed, stream);
     ev->ctlBytes = ev->ctl ? (size_t)bin_bytes_for(ctlNeed) : 0;
     if (!ev->ctl) return PR_ERR_OOM;
+    ctlFresh = true;
   }
   if (ev->hostCountersCap < n) {
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
@@ -256,7 +318,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   }
   // one block, one H2D copy: event descriptors and the tile -> event map (batches), then the export table (mirrors)
   const size_t descPart = n > 1 ? align_up(sizeof(EvDesc) * n + sizeof(u16) * totalTiles, 16) : 0;
-  const size_t descBytes = descPart + (want ? sizeof(ExportItem) * 18 * n : 0);
+  const size_t descBytes = descPart + (want ? sizeof(ExportItem) * kMaxExportItems * n : 0);
   if (descBytes) {
     ev->descStage = h->hostPool->alloc(descBytes, stream);
     ev->descDev = h->devPool->alloc(descBytes, stream);
@@ -268,71 +330,61 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   LaunchCtl* lc = (LaunchCtl*)ctl;
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
   u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
-  u32* bigList = denseKernel ? (u32*)(tileState + totalTiles) + grpPerEv * n : nullptr;
+  u32* grpAgg = (u32*)(tileState + totalTiles);
   Carver cd(ev->devSlab), ch(ev->hostSlab);
-  std::vector<uint32_t*> stW(n, nullptr); std::vector<uint16_t*> stA(n, nullptr);
   char *spanW = nullptr, *spanA = nullptr;
   if (merged) { spanW = cd.take<char>(wHi - wLo); spanA = cd.take<char>(aHi - aLo); }
   for (uint32_t k = 0; k < n; ++k) {
     SubEvent& s = ev->sub[k];
     EvDesc& d = s.desc;
-    carve_device(cd, d, s.cap, M, stage && !merged, &stW[k], &stA[k]);
+    ev->stW[k] = nullptr; ev->stA[k] = nullptr;
+    carve_device(cd, d, s.cap, M, stage && !merged, &ev->stW[k], &ev->stA[k]);
     if (merged && s.in.n_words) {
-      stW[k] = (uint32_t*)(spanW + ((uintptr_t)s.in.words - wLo)); stA[k] = (uint16_t*)(spanA + ((uintptr_t)s.in.adc - aLo));
+      ev->stW[k] = (uint32_t*)(spanW + ((uintptr_t)s.in.words - wLo)); ev->stA[k] = (uint16_t*)(spanA + ((uintptr_t)s.in.adc - aLo));
     }
-    d.words = stage ? stW[k] : s.in.words;
-    d.adc = stage ? stA[k] : s.in.adc;
+    d.words = stage ? ev->stW[k] : s.in.words;
+    d.adc = stage ? ev->stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
     d.tileState = tileState + d.tileBase;
-    d.grpCount = (u32*)(tileState + totalTiles) + grpPerEv * k;
+    d.grpAgg = grpAgg + (size_t)nGroups * k;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
   }
 
-  // ---- enqueue (all asynchronous, one stream: P:L82)
+  // ---- enqueue (all asynchronous, one stream: P:L82).  From here on a failure goes through fail_after_enqueue.
   uint64_t nMemcpy = 0, nLaunch = 0;
-  PR_CUDA(h, cudaMemsetAsync(ev->ctl, 0, ctlNeed, stream));
+  if (ctlFresh) PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ev->ctlBytes, stream));   // only a new control block is cleared
   if (merged) {
-    PR_CUDA(h, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
-    PR_CUDA(h, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
+    PR_CUDA_Q(ev, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
+    PR_CUDA_Q(ev, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
     nMemcpy += 2;
   } else if (stage)
     for (uint32_t k = 0; k < n; ++k) {
       const SubEvent& s = ev->sub[k];
       if (!s.in.n_words) continue;
-      PR_CUDA(h, cudaMemcpyAsync(stW[k], s.in.words, (size_t)s.in.n_words * 4, cudaMemcpyHostToDevice, stream));
-      PR_CUDA(h, cudaMemcpyAsync(stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
+      PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stW[k], s.in.words, (size_t)s.in.n_words * 4, cudaMemcpyHostToDevice, stream));
+      PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
       nMemcpy += 2;
     }
-  // k_cluster: persistent CTAs (dense scan + warp tickets).  A small launch gets one CTA per warp
-  // ticket or per possible dense module (a dense module has more than kWarpCap digis).
-  const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
-  // tickets of 4 modules when there are plenty, of 2 or 1 when the launch is small (a single event): every warp gets work
-  const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
-  const uint32_t modBatch = (uint64_t)n * M >= 4 * warpsResident ? kModBatch : (uint64_t)n * M >= 2 * warpsResident ? 2u : 1u;
-  const uint64_t warpTickets = ((uint64_t)n * ((M + modBatch - 1) / modBatch) + 7) / 8, maxDense = totalWords / (kWarpCap + 1);
-  const uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
-  uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
-  if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
-  if (clusterGrid < 1) clusterGrid = 1;
-  // k_finalize: one CTA per (event, 32 modules); huge events get several CTAs per group (about 8k words each)
-  uint32_t finSplits = (uint32_t)(totalWords / ((uint64_t)n * unitsPerEvent * 8192) + 1);
-  if (finSplits > 64) finSplits = 64;
-  uint32_t denseGrid = (uint32_t)(h->smCount * h->denseBlocksPerSM);
-  if (denseGrid > bigCap) denseGrid = bigCap ? (uint32_t)bigCap : 1u;
-  // k_unpack: persistent CTAs striding over the tiles; never more than are co-resident (its look-back
-  // waits on earlier tiles, which must therefore be running or done)
+  // k_cluster / k_dense: persistent CTAs taking units by ticket
+  const uint64_t units = (uint64_t)n * nGroups;
+  uint32_t clusterGrid = (uint32_t)(h->smCount * (denseKernel ? h->denseBlocksPerSM : h->clusterBlocksPerSM));
+  if (clusterGrid > units) clusterGrid = (uint32_t)units;
+  // k_unpack: persistent CTAs taking tiles by ticket; a CTA holds at most `pro` tiles at a time (7 = a full pipeline)
   uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
   if (unpackGrid > totalTiles) unpackGrid = totalTiles;
+  uint32_t pro = (totalTiles + unpackGrid - 1) / unpackGrid;
+  if (pro >= 4) pro = 7;
   // descriptor block: [EvDesc x n][tile -> event map] for batches, then the export table (exact-size mirrors)
-  std::vector<ExportItem> items;
+  std::vector<ExportItem>& items = ev->items;
+  items.clear();
   if (want) {
     for (uint32_t k = 0; k < n; ++k) {
       const EvDesc& d = ev->sub[k].desc; const pr_output& o = ev->sub[k].hostViews;
       auto add = [&](const void* src, const void* dst, uint32_t eb, uint32_t sel, uint32_t fixed) {
-        if (dst) items.push_back(ExportItem{src, const_cast<void*>(dst), eb, sel, fixed, k});
+        if (dst) items.push_back(ExportItem{src, const_cast<void*>(dst), d.result, eb, sel, fixed, 0u});
       };
       add(d.module, o.h_module, 2, 0, 0); add(d.row, o.h_row, 2, 0, 0); add(d.col, o.h_col, 2, 0, 0);
       add(d.adcOut, o.h_adc, 2, 0, 0); add(d.wordIdx, o.h_word_idx, 4, 0, 0);
@@ -342,6 +394,8 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       add(d.clCharge, o.h_cl_charge, 4, 2, 0); add(d.clRow, o.h_cl_row, 4, 2, 0); add(d.clCol, o.h_cl_col, 4, 2, 0);
       add(d.modClusStart, o.h_mod_clus_start, 4, 3, M + 1);
       add(d.errWord, o.h_err_word, 4, 1, 0); add(d.errIdx, o.h_err_idx, 4, 1, 0);
+      add(d.htX, o.h_ht_x, 4, 2, 0); add(d.htY, o.h_ht_y, 4, 2, 0); add(d.htXerr, o.h_ht_xerr, 4, 2, 0); add(d.htYerr, o.h_ht_yerr, 4, 2, 0);
+      add(d.htRows, o.h_ht_rows, 4, 2, 0); add(d.htCols, o.h_ht_cols, 4, 2, 0); add(d.htFlags, o.h_ht_flags, 2, 2, 0);
     }
   }
   if (descBytes) {
@@ -355,30 +409,26 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       }
     }
     if (!items.empty()) memcpy(st8 + descPart, items.data(), items.size() * sizeof(ExportItem));
-    PR_CUDA(h, cudaMemcpyAsync(ev->descDev, st8, descPart + items.size() * sizeof(ExportItem), cudaMemcpyHostToDevice, stream));
+    PR_CUDA_Q(ev, cudaMemcpyAsync(ev->descDev, st8, descPart + items.size() * sizeof(ExportItem), cudaMemcpyHostToDevice, stream));
     ++nMemcpy;
   }
-  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[0], stream));
+  if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[0], stream));
+  const EvDesc& d0 = ev->sub[0].desc;
   if (n == 1) {
-    const EvDesc& d = ev->sub[0].desc;
-    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, totalTiles, lc, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
-    if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, lc, h->geom);
+    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, nullptr, nullptr, totalTiles, pro, lc, tileState, h->geom);
+    if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
+    if (denseKernel) k_dense<true><<<clusterGrid, kDenseThreads, h->denseSmem, stream>>>(d0, nullptr, 1, lc, h->geom);
+    else k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, nullptr, 1, lc, G, nGroups, h->geom);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(ev->sub[0].desc, dd, (const u16*)(dd + n), totalTiles, lc, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[1], stream));
-    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(ev->sub[0].desc, dd, n, lc, bigList, modBatch, h->geom);
-    if (denseKernel) k_dense<false><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(ev->sub[0].desc, dd, lc, bigList, h->geom);
-    if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(ev->sub[0].desc, dd, n, unitsPerEvent, finSplits, lc, h->geom);
+    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, dd, (const u16*)(dd + n), totalTiles, pro, lc, tileState, h->geom);
+    if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
+    if (denseKernel) k_dense<false><<<clusterGrid, kDenseThreads, h->denseSmem, stream>>>(d0, dd, n, lc, h->geom);
+    else k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, dd, n, lc, G, nGroups, h->geom);
   }
-  nLaunch += denseKernel ? 4 : 3;
-  PR_CUDA(h, cudaGetLastError());
-  if (h->timing) PR_CUDA(h, cudaEventRecord(ev->tev[3], stream));
+  nLaunch += 2;
+  PR_CUDA_Q(ev, cudaGetLastError());
+  if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
   ev->exported = want != 0;
   if (want && !items.empty()) {
     const ExportItem* itab = (const ExportItem*)((const char*)ev->descDev + descPart);   // device-resident export table
@@ -389,26 +439,30 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     if (gx > 64) gx = 64;
     uint32_t gy = (uint32_t)items.size();
     if (gy > 2048) gy = 2048;
-    k_export<<<dim3(gx, gy), 256, 0, stream>>>(itab, (uint32_t)items.size(), counters);
+    k_export<<<dim3(gx, gy), 256, 0, stream>>>(itab, (uint32_t)items.size());
     ++nLaunch;
-    PR_CUDA(h, cudaGetLastError());
+    PR_CUDA_Q(ev, cudaGetLastError());
   }
-  if (h->timing && want) PR_CUDA(h, cudaEventRecord(ev->tev[4], stream));
-  PR_CUDA(h, cudaEventRecord(ev->done, stream));
+  if (h->timing && want) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[3], stream));
+  PR_CUDA_Q(ev, cudaEventRecord(ev->done, stream));
   ev->n = n;
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
   ev->status = PR_OK;
   ev->state = kInFlight;
   ev->transferStage = false;
-  if (ev->doneFn) PR_CUDA(h, cudaLaunchHostFunc(stream, trampoline, ev));
-
+  if (ev->doneFn) {
+    ev->cbPending.store(1, std::memory_order_release);
+    cudaError_t ce = cudaLaunchHostFunc(stream, trampoline, ev);
+    if (ce != cudaSuccess) {                      // the work is queued and will complete; only the callback is missing
+      ev->cbPending.store(0);
+      cuda_fail(h, ce, "cudaLaunchHostFunc");
+    }
+  }
   h->evAcquired.fetch_add(n); h->launches.fetch_add(nLaunch); h->memcpys.fetch_add(nMemcpy);
-  uint64_t w = 0;
-  for (uint32_t k = 0; k < n; ++k) w += ins[k].n_words;
-  h->words.fetch_add(w);
+  h->words.fetch_add(totalWords);
   uint32_t f = h->inFlight.fetch_add(1) + 1, mx = h->maxInFlight.load();
   while (f > mx && !h->maxInFlight.compare_exchange_weak(mx, f)) {}
-  return PR_OK;
+  return h->sticky.load() ? PR_ERR_CUDA : PR_OK;
 }
 
 // Non-blocking completion check; moves kInFlight -> kDone.
@@ -429,12 +483,11 @@ int poll(pr_event* ev) {
   ev->state = kDone;
   if (ev->transferStage) { ev->transferStage = false; ev->h->inFlight.fetch_sub(1); return PR_OK; }
   if (ev->h->timing) {
-    float a = 0, b = 0, c = 0, f = 0;
-    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess &&
-        cudaEventElapsedTime(&f, ev->tev[2], ev->tev[3]) == cudaSuccess) {
-      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[3], ev->tev[4]) != cudaSuccess) c = 0;
+    float a = 0, b = 0, c = 0;
+    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess) {
+      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[2], ev->tev[3]) != cudaSuccess) c = 0;
       std::lock_guard<std::mutex> g(ev->h->mu);
-      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msFinalize += f; ev->h->msExport += c;
+      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msExport += c;
     } else cudaGetLastError();
   }
   ev->h->inFlight.fetch_sub(1);
@@ -458,6 +511,8 @@ void fill_output(pr_event* ev, uint32_t k, pr_output* out) {
   out->d_cl_label = d.clLabel; out->d_cl_size = d.clSize; out->d_cl_module = d.clModule;
   out->d_cl_charge = d.clCharge; out->d_cl_row = d.clRow; out->d_cl_col = d.clCol;
   out->d_err_word = d.errWord; out->d_err_idx = d.errIdx;
+  out->d_ht_x = d.htX; out->d_ht_y = d.htY; out->d_ht_xerr = d.htXerr; out->d_ht_yerr = d.htYerr;
+  out->d_ht_rows = d.htRows; out->d_ht_cols = d.htCols; out->d_ht_flags = d.htFlags;
 }
 
 }  // namespace
@@ -498,6 +553,8 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||
       !std::isfinite(cfg->cluster_threshold_e) || !(std::fabs(cfg->cluster_threshold_e) < 1e12f))
     return PR_ERR_BAD_CALIB;
+  if (!(cfg->pitch_row_um >= 0.0f) || !(cfg->pitch_col_um >= 0.0f) || !std::isfinite(cfg->pitch_row_um) || !std::isfinite(cfg->pitch_col_um))
+    return PR_ERR_INVALID_ARG;
   for (uint32_t m = 0; m < cfg->n_modules; ++m) {
     const float g = cfg->gain[m], p = cfg->pedestal[m];
     if (!std::isfinite(g) || !(g > 0.0f) || !(g < 128.0f) || !std::isfinite(p) || !(std::fabs(p) < 65536.0f)) return PR_ERR_BAD_CALIB;
@@ -529,6 +586,8 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   g.bitmapWords = (g.R + 2) * g.stride + 1;
   g.pixThr = cfg->pixel_threshold_e;
   g.clusThrFixed = (i64)llrint((double)cfg->cluster_threshold_e * 16384.0);
+  g.pitchRow = cfg->pitch_row_um > 0.0f ? (double)cfg->pitch_row_um : 100.0;       // A26
+  g.pitchCol = cfg->pitch_col_um > 0.0f ? (double)cfg->pitch_col_um : 150.0;
   g.calib = h->dCalib;
   h->clusterSmem = cluster_smem_bytes(g.bitmapWords);
   if (cudaFuncSetAttribute(k_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->clusterSmem) != cudaSuccess ||
@@ -563,7 +622,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + 4 * align_up((g.M + 31) / 32, 16);
+    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + (size_t)4 * g.M;
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
@@ -589,7 +648,7 @@ int pr_destroy(pr_handle* h) {
     if (ev->ctl) h->devPool->free(ev->ctl, nullptr, true);
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
     if (ev->done) cudaEventDestroy(ev->done);
-    for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+    for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
@@ -609,7 +668,7 @@ int pr_event_create(pr_handle* h, pr_event** out) {
   cudaError_t e = cudaEventCreateWithFlags(&ev->done, cudaEventDisableTiming);
   if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
   if (h->timing)
-    for (int i = 0; i < 5; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
+    for (int i = 0; i < 4; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
   { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
   *out = ev;
   return PR_OK;
@@ -619,11 +678,12 @@ int pr_event_destroy(pr_event* ev) {
   if (!ev) return PR_ERR_INVALID_ARG;
   pr_handle* h = ev->h;
   if (ev->state == kInFlight && poll(ev) != PR_OK) return PR_ERR_BAD_STATE;
+  if (ev->cbPending.load(std::memory_order_acquire)) return PR_ERR_BAD_STATE;   // its completion callback has not returned yet
   release_blocks(ev, true);
   if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
   if (ev->done) cudaEventDestroy(ev->done);
-  for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+  for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
   {
     std::lock_guard<std::mutex> g(h->mu);
     for (size_t i = 0; i < h->slots.size(); ++i)
@@ -658,18 +718,34 @@ int pr_release(pr_event* ev) {
   if (ev->state == kIdle) return PR_ERR_BAD_STATE;
   int r = poll(ev);
   if (r != PR_OK) return r;
+  if (ev->cbPending.load(std::memory_order_acquire)) return PR_NOT_READY;   // the callback still reads the slot
   release_blocks(ev, true);                      // completion observed: reusable by any stream at once
   ev->state = kIdle;
   ev->n = 0;
   return PR_OK;
 }
 
+int pr_release_on(pr_event* ev, void* consumer_stream) {
+  if (!ev) return PR_ERR_INVALID_ARG;
+  if (ev->state == kIdle) return PR_ERR_BAD_STATE;
+  int r = poll(ev);
+  if (r != PR_OK) return r;
+  if (ev->cbPending.load(std::memory_order_acquire)) return PR_NOT_READY;
+  PR_CUDA(ev->h, cudaSetDevice(ev->h->cfg.device));
+  ev->stream = (cudaStream_t)consumer_stream;    // the pool records an event on it and defers reuse by other streams
+  release_blocks(ev, false);
+  ev->state = kIdle;
+  ev->n = 0;
+  return PR_OK;
+}
+
 int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done, void* user) {
-  if (!ev || (want & ~0x1Fu)) return PR_ERR_INVALID_ARG;
+  if (!ev || (want & ~PR_WANT_ALL)) return PR_ERR_INVALID_ARG;
   pr_handle* h = ev->h;
   if (h->sticky.load()) return PR_ERR_CUDA;
   if (ev->state == kIdle) return PR_ERR_BAD_STATE;
   if (ev->state == kInFlight && poll(ev) != PR_OK) return PR_ERR_BAD_STATE;
+  if (ev->cbPending.load(std::memory_order_acquire)) return PR_ERR_BAD_STATE;
   PR_CUDA(h, cudaSetDevice(h->cfg.device));
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const uint32_t M = h->cfg.n_modules;
@@ -701,6 +777,12 @@ int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done,
       add(d.modClusStart, (const void**)&o.h_mod_clus_start, M + 1, 4);
     }
     if (want & PR_WANT_ERRORS) { add(d.errWord, (const void**)&o.h_err_word, E, 4); add(d.errIdx, (const void**)&o.h_err_idx, E, 4); }
+    if (want & PR_WANT_HITS) {
+      add(d.htX, (const void**)&o.h_ht_x, N, 4); add(d.htY, (const void**)&o.h_ht_y, N, 4);
+      add(d.htXerr, (const void**)&o.h_ht_xerr, N, 4); add(d.htYerr, (const void**)&o.h_ht_yerr, N, 4);
+      add(d.htRows, (const void**)&o.h_ht_rows, N, 4); add(d.htCols, (const void**)&o.h_ht_cols, N, 4);
+      add(d.htFlags, (const void**)&o.h_ht_flags, N, 2);
+    }
   }
   char* slab = nullptr;
   if (total) {
@@ -727,12 +809,12 @@ int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done,
     uint32_t nItems = 0;
     for (const Copy& c : copies) {
       *c.view = slab + off;
-      if (c.bytes) htab[nItems++] = ExportItem{c.src, dstage + tabBytes + off, 1u, 3u, (uint32_t)c.bytes, 0u};
+      if (c.bytes) htab[nItems++] = ExportItem{c.src, dstage + tabBytes + off, nullptr, 1u, 3u, (uint32_t)c.bytes, 0u};
       off += align_up(c.bytes ? c.bytes : 1, 256);
     }
     if (nItems) {
       PR_CUDA(h, cudaMemcpyAsync(dstage, htab, sizeof(ExportItem) * nItems, cudaMemcpyHostToDevice, stream));
-      k_export<<<dim3(4, nItems < 2048u ? nItems : 2048u), 256, 0, stream>>>((const ExportItem*)dstage, nItems, (const DevCounters*)ev->ctl);
+      k_export<<<dim3(4, nItems < 2048u ? nItems : 2048u), 256, 0, stream>>>((const ExportItem*)dstage, nItems);
       PR_CUDA(h, cudaGetLastError());
       PR_CUDA(h, cudaMemcpyAsync(slab, dstage + tabBytes, total, cudaMemcpyDeviceToHost, stream));
       nMemcpy += 2; nLaunch += 1;
@@ -744,7 +826,11 @@ int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done,
   ev->doneFn = done; ev->doneUser = user;
   ev->state = kInFlight;
   ev->transferStage = true;
-  if (done) PR_CUDA(h, cudaLaunchHostFunc(stream, trampoline, ev));
+  if (done) {
+    ev->cbPending.store(1, std::memory_order_release);
+    cudaError_t ce = cudaLaunchHostFunc(stream, trampoline, ev);
+    if (ce != cudaSuccess) { ev->cbPending.store(0); return cuda_fail(h, ce, "cudaLaunchHostFunc"); }
+  }
   h->memcpys.fetch_add(nMemcpy);
   uint32_t f = h->inFlight.fetch_add(1) + 1, mx = h->maxInFlight.load();
   while (f > mx && !h->maxInFlight.compare_exchange_weak(mx, f)) {}
@@ -779,17 +865,9 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
   h->devPool->stats(&out->device_pool); h->hostPool->stats(&out->host_pool);
   {
     std::lock_guard<std::mutex> g(h->mu);
-    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->finalize_ms = h->msFinalize; out->export_ms = h->msExport;
+    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->export_ms = h->msExport;
   }
   return PR_OK;
 }
-
-#ifdef PIXRECO_TRACE
-int pr_debug_trace(unsigned long long* out, int n, int reset) {
-  if (out && cudaMemcpyFromSymbol(out, g_trace, sizeof(unsigned long long) * n) != cudaSuccess) return -1;
-  if (reset) { static unsigned long long z[1024 * 32]; cudaMemcpyToSymbol(g_trace, z, sizeof z); }
-  return 0;
-}
-#endif
 
 }  // extern "C"

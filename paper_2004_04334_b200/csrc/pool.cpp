@@ -41,8 +41,8 @@ struct DeviceBackend : PoolBackend {
   bool event_record(void* e, void* s) override { return cudaEventRecord((cudaEvent_t)e, (cudaStream_t)s) == cudaSuccess; }
   bool event_done(void* e) override {
     cudaError_t r = cudaEventQuery((cudaEvent_t)e);
-    if (r == cudaErrorNotReady) { cudaGetLastError(); return false; }
-    return true;                                        // success, or an error the owner will see elsewhere
+    if (r != cudaSuccess) { cudaGetLastError(); return false; }   // not ready — or an error: never hand out a block whose completion is unknown
+    return true;
   }
 };
 struct PinnedBackend : DeviceBackend {
@@ -117,7 +117,7 @@ void* CachingPool::alloc(size_t bytes, void* stream) {
       v.erase(v.begin() + pick);
       if (b->stream != stream) st_.cross_stream_reuses++;
       b->stream = stream; b->pending = false;
-      live_[b->ptr] = b;
+      live_[(uintptr_t)b->ptr] = b;
       st_.hits++; st_.bytes_cached -= b->bytes; st_.bytes_live += b->bytes;
       return b->ptr;
     }
@@ -130,7 +130,7 @@ void* CachingPool::alloc(size_t bytes, void* stream) {
   }
   Block* b = new Block();
   b->ptr = p; b->bytes = bin; b->stream = stream;
-  live_[p] = b;
+  live_[(uintptr_t)p] = b;
   st_.misses++; st_.backend_allocs++; st_.bytes_live += bin;
   st_.bytes_peak = std::max(st_.bytes_peak, st_.bytes_live + st_.bytes_cached);
   return p;
@@ -139,7 +139,7 @@ void* CachingPool::alloc(size_t bytes, void* stream) {
 int CachingPool::free(void* ptr, void* stream, bool completed) {
   if (!ptr) return PR_OK;
   std::lock_guard<std::mutex> g(mu_);
-  auto it = live_.find(ptr);
+  auto it = live_.find((uintptr_t)ptr);
   if (it == live_.end()) return PR_ERR_INVALID_ARG;
   Block* b = it->second;
   live_.erase(it);
@@ -188,6 +188,16 @@ void CachingPool::trim_locked(uint64_t keep) {
     st_.bytes_cached -= b->bytes;
     release_block_locked(b);
   }
+}
+
+bool CachingPool::find_live(const void* p, uintptr_t* base, size_t* bytes) {
+  std::lock_guard<std::mutex> g(mu_);
+  auto it = live_.upper_bound((uintptr_t)p);
+  if (it == live_.begin()) return false;
+  --it;
+  if ((uintptr_t)p >= it->first + it->second->bytes) return false;
+  *base = it->first; *bytes = (size_t)it->second->bytes;
+  return true;
 }
 
 int CachingPool::trim(uint64_t keep) {

@@ -9,6 +9,7 @@
 #pragma once
 #include <cstddef>
 #include <cstdint>
+#include <map>
 #include <mutex>
 #include <unordered_map>
 #include <vector>
@@ -47,6 +48,8 @@ class CachingPool {
   int   trim(uint64_t keep_cached_bytes);
   void  stats(pr_pool_stats* out);
   void  fake_complete(void* stream) { backend_->fake_complete(stream); }
+  // The live (handed out) block that contains p: its start and size.  False if p is not inside one.
+  bool  find_live(const void* p, uintptr_t* base, size_t* bytes);
 
  private:
   struct Block {
@@ -64,7 +67,7 @@ class CachingPool {
   uint64_t max_cached_;
   std::mutex mu_;
   std::unordered_map<uint64_t, std::vector<Block*>> free_;   // bin bytes -> idle blocks
-  std::unordered_map<void*, Block*> live_;
+  std::map<uintptr_t, Block*> live_;                         // by start address (find_live looks up a containing block)
   pr_pool_stats st_{};
   uint64_t seq_ = 0;
 };

@@ -1,0 +1,87 @@
+// stream_driver.cpp — see include/pixreco_driver.h.  Host-only C++17; calls the C ABI of libpixreco.so only.
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <thread>
+#include <vector>
+
+#include "../../include/pixreco_driver.h"
+
+namespace {
+using clk = std::chrono::steady_clock;
+inline double us_since(clk::time_point t0) { return std::chrono::duration<double, std::micro>(clk::now() - t0).count(); }
+}  // namespace
+
+extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slots,
+                               const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
+                               uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res) {
+  if (!slots || !streams || !pool || !res || !n_slots || !n_pool || !n_threads) return PR_ERR_INVALID_ARG;
+  if (n_threads > n_slots) n_threads = n_slots;
+  std::atomic<int> status{PR_OK};
+  std::atomic<uint32_t> ready{0};
+  std::atomic<bool> go{false};
+  std::vector<std::vector<float>> acqUs(n_threads);
+  std::vector<uint64_t> digis(n_threads, 0), clusters(n_threads, 0), polls(n_threads, 0), done(n_threads, 0);
+  std::vector<clk::time_point> tBegin(n_threads), tEnd(n_threads);
+
+  auto worker = [&](uint32_t t) {
+    std::vector<int64_t> inFlight(n_slots, -1);               // event in flight on the slots this thread drives
+    acqUs[t].reserve(n_events / n_threads + 8);
+    pr_output out;
+    auto finish = [&](uint32_t s) -> bool {
+      int r;
+      while ((r = pr_produce(slots[s], &out)) == PR_NOT_READY) ++polls[t];
+      if (r != PR_OK) { int ok = PR_OK; status.compare_exchange_strong(ok, r); return false; }
+      const int64_t e = inFlight[s];
+      digis[t] += out.n_digis; clusters[t] += out.n_clusters; ++done[t];
+      if (t_start_ns) t_start_ns[e] = out.t_start_ns;
+      if (t_end_ns) t_end_ns[e] = out.t_end_ns;
+      while ((r = pr_release(slots[s])) == PR_NOT_READY) {}
+      inFlight[s] = -1;
+      return r == PR_OK;
+    };
+    ready.fetch_add(1);
+    while (!go.load(std::memory_order_acquire)) {}
+    tBegin[t] = clk::now();
+    for (uint32_t e = 0; e < n_events && status.load(std::memory_order_relaxed) == PR_OK; ++e) {
+      const uint32_t s = e % n_slots;
+      if (s % n_threads != t) continue;
+      if (inFlight[s] >= 0 && !finish(s)) break;
+      const auto a0 = clk::now();
+      const int r = pr_acquire(slots[s], pool + (first + e) % n_pool, streams[s]);
+      acqUs[t].push_back((float)us_since(a0));
+      if (r != PR_OK) { int ok = PR_OK; status.compare_exchange_strong(ok, r); break; }
+      inFlight[s] = e;
+    }
+    for (uint32_t s = t; s < n_slots; s += n_threads)
+      if (inFlight[s] >= 0) finish(s);
+    tEnd[t] = clk::now();
+  };
+
+  std::vector<std::thread> th;
+  for (uint32_t t = 0; t < n_threads; ++t) th.emplace_back(worker, t);
+  while (ready.load() < n_threads) {}
+  go.store(true, std::memory_order_release);
+  for (auto& x : th) x.join();
+
+  clk::time_point b = tBegin[0], e = tEnd[0];
+  std::vector<float> all;
+  *res = prd_result{};
+  for (uint32_t t = 0; t < n_threads; ++t) {
+    b = std::min(b, tBegin[t]); e = std::max(e, tEnd[t]);
+    all.insert(all.end(), acqUs[t].begin(), acqUs[t].end());
+    res->digis += digis[t]; res->clusters += clusters[t]; res->produce_polls += polls[t]; res->events += done[t];
+  }
+  res->wall_s = std::chrono::duration<double>(e - b).count();
+  if (!all.empty()) {
+    std::sort(all.begin(), all.end());
+    double sum = 0;
+    for (float v : all) sum += v;
+    res->acquire_us_median = all[all.size() / 2];
+    res->acquire_us_mean = sum / all.size();
+    res->acquire_us_p99 = all[std::min(all.size() - 1, (size_t)(all.size() * 0.99))];
+  }
+  res->status = status.load();
+  res->threads = n_threads;
+  return res->status;
+}

@@ -24,8 +24,9 @@ PR_OK, PR_NOT_READY = 0, 1
 PR_ERR_INVALID_ARG, PR_ERR_BAD_STATE, PR_ERR_CAPACITY, PR_ERR_INPUT_ORDER = -1, -2, -3, -4
 PR_ERR_BAD_CALIB, PR_ERR_OOM, PR_ERR_CUDA = -5, -6, -7
 PR_MEM_HOST_PINNED, PR_MEM_DEVICE = 1, 2
-PR_WANT_DIGIS, PR_WANT_CHARGE, PR_WANT_LABELS, PR_WANT_CLUSTERS, PR_WANT_ERRORS = 1, 2, 4, 8, 16
-PR_WANT_ALL = 31
+PR_WANT_DIGIS, PR_WANT_CHARGE, PR_WANT_LABELS, PR_WANT_CLUSTERS, PR_WANT_ERRORS, PR_WANT_HITS = 1, 2, 4, 8, 16, 32
+PR_WANT_ALL = 63
+PR_STATUS_INPUT_ORDER, PR_STATUS_CAPACITY = 1, 2
 PR_POOL_DEVICE, PR_POOL_PINNED, PR_POOL_FAKE = 0, 1, 2
 PR_INVALID_LABEL = 0xFFFFFFFF
 PR_FLAG_KERNEL_TIMING = 1
@@ -38,7 +39,8 @@ class pr_config(ctypes.Structure):
                 ("n_rows", c_uint16), ("n_cols", c_uint16), ("gain", c_void_p), ("pedestal", c_void_p),
                 ("pixel_threshold_e", c_float), ("cluster_threshold_e", c_float),
                 ("max_words_hint", c_uint32), ("max_events_in_flight", c_uint32),
-                ("max_cached_bytes_device", c_uint64), ("max_cached_bytes_host", c_uint64), ("flags", c_uint32)]
+                ("max_cached_bytes_device", c_uint64), ("max_cached_bytes_host", c_uint64), ("flags", c_uint32),
+                ("pitch_row_um", c_float), ("pitch_col_um", c_float)]
 
 
 class pr_input(ctypes.Structure):
@@ -48,7 +50,7 @@ class pr_input(ctypes.Structure):
 
 _VIEWS = ["module", "row", "col", "adc", "word_idx", "charge", "label", "clus", "mod_digi_start",
           "mod_clus_start", "cl_label", "cl_size", "cl_module", "cl_charge", "cl_row", "cl_col",
-          "err_word", "err_idx"]
+          "err_word", "err_idx", "ht_x", "ht_y", "ht_xerr", "ht_yerr", "ht_rows", "ht_cols", "ht_flags"]
 # name -> (numpy dtype, which counter gives the length)
 VIEW_SPEC = {
     "module": (np.uint16, "n_digis"), "row": (np.uint16, "n_digis"), "col": (np.uint16, "n_digis"),
@@ -59,6 +61,9 @@ VIEW_SPEC = {
     "cl_module": (np.uint16, "n_clusters"), "cl_charge": (np.float32, "n_clusters"),
     "cl_row": (np.float32, "n_clusters"), "cl_col": (np.float32, "n_clusters"),
     "err_word": (np.uint32, "n_errors"), "err_idx": (np.uint32, "n_errors"),
+    "ht_x": (np.float32, "n_clusters"), "ht_y": (np.float32, "n_clusters"), "ht_xerr": (np.float32, "n_clusters"),
+    "ht_yerr": (np.float32, "n_clusters"), "ht_rows": (np.uint32, "n_clusters"), "ht_cols": (np.uint32, "n_clusters"),
+    "ht_flags": (np.uint16, "n_clusters"),
 }
 
 
@@ -80,8 +85,7 @@ class pr_stats(ctypes.Structure):
                                          "kernel_launches", "memcpy_calls", "callbacks_fired")] +
                 [("events_in_flight", c_uint32), ("max_events_in_flight", c_uint32),
                  ("device_pool", pr_pool_stats), ("host_pool", pr_pool_stats), ("timed_acquires", c_uint64),
-                 ("unpack_ms", ctypes.c_double), ("cluster_ms", ctypes.c_double), ("finalize_ms", ctypes.c_double),
-                 ("export_ms", ctypes.c_double)])
+                 ("unpack_ms", ctypes.c_double), ("cluster_ms", ctypes.c_double), ("export_ms", ctypes.c_double)])
 
 
 # every symbol include/pixreco.h declares: name -> (restype, argtypes)
@@ -96,6 +100,7 @@ SIGNATURES = {
     "pr_produce": (c_int, [c_void_p, POINTER(pr_output)]),
     "pr_produce_batch": (c_int, [c_void_p, POINTER(pr_output), c_uint32]),
     "pr_release": (c_int, [c_void_p]),
+    "pr_release_on": (c_int, [c_void_p, c_void_p]),
     "pr_event_cuda_event": (c_void_p, [c_void_p]),
     "pr_stream_wait_event": (c_int, [c_void_p, c_void_p]),
     "pr_host_alloc": (c_void_p, [c_void_p, c_size_t]),
@@ -134,6 +139,51 @@ def __getattr__(name):          # pr_* functions as module attributes, same name
     if name in SIGNATURES:
         return getattr(lib(), name)
     raise AttributeError(name)
+
+
+class prd_result(ctypes.Structure):
+    _fields_ = [("wall_s", ctypes.c_double), ("acquire_us_median", ctypes.c_double), ("acquire_us_mean", ctypes.c_double),
+                ("acquire_us_p99", ctypes.c_double), ("events", c_uint64), ("digis", c_uint64), ("clusters", c_uint64),
+                ("produce_polls", c_uint64), ("status", c_int32), ("threads", c_uint32)]
+
+
+DRIVER_SIGNATURES = {
+    "prd_run_streams": (c_int, [POINTER(c_void_p), POINTER(c_void_p), c_uint32, POINTER(pr_input), c_uint32, c_uint32, c_uint32,
+                                c_uint32, c_void_p, c_void_p, POINTER(prd_result)]),
+}
+_driver = None
+
+
+def driver() -> ctypes.CDLL:
+    """libpixreco_driver.so: the multi-threaded C++ client of the C ABI (include/pixreco_driver.h)."""
+    global _driver
+    if _driver is None:
+        lib()                                   # libpixreco.so first (the driver links against it)
+        cdll = ctypes.CDLL(_build.build_driver())
+        for name, (res, args) in DRIVER_SIGNATURES.items():
+            fn = getattr(cdll, name)
+            fn.restype, fn.argtypes = res, args
+        _driver = cdll
+    return _driver
+
+
+def run_streams(slots, streams, inputs, n_events, n_threads=1, first=0, spans=False):
+    """One pr_acquire per event on its own stream (slot = stream = e mod len(slots)), issued from ``n_threads`` C++
+    host threads.  ``inputs``: a ctypes array of pr_input.  Returns a dict of the prd_result fields (+ spans)."""
+    n = len(slots)
+    sl = (c_void_p * n)(*[s.ptr for s in slots])
+    st = (c_void_p * n)(*[getattr(s, "cuda_stream", s) for s in streams])
+    t0 = np.zeros(n_events, np.uint64) if spans else None
+    t1 = np.zeros(n_events, np.uint64) if spans else None
+    res = prd_result()
+    rc = driver().prd_run_streams(sl, st, n, inputs, len(inputs), first, n_events, n_threads,
+                                  t0.ctypes.data if spans else None, t1.ctypes.data if spans else None, ctypes.byref(res))
+    if rc != 0:
+        raise PixRecoError(rc, "prd_run_streams")
+    out = {k: getattr(res, k) for k, _ in prd_result._fields_}
+    if spans:
+        out["t_start_ns"], out["t_end_ns"] = t0, t1
+    return out
 
 
 class PixRecoError(RuntimeError):
@@ -277,6 +327,14 @@ class EventSlot:
             self._keep = None
         return code
 
+    def release_on(self, consumer_stream) -> int:
+        """Release while work queued on ``consumer_stream`` may still read the device views."""
+        s = getattr(consumer_stream, "cuda_stream", consumer_stream)
+        code = _check(lib().pr_release_on(self.ptr, c_void_p(s)), "pr_release_on", self.owner.handle)
+        if code == PR_OK:
+            self._keep = None
+        return code
+
     @property
     def cuda_event(self) -> int:
         return lib().pr_event_cuda_event(self.ptr)
@@ -297,14 +355,14 @@ class PixReco:
 
     def __init__(self, gain, pedestal, n_rows=160, n_cols=416, pixel_threshold_e=1000.0, cluster_threshold_e=4000.0,
                  device=0, max_words_hint=0, max_events_in_flight=0, max_cached_bytes_device=0, max_cached_bytes_host=0,
-                 flags=0):
+                 flags=0, pitch_row_um=0.0, pitch_col_um=0.0):
         gain = np.ascontiguousarray(gain, np.float32)
         pedestal = np.ascontiguousarray(pedestal, np.float32)
         if gain.shape != pedestal.shape or gain.ndim != 1:
             raise ValueError("gain/pedestal must be 1-D arrays of equal length")
         cfg = pr_config(ctypes.sizeof(pr_config), device, gain.shape[0], n_rows, n_cols, gain.ctypes.data,
                         pedestal.ctypes.data, pixel_threshold_e, cluster_threshold_e, max_words_hint,
-                        max_events_in_flight, max_cached_bytes_device, max_cached_bytes_host, flags)
+                        max_events_in_flight, max_cached_bytes_device, max_cached_bytes_host, flags, pitch_row_um, pitch_col_um)
         h = c_void_p()
         _check(lib().pr_create(ctypes.byref(cfg), ctypes.byref(h)), "pr_create")
         self.handle, self.device, self.n_modules = h, device, int(gain.shape[0])

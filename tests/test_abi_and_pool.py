@@ -20,15 +20,15 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pr.lib()
     for name in declared:
         assert getattr(lib, name) is not None
-    assert lib.pr_abi_version() == 2
+    assert lib.pr_abi_version() == 3
     assert lib.pr_strerror(pr.PR_ERR_INPUT_ORDER).decode().startswith("input words")
 
 
 def test_struct_layouts_match_the_header():
     # sizes the C side checks (struct_size) or relies on
-    assert ctypes.sizeof(pr.pr_config) == 72
+    assert ctypes.sizeof(pr.pr_config) == 80
     assert ctypes.sizeof(pr.pr_input) == 56
-    assert ctypes.sizeof(pr.pr_output) == 8 + 8 * 4 + 2 * 8 + 36 * 8       # event_id, counters, two device time stamps, 36 views
+    assert ctypes.sizeof(pr.pr_output) == 8 + 8 * 4 + 2 * 8 + 50 * 8       # event_id, counters, two device time stamps, 2 x 25 views
     assert ctypes.sizeof(pr.pr_pool_stats) == 64
 
 
@@ -50,6 +50,7 @@ def test_create_rejects_bad_arguments_without_a_device():
     assert lib.pr_create(ctypes.byref(cfg(n_rows=257)), ctypes.byref(h)) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_create(ctypes.byref(cfg(n_cols=513)), ctypes.byref(h)) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_create(ctypes.byref(cfg(pixel_threshold_e=100.0)), ctypes.byref(h)) == pr.PR_ERR_BAD_CALIB   # A9: >= 512
+    assert lib.pr_create(ctypes.byref(cfg(pitch_row_um=-1.0)), ctypes.byref(h)) == pr.PR_ERR_INVALID_ARG      # A26
     g[2] = 0.0
     assert lib.pr_create(ctypes.byref(cfg()), ctypes.byref(h)) == pr.PR_ERR_BAD_CALIB
     g[2] = float("nan")
@@ -93,6 +94,7 @@ def test_null_slots_are_rejected_without_a_device():
     assert lib.pr_query(None) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_produce(None, ctypes.byref(out)) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_release(None) == pr.PR_ERR_INVALID_ARG
+    assert lib.pr_release_on(None, None) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_transfer(None, pr.PR_WANT_CLUSTERS, None, pr.pr_done_fn(), None) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_stream_wait_event(None, None) == pr.PR_ERR_INVALID_ARG
     assert lib.pr_event_destroy(None) == pr.PR_ERR_INVALID_ARG

@@ -41,7 +41,8 @@ def wait(slot, timeout=60.0):
 
 
 INT_FIELDS = ["module", "row", "col", "adc", "word_idx", "err_word", "err_idx", "mod_digi_start", "label", "clus",
-              "cl_label", "cl_module", "cl_size", "mod_clus_start"]
+              "cl_label", "cl_module", "cl_size", "mod_clus_start", "ht_rows", "ht_cols", "ht_flags"]
+HIT_FLOATS = ["ht_x", "ht_y", "ht_xerr", "ht_yerr"]
 
 
 def compare(out, ref, getter, strict_float=True):
@@ -62,6 +63,15 @@ def compare(out, ref, getter, strict_float=True):
         assert np.all(np.abs(getter("cl_row") - ref.cl_row) <= 1e-4) and np.all(np.abs(getter("cl_col") - ref.cl_col) <= 1e-4)
         if strict_float:
             for f in ("cl_charge", "cl_row", "cl_col"):
+                assert np.array_equal(getter(f).view(np.uint32), getattr(ref, f).view(np.uint32)), f
+    if getter("ht_x") is not None:
+        # hits (A26-A30): positions within 1e-4 pixel = 0.01 / 0.015 um (BASELINE.json's centroid tolerance times the
+        # pitch), errors within 1e-5 relative — and bit-equal, because both sides do the same binary64 operations
+        assert np.all(np.abs(getter("ht_x") - ref.ht_x) <= 1e-2) and np.all(np.abs(getter("ht_y") - ref.ht_y) <= 1.5e-2)
+        for f in ("ht_xerr", "ht_yerr"):
+            assert np.all(np.abs(getter(f) - getattr(ref, f)) <= 1e-5 * getattr(ref, f)), f
+        if strict_float:
+            for f in HIT_FLOATS:
                 assert np.array_equal(getter(f).view(np.uint32), getattr(ref, f).view(np.uint32)), f
 
 
