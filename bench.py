@@ -1,26 +1,31 @@
 #!/usr/bin/env python
-"""bench.py — pixel local reconstruction throughput on B200 (BASELINE.json `metric`).
+"""bench.py — pixel local reconstruction throughput on B200 (BASELINE.json `metric`: events/s & Mdigis/s; achieved
+HBM GB/s vs ~8 TB/s).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extra]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--slots S] [--no-extra]
 
-Metric: events/s (plus Mdigis/s) on seeded synthetic events of the configs[1] shape (Run-3
-HLT-like, ~50k digis in 1856 modules).  One *step* = one pass of the whole hot path (unpack +
-calibrate + compact, cluster + reduce + numbering, counters to the host) over 64 such events.
+Headline workload (`config.workload`): BASELINE.json configs[3], the largest batch workload that fits one GPU —
+256-event high-pile-up batches (1856 modules, ~200k digis and ~30k clusters per event), each batch ONE
+pr_acquire_batch / pr_produce_batch through the C ABI, `--slots` batches in flight on their own streams, timed
+wall-clock on the device (CUDA events around a gate/join of all streams) from the first acquire to the last produce.
+One *step* = `batches_per_step` such batches back to back (chosen from the warm-up so that K steps last >= 0.6 s
+even at K = 20); every step is one pass of the whole hot path (unpack + calibrate + compact, cluster + reduce +
+numbering + hits, counters to the host) over its events.
 
-  value     device-resident inputs (R1): 64-event batches through pr_acquire_batch/pr_produce_batch,
-            `--slots` batches in flight on their own streams.
-  e2e       the same through the same public API with pinned HOST inputs and the cluster table
-            copied back (want = CLUSTERS): H2D and D2H inside the timed region (R2).
-  extra     configs[2] exactly as BASELINE.json words it (one pr_acquire per event, 8 streams in
-            flight), and HBM-sized launches for the unpack kernel roofline (configs[3] batch of
-            256 events, configs[4] single event).
-  roofline  dominant kernel of the step: algorithmic bytes per launch / CUDA-event duration of
-            that kernel on its own stream (PR_FLAG_KERNEL_TIMING pass over the same steps).
-  cpu_baseline  the oracle (oracle/, single thread, as it stands) on a bounded sample.
+  value     device-resident inputs (R1).
+  e2e       the same API with pinned HOST inputs and the cluster + hit tables copied back (R2): H2D and D2H inside the
+            timed region.
+  roofline  dominant kernel of the step from a PR_FLAG_KERNEL_TIMING pass (CUDA events on the launching stream, one
+            batch in flight), every kernel with its own bound; chain fractions of the bytes-moved roofline; and
+            `by_config`: all five BASELINE.json configs wall-clock through pr_acquire*/pr_produce* (configs[2] as worded:
+            one pr_acquire per event on its own stream, 8 in flight, issued by 1, 2 and 4 C++ host threads).
+  cpu_baseline  the oracle (oracle/, as it stands) on one host core AND on all host cores (one process per core), on a
+            bounded sample of every config.
 
-Inputs rotate through a pool larger than the 126 MB L2.  N>1 (torchrun): each rank runs the same
-per-GPU workload on its own device (events are independent: no collective on the data path),
-time = max over ranks, value = all ranks' events / that time ("scaling": "weak").
+After every timed loop the last step's outputs are compared with the oracle (untimed).  Inputs are larger than the
+126 MB L2 (a 256-event batch is 309 MB of input and ~10 GB of slab).  N>1 (torchrun): every rank runs the same
+per-GPU workload on its own device (events are independent: no collective on the data path), time = max over ranks,
+value = all ranks' events / that time ("scaling": "weak").
 """
 from __future__ import annotations
 
@@ -39,45 +44,39 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-EVENTS_PER_STEP = 64
-POOL_EVENTS = 512            # 512 x ~0.30 MB = ~154 MB of distinct input > 126 MB L2
+HEAD_CONFIG = 3
+HEAD_BATCH = 256             # events per pr_acquire_batch (BASELINE.json configs[3]: 256 events)
+HEAD_POOL_BATCHES = 2        # distinct batches the steps rotate through (2 x 309 MB of input)
+CFG1_BATCH = 64
 STREAMS_IN_FLIGHT = 8        # configs[2]
+NOMINAL_GBS = 8000.0         # BASELINE.json: "~8 TB/s"
+# Thread-level operations the method needs per digi for a3 + a4 + hits (DESIGN.md section 6 derives it): the
+# numerator of the ALU roofline of k_cluster; the denominator is 148 SMs x 128 lane-operations per cycle x the clock.
+CLUSTER_OPS_PER_DIGI = 96.0
+UNPACK_OPS_PER_WORD = 40.0
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--slots", type=int, default=4, help="batches in flight (batch mode)")
-    ap.add_argument("--no-extra", action="store_true")
-    ap.add_argument("--pool-events", type=int, default=POOL_EVENTS)
-    ap.add_argument("--only", default=None, choices=["configs2", "configs3", "configs4"],
-                    help="run just this extra case and print its JSON (for ncu captures of HBM-sized launches)")
-    ap.add_argument("--reps", type=int, default=6, help="timed launches per extra case")
+    ap.add_argument("--slots", type=int, default=3, help="batches in flight")
+    ap.add_argument("--no-extra", action="store_true", help="skip roofline.by_config and the all-config CPU baseline")
+    ap.add_argument("--only", default=None, choices=["configs1", "configs3", "configs4"],
+                    help="run a few lone launches of this config's shape and exit (for ncu captures)")
+    ap.add_argument("--reps", type=int, default=3, help="launches with --only")
+    ap.add_argument("--min-seconds", type=float, default=0.6, help="length of the timed region the step size is chosen for")
     return ap.parse_args()
 
 
-def load_traffic(kernel):
-    """DRAM bytes per launch of `kernel` (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
-    ncu --set full capture of this bench's step (profiles/traffic.json), or None."""
+def load_profile(kernel):
+    """Per-launch DRAM bytes / warp instructions of `kernel` on the headline launch, from profiles/traffic.json
+    (written by `python -m paper_2004_04334_b200.ncu_summary` from an ncu --set full capture), or None."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f)["kernels"][kernel]["dram_bytes_per_launch"]
-    except Exception:
-        return None
-
-
-def load_issue(kernel, ms, sm_mhz, n_sm=148):
-    """Context for a kernel that is not HBM-bound: warp-instructions per launch (same ncu capture as `traffic`)
-    over the measured duration, against 4 schedulers x 1 warp-instruction per cycle per SM at the sampled clock."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            wi = json.load(f)["kernels"][kernel]["warp_inst_per_launch"]
-        peak = n_sm * 4 * (sm_mhz or 1965.0) * 1e6
-        return {"warp_inst_per_launch": wi, "achieved_per_s": wi / (ms * 1e-3), "peak_per_s": peak,
-                "frac": wi / (ms * 1e-3) / peak, "note": "instruction issue, not an algorithmic roofline"}
+            return json.load(f)["kernels"][kernel]
     except Exception:
         return None
 
@@ -143,47 +142,94 @@ def make_pool(wl, config, n_events, first_event=0):
 
 
 def algorithmic_bytes(W, D, E, N, M):
-    """per event."""
+    """DESIGN.md 'algorithmic bytes per unit', per event: k_unpack, k_cluster, chain minimum."""
     unpack = 6 * W + 16 * D + 8 * E + 4 * (M + 1)            # a1+a2 fused: read words+adc, write digi SoA+charge+errors
     cluster = 16 * D + 24 * N + 8 * (M + 1)                  # a3+a4 fused: read row,col,charge; write label,clus; cluster SoA
     chain = 6 * W + 24 * D + 24 * N + 8 * E + 8 * (M + 1) + 32
     return unpack, cluster, chain
 
 
-# ------------------------------------------------------------------ reference arm (the oracle)
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+# ------------------------------------------------------------------ the oracle, timed (reference arm and cpu_baseline)
+def _oracle_worker(args):
+    """One process = one oracle instance over its own events for about `budget` seconds.  Returns (events, digis, seconds)."""
+    import oracle
+    events, cal, budget, min_events = args
+    ws = oracle.Workspace(max(e.n_words for e in events), cal.n_modules)
+    n = d = 0
+    t0 = time.perf_counter()
+    while True:
+        e = events[n % len(events)]
+        oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
+                       cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
+        n += 1
+        d += int(ws.counters[0])
+        dt = time.perf_counter() - t0
+        if (dt >= budget and n >= min_events) or n >= 1 << 20:
+            return n, d, dt
+
+
+def oracle_rates(pool, cal, budget_s, cores):
+    """The oracle as it stands on 1 core and on `cores` cores (one independent process per core, each over its own
+    slice of `pool`; if the pool has fewer events than cores the slices repeat, said in `sample`)."""
+    import multiprocessing as mp
+    n1, d1, t1 = _oracle_worker((pool, cal, budget_s, 1))
+    res = {"cores_1": {"events_per_s": n1 / t1, "mdigis_per_s": d1 / t1 / 1e6, "sample": f"{n1} events in {t1:.2f} s"}}
+    if cores > 1:
+        slices = [pool[i::cores] if len(pool) >= cores else [pool[i % len(pool)]] for i in range(cores)]
+        ctx = mp.get_context("fork")
+        t0 = time.perf_counter()
+        with ctx.Pool(cores) as p:
+            out = p.map(_oracle_worker, [(s, cal, budget_s, 1) for s in slices])
+        wall = time.perf_counter() - t0
+        ev, dg, tmax = sum(o[0] for o in out), sum(o[1] for o in out), max(o[2] for o in out)
+        res[f"cores_{cores}"] = {"events_per_s": ev / tmax, "mdigis_per_s": dg / tmax / 1e6,
+                                 "sample": f"{ev} events, slowest process {tmax:.2f} s (wall incl. fork {wall:.2f} s)"
+                                           + ("" if len(pool) >= cores else f"; {len(pool)} distinct events shared by the processes")}
+    return res
+
+
 def run_reference(args, rank):
+    """The reference arm of the contract for this tier: the oracle on the box's host cores, same metric and workload."""
     if rank != 0:
         return
-    import oracle
     from paper_2004_04334_b200 import workloads as wl
-    cal = wl.make_calib(1)
-    sample = 16                                              # events per step (bounded sample of the 64-event step)
-    pool = make_pool(wl, 1, sample * 4)
-    ws = oracle.Workspace(max(e.n_words for e in pool), cal.n_modules)
-
-    def step(s):
-        d = 0
-        for k in range(sample):
-            e = pool[(s * sample + k) % len(pool)]
-            oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
-                           cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
-            d += int(ws.counters[0])
-        return d
-    steps = min(args.steps, 400)
-    for s in range(min(args.warmup, 10)):
-        step(s)
-    t0 = time.perf_counter()
-    digis = sum(step(s) for s in range(steps))
-    dt = time.perf_counter() - t0
+    import multiprocessing as mp
+    cores = os.cpu_count() or 1
+    cal = wl.make_calib(HEAD_CONFIG)
+    per_proc = 2
+    pool = make_pool(wl, HEAD_CONFIG, cores * per_proc)
+    sample = len(pool)                                      # events per step: every process does `per_proc` events
+    steps, warm = min(args.steps, 40), min(max(args.warmup, 1), 3)
+    ctx = mp.get_context("fork")
+    with ctx.Pool(cores) as p:
+        jobs = [(pool[i * per_proc:(i + 1) * per_proc], cal, 0.0, per_proc) for i in range(cores)]
+        for _ in range(warm):
+            p.map(_oracle_worker, jobs)
+        t0 = time.perf_counter()
+        digis = 0
+        for _ in range(steps):
+            digis += sum(o[1] for o in p.map(_oracle_worker, jobs))
+        dt = time.perf_counter() - t0
     v = sample * steps / dt
     line = {"impl": "reference", "metric": "pixel-reco events/s", "value": v, "unit": "events/s", "n_gpus": args.gpus,
-            "steps": steps, "warmup": min(args.warmup, 10), "ms_per_step": dt / steps * 1e3 * (EVENTS_PER_STEP / sample),
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32 (exact int64 sums)",
-            "data": "synthetic", "mdigis_per_s": digis / dt / 1e6,
-            "config": {"workload": "configs[1] Run-3 HLT-like events, oracle on host cores", "events_per_step": EVENTS_PER_STEP,
-                       "sample": f"{sample} of the step's {EVENTS_PER_STEP} events per step"},
-            "cpu_baseline": {"value": v, "unit": "events/s", "cores": 1, "kind": "oracle",
-                             "sample": f"{sample * steps} events of the configs[1] shape, single thread"},
+            "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u32+f32 (exact int64 sums)", "data": "synthetic", "mdigis_per_s": digis / dt / 1e6,
+            "config": {"workload": "configs[3] high-pile-up events (1856 modules, ~200k digis, ~30k clusters per event); the oracle on the host cores",
+                       "sample": f"a step = {sample} events = {per_proc} per process on {cores} processes (a bounded sample of our arm's step)",
+                       "cpu_model": cpu_model()},
+            "cpu_baseline": {"value": v, "unit": "events/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{sample * steps} events of the configs[3] shape, one process per core"},
             "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -191,14 +237,15 @@ def run_reference(args, rank):
 
 # ------------------------------------------------------------------ our arm
 class Bench:
-    def __init__(self, torch, pr, wl, device, flags=0, M=None, cal=None):
-        self.torch, self.pr, self.wl, self.device = torch, pr, wl, device
-        self.cal = cal
+    def __init__(self, torch, pr, device, cal, flags=0):
+        self.torch, self.pr, self.device, self.cal = torch, pr, device, cal
         self.p = pr.PixReco(cal.gain, cal.pedestal, device=device, flags=flags)
         self.lib = pr.lib()
+        self._keep = []
 
     def close(self):
         self.p.close()
+        self._keep = []
 
     # -- inputs
     def upload(self, pool):
@@ -213,20 +260,25 @@ class Bench:
             W[o:o + e.n_words] = e.words; A[o:o + e.n_words] = e.adc
         dW = torch.from_numpy(W.view(np.int32)).to(f"cuda:{self.device}")
         dA = torch.from_numpy(A.view(np.int16)).to(f"cuda:{self.device}")
-        self._keep_dev = (dW, dA)
+        self._keep.append((dW, dA))
         return [(dW.data_ptr() + 4 * o, dA.data_ptr() + 2 * o, e.n_words) for e, o in zip(pool, offs)]
 
-    def pin(self, pool):
-        """Pinned host copies from the library's host pool."""
-        offs, tot = [], 0
-        for e in pool:
-            offs.append(tot)
-            tot += (e.n_words + 63) // 64 * 64
-        W = self.p.host_array(max(tot, 64), np.uint32); A = self.p.host_array(max(tot, 64), np.uint16)
-        for e, o in zip(pool, offs):
-            W[o:o + e.n_words] = e.words; A[o:o + e.n_words] = e.adc
-        self._keep_pin = (W, A)
-        return [(W.ctypes.data + 4 * o, A.ctypes.data + 2 * o, e.n_words) for e, o in zip(pool, offs)]
+    def pin(self, pool, per_batch=None):
+        """Pinned host copies from the library's host pool; one block per `per_batch` events (a DAQ buffer)."""
+        per_batch = per_batch or len(pool)
+        ptrs = []
+        for b0 in range(0, len(pool), per_batch):
+            chunk = pool[b0:b0 + per_batch]
+            offs, tot = [], 0
+            for e in chunk:
+                offs.append(tot)
+                tot += (e.n_words + 63) // 64 * 64
+            W = self.p.host_array(max(tot, 64), np.uint32); A = self.p.host_array(max(tot, 64), np.uint16)
+            for e, o in zip(chunk, offs):
+                W[o:o + e.n_words] = e.words; A[o:o + e.n_words] = e.adc
+            self._keep.append((W, A))
+            ptrs += [(W.ctypes.data + 4 * o, A.ctypes.data + 2 * o, e.n_words) for e, o in zip(chunk, offs)]
+        return ptrs
 
     def inputs(self, ptrs, kind, want):
         pr = self.pr
@@ -258,96 +310,52 @@ class Bench:
         wall = time.perf_counter() - t0
         return start.elapsed_time(end) * 1e-3, wall
 
-    # -- batch mode: `slots` batches of 64 events in flight
-    def run_batches(self, inp, n_events_pool, steps, slots, streams, first_step=0):
+    # -- batches of `nb` events, len(slots) batches in flight; returns (digis, clusters, outputs of the last batch, its index)
+    def run_batches(self, inp, n_pool, nb, n_batches, slots, streams, first=0):
         lib, pr = self.lib, self.pr
-        outs = (pr.pr_output * EVENTS_PER_STEP)()
-        nb = n_events_pool // EVENTS_PER_STEP
-        busy = [False] * len(slots)
-        digis = clusters = 0
+        outs = [(pr.pr_output * nb)() for _ in slots]
+        pool_batches = n_pool // nb
+        busy = [None] * len(slots)
+        tot = [0, 0]
+        last = [None, None]
 
         def finish(i):
-            nonlocal digis, clusters
             while True:
-                r = lib.pr_produce_batch(slots[i].ptr, outs, EVENTS_PER_STEP)
+                r = lib.pr_produce_batch(slots[i].ptr, outs[i], nb)
                 if r != pr.PR_NOT_READY:
                     break
             if r != 0:
                 raise RuntimeError(f"pr_produce_batch -> {r}")
-            for k in range(EVENTS_PER_STEP):
-                digis += outs[k].n_digis; clusters += outs[k].n_clusters
-            lib.pr_release(slots[i].ptr)
-            busy[i] = False
-        for s in range(steps):
+            for k in range(nb):
+                tot[0] += outs[i][k].n_digis; tot[1] += outs[i][k].n_clusters
+            last[0], last[1] = i, busy[i]
+        for s in range(n_batches):
             i = s % len(slots)
-            if busy[i]:
+            if busy[i] is not None:
                 finish(i)
-            b = (first_step + s) % nb
-            r = lib.pr_acquire_batch(slots[i].ptr, self.at(pr, inp, b * EVENTS_PER_STEP), EVENTS_PER_STEP,
-                                     ctypes.c_void_p(streams[i].cuda_stream))
+                lib.pr_release(slots[i].ptr)
+            b = (first + s) % pool_batches
+            r = lib.pr_acquire_batch(slots[i].ptr, self.at(pr, inp, b * nb), nb, ctypes.c_void_p(streams[i].cuda_stream))
             if r != 0:
                 raise RuntimeError(f"pr_acquire_batch -> {r}: {lib.pr_last_cuda_error(self.p.handle).decode()}")
-            busy[i] = True
-        for i in range(len(slots)):
-            if busy[i]:
-                finish(i)
-        return digis, clusters
+            busy[i] = b
+        order = sorted((i for i in range(len(slots)) if busy[i] is not None), key=lambda i: (i - (n_batches % len(slots))) % len(slots))
+        for i in order:
+            finish(i)
+        self.last = (outs[last[0]], last[1] * nb, slots[last[0]]) if last[0] is not None else None
+        return tot[0], tot[1]
 
-    # -- the same with the host copy as a stage of its own (pr_transfer): acquire with want = 0, produce,
-    #    then transfer the cluster table (device gather + one exact-size DMA copy), produce again
-    def run_batches_transfer(self, inp, n_events_pool, steps, slots, streams, want, first_step=0):
-        lib, pr = self.lib, self.pr
-        outs = (pr.pr_output * EVENTS_PER_STEP)()
-        nb = n_events_pool // EVENTS_PER_STEP
-        stage = [0] * len(slots)                      # 0 idle, 1 acquire in flight, 2 transfer in flight
-        clusters = 0
+    def release_all(self, slots):
+        for s in slots:
+            self.lib.pr_release(s.ptr)
 
-        def advance(i, block):
-            """Moves slot i forward; returns True when it is idle again."""
-            nonlocal clusters
-            while stage[i]:
-                r = lib.pr_produce_batch(slots[i].ptr, outs, EVENTS_PER_STEP)
-                if r == pr.PR_NOT_READY:
-                    if not block:
-                        return False
-                    continue
-                if r != 0:
-                    raise RuntimeError(f"pr_produce_batch -> {r}")
-                if stage[i] == 1:
-                    r = lib.pr_transfer(slots[i].ptr, want, ctypes.c_void_p(streams[i].cuda_stream), pr.pr_done_fn(), None)
-                    if r != 0:
-                        raise RuntimeError(f"pr_transfer -> {r}")
-                    stage[i] = 2
-                else:
-                    for k in range(EVENTS_PER_STEP):
-                        clusters += outs[k].n_clusters
-                    lib.pr_release(slots[i].ptr)
-                    stage[i] = 0
-            return True
-        for s in range(steps):
-            i = s % len(slots)
-            for j in range(len(slots)):               # keep the other slots' stages moving
-                if j != i:
-                    advance(j, False)
-            advance(i, True)
-            b = (first_step + s) % nb
-            r = lib.pr_acquire_batch(slots[i].ptr, self.at(pr, inp, b * EVENTS_PER_STEP), EVENTS_PER_STEP,
-                                     ctypes.c_void_p(streams[i].cuda_stream))
-            if r != 0:
-                raise RuntimeError(f"pr_acquire_batch -> {r}")
-            stage[i] = 1
-        for i in range(len(slots)):
-            advance(i, True)
-        return clusters
-
-    # -- configs[2]: one pr_acquire per event, 8 slots/streams in flight (A25: slot = stream = e mod 8)
-    def run_streams(self, inp, n_events_pool, n_events, slots, streams, first=0):
+    # -- one pr_acquire per event, Python loop (latency probes and the Python-driven configs[2])
+    def run_single(self, inp, n_pool, n_events, slots, streams, first=0):
         lib, pr = self.lib, self.pr
         out = pr.pr_output()
         busy = [False] * len(slots)
         digis = clusters = 0
-        self.spans = []
-        ptrs = [self.at(pr, inp, k) for k in range(n_events_pool)]
+        ptrs = [self.at(pr, inp, k) for k in range(n_pool)]
 
         def finish(i):
             nonlocal digis, clusters
@@ -358,15 +366,13 @@ class Bench:
             if r != 0:
                 raise RuntimeError(f"pr_produce -> {r}")
             digis += out.n_digis; clusters += out.n_clusters
-            self.spans.append((out.t_start_ns, out.t_end_ns))
             lib.pr_release(slots[i].ptr)
             busy[i] = False
         for e in range(n_events):
             i = e % len(slots)
             if busy[i]:
                 finish(i)
-            k = (first + e) % n_events_pool
-            r = lib.pr_acquire(slots[i].ptr, ptrs[k], ctypes.c_void_p(streams[i].cuda_stream))
+            r = lib.pr_acquire(slots[i].ptr, ptrs[(first + e) % n_pool], ctypes.c_void_p(streams[i].cuda_stream))
             if r != 0:
                 raise RuntimeError(f"pr_acquire -> {r}: {lib.pr_last_cuda_error(self.p.handle).decode()}")
             busy[i] = True
@@ -376,9 +382,69 @@ class Bench:
         return digis, clusters
 
 
+def verify_against_oracle(pr, device, outs, events, cal, sample):
+    """Untimed: events `sample` (indices into outs/events) of a finished step against the oracle — every counter, the
+    cluster table and the hit table (device views copied back).  Raises on any difference."""
+    import oracle
+    for k in sample:
+        ev = events[k]
+        ref = oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal, cal.pixel_threshold_e, cal.cluster_threshold_e,
+                         ev.n_rows, ev.n_cols)
+        o = pr.Output(outs[k], device)
+        got = (o.n_words, o.n_digis, o.n_errors, o.n_kept_digis, o.n_clusters_all, o.n_clusters, o.status_bits)
+        want = (ref.n_words, ref.n_digis, ref.n_errors, ref.n_kept_digis, ref.n_clusters_all, ref.n_clusters, 0)
+        if got != want:
+            raise RuntimeError(f"bench verification: counters {got} != oracle {want} (event {k})")
+        for f in ("label", "clus", "cl_label", "cl_size", "cl_module", "mod_clus_start", "ht_rows", "ht_cols", "ht_flags"):
+            if not np.array_equal(o.to_numpy(f), getattr(ref, f)):
+                raise RuntimeError(f"bench verification: {f} differs from the oracle (event {k})")
+        for f in ("charge", "cl_charge", "cl_row", "cl_col", "ht_x", "ht_y", "ht_xerr", "ht_yerr"):
+            if not np.array_equal(o.to_numpy(f).view(np.uint32), getattr(ref, f).view(np.uint32)):
+                raise RuntimeError(f"bench verification: {f} differs from the oracle (event {k})")
+    return len(sample)
+
+
+def chain_entry(events, digis, seconds, W, D, N, M, peak, E=None):
+    E = W - D if E is None else E
+    _, _, bchain = algorithmic_bytes(W, D, E, N, M)
+    eps = events / seconds
+    return {"events_per_s": eps, "mdigis_per_s": digis / seconds / 1e6, "chain_bytes_per_event": bchain,
+            "chain_gbs": bchain * eps / 1e9, "chain_frac_of_measured_peak": bchain * eps / 1e9 / peak,
+            "chain_frac_of_8TBs": bchain * eps / 1e9 / NOMINAL_GBS}
+
+
 def run_ours(args, rank, world):
+    from paper_2004_04334_b200 import workloads as wl
+    peak, peak_src = load_peaks()
+    K, Wm = args.steps, max(args.warmup, 3)
+    cores = os.cpu_count() or 1
+    extra = not args.no_extra
+
+    # ---------------- inputs (seeded, synthetic; every rank its own events: weak scaling)
+    cal3 = wl.make_calib(HEAD_CONFIG)
+    M = cal3.n_modules
+    n_pool = HEAD_BATCH * HEAD_POOL_BATCHES
+    pool3 = make_pool(wl, HEAD_CONFIG, n_pool, first_event=rank * n_pool)
+    meanW = float(np.mean([e.n_words for e in pool3]))
+
+    # ---------------- the oracle on the host cores, before this process touches CUDA (fork-safe); rank 0 at N = 1 only
+    cpu = None
+    if rank == 0 and world == 1:
+        budget = 1.5
+        by = {"configs[3]": oracle_rates(pool3[:max(cores, 8)], cal3, budget, cores)}
+        if extra:
+            for cfg, n_ev in ((0, max(cores, 8)), (1, max(cores, 8)), (4, 2)):
+                by[f"configs[{cfg}]"] = oracle_rates(make_pool(wl, cfg, n_ev), wl.make_calib(cfg), budget if cfg != 4 else 0.5, cores)
+            by["configs[2]"] = {"note": "the events of configs[2] are 64 events of the configs[1] shape: same per-event oracle rate as configs[1]",
+                                **by["configs[1]"]}
+        head = by["configs[3]"]
+        best = head.get(f"cores_{cores}", head["cores_1"])
+        cpu = {"value": best["events_per_s"], "unit": "events/s", "cores": cores if f"cores_{cores}" in head else 1, "kind": "oracle",
+               "sample": "configs[3] events: " + best["sample"] + "; one process per core over disjoint events",
+               "value_1_core": head["cores_1"]["events_per_s"], "cpu_model": cpu_model(), "host_cores": cores, "by_config": by}
+
     import torch
-    from paper_2004_04334_b200 import pixreco as pr, workloads as wl
+    from paper_2004_04334_b200 import pixreco as pr
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
     local = int(os.environ.get("LOCAL_RANK", 0))
@@ -387,22 +453,6 @@ def run_ours(args, rank, world):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
-    peak, peak_src = load_peaks()
-    K, Wm = args.steps, max(args.warmup, 3)
-    cal = wl.make_calib(1)
-    M = cal.n_modules
-    n_pool = max(args.pool_events // EVENTS_PER_STEP, 1) * EVENTS_PER_STEP
-    pool = make_pool(wl, 1, n_pool, first_event=rank * n_pool)       # every rank its own events (weak scaling)
-    meanW = float(np.mean([e.n_words for e in pool]))
-
-    b = Bench(torch, pr, wl, local, cal=cal)
-    dev_ptrs = b.upload(pool)
-    pin_ptrs = b.pin(pool)
-    inp_dev = b.inputs(dev_ptrs, pr.PR_MEM_DEVICE, 0)
-    inp_host = b.inputs(pin_ptrs, pr.PR_MEM_HOST_PINNED, pr.PR_WANT_CLUSTERS)
-    nslots = max(1, args.slots)
-    slots = [b.p.slot() for _ in range(nslots)]
-    streams = [torch.cuda.Stream(device=local) for _ in range(nslots)]
 
     def barrier():
         if dist is not None:
@@ -416,216 +466,253 @@ def run_ours(args, rank, world):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    # ---------------- R1: device-resident, batch mode (the headline `value`)
-    b.run_batches(inp_dev, n_pool, Wm, slots, streams)                 # warm-up (fills the pools)
+    b = Bench(torch, pr, local, cal3)
+    inp_dev = b.inputs(b.upload(pool3), pr.PR_MEM_DEVICE, 0)
+    nslots = max(1, args.slots)
+    slots = [b.p.slot() for _ in range(nslots)]
+    streams = [torch.cuda.Stream(device=local) for _ in range(nslots)]
+
+    # ---------------- R1: device-resident (the headline `value`)
+    b.run_batches(inp_dev, n_pool, HEAD_BATCH, Wm * 2, slots, streams); b.release_all(slots)      # warm-up (fills the pools)
+    t_probe, _ = b.timed(streams, lambda: b.run_batches(inp_dev, n_pool, HEAD_BATCH, 2 * nslots, slots, streams)); b.release_all(slots)
+    t_batch = max_over_ranks(t_probe) / (2 * nslots)
+    bps = int(min(64, max(1, np.ceil(args.min_seconds / (K * t_batch)))))              # batches per step
     st0 = b.p.stats()
     barrier()
     clk = ClockSampler(local)
     res = {}
-
-    def r1():
-        res["dc"] = b.run_batches(inp_dev, n_pool, K, slots, streams, first_step=Wm)
-    t_dev, t_wall = b.timed(streams, r1)
+    t_dev, t_wall = b.timed(streams, lambda: res.update(dc=b.run_batches(inp_dev, n_pool, HEAD_BATCH, K * bps, slots, streams, first=1)))
     barrier()
     clocks = clk.stop()
     st1 = b.p.stats()
     t_dev = max_over_ranks(t_dev)
     digis, clusters = res["dc"]
-    n_events = K * EVENTS_PER_STEP
+    n_events = K * bps * HEAD_BATCH
     value = world * n_events / t_dev
     launches = st1["kernel_launches"] - st0["kernel_launches"]
     new_mallocs = st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"]
+    outs_last, first_ev, _ = b.last
+    verified = verify_against_oracle(pr, local, outs_last, pool3[first_ev:first_ev + HEAD_BATCH], cal3, (0, 97, HEAD_BATCH - 1))
+    b.release_all(slots)
+    Dm, Nm = digis / n_events, clusters / n_events
+    head_chain = chain_entry(world * n_events, world * digis, t_dev, meanW, Dm, Nm, M, peak)
 
-    # ---------------- R2: end to end, pinned host inputs + cluster table back (same API)
-    b.run_batches(inp_host, n_pool, Wm, slots, streams)
+    # ---------------- R2: end to end — pinned host inputs, cluster + hit tables back, same API
+    want_e2e = pr.PR_WANT_CLUSTERS | pr.PR_WANT_HITS
+    inp_host = b.inputs(b.pin(pool3, per_batch=HEAD_BATCH), pr.PR_MEM_HOST_PINNED, want_e2e)
+    b.run_batches(inp_host, n_pool, HEAD_BATCH, 2 * nslots, slots, streams); b.release_all(slots)
+    n_e2e = max(2 * nslots, min(K * bps, 24))
     barrier()
-    t_e2e, _ = b.timed(streams, lambda: b.run_batches(inp_host, n_pool, K, slots, streams, first_step=Wm))
+    t_e2e, _ = b.timed(streams, lambda: b.run_batches(inp_host, n_pool, HEAD_BATCH, n_e2e, slots, streams, first=1))
     barrier()
     t_e2e = max_over_ranks(t_e2e)
-    e2e_value = world * n_events / t_e2e
-    # ---------------- R2': the same with the host copy as a stage of its own (pr_transfer)
-    inp_host0 = b.inputs(pin_ptrs, pr.PR_MEM_HOST_PINNED, 0)
-    b.run_batches_transfer(inp_host0, n_pool, Wm, slots, streams, pr.PR_WANT_CLUSTERS)
-    barrier()
-    t_tr, _ = b.timed(streams, lambda: b.run_batches_transfer(inp_host0, n_pool, min(K, 400), slots, streams, pr.PR_WANT_CLUSTERS, first_step=Wm))
-    barrier()
-    t_tr = max_over_ranks(t_tr)
-    e2e_transfer = world * min(K, 400) * EVENTS_PER_STEP / t_tr
-    h2d = int(6 * meanW * EVENTS_PER_STEP)
-    meanN = clusters / n_events
-    d2h = int((22 * meanN + 4 * (M + 1) + 32) * EVENTS_PER_STEP)
+    outs_last, first_ev, _ = b.last
+    o = pr.Output(outs_last[5], local)
+    import oracle
+    ev5 = pool3[first_ev + 5]
+    ref5 = oracle.run(ev5.words, ev5.adc, ev5.n_modules, cal3.gain, cal3.pedestal)
+    if not (np.array_equal(o.host("cl_label"), ref5.cl_label) and np.array_equal(o.host("ht_x").view(np.uint32), ref5.ht_x.view(np.uint32))):
+        raise RuntimeError("bench verification: end-to-end host mirrors differ from the oracle")
+    b.release_all(slots)
+    e2e_value = world * n_e2e * HEAD_BATCH / t_e2e
+    h2d = int(6 * meanW * HEAD_BATCH * bps)
+    d2h = int((48 * Nm + 4 * (M + 1) + 40) * HEAD_BATCH * bps)
     b.close()
 
     line = {"metric": "pixel-reco events/s", "value": value, "unit": "events/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_dev / K * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u32+f32 (exact int64 sums)", "data": "synthetic",
             "mdigis_per_s": world * digis / t_dev / 1e6,
-            "config": {"workload": "configs[1] Run-3 HLT-like events (1856 modules, ~50k digis, ~8k clusters/event); "
-                                   "step = 64 events = one pr_acquire_batch/pr_produce_batch",
-                       "events_per_step": EVENTS_PER_STEP, "batches_in_flight": nslots, "mean_words_per_event": meanW,
-                       "l2_policy": f"inputs rotate through {n_pool} distinct events ({n_pool * meanW * 6 / 1e6:.0f} MB) > 126 MB L2",
-                       "residency": "R1 device-resident inputs, counters to mapped pinned host"},
+            "config": {"workload": "configs[3] high-pile-up: batches of 256 events (1856 modules, ~200k digis, ~30k clusters per event), "
+                                   "one pr_acquire_batch/pr_produce_batch per batch",
+                       "events_per_batch": HEAD_BATCH, "batches_per_step": bps, "events_per_step": HEAD_BATCH * bps,
+                       "batches_in_flight": nslots, "mean_words_per_event": meanW, "mean_digis_per_event": Dm, "mean_clusters_per_event": Nm,
+                       "timed_region_s": t_dev,
+                       "l2_policy": f"inputs larger than L2: a batch reads {meanW * 6 * HEAD_BATCH / 1e6:.0f} MB and writes ~{(24 * Dm + 48 * Nm) * HEAD_BATCH / 1e6:.0f} MB; "
+                                    f"steps rotate through {HEAD_POOL_BATCHES} distinct batches",
+                       "residency": "R1 device-resident inputs, counters to mapped pinned host",
+                       "verified_vs_oracle": f"{verified} events of the last timed batch: counters, labels, cluster and hit tables bit-equal (untimed)"},
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": t_e2e / K * 1e3, "what": "pinned host inputs, want=CLUSTERS, same batch API",
-                    "with_transfer_stage": {"value": e2e_transfer, "unit": "events/s",
-                                            "what": "want=0, then pr_transfer(CLUSTERS) after produce: device gather + one exact-size DMA copy per batch (P:L112)"}},
+                    "ms_per_step": t_e2e / n_e2e * bps * 1e3, "batches_timed": n_e2e,
+                    "what": "pinned host inputs (one block per batch from pr_host_alloc), want = CLUSTERS | HITS, same batch API; PCIe-bound"},
             "steady_state_cudaMalloc": int(new_mallocs), "wall_s": t_wall}
 
     if rank == 0:
-        # ---------------- kernel timing pass for the roofline (same steps, PR_FLAG_KERNEL_TIMING)
-        bt = Bench(torch, pr, wl, local, flags=pr.PR_FLAG_KERNEL_TIMING, cal=cal)
-        dp = bt.upload(pool)
-        it = bt.inputs(dp, pr.PR_MEM_DEVICE, 0)
-        sl = [bt.p.slot()]                      # ONE batch in flight: event deltas are kernel durations
-        bt.run_batches(it, n_pool, Wm, sl, streams[:1])
+        # ---------------- kernel timing pass for the roofline (same batches, PR_FLAG_KERNEL_TIMING, ONE batch in flight)
+        bt = Bench(torch, pr, local, cal3, flags=pr.PR_FLAG_KERNEL_TIMING)
+        it = bt.inputs(bt.upload(pool3), pr.PR_MEM_DEVICE, 0)
+        sl = [bt.p.slot()]
+        bt.run_batches(it, n_pool, HEAD_BATCH, 3, sl, streams[:1]); bt.release_all(sl)
         s0 = bt.p.stats()
-        dg, cl = bt.run_batches(it, n_pool, K, sl, streams[:1], first_step=Wm)
+        nrep = max(6, min(K * bps, 20))
+        dg, cl = bt.run_batches(it, n_pool, HEAD_BATCH, nrep, sl, streams[:1], first=1); bt.release_all(sl)
         torch.cuda.synchronize(local)
         s1 = bt.p.stats()
         nt = s1["timed_acquires"] - s0["timed_acquires"]
         t_un = (s1["unpack_ms"] - s0["unpack_ms"]) / nt * 1e-3
         t_cl = (s1["cluster_ms"] - s0["cluster_ms"]) / nt * 1e-3
-        t_fi = (s1["finalize_ms"] - s0["finalize_ms"]) / nt * 1e-3
-        Dm, Nm = dg / (K * EVENTS_PER_STEP), cl / (K * EVENTS_PER_STEP)
-        Em = meanW - Dm
-        bu, bc, bchain = algorithmic_bytes(meanW, Dm, Em, Nm, M)
-        # a3+a4 = k_cluster + k_finalize: the algorithmic bytes of the fused step are charged to k_cluster
-        kern = {"k_unpack": {"ms": t_un * 1e3, "bytes": bu * EVENTS_PER_STEP, "gbs": bu * EVENTS_PER_STEP / t_un / 1e9},
-                "k_cluster": {"ms": t_cl * 1e3, "bytes": bc * EVENTS_PER_STEP, "gbs": bc * EVENTS_PER_STEP / t_cl / 1e9},
-                "k_finalize": {"ms": t_fi * 1e3, "bytes": (8 * Dm + 56 * Nm + 4 * (M + 1)) * EVENTS_PER_STEP,
-                               "gbs": (8 * Dm + 56 * Nm + 4 * (M + 1)) * EVENTS_PER_STEP / t_fi / 1e9}}
-        dom = max(kern, key=lambda k: kern[k]["ms"])
-        line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                            "frac": kern[dom]["gbs"] / peak, "traffic": load_traffic(dom), "peak_source": peak_src,
-                            "frac_of_8TBs_nominal": kern[dom]["gbs"] / 8000.0,
-                            "algorithmic_bytes_per_launch": kern[dom]["bytes"], "ms_per_launch": kern[dom]["ms"],
-                            "units_per_launch": f"{EVENTS_PER_STEP} events", "kernels": kern,
-                            "issue_slots": load_issue(dom, kern[dom]["ms"], clocks.get("sm_mhz")),
-                            "chain": {"bytes_per_event": bchain, "gbs": bchain * value / world / 1e9,
-                                      "frac": bchain * value / world / 1e9 / peak}}
         bt.close()
-        extra = {}
-        if not args.no_extra:
-            extra = run_extra(torch, pr, wl, local, peak)
-        line["extra"] = extra
-        line["cpu_baseline"] = cpu_baseline(wl, pool, cal)
+        Dk, Nk = dg / (nrep * HEAD_BATCH), cl / (nrep * HEAD_BATCH)
+        bu, bc, bchain = algorithmic_bytes(meanW, Dk, meanW - Dk, Nk, M)
+        sm_mhz = clocks.get("sm_mhz") or 1965.0
+        alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9                                    # G thread-operations per second
+        kern = {
+            "k_unpack": {"bound": "hbm", "ms": t_un * 1e3, "algorithmic_bytes": bu * HEAD_BATCH, "gbs": bu * HEAD_BATCH / t_un / 1e9,
+                         "frac_of_measured_peak": bu * HEAD_BATCH / t_un / 1e9 / peak, "frac_of_8TBs": bu * HEAD_BATCH / t_un / 1e9 / NOMINAL_GBS,
+                         "profile": load_profile("k_unpack")},
+            "k_cluster": {"bound": "alu", "ms": t_cl * 1e3, "algorithmic_bytes": bc * HEAD_BATCH, "gbs": bc * HEAD_BATCH / t_cl / 1e9,
+                          "frac_of_measured_peak": bc * HEAD_BATCH / t_cl / 1e9 / peak, "frac_of_8TBs": bc * HEAD_BATCH / t_cl / 1e9 / NOMINAL_GBS,
+                          "algorithmic_gops": CLUSTER_OPS_PER_DIGI * Dk * HEAD_BATCH / t_cl / 1e9, "alu_peak_gops": alu_peak,
+                          "alu_frac": CLUSTER_OPS_PER_DIGI * Dk * HEAD_BATCH / t_cl / 1e9 / alu_peak, "profile": load_profile("k_cluster")}}
+        dom = max(kern, key=lambda k: kern[k]["ms"])
+        prof = kern[dom]["profile"] or {}
+        if dom == "k_cluster":
+            roof = {"bound": "alu", "kernel": dom, "achieved": kern[dom]["algorithmic_gops"], "peak": alu_peak, "unit": "Gop/s",
+                    "frac": kern[dom]["alu_frac"],
+                    "peak_source": f"148 SMs x 128 lane-operations per cycle x {sm_mhz:.0f} MHz (sampled clock); {CLUSTER_OPS_PER_DIGI:.0f} thread-operations per digi (DESIGN.md 6)",
+                    "hbm": {"achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s", "frac": kern[dom]["frac_of_measured_peak"],
+                            "frac_of_8TBs_nominal": kern[dom]["frac_of_8TBs"], "peak_source": peak_src}}
+        else:
+            roof = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": kern[dom]["frac_of_measured_peak"], "frac_of_8TBs_nominal": kern[dom]["frac_of_8TBs"], "peak_source": peak_src}
+        roof.update({"traffic": prof.get("dram_bytes_per_launch"), "algorithmic_bytes_per_launch": kern[dom]["algorithmic_bytes"],
+                     "ms_per_launch": kern[dom]["ms"], "units_per_launch": f"{HEAD_BATCH} events", "kernels": kern,
+                     "chain": {"bytes_per_event": bchain, "gbs": head_chain["chain_gbs"], "frac": head_chain["chain_frac_of_measured_peak"],
+                               "frac_of_8TBs_nominal": head_chain["chain_frac_of_8TBs"],
+                               "lone_launch_ms": (t_un + t_cl) * 1e3, "lone_launch_frac": bchain * HEAD_BATCH / (t_un + t_cl) / 1e9 / peak}})
+        if extra:
+            roof["by_config"] = run_by_config(torch, pr, wl, local, peak, head_chain)
+        line["roofline"] = roof
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
 
 
-def cpu_baseline(wl, pool, cal, budget_s=12.0):
-    import oracle
-    ws = oracle.Workspace(max(e.n_words for e in pool), cal.n_modules)
-    n, t0 = 0, time.perf_counter()
-    while True:
-        e = pool[n % len(pool)]
-        oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
-                       cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
-        n += 1
-        dt = time.perf_counter() - t0
-        if dt > budget_s or n >= 4096:
-            break
-    return {"value": n / dt, "unit": "events/s", "cores": 1, "kind": "oracle",
-            "sample": f"{n} events of the configs[1] shape, {dt:.1f} s, single thread (host has {os.cpu_count()} cores)"}
-
-
-def run_extra(torch, pr, wl, local, peak, only=None, reps_hbm=6):
-    """configs[2] as worded (per-event streams), and HBM-sized launches for the unpack roofline."""
-    extra = {}
-    if only in (None, "configs2"):
-        extra.update(run_configs2(torch, pr, wl, local))
-    # ---- HBM-sized launches, kernel timing on
-    for name, config, n_ev, batch in (("configs[3] 256-event batch", 3, 256, True), ("configs[4] single event", 4, 2, False)):
-        if only is not None and only != f"configs{config}":
-            continue
-        extra[name] = run_hbm_case(torch, pr, wl, local, peak, config, n_ev, batch, reps_hbm)
-    return extra
-
-
-def run_configs2(torch, pr, wl, local):
-    extra = {}
-    # ---- configs[2]: 64 events, one pr_acquire each, 8 streams in flight
+# ------------------------------------------------------------------ all five configs, wall-clock through the C ABI
+def run_by_config(torch, pr, wl, local, peak, head_chain):
+    out = {"configs[3]": {"what": "the headline: 256-event batches, device-resident", **head_chain}}
+    # ---- configs[1]: 64-event batches of Run-3-like events, 4 batches in flight (round 1's headline)
     cal = wl.make_calib(1)
-    pool = make_pool(wl, 1, 256)
-    b = Bench(torch, pr, wl, local, cal=cal)
+    pool = make_pool(wl, 1, 512)
+    meanW = float(np.mean([e.n_words for e in pool]))
+    b = Bench(torch, pr, local, cal)
     inp = b.inputs(b.upload(pool), pr.PR_MEM_DEVICE, 0)
     slots = [b.p.slot() for _ in range(STREAMS_IN_FLIGHT)]
     streams = [torch.cuda.Stream(device=local) for _ in range(STREAMS_IN_FLIGHT)]
-    b.run_streams(inp, len(pool), 256, slots, streams)
+    b.run_batches(inp, 512, CFG1_BATCH, 16, slots[:4], streams[:4]); b.release_all(slots[:4])
+    nb = 1500
+    r = {}
+    t, _ = b.timed(streams[:4], lambda: r.update(dc=b.run_batches(inp, 512, CFG1_BATCH, nb, slots[:4], streams[:4], first=3)))
+    outs_last, first_ev, _ = b.last
+    verify_against_oracle(pr, local, outs_last, pool[first_ev:first_ev + CFG1_BATCH], cal, (0, 31, 63))
+    b.release_all(slots[:4])
+    D1, N1 = r["dc"][0] / (nb * CFG1_BATCH), r["dc"][1] / (nb * CFG1_BATCH)
+    out["configs[1]"] = {"what": f"{CFG1_BATCH}-event batches through pr_acquire_batch, 4 in flight, device-resident, {nb} batches",
+                         **chain_entry(nb * CFG1_BATCH, r["dc"][0], t, meanW, D1, N1, cal.n_modules, peak)}
+    # one event at a time, one stream: the latency of a single pr_acquire -> pr_produce
+    b.run_single(inp, 512, 64, slots[:1], streams[:1])
+    t, _ = b.timed(streams[:1], lambda: b.run_single(inp, 512, 400, slots[:1], streams[:1], first=64))
+    out["configs[1]"]["single_event_latency_us"] = t / 400 * 1e6
+    # ---- configs[2] exactly as worded: 64 events, one pr_acquire each on its own stream, 8 in flight (A25), C++ host threads
+    c2 = {}
+    pr.run_streams(slots, streams, inp, 256, n_threads=1)                     # warm-up of the 8 slots
     st0 = b.p.stats()
-    reps = 40
-    t, wall = b.timed(streams, lambda: [b.run_streams(inp, len(pool), 64, slots, streams, first=64 * r) for r in range(reps)])
+    for nthr in (1, 2, 4):
+        reps, best = 5, None
+        for rep in range(reps):
+            d = pr.run_streams(slots, streams, inp, 64 * 40, n_threads=nthr, first=64 * rep, spans=(rep == reps - 1))
+            if best is None or d["wall_s"] < best["wall_s"]:
+                best = {k: v for k, v in d.items() if not k.startswith("t_")}
+            last = d
+        sp = sorted(zip(last["t_start_ns"].tolist(), last["t_end_ns"].tolist()))
+        busy_ns = sum(t1 - t0 for t0, t1 in sp)
+        wall_ns = max(t1 for _, t1 in sp) - min(t0 for t0, _ in sp)
+        ent = chain_entry(best["events"], best["digis"], best["wall_s"], meanW, D1, N1, cal.n_modules, peak)
+        ent.update({"host_threads": nthr, "events": best["events"], "us_per_event": best["wall_s"] / best["events"] * 1e6,
+                    "acquire_host_us_median": best["acquire_us_median"], "acquire_host_us_p99": best["acquire_us_p99"],
+                    "mean_events_in_flight_on_device": busy_ns / max(wall_ns, 1),
+                    "consecutive_events_overlapping": sum(1 for a, c in zip(sp, sp[1:]) if c[0] < a[1]) / max(len(sp) - 1, 1)})
+        c2[f"threads_{nthr}"] = ent
     st1 = b.p.stats()
-    sp = sorted(b.spans)                             # device %globaltimer intervals of the last pass's events
-    busy_ns = sum(t1 - t0 for t0, t1 in sp)
-    wall_ns = max(t1 for _, t1 in sp) - min(t0 for t0, _ in sp)
-    extra["configs[2] per-event streams"] = {
-        "mean_events_in_flight_on_device": busy_ns / max(wall_ns, 1),
-        "consecutive_events_overlapping": sum(1 for a, c in zip(sp, sp[1:]) if c[0] < a[1]) / max(len(sp) - 1, 1),
-        "events_per_s": 64 * reps / t, "events": 64 * reps, "streams_in_flight": STREAMS_IN_FLIGHT,
-        "us_per_event": t / (64 * reps) * 1e6, "max_events_in_flight": st1["max_events_in_flight"],
-        "new_cudaMalloc_in_timed_region": st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"],
-        "note": "one pr_acquire/pr_produce/pr_release per event from one host thread (Python driver); launch-latency bound"}
+    t, _ = b.timed(streams, lambda: b.run_single(inp, 512, 64 * 20, slots, streams))
+    c2["python_loop_events_per_s"] = 64 * 20 / t
+    c2["new_cudaMalloc_in_timed_region"] = st1["device_pool"]["backend_allocs"] - st0["device_pool"]["backend_allocs"]
+    c2["what"] = ("one pr_acquire / pr_produce / pr_release per event, slot = stream = event mod 8 (A25), device-resident inputs, "
+                  "issued by C++ host threads (libpixreco_driver.so); wall clock from the first acquire to the last produce")
+    best_thr = max((k for k in c2 if k.startswith("threads_")), key=lambda k: c2[k]["events_per_s"])
+    out["configs[2]"] = {**{k: v for k, v in c2[best_thr].items()}, "best": best_thr, **c2}
     b.close()
-    return extra
+    # ---- configs[0]: the tiny event, one at a time and 8 streams
+    cal = wl.make_calib(0)
+    pool = make_pool(wl, 0, 64)
+    meanW0 = float(np.mean([e.n_words for e in pool]))
+    b = Bench(torch, pr, local, cal)
+    inp = b.inputs(b.upload(pool), pr.PR_MEM_DEVICE, 0)
+    slots = [b.p.slot() for _ in range(STREAMS_IN_FLIGHT)]
+    streams = [torch.cuda.Stream(device=local) for _ in range(STREAMS_IN_FLIGHT)]
+    b.run_single(inp, 64, 64, slots[:1], streams[:1])
+    r = {}
+    t, _ = b.timed(streams[:1], lambda: r.update(dc=b.run_single(inp, 64, 400, slots[:1], streams[:1])))
+    pr.run_streams(slots, streams, inp, 256, n_threads=2)
+    d = pr.run_streams(slots, streams, inp, 64 * 40, n_threads=2)
+    D0, N0 = r["dc"][0] / 400, r["dc"][1] / 400
+    out["configs[0]"] = {"what": "1 tiny event per pr_acquire; `events_per_s` = 8 streams in flight from 2 C++ host threads; latency = one event at a time",
+                         **chain_entry(d["events"], d["digis"], d["wall_s"], meanW0, D0, N0, cal.n_modules, peak),
+                         "single_event_latency_us": t / 400 * 1e6}
+    b.close()
+    # ---- configs[4]: clustering stress, one event per pr_acquire, 2 in flight; 16 events (4 distinct ones, cycled)
+    cal = wl.make_calib(4)
+    pool = make_pool(wl, 4, 4)
+    meanW4 = float(np.mean([e.n_words for e in pool]))
+    b = Bench(torch, pr, local, cal)
+    inp = b.inputs(b.upload(pool), pr.PR_MEM_DEVICE, 0)
+    slots = [b.p.slot() for _ in range(2)]
+    streams = [torch.cuda.Stream(device=local) for _ in range(2)]
+    b.run_single(inp, 4, 4, slots, streams)
+    r = {}
+    t, _ = b.timed(streams, lambda: r.update(dc=b.run_single(inp, 4, 16, slots, streams)))
+    D4, N4 = r["dc"][0] / 16, r["dc"][1] / 16
+    out["configs[4]"] = {"what": "16 events (4 distinct, cycled), one pr_acquire per event, 2 in flight, device-resident",
+                         **chain_entry(16, r["dc"][0], t, meanW4, D4, N4, cal.n_modules, peak)}
+    # one of them against the oracle
+    s = slots[0]
+    s.acquire(b._keep[0][0][:pool[0].n_words], b._keep[0][1][:pool[0].n_words], stream=streams[0])
+    while s.query() == pr.PR_NOT_READY:
+        pass
+    outs = (pr.pr_output * 1)()
+    pr.lib().pr_produce_batch(s.ptr, outs, 1)
+    verify_against_oracle(pr, local, outs, pool[:1], cal, (0,))
+    s.release()
+    b.close()
+    return out
 
 
-def run_hbm_case(torch, pr, wl, local, peak, config, n_ev, batch, reps):
-    if True:
-        cal = wl.make_calib(config)
-        pool = make_pool(wl, config, n_ev)
-        bt = Bench(torch, pr, wl, local, flags=pr.PR_FLAG_KERNEL_TIMING, cal=cal)
-        ptrs = bt.upload(pool)
-        inp = bt.inputs(ptrs, pr.PR_MEM_DEVICE, 0)
-        slot = bt.p.slot()
-        s = torch.cuda.Stream(device=local)
-        lib = pr.lib()
-        tot = {"W": 0, "D": 0, "N": 0}
-        outs = (pr.pr_output * n_ev)()
-        flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}")
-        s0 = None
-        for r in range(reps + 2):
-            if r == 2:
-                torch.cuda.synchronize(local)
-                s0 = bt.p.stats()
-            flush.fill_(r)                                   # evict L2 between iterations
-            torch.cuda.synchronize(local)
-            if batch:
-                rc = lib.pr_acquire_batch(slot.ptr, inp, n_ev, ctypes.c_void_p(s.cuda_stream))
-                n_out = n_ev
-            else:
-                rc = lib.pr_acquire(slot.ptr, Bench.at(pr, inp, r % n_ev), ctypes.c_void_p(s.cuda_stream))
-                n_out = 1
-            assert rc == 0, rc
-            while lib.pr_produce_batch(slot.ptr, outs, n_out) == pr.PR_NOT_READY:
-                pass
-            if r >= 2:
-                for k in range(n_out):
-                    tot["W"] += outs[k].n_words; tot["D"] += outs[k].n_digis; tot["N"] += outs[k].n_clusters
-            lib.pr_release(slot.ptr)
-        s1 = bt.p.stats()
-        nt = s1["timed_acquires"] - s0["timed_acquires"]
-        t_un = (s1["unpack_ms"] - s0["unpack_ms"]) / nt * 1e-3
-        t_cl = (s1["cluster_ms"] - s0["cluster_ms"]) / nt * 1e-3
-        t_fi = (s1["finalize_ms"] - s0["finalize_ms"]) / nt * 1e-3
-        W, D, N = tot["W"] / nt, tot["D"] / nt, tot["N"] / nt
-        n_per = n_ev if batch else 1
-        bu, bc, bchain = algorithmic_bytes(W, D, W - D, N, cal.n_modules * n_per)
-        res = {"events_per_launch": n_per, "words_per_launch": W, "digis_per_launch": D, "clusters_per_launch": N,
-                       "k_unpack": {"ms": t_un * 1e3, "gbs": bu / t_un / 1e9, "frac_of_measured_peak": bu / t_un / 1e9 / peak,
-                                    "frac_of_8TBs": bu / t_un / 1e9 / 8000.0, "algorithmic_bytes": bu},
-                       "k_cluster": {"ms": t_cl * 1e3, "gbs": bc / t_cl / 1e9, "frac_of_measured_peak": bc / t_cl / 1e9 / peak,
-                                     "algorithmic_bytes": bc},
-                       "k_finalize": {"ms": t_fi * 1e3},
-                       "chain": {"events_per_s": n_per / (t_un + t_cl + t_fi), "mdigis_per_s": D / (t_un + t_cl + t_fi) / 1e6,
-                                 "gbs": bchain / (t_un + t_cl + t_fi) / 1e9, "frac_of_measured_peak": bchain / (t_un + t_cl + t_fi) / 1e9 / peak},
-                       "l2_policy": "256 MiB fill between iterations"}
-        bt.close()
-        del flush
-        return res
+def run_only(args):
+    """A few lone launches of one config's shape (for ncu captures of HBM-sized launches)."""
+    import torch
+    from paper_2004_04334_b200 import pixreco as pr, workloads as wl
+    config, n_ev, batch = {"configs1": (1, CFG1_BATCH, True), "configs3": (3, HEAD_BATCH, True), "configs4": (4, 1, False)}[args.only]
+    cal = wl.make_calib(config)
+    pool = make_pool(wl, config, n_ev)
+    b = Bench(torch, pr, 0, cal, flags=pr.PR_FLAG_KERNEL_TIMING)
+    inp = b.inputs(b.upload(pool), pr.PR_MEM_DEVICE, 0)
+    slots, streams = [b.p.slot()], [torch.cuda.Stream(device=0)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda:0")
+    for r in range(args.reps):
+        flush.fill_(r)
+        torch.cuda.synchronize(0)
+        if batch:
+            b.run_batches(inp, n_ev, n_ev, 1, slots, streams); b.release_all(slots)
+        else:
+            b.run_single(inp, n_ev, 1, slots, streams)
+    st = b.p.stats()
+    print(json.dumps({"config": args.only, "launches": args.reps, "unpack_ms": st["unpack_ms"] / st["timed_acquires"],
+                      "cluster_ms": st["cluster_ms"] / st["timed_acquires"]}), flush=True)
+    b.close()
 
 
 def main():
@@ -636,10 +723,7 @@ def main():
         run_reference(args, rank)
         return
     if args.only:
-        import torch
-        from paper_2004_04334_b200 import pixreco as pr, workloads as wl
-        peak, _ = load_peaks()
-        print(json.dumps(run_extra(torch, pr, wl, 0, peak, only=args.only, reps_hbm=args.reps)), flush=True)
+        run_only(args)
         return
     run_ours(args, rank, world)
 

@@ -108,7 +108,7 @@ typedef struct {
 /* pr_config.flags */
 #define PR_FLAG_KERNEL_TIMING 0x1u /* record CUDA events around each kernel on its stream and sum the
                                       per-kernel device times into pr_stats (measurement aid; adds
-                                      three cudaEventRecord per acquire)                           */
+                                      four cudaEventRecord per acquire)                            */
 
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
@@ -164,7 +164,7 @@ typedef struct {
   pr_pool_stats device_pool, host_pool;
   /* PR_FLAG_KERNEL_TIMING only: device time summed over `timed_acquires` completed acquires */
   uint64_t timed_acquires;
-  double   unpack_ms, cluster_ms, export_ms;
+  double   unpack_ms, cluster_ms, finalize_ms, export_ms;
 } pr_stats;
 
 /* ---- handle: job start / job end (may block and allocate) ---- */

@@ -21,24 +21,24 @@ constexpr int kLookBack = 8;                                         // predeces
 
 // ---- cluster kernel geometry ----
 constexpr int kClusterThreads = 256;
-constexpr u32 kUnitCap = 2047;        // digis of one unit (consecutive modules of one event) on the fast path: 11-bit local index
-constexpr u32 kMaxGroup = 16;         // modules per unit at most (4-bit module index inside the hash key)
-constexpr u32 kDenseDigis = 8192;     // shared-memory tiers of k_dense (one module per CTA); beyond: global workspace
-constexpr u32 kDenseClusters = 384;
-constexpr u32 kAccWords = 14;         // u32 accumulators / record words per cluster (see k_cluster.cuh)
+constexpr u32 kSmemDigis = 2048;      // modules with more digis use the global workspace tier
+constexpr u32 kSmemClusters = 384;    // likewise for per-cluster accumulators
+constexpr u32 kDenseDigis = 8192;     // the same tiers of k_dense (two CTAs per SM with their own, larger shared memory)
+constexpr u32 kDenseClusters = 512;
 constexpr u32 kMaxModuleDigis = (1u << 17) - 1u;   // A9: the exact sums are overflow-free up to 2^17 digis per module; more -> PR_STATUS_CAPACITY
 
-// Per-event device counters.  They live in the slot's control block, which is ALL ZERO between acquires: whoever
-// uses a word last puts the zero back (no per-acquire memset).
+// Per-event device counters (lives in the slot's control block, zeroed per acquire).
 struct DevCounters {
-  u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, unitsDone;
+  u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, pad;
 };
-// Per-launch control words (all zero between acquires).
+// Per-launch control words.  The first two are put back to zero by the last CTA of k_unpack (with the look-back
+// states); the rest is zeroed per acquire together with the counters.
 struct LaunchCtl {
   u32 tileTicket, unpackExited;     // k_unpack: next tile of the launch, CTAs that have left
-  u32 unitTicket, clusterExited;    // k_cluster / k_dense: next unit, CTAs that have left
+  u32 modTicket, modDone;           // k_cluster: next warp ticket
   u64 tStart;                       // %globaltimer at the start of the acquire's first kernel
-  u32 pad[10];
+  u32 nBig, bigTicket;              // modules handed from k_cluster to k_dense, next one to take
+  u32 pad[8];
 };
 // What the host reads after completion (mapped pinned memory, written by the CTA that finishes the event).
 struct HostCounters {
@@ -70,13 +70,15 @@ struct EvDesc {
   u32 *clLabel, *clSize; u16* clModule; float *clCharge, *clRow, *clCol;
   // hit SoA [cap], hit k belongs to cluster k (A26-A30)
   float *htX, *htY, *htXerr, *htYerr; u32 *htRows, *htCols; u16* htFlags;
-  // global workspace tier of the dense path [cap] each (modules beyond the shared-memory tiers)
-  u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum;
-  u32* wsAcc;                       // [kAccWords * cap] per-cluster accumulators
-  u32* stage;                       // [kAccWords * cap] finished cluster records of units that could not be written in place
+  // global workspace tier for large modules [cap] each (wsBox: 4 per digi slot)
+  u32 *wsPerm, *wsParent, *wsRoot; int32_t* wsKnum; u32* wsSize; u64 *wsS, *wsSx, *wsSy; u32* wsBox;
   HostCounters* hostCounters;
   DevCounters* result;              // device copy of the event's final counters (per acquire; k_export reads its sizes there)
-  u32* grpAgg;                      // [nGroups] kept clusters of each unit | ready bit (numbering look-back)
+  u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
+  u32* grpCount;                    // [ceil(M / 32)] the same summed over groups of kFinMods modules (zeroed per acquire)
+  // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
+  double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
+  u32 *stBoxR, *stBoxC;             // bounding box (A28): max(255 - row) << 16 | max(row), max(511 - col) << 16 | max(col)
 };
 static_assert(offsetof(EvDesc, label) == 128, "k_unpack's part of the descriptor is one 128-byte line");
 

@@ -1,0 +1,133 @@
+// k_finalize.cuh — numbering of a4, cluster table, hit table, counters to the host (k_finalize); exact-size gathers (k_export)
+// Part of kernels.cuh (include that, not this file).
+#pragma once
+#include "common.cuh"
+
+namespace pixreco {
+
+// ================================================================== k_finalize (numbering of a4)
+// One CTA per (event, group of kFinMods consecutive modules): the group's first dense cluster
+// number is the sum of the kept-cluster counts of all earlier modules (at most 2048 values), so
+// no CTA depends on another.  Turns clus[] ranks into event-wide cluster numbers, converts the
+// staged sums into the cluster SoA (A9: binary64 division, one rounding to binary32) and the hit SoA (the step after
+// clustering in the paper's Fig. 1; A26-A30: position from the same exact sums, bounding box, border flags, error
+// estimate), writes modClusStart[]; the CTA of an event's last module group publishes that event's counters to mapped
+// pinned host memory.
+constexpr u32 kFinMods = 32;
+static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
+template <bool kSingle>
+__global__ void __launch_bounds__(256)
+k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent, u32 splits,
+           LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+  __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8];
+  const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
+  // `splits` CTAs share one (event, group) when events are huge: slice sp of the group's digis and clusters
+  const u32 unit = blockIdx.x / splits, sp = blockIdx.x - unit * splits;
+  const u32 e = unit / unitsPerEvent, u = unit - e * unitsPerEvent;
+  const EvDesc& ev = kSingle ? single : batch[e];
+  const u32 m0 = u * kFinMods, m1 = min(m0 + kFinMods, M);
+  if (!(ev.counters->status & 1u)) {
+    u32 sum = 0, base;
+    for (u32 k = tid; k < u; k += 256) sum += ev.grpCount[k];      // groups of kFinMods modules before this one
+    block_excl_scan(sum, sScan, &base);
+    if (warp == 0) {
+      const u32 c = m0 + lane < m1 ? ev.modCount[m0 + lane] : 0u;
+      const u32 incl = warp_incl_scan(c, lane);
+      sStart[lane] = base + incl - c;
+      if (lane == 31) sStart[32] = base + incl;
+      sDigi[lane] = ev.modDigiStart[min(m0 + lane, M)];
+      if (lane == 31) sDigi[32] = ev.modDigiStart[min(m0 + 32u, M)];
+    }
+    __syncthreads();
+    if (sp == 0) {
+      for (u32 m = m0 + tid; m < m1; m += 256) ev.modClusStart[m] = sStart[m - m0];
+      if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
+    }
+    const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
+    if (d0 <= d1 && d1 <= ev.cap) {
+      for (u32 dd = d0 + sp * 1024u + tid; dd < d1; dd += splits * 1024u) {     // four independent digis per thread and trip
+        int32_t c[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const u32 d = dd + 256u * k;
+          c[k] = d < d1 ? ev.clus[d] : -1;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (c[k] < 0) continue;
+          // the digi's module within the group: the last one that starts at or before the digi (no read of module[])
+          const u32 d = dd + 256u * k;
+          u32 li = 0;
+#pragma unroll
+          for (u32 step = 16; step > 0; step >>= 1)
+            if (li + step < m1 - m0 && sDigi[li + step] <= d) li += step;
+          ev.clus[d] = (int32_t)(sStart[li] + (u32)c[k]);
+        }
+      }
+      for (u32 o = sStart[0] + sp * 256u + tid; o < sStart[32]; o += splits * 256u) {
+        u32 li = 0;
+#pragma unroll
+        for (u32 step = 16; step > 0; step >>= 1)
+          if (li + step < kFinMods + 1 && sStart[li + step] <= o) li += step;   // last module with start <= o and a cluster there
+        const u32 src = sDigi[li] + (o - sStart[li]);
+        if (o < ev.cap && src < ev.cap) {
+          const double S = ev.stS[src];
+          ev.clLabel[o] = ev.stLabel[src]; ev.clModule[o] = (u16)(m0 + li); ev.clSize[o] = ev.stSize[src];
+          ev.clCharge[o] = __double2float_rn(S * (1.0 / 16384.0));
+          const double rc = __ddiv_rn(ev.stSx[src], S), cc = __ddiv_rn(ev.stSy[src], S);                   // A9
+          ev.clRow[o] = __double2float_rn(rc);
+          ev.clCol[o] = __double2float_rn(cc);
+          // the hit of this cluster.  A27: divide, add 0.5, subtract half the module, multiply by the pitch — binary64, in
+          // this order, one cast; A28 box; A29 border flags; A30 error = pitch/sqrt(12) * {span at a border, 1 for span 1, else 0.5}
+          const u32 bR = ev.stBoxR[src], bC = ev.stBoxC[src];
+          const u32 rmin = 255u - (bR >> 16), rmax = bR & 0xFFFFu, cmin = 511u - (bC >> 16), cmax = bC & 0xFFFFu;
+          const bool er = rmin == 0u || rmax == g.R - 1u, ec = cmin == 0u || cmax == g.C - 1u;
+          const u32 sr = rmax - rmin + 1u, sc = cmax - cmin + 1u;
+          const double fr = er ? (double)sr : (sr == 1u ? 1.0 : 0.5), fc = ec ? (double)sc : (sc == 1u ? 1.0 : 0.5);
+          ev.htX[o] = __double2float_rn(__dmul_rn(__dsub_rn(__dadd_rn(rc, 0.5), 0.5 * (double)g.R), g.pitchRow));
+          ev.htY[o] = __double2float_rn(__dmul_rn(__dsub_rn(__dadd_rn(cc, 0.5), 0.5 * (double)g.C), g.pitchCol));
+          ev.htXerr[o] = __double2float_rn(__dmul_rn(__dmul_rn(g.pitchRow, 0.28867513459481287), fr));
+          ev.htYerr[o] = __double2float_rn(__dmul_rn(__dmul_rn(g.pitchCol, 0.28867513459481287), fc));
+          ev.htRows[o] = rmin | rmax << 16; ev.htCols[o] = cmin | cmax << 16;
+          ev.htFlags[o] = (u16)((er ? 1u : 0u) | (ec ? 2u : 0u));
+        }
+      }
+    }
+  }
+  // The CTA of the event's last module group publishes the event's counters to mapped pinned host memory: all
+  // the others were final when this kernel started, nClusters is this CTA's own result.
+  if (m1 == M && sp == 0 && tid == 0) {
+    const DevCounters* c = ev.counters;
+    const u32 status = c->status;
+    HostCounters h;
+    h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
+    h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[32]; h.status = status; h.seq = 1;
+    h.tStart = lc->tStart; h.tEnd = global_timer();
+    *ev.hostCounters = h;
+    DevCounters r;                                   // device copy of the final counters: k_export takes its sizes from it
+    r.nWords = h.nWords; r.nDigis = h.nDigis; r.nErrors = h.nErrors; r.nKept = h.nKept; r.nClustersAll = h.nClustersAll;
+    r.nClusters = h.nClusters; r.status = status; r.pad = 0;
+    *ev.result = r;
+  }
+}
+
+// ================================================================== k_export
+// Exact-size copies of requested outputs to mapped pinned host memory (transfers only
+// when asked).  Element counts are read from the device counters, so no host round trip.
+struct ExportItem { const void* src; void* dst; const DevCounters* cnt; u32 elemBytes; u32 countSel; u32 fixedCount; u32 pad; };
+// countSel: 0 = nDigis, 1 = nErrors, 2 = nClusters of *cnt (the event's final counters), 3 = fixedCount
+__global__ void __launch_bounds__(256)
+k_export(const ExportItem* __restrict__ items, u32 nItems) {
+  for (u32 it = blockIdx.y; it < nItems; it += gridDim.y) {
+    const ExportItem x = items[it];
+    u32 cnt = x.fixedCount;
+    if (x.countSel < 3u) { const DevCounters c = *x.cnt; cnt = x.countSel == 0 ? c.nDigis : x.countSel == 1 ? c.nErrors : c.nClusters; }
+    const size_t bytes = (size_t)cnt * x.elemBytes;
+    const size_t nVec = (bytes + 15) >> 4;                 // buffers are padded to 16 B
+    const uint4* s = reinterpret_cast<const uint4*>(x.src);
+    uint4* d = reinterpret_cast<uint4*>(x.dst);
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nVec; v += (size_t)gridDim.x * blockDim.x) d[v] = s[v];
+  }
+}
+
+}  // namespace pixreco

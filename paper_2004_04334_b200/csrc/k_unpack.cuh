@@ -124,12 +124,13 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
 #pragma unroll
     for (int s = 0; s < kRawSlots; ++s) mbar_init(&sh.full[s], 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    const u32 blk = min(pro, (u32)kDrawAhead);               // the first block of consecutive tiles: one atomic
-    const u32 t0 = atomicAdd(&lc->tileTicket, blk);
+    // ONE ticket now, the next ones one per iteration: consecutive tiles go to different CTAs, which count (and
+    // publish) them at about the same time — a block of consecutive tiles per CTA would make every CTA's first
+    // look-back wait for its predecessor's third iteration, a chain through the whole grid
+    const u32 t0 = atomicAdd(&lc->tileTicket, 1u);
     if (t0 == 0u) lc->tStart = global_timer();
 #pragma unroll
-    for (u32 j = 0; j < (u32)kDescRing; ++j)
-      sh.tile[j] = j < blk ? (t0 + j < totalTiles ? t0 + j : kTileEnd) : (j < (u32)kDrawAhead && t0 + blk <= totalTiles ? kTileSkip : kTileEnd);
+    for (u32 j = 0; j < (u32)kDescRing; ++j) sh.tile[j] = j == 0u ? (t0 < totalTiles ? t0 : kTileEnd) : (j < (u32)kDrawAhead && t0 < totalTiles ? kTileSkip : kTileEnd);
     sh.last = 0u;
   }
   __syncthreads();
@@ -155,7 +156,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     u64 lb[kLookBack];
     if (ctl) {
       // a new ticket (it becomes local tile i + kDrawAhead); the descriptor of the one drawn an iteration ago
-      if (i >= 0 && !ended && inflight < pro && lane == 0) tkt = atomicAdd(&lc->tileTicket, 1u);
+      if (!ended && inflight < pro && lane == 0) tkt = atomicAdd(&lc->tileTicket, 1u);
       if (!kSingle && tktP < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(batch + eP) + lane);
       if (lane == 0 && i > 0) bulk_wait_read();               // the staging arrays are free again
     } else if (!scn && vc) {
@@ -272,12 +273,12 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         --inflight;
       }
       if (i >= 0) issue_load(i + kRawSlots);                   // into the slot this tile vacated (its ring entry was written an iteration ago)
-      if (i >= 1) {
+      if (i >= 1 - kCountAhead) {
         // ring entry of local tile i + kDrawAhead - 1: the ticket drawn in the previous iteration
         if (!kSingle && tktP < totalTiles) sh.desc[kd & (kDescRing - 1)][lane] = dword;
         if (lane == 0) sh.tile[kd & (kDescRing - 1)] = tktP < totalTiles ? tktP : (ended ? kTileEnd : kTileSkip);
       }
-      if (i >= 0) {
+      {
         // this iteration's draw: its event now, its descriptor in the next iteration
         tkt = __shfl_sync(0xFFFFFFFFu, tkt, 0);
         if (tkt < totalTiles) { ++inflight; if (!kSingle) eP = tileEvent[tkt]; }

@@ -23,4 +23,4 @@
 #include "common.cuh"
 #include "k_unpack.cuh"
 #include "k_cluster.cuh"
-#include "k_export.cuh"
+#include "k_finalize.cuh"

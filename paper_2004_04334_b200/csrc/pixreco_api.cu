@@ -44,7 +44,7 @@ struct pr_handle {
   std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
   std::atomic<int> sticky{0};
   bool timing = false;
-  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msExport = 0;   // guarded by mu
+  uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msFinalize = 0, msExport = 0;   // guarded by mu
   std::string lastCuda;
 };
 
@@ -66,14 +66,15 @@ struct pr_event {
   std::vector<uint32_t*> stW; std::vector<uint16_t*> stA; std::vector<ExportItem> items;   // per-acquire scratch, kept
   // per-acquire pool blocks
   void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr;
-  // persistent per-slot blocks (grown on demand).  The control block is ALL ZERO between acquires: the kernels put the
-  // zeros back themselves, so it is cleared only when it is (re)allocated.
+  // persistent per-slot blocks (grown on demand).  Control block: [LaunchCtl | counters | group counts | big-module list]
+  // zeroed by one small memset per acquire, then [look-back states of k_unpack], which k_unpack's last CTA puts back
+  // to zero itself (so that part is cleared only when the block is (re)allocated).
   void* ctl = nullptr; size_t ctlBytes = 0;
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
   int status = PR_OK;        // filled when completion is observed
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
   std::atomic<int> cbPending{0};             // a completion callback is queued and has not returned yet
-  cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, export
+  cudaEvent_t tev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // PR_FLAG_KERNEL_TIMING: start, unpack, cluster, finalize, export
   bool exported = false;
   bool transferStage = false;  // the work in flight is a pr_transfer: completion does not count the events again
   std::vector<void*> extraHost, extraDev;  // pinned / device blocks of pr_transfer stages, returned at release
@@ -121,9 +122,13 @@ void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, ui
   d.htX = c.take<float>(cap); d.htY = c.take<float>(cap); d.htXerr = c.take<float>(cap); d.htYerr = c.take<float>(cap);
   d.htRows = c.take<u32>(cap); d.htCols = c.take<u32>(cap); d.htFlags = c.take<u16>(cap);
   d.result = c.take<DevCounters>(1);
-  // touched only by units beyond the shared-memory caps
-  d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap); d.wsKnum = c.take<int32_t>(cap);
-  d.wsAcc = c.take<u32>((size_t)cap * kAccWords); d.stage = c.take<u32>((size_t)cap * kAccWords);
+  d.modCount = c.take<u32>(M + 4);
+  d.stS = c.take<double>(cap); d.stSx = c.take<double>(cap); d.stSy = c.take<double>(cap);
+  d.stLabel = c.take<u32>(cap); d.stSize = c.take<u32>(cap); d.stBoxR = c.take<u32>(cap); d.stBoxC = c.take<u32>(cap);
+  // touched only by modules beyond the shared-memory tiers
+  d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
+  d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
+  d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap); d.wsBox = c.take<u32>((size_t)cap * 4);
 }
 
 void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M) {
@@ -212,17 +217,6 @@ int fail_after_enqueue(pr_event* ev, int code) {
     if (e__ != cudaSuccess) return fail_after_enqueue((ev), cuda_fail((ev)->h, e__, #call)); \
   } while (0)
 
-// Modules per unit of k_cluster: a power of two <= kMaxGroup with a few hundred digis per unit, and enough units to
-// fill the GPU when the launch allows it.
-uint32_t pick_group(pr_handle* h, uint64_t totalWords, uint32_t n, uint32_t M) {
-  const double perModule = (double)totalWords / ((double)n * M) + 1e-9;
-  uint32_t G = kMaxGroup;
-  while (G > 1 && perModule * G > 448.0) G >>= 1;
-  const uint64_t resident = (uint64_t)h->smCount * h->clusterBlocksPerSM;
-  while (G > 2 && (uint64_t)n * ((M + G - 1) / G) < resident / 2) G >>= 1;
-  return G;
-}
-
 int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
   if (!ev || !ins || n == 0 || n > kMaxBatch) return PR_ERR_INVALID_ARG;
   pr_handle* h = ev->h;
@@ -288,11 +282,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     totalTiles += s.desc.nTiles;
     totalWords += s.in.n_words;
   }
-  // launches whose modules are large on average (configs[4]) go to k_dense: one module per unit
-  const bool denseKernel = totalWords > (uint64_t)256 * M * n;
-  const uint32_t G = denseKernel ? 1u : pick_group(h, totalWords, n, M);
-  const uint32_t nGroups = (M + G - 1) / G;
-  const size_t ctlNeed = sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + (size_t)8 * totalTiles + (size_t)4 * nGroups * n;
+  const size_t grpPerEv = align_up((M + 31) / 32, 16);      // u32 per event
+  // launches whose modules are large on average (configs[4]) hand their large modules to k_dense
+  const bool denseKernel = totalWords > (uint64_t)kWarpCap * M * n;
+  const size_t bigCap = denseKernel ? (size_t)(totalWords / (kWarpCap + 1) + 2) : 0;
+  // control block: [LaunchCtl | counters | group counts | big list] (zeroed per acquire), [tile states] (self-cleaning)
+  const size_t ctlZero = align_up(sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + 4 * grpPerEv * n + 4 * bigCap, 256);
+  const size_t ctlNeed = ctlZero + (size_t)8 * totalTiles;
 
   // ---- buffers from the pools (steady state: cache hits only)
   bool ctlFresh = false;
@@ -329,8 +325,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   char* ctl = (char*)ev->ctl;
   LaunchCtl* lc = (LaunchCtl*)ctl;
   DevCounters* counters = (DevCounters*)(ctl + sizeof(LaunchCtl));
-  u64* tileState = (u64*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
-  u32* grpAgg = (u32*)(tileState + totalTiles);
+  u32* grpCount = (u32*)(ctl + sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64));
+  u32* bigList = denseKernel ? grpCount + grpPerEv * n : nullptr;
+  u64* tileState = (u64*)(ctl + ctlZero);
   Carver cd(ev->devSlab), ch(ev->hostSlab);
   char *spanW = nullptr, *spanA = nullptr;
   if (merged) { spanW = cd.take<char>(wHi - wLo); spanA = cd.take<char>(aHi - aLo); }
@@ -347,7 +344,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.nWords = s.in.n_words; d.cap = s.cap;
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
     d.tileState = tileState + d.tileBase;
-    d.grpAgg = grpAgg + (size_t)nGroups * k;
+    d.grpCount = grpCount + grpPerEv * k;
     s.hostViews = pr_output{};
     if (want) carve_host(ch, s.hostViews, want, s.cap, M);
     ev->hostCounters[k] = HostCounters{};
@@ -355,7 +352,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
 
   // ---- enqueue (all asynchronous, one stream: P:L82).  From here on a failure goes through fail_after_enqueue.
   uint64_t nMemcpy = 0, nLaunch = 0;
-  if (ctlFresh) PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ev->ctlBytes, stream));   // only a new control block is cleared
+  // tickets, counters, group counts: one small memset; the look-back states only when the block is new (k_unpack's last
+  // CTA puts their zeros back, and those of its two ticket words, harmlessly cleared again here)
+  PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ctlFresh ? ev->ctlBytes : ctlZero, stream));
   if (merged) {
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
@@ -368,10 +367,22 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stA[k], s.in.adc, (size_t)s.in.n_words * 2, cudaMemcpyHostToDevice, stream));
       nMemcpy += 2;
     }
-  // k_cluster / k_dense: persistent CTAs taking units by ticket
-  const uint64_t units = (uint64_t)n * nGroups;
-  uint32_t clusterGrid = (uint32_t)(h->smCount * (denseKernel ? h->denseBlocksPerSM : h->clusterBlocksPerSM));
-  if (clusterGrid > units) clusterGrid = (uint32_t)units;
+  // k_cluster: persistent CTAs (dense scan + warp tickets).  A small launch gets one CTA per warp
+  // ticket or per possible dense module (a dense module has more than kWarpCap digis).
+  const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
+  // tickets of 4 modules when there are plenty, of 2 or 1 when the launch is small (a single event): every warp gets work
+  const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
+  const uint32_t modBatch = (uint64_t)n * M >= 4 * warpsResident ? kModBatch : (uint64_t)n * M >= 2 * warpsResident ? 2u : 1u;
+  const uint64_t warpTickets = ((uint64_t)n * ((M + modBatch - 1) / modBatch) + 7) / 8, maxDense = totalWords / (kWarpCap + 1);
+  const uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
+  uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
+  if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
+  if (clusterGrid < 1) clusterGrid = 1;
+  // k_finalize: one CTA per (event, 32 modules); huge events get several CTAs per group (about 8k words each)
+  uint32_t finSplits = (uint32_t)(totalWords / ((uint64_t)n * unitsPerEvent * 8192) + 1);
+  if (finSplits > 64) finSplits = 64;
+  uint32_t denseGrid = (uint32_t)(h->smCount * h->denseBlocksPerSM);
+  if (denseGrid > bigCap) denseGrid = bigCap ? (uint32_t)bigCap : 1u;
   // k_unpack: persistent CTAs taking tiles by ticket; a CTA holds at most `pro` tiles at a time (7 = a full pipeline)
   uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
   if (unpackGrid > totalTiles) unpackGrid = totalTiles;
@@ -417,18 +428,22 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   if (n == 1) {
     k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, nullptr, nullptr, totalTiles, pro, lc, tileState, h->geom);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
-    if (denseKernel) k_dense<true><<<clusterGrid, kDenseThreads, h->denseSmem, stream>>>(d0, nullptr, 1, lc, h->geom);
-    else k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, nullptr, 1, lc, G, nGroups, h->geom);
+    k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, nullptr, 1, lc, bigList, modBatch, h->geom);
+    if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d0, nullptr, lc, bigList, h->geom);
+    if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d0, nullptr, 1, unitsPerEvent, finSplits, lc, h->geom);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
     k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, dd, (const u16*)(dd + n), totalTiles, pro, lc, tileState, h->geom);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
-    if (denseKernel) k_dense<false><<<clusterGrid, kDenseThreads, h->denseSmem, stream>>>(d0, dd, n, lc, h->geom);
-    else k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, dd, n, lc, G, nGroups, h->geom);
+    k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, dd, n, lc, bigList, modBatch, h->geom);
+    if (denseKernel) k_dense<false><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d0, dd, lc, bigList, h->geom);
+    if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
+    k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(d0, dd, n, unitsPerEvent, finSplits, lc, h->geom);
   }
-  nLaunch += 2;
+  nLaunch += denseKernel ? 4 : 3;
   PR_CUDA_Q(ev, cudaGetLastError());
-  if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
+  if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[3], stream));
   ev->exported = want != 0;
   if (want && !items.empty()) {
     const ExportItem* itab = (const ExportItem*)((const char*)ev->descDev + descPart);   // device-resident export table
@@ -443,7 +458,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ++nLaunch;
     PR_CUDA_Q(ev, cudaGetLastError());
   }
-  if (h->timing && want) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[3], stream));
+  if (h->timing && want) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[4], stream));
   PR_CUDA_Q(ev, cudaEventRecord(ev->done, stream));
   ev->n = n;
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
@@ -483,11 +498,12 @@ int poll(pr_event* ev) {
   ev->state = kDone;
   if (ev->transferStage) { ev->transferStage = false; ev->h->inFlight.fetch_sub(1); return PR_OK; }
   if (ev->h->timing) {
-    float a = 0, b = 0, c = 0;
-    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess) {
-      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[2], ev->tev[3]) != cudaSuccess) c = 0;
+    float a = 0, b = 0, c = 0, f = 0;
+    if (cudaEventElapsedTime(&a, ev->tev[0], ev->tev[1]) == cudaSuccess && cudaEventElapsedTime(&b, ev->tev[1], ev->tev[2]) == cudaSuccess &&
+        cudaEventElapsedTime(&f, ev->tev[2], ev->tev[3]) == cudaSuccess) {
+      if (ev->exported && cudaEventElapsedTime(&c, ev->tev[3], ev->tev[4]) != cudaSuccess) c = 0;
       std::lock_guard<std::mutex> g(ev->h->mu);
-      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msExport += c;
+      ev->h->timedAcquires++; ev->h->msUnpack += a; ev->h->msCluster += b; ev->h->msFinalize += f; ev->h->msExport += c;
     } else cudaGetLastError();
   }
   ev->h->inFlight.fetch_sub(1);
@@ -622,7 +638,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, cap, g.M, true, &sw, &sa);
     const uint32_t tiles = (cap + kTileWords - 1) / kTileWords;
-    const size_t ctlNeed = sizeof(LaunchCtl) + 64 + (size_t)8 * tiles + (size_t)4 * g.M;
+    const size_t ctlNeed = align_up(sizeof(LaunchCtl) + 64 + 4 * align_up((g.M + 31) / 32, 16), 256) + (size_t)8 * tiles;
     std::vector<void*> a, b, c;
     for (uint32_t i = 0; i < cfg->max_events_in_flight; ++i) {
       a.push_back(h->devPool->alloc(cd.off, nullptr));
@@ -648,7 +664,7 @@ int pr_destroy(pr_handle* h) {
     if (ev->ctl) h->devPool->free(ev->ctl, nullptr, true);
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
     if (ev->done) cudaEventDestroy(ev->done);
-    for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+    for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
@@ -668,7 +684,7 @@ int pr_event_create(pr_handle* h, pr_event** out) {
   cudaError_t e = cudaEventCreateWithFlags(&ev->done, cudaEventDisableTiming);
   if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
   if (h->timing)
-    for (int i = 0; i < 4; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
+    for (int i = 0; i < 5; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
   { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
   *out = ev;
   return PR_OK;
@@ -683,7 +699,7 @@ int pr_event_destroy(pr_event* ev) {
   if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
   if (ev->done) cudaEventDestroy(ev->done);
-  for (int i = 0; i < 4; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+  for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
   {
     std::lock_guard<std::mutex> g(h->mu);
     for (size_t i = 0; i < h->slots.size(); ++i)
@@ -865,7 +881,7 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
   h->devPool->stats(&out->device_pool); h->hostPool->stats(&out->host_pool);
   {
     std::lock_guard<std::mutex> g(h->mu);
-    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->export_ms = h->msExport;
+    out->timed_acquires = h->timedAcquires; out->unpack_ms = h->msUnpack; out->cluster_ms = h->msCluster; out->finalize_ms = h->msFinalize; out->export_ms = h->msExport;
   }
   return PR_OK;
 }

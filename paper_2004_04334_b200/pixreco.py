@@ -85,7 +85,8 @@ class pr_stats(ctypes.Structure):
                                          "kernel_launches", "memcpy_calls", "callbacks_fired")] +
                 [("events_in_flight", c_uint32), ("max_events_in_flight", c_uint32),
                  ("device_pool", pr_pool_stats), ("host_pool", pr_pool_stats), ("timed_acquires", c_uint64),
-                 ("unpack_ms", ctypes.c_double), ("cluster_ms", ctypes.c_double), ("export_ms", ctypes.c_double)])
+                 ("unpack_ms", ctypes.c_double), ("cluster_ms", ctypes.c_double), ("finalize_ms", ctypes.c_double),
+                 ("export_ms", ctypes.c_double)])
 
 
 # every symbol include/pixreco.h declares: name -> (restype, argtypes)
