@@ -110,6 +110,9 @@ typedef struct {
                                       per-kernel device times into pr_stats (measurement aid; adds
                                       four cudaEventRecord per acquire)                            */
 
+#define PR_FLAG_NO_GRAPH      0x2u /* never replay a single event's chain from a CUDA graph (see pr_acquire); for A/B
+                                      measurements                                                 */
+
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
   const uint16_t* adc;            /* [n_words] parallel ADC values (<= 4095)                      */
@@ -182,7 +185,11 @@ int pr_event_destroy(pr_event* ev);                  /* PR_ERR_BAD_STATE while w
  * cluster+reduce, optional exact-size host mirrors, completion event, optional callback — on
  * `cuda_stream` (a cudaStream_t passed as void*, e.g. torch.cuda.Stream().cuda_stream; NULL is
  * the legacy default stream) and return at once.  Argument/state errors are returned here and
- * nothing is enqueued.  The slot must be idle (fresh or released).                               */
+ * nothing is enqueued.  The slot must be idle (fresh or released).
+ * A device-resident event without host mirrors is enqueued with ONE call: the slot keeps an instantiated CUDA graph of
+ * its chain (clear control words, descriptor upload, the three kernels, completion event), everything that changes
+ * from event to event travels in the descriptor; it is rebuilt only when the event size class changes.  The paper
+ * found CUDA graphs "too restrictive" for its modules in 2020; for one module's fixed chain they fit.     */
 int pr_acquire(pr_event* ev, const pr_input* in, void* cuda_stream);
 /* Same for a batch of n independent events processed by ONE chain of launches on one stream
  * (B200-first: one Run-3 event is ~1000x too small to fill the GPU).  All inputs share mem_kind

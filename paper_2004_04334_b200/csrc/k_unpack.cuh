@@ -38,6 +38,7 @@ constexpr int kRawSlots = 4;                      // raw tiles in the shared-mem
 constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
 constexpr int kDescRing = 8;                      // descriptor / tile-index ring, power of two >= kRawSlots + 4
 constexpr int kDrawAhead = 6;                     // a ticket drawn in iteration i becomes local tile i + kDrawAhead
+constexpr u32 kTilesFromDesc = 0xFFFFFFFDu;       // totalTiles argument of a graph launch: take nTiles of the (one) event
 constexpr u32 kTileSkip = 0xFFFFFFFEu, kTileEnd = 0xFFFFFFFFu;   // pipeline slot without a tile: a bubble / no more tiles
 constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
 static_assert(kCountAhead >= 1 && kCountAhead <= kRawSlots - 2, "a raw tile needs a full iteration to arrive before it is counted");
@@ -92,6 +93,9 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u;
+  // a launch replayed from a CUDA graph does not know its size when it is recorded: a one-event launch then reads it
+  // from the event's descriptor
+  if (!kSingle && totalTiles == kTilesFromDesc) totalTiles = batch[0].nTiles;
   const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA and draws the tickets; warp 9 publishes and looks back
   const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
   auto desc_of = [&](int k) -> const EvDesc& {
@@ -194,6 +198,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
       if (lane == 0) { sh.wcnt[slot][warp] = cnt; sh.wmax[slot][warp] = cnt ? (mx >> 20) + 1u : 0u; }
     }
     __syncthreads();                                                                                           // #1
+    if (sh.last) break;                                        // the control warp saw the end with nothing in flight (written before this barrier)
     if (scn) {
       // ---- publish the aggregate of tile i + kCountAhead, issue the look-back loads of tile i + 1
       if (vc) {
@@ -284,6 +289,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
         if (tkt < totalTiles) { ++inflight; if (!kSingle) eP = tileEvent[tkt]; }
         else if (tkt != kTileSkip) ended = true;               // the launch has no more tiles
         tktP = tkt;
+        if (ended && inflight == 0u && lane == 0) sh.last = 1u;  // nothing left to do: everybody leaves at the next iteration
       }
       __syncwarp();
     } else if (scn) {
@@ -367,7 +373,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   __syncthreads();
   if (tid == 0) {
     __threadfence();
-    sh.last = atomicAdd(&lc->unpackExited, 1u) == gridDim.x - 1u ? 1u : 0u;
+    sh.last = atomicAdd(&lc->unpackExited, 1u) == gridDim.x - 1u ? 1u : 0u;     // (sh.last is reused: now "last CTA to leave")
   }
   __syncthreads();
   if (sh.last) {

@@ -43,7 +43,7 @@ struct pr_handle {
   std::atomic<uint64_t> evAcquired{0}, evProduced{0}, words{0}, digis{0}, clusters{0}, launches{0}, memcpys{0}, callbacks{0};
   std::atomic<uint32_t> inFlight{0}, maxInFlight{0};
   std::atomic<int> sticky{0};
-  bool timing = false;
+  bool timing = false, noGraph = false;
   uint64_t timedAcquires = 0; double msUnpack = 0, msCluster = 0, msFinalize = 0, msExport = 0;   // guarded by mu
   std::string lastCuda;
 };
@@ -80,6 +80,12 @@ struct pr_event {
   std::vector<void*> extraHost, extraDev;  // pinned / device blocks of pr_transfer stages, returned at release
   // last validated input pointers (their memory kind is not asked again)
   const void *lastWords = nullptr, *lastAdc = nullptr; uint32_t lastKind = 0;
+  // the single-event chain as an instantiated CUDA graph: everything that changes between events travels in the
+  // descriptor (gDescHost -> gDescDev by a copy node); rebuilt when the control block or the size class changes
+  cudaGraphExec_t gExec = nullptr; cudaStream_t capStream = nullptr;
+  EvDesc* gDescHost = nullptr; char* gDescDev = nullptr;      // [EvDesc][tile -> event map: zeros]
+  void* gCtl = nullptr; uint32_t gTilesClass = 0; size_t gCtlZero = 0;
+  uint64_t graphLaunches = 0, graphBuilds = 0;
 };
 
 namespace {
@@ -169,6 +175,14 @@ void CUDART_CB trampoline(void* p) {
   ev->cbPending.store(0, std::memory_order_release);   // only now may the slot be released, re-armed or destroyed
 }
 
+void destroy_graph(pr_event* ev) {
+  pr_handle* h = ev->h;
+  if (ev->gExec) { cudaGraphExecDestroy(ev->gExec); ev->gExec = nullptr; }
+  if (ev->capStream) { cudaStreamDestroy(ev->capStream); ev->capStream = nullptr; }
+  if (ev->gDescHost) { h->hostPool->free(ev->gDescHost, nullptr, true); ev->gDescHost = nullptr; }
+  if (ev->gDescDev) { h->devPool->free(ev->gDescDev, nullptr, true); ev->gDescDev = nullptr; }
+}
+
 void release_blocks(pr_event* ev, bool completed) {
   pr_handle* h = ev->h;
   if (ev->devSlab) { h->devPool->free(ev->devSlab, ev->stream, completed); ev->devSlab = nullptr; }
@@ -216,6 +230,60 @@ int fail_after_enqueue(pr_event* ev, int code) {
     cudaError_t e__ = (call);                               \
     if (e__ != cudaSuccess) return fail_after_enqueue((ev), cuda_fail((ev)->h, e__, #call)); \
   } while (0)
+
+// The chain of ONE device-resident event as a CUDA graph, recorded by stream capture on the slot's private stream (thread-
+// local capture mode: other threads' CUDA calls are not affected) and instantiated: clear the per-acquire control words,
+// upload the descriptor, k_unpack / k_cluster / k_finalize in their batch form with one event (the descriptor is read
+// from device memory), record the completion event.  Grids are those of the size class; CTAs without a tile or a ticket
+// leave at once.  Only here may a slot's acquire allocate (first use of a size class).
+int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc, u64* tileState, cudaStream_t stream) {
+  pr_handle* h = ev->h;
+  const uint32_t M = h->cfg.n_modules;
+  if (ev->gExec) { cudaGraphExecDestroy(ev->gExec); ev->gExec = nullptr; }
+  const size_t descBytes = align_up(sizeof(EvDesc) + sizeof(u16) * 4096, 256);
+  if (!ev->gDescHost) {
+    ev->gDescHost = (EvDesc*)h->hostPool->alloc(sizeof(EvDesc), nullptr);
+    ev->gDescDev = (char*)h->devPool->alloc(descBytes, nullptr);
+    if (!ev->gDescHost || !ev->gDescDev) return PR_ERR_OOM;
+  }
+  const EvDesc* dd = (const EvDesc*)ev->gDescDev;
+  const u16* tileEvent = (const u16*)(ev->gDescDev + sizeof(EvDesc));
+  const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
+  const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
+  const uint32_t modBatch = (uint64_t)M >= 4 * warpsResident ? kModBatch : (uint64_t)M >= 2 * warpsResident ? 2u : 1u;
+  const uint64_t warpTickets = ((uint64_t)((M + modBatch - 1) / modBatch) + 7) / 8, maxDense = (uint64_t)tilesClass * kTileWords / (kWarpCap + 1);
+  uint64_t wantCtas = warpTickets > maxDense ? warpTickets : maxDense;
+  uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
+  if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
+  if (clusterGrid < 1) clusterGrid = 1;
+  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
+  if (unpackGrid > tilesClass) unpackGrid = tilesClass;
+  uint32_t pro = (tilesClass + unpackGrid - 1) / unpackGrid;
+  if (pro >= 4) pro = 7;
+  const uint32_t finSplits = 1;                                  // (the class stays below 8192 words per module group on average)
+  cudaStream_t cs = ev->capStream;
+  cudaGraph_t graph = nullptr;
+  // the tile -> event map of a one-event launch is all zeros: cleared on the event's stream, ahead of the graph's first
+  // launch there (a later launch on another stream comes after this acquire was seen complete)
+  PR_CUDA(h, cudaMemsetAsync(ev->gDescDev, 0, descBytes, stream));
+  cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+  if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamBeginCapture");
+  cudaMemsetAsync(ev->ctl, 0, ctlZero, cs);
+  cudaMemcpyAsync(ev->gDescDev, ev->gDescHost, sizeof(EvDesc), cudaMemcpyHostToDevice, cs);
+  EvDesc none{};
+  k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), cs>>>(none, dd, tileEvent, kTilesFromDesc, pro, lc, tileState, h->geom);
+  k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, cs>>>(none, dd, 1, lc, nullptr, modBatch, h->geom);
+  k_finalize<false><<<unitsPerEvent * finSplits, 256, 0, cs>>>(none, dd, 1, unitsPerEvent, finSplits, lc, h->geom);
+  cudaEventRecordWithFlags(ev->done, cs, cudaEventRecordExternal);   // an event-record NODE: ev->done stays an ordinary event the host can query
+  e = cudaStreamEndCapture(cs, &graph);
+  if (e != cudaSuccess || !graph) { cudaGetLastError(); return cuda_fail(h, e, "cudaStreamEndCapture"); }
+  e = cudaGraphInstantiate(&ev->gExec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { ev->gExec = nullptr; return cuda_fail(h, e, "cudaGraphInstantiate"); }
+  ev->gCtl = ev->ctl; ev->gTilesClass = tilesClass; ev->gCtlZero = ctlZero;
+  ++ev->graphBuilds;
+  return PR_OK;
+}
 
 int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_stream) {
   if (!ev || !ins || n == 0 || n > kMaxBatch) return PR_ERR_INVALID_ARG;
@@ -288,7 +356,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   const size_t bigCap = denseKernel ? (size_t)(totalWords / (kWarpCap + 1) + 2) : 0;
   // control block: [LaunchCtl | counters | group counts | big list] (zeroed per acquire), [tile states] (self-cleaning)
   const size_t ctlZero = align_up(sizeof(LaunchCtl) + align_up(sizeof(DevCounters) * n, 64) + 4 * grpPerEv * n + 4 * bigCap, 256);
-  const size_t ctlNeed = ctlZero + (size_t)8 * totalTiles;
+  // one device-resident event without mirrors: replayed from the slot's CUDA graph, built for its size class (tiles
+  // rounded up to a power of two, at least 8) — the whole class must stay on the warp-ticket path
+  uint32_t tilesClass = 8;
+  while (tilesClass < totalTiles) tilesClass <<= 1;
+  const bool useGraph = n == 1 && !stage && want == 0 && !h->timing && !h->noGraph && ev->capStream &&
+                        (uint64_t)tilesClass * kTileWords <= (uint64_t)kWarpCap * M && tilesClass <= 4096;
+  const size_t ctlNeed = ctlZero + (size_t)8 * (useGraph ? tilesClass : totalTiles);
 
   // ---- buffers from the pools (steady state: cache hits only)
   bool ctlFresh = false;
@@ -352,6 +426,17 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
 
   // ---- enqueue (all asynchronous, one stream: P:L82).  From here on a failure goes through fail_after_enqueue.
   uint64_t nMemcpy = 0, nLaunch = 0;
+  if (useGraph) {
+    if (ctlFresh) PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ev->ctlBytes, stream));     // a new control block: look-back states too
+    if (!ev->gExec || ev->gCtl != ev->ctl || ev->gTilesClass != tilesClass || ev->gCtlZero != ctlZero) {
+      int rc = build_graph(ev, tilesClass, ctlZero, lc, tileState, stream);
+      if (rc != PR_OK) return fail_after_enqueue(ev, rc);
+    }
+    *ev->gDescHost = ev->sub[0].desc;
+    PR_CUDA_Q(ev, cudaGraphLaunch(ev->gExec, stream));
+    ++ev->graphLaunches;
+    nLaunch = 3; nMemcpy = 1;
+  } else {
   // tickets, counters, group counts: one small memset; the look-back states only when the block is new (k_unpack's last
   // CTA puts their zeros back, and those of its two ticket words, harmlessly cleared again here)
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ctlFresh ? ev->ctlBytes : ctlZero, stream));
@@ -460,6 +545,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   }
   if (h->timing && want) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[4], stream));
   PR_CUDA_Q(ev, cudaEventRecord(ev->done, stream));
+  }
   ev->n = n;
   ev->doneFn = ins[0].done; ev->doneUser = ins[0].user;
   ev->status = PR_OK;
@@ -563,7 +649,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   *out = nullptr;
   if (!cfg || cfg->struct_size != sizeof(pr_config)) return PR_ERR_INVALID_ARG;
   if (cfg->n_modules < 1 || cfg->n_modules > 2048 || cfg->n_rows < 1 || cfg->n_rows > 256 || cfg->n_cols < 1 ||
-      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~PR_FLAG_KERNEL_TIMING))
+      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~(PR_FLAG_KERNEL_TIMING | PR_FLAG_NO_GRAPH)))
     return PR_ERR_INVALID_ARG;
   // A9/A21: ranges that make the 2^-14 fixed-point sums exact and overflow-free
   if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||
@@ -584,6 +670,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   h->cfg = *cfg;
   h->cfg.gain = h->cfg.pedestal = nullptr;
   h->timing = (cfg->flags & PR_FLAG_KERNEL_TIMING) != 0;
+  h->noGraph = (cfg->flags & PR_FLAG_NO_GRAPH) != 0;
   auto fail = [&](int code) { pr_destroy(h); return code; };
   if (cudaSetDevice(cfg->device) != cudaSuccess) { cudaGetLastError(); return fail(PR_ERR_CUDA); }
   cudaDeviceProp prop{};
@@ -665,6 +752,7 @@ int pr_destroy(pr_handle* h) {
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, nullptr, true);
     if (ev->done) cudaEventDestroy(ev->done);
     for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+    destroy_graph(ev);
     delete ev;
   }
   delete h->devPool; delete h->hostPool;
@@ -685,6 +773,7 @@ int pr_event_create(pr_handle* h, pr_event** out) {
   if (e != cudaSuccess) { delete ev; return cuda_fail(h, e, "cudaEventCreateWithFlags"); }
   if (h->timing)
     for (int i = 0; i < 5; ++i) PR_CUDA(h, cudaEventCreate(&ev->tev[i]));
+  if (!h->noGraph && cudaStreamCreateWithFlags(&ev->capStream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); ev->capStream = nullptr; }
   { std::lock_guard<std::mutex> g(h->mu); h->slots.push_back(ev); }
   *out = ev;
   return PR_OK;
@@ -700,6 +789,7 @@ int pr_event_destroy(pr_event* ev) {
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
   if (ev->done) cudaEventDestroy(ev->done);
   for (int i = 0; i < 5; ++i) if (ev->tev[i]) cudaEventDestroy(ev->tev[i]);
+  destroy_graph(ev);
   {
     std::lock_guard<std::mutex> g(h->mu);
     for (size_t i = 0; i < h->slots.size(); ++i)
