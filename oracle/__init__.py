@@ -48,6 +48,7 @@ def _load():
             getattr(_lib, name).restype = ctypes.c_int
         _lib.po_decode.restype = None
         _lib.po_calibrate.restype = None
+        _lib.po_occupancy.restype = None
     return _lib
 
 
@@ -191,6 +192,16 @@ def hits(clus, charge, row, col, n_clusters, n_rows=160, n_cols=416, pitch_row_u
         raise MemoryError("po_hits")
     return dict(ht_x=x[:N], ht_y=y[:N], ht_xerr=xe[:N], ht_yerr=ye[:N], ht_rows=rows[:N], ht_cols=cols[:N],
                 ht_flags=flags[:N])
+
+
+def occupancy(module, adc, kept, n_modules):
+    """Kept digis and their ADC sum per module (the second consumer of the digis, NEXT-2).  Returns (count u32[M], adc_sum u32[M])."""
+    module = np.ascontiguousarray(module, np.uint16)
+    adc = np.ascontiguousarray(adc, np.uint16)
+    kept = np.ascontiguousarray(kept, np.uint8)
+    cnt, tot = np.zeros(n_modules, np.uint32), np.zeros(n_modules, np.uint32)
+    _load().po_occupancy(_u32(module.shape[0]), _u32(n_modules), _p(module), _p(adc), _p(kept), _p(cnt), _p(tot))
+    return cnt, tot
 
 
 class Workspace:

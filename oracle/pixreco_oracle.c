@@ -254,6 +254,16 @@ int po_hits(uint32_t D, uint32_t N, uint32_t R, uint32_t C,
   return 0;
 }
 
+/* ---- occupancy (a second consumer of the digis on a parallel branch; the paper's Fig. 1 and
+ * section 4.2, only say that several modules may consume one product).  Per module m: the number of
+ * kept digis (charge >= pixThr, A8) and the sum of their ADC values (uint32, exact).                                   */
+void po_occupancy(uint32_t D, uint32_t M, const uint16_t *d_module, const uint16_t *d_adc, const uint8_t *kept,
+                  uint32_t *occ_count /* [M] */, uint32_t *occ_adc_sum /* [M] */) {
+  for (uint32_t m = 0; m < M; ++m) { occ_count[m] = 0; occ_adc_sum[m] = 0; }
+  for (uint32_t d = 0; d < D; ++d)
+    if (kept[d]) { occ_count[d_module[d]] += 1; occ_adc_sum[d_module[d]] += d_adc[d]; }
+}
+
 /* ---- the whole chain, in order O1..O5 (what bench.py's cpu_baseline times) ----
  * All output arrays have capacity W (mod_* arrays M+1) and are owned by the caller.
  * Hit arrays have capacity W too.

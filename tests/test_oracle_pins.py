@@ -245,3 +245,21 @@ def test_exact_sum_claim():
     cal = wl.Calib(np.array([33.333332, 80], np.float32), np.array([0.0001, 0], np.float32), 50.0, 60.0)
     with pytest.raises(ArithmeticError):
         oracle.run(ev.words, ev.adc, 2, cal.gain, cal.pedestal, 50.0, 60.0)
+
+
+def test_occupancy_against_numpy_and_worked_values():
+    """po_occupancy (second consumer of the digis): a worked example and numpy bincount on generated events."""
+    ev = wl.event_from_pixels([(0, 1, 1, 60), (0, 1, 2, 12), (2, 5, 5, 200), (2, 9, 9, 13), (2, 5, 6, 255)], 4)
+    cal = wl.flat_calib(4, 80.0, 0.0)
+    o = oracle.run(ev.words, ev.adc, 4, cal.gain, cal.pedestal)
+    cnt, tot = oracle.occupancy(o.module, o.adc, o.kept, 4)        # adc 12 -> 960 e is below the pixel threshold
+    assert list(cnt) == [1, 0, 3, 0] and list(tot) == [60, 0, 200 + 13 + 255, 0]
+    for config in (0, 1):
+        ev = wl.make_event(config, 3)
+        cal = wl.make_calib(config)
+        o = oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal)
+        cnt, tot = oracle.occupancy(o.module, o.adc, o.kept, ev.n_modules)
+        k = o.kept.astype(bool)
+        assert np.array_equal(cnt, np.bincount(o.module[k], minlength=ev.n_modules).astype(np.uint32))
+        assert np.array_equal(tot, np.bincount(o.module[k], weights=o.adc[k].astype(np.float64), minlength=ev.n_modules).astype(np.uint32))
+        assert int(cnt.sum()) == o.n_kept_digis
