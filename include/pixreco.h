@@ -47,7 +47,7 @@
 extern "C" {
 #endif
 
-#define PR_ABI_VERSION 3
+#define PR_ABI_VERSION 4
 
 /* ---- return codes (int).  Negative = error.  pr_strerror() names them. ---- */
 #define PR_OK               0
@@ -228,6 +228,41 @@ void* pr_event_cuda_event(pr_event* ev);
  * `consumer_stream` may read the slot's device buffers (addresses: a previous pr_produce of a same-
  * sized event on this slot, or any pr_produce after completion).                                 */
 int pr_stream_wait_event(pr_event* ev, void* consumer_stream);
+
+/* ---- chained modules (section 4.2; P:L76 Product<T> / ScopedContext) -------------------------------
+ * The chain of pr_acquire as separate modules that hand a PRODUCT to one another without a host wait:
+ *     raw --pr_digis_acquire--> digis --pr_clusters_acquire--> clusters + hits
+ *                                  \--pr_occupancy_acquire--> kept digis and ADC sum per module (a parallel branch)
+ * A product is what the paper's Product<T> carries: {device, the stream the producer's work was queued in, an event
+ * recorded after it} plus the device views.  It is available as soon as the producer's acquire has returned — the
+ * producer need not be complete — and stays valid until the producer's slot is released; pr_release of the producer
+ * answers PR_NOT_READY while a consumer that took the product has not been released.
+ * A consumer's acquire is the ScopedContext rule of P:L100 and L106-108: the FIRST consumer to ask for the product
+ * reuses the producer's stream (its work is simply queued behind the producer's: no synchronisation at all); every
+ * other consumer runs on the stream it brings along (`own_stream`) and makes it wait for the product's event with
+ * cudaStreamWaitEvent, unless cudaEventQuery says the event has completed already.  *used_stream (may be NULL) receives
+ * the stream the work went to.  Every module's slot completes like any other: pr_query / pr_produce / callback of
+ * pr_input (digis) / pr_release; a consumer's pr_produce fills the digi views of the product it consumed as well.   */
+typedef struct pr_product pr_product;
+/* raw -> digis: optional H2D staging, unpack + calibrate + compact, digi counters to the host.  pr_produce on this slot
+ * gives the digi and error views and n_digis / n_errors (cluster views NULL); `want` may hold DIGIS, CHARGE, ERRORS.  */
+int pr_digis_acquire(pr_event* ev, const pr_input* in, void* cuda_stream);
+/* The product of the slot's digis acquire (PR_ERR_BAD_STATE if there is none).  Never blocks.                         */
+int pr_digis_product(pr_event* ev, pr_product** out);
+/* {device, stream, event} of a product, as the paper's Product<T> exposes them.                             */
+int pr_product_info(const pr_product* p, int32_t* device, void** cuda_stream, void** cuda_event);
+/* digis -> clusters + hits on slot `ev` (idle, another slot than the producer's): the clustering and hit kernels of
+ * pr_acquire on the product's digi views.  `want`: mirrors as in pr_input (any PR_WANT_* bit); `done`/`user`: completion
+ * callback as in pr_input (may be NULL).  pr_produce on this slot gives everything pr_acquire's does.                   */
+int pr_clusters_acquire(pr_event* ev, pr_product* digis, uint32_t want, void* own_stream, void** used_stream,
+                        pr_done_fn done, void* user);
+/* digis -> occupancy on slot `ev`: per module the number of kept digis (charge >= pixel threshold) and the sum of
+ * their ADC values; both arrays [n_modules] are mirrored to pinned host memory (they are small).  All zero if the
+ * product's input order was violated (PR_STATUS_INPUT_ORDER: module boundaries undefined).                            */
+int pr_occupancy_acquire(pr_event* ev, pr_product* digis, void* own_stream, void** used_stream, pr_done_fn done, void* user);
+/* produce of an occupancy slot: PR_NOT_READY if early; views valid until pr_release(ev).                             */
+int pr_occupancy_produce(pr_event* ev, const uint32_t** d_count, const uint32_t** d_adc_sum,
+                         const uint32_t** h_count, const uint32_t** h_adc_sum);
 
 /* ---- pinned host memory from the handle's host pool, for inputs ---- */
 void* pr_host_alloc(pr_handle* h, size_t bytes);     /* NULL on failure */

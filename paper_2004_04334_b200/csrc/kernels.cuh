@@ -11,6 +11,7 @@
 //   k_dense    the same for launches whose modules are large on average: one module per CTA,
 //              occupancy bitmap + popcount ranks + union-find, larger shared-memory tiers.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
+//   k_publish_digis / k_import_digis / k_occupancy   the seams of the chained modules (k_chain.cuh).
 //
 // Kernels are batch-capable: a launch processes nEv independent events described by EvDesc
 // records (one Run-3-like event is ~1000x too small to fill a B200).  The single-event path
@@ -24,3 +25,4 @@
 #include "k_unpack.cuh"
 #include "k_cluster.cuh"
 #include "k_finalize.cuh"
+#include "k_chain.cuh"

@@ -56,8 +56,28 @@ struct SubEvent {            // host-side record of one event of the slot's batc
   pr_output hostViews{};
 };
 
+// What a module puts into the event for its consumers (the paper's Product<T>): device, the stream its work was
+// queued in, the event recorded after it — and the device views (the digi part of the descriptor).
+struct pr_product {
+  pr_event* producer = nullptr;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  cudaEvent_t event = nullptr;
+  std::atomic<int> streamTaken{0};   // the first consumer to ask reuses `stream`
+  std::atomic<int> consumers{0};     // consumers that took the product and have not been released yet
+  EvDesc desc{};                     // digi views, modDigiStart, result (the producer's final counters on the device)
+  uint32_t nWords = 0;
+  bool valid = false;
+};
+
+enum ModuleKind { kFullChain = 0, kDigisModule = 1, kClustersModule = 2, kOccupancyModule = 3 };
+
 struct pr_event {
   pr_handle* h = nullptr;
+  int module = kFullChain;           // which module's work the slot holds (chained modules: P:L98-108)
+  pr_product product;                // kDigisModule: what consumers take
+  pr_product* consumed = nullptr;    // consumers: the product they took (released with the slot)
+  uint32_t *occCount = nullptr, *occAdcSum = nullptr, *occHost = nullptr;   // kOccupancyModule: views into devSlab / hostSlab
   int state = kIdle;
   cudaEvent_t done = nullptr;
   cudaStream_t stream = nullptr;
@@ -70,6 +90,7 @@ struct pr_event {
   // zeroed by one small memset per acquire, then [look-back states of k_unpack], which k_unpack's last CTA puts back
   // to zero itself (so that part is cleared only when the block is (re)allocated).
   void* ctl = nullptr; size_t ctlBytes = 0;
+  size_t ctlZeroLast = 0;    // where the self-cleaning part began at the last acquire: if that moves, the whole block is cleared again
   HostCounters* hostCounters = nullptr; size_t hostCountersCap = 0;
   int status = PR_OK;        // filled when completion is observed
   pr_done_fn doneFn = nullptr; void* doneUser = nullptr;
@@ -116,18 +137,23 @@ struct Carver {
   }
 };
 
-// Device slab of one sub-event.  `stage`: room for the H2D copy of the inputs.
-void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, uint32_t** stageWords, uint16_t** stageAdc) {
+// Device slab of one sub-event, digi part (what k_unpack writes).  `stage`: room for the H2D copy of the inputs.
+void carve_digis(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, uint32_t** stageWords, uint16_t** stageAdc) {
   if (stage) { *stageWords = c.take<uint32_t>(cap); *stageAdc = c.take<uint16_t>(cap); }
   d.module = c.take<u16>(cap); d.row = c.take<u16>(cap); d.col = c.take<u16>(cap); d.adcOut = c.take<u16>(cap);
-  d.wordIdx = c.take<u32>(cap); d.charge = c.take<float>(cap); d.label = c.take<u32>(cap); d.clus = c.take<int32_t>(cap);
+  d.wordIdx = c.take<u32>(cap); d.charge = c.take<float>(cap);
   d.errWord = c.take<u32>(cap); d.errIdx = c.take<u32>(cap);
-  d.modDigiStart = c.take<u32>(M + 4); d.modClusStart = c.take<u32>(M + 4);
+  d.modDigiStart = c.take<u32>(M + 4);
+  d.result = c.take<DevCounters>(1);
+}
+// ... and the cluster part (k_cluster / k_dense / k_finalize).
+void carve_clusters(Carver& c, EvDesc& d, uint32_t cap, uint32_t M) {
+  d.label = c.take<u32>(cap); d.clus = c.take<int32_t>(cap);
+  d.modClusStart = c.take<u32>(M + 4);
   d.clLabel = c.take<u32>(cap); d.clSize = c.take<u32>(cap); d.clModule = c.take<u16>(cap);
   d.clCharge = c.take<float>(cap); d.clRow = c.take<float>(cap); d.clCol = c.take<float>(cap);
   d.htX = c.take<float>(cap); d.htY = c.take<float>(cap); d.htXerr = c.take<float>(cap); d.htYerr = c.take<float>(cap);
   d.htRows = c.take<u32>(cap); d.htCols = c.take<u32>(cap); d.htFlags = c.take<u16>(cap);
-  d.result = c.take<DevCounters>(1);
   d.modCount = c.take<u32>(M + 4);
   d.stS = c.take<double>(cap); d.stSx = c.take<double>(cap); d.stSy = c.take<double>(cap);
   d.stLabel = c.take<u32>(cap); d.stSize = c.take<u32>(cap); d.stBoxR = c.take<u32>(cap); d.stBoxC = c.take<u32>(cap);
@@ -135,6 +161,10 @@ void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, ui
   d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
   d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
   d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap); d.wsBox = c.take<u32>((size_t)cap * 4);
+}
+void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, uint32_t** stageWords, uint16_t** stageAdc) {
+  carve_digis(c, d, cap, M, stage, stageWords, stageAdc);
+  carve_clusters(c, d, cap, M);
 }
 
 void carve_host(Carver& c, pr_output& o, uint32_t want, uint32_t cap, uint32_t M) {
@@ -185,6 +215,9 @@ void destroy_graph(pr_event* ev) {
 
 void release_blocks(pr_event* ev, bool completed) {
   pr_handle* h = ev->h;
+  if (ev->consumed) { ev->consumed->consumers.fetch_sub(1); ev->consumed = nullptr; }   // the producer may be released now
+  ev->product.valid = false;
+  ev->module = kFullChain;
   if (ev->devSlab) { h->devPool->free(ev->devSlab, ev->stream, completed); ev->devSlab = nullptr; }
   if (ev->descDev) { h->devPool->free(ev->descDev, ev->stream, completed); ev->descDev = nullptr; }
   if (ev->hostSlab) { h->hostPool->free(ev->hostSlab, ev->stream, completed); ev->hostSlab = nullptr; }
@@ -373,6 +406,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     if (!ev->ctl) return PR_ERR_OOM;
     ctlFresh = true;
   }
+  if (ev->ctlZeroLast != ctlZero) { ctlFresh = true; ev->ctlZeroLast = ctlZero; }   // another layout: its look-back states must start at zero too
   if (ev->hostCountersCap < n) {
     if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
     ev->hostCounters = (HostCounters*)h->hostPool->alloc(sizeof(HostCounters) * n, stream);
@@ -593,7 +627,9 @@ int poll(pr_event* ev) {
     } else cudaGetLastError();
   }
   ev->h->inFlight.fetch_sub(1);
-  ev->h->evProduced.fetch_add(ev->n); ev->h->digis.fetch_add(dg); ev->h->clusters.fetch_add(cl);
+  // chained modules: an event counts once, where it enters (digis) — its clusters where they are made
+  if (ev->module == kFullChain || ev->module == kDigisModule) { ev->h->evProduced.fetch_add(ev->n); ev->h->digis.fetch_add(dg); }
+  if (ev->module == kFullChain || ev->module == kClustersModule) ev->h->clusters.fetch_add(cl);
   return PR_OK;
 }
 
@@ -784,6 +820,7 @@ int pr_event_destroy(pr_event* ev) {
   pr_handle* h = ev->h;
   if (ev->state == kInFlight && poll(ev) != PR_OK) return PR_ERR_BAD_STATE;
   if (ev->cbPending.load(std::memory_order_acquire)) return PR_ERR_BAD_STATE;   // its completion callback has not returned yet
+  if (ev->product.consumers.load() > 0) return PR_ERR_BAD_STATE;               // a consumer still holds its product
   release_blocks(ev, true);
   if (ev->ctl) h->devPool->free(ev->ctl, ev->stream, true);
   if (ev->hostCounters) h->hostPool->free(ev->hostCounters, ev->stream, true);
@@ -825,6 +862,7 @@ int pr_release(pr_event* ev) {
   int r = poll(ev);
   if (r != PR_OK) return r;
   if (ev->cbPending.load(std::memory_order_acquire)) return PR_NOT_READY;   // the callback still reads the slot
+  if (ev->product.consumers.load() > 0) return PR_NOT_READY;                // a consumer still holds this slot's product
   release_blocks(ev, true);                      // completion observed: reusable by any stream at once
   ev->state = kIdle;
   ev->n = 0;
@@ -837,6 +875,7 @@ int pr_release_on(pr_event* ev, void* consumer_stream) {
   int r = poll(ev);
   if (r != PR_OK) return r;
   if (ev->cbPending.load(std::memory_order_acquire)) return PR_NOT_READY;
+  if (ev->product.consumers.load() > 0) return PR_NOT_READY;
   PR_CUDA(ev->h, cudaSetDevice(ev->h->cfg.device));
   ev->stream = (cudaStream_t)consumer_stream;    // the pool records an event on it and defers reuse by other streams
   release_blocks(ev, false);
@@ -977,3 +1016,5 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
 }
 
 }  // extern "C"
+
+#include "chain_api.cuh"

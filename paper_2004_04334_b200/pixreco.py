@@ -111,6 +111,12 @@ SIGNATURES = {
     "pr_last_cuda_error": (c_char_p, [c_void_p]),
     "pr_abi_version": (c_int, []),
     "pr_transfer": (c_int, [c_void_p, c_uint32, c_void_p, pr_done_fn, c_void_p]),
+    "pr_digis_acquire": (c_int, [c_void_p, POINTER(pr_input), c_void_p]),
+    "pr_digis_product": (c_int, [c_void_p, POINTER(c_void_p)]),
+    "pr_product_info": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_void_p), POINTER(c_void_p)]),
+    "pr_clusters_acquire": (c_int, [c_void_p, c_void_p, c_uint32, c_void_p, POINTER(c_void_p), pr_done_fn, c_void_p]),
+    "pr_occupancy_acquire": (c_int, [c_void_p, c_void_p, c_void_p, POINTER(c_void_p), pr_done_fn, c_void_p]),
+    "pr_occupancy_produce": (c_int, [c_void_p, POINTER(c_void_p), POINTER(c_void_p), POINTER(c_void_p), POINTER(c_void_p)]),
     "pr_pool_create": (c_int, [c_int, c_int, c_uint64, POINTER(c_void_p)]),
     "pr_pool_alloc": (c_void_p, [c_void_p, c_size_t, c_void_p]),
     "pr_pool_free": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -321,6 +327,50 @@ class EventSlot:
         if code < 0 and (raise_on_error or code in (PR_ERR_INVALID_ARG, PR_ERR_BAD_STATE, PR_ERR_CUDA)):
             _check(code, "pr_produce_batch", self.owner.handle)
         return code, [Output(outs[k], self.owner.device) for k in range(n)]
+
+    # ---- chained modules: raw -> digis | digis -> clusters + hits | digis -> occupancy
+    def digis_acquire(self, words, adc, stream=0, want=0, event_id=0, done=None) -> int:
+        inp, cb = self._input(words, adc, want, event_id, done)
+        self._keep = (words, adc, cb)
+        s = getattr(stream, "cuda_stream", stream)
+        return _check(lib().pr_digis_acquire(self.ptr, ctypes.byref(inp), c_void_p(s)), "pr_digis_acquire", self.owner.handle)
+
+    def digis_product(self) -> int:
+        """The product handle (an address) of this slot's digis acquire."""
+        p = c_void_p()
+        _check(lib().pr_digis_product(self.ptr, ctypes.byref(p)), "pr_digis_product", self.owner.handle)
+        return p.value
+
+    def clusters_acquire(self, product, want=0, own_stream=0, done=None) -> int:
+        """Returns the raw stream the work went to (the producer's for the first consumer, else ``own_stream``)."""
+        cb = pr_done_fn(done) if done is not None else pr_done_fn()
+        self._keep = cb
+        used = c_void_p()
+        s = getattr(own_stream, "cuda_stream", own_stream)
+        _check(lib().pr_clusters_acquire(self.ptr, c_void_p(product), want, c_void_p(s), ctypes.byref(used), cb, None),
+               "pr_clusters_acquire", self.owner.handle)
+        return used.value or 0
+
+    def occupancy_acquire(self, product, own_stream=0, done=None) -> int:
+        cb = pr_done_fn(done) if done is not None else pr_done_fn()
+        self._keep = cb
+        used = c_void_p()
+        s = getattr(own_stream, "cuda_stream", own_stream)
+        _check(lib().pr_occupancy_acquire(self.ptr, c_void_p(product), c_void_p(s), ctypes.byref(used), cb, None),
+               "pr_occupancy_acquire", self.owner.handle)
+        return used.value or 0
+
+    def occupancy_produce(self):
+        """Returns (code, count, adc_sum): numpy views of the pinned mirrors [n_modules] (None if early)."""
+        hc, ha = c_void_p(), c_void_p()
+        code = lib().pr_occupancy_produce(self.ptr, None, None, ctypes.byref(hc), ctypes.byref(ha))
+        if code == PR_NOT_READY:
+            return code, None, None
+        if code in (PR_ERR_INVALID_ARG, PR_ERR_BAD_STATE, PR_ERR_CUDA):
+            _check(code, "pr_occupancy_produce", self.owner.handle)
+        M = self.owner.n_modules
+        mk = lambda p: np.frombuffer((ctypes.c_char * (4 * M)).from_address(p.value), dtype=np.uint32, count=M)
+        return code, mk(hc), mk(ha)
 
     def release(self) -> int:
         code = _check(lib().pr_release(self.ptr), "pr_release", self.owner.handle)

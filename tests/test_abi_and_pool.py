@@ -20,7 +20,7 @@ def test_every_declared_symbol_is_exported_and_bound():
     lib = pr.lib()
     for name in declared:
         assert getattr(lib, name) is not None
-    assert lib.pr_abi_version() == 3
+    assert lib.pr_abi_version() == 4
     assert lib.pr_strerror(pr.PR_ERR_INPUT_ORDER).decode().startswith("input words")
 
 

@@ -62,22 +62,35 @@ def test_acquire_returns_at_once_behind_a_long_queue(pr):
         for sl, s in zip(slots, streams):          # warm every slot (ctl buffers, pool bins)
             sl.acquire(w, a, stream=s); wait(sl); sl.produce(); sl.release()
         torch.cuda.synchronize()
+        # warm the process for CONCURRENT streams too: the first launches behind busy streams make the driver set up its
+        # per-stream work queues (2-30 ms per call, once per process, whatever is launched) — not part of an acquire
+        for s in streams:
+            with torch.cuda.stream(s):
+                torch.cuda._sleep(int(0.02 * 2.0e9))
+        for sl, s in zip(slots, streams):
+            sl.acquire(w, a, stream=s)
+        for sl in slots:
+            wait(sl); sl.produce(); sl.release()
+        torch.cuda.synchronize()
         spin_cycles = int(0.3 * 2.0e9)                # ~300 ms at the B200's 1.97 GHz
         for s in streams:
             with torch.cuda.stream(s):
                 torch.cuda._sleep(spin_cycles)
-        t0 = time.perf_counter()
+        t_each = []
         for sl, s in zip(slots, streams):
+            t0 = time.perf_counter()
             sl.acquire(w, a, stream=s)
-        t_acq = time.perf_counter() - t0
+            t_each.append(time.perf_counter() - t0)
+        t_acq = sum(t_each)
         t0 = time.perf_counter()
         states = [sl.query() for sl in slots]
         codes = [sl.produce()[0] for sl in slots]
         t_poll = time.perf_counter() - t0
         assert states == [pr.PR_NOT_READY] * 8 and codes == [pr.PR_NOT_READY] * 8
-        # typically 0.2 ms and 0.05 ms; the slack is for a cold box (first process after boot)
-        assert t_acq < 0.05, f"8 acquires took {t_acq * 1e3:.2f} ms behind a 300 ms queue"
-        assert t_poll < 0.05
+        # typically 10-40 us per acquire through ctypes ("<< 1 ms"), against a 300 ms queue in front
+        assert float(np.median(t_each)) < 1e-3, f"median acquire {np.median(t_each) * 1e6:.0f} us: {t_each}"
+        assert t_acq < 0.02, f"8 acquires took {t_acq * 1e3:.2f} ms behind a 300 ms queue: {t_each}"
+        assert t_poll < 0.02
         assert slots[0].release() == pr.PR_NOT_READY            # nothing is released while in flight
         with pytest.raises(pr.PixRecoError):                    # acquire on a busy slot
             slots[0].acquire(w, a, stream=streams[0])
