@@ -24,20 +24,25 @@ namespace pixreco {
 // (first digi of the module + rank).  k_finalize turns the ranks into the event-wide dense
 // numbering (ascending label order, A12) and writes the cluster SoA.
 constexpr u32 kWarpCap = 256;                    // warp path: modules with at most this many digis
-constexpr u32 kWarpTab = 2 * kWarpCap;           // hash slots per warp (load <= 1/4 up to 128 digis, <= 1/2 beyond)
-constexpr u32 kAccRoots = 84;                    // clusters accumulated per pass over a module
+constexpr u32 kWarpScratch = 6144 - kWarpCap * (4 + 4 + 1 + 1 + 1 + 2);   // 2816 bytes
+constexpr u32 kAccRoots = kWarpScratch / 36;     // 78 clusters accumulated per pass over a module
 constexpr u32 kModBatch = 4;                     // most modules per warp ticket (small tickets: a short tail; 8 was 6 % slower, 16 17 %);
                                                  // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
-constexpr u32 kEmpty = 0xFFFFFFFFu;
 constexpr u32 kNoKey = 0xFFFFFFFFu;
+constexpr u32 kNoIdx = 0x1FFu;                   // "no digi" in a 9-bit index field (and the low bits of an empty column head)
 constexpr u32 kNoRank = 0xFFFFu;
 
-struct WarpRegion {                 // 5 KB of shared memory per warp
-  u32 tab[kWarpTab];                // hash table; afterwards L[256] then the head of the accumulators
-  uint2 nb[kWarpCap];               // 8 neighbour digi indices, one byte each (self = none); afterwards accumulators
-  u32 key[kWarpCap];                // row << 9 | col of kept digis, kNoKey otherwise
+struct WarpRegion {                 // 6 KB of shared memory per warp
+  u32 info[kWarpCap];               // col | row << 9 | next digi of the column << 17 (kNoIdx: none); kNoKey for a digi below the pixel threshold
+  float q[kWarpCap];                // charge
+  unsigned char L[kWarpCap];        // label-equivalence forest, finally the root = minimum digi index of the cluster
+  unsigned char rk[kWarpCap];       // at a root: rank of its cluster among the module's clusters (ascending label)
+  unsigned char rootAt[kWarpCap];   // root of the cluster with that rank
+  u16 edge[kWarpCap];               // the (at most two) kept backward neighbours, e1 | e2 << 8, self = none; then the kept-cluster rank per root
+  __align__(16) unsigned char scratch[kWarpScratch];   // column heads, then the unresolved edges, then the accumulators
 };
-static_assert(sizeof(u32) * (kWarpTab - kWarpCap) + sizeof(uint2) * kWarpCap >= kAccRoots * 36, "accumulators must fit");
+static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 2 * (512 + 4) && kWarpScratch >= 2 * 2 * kWarpCap, "scratch holds the accumulators, the column heads and the edge list");
+static_assert(sizeof(WarpRegion) == 6144, "6 KB per warp");
 
 __host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords, u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
   size_t w = (bitmapWords + 3) & ~3u;
@@ -88,28 +93,6 @@ struct ClusterShared {
 // max(511 - col) << 16 | max(col); __vmaxu2 combines two boxes.
 __device__ __forceinline__ u32 box_rows(u32 row) { return (255u - row) << 16 | row; }
 __device__ __forceinline__ u32 box_cols(u32 col) { return (511u - col) << 16 | col; }
-
-__device__ __forceinline__ u32 wm_slot(u32 key, u32 shift) { return (key * 0x9E3779B1u) >> shift; }
-// First digi on pixel `key` (a module without duplicate pixels), kEmpty if none.
-__device__ __forceinline__ u32 wm_find(const u32* tab, u32 pmask, u32 shift, u32 key) {
-  u32 h = wm_slot(key, shift);
-  for (;;) {
-    const u32 v = tab[h];
-    if (v == kEmpty) return kEmpty;
-    if ((v >> 8) == key) return v & 0xFFu;
-    h = (h + 1) & pmask;
-  }
-}
-// Minimum digi index on pixel `key` (duplicate pixels present: owner = min index, A6).
-__device__ __forceinline__ u32 wm_find_min(const u32* tab, u32 pmask, u32 shift, u32 key) {
-  u32 h = wm_slot(key, shift), best = kEmpty;
-  for (;;) {
-    const u32 v = tab[h];
-    if (v == kEmpty) return best;
-    if ((v >> 8) == key) best = min(best, v & 0xFFu);
-    h = (h + 1) & pmask;
-  }
-}
 
 // ---- warp path, one digi per lane: a PACK of consecutive modules with at most 32 digis together, digis
 // [s, s+n).  Everything lives in registers: lane i learns its neighbours by comparing its (module, row,
@@ -175,139 +158,184 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
   *keptDigis = __ballot_sync(0xFFFFFFFFu, kept); *roots = __ballot_sync(0xFFFFFFFFu, isRoot); *keptRoots = kb;
 }
 
-// ---- warp path: one module = digis [s, s+n), 0 < n <= kWarpCap, processed by the calling warp.
-// Returns (kept digis, clusters, kept clusters) in all lanes.
+// ---- warp path: one module = digis [s, s+n), 32 < n <= kWarpCap, processed by the calling warp with only __syncwarp
+// between its passes.  Returns (kept digis, clusters, kept clusters) in all lanes.
+//   P1  load; kept flag (A8); every kept digi is pushed on the list of its COLUMN (head per column, `next` inside the
+//       digi's info word).  The push is a plain store that is read back: of the lanes that hit one column in the same
+//       instruction one store lands, that lane links to the previous head, the others try again (no atomics).
+//   P2  neighbours: a walk over the digi's own column list (N = row - 1; a second digi on the same pixel, A6) and over
+//       the list of the column before (NW, W, SW).  Of these backward neighbours (column-major order) at most two
+//       edges are kept:  W ? {W} : { N ? N : NW,  SW }  — the dropped ones are adjacent to a kept one and are found from
+//       there, so the kept edges span every 8-adjacency.  A digi that shares its pixel with one of lower index keeps
+//       only the edge to that one.  Round 1 of the label equivalence is taken at once (labels = identity): the
+//       larger end of an edge is put under the smaller one.
+//   P3  label equivalence on the forest L[] (L[i] <= i, a digi of i's component; a root has L[i] == i): an edge
+//       whose ends have different roots hooks the larger root under the smaller one with a plain store (only while
+//       it still is a root: a tree is never split; of several lanes hooking one root in the same instruction one
+//       wins, the others find their edge unresolved in the next round) and stays on the list of unresolved edges; an
+//       edge whose ends share their root is resolved for good.  The first round looks at every edge, the following
+//       ones only at the list, until it is empty.  Roots only ever go under smaller roots: the final root of a
+//       component is its minimum digi index = the canonical label (A10).
+//   P4  flatten; rank of every root in ascending index (= label) order.
+//   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory (exact: at most 256 terms below
+//       2^43), size and bounding box, kAccRoots clusters per pass: the lanes of a 32-digi chunk that share a cluster
+//       are reduced with shuffles, their first lane owns the read-modify-write.
+//   P6  the roots apply the cluster threshold (A8), number the kept clusters and stage their sums.
+//   P7  per-digi outputs: label (final), cluster rank within the module.
+__device__ __forceinline__ u32 wm_find(const unsigned char* L, u32 x) {
+  u32 l = L[x];
+  for (;;) {
+    const u32 p = L[l];
+    if (p == l) return l;
+    l = p;
+  }
+}
+// Root a and root b are different: the larger one goes under the smaller one if it still is a root.
+__device__ __forceinline__ void wm_hook(unsigned char* L, u32 a, u32 b) {
+  const u32 hi = max(a, b), lo = min(a, b);
+  if (L[hi] == hi) L[hi] = (unsigned char)lo;
+}
+
 __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr, float q0, u32 rc0,
                                             u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   const u32 nPad = (n + 31u) & ~31u;
-  const u32 lg = min(32u - (u32)__clz((int)(max(4u * n, 128u) - 1u)), 9u);   // log2 table size: >= 4n up to 128 digis, 512 beyond
-  const u32 pmask = (1u << lg) - 1u, shift = 32u - lg;
-  u32* tab = wr.tab;
-  unsigned char* nbB = reinterpret_cast<unsigned char*>(wr.nb);
+  u16* head = reinterpret_cast<u16*>(wr.scratch);           // [C + 2]: head[c + 1] = last digi pushed on column c, head[0] stays empty
+  u16* active = reinterpret_cast<u16*>(wr.scratch);         // after P2: unresolved edges, i | e << 8
+  u16* krAt = wr.edge;                                      // after P3: rank among the module's KEPT clusters of the cluster rooted at i
 
-  // A: clear the table
-  for (u32 i = lane * 4u; i <= pmask; i += 128u) *reinterpret_cast<uint4*>(tab + i) = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
+  // P1
+  for (u32 i = lane; 2u * i < g.C + 3u; i += 32u) reinterpret_cast<u32*>(head)[i] = 0xFFFFFFFFu;
   __syncwarp();
-  // B: load, kept flag (A8), insert; every digi starts with no neighbours (all bytes = self)
-  // The loads run one chunk ahead (the first chunk came with the call): charge, row and col together.
-  u32 nKept = 0; bool dup = false;
+  u32 nKept = 0;
   float qc = q0; u32 rcc = rc0;
   for (u32 i = lane; i < nPad; i += 32u) {
     float qn = 0.f; u32 rcn = 0;
     if (i + 32u < n) { qn = ev.charge[s + i + 32u]; rcn = (u32)ev.row[s + i + 32u] << 9 | (u32)ev.col[s + i + 32u]; }
-    const u32 key = (i < n && qc >= g.pixThr) ? rcc : kNoKey;                  // A8
+    const bool kept = i < n && qc >= g.pixThr;                                   // A8
+    wr.q[i] = qc; wr.L[i] = (unsigned char)i;
+    u16* hp = head + (rcc & 511u) + 1u;
+    u32 next = kNoIdx;
+    bool pending = kept;
+    while (__any_sync(0xFFFFFFFFu, pending)) {
+      u32 old = 0;
+      if (pending) { old = *hp; *hp = (u16)i; }
+      __syncwarp();
+      if (pending && *hp == i) { next = old & kNoIdx; pending = false; }
+      __syncwarp();
+    }
+    wr.info[i] = kept ? (rcc | next << 17) : kNoKey;
+    nKept += __popc(__ballot_sync(0xFFFFFFFFu, kept));
     qc = qn; rcc = rcn;
-    wr.key[i] = key;
-    wr.nb[i] = make_uint2(i * 0x01010101u, i * 0x01010101u);
-    if (key != kNoKey) {
-      const u32 ent = key << 8 | i;
-      u32 h = wm_slot(key, shift);
+  }
+  __syncwarp();
+  // P2
+  for (u32 i = lane; i < nPad; i += 32u) {
+    const u32 x = wr.info[i];
+    u32 e1 = i, e2 = i;
+    if (x != kNoKey) {
+      const u32 c = x & 511u, r = (x >> 9) & 255u;
+      u32 W = kNoIdx, N = kNoIdx, NW = kNoIdx, SW = kNoIdx, own = kNoIdx;
+      u32 j = head[c + 1u];                        // the digi's own column: never empty
+      bool before = false;
       for (;;) {
-        const u32 old = atomicCAS(tab + h, kEmpty, ent);
-        if (old == kEmpty) break;
-        if ((old >> 8) == key) dup = true;
-        h = (h + 1) & pmask;
+        if (j >= kNoIdx) {
+          if (before) break;
+          before = true; j = head[c];
+          if (j >= kNoIdx) break;
+        }
+        const u32 y = wr.info[j], rj = (y >> 9) & 255u;
+        if (!before) {
+          if (rj == r) { if (j < i) own = min(own, j); }
+          else if (rj + 1u == r) N = j;
+        } else {
+          if (rj == r) W = j;
+          else if (rj + 1u == r) NW = j;
+          else if (rj == r + 1u) SW = j;
+        }
+        j = y >> 17;
+      }
+      if (own != kNoIdx) e1 = own;
+      else if (W != kNoIdx) e1 = W;
+      else {
+        e1 = N != kNoIdx ? N : NW;
+        if (e1 == kNoIdx) { e1 = SW != kNoIdx ? SW : i; }
+        else if (SW != kNoIdx) e2 = SW;
+      }
+      if (e1 != i) { const u32 hi = max(i, e1), lo = min(i, e1); if (wr.L[hi] > lo) wr.L[hi] = (unsigned char)lo; }
+      if (e2 != i) { const u32 hi = max(i, e2), lo = min(i, e2); if (wr.L[hi] > lo) wr.L[hi] = (unsigned char)lo; }
+    }
+    wr.edge[i] = (u16)(e1 | e2 << 8);
+  }
+  __syncwarp();
+  // P3: first every edge, then the unresolved ones
+  u32 nAct = 0;
+  for (u32 i = lane; i < nPad; i += 32u) {
+    const u32 ed = wr.edge[i], e1 = ed & 255u, e2 = ed >> 8;
+    bool u1 = false, u2 = false;
+    if (e1 != i) {
+      const u32 a = wm_find(wr.L, i), b = wm_find(wr.L, e1);
+      if (a != b) { u1 = true; wm_hook(wr.L, a, b); }
+      if (e2 != i) {
+        const u32 b2 = wm_find(wr.L, e2);
+        if (a != b2) { u2 = true; wm_hook(wr.L, a, b2); }
       }
     }
-    nKept += __popc(__ballot_sync(0xFFFFFFFFu, key != kNoKey));
-  }
-  dup = __any_sync(0xFFFFFFFFu, dup);
-  __syncwarp();
-  // C: backward neighbours W, NW, N, NE of every kept digi; an edge found is recorded on both
-  // ends (slot d of i, slot d+4 of the neighbour: one writer per slot).  A duplicate only follows
-  // its pixel's owner (A6).
-  for (u32 i = lane; i < nPad; i += 32u) {
-    const u32 key = wr.key[i];
-    if (key == kNoKey) continue;
-    const u32 row = key >> 9, col = key & 511u;
-    if (dup) {
-      const u32 owner = wm_find_min(tab, pmask, shift, key);
-      if (owner != i) { nbB[i * 8u] = (unsigned char)owner; continue; }
+    const u32 b1 = __ballot_sync(0xFFFFFFFFu, u1);
+    if (u1) active[nAct + __popc(b1 & lt)] = (u16)(i | e1 << 8);
+    nAct += __popc(b1);
+    const u32 b2 = __ballot_sync(0xFFFFFFFFu, u2);
+    if (b2) {
+      if (u2) active[nAct + __popc(b2 & lt)] = (u16)(i | e2 << 8);
+      nAct += __popc(b2);
     }
-    const bool up = row > 0, left = col > 0, right = col + 1 < g.C;
-#define WM_NB(cond, delta, d)                                                                      \
-    if (cond) {                                                                                    \
-      const u32 j = dup ? wm_find_min(tab, pmask, shift, key - (delta)) : wm_find(tab, pmask, shift, key - (delta)); \
-      if (j != kEmpty) { nbB[i * 8u + (d)] = (unsigned char)j; nbB[j * 8u + (d) + 4u] = (unsigned char)i; }          \
-    }
-    WM_NB(left, 1u, 0u)
-    WM_NB(up && left, 513u, 1u)
-    WM_NB(up, 512u, 2u)
-    WM_NB(up && right, 511u, 3u)
-#undef WM_NB
   }
   __syncwarp();
-  // D: label equivalence.  L[i] only decreases and always names a digi of i's component; a round
-  // takes the minimum over the neighbours, hooks the old representative under it, then flattens.
-  // The first round needs no look-ups: with L = identity the minimum over the neighbours is the minimum
-  // neighbour index.
-  u32* L = tab;
-  for (u32 i = lane; i < nPad; i += 32u) {
-    const uint2 nb = wr.nb[i];
-    u32 v = __vminu4(nb.x, nb.y);
-    v = __vminu4(v, v >> 16); v = __vminu4(v, v >> 8);
-    L[i] = min(i, v & 0xFFu);
-  }
-  __syncwarp();
-  for (u32 i = lane; i < nPad; i += 32u) {
-    u32 l = L[i], p;
-    while ((p = L[l]) != l) l = p;
-    L[i] = l;
-  }
-  __syncwarp();
-  for (;;) {
-    bool changed = false;
-    for (u32 i = lane; i < nPad; i += 32u) {
-      const uint2 nb = wr.nb[i];
-      const u32 li = L[i];
-      u32 m = li;
-      m = min(m, L[nb.x & 0xFFu]); m = min(m, L[(nb.x >> 8) & 0xFFu]); m = min(m, L[(nb.x >> 16) & 0xFFu]); m = min(m, L[nb.x >> 24]);
-      m = min(m, L[nb.y & 0xFFu]); m = min(m, L[(nb.y >> 8) & 0xFFu]); m = min(m, L[(nb.y >> 16) & 0xFFu]); m = min(m, L[nb.y >> 24]);
-      if (m < li) {
-        atomicMin(L + li, m);
-        if (li != i) atomicMin(L + i, m);
-        changed = true;
+  while (nAct) {
+    u32 nNew = 0;
+    for (u32 k = lane; k < ((nAct + 31u) & ~31u); k += 32u) {
+      bool keep = false; u32 pr = 0;
+      if (k < nAct) {
+        pr = active[k];
+        const u32 a = wm_find(wr.L, pr & 255u), b = wm_find(wr.L, pr >> 8);
+        if (a != b) { keep = true; wm_hook(wr.L, a, b); }
       }
-    }
-    if (!__any_sync(0xFFFFFFFFu, changed)) break;
-    __syncwarp();
-    for (u32 i = lane; i < nPad; i += 32u) {
-      u32 l = L[i], p;
-      while ((p = L[l]) != l) l = p;
-      L[i] = l;
+      __syncwarp();
+      const u32 kb = __ballot_sync(0xFFFFFFFFu, keep);
+      if (keep) active[nNew + __popc(kb & lt)] = (u16)pr;
+      nNew += __popc(kb);
     }
     __syncwarp();
+    nAct = nNew;
   }
-  // E: rank of every root among the module's clusters (ascending index): L[root] |= rank << 8
+  // P4
   u32 nR = 0;
   for (u32 i = lane; i < nPad; i += 32u) {
-    const bool isRoot = wr.key[i] != kNoKey && L[i] == i;
+    const bool kept = wr.info[i] != kNoKey;
+    u32 l = i;
+    if (kept) { l = wm_find(wr.L, i); wr.L[i] = (unsigned char)l; }
+    const bool isRoot = kept && l == i;
     const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
-    if (isRoot) L[i] = i | (nR + __popc(rb & lt)) << 8 | kNoRank << 16;
+    if (isRoot) { const u32 k = nR + __popc(rb & lt); wr.rk[i] = (unsigned char)k; wr.rootAt[k] = (unsigned char)i; }
     nR += __popc(rb);
   }
   __syncwarp();
-  // F: per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory, kAccRoots
-  // clusters per pass.  The lanes of one 32-digi chunk that share a cluster are reduced with
-  // shuffles, their first lane owns the read-modify-write; then the roots apply the cluster
-  // threshold (A8), number the kept clusters and stage their sums.
-  double* acc = reinterpret_cast<double*>(tab + kWarpCap);
-  u32* cnt = reinterpret_cast<u32*>(acc + kAccRoots * 3u);
-  u32* box = cnt + kAccRoots;                      // two words per cluster: rows, cols
+  // P5, P6
+  double* acc = reinterpret_cast<double*>(wr.scratch);
+  u32* cb = reinterpret_cast<u32*>(acc + kAccRoots * 3u);      // three words per cluster: size, box rows, box cols
   u32 nK = 0;
   for (u32 p0 = 0; p0 < nR; p0 += kAccRoots) {
     const u32 nAcc = min(nR - p0, kAccRoots);
     for (u32 i = lane; i < nAcc * 3u; i += 32u) acc[i] = 0.0;
-    for (u32 i = lane; i < nAcc; i += 32u) { cnt[i] = 0u; box[2u * i] = 0u; box[2u * i + 1u] = 0u; }
+    for (u32 i = lane; i < nAcc * 3u; i += 32u) cb[i] = 0u;
     __syncwarp();
     for (u32 i = lane; i < nPad; i += 32u) {
-      const u32 key = wr.key[i];
+      const u32 x = wr.info[i];
       u32 rk = 0; bool in = false;
       u32 r = 256u + lane;
-      if (key != kNoKey) {
-        r = L[i] & 0xFFu;
-        rk = ((L[r] >> 8) & 0xFFu) - p0;
+      if (x != kNoKey) {
+        r = wr.L[i];
+        rk = (u32)wr.rk[r] - p0;
         in = rk < nAcc;
         if (!in) r = 256u + lane;
       }
@@ -316,9 +344,10 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       double qf = 0.0, qx = 0.0, qy = 0.0;
       u32 bR = 0, bC = 0;
       if (in) {
-        qf = (double)(ev.charge[s + i] * 16384.0f);
-        qx = qf * (double)(key >> 9); qy = qf * (double)(key & 511u);
-        bR = box_rows(key >> 9); bC = box_cols(key & 511u);
+        const u32 row = (x >> 9) & 255u, col = x & 511u;
+        qf = (double)(wr.q[i] * 16384.0f);
+        qx = qf * (double)row; qy = qf * (double)col;
+        bR = box_rows(row); bC = box_cols(col);
       }
       // suffix sums along each cluster's lane list by pointer jumping: the first lane ends with the total
       const u32 above = peers & (0xFFFFFFFEu << lane);
@@ -333,36 +362,37 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       if (in && (peers & lt) == 0u) {                 // one owner per cluster and chunk
         double* a = acc + rk * 3u;
         a[0] += qf; a[1] += qx; a[2] += qy;
-        cnt[rk] += (u32)__popc(peers);
-        box[2u * rk] = __vmaxu2(box[2u * rk], bR); box[2u * rk + 1u] = __vmaxu2(box[2u * rk + 1u], bC);
+        u32* c = cb + rk * 3u;
+        c[0] += (u32)__popc(peers); c[1] = __vmaxu2(c[1], bR); c[2] = __vmaxu2(c[2], bC);
       }
       __syncwarp();
     }
-    for (u32 i = lane; i < nPad; i += 32u) {
-      const u32 w = wr.key[i] != kNoKey ? L[i] : 0u;
-      const u32 rk = ((w >> 8) & 0xFFu) - p0;
-      const bool mine = wr.key[i] != kNoKey && (w & 0xFFu) == i && rk < nAcc;
+    for (u32 k = lane; k < ((nAcc + 31u) & ~31u); k += 32u) {
       double S = 0.0;
-      if (mine) S = acc[rk * 3u];
-      const bool keptC = mine && __double2ll_rz(S) >= g.clusThrFixed;
+      if (k < nAcc) S = acc[k * 3u];
+      const bool keptC = k < nAcc && __double2ll_rz(S) >= g.clusThrFixed;
       const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
-      if (keptC) {
-        const u32 kr = nK + __popc(kb & lt), o = s + kr;
-        ev.stS[o] = S; ev.stSx[o] = acc[rk * 3u + 1u]; ev.stSy[o] = acc[rk * 3u + 2u];
-        ev.stLabel[o] = s + i; ev.stSize[o] = cnt[rk];
-        ev.stBoxR[o] = box[2u * rk]; ev.stBoxC[o] = box[2u * rk + 1u];
-        L[i] = (w & 0xFFFFu) | kr << 16;
+      if (k < nAcc) {
+        const u32 root = wr.rootAt[p0 + k];
+        u32 kr = kNoRank;
+        if (keptC) {
+          kr = nK + __popc(kb & lt);
+          const u32 o = s + kr;
+          ev.stS[o] = S; ev.stSx[o] = acc[k * 3u + 1u]; ev.stSy[o] = acc[k * 3u + 2u];
+          ev.stLabel[o] = s + root; ev.stSize[o] = cb[k * 3u];
+          ev.stBoxR[o] = cb[k * 3u + 1u]; ev.stBoxC[o] = cb[k * 3u + 2u];
+        }
+        krAt[root] = (u16)kr;
       }
       nK += __popc(kb);
     }
     __syncwarp();
   }
-  // G: per-digi outputs: label (final), cluster rank within the module
+  // P7
   for (u32 i = lane; i < n; i += 32u) {
-    const bool kept = wr.key[i] != kNoKey;
     u32 lab = kInvalid; int32_t cl = -1;
-    if (kept) {
-      const u32 r = L[i] & 0xFFu, kr = L[r] >> 16;
+    if (wr.info[i] != kNoKey) {
+      const u32 r = wr.L[i], kr = krAt[r];
       lab = s + r;
       if (kr != kNoRank) cl = (int32_t)kr;
     }
