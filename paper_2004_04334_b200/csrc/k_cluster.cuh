@@ -24,12 +24,12 @@ namespace pixreco {
 // (first digi of the module + rank).  k_finalize turns the ranks into the event-wide dense
 // numbering (ascending label order, A12) and writes the cluster SoA.
 constexpr u32 kWarpCap = 256;                    // warp path: modules with at most this many digis
+constexpr u32 kMediumCap = 1024;                 // one warp with its large arrays in the global workspace: up to this many digis
 constexpr u32 kWarpScratch = 6144 - kWarpCap * (4 + 4 + 1 + 1 + 1 + 2);   // 2816 bytes
 constexpr u32 kAccRoots = kWarpScratch / 36;     // 78 clusters accumulated per pass over a module
 constexpr u32 kModBatch = 4;                     // most modules per warp ticket (small tickets: a short tail; 8 was 6 % slower, 16 17 %);
                                                  // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
 constexpr u32 kNoKey = 0xFFFFFFFFu;
-constexpr u32 kNoIdx = 0x1FFu;                   // "no digi" in a 9-bit index field (and the low bits of an empty column head)
 constexpr u32 kNoRank = 0xFFFFu;
 
 struct WarpRegion {                 // 6 KB of shared memory per warp
@@ -41,7 +41,7 @@ struct WarpRegion {                 // 6 KB of shared memory per warp
   u16 edge[kWarpCap];               // the (at most two) kept backward neighbours, e1 | e2 << 8, self = none; then the kept-cluster rank per root
   __align__(16) unsigned char scratch[kWarpScratch];   // column heads, then the unresolved edges, then the accumulators
 };
-static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 2 * (512 + 4) && kWarpScratch >= 2 * 2 * kWarpCap, "scratch holds the accumulators, the column heads and the edge list");
+static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 4 * (512 + 2) && kWarpScratch >= 2 * 2 * kWarpCap, "scratch holds the accumulators, the column heads and the edge list");
 static_assert(sizeof(WarpRegion) == 6144, "6 KB per warp");
 
 __host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords, u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
@@ -86,7 +86,7 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
 
 struct ClusterShared {
   u32 scan[16];
-  u32 nBig, big[kClusterThreads];
+  u32 nBig, take, big[kClusterThreads];
 };
 
 // Bounding box (A28) as two words of two halfword maxima each: rows max(255 - row) << 16 | max(row), cols
@@ -182,7 +182,41 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
 //       are reduced with shuffles, their first lane owns the read-modify-write.
 //   P6  the roots apply the cluster threshold (A8), number the kept clusters and stage their sums.
 //   P7  per-digi outputs: label (final), cluster rank within the module.
-__device__ __forceinline__ u32 wm_find(const unsigned char* L, u32 x) {
+// Where warp_module keeps its arrays.  A module of at most kWarpCap digis lives in the warp's own 6 KB of shared memory
+// with one-byte digi indices; a module of up to kMediumCap digis (kMedium) keeps only the forest L[] (two-byte
+// indices), the column heads and the accumulators there, the rest lies in the event's global workspace at the
+// module's own digi range (cached in L1/L2; the module belongs to this warp alone).
+template <bool kMedium> struct WmStore;
+template <> struct WmStore<false> {
+  typedef unsigned char idx_t; typedef u16 pair_t;
+  static constexpr u32 kNoIdx = 0x1FFu, kIdxMask = 0xFFu, kPairShift = 8;
+  u32* info; float* q; idx_t *L, *rk, *rootAt; pair_t *edge, *active; u16* krAt; unsigned char* scratch; u32 accRoots;
+};
+template <> struct WmStore<true> {
+  typedef u16 idx_t; typedef u32 pair_t;
+  static constexpr u32 kNoIdx = 0x7FFu, kIdxMask = 0xFFFFu, kPairShift = 16;
+  u32* info; float* q; idx_t *L, *rk, *rootAt; pair_t *edge, *active; u16* krAt; unsigned char* scratch; u32 accRoots;
+};
+__device__ __forceinline__ WmStore<false> wm_store_small(WarpRegion& r) {
+  WmStore<false> st;
+  st.info = r.info; st.q = r.q; st.L = r.L; st.rk = r.rk; st.rootAt = r.rootAt; st.edge = r.edge;
+  st.active = reinterpret_cast<u16*>(r.scratch); st.krAt = r.edge; st.scratch = r.scratch; st.accRoots = kAccRoots;
+  return st;
+}
+// Medium module = digis [s, s + n), n <= kMediumCap: the warp's region holds L (2 KB) and 4 KB of scratch.
+__device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const EvDesc& ev, u32 s) {
+  WmStore<true> st;
+  unsigned char* base = reinterpret_cast<unsigned char*>(&r);
+  st.L = reinterpret_cast<u16*>(base); st.scratch = base + 2u * kMediumCap; st.accRoots = (sizeof(WarpRegion) - 2u * kMediumCap) / 36u;
+  st.info = ev.wsPerm + s; st.q = nullptr; st.edge = ev.wsParent + s;
+  st.rk = reinterpret_cast<u16*>(ev.wsRoot + s); st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
+  st.krAt = reinterpret_cast<u16*>(ev.wsKnum + s); st.active = reinterpret_cast<u32*>(ev.wsS + s);   // 2 n entries
+  return st;
+}
+static_assert(sizeof(WarpRegion) - 2u * kMediumCap >= 4u * (512u + 2u), "the medium layout's scratch holds the column heads");
+
+template <typename idx_t>
+__device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
   u32 l = L[x];
   for (;;) {
     const u32 p = L[l];
@@ -191,21 +225,27 @@ __device__ __forceinline__ u32 wm_find(const unsigned char* L, u32 x) {
   }
 }
 // Root a and root b are different: the larger one goes under the smaller one if it still is a root.
-__device__ __forceinline__ void wm_hook(unsigned char* L, u32 a, u32 b) {
+template <typename idx_t>
+__device__ __forceinline__ void wm_hook(idx_t* L, u32 a, u32 b) {
   const u32 hi = max(a, b), lo = min(a, b);
-  if (L[hi] == hi) L[hi] = (unsigned char)lo;
+  if (L[hi] == hi) L[hi] = (idx_t)lo;
 }
 
-__device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, WarpRegion& wr, float q0, u32 rc0,
+template <bool kMedium>
+__device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, const WmStore<kMedium>& wr, float q0, u32 rc0,
                                             u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
+  typedef typename WmStore<kMedium>::idx_t idx_t;
+  typedef typename WmStore<kMedium>::pair_t pair_t;
+  constexpr u32 kNoIdx = WmStore<kMedium>::kNoIdx, kIdxMask = WmStore<kMedium>::kIdxMask, kPairShift = WmStore<kMedium>::kPairShift;
+  const u32 kAccRoots = wr.accRoots;
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   const u32 nPad = (n + 31u) & ~31u;
-  u16* head = reinterpret_cast<u16*>(wr.scratch);           // [C + 2]: head[c + 1] = last digi pushed on column c, head[0] stays empty
-  u16* active = reinterpret_cast<u16*>(wr.scratch);         // after P2: unresolved edges, i | e << 8
-  u16* krAt = wr.edge;                                      // after P3: rank among the module's KEPT clusters of the cluster rooted at i
+  u32* head = reinterpret_cast<u32*>(wr.scratch);            // [C + 2]: head[c + 1] = last digi pushed on column c, head[0] stays empty
+  pair_t* active = wr.active;                               // after P2: unresolved edges, i | e << kPairShift
+  u16* krAt = wr.krAt;                                      // after P3: rank among the module's KEPT clusters of the cluster rooted at i
 
   // P1
-  for (u32 i = lane; 2u * i < g.C + 3u; i += 32u) reinterpret_cast<u32*>(head)[i] = 0xFFFFFFFFu;
+  for (u32 i = lane; i < g.C + 2u; i += 32u) head[i] = 0xFFFFFFFFu;
   __syncwarp();
   u32 nKept = 0;
   float qc = q0; u32 rcc = rc0;
@@ -213,68 +253,56 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     float qn = 0.f; u32 rcn = 0;
     if (i + 32u < n) { qn = ev.charge[s + i + 32u]; rcn = (u32)ev.row[s + i + 32u] << 9 | (u32)ev.col[s + i + 32u]; }
     const bool kept = i < n && qc >= g.pixThr;                                   // A8
-    wr.q[i] = qc; wr.L[i] = (unsigned char)i;
-    u16* hp = head + (rcc & 511u) + 1u;
+    if (!kMedium) wr.q[i] = qc;
+    wr.L[i] = (idx_t)i;
     u32 next = kNoIdx;
-    bool pending = kept;
-    while (__any_sync(0xFFFFFFFFu, pending)) {
-      u32 old = 0;
-      if (pending) { old = *hp; *hp = (u16)i; }
-      __syncwarp();
-      if (pending && *hp == i) { next = old & kNoIdx; pending = false; }
-      __syncwarp();
-    }
-    wr.info[i] = kept ? (rcc | next << 17) : kNoKey;
+    if (kept) next = atomicExch(head + (rcc & 511u) + 1u, i) & kNoIdx;
+    if (!kMedium || i < n) wr.info[i] = kept ? (rcc | next << 17) : kNoKey;      // (the global workspace ends at n)
     nKept += __popc(__ballot_sync(0xFFFFFFFFu, kept));
     qc = qn; rcc = rcn;
   }
   __syncwarp();
   // P2
   for (u32 i = lane; i < nPad; i += 32u) {
-    const u32 x = wr.info[i];
+    const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
     u32 e1 = i, e2 = i;
     if (x != kNoKey) {
       const u32 c = x & 511u, r = (x >> 9) & 255u;
-      u32 W = kNoIdx, N = kNoIdx, NW = kNoIdx, SW = kNoIdx, own = kNoIdx;
-      u32 j = head[c + 1u];                        // the digi's own column: never empty
-      bool before = false;
-      for (;;) {
-        if (j >= kNoIdx) {
-          if (before) break;
-          before = true; j = head[c];
-          if (j >= kNoIdx) break;
-        }
+      u32 W = kNoIdx, N = kNoIdx, NW = kNoIdx, SW = kNoIdx, own = i;
+      for (u32 j = head[c + 1u]; j < kNoIdx;) {    // the digi's own column (never empty): N, and the lowest digi on the same pixel
         const u32 y = wr.info[j], rj = (y >> 9) & 255u;
-        if (!before) {
-          if (rj == r) { if (j < i) own = min(own, j); }
-          else if (rj + 1u == r) N = j;
-        } else {
-          if (rj == r) W = j;
-          else if (rj + 1u == r) NW = j;
-          else if (rj == r + 1u) SW = j;
-        }
+        if (rj == r) own = min(own, j);
+        if (rj + 1u == r) N = j;
         j = y >> 17;
       }
-      if (own != kNoIdx) e1 = own;
+      for (u32 j = head[c]; j < kNoIdx;) {         // the column before: NW, W, SW
+        const u32 y = wr.info[j], d = ((y >> 9) & 255u) - r;
+        if (d == 0u) W = j;
+        if (d == 0xFFFFFFFFu) NW = j;
+        if (d == 1u) SW = j;
+        j = y >> 17;
+      }
+      if (own != i) e1 = own;
       else if (W != kNoIdx) e1 = W;
       else {
         e1 = N != kNoIdx ? N : NW;
         if (e1 == kNoIdx) { e1 = SW != kNoIdx ? SW : i; }
         else if (SW != kNoIdx) e2 = SW;
       }
-      if (e1 != i) { const u32 hi = max(i, e1), lo = min(i, e1); if (wr.L[hi] > lo) wr.L[hi] = (unsigned char)lo; }
-      if (e2 != i) { const u32 hi = max(i, e2), lo = min(i, e2); if (wr.L[hi] > lo) wr.L[hi] = (unsigned char)lo; }
+      if (e1 != i) { const u32 hi = max(i, e1), lo = min(i, e1); if (wr.L[hi] > lo) wr.L[hi] = (idx_t)lo; }
+      if (e2 != i) { const u32 hi = max(i, e2), lo = min(i, e2); if (wr.L[hi] > lo) wr.L[hi] = (idx_t)lo; }
     }
-    wr.edge[i] = (u16)(e1 | e2 << 8);
+    if (!kMedium || i < n) wr.edge[i] = (pair_t)(e1 | e2 << kPairShift);
   }
   __syncwarp();
   // P3: first every edge, then the unresolved ones
   u32 nAct = 0;
   for (u32 i = lane; i < nPad; i += 32u) {
-    const u32 ed = wr.edge[i], e1 = ed & 255u, e2 = ed >> 8;
+    const u32 ed = (!kMedium || i < n) ? (u32)wr.edge[i] : (i | i << kPairShift), e1 = ed & kIdxMask, e2 = ed >> kPairShift;
     bool u1 = false, u2 = false;
     if (e1 != i) {
       const u32 a = wm_find(wr.L, i), b = wm_find(wr.L, e1);
+      wr.L[i] = (idx_t)a;                   // (a root stays one; otherwise a shorter path for the finds to come)
       if (a != b) { u1 = true; wm_hook(wr.L, a, b); }
       if (e2 != i) {
         const u32 b2 = wm_find(wr.L, e2);
@@ -282,11 +310,11 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       }
     }
     const u32 b1 = __ballot_sync(0xFFFFFFFFu, u1);
-    if (u1) active[nAct + __popc(b1 & lt)] = (u16)(i | e1 << 8);
+    if (u1) active[nAct + __popc(b1 & lt)] = (pair_t)(i | e1 << kPairShift);
     nAct += __popc(b1);
     const u32 b2 = __ballot_sync(0xFFFFFFFFu, u2);
     if (b2) {
-      if (u2) active[nAct + __popc(b2 & lt)] = (u16)(i | e2 << 8);
+      if (u2) active[nAct + __popc(b2 & lt)] = (pair_t)(i | e2 << kPairShift);
       nAct += __popc(b2);
     }
   }
@@ -297,12 +325,12 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       bool keep = false; u32 pr = 0;
       if (k < nAct) {
         pr = active[k];
-        const u32 a = wm_find(wr.L, pr & 255u), b = wm_find(wr.L, pr >> 8);
+        const u32 a = wm_find(wr.L, pr & kIdxMask), b = wm_find(wr.L, pr >> kPairShift);
         if (a != b) { keep = true; wm_hook(wr.L, a, b); }
       }
       __syncwarp();
       const u32 kb = __ballot_sync(0xFFFFFFFFu, keep);
-      if (keep) active[nNew + __popc(kb & lt)] = (u16)pr;
+      if (keep) active[nNew + __popc(kb & lt)] = (pair_t)pr;
       nNew += __popc(kb);
     }
     __syncwarp();
@@ -311,12 +339,12 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   // P4
   u32 nR = 0;
   for (u32 i = lane; i < nPad; i += 32u) {
-    const bool kept = wr.info[i] != kNoKey;
+    const bool kept = (!kMedium || i < n) && wr.info[i] != kNoKey;
     u32 l = i;
-    if (kept) { l = wm_find(wr.L, i); wr.L[i] = (unsigned char)l; }
+    if (kept) { l = wm_find(wr.L, i); wr.L[i] = (idx_t)l; }
     const bool isRoot = kept && l == i;
     const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
-    if (isRoot) { const u32 k = nR + __popc(rb & lt); wr.rk[i] = (unsigned char)k; wr.rootAt[k] = (unsigned char)i; }
+    if (isRoot) { const u32 k = nR + __popc(rb & lt); wr.rk[i] = (idx_t)k; wr.rootAt[k] = (idx_t)i; }
     nR += __popc(rb);
   }
   __syncwarp();
@@ -330,14 +358,14 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     for (u32 i = lane; i < nAcc * 3u; i += 32u) cb[i] = 0u;
     __syncwarp();
     for (u32 i = lane; i < nPad; i += 32u) {
-      const u32 x = wr.info[i];
+      const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
       u32 rk = 0; bool in = false;
-      u32 r = 256u + lane;
+      u32 r = 0x10000u + lane;
       if (x != kNoKey) {
         r = wr.L[i];
         rk = (u32)wr.rk[r] - p0;
         in = rk < nAcc;
-        if (!in) r = 256u + lane;
+        if (!in) r = 0x10000u + lane;
       }
       const u32 peers = __match_any_sync(0xFFFFFFFFu, r);
       const u32 most = __reduce_max_sync(0xFFFFFFFFu, in ? (u32)__popc(peers) : 0u);
@@ -345,7 +373,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       u32 bR = 0, bC = 0;
       if (in) {
         const u32 row = (x >> 9) & 255u, col = x & 511u;
-        qf = (double)(wr.q[i] * 16384.0f);
+        qf = (double)((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
         qx = qf * (double)row; qy = qf * (double)col;
         bR = box_rows(row); bC = box_cols(col);
       }
@@ -601,15 +629,40 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       if (big) bigList[atomicAdd(&lc->nBig, 1u)] = gi;
       continue;
     }
-    if (tid == 0) sh.nBig = 0;
+    if (tid == 0) { sh.nBig = 0; sh.take = 0; }
     __syncthreads();
     if (big) sh.big[atomicAdd(&sh.nBig, 1u)] = gi;
     __syncthreads();
     const u32 nBig = sh.nBig;
+    // modules of at most kMediumCap digis: ONE warp each (the warp path with its large arrays in the global workspace),
+    // taken from the CTA's list; no warp waits for another one
+    for (;;) {
+      u32 k = 0;
+      if (lane == 0) k = atomicAdd(&sh.take, 1u);
+      k = __shfl_sync(0xFFFFFFFFu, k, 0);
+      if (k >= nBig) break;
+      const u32 gk = sh.big[k], e = gk / M, m = gk - e * M;
+      const EvDesc& ev = kSingle ? single : batch[e];
+      const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
+      if (nn > kMediumCap) continue;
+      const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
+      u32 nk, nr, cnt;
+      warp_module<true>(ev, g, s, nn, wm_store_medium(reinterpret_cast<WarpRegion*>(smemRaw)[warp], ev, s), q0, rc0, &nk, &nr, &cnt);
+      if (lane == 0) {
+        ev.modCount[m] = cnt;
+        if (cnt) atomicAdd(&ev.grpCount[m / 32u], cnt);
+        if (nk) atomicAdd(&ev.counters->nKept, nk);
+        if (nr) atomicAdd(&ev.counters->nClustersAll, nr);
+      }
+      __syncwarp();
+    }
+    __syncthreads();
+    // larger ones: the whole CTA
     for (u32 k = 0; k < nBig; ++k) {
       const u32 gk = sh.big[k], e = gk / M, m = gk - e * M;
       const EvDesc& ev = kSingle ? single : batch[e];
       const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
+      if (nn <= kMediumCap) continue;
       DenseCtx cx;
       dense_count(ev, g, s, nn, smemRaw, sh, cx);
       dense_stage(ev, m, s, nn, cx);
@@ -661,7 +714,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         preload(t1, &qNext, &rcNext);
         if (n <= kWarpCap) {                                 // else: the dense path wrote this module
           u32 nk, nr, cnt;
-          warp_module(ev, g, s, n, wr, q0, rc0, &nk, &nr, &cnt);
+          warp_module<false>(ev, g, s, n, wm_store_small(wr), q0, rc0, &nk, &nr, &cnt);
           accK += nk; accA += nr; accG += cnt;
           if (lane == 0) ev.modCount[m0 + k] = cnt;
         }
