@@ -86,7 +86,7 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
 
 struct ClusterShared {
   u32 scan[16];
-  u32 nBig, take, big[kClusterThreads];
+  u32 nBig, big[kClusterThreads];
 };
 
 // Bounding box (A28) as two words of two halfword maxima each: rows max(255 - row) << 16 | max(row), cols
@@ -611,17 +611,48 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const u32 M = g.M, total = nEv * M;
 
-  // ---- phase 1: dense path.  Module (e, m) has index e * M + m; CTA b looks at the indices
-  // congruent to b modulo the grid size (neighbouring hot modules go to different CTAs).
-  for (u32 base = 0; base < total; base += gridDim.x * kClusterThreads) {
-    const u32 gi = base + tid * gridDim.x + blockIdx.x;
+  // ---- phase 1: modules with more than kWarpCap digis.  Module (e, m) has index e * M + m; lane l of warp w of the
+  // launch looks at the indices congruent to l * (number of warps) + w, one per trip (neighbouring hot modules go to
+  // different warps).  More than kMediumCap digis (with a bigList: more than kWarpCap, handed to k_dense): the whole
+  // CTA on one module at a time (dense path).  kWarpCap + 1 .. kMediumCap digis: remembered (one bit per trip) and
+  // clustered afterwards by ONE warp each (the warp path with its large arrays in the global workspace): no warp
+  // waits for another one there, and these heavy modules are done before the tickets of phase 2.
+  WarpRegion& wr = reinterpret_cast<WarpRegion*>(smemRaw)[warp];
+  const u32 nWarps = gridDim.x * (kClusterThreads / 32u), gw = blockIdx.x * (kClusterThreads / 32u) + warp;
+  const u32 bigAbove = bigList ? kWarpCap : kMediumCap;
+  auto medium_modules = [&](u32 base0, u32 bits) {
+    for (u32 it = 0; it < 32u; ++it) {
+      const u32 gi = base0 + it * 32u * nWarps + lane * nWarps + gw;
+      for (u32 todo = __ballot_sync(0xFFFFFFFFu, (bits >> it) & 1u); todo; todo &= todo - 1u) {
+        const u32 gk = __shfl_sync(0xFFFFFFFFu, gi, __ffs((int)todo) - 1), e = gk / M, m = gk - e * M;
+        const EvDesc& ev = kSingle ? single : batch[e];
+        const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
+        const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
+        u32 nk, nr, cnt;
+        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, &nk, &nr, &cnt);
+        if (lane == 0) {
+          ev.modCount[m] = cnt;
+          if (cnt) atomicAdd(&ev.grpCount[m / 32u], cnt);
+          if (nk) atomicAdd(&ev.counters->nKept, nk);
+          if (nr) atomicAdd(&ev.counters->nClustersAll, nr);
+        }
+        __syncwarp();
+      }
+    }
+  };
+  u32 medBits = 0, trip = 0, base0 = 0;
+  for (u32 base = 0; base < total; base += 32u * nWarps, ++trip) {
+    if (trip == 32u) { if (__any_sync(0xFFFFFFFFu, medBits != 0u)) medium_modules(base0, medBits); medBits = 0; trip = 0; base0 = base; }
+    const u32 gi = base + lane * nWarps + gw;
     bool big = false;
     if (gi < total) {
       const u32 e = gi / M, m = gi - e * M;
       const EvDesc& ev = kSingle ? single : batch[e];
       if (!(ev.counters->status & 1u)) {              // A5 violated: modDigiStart is undefined, no per-digi work
         const u32 s = ev.modDigiStart[m], t = ev.modDigiStart[m + 1];
-        big = t >= s && t <= ev.cap && t - s > kWarpCap;
+        const bool ok = t >= s && t <= ev.cap;
+        big = ok && t - s > bigAbove;
+        if (ok && !big && t - s > kWarpCap) medBits |= 1u << trip;
         if (big && t - s > kMaxModuleDigis) { big = false; atomicOr(&ev.counters->status, 2u); ev.modCount[m] = 0u; }   // A9's own limit: PR_STATUS_CAPACITY, the module stays unclustered
       }
     }
@@ -629,40 +660,15 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       if (big) bigList[atomicAdd(&lc->nBig, 1u)] = gi;
       continue;
     }
-    if (tid == 0) { sh.nBig = 0; sh.take = 0; }
+    if (tid == 0) sh.nBig = 0;
     __syncthreads();
     if (big) sh.big[atomicAdd(&sh.nBig, 1u)] = gi;
     __syncthreads();
     const u32 nBig = sh.nBig;
-    // modules of at most kMediumCap digis: ONE warp each (the warp path with its large arrays in the global workspace),
-    // taken from the CTA's list; no warp waits for another one
-    for (;;) {
-      u32 k = 0;
-      if (lane == 0) k = atomicAdd(&sh.take, 1u);
-      k = __shfl_sync(0xFFFFFFFFu, k, 0);
-      if (k >= nBig) break;
-      const u32 gk = sh.big[k], e = gk / M, m = gk - e * M;
-      const EvDesc& ev = kSingle ? single : batch[e];
-      const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
-      if (nn > kMediumCap) continue;
-      const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
-      u32 nk, nr, cnt;
-      warp_module<true>(ev, g, s, nn, wm_store_medium(reinterpret_cast<WarpRegion*>(smemRaw)[warp], ev, s), q0, rc0, &nk, &nr, &cnt);
-      if (lane == 0) {
-        ev.modCount[m] = cnt;
-        if (cnt) atomicAdd(&ev.grpCount[m / 32u], cnt);
-        if (nk) atomicAdd(&ev.counters->nKept, nk);
-        if (nr) atomicAdd(&ev.counters->nClustersAll, nr);
-      }
-      __syncwarp();
-    }
-    __syncthreads();
-    // larger ones: the whole CTA
     for (u32 k = 0; k < nBig; ++k) {
       const u32 gk = sh.big[k], e = gk / M, m = gk - e * M;
       const EvDesc& ev = kSingle ? single : batch[e];
       const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
-      if (nn <= kMediumCap) continue;
       DenseCtx cx;
       dense_count(ev, g, s, nn, smemRaw, sh, cx);
       dense_stage(ev, m, s, nn, cx);
@@ -670,9 +676,9 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     }
     __syncthreads();
   }
+  if (__any_sync(0xFFFFFFFFu, medBits != 0u)) medium_modules(base0, medBits);
 
   // ---- phase 2: warp path.  A ticket is a batch of modBatch (1, 2 or 4) consecutive modules of one event.
-  WarpRegion& wr = reinterpret_cast<WarpRegion*>(smemRaw)[warp];
   // Tickets shrink towards the end of a large launch (modBatch 4): the first nEvA events are handed out four
   // modules at a time, the next nEvB events two at a time, the rest one by one, so that the last tickets are short.
   const u32 bpe = (M + modBatch - 1) / modBatch, bpeB = (M + 1u) / 2u;
