@@ -113,6 +113,10 @@ typedef struct {
 #define PR_FLAG_NO_GRAPH      0x2u /* never replay a single event's chain from a CUDA graph (see pr_acquire); for A/B
                                       measurements                                                 */
 
+#define PR_FLAG_UNPACK_OVERSUBSCRIBE 0x4u /* test aid: launch k_unpack with eight times as many CTAs as fit the device
+                                      at once.  Tiles are handed out by ticket, so a tile only ever waits for tiles of
+                                      CTAs that are already running: the launch must end all the same    */
+
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
   const uint16_t* adc;            /* [n_words] parallel ADC values (<= 4095)                      */

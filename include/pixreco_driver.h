@@ -33,6 +33,22 @@ int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slo
                     const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
                     uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res);
 
+/* What one event produced, as the issuing thread saw it in pr_produce: the counters, and FNV-1a (64-bit, over
+ * 32-bit words) fingerprints of the pinned-host mirrors h_label[n_digis] and h_cl_label[n_clusters] (0 when the
+ * input's `want` did not ask for that mirror), so that a caller can check EVERY event of a multi-threaded run
+ * against its own expectation.                                                                                   */
+typedef struct {
+  uint64_t event_id;
+  uint32_t n_digis, n_errors, n_kept_digis, n_clusters_all, n_clusters, status_bits;
+  uint32_t thread, pad;
+  uint64_t hash_label, hash_cl_label;
+} prd_event_record;
+
+/* As prd_run_streams; rec (may be NULL, else [n_events]) receives one record per event.                          */
+int prd_run_streams_rec(pr_event* const* slots, void* const* streams, uint32_t n_slots,
+                        const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
+                        uint64_t* t_start_ns, uint64_t* t_end_ns, prd_event_record* rec, prd_result* res);
+
 #ifdef __cplusplus
 }
 #endif

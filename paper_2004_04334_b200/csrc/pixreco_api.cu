@@ -289,7 +289,7 @@ int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc
   uint32_t clusterGrid = (uint32_t)(h->smCount * h->clusterBlocksPerSM);
   if (clusterGrid > wantCtas) clusterGrid = (uint32_t)wantCtas;
   if (clusterGrid < 1) clusterGrid = 1;
-  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
+  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM) * ((h->cfg.flags & PR_FLAG_UNPACK_OVERSUBSCRIBE) ? 8u : 1u);
   if (unpackGrid > tilesClass) unpackGrid = tilesClass;
   uint32_t pro = (tilesClass + unpackGrid - 1) / unpackGrid;
   if (pro >= 4) pro = 7;
@@ -503,7 +503,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   uint32_t denseGrid = (uint32_t)(h->smCount * h->denseBlocksPerSM);
   if (denseGrid > bigCap) denseGrid = bigCap ? (uint32_t)bigCap : 1u;
   // k_unpack: persistent CTAs taking tiles by ticket; a CTA holds at most `pro` tiles at a time (7 = a full pipeline)
-  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM);
+  uint32_t unpackGrid = (uint32_t)(h->smCount * h->unpackBlocksPerSM) * ((h->cfg.flags & PR_FLAG_UNPACK_OVERSUBSCRIBE) ? 8u : 1u);
   if (unpackGrid > totalTiles) unpackGrid = totalTiles;
   uint32_t pro = (totalTiles + unpackGrid - 1) / unpackGrid;
   if (pro >= 4) pro = 7;
@@ -685,7 +685,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   *out = nullptr;
   if (!cfg || cfg->struct_size != sizeof(pr_config)) return PR_ERR_INVALID_ARG;
   if (cfg->n_modules < 1 || cfg->n_modules > 2048 || cfg->n_rows < 1 || cfg->n_rows > 256 || cfg->n_cols < 1 ||
-      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~(PR_FLAG_KERNEL_TIMING | PR_FLAG_NO_GRAPH)))
+      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~(PR_FLAG_KERNEL_TIMING | PR_FLAG_NO_GRAPH | PR_FLAG_UNPACK_OVERSUBSCRIBE)))
     return PR_ERR_INVALID_ARG;
   // A9/A21: ranges that make the 2^-14 fixed-point sums exact and overflow-free
   if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||

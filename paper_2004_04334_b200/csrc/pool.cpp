@@ -87,6 +87,12 @@ CachingPool::~CachingPool() {
   {
     std::lock_guard<std::mutex> g(mu_);
     trim_locked(0);
+    for (auto& kv : free_)                               // still pending (work queued behind them when they were freed):
+      for (Block* b : kv.second) {                       // destroy is the end of the job, the owner has waited for its streams
+        st_.bytes_cached -= b->bytes;
+        release_block_locked(b);
+      }
+    free_.clear();
     for (auto& kv : live_) {                             // leaked by the user: give back anyway
       if (kv.second->event) backend_->event_destroy(kv.second->event);
       backend_->mem_free(kv.second->ptr);

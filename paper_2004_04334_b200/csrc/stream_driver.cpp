@@ -10,11 +10,18 @@
 namespace {
 using clk = std::chrono::steady_clock;
 inline double us_since(clk::time_point t0) { return std::chrono::duration<double, std::micro>(clk::now() - t0).count(); }
+
+// FNV-1a over 32-bit words: the per-event fingerprint a caller compares with its own hash of the expected array
+inline uint64_t fnv1a32(const uint32_t* p, size_t n) {
+  uint64_t h = 1469598103934665603ull;
+  for (size_t i = 0; i < n; ++i) { h ^= p[i]; h *= 1099511628211ull; }
+  return h;
+}
 }  // namespace
 
-extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slots,
-                               const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
-                               uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res) {
+extern "C" int prd_run_streams_rec(pr_event* const* slots, void* const* streams, uint32_t n_slots,
+                                   const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
+                                   uint64_t* t_start_ns, uint64_t* t_end_ns, prd_event_record* rec, prd_result* res) {
   if (!slots || !streams || !pool || !res || !n_slots || !n_pool || !n_threads) return PR_ERR_INVALID_ARG;
   if (n_threads > n_slots) n_threads = n_slots;
   std::atomic<int> status{PR_OK};
@@ -36,6 +43,14 @@ extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uin
       digis[t] += out.n_digis; clusters[t] += out.n_clusters; ++done[t];
       if (t_start_ns) t_start_ns[e] = out.t_start_ns;
       if (t_end_ns) t_end_ns[e] = out.t_end_ns;
+      if (rec) {
+        prd_event_record& q = rec[e];
+        q.event_id = out.event_id; q.n_digis = out.n_digis; q.n_errors = out.n_errors; q.n_kept_digis = out.n_kept_digis;
+        q.n_clusters_all = out.n_clusters_all; q.n_clusters = out.n_clusters; q.status_bits = out.status_bits;
+        q.thread = t;
+        q.hash_label = out.h_label ? fnv1a32(out.h_label, out.n_digis) : 0;
+        q.hash_cl_label = out.h_cl_label ? fnv1a32(out.h_cl_label, out.n_clusters) : 0;
+      }
       while ((r = pr_release(slots[s])) == PR_NOT_READY) {}
       inFlight[s] = -1;
       return r == PR_OK;
@@ -84,4 +99,10 @@ extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uin
   res->status = status.load();
   res->threads = n_threads;
   return res->status;
+}
+
+extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slots,
+                               const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
+                               uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res) {
+  return prd_run_streams_rec(slots, streams, n_slots, pool, n_pool, first, n_events, n_threads, t_start_ns, t_end_ns, nullptr, res);
 }

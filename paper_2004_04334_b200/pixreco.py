@@ -29,7 +29,7 @@ PR_WANT_ALL = 63
 PR_STATUS_INPUT_ORDER, PR_STATUS_CAPACITY = 1, 2
 PR_POOL_DEVICE, PR_POOL_PINNED, PR_POOL_FAKE = 0, 1, 2
 PR_INVALID_LABEL = 0xFFFFFFFF
-PR_FLAG_KERNEL_TIMING, PR_FLAG_NO_GRAPH = 1, 2
+PR_FLAG_KERNEL_TIMING, PR_FLAG_NO_GRAPH, PR_FLAG_UNPACK_OVERSUBSCRIBE = 1, 2, 4
 
 pr_done_fn = ctypes.CFUNCTYPE(None, c_void_p, c_int)
 
@@ -154,9 +154,17 @@ class prd_result(ctypes.Structure):
                 ("produce_polls", c_uint64), ("status", c_int32), ("threads", c_uint32)]
 
 
+class prd_event_record(ctypes.Structure):
+    _fields_ = [("event_id", c_uint64), ("n_digis", c_uint32), ("n_errors", c_uint32), ("n_kept_digis", c_uint32),
+                ("n_clusters_all", c_uint32), ("n_clusters", c_uint32), ("status_bits", c_uint32), ("thread", c_uint32),
+                ("pad", c_uint32), ("hash_label", c_uint64), ("hash_cl_label", c_uint64)]
+
+
 DRIVER_SIGNATURES = {
     "prd_run_streams": (c_int, [POINTER(c_void_p), POINTER(c_void_p), c_uint32, POINTER(pr_input), c_uint32, c_uint32, c_uint32,
                                 c_uint32, c_void_p, c_void_p, POINTER(prd_result)]),
+    "prd_run_streams_rec": (c_int, [POINTER(c_void_p), POINTER(c_void_p), c_uint32, POINTER(pr_input), c_uint32, c_uint32,
+                                    c_uint32, c_uint32, c_void_p, c_void_p, POINTER(prd_event_record), POINTER(prd_result)]),
 }
 _driver = None
 
@@ -174,22 +182,34 @@ def driver() -> ctypes.CDLL:
     return _driver
 
 
-def run_streams(slots, streams, inputs, n_events, n_threads=1, first=0, spans=False):
+def fnv1a32(words) -> int:
+    """The fingerprint of prd_event_record (FNV-1a, 64 bit, over 32-bit words) of a numpy u32 array."""
+    h = 1469598103934665603
+    for v in np.asarray(words, dtype=np.uint32).tolist():
+        h = ((h ^ v) * 1099511628211) & 0xFFFFFFFFFFFFFFFF
+    return h
+
+
+def run_streams(slots, streams, inputs, n_events, n_threads=1, first=0, spans=False, records=False):
     """One pr_acquire per event on its own stream (slot = stream = e mod len(slots)), issued from ``n_threads`` C++
-    host threads.  ``inputs``: a ctypes array of pr_input.  Returns a dict of the prd_result fields (+ spans)."""
+    host threads.  ``inputs``: a ctypes array of pr_input.  Returns a dict of the prd_result fields (+ spans, + one
+    prd_event_record per event under "records")."""
     n = len(slots)
     sl = (c_void_p * n)(*[s.ptr for s in slots])
     st = (c_void_p * n)(*[getattr(s, "cuda_stream", s) for s in streams])
     t0 = np.zeros(n_events, np.uint64) if spans else None
     t1 = np.zeros(n_events, np.uint64) if spans else None
     res = prd_result()
-    rc = driver().prd_run_streams(sl, st, n, inputs, len(inputs), first, n_events, n_threads,
-                                  t0.ctypes.data if spans else None, t1.ctypes.data if spans else None, ctypes.byref(res))
+    rec = (prd_event_record * n_events)() if records else None
+    rc = driver().prd_run_streams_rec(sl, st, n, inputs, len(inputs), first, n_events, n_threads,
+                                      t0.ctypes.data if spans else None, t1.ctypes.data if spans else None, rec, ctypes.byref(res))
     if rc != 0:
         raise PixRecoError(rc, "prd_run_streams")
     out = {k: getattr(res, k) for k, _ in prd_result._fields_}
     if spans:
         out["t_start_ns"], out["t_end_ns"] = t0, t1
+    if records:
+        out["records"] = rec
     return out
 
 

@@ -78,6 +78,16 @@ def test_sources_keep_the_papers_rules():
         if name in ("pr_create", "pr_destroy"):
             continue
         assert not hits, (name, hits)
+    # the pool: blocking or allocating CUDA calls only inside the backends' mem_alloc / mem_free (reached from a miss,
+    # from trim and from destroy); a wait on an event or a stream nowhere at all
+    pool = re.sub(r"//.*", "", open(os.path.join(csrc, "pool.cpp")).read())
+    assert not re.search(r"\bcuda(DeviceSynchronize|StreamSynchronize|EventSynchronize|StreamWaitEvent|Memcpy|Memset)\w*\s*\(", pool)
+    for m in re.finditer(r"\bcuda(Malloc|Free|HostAlloc|FreeHost)\w*\s*\(", pool):
+        line_start = pool.rfind("\n", 0, m.start()) + 1
+        head = pool[pool.rfind("\n", 0, pool.rfind("override", 0, m.end()) if "override" in pool[line_start:m.start()] else line_start):m.start()]
+        fn_decl = max(pool.rfind("mem_alloc(", 0, m.start()), pool.rfind("mem_free(", 0, m.start()))
+        other = max(pool.rfind(name, 0, m.start()) for name in ("event_create(", "event_destroy(", "event_record(", "event_done(", "::alloc(", "::free(", "::trim"))
+        assert fn_decl > other, ("pool.cpp", m.group(0), pool[line_start:pool.find("\n", m.end())])
     for fn in os.listdir(csrc):
         if fn.endswith(".cuh"):
             code = re.sub(r"//.*", "", open(os.path.join(csrc, fn)).read())
