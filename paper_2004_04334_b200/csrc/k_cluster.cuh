@@ -33,7 +33,7 @@ constexpr u32 kNoKey = 0xFFFFFFFFu;
 constexpr u32 kNoRank = 0xFFFFu;
 
 struct WarpRegion {                 // 6 KB of shared memory per warp
-  u32 info[kWarpCap];               // col | row << 9 | next digi of the column << 17 (kNoIdx: none); kNoKey for a digi below the pixel threshold
+  u32 info[kWarpCap];               // col | row' << 9 | next digi of the column << 20 (kNoIdx: none); kNoKey for a digi below the pixel threshold
   float q[kWarpCap];                // charge
   unsigned char L[kWarpCap];        // label-equivalence forest, finally the root = minimum digi index of the cluster
   unsigned char rk[kWarpCap];       // at a root: rank of its cluster among the module's clusters (ascending label)
@@ -189,7 +189,7 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
 template <bool kMedium> struct WmStore;
 template <> struct WmStore<false> {
   typedef unsigned char idx_t; typedef u16 pair_t;
-  static constexpr u32 kNoIdx = 0x1FFu, kIdxMask = 0xFFu, kPairShift = 8;
+  static constexpr u32 kNoIdx = 0x7FFu, kIdxMask = 0xFFu, kPairShift = 8;
   u32* info; float* q; idx_t *L, *rk, *rootAt; pair_t *edge, *active; u16* krAt; unsigned char* scratch; u32 accRoots;
 };
 template <> struct WmStore<true> {
@@ -231,9 +231,17 @@ __device__ __forceinline__ void wm_hook(idx_t* L, u32 a, u32 b) {
   if (L[hi] == hi) L[hi] = (idx_t)lo;
 }
 
+// A UNIT may hold up to four consecutive modules (digis [s, s + n); module j + 1 of the unit starts at digi s + bnd.b[j],
+// kNoBnd if the unit has no such module): their pixels are stacked along the row index with one empty row between two
+// modules (row' = row + j * (R + 1)), so that one pass clusters them all and no edge crosses a module border.  Kept
+// clusters are ranked per module; cntOut[j] receives module j's number of kept clusters.
+constexpr u32 kNoBnd = 0xFFFFFFFFu;
+struct UnitBounds { u32 b[3]; };
+__device__ __forceinline__ u32 unit_module(const UnitBounds& bnd, u32 i) { return (i >= bnd.b[0] ? 1u : 0u) + (i >= bnd.b[1] ? 1u : 0u) + (i >= bnd.b[2] ? 1u : 0u); }
+
 template <bool kMedium>
 __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, const WmStore<kMedium>& wr, float q0, u32 rc0,
-                                            u32* nKeptDigis, u32* nRootsOut, u32* nKeptClusters) {
+                                            const UnitBounds& bnd, u32* nKeptDigis, u32* nRootsOut, u32 (&cntOut)[4]) {
   typedef typename WmStore<kMedium>::idx_t idx_t;
   typedef typename WmStore<kMedium>::pair_t pair_t;
   constexpr u32 kNoIdx = WmStore<kMedium>::kNoIdx, kIdxMask = WmStore<kMedium>::kIdxMask, kPairShift = WmStore<kMedium>::kPairShift;
@@ -257,7 +265,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     wr.L[i] = (idx_t)i;
     u32 next = kNoIdx;
     if (kept) next = atomicExch(head + (rcc & 511u) + 1u, i) & kNoIdx;
-    if (!kMedium || i < n) wr.info[i] = kept ? (rcc | next << 17) : kNoKey;      // (the global workspace ends at n)
+    if (!kMedium || i < n) wr.info[i] = kept ? ((rcc + (unit_module(bnd, i) * (g.R + 1u) << 9)) | next << 20) : kNoKey;   // (the global workspace ends at n)
     nKept += __popc(__ballot_sync(0xFFFFFFFFu, kept));
     qc = qn; rcc = rcn;
   }
@@ -267,20 +275,20 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
     u32 e1 = i, e2 = i;
     if (x != kNoKey) {
-      const u32 c = x & 511u, r = (x >> 9) & 255u;
+      const u32 c = x & 511u, r = (x >> 9) & 0x7FFu;
       u32 W = kNoIdx, N = kNoIdx, NW = kNoIdx, SW = kNoIdx, own = i;
       for (u32 j = head[c + 1u]; j < kNoIdx;) {    // the digi's own column (never empty): N, and the lowest digi on the same pixel
-        const u32 y = wr.info[j], rj = (y >> 9) & 255u;
+        const u32 y = wr.info[j], rj = (y >> 9) & 0x7FFu;
         if (rj == r) own = min(own, j);
         if (rj + 1u == r) N = j;
-        j = y >> 17;
+        j = y >> 20;
       }
       for (u32 j = head[c]; j < kNoIdx;) {         // the column before: NW, W, SW
-        const u32 y = wr.info[j], d = ((y >> 9) & 255u) - r;
+        const u32 y = wr.info[j], d = ((y >> 9) & 0x7FFu) - r;
         if (d == 0u) W = j;
         if (d == 0xFFFFFFFFu) NW = j;
         if (d == 1u) SW = j;
-        j = y >> 17;
+        j = y >> 20;
       }
       if (own != i) e1 = own;
       else if (W != kNoIdx) e1 = W;
@@ -351,7 +359,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   // P5, P6
   double* acc = reinterpret_cast<double*>(wr.scratch);
   u32* cb = reinterpret_cast<u32*>(acc + kAccRoots * 3u);      // three words per cluster: size, box rows, box cols
-  u32 nK = 0;
+  cntOut[0] = cntOut[1] = cntOut[2] = cntOut[3] = 0u;
   for (u32 p0 = 0; p0 < nR; p0 += kAccRoots) {
     const u32 nAcc = min(nR - p0, kAccRoots);
     for (u32 i = lane; i < nAcc * 3u; i += 32u) acc[i] = 0.0;
@@ -372,7 +380,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       double qf = 0.0, qx = 0.0, qy = 0.0;
       u32 bR = 0, bC = 0;
       if (in) {
-        const u32 row = (x >> 9) & 255u, col = x & 511u;
+        const u32 row = ((x >> 9) & 0x7FFu) - unit_module(bnd, i) * (g.R + 1u), col = x & 511u;
         qf = (double)((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
         qx = qf * (double)row; qy = qf * (double)col;
         bR = box_rows(row); bC = box_cols(col);
@@ -397,22 +405,30 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     }
     for (u32 k = lane; k < ((nAcc + 31u) & ~31u); k += 32u) {
       double S = 0.0;
-      if (k < nAcc) S = acc[k * 3u];
+      u32 root = 0, mr = 4u;
+      if (k < nAcc) { S = acc[k * 3u]; root = wr.rootAt[p0 + k]; mr = unit_module(bnd, root); }
       const bool keptC = k < nAcc && __double2ll_rz(S) >= g.clusThrFixed;
       const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
+      u32 mine = 0;                                  // the kept roots of this chunk in my module; the roots come in ascending order
+#pragma unroll
+      for (u32 j = 0; j < 4u; ++j) {
+        const u32 mj = __ballot_sync(0xFFFFFFFFu, mr == j) & kb;
+        if (mr == j) mine = mj;
+        cntOut[j] += (u32)__popc(mj);
+      }
       if (k < nAcc) {
-        const u32 root = wr.rootAt[p0 + k];
         u32 kr = kNoRank;
         if (keptC) {
-          kr = nK + __popc(kb & lt);
-          const u32 o = s + kr;
+          // rank among the kept clusters of the root's own module: those of earlier chunks + those before me in this one
+          const u32 before = mr == 0u ? cntOut[0] : mr == 1u ? cntOut[1] : mr == 2u ? cntOut[2] : cntOut[3];
+          kr = before - (u32)__popc(mine) + (u32)__popc(mine & lt);
+          const u32 o = s + (mr ? bnd.b[mr - 1u] : 0u) + kr;
           ev.stS[o] = S; ev.stSx[o] = acc[k * 3u + 1u]; ev.stSy[o] = acc[k * 3u + 2u];
           ev.stLabel[o] = s + root; ev.stSize[o] = cb[k * 3u];
           ev.stBoxR[o] = cb[k * 3u + 1u]; ev.stBoxC[o] = cb[k * 3u + 2u];
         }
         krAt[root] = (u16)kr;
       }
-      nK += __popc(kb);
     }
     __syncwarp();
   }
@@ -426,7 +442,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     }
     ev.label[s + i] = lab; ev.clus[s + i] = cl;
   }
-  *nKeptDigis = nKept; *nRootsOut = nR; *nKeptClusters = nK;
+  *nKeptDigis = nKept; *nRootsOut = nR;
 }
 
 // ---- dense path: one module = digis [s, s+nn), nn > kWarpCap, processed by the whole CTA.
@@ -628,8 +644,10 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         const EvDesc& ev = kSingle ? single : batch[e];
         const u32 s = ev.modDigiStart[m], nn = ev.modDigiStart[m + 1] - s;
         const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
-        u32 nk, nr, cnt;
-        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, &nk, &nr, &cnt);
+        u32 nk, nr, cnts[4];
+        const UnitBounds one = {{kNoBnd, kNoBnd, kNoBnd}};
+        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, one, &nk, &nr, cnts);
+        const u32 cnt = cnts[0];
         if (lane == 0) {
           ev.modCount[m] = cnt;
           if (cnt) atomicAdd(&ev.grpCount[m / 32u], cnt);
@@ -715,28 +733,35 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         continue;
       }
       const float q0 = qNext; const u32 rc0 = rcNext;
-      if (t1 - s > 32u) {                                    // one module of its own
-        const u32 n = t1 - s;
+      if (t1 - s > kWarpCap) {                               // phase 1 wrote this module
         preload(t1, &qNext, &rcNext);
-        if (n <= kWarpCap) {                                 // else: the dense path wrote this module
-          u32 nk, nr, cnt;
-          warp_module<false>(ev, g, s, n, wm_store_small(wr), q0, rc0, &nk, &nr, &cnt);
-          accK += nk; accA += nr; accG += cnt;
-          if (lane == 0) ev.modCount[m0 + k] = cnt;
-        }
         ++k;
         continue;
       }
-      // pack: modules k .. k2-1, consecutive, consistent, at most 32 digis together
+      // unit: modules k .. k2-1, consecutive, consistent, at most kWarpCap digis together
       u32 k2 = k + 1u, e2 = t1, mIdx = 0, mStart = s;
       while (k2 < nm) {
         const u32 en = __shfl_sync(0xFFFFFFFFu, st, k2 + 1u);
-        if (en < e2 || en > ev.cap || en - s > 32u) break;
-        if (e2 - s <= lane) { mIdx = k2 - k; mStart = e2; }   // module k2 starts at e2
+        if (en < e2 || en > ev.cap || en - s > kWarpCap) break;
+        if (e2 - s <= lane) { mIdx = k2 - k; mStart = e2; }   // module k2 starts at e2 (what a pack of at most 32 digis needs)
         e2 = en; ++k2;
       }
       preload(e2, &qNext, &rcNext);
       const u32 n = e2 - s;
+      if (n > 32u) {                                         // shared-memory path, all modules of the unit in one pass
+        UnitBounds bnd;
+#pragma unroll
+        for (u32 j = 0; j < 3u; ++j) {
+          const u32 v = __shfl_sync(0xFFFFFFFFu, st, min(k + 1u + j, nm));
+          bnd.b[j] = k + 1u + j < k2 ? v - s : kNoBnd;
+        }
+        u32 nk, nr, cnts[4];
+        warp_module<false>(ev, g, s, n, wm_store_small(wr), q0, rc0, bnd, &nk, &nr, cnts);
+        accK += nk; accA += nr; accG += cnts[0] + cnts[1] + cnts[2] + cnts[3];
+        if (lane < k2 - k) ev.modCount[m0 + k + lane] = lane == 0u ? cnts[0] : lane == 1u ? cnts[1] : lane == 2u ? cnts[2] : cnts[3];
+        k = k2;
+        continue;
+      }
       u32 kd = 0, rb = 0, kb = 0;
       if (n) warp_pack(ev, g, s, n, q0, rc0, mIdx, mStart, &kd, &rb, &kb);
       accK += (u32)__popc(kd); accA += (u32)__popc(rb); accG += (u32)__popc(kb);
