@@ -246,7 +246,7 @@ int pr_clusters_acquire(pr_event* ev, pr_product* p, uint32_t want, void* own_st
   k_import_digis<<<1, 32, 0, stream>>>(d.counters, p->desc.result, lc);
   k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
   if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
-  k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, lc, h->geom);
+  k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, 1u, lc, h->geom);
   nLaunch += denseKernel ? 4 : 3;
   if (want) {
     std::vector<ExportItem>& items = ev->items;

@@ -84,6 +84,11 @@ __device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
   }
 }
 
+// What k_cluster / k_dense leave in clus[] for k_finalize: the digi's cluster as its rank among the kept clusters of
+// its module (below 2^17, A9) with the module's position among 128 consecutive modules above it, so that k_finalize
+// adds the module's first event-wide cluster number without looking the module up.
+__device__ __forceinline__ u32 clus_ranked(u32 rank, u32 module) { return rank | (module & 127u) << 20; }
+
 struct ClusterShared {
   u32 scan[16];
   u32 nBig, big[kClusterThreads];
@@ -101,7 +106,7 @@ __device__ __forceinline__ u32 box_cols(u32 col) { return (511u - col) << 16 | c
 // minimum lane is its root, sums run along each cluster's lane list.  mIdx/mStart: the lane's module
 // (index within the pack) and that module's first digi.  Returns the ballots of kept digis, of roots
 // and of roots of kept clusters.
-__device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s, u32 n, float q0, u32 rc0, u32 mIdx, u32 mStart,
+__device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s, u32 n, float q0, u32 rc0, u32 mFirst, u32 mIdx, u32 mStart,
                                           u32* keptDigis, u32* roots, u32* keptRoots) {
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   const float q = lane < n ? q0 : 0.f;
@@ -153,7 +158,7 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
   const u32 krRoot = __shfl_sync(0xFFFFFFFFu, keptC ? kr : kNoRank, root);
   if (lane < n) {
     ev.label[s + lane] = kept ? s + root : kInvalid;
-    ev.clus[s + lane] = (kept && krRoot != kNoRank) ? (int32_t)krRoot : -1;
+    ev.clus[s + lane] = (kept && krRoot != kNoRank) ? (int32_t)clus_ranked(krRoot, mFirst + mIdx) : -1;
   }
   *keptDigis = __ballot_sync(0xFFFFFFFFu, kept); *roots = __ballot_sync(0xFFFFFFFFu, isRoot); *keptRoots = kb;
 }
@@ -241,7 +246,7 @@ __device__ __forceinline__ u32 unit_module(const UnitBounds& bnd, u32 i) { retur
 
 template <bool kMedium>
 __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, const WmStore<kMedium>& wr, float q0, u32 rc0,
-                                            const UnitBounds& bnd, u32* nKeptDigis, u32* nRootsOut, u32 (&cntOut)[4]) {
+                                            u32 mFirst, const UnitBounds& bnd, u32* nKeptDigis, u32* nRootsOut, u32 (&cntOut)[4]) {
   typedef typename WmStore<kMedium>::idx_t idx_t;
   typedef typename WmStore<kMedium>::pair_t pair_t;
   constexpr u32 kNoIdx = WmStore<kMedium>::kNoIdx, kIdxMask = WmStore<kMedium>::kIdxMask, kPairShift = WmStore<kMedium>::kPairShift;
@@ -438,7 +443,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     if (wr.info[i] != kNoKey) {
       const u32 r = wr.L[i], kr = krAt[r];
       lab = s + r;
-      if (kr != kNoRank) cl = (int32_t)kr;
+      if (kr != kNoRank) cl = (int32_t)clus_ranked(kr, mFirst + unit_module(bnd, i));
     }
     ev.label[s + i] = lab; ev.clus[s + i] = cl;
   }
@@ -607,7 +612,7 @@ __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 
   for (u32 i = tid; i < nn; i += kT) {
     const u32 p = cx.parent[i];
     u32 lab = kInvalid; int32_t cl = -1;
-    if (p != kInvalid) { lab = s + p; cl = cx.knum[cx.perm[p]]; }
+    if (p != kInvalid) { lab = s + p; cl = cx.knum[cx.perm[p]]; if (cl >= 0) cl = (int32_t)clus_ranked((u32)cl, m); }
     ev.label[s + i] = lab;
     ev.clus[s + i] = cl;
   }
@@ -646,7 +651,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
         u32 nk, nr, cnts[4];
         const UnitBounds one = {{kNoBnd, kNoBnd, kNoBnd}};
-        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, one, &nk, &nr, cnts);
+        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, m, one, &nk, &nr, cnts);
         const u32 cnt = cnts[0];
         if (lane == 0) {
           ev.modCount[m] = cnt;
@@ -756,14 +761,14 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
           bnd.b[j] = k + 1u + j < k2 ? v - s : kNoBnd;
         }
         u32 nk, nr, cnts[4];
-        warp_module<false>(ev, g, s, n, wm_store_small(wr), q0, rc0, bnd, &nk, &nr, cnts);
+        warp_module<false>(ev, g, s, n, wm_store_small(wr), q0, rc0, m0 + k, bnd, &nk, &nr, cnts);
         accK += nk; accA += nr; accG += cnts[0] + cnts[1] + cnts[2] + cnts[3];
         if (lane < k2 - k) ev.modCount[m0 + k + lane] = lane == 0u ? cnts[0] : lane == 1u ? cnts[1] : lane == 2u ? cnts[2] : cnts[3];
         k = k2;
         continue;
       }
       u32 kd = 0, rb = 0, kb = 0;
-      if (n) warp_pack(ev, g, s, n, q0, rc0, mIdx, mStart, &kd, &rb, &kb);
+      if (n) warp_pack(ev, g, s, n, q0, rc0, m0 + k, mIdx, mStart, &kd, &rb, &kb);
       accK += (u32)__popc(kd); accA += (u32)__popc(rb); accG += (u32)__popc(kb);
       // kept clusters per module of the pack: lane j - k writes module j's
       {

@@ -8,42 +8,49 @@ namespace pixreco {
 // ================================================================== k_finalize (numbering of a4)
 // One CTA per (event, group of kFinMods consecutive modules): the group's first dense cluster
 // number is the sum of the kept-cluster counts of all earlier modules (at most 2048 values), so
-// no CTA depends on another.  Turns clus[] ranks into event-wide cluster numbers, converts the
+// no CTA depends on another.  Turns clus[] ranks (clus_ranked) into event-wide cluster numbers, converts the
 // staged sums into the cluster SoA (A9: binary64 division, one rounding to binary32) and the hit SoA (the step after
 // clustering in the paper's Fig. 1; A26-A30: position from the same exact sums, bounding box, border flags, error
 // estimate), writes modClusStart[]; the CTA of an event's last module group publishes that event's counters to mapped
 // pinned host memory.
-constexpr u32 kFinMods = 32;
+constexpr u32 kFinMods = 32;                     // modules per group of grpCount[] (k_cluster adds whole tickets to one group)
+constexpr u32 kFinMaxGroups = 4;                 // a CTA takes 1, 2 or 4 consecutive groups (launches with many units: less set-up per digi)
 static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
 template <bool kSingle>
 __global__ void __launch_bounds__(256)
 k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent, u32 splits,
-           LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
-  __shared__ u32 sStart[kFinMods + 1], sDigi[kFinMods + 1], sScan[8];
+           u32 groupsPerUnit, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+  __shared__ u32 sStart[kFinMods * kFinMaxGroups + 1], sDigi[kFinMods * kFinMaxGroups + 1], sScan[8], sTot[kFinMaxGroups];
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
-  // `splits` CTAs share one (event, group) when events are huge: slice sp of the group's digis and clusters
+  // `splits` CTAs share one unit when events are huge: slice sp of the unit's digis and clusters
   const u32 unit = blockIdx.x / splits, sp = blockIdx.x - unit * splits;
   const u32 e = unit / unitsPerEvent, u = unit - e * unitsPerEvent;
   const EvDesc& ev = kSingle ? single : batch[e];
-  const u32 m0 = u * kFinMods, m1 = min(m0 + kFinMods, M);
+  const u32 nMods = kFinMods * groupsPerUnit;
+  const u32 m0 = u * nMods, m1 = min(m0 + nMods, M), nm = m1 - m0;
   if (!(ev.counters->status & 1u)) {
     u32 sum = 0, base;
-    for (u32 k = tid; k < u; k += 256) sum += ev.grpCount[k];      // groups of kFinMods modules before this one
-    block_excl_scan(sum, sScan, &base);
-    if (warp == 0) {
-      const u32 c = m0 + lane < m1 ? ev.modCount[m0 + lane] : 0u;
-      const u32 incl = warp_incl_scan(c, lane);
-      sStart[lane] = base + incl - c;
-      if (lane == 31) sStart[32] = base + incl;
-      sDigi[lane] = ev.modDigiStart[min(m0 + lane, M)];
-      if (lane == 31) sDigi[32] = ev.modDigiStart[min(m0 + 32u, M)];
+    for (u32 k = tid; k < u * groupsPerUnit; k += 256) sum += ev.grpCount[k];      // the groups before this unit
+    u32 c = 0, incl = 0;
+    if (warp < groupsPerUnit) {                       // warp w scans the unit's group w
+      c = m0 + tid < m1 ? ev.modCount[m0 + tid] : 0u;
+      incl = warp_incl_scan(c, lane);
+      if (lane == 31) sTot[warp] = incl;
+    }
+    if (tid <= nMods) sDigi[tid] = ev.modDigiStart[min(m0 + tid, M)];
+    block_excl_scan(sum, sScan, &base);               // (two barriers: sTot is visible after it)
+    if (warp < groupsPerUnit) {
+      u32 off = base;
+      for (u32 w = 0; w < warp; ++w) off += sTot[w];
+      sStart[tid] = off + incl - c;
+      if (tid == nMods - 1u) sStart[nMods] = off + incl;
     }
     __syncthreads();
     if (sp == 0) {
       for (u32 m = m0 + tid; m < m1; m += 256) ev.modClusStart[m] = sStart[m - m0];
-      if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[32]; ev.counters->nClusters = sStart[32]; }
+      if (m1 == M && tid == 0) { ev.modClusStart[M] = sStart[nMods]; ev.counters->nClusters = sStart[nMods]; }
     }
-    const u32 d0 = sDigi[0], d1 = sDigi[m1 - m0];
+    const u32 d0 = sDigi[0], d1 = sDigi[nm];
     if (d0 <= d1 && d1 <= ev.cap) {
       for (u32 dd = d0 + sp * 1024u + tid; dd < d1; dd += splits * 1024u) {     // four independent digis per thread and trip
         int32_t c[4];
@@ -55,20 +62,16 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           if (c[k] < 0) continue;
-          // the digi's module within the group: the last one that starts at or before the digi (no read of module[])
-          const u32 d = dd + 256u * k;
-          u32 li = 0;
-#pragma unroll
-          for (u32 step = 16; step > 0; step >>= 1)
-            if (li + step < m1 - m0 && sDigi[li + step] <= d) li += step;
-          ev.clus[d] = (int32_t)(sStart[li] + (u32)c[k]);
+          // clus_ranked: rank among the module's kept clusters | the module's position among 128 << 20
+          const u32 d = dd + 256u * k, li = ((u32)c[k] >> 20) & (nMods - 1u);
+          ev.clus[d] = (int32_t)(sStart[li] + ((u32)c[k] & 0xFFFFFu));
         }
       }
-      for (u32 o = sStart[0] + sp * 256u + tid; o < sStart[32]; o += splits * 256u) {
+      for (u32 o = sStart[0] + sp * 256u + tid; o < sStart[nMods]; o += splits * 256u) {
         u32 li = 0;
 #pragma unroll
-        for (u32 step = 16; step > 0; step >>= 1)
-          if (li + step < kFinMods + 1 && sStart[li + step] <= o) li += step;   // last module with start <= o and a cluster there
+        for (u32 step = kFinMods * kFinMaxGroups / 2; step > 0; step >>= 1)
+          if (li + step < nMods + 1 && sStart[li + step] <= o) li += step;       // last module with start <= o and a cluster there
         const u32 src = sDigi[li] + (o - sStart[li]);
         if (o < ev.cap && src < ev.cap) {
           const double S = ev.stS[src];
@@ -101,7 +104,7 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     const u32 status = c->status;
     HostCounters h;
     h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
-    h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[32]; h.status = status; h.seq = 1;
+    h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[nMods]; h.status = status; h.seq = 1;
     h.tStart = lc->tStart; h.tEnd = global_timer();
     *ev.hostCounters = h;
     DevCounters r;                                   // device copy of the final counters: k_export takes its sizes from it
