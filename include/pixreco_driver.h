@@ -26,7 +26,8 @@ typedef struct {
 
 /* Run `n_events` events: event e takes input pool[(first + e) % n_pool], slot e % n_slots and stream e % n_slots
  * (A25); a slot is acquired again only after its previous event was produced and released.  Thread t of `n_threads`
- * drives the slots s with s % n_threads == t.  t_start_ns / t_end_ns (may be NULL, else [n_events]) receive the
+ * drives the slots s with s % n_threads == t, each slot through its own sequence of events (s, s + n_slots, ...), serving
+ * whichever of its slots has completed (polling pr_produce): no slot waits for another slot's event.  t_start_ns / t_end_ns (may be NULL, else [n_events]) receive the
  * device time stamps of every event (pr_output.t_start_ns / t_end_ns).  `want` and `mem_kind` come with the inputs.
  * Returns res->status.                                                                                            */
 int prd_run_streams(pr_event* const* slots, void* const* streams, uint32_t n_slots,

@@ -32,44 +32,56 @@ extern "C" int prd_run_streams_rec(pr_event* const* slots, void* const* streams,
   std::vector<clk::time_point> tBegin(n_threads), tEnd(n_threads);
 
   auto worker = [&](uint32_t t) {
-    std::vector<int64_t> inFlight(n_slots, -1);               // event in flight on the slots this thread drives
+    // Every slot runs its own sequence of events (s, s + n_slots, s + 2 n_slots, ...: A25) and is served as soon as it
+    // is ready: the thread goes round its slots, takes the product of a slot whose event has completed (pr_produce
+    // answers PR_NOT_READY otherwise: a poll, never a wait), releases it and issues the slot's next event.  No slot
+    // waits for another slot's event.
+    std::vector<int64_t> inFlight(n_slots, -1), next(n_slots, -1);
+    uint32_t mine = 0, open = 0;
+    for (uint32_t s = t; s < n_slots; s += n_threads) { next[s] = s < n_events ? (int64_t)s : -1; ++mine; if (next[s] >= 0) ++open; }
     acqUs[t].reserve(n_events / n_threads + 8);
     pr_output out;
-    auto finish = [&](uint32_t s) -> bool {
-      int r;
-      while ((r = pr_produce(slots[s], &out)) == PR_NOT_READY) ++polls[t];
-      if (r != PR_OK) { int ok = PR_OK; status.compare_exchange_strong(ok, r); return false; }
-      const int64_t e = inFlight[s];
-      digis[t] += out.n_digis; clusters[t] += out.n_clusters; ++done[t];
-      if (t_start_ns) t_start_ns[e] = out.t_start_ns;
-      if (t_end_ns) t_end_ns[e] = out.t_end_ns;
-      if (rec) {
-        prd_event_record& q = rec[e];
-        q.event_id = out.event_id; q.n_digis = out.n_digis; q.n_errors = out.n_errors; q.n_kept_digis = out.n_kept_digis;
-        q.n_clusters_all = out.n_clusters_all; q.n_clusters = out.n_clusters; q.status_bits = out.status_bits;
-        q.thread = t;
-        q.hash_label = out.h_label ? fnv1a32(out.h_label, out.n_digis) : 0;
-        q.hash_cl_label = out.h_cl_label ? fnv1a32(out.h_cl_label, out.n_clusters) : 0;
-      }
-      while ((r = pr_release(slots[s])) == PR_NOT_READY) {}
-      inFlight[s] = -1;
-      return r == PR_OK;
-    };
+    bool failed = false;
+    auto fail = [&](int r) { int ok = PR_OK; status.compare_exchange_strong(ok, r); failed = true; };
     ready.fetch_add(1);
     while (!go.load(std::memory_order_acquire)) {}
     tBegin[t] = clk::now();
-    for (uint32_t e = 0; e < n_events && status.load(std::memory_order_relaxed) == PR_OK; ++e) {
-      const uint32_t s = e % n_slots;
-      if (s % n_threads != t) continue;
-      if (inFlight[s] >= 0 && !finish(s)) break;
-      const auto a0 = clk::now();
-      const int r = pr_acquire(slots[s], pool + (first + e) % n_pool, streams[s]);
-      acqUs[t].push_back((float)us_since(a0));
-      if (r != PR_OK) { int ok = PR_OK; status.compare_exchange_strong(ok, r); break; }
-      inFlight[s] = e;
+    while (open && !failed && status.load(std::memory_order_relaxed) == PR_OK) {
+      for (uint32_t s = t; s < n_slots && !failed; s += n_threads) {
+        if (inFlight[s] >= 0) {
+          const int r = pr_produce(slots[s], &out);
+          if (r == PR_NOT_READY) { ++polls[t]; continue; }
+          if (r != PR_OK) { fail(r); break; }
+          const int64_t e = inFlight[s];
+          digis[t] += out.n_digis; clusters[t] += out.n_clusters; ++done[t];
+          if (t_start_ns) t_start_ns[e] = out.t_start_ns;
+          if (t_end_ns) t_end_ns[e] = out.t_end_ns;
+          if (rec) {
+            prd_event_record& q = rec[e];
+            q.event_id = out.event_id; q.n_digis = out.n_digis; q.n_errors = out.n_errors; q.n_kept_digis = out.n_kept_digis;
+            q.n_clusters_all = out.n_clusters_all; q.n_clusters = out.n_clusters; q.status_bits = out.status_bits;
+            q.thread = t;
+            q.hash_label = out.h_label ? fnv1a32(out.h_label, out.n_digis) : 0;
+            q.hash_cl_label = out.h_cl_label ? fnv1a32(out.h_cl_label, out.n_clusters) : 0;
+          }
+          int rr;
+          while ((rr = pr_release(slots[s])) == PR_NOT_READY) {}
+          if (rr != PR_OK) { fail(rr); break; }
+          inFlight[s] = -1;
+          if (next[s] < 0) --open;
+        }
+        if (inFlight[s] < 0 && next[s] >= 0) {
+          const int64_t e = next[s];
+          const auto a0 = clk::now();
+          const int r = pr_acquire(slots[s], pool + (first + e) % n_pool, streams[s]);
+          acqUs[t].push_back((float)us_since(a0));
+          if (r != PR_OK) { fail(r); break; }
+          inFlight[s] = e;
+          next[s] = e + n_slots < n_events ? e + n_slots : -1;
+        }
+      }
     }
-    for (uint32_t s = t; s < n_slots; s += n_threads)
-      if (inFlight[s] >= 0) finish(s);
+    (void)mine;
     tEnd[t] = clk::now();
   };
 
