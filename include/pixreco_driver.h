@@ -50,6 +50,23 @@ int prd_run_streams_rec(pr_event* const* slots, void* const* streams, uint32_t n
                         const pr_input* pool, uint32_t n_pool, uint32_t first, uint32_t n_events, uint32_t n_threads,
                         uint64_t* t_start_ns, uint64_t* t_end_ns, prd_event_record* rec, prd_result* res);
 
+/* The consumer of the transfer stage: a "legacy" CPU module that wants one record per
+ * cluster (array of structures) instead of the library's structure of arrays.  It reads the pinned-host mirrors of a
+ * produced event — so the event must have been acquired with PR_WANT_CLUSTERS (| PR_WANT_HITS), or those must have
+ * been fetched after the fact with pr_transfer — and writes min(n_clusters, cap) records into dst (host memory of the
+ * caller).  Returns the number of records written, or PR_ERR_INVALID_ARG (NULL arguments) / PR_ERR_BAD_STATE (the
+ * cluster mirrors are not there).  Hit fields are zero when the hit mirrors are absent.  Pure host code.          */
+typedef struct {
+  uint32_t label;                 /* canonical label = minimum digi index of the cluster (A10)                      */
+  uint32_t size;
+  uint16_t module, flags;         /* flags: hit border bits (A29)                                                   */
+  float charge, row, col;         /* electrons; charge-weighted centroid in pixel units (A13)                       */
+  float x_um, y_um, xerr_um, yerr_um;   /* hit position and error estimate (A26, A27, A30)                          */
+  uint16_t row_min, row_max, col_min, col_max;   /* bounding box (A28)                                              */
+} prd_cluster_aos;
+
+int prd_clusters_to_aos(const pr_output* out, prd_cluster_aos* dst, uint32_t cap);
+
 #ifdef __cplusplus
 }
 #endif

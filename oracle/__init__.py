@@ -49,6 +49,7 @@ def _load():
         _lib.po_decode.restype = None
         _lib.po_calibrate.restype = None
         _lib.po_occupancy.restype = None
+        _lib.po_bucket.restype = None
     return _lib
 
 
@@ -264,6 +265,27 @@ def run(words, adc, n_modules, gain, pedestal, pixel_threshold_e=1000.0, cluster
                   ew[:E], ei[:E], ws.mds, q[:D], ws.kept[:D], label[:D], cll[:N], clm[:N], cls[:N], clq[:N],
                   clr[:N], clc[:N], ws.clus[:D], ws.mcs, hx[:N], hy[:N], hxe[:N], hye[:N], hr[:N], hc[:N],
                   ws.hit_flags[:N])
+
+
+def bucket(words, adc, n_modules, n_rows=160, n_cols=416):
+    """O0 (A31): stable bucket sort of the words by module (error / invalid words last).  Returns (words, adc, orig)."""
+    words = np.ascontiguousarray(words, np.uint32)
+    adc = np.ascontiguousarray(adc, np.uint16)
+    W = words.shape[0]
+    ow, oa, orig = np.zeros(W, np.uint32), np.zeros(W, np.uint16), np.zeros(W, np.uint32)
+    _load().po_bucket(_p(words), _p(adc), _u32(W), _u32(n_modules), _u32(n_rows), _u32(n_cols), _p(ow), _p(oa), _p(orig))
+    return ow, oa, orig
+
+
+def run_unordered(words, adc, n_modules, gain, pedestal, pixel_threshold_e=1000.0, cluster_threshold_e=4000.0,
+                  n_rows=160, n_cols=416, pitch_row_um=PITCH_ROW_UM, pitch_col_um=PITCH_COL_UM) -> Result:
+    """The chain for words in arbitrary order (A31): O0 bucket, then O1..O5 on the bucketed stream, with word_idx and
+    err_idx mapped back to the positions of the words in the INPUT."""
+    ow, oa, orig = bucket(words, adc, n_modules, n_rows, n_cols)
+    r = run(ow, oa, n_modules, gain, pedestal, pixel_threshold_e, cluster_threshold_e, n_rows, n_cols, pitch_row_um, pitch_col_um)
+    r.word_idx = orig[r.word_idx]
+    r.err_idx = orig[r.err_idx]
+    return r
 
 
 def check_exact_sums(label, charge, col) -> int:

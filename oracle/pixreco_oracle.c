@@ -21,7 +21,8 @@
  * round trip, closed-form calibration values and the float64 single-rounding identity, exhaustive
  * 4x4 occupancy patterns against an O(n^2) transitive closure, scipy.ndimage.label /
  * sum_labels / center_of_mass, networkx components for duplicate pixels, special shapes,
- * permutation invariance, worked reduce example; for hits: worked values, closed forms (single
+ * permutation invariance, worked reduce example; for the bucket step: a worked example, numpy's stable argsort,
+ * identity on grouped input; for hits: worked values, closed forms (single
  * pixel, strips, centred and translated clusters), numpy min/max and scipy.ndimage.center_of_mass.  Against the PAPER there is nothing to pin:
  * it prints no value for this path ("parity unpinned" with respect to the paper).
  *
@@ -262,6 +263,33 @@ void po_occupancy(uint32_t D, uint32_t M, const uint16_t *d_module, const uint16
   for (uint32_t m = 0; m < M; ++m) { occ_count[m] = 0; occ_adc_sum[m] = 0; }
   for (uint32_t d = 0; d < D; ++d)
     if (kept[d]) { occ_count[d_module[d]] += 1; occ_adc_sum[d_module[d]] += d_adc[d]; }
+}
+
+/* ---- O0 bucket by module (reading A31; arbitrary word order) ----
+ * The step BEFORE decode when the words of an event come in arbitrary order: a STABLE bucket sort of the words by
+ * module.  Key of word i = its module if it is a digi word (bit 31 clear, module < M, row < R, col < C: the test of
+ * O1), else M (error and invalid words form one last bucket).  out_* receive the words and ADC values in key order,
+ * equal keys in their input order; orig[p] = input index of the word now at position p.  Decoding the bucketed
+ * stream (O1) then yields the digi list "by module, input order inside a module" and the error list in input order;
+ * word indices are mapped back to input positions through orig[] by the caller (oracle.run_unordered).
+ * Plain counting sort: count, prefix, place.                                                                       */
+void po_bucket(const uint32_t *words, const uint16_t *adc, uint32_t W, uint32_t M, uint32_t R, uint32_t C,
+               uint32_t *out_words, uint16_t *out_adc, uint32_t *orig) {
+  uint32_t *start = (uint32_t *)calloc((size_t)M + 2, sizeof(uint32_t));
+  if (!start) return;
+  for (uint32_t i = 0; i < W; ++i) {
+    uint32_t w = words[i], mod = (w >> 20) & 0x7FFu, row = (w >> 12) & 0xFFu, col = (w >> 3) & 0x1FFu;
+    uint32_t key = ((w >> 31) || mod >= M || row >= R || col >= C) ? M : mod;
+    start[key + 1] += 1;
+  }
+  for (uint32_t k = 0; k <= M; ++k) start[k + 1] += start[k];     /* start[k] = number of words with key < k */
+  for (uint32_t i = 0; i < W; ++i) {
+    uint32_t w = words[i], mod = (w >> 20) & 0x7FFu, row = (w >> 12) & 0xFFu, col = (w >> 3) & 0x1FFu;
+    uint32_t key = ((w >> 31) || mod >= M || row >= R || col >= C) ? M : mod;
+    uint32_t p = start[key]++;
+    out_words[p] = w; out_adc[p] = adc[i]; orig[p] = i;
+  }
+  free(start);
 }
 
 /* ---- the whole chain, in order O1..O5 (what bench.py's cpu_baseline times) ----

@@ -118,3 +118,24 @@ extern "C" int prd_run_streams(pr_event* const* slots, void* const* streams, uin
                                uint64_t* t_start_ns, uint64_t* t_end_ns, prd_result* res) {
   return prd_run_streams_rec(slots, streams, n_slots, pool, n_pool, first, n_events, n_threads, t_start_ns, t_end_ns, nullptr, res);
 }
+
+extern "C" int prd_clusters_to_aos(const pr_output* out, prd_cluster_aos* dst, uint32_t cap) {
+  if (!out || (!dst && cap)) return PR_ERR_INVALID_ARG;
+  const uint32_t n = out->n_clusters < cap ? out->n_clusters : cap;
+  if (n && !(out->h_cl_label && out->h_cl_size && out->h_cl_module && out->h_cl_charge && out->h_cl_row && out->h_cl_col))
+    return PR_ERR_BAD_STATE;
+  const bool hits = out->h_ht_x && out->h_ht_y && out->h_ht_xerr && out->h_ht_yerr && out->h_ht_rows && out->h_ht_cols && out->h_ht_flags;
+  for (uint32_t k = 0; k < n; ++k) {
+    prd_cluster_aos r{};
+    r.label = out->h_cl_label[k]; r.size = out->h_cl_size[k]; r.module = out->h_cl_module[k];
+    r.charge = out->h_cl_charge[k]; r.row = out->h_cl_row[k]; r.col = out->h_cl_col[k];
+    if (hits) {
+      r.flags = out->h_ht_flags[k];
+      r.x_um = out->h_ht_x[k]; r.y_um = out->h_ht_y[k]; r.xerr_um = out->h_ht_xerr[k]; r.yerr_um = out->h_ht_yerr[k];
+      r.row_min = (uint16_t)(out->h_ht_rows[k] & 0xFFFFu); r.row_max = (uint16_t)(out->h_ht_rows[k] >> 16);
+      r.col_min = (uint16_t)(out->h_ht_cols[k] & 0xFFFFu); r.col_max = (uint16_t)(out->h_ht_cols[k] >> 16);
+    }
+    dst[k] = r;
+  }
+  return (int)n;
+}

@@ -160,7 +160,20 @@ class prd_event_record(ctypes.Structure):
                 ("pad", c_uint32), ("hash_label", c_uint64), ("hash_cl_label", c_uint64)]
 
 
+class prd_cluster_aos(ctypes.Structure):
+    _fields_ = [("label", c_uint32), ("size", c_uint32), ("module", ctypes.c_uint16), ("flags", ctypes.c_uint16),
+                ("charge", c_float), ("row", c_float), ("col", c_float), ("x_um", c_float), ("y_um", c_float),
+                ("xerr_um", c_float), ("yerr_um", c_float), ("row_min", ctypes.c_uint16), ("row_max", ctypes.c_uint16),
+                ("col_min", ctypes.c_uint16), ("col_max", ctypes.c_uint16)]
+
+
+AOS_DTYPE = np.dtype([("label", "<u4"), ("size", "<u4"), ("module", "<u2"), ("flags", "<u2"), ("charge", "<f4"), ("row", "<f4"),
+                      ("col", "<f4"), ("x_um", "<f4"), ("y_um", "<f4"), ("xerr_um", "<f4"), ("yerr_um", "<f4"),
+                      ("row_min", "<u2"), ("row_max", "<u2"), ("col_min", "<u2"), ("col_max", "<u2")])
+
+
 DRIVER_SIGNATURES = {
+    "prd_clusters_to_aos": (c_int, [POINTER(pr_output), c_void_p, c_uint32]),
     "prd_run_streams": (c_int, [POINTER(c_void_p), POINTER(c_void_p), c_uint32, POINTER(pr_input), c_uint32, c_uint32, c_uint32,
                                 c_uint32, c_void_p, c_void_p, POINTER(prd_result)]),
     "prd_run_streams_rec": (c_int, [POINTER(c_void_p), POINTER(c_void_p), c_uint32, POINTER(pr_input), c_uint32, c_uint32,
@@ -211,6 +224,18 @@ def run_streams(slots, streams, inputs, n_events, n_threads=1, first=0, spans=Fa
     if records:
         out["records"] = rec
     return out
+
+
+def clusters_to_aos(out: "Output") -> np.ndarray:
+    """The legacy consumer of the transfer stage: one record per cluster (numpy structured array, AOS_DTYPE) from the
+    pinned-host mirrors of a produced event (prd_clusters_to_aos)."""
+    n = out.n_clusters
+    dst = np.zeros(n, AOS_DTYPE)
+    assert dst.itemsize == ctypes.sizeof(prd_cluster_aos)
+    rc = driver().prd_clusters_to_aos(ctypes.byref(out.raw), dst.ctypes.data if n else None, n)
+    if rc < 0:
+        raise PixRecoError(rc, "prd_clusters_to_aos")
+    return dst[:rc]
 
 
 class PixRecoError(RuntimeError):

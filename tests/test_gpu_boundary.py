@@ -319,3 +319,33 @@ def test_argument_and_state_errors(pr):
         assert slot.produce()[0] == 0
         slot.release()
         slot.destroy()
+
+
+def test_legacy_aos_consumer_of_the_transfer_stage(pr):
+    """P:L112-114 / SURVEY 8(f) NEXT-1, the consumer half: a CPU module that wants one record per cluster turns up after
+    the event was produced without mirrors; pr_transfer fetches the cluster and hit tables (a stage of its own), and
+    prd_clusters_to_aos turns the structure of arrays into an array of structures on the host — compared with the oracle."""
+    cal = wl.make_calib(1)
+    ev = wl.make_event(1, 11)
+    r = oracle.run(ev.words, ev.adc, ev.n_modules, cal.gain, cal.pedestal)
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(ev.words), to_dev(ev.adc), stream=torch.cuda.Stream(), want=0)
+        wait(slot)
+        code, out = slot.produce()
+        assert code == 0 and out.host("cl_label") is None
+        assert lib_code(lambda: pr.clusters_to_aos(out)) == pr.PR_ERR_BAD_STATE      # no mirrors yet: nothing to convert
+        slot.transfer(pr.PR_WANT_CLUSTERS | pr.PR_WANT_HITS, stream=torch.cuda.Stream())
+        wait(slot)
+        code, out = slot.produce()
+        assert code == 0
+        aos = pr.clusters_to_aos(out)
+        assert len(aos) == r.n_clusters > 1000
+        assert np.array_equal(aos["label"], r.cl_label) and np.array_equal(aos["size"], r.cl_size)
+        assert np.array_equal(aos["module"], r.cl_module) and np.array_equal(aos["flags"], r.ht_flags)
+        for f, ref in (("charge", r.cl_charge), ("row", r.cl_row), ("col", r.cl_col), ("x_um", r.ht_x), ("y_um", r.ht_y),
+                       ("xerr_um", r.ht_xerr), ("yerr_um", r.ht_yerr)):
+            assert np.array_equal(aos[f].view(np.uint32), ref.view(np.uint32)), f
+        assert np.array_equal(aos["row_min"], r.ht_rows & 0xFFFF) and np.array_equal(aos["row_max"], r.ht_rows >> 16)
+        assert np.array_equal(aos["col_min"], r.ht_cols & 0xFFFF) and np.array_equal(aos["col_max"], r.ht_cols >> 16)
+        slot.release()
