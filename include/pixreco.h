@@ -117,6 +117,14 @@ typedef struct {
                                       at once.  Tiles are handed out by ticket, so a tile only ever waits for tiles of
                                       CTAs that are already running: the launch must end all the same    */
 
+#define PR_FLAG_UNORDERED_INPUT 0x8u /* the words of an event may come in ANY order (reading A31; the step before the decode in
+                                      the paper's Fig. 1): pr_acquire / pr_acquire_batch first bucket them
+                                      stably by module on the device (error and out-of-range words last), then run the
+                                      chain on the bucketed stream.  The digi list is then "by module, input order inside
+                                      a module", the error list in input order, word_idx / err_idx are positions in the
+                                      INPUT.  Costs three more launches and ~10 bytes per word of slab; the chained
+                                      modules (pr_digis_acquire) answer PR_ERR_INVALID_ARG on such a handle           */
+
 typedef struct {                  /* one event's input, filled by the caller before pr_acquire    */
   const uint32_t* words;          /* [n_words] raw words; caller-owned, valid until completion    */
   const uint16_t* adc;            /* [n_words] parallel ADC values (<= 4095)                      */

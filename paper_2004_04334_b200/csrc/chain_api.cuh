@@ -84,6 +84,7 @@ int pr_digis_acquire(pr_event* ev, const pr_input* in, void* cuda_stream) {
   pr_handle* h = ev->h;
   if (h->sticky.load()) return PR_ERR_CUDA;
   if (ev->state != kIdle) return PR_ERR_BAD_STATE;
+  if (h->cfg.flags & PR_FLAG_UNORDERED_INPUT) return PR_ERR_INVALID_ARG;                       // A31 is built into pr_acquire* only
   const uint32_t M = h->cfg.n_modules, kind = in->mem_kind, want = in->want;
   if (kind != PR_MEM_HOST_PINNED && kind != PR_MEM_DEVICE) return PR_ERR_INVALID_ARG;
   if (want & ~(PR_WANT_DIGIS | PR_WANT_CHARGE | PR_WANT_ERRORS)) return PR_ERR_INVALID_ARG;   // this module makes nothing else

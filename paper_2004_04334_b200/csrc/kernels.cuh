@@ -4,14 +4,16 @@
 //              single-pass decoupled look-back scan, modDigiStart, input-order check; TMA bulk
 //              loads into a shared-memory ring, staged SoA output written by TMA bulk stores; tiles
 //              handed out by an atomic ticket.
-//   k_cluster  a3+a4+hits fused, one CTA per unit of consecutive modules, one thread per digi:
-//              shared-memory hash + min-index union-find, exact cluster sums by 32-bit limb
-//              reductions, cluster threshold, EVENT-WIDE numbering by a look-back over the units,
-//              cluster and hit tables, counters to the host.  One pass, nothing re-read.
-//   k_dense    the same for launches whose modules are large on average: one module per CTA,
+//   k_cluster  a3+a4 fused: a warp clusters a unit of up to four small modules (register packs up to 32 digis;
+//              column lists + reduced edge set + label equivalence on a byte forest up to 256; one warp with its
+//              large arrays in the global workspace up to 1024), exact cluster sums and bounding boxes, cluster
+//              threshold, numbering inside the module; a whole CTA (bitmap + union-find) beyond.
+//   k_finalize event-wide numbering, cluster table, hit table, counters to the host.
+//   k_dense    the dense path for launches whose modules are large on average: one module per CTA,
 //              occupancy bitmap + popcount ranks + union-find, larger shared-memory tiers.
 //   k_export   exact-size copies of requested outputs into mapped pinned host memory.
 //   k_publish_digis / k_import_digis / k_occupancy   the seams of the chained modules (k_chain.cuh).
+//   k_bucket / k_bucket_scan / k_unbucket_idx   words in arbitrary order: stable bucket sort by module first (A31).
 //
 // Kernels are batch-capable: a launch processes nEv independent events described by EvDesc
 // records (one Run-3-like event is ~1000x too small to fill a B200).  The single-event path
@@ -26,3 +28,4 @@
 #include "k_cluster.cuh"
 #include "k_finalize.cuh"
 #include "k_chain.cuh"
+#include "k_bucket.cuh"

@@ -162,6 +162,11 @@ void carve_clusters(Carver& c, EvDesc& d, uint32_t cap, uint32_t M) {
   d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
   d.wsS = c.take<u64>(cap); d.wsSx = c.take<u64>(cap); d.wsSy = c.take<u64>(cap); d.wsBox = c.take<u32>((size_t)cap * 4);
 }
+// ... and the bucketed copy of the input for words in arbitrary order (A31; k_bucket.cuh)
+void carve_bucket(Carver& c, BucketDesc& b, uint32_t cap, uint32_t M, uint32_t nTiles) {
+  b.dstW = c.take<u32>(cap); b.dstA = c.take<u16>(cap); b.orig = c.take<u32>(cap);
+  b.hist = c.take<u32>((size_t)(M + 1) * nTiles);
+}
 void carve_device(Carver& c, EvDesc& d, uint32_t cap, uint32_t M, bool stage, uint32_t** stageWords, uint16_t** stageAdc) {
   carve_digis(c, d, cap, M, stage, stageWords, stageAdc);
   carve_clusters(c, d, cap, M);
@@ -339,6 +344,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   }
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const bool stage = kind == PR_MEM_HOST_PINNED;
+  const bool unordered = (h->cfg.flags & PR_FLAG_UNORDERED_INPUT) != 0;      // A31: bucket the words by module first
 
   // ---- host inputs of a batch that lie in ONE pinned block of the handle's pool and form a nearly dense span per array (a
   // DAQ buffer from pr_host_alloc, the bench's pool) are staged by ONE copy per array, each event keeping its offset
@@ -375,11 +381,12 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     s.cap = (uint32_t)align_up(s.in.n_words ? s.in.n_words : 1, 8);
     Carver cd(nullptr); EvDesc tmp{}; uint32_t* sw; uint16_t* sa;
     carve_device(cd, tmp, s.cap, M, stage && !merged, &sw, &sa);
-    devBytes += cd.off;
-    if (want) { Carver ch(nullptr); pr_output o{}; carve_host(ch, o, want, s.cap, M); hostBytes += ch.off; }
     s.desc = EvDesc{};
     s.desc.tileBase = totalTiles;
     s.desc.nTiles = s.in.n_words ? (s.in.n_words + kTileWords - 1) / kTileWords : 1;
+    if (unordered) { BucketDesc b{}; carve_bucket(cd, b, s.cap, M, s.desc.nTiles); }
+    devBytes += cd.off;
+    if (want) { Carver ch(nullptr); pr_output o{}; carve_host(ch, o, want, s.cap, M); hostBytes += ch.off; }
     totalTiles += s.desc.nTiles;
     totalWords += s.in.n_words;
   }
@@ -393,7 +400,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // rounded up to a power of two, at least 8) — the whole class must stay on the warp-ticket path
   uint32_t tilesClass = 8;
   while (tilesClass < totalTiles) tilesClass <<= 1;
-  const bool useGraph = n == 1 && !stage && want == 0 && !h->timing && !h->noGraph && ev->capStream &&
+  const bool useGraph = n == 1 && !stage && want == 0 && !h->timing && !h->noGraph && !unordered && ev->capStream &&
                         (uint64_t)tilesClass * kTileWords <= (uint64_t)kWarpCap * M && tilesClass <= 4096;
   const size_t ctlNeed = ctlZero + (size_t)8 * (useGraph ? tilesClass : totalTiles);
 
@@ -429,6 +436,16 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     if (!ev->descStage || !ev->descDev) { release_blocks(ev, true); return PR_ERR_OOM; }
   }
 
+  BucketDesc* bkHost = nullptr; BucketDesc* bkDev = nullptr;
+  const size_t bkBytes = unordered ? sizeof(BucketDesc) * n + align_up(sizeof(u16) * totalTiles, 16) : 0;
+  if (unordered) {
+    bkHost = (BucketDesc*)h->hostPool->alloc(bkBytes, stream);
+    bkDev = (BucketDesc*)h->devPool->alloc(bkBytes, stream);
+    if (bkHost) ev->extraHost.push_back(bkHost);
+    if (bkDev) ev->extraDev.push_back(bkDev);
+    if (!bkHost || !bkDev) { release_blocks(ev, true); return PR_ERR_OOM; }
+  }
+
   // ---- carve
   char* ctl = (char*)ev->ctl;
   LaunchCtl* lc = (LaunchCtl*)ctl;
@@ -450,6 +467,16 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     d.words = stage ? ev->stW[k] : s.in.words;
     d.adc = stage ? ev->stA[k] : s.in.adc;
     d.nWords = s.in.n_words; d.cap = s.cap;
+    if (unordered) {                               // k_unpack reads the bucketed stream
+      BucketDesc& b = bkHost[k];
+      b = BucketDesc{};
+      carve_bucket(cd, b, s.cap, M, d.nTiles);
+      b.srcW = d.words; b.srcA = d.adc; b.wordIdx = d.wordIdx; b.errIdx = d.errIdx; b.counters = counters + k;
+      b.nWords = d.nWords; b.nTiles = d.nTiles; b.tileBase = d.tileBase;
+      d.words = b.dstW; d.adc = b.dstA;
+      u16* te = (u16*)(bkHost + n);
+      for (uint32_t t = 0; t < d.nTiles; ++t) te[d.tileBase + t] = (u16)k;
+    }
     d.counters = counters + k; d.hostCounters = ev->hostCounters + k;
     d.tileState = tileState + d.tileBase;
     d.grpCount = grpCount + grpPerEv * k;
@@ -548,6 +575,15 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     ++nMemcpy;
   }
   if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[0], stream));
+  if (unordered) {
+    PR_CUDA_Q(ev, cudaMemcpyAsync(bkDev, bkHost, bkBytes, cudaMemcpyHostToDevice, stream));
+    ++nMemcpy;
+    const u16* te = (const u16*)(bkDev + n);
+    k_bucket<false><<<totalTiles, kBucketThreads, 0, stream>>>(bkDev, te, h->geom);
+    k_bucket_scan<<<n, 1024, 0, stream>>>(bkDev, h->geom);
+    k_bucket<true><<<totalTiles, kBucketThreads, 0, stream>>>(bkDev, te, h->geom);
+    nLaunch += 3;
+  }
   const EvDesc& d0 = ev->sub[0].desc;
   if (n == 1) {
     k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, nullptr, nullptr, totalTiles, pro, lc, tileState, h->geom);
@@ -566,6 +602,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
     k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(d0, dd, n, unitsPerEvent, finSplits, finGroupsPerUnit, lc, h->geom);
   }
   nLaunch += denseKernel ? 4 : 3;
+  if (unordered) {                                 // wordIdx / errIdx: positions in the input, not in the bucketed stream
+    uint32_t gx = (uint32_t)((totalWords / n + 1023) / 1024);
+    if (gx < 1) gx = 1;
+    if (gx > 256) gx = 256;
+    k_unbucket_idx<<<dim3(gx, n), 256, 0, stream>>>(bkDev);
+    ++nLaunch;
+  }
   PR_CUDA_Q(ev, cudaGetLastError());
   if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[3], stream));
   ev->exported = want != 0;
@@ -690,7 +733,7 @@ int pr_create(const pr_config* cfg, pr_handle** out) {
   *out = nullptr;
   if (!cfg || cfg->struct_size != sizeof(pr_config)) return PR_ERR_INVALID_ARG;
   if (cfg->n_modules < 1 || cfg->n_modules > 2048 || cfg->n_rows < 1 || cfg->n_rows > 256 || cfg->n_cols < 1 ||
-      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~(PR_FLAG_KERNEL_TIMING | PR_FLAG_NO_GRAPH | PR_FLAG_UNPACK_OVERSUBSCRIBE)))
+      cfg->n_cols > 512 || !cfg->gain || !cfg->pedestal || (cfg->flags & ~(PR_FLAG_KERNEL_TIMING | PR_FLAG_NO_GRAPH | PR_FLAG_UNPACK_OVERSUBSCRIBE | PR_FLAG_UNORDERED_INPUT)))
     return PR_ERR_INVALID_ARG;
   // A9/A21: ranges that make the 2^-14 fixed-point sums exact and overflow-free
   if (!(cfg->pixel_threshold_e >= 512.0f) || !std::isfinite(cfg->pixel_threshold_e) ||

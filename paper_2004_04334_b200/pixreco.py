@@ -29,7 +29,7 @@ PR_WANT_ALL = 63
 PR_STATUS_INPUT_ORDER, PR_STATUS_CAPACITY = 1, 2
 PR_POOL_DEVICE, PR_POOL_PINNED, PR_POOL_FAKE = 0, 1, 2
 PR_INVALID_LABEL = 0xFFFFFFFF
-PR_FLAG_KERNEL_TIMING, PR_FLAG_NO_GRAPH, PR_FLAG_UNPACK_OVERSUBSCRIBE = 1, 2, 4
+PR_FLAG_KERNEL_TIMING, PR_FLAG_NO_GRAPH, PR_FLAG_UNPACK_OVERSUBSCRIBE, PR_FLAG_UNORDERED_INPUT = 1, 2, 4, 8
 
 pr_done_fn = ctypes.CFUNCTYPE(None, c_void_p, c_int)
 

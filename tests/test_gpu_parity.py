@@ -392,3 +392,56 @@ def test_module_size_boundaries(pr, sizes, dup):
     cal = wl.Calib(rng.uniform(60, 100, M).astype(np.float32), rng.normal(0, 200, M).astype(np.float32), 1000.0, 4000.0)
     out, got = run_device(pr, ev, cal)
     compare(out, oracle_of(ev, cal), lambda f: got[f])
+
+
+@pytest.mark.parametrize("config,event,batch", [(0, 0, 1), (1, 3, 1), (3, 2, 1), (1, 20, 5)])
+def test_words_in_arbitrary_order_are_bucketed_by_module_on_the_device(pr, config, event, batch):
+    """A31 (PR_FLAG_UNORDERED_INPUT; the step before the decode in the paper's Fig. 1): every word of the event at a
+    random place.  The device buckets the words stably by module, then runs the chain; every output equals the oracle's
+    bucket step followed by its unchanged chain, word and error indices pointing into the shuffled INPUT.  Without the
+    flag the same input ends with PR_ERR_INPUT_ORDER."""
+    cal = wl.make_calib(config)
+    rng = np.random.default_rng(100 + config)
+    evs = []
+    for k in range(batch):
+        ev = wl.make_event(config, event + k)
+        perm = rng.permutation(ev.n_words)
+        evs.append(wl.Event(ev.words[perm].copy(), ev.adc[perm].copy(), ev.n_modules))
+    if batch > 1:
+        evs[2] = wl.Event(np.zeros(0, np.uint32), np.zeros(0, np.uint16), evs[0].n_modules)        # an empty event inside the batch
+    refs = [oracle.run_unordered(e.words, e.adc, e.n_modules, cal.gain, cal.pedestal) for e in evs]
+    with pr.PixReco(cal.gain, cal.pedestal, flags=pr.PR_FLAG_UNORDERED_INPUT) as p:
+        slot = p.slot()
+        for kind in ("device", "host"):
+            if kind == "device":
+                ins = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+            else:
+                ins = []
+                for e in evs:
+                    hw, ha = p.host_array(max(e.n_words, 1), np.uint32)[:e.n_words], p.host_array(max(e.n_words, 1), np.uint16)[:e.n_words]
+                    hw[:], ha[:] = e.words, e.adc
+                    ins.append((hw, ha))
+            slot.acquire_batch(ins, stream=torch.cuda.Stream(), want=pr.PR_WANT_ALL if kind == "host" else 0)
+            wait(slot)
+            code, outs = slot.produce_batch(len(evs))
+            assert code == 0
+            for out, ref in zip(outs, refs):
+                getter = (lambda f, o=out: o.host(f)) if kind == "host" else (lambda f, o=out: o.to_numpy(f))
+                compare(out, ref, getter)
+            slot.release()
+        assert lib_code_of(pr, lambda: slot.digis_acquire(to_dev(evs[0].words), to_dev(evs[0].adc))) == pr.PR_ERR_INVALID_ARG
+    if config == 1 and batch == 1:
+        with pr.PixReco(cal.gain, cal.pedestal) as p:                       # the ordered contract (A5) still holds without the flag
+            slot = p.slot()
+            slot.acquire(to_dev(evs[0].words), to_dev(evs[0].adc), stream=torch.cuda.Stream())
+            wait(slot)
+            code, _ = slot.produce(raise_on_error=False)
+            assert code == pr.PR_ERR_INPUT_ORDER
+            slot.release()
+
+
+def lib_code_of(pr, fn):
+    try:
+        return fn()
+    except pr.PixRecoError as e:
+        return e.code
