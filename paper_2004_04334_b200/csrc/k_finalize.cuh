@@ -17,7 +17,7 @@ constexpr u32 kFinMods = 32;                     // modules per group of grpCoun
 constexpr u32 kFinMaxGroups = 4;                 // a CTA takes 1, 2 or 4 consecutive groups (launches with many units: less set-up per digi)
 static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
 template <bool kSingle>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 8)
 k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent, u32 splits,
            u32 groupsPerUnit, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
   __shared__ u32 sStart[kFinMods * kFinMaxGroups + 1], sDigi[kFinMods * kFinMaxGroups + 1], sScan[8], sTot[kFinMaxGroups];
@@ -52,15 +52,15 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     }
     const u32 d0 = sDigi[0], d1 = sDigi[nm];
     if (d0 <= d1 && d1 <= ev.cap) {
-      for (u32 dd = d0 + sp * 1024u + tid; dd < d1; dd += splits * 1024u) {     // four independent digis per thread and trip
-        int32_t c[4];
+      for (u32 dd = d0 + sp * 2048u + tid; dd < d1; dd += splits * 2048u) {     // eight independent digis per thread and trip
+        int32_t c[8];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < 8; ++k) {
           const u32 d = dd + 256u * k;
           c[k] = d < d1 ? ev.clus[d] : -1;
         }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < 8; ++k) {
           if (c[k] < 0) continue;
           // clus_ranked: rank among the module's kept clusters | the module's position among 128 << 20
           const u32 d = dd + 256u * k, li = ((u32)c[k] >> 20) & (nMods - 1u);
