@@ -136,6 +136,7 @@ int pr_digis_acquire(pr_event* ev, const pr_input* in, void* cuda_stream) {
   // ---- enqueue: clear the control words, stage the input, unpack, close the product
   uint64_t nMemcpy = 0, nLaunch = 0;
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, fresh ? ev->ctlBytes : ctlZero, stream));
+  ev->ctlDirty = true;
   if (stage && in->n_words) {
     PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stW[0], in->words, (size_t)in->n_words * 4, cudaMemcpyHostToDevice, stream));
     PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stA[0], in->adc, (size_t)in->n_words * 2, cudaMemcpyHostToDevice, stream));
@@ -145,7 +146,7 @@ int pr_digis_acquire(pr_event* ev, const pr_input* in, void* cuda_stream) {
   if (unpackGrid > nTiles) unpackGrid = nTiles;
   uint32_t pro = (nTiles + unpackGrid - 1) / unpackGrid;
   if (pro >= 4) pro = 7;
-  k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, nTiles, pro, lc, d.tileState, h->geom);
+  k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d, nullptr, nullptr, nTiles, pro, lc, d.tileState, h->geom, nullptr);
   k_publish_digis<<<1, 32, 0, stream>>>(d, lc);
   nLaunch += 2;
   if (want) {
@@ -232,6 +233,7 @@ int pr_clusters_acquire(pr_event* ev, pr_product* p, uint32_t want, void* own_st
 
   uint64_t nMemcpy = 0, nLaunch = 0;
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, fresh ? ev->ctlBytes : ctlZero, stream));
+  ev->ctlDirty = true;
   const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
   const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
   const uint32_t modBatch = (uint64_t)M >= 4 * warpsResident ? kModBatch : (uint64_t)M >= 2 * warpsResident ? 2u : 1u;
@@ -247,7 +249,7 @@ int pr_clusters_acquire(pr_event* ev, pr_product* p, uint32_t want, void* own_st
   k_import_digis<<<1, 32, 0, stream>>>(d.counters, p->desc.result, lc);
   k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d, nullptr, 1, lc, bigList, modBatch, h->geom);
   if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d, nullptr, lc, bigList, h->geom);
-  k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, 1u, lc, h->geom);
+  k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d, nullptr, 1, unitsPerEvent, finSplits, 1u, lc, h->geom, 0u);
   nLaunch += denseKernel ? 4 : 3;
   if (want) {
     std::vector<ExportItem>& items = ev->items;

@@ -19,7 +19,7 @@ static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 mod
 template <bool kSingle>
 __global__ void __launch_bounds__(256, 8)
 k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, u32 nEv, u32 unitsPerEvent, u32 splits,
-           u32 groupsPerUnit, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g) {
+           u32 groupsPerUnit, LaunchCtl* __restrict__ lc, const __grid_constant__ Geom g, u32 selfClean) {
   __shared__ u32 sStart[kFinMods * kFinMaxGroups + 1], sDigi[kFinMods * kFinMaxGroups + 1], sScan[8], sTot[kFinMaxGroups];
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, M = g.M;
   // `splits` CTAs share one unit when events are huge: slice sp of the unit's digis and clusters
@@ -112,7 +112,24 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     r.nClusters = h.nClusters; r.status = status; r.pad = 0;
     *ev.result = r;
   }
+  // selfClean (a slot's graph, one event): the last CTA to leave puts the zeros back into the words that the next
+  // launch of the graph expects cleared — the module ticket, the event's counters and group counts — so that the graph
+  // needs no memset node (k_unpack does the same for its ticket and its look-back states).
+  if (selfClean) {
+    __shared__ u32 sLast;
+    __syncthreads();
+    if (tid == 0) { __threadfence(); sLast = atomicAdd(&lc->modDone, 1u) == gridDim.x - 1u ? 1u : 0u; }
+    __syncthreads();
+    if (sLast) {
+      __threadfence();
+      u32* c = reinterpret_cast<u32*>(ev.counters);
+      if (tid < sizeof(DevCounters) / 4u) c[tid] = 0u;
+      for (u32 k = tid; k < (M + kFinMods - 1u) / kFinMods; k += 256u) ev.grpCount[k] = 0u;
+      if (tid == 0) { lc->modTicket = 0u; lc->modDone = 0u; }
+    }
+  }
 }
+
 
 // ================================================================== k_export
 // Exact-size copies of requested outputs to mapped pinned host memory (transfers only

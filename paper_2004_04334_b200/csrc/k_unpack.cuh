@@ -89,13 +89,17 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 template <bool kSingle>
 __global__ void __launch_bounds__(kUnpackThreads + 64, kUnpackCtasPerSM)
 k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch, const u16* __restrict__ tileEvent,
-         u32 totalTiles, u32 pro, LaunchCtl* __restrict__ lc, u64* __restrict__ tileStateAll, const __grid_constant__ Geom g) {
+         u32 totalTiles, u32 pro, LaunchCtl* __restrict__ lc, u64* __restrict__ tileStateAll, const __grid_constant__ Geom g,
+         const EvDesc* __restrict__ hostDesc) {
   extern __shared__ __align__(128) unsigned char unpackSmem[];
   UnpackShared& sh = *reinterpret_cast<UnpackShared*>(unpackSmem);
   const u32 tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, lt = (1u << lane) - 1u;
   // a launch replayed from a CUDA graph does not know its size when it is recorded: a one-event launch then reads it
   // from the event's descriptor
-  if (!kSingle && totalTiles == kTilesFromDesc) totalTiles = batch[0].nTiles;
+  // hostDesc (a slot's graph): the one event's descriptor lies in mapped pinned HOST memory and is read from there (no
+  // copy node in the graph); the CTA that draws ticket 0 leaves a device copy in batch[0] for the kernels that follow
+  const EvDesc* descs = (!kSingle && hostDesc) ? hostDesc : batch;
+  if (!kSingle && totalTiles == kTilesFromDesc) totalTiles = descs[0].nTiles;
   const bool ctl = warp == 8u, scn = warp == 9u;             // warps 0..7 work on words; warp 8 drives the TMA and draws the tickets; warp 9 publishes and looks back
   const u32 limM = g.M, limR = g.R << 12, limC = g.C << 3;
   auto desc_of = [&](int k) -> const EvDesc& {
@@ -139,7 +143,9 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   }
   __syncthreads();
   if (!kSingle && (int)warp < kDrawAhead && tile_of((int)warp) < totalTiles)
-    sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(batch + tileEvent[tile_of((int)warp)]) + lane);
+    sh.desc[warp][lane] = __ldg(reinterpret_cast<const u32*>(descs + tileEvent[tile_of((int)warp)]) + lane);
+  if (!kSingle && hostDesc && tile_of(0) == 0u && tid < sizeof(EvDesc) / 4u)
+    reinterpret_cast<u32*>(const_cast<EvDesc*>(batch))[tid] = reinterpret_cast<const u32*>(hostDesc)[tid];
   // control warp: tiles in flight, whether a draw came back empty, the ticket drawn in the previous iteration and its event
   u32 inflight = 0, tktP = kTileSkip, eP = 0;
   bool ended = false;
@@ -161,7 +167,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     if (ctl) {
       // a new ticket (it becomes local tile i + kDrawAhead); the descriptor of the one drawn an iteration ago
       if (!ended && inflight < pro && lane == 0) tkt = atomicAdd(&lc->tileTicket, 1u);
-      if (!kSingle && tktP < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(batch + eP) + lane);
+      if (!kSingle && tktP < totalTiles) dword = __ldg(reinterpret_cast<const u32*>(descs + eP) + lane);
       if (lane == 0 && i > 0) bulk_wait_read();               // the staging arrays are free again
     } else if (!scn && vc) {
       // ---- count: local tile i + kCountAhead

@@ -86,6 +86,7 @@ struct pr_event {
   std::vector<uint32_t*> stW; std::vector<uint16_t*> stA; std::vector<ExportItem> items;   // per-acquire scratch, kept
   // per-acquire pool blocks
   void* devSlab = nullptr; void* hostSlab = nullptr; void* descStage = nullptr; void* descDev = nullptr;
+  bool ctlDirty = false;                    // the control block holds the counters of an acquire that ran outside the slot's graph
   // persistent per-slot blocks (grown on demand).  Control block: [LaunchCtl | counters | group counts | big-module list]
   // zeroed by one small memset per acquire, then [look-back states of k_unpack], which k_unpack's last CTA puts back
   // to zero itself (so that part is cleared only when the block is (re)allocated).
@@ -306,12 +307,15 @@ int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc
   PR_CUDA(h, cudaMemsetAsync(ev->gDescDev, 0, descBytes, stream));
   cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamBeginCapture");
-  cudaMemsetAsync(ev->ctl, 0, ctlZero, cs);
+  // no memset node: the kernels leave the control words zeroed behind them (k_unpack: tile ticket and look-back states;
+  // k_finalize with selfClean: module ticket, counters, group counts).  The descriptor travels by a copy node: reading it
+  // from the slot's mapped pinned block inside k_unpack (hostDesc) put two PCIe round trips at the head of the chain and
+  // was 2 us slower per event than the copy node
   cudaMemcpyAsync(ev->gDescDev, ev->gDescHost, sizeof(EvDesc), cudaMemcpyHostToDevice, cs);
   EvDesc none{};
-  k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), cs>>>(none, dd, tileEvent, kTilesFromDesc, pro, lc, tileState, h->geom);
+  k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), cs>>>(none, dd, tileEvent, kTilesFromDesc, pro, lc, tileState, h->geom, nullptr);
   k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, cs>>>(none, dd, 1, lc, nullptr, modBatch, h->geom);
-  k_finalize<false><<<unitsPerEvent * finSplits, 256, 0, cs>>>(none, dd, 1, unitsPerEvent, finSplits, 1u, lc, h->geom);
+  k_finalize<false><<<unitsPerEvent * finSplits, 256, 0, cs>>>(none, dd, 1, unitsPerEvent, finSplits, 1u, lc, h->geom, 1u);
   cudaEventRecordWithFlags(ev->done, cs, cudaEventRecordExternal);   // an event-record NODE: ev->done stays an ordinary event the host can query
   e = cudaStreamEndCapture(cs, &graph);
   if (e != cudaSuccess || !graph) { cudaGetLastError(); return cuda_fail(h, e, "cudaStreamEndCapture"); }
@@ -488,7 +492,9 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // ---- enqueue (all asynchronous, one stream: P:L82).  From here on a failure goes through fail_after_enqueue.
   uint64_t nMemcpy = 0, nLaunch = 0;
   if (useGraph) {
-    if (ctlFresh) PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ev->ctlBytes, stream));     // a new control block: look-back states too
+    // a new control block (look-back states too), or one that an acquire outside the graph left with its counters in it
+    if (ctlFresh || ev->ctlDirty) PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ctlFresh ? ev->ctlBytes : ctlZero, stream));
+    ev->ctlDirty = false;
     if (!ev->gExec || ev->gCtl != ev->ctl || ev->gTilesClass != tilesClass || ev->gCtlZero != ctlZero) {
       int rc = build_graph(ev, tilesClass, ctlZero, lc, tileState, stream);
       if (rc != PR_OK) return fail_after_enqueue(ev, rc);
@@ -501,6 +507,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // tickets, counters, group counts: one small memset; the look-back states only when the block is new (k_unpack's last
   // CTA puts their zeros back, and those of its two ticket words, harmlessly cleared again here)
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ctlFresh ? ev->ctlBytes : ctlZero, stream));
+  ev->ctlDirty = true;                             // (only the slot's graph leaves the control words zeroed behind it)
   if (merged) {
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
@@ -586,20 +593,20 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   }
   const EvDesc& d0 = ev->sub[0].desc;
   if (n == 1) {
-    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, nullptr, nullptr, totalTiles, pro, lc, tileState, h->geom);
+    k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, nullptr, nullptr, totalTiles, pro, lc, tileState, h->geom, nullptr);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
     k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, nullptr, 1, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<true><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d0, nullptr, lc, bigList, h->geom);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d0, nullptr, 1, unitsPerEvent, finSplits, finGroupsPerUnit, lc, h->geom);
+    k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, stream>>>(d0, nullptr, 1, unitsPerEvent, finSplits, finGroupsPerUnit, lc, h->geom, 0u);
   } else {
     const EvDesc* dd = (const EvDesc*)ev->descDev;
-    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, dd, (const u16*)(dd + n), totalTiles, pro, lc, tileState, h->geom);
+    k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), stream>>>(d0, dd, (const u16*)(dd + n), totalTiles, pro, lc, tileState, h->geom, nullptr);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[1], stream));
     k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, stream>>>(d0, dd, n, lc, bigList, modBatch, h->geom);
     if (denseKernel) k_dense<false><<<denseGrid, kDenseThreads, h->denseSmem, stream>>>(d0, dd, lc, bigList, h->geom);
     if (h->timing) PR_CUDA_Q(ev, cudaEventRecord(ev->tev[2], stream));
-    k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(d0, dd, n, unitsPerEvent, finSplits, finGroupsPerUnit, lc, h->geom);
+    k_finalize<false><<<n * unitsPerEvent * finSplits, 256, 0, stream>>>(d0, dd, n, unitsPerEvent, finSplits, finGroupsPerUnit, lc, h->geom, 0u);
   }
   nLaunch += denseKernel ? 4 : 3;
   if (unordered) {                                 // wordIdx / errIdx: positions in the input, not in the bucketed stream
