@@ -27,7 +27,7 @@ constexpr u32 kWarpCap = 256;                    // warp path: modules with at m
 constexpr u32 kMediumCap = 1024;                 // one warp with its large arrays in the global workspace: up to this many digis
 constexpr u32 kWarpScratch = 6144 - kWarpCap * (4 + 4 + 1 + 1 + 1 + 2);   // 2816 bytes
 constexpr u32 kAccRoots = kWarpScratch / 36;     // 78 clusters accumulated per pass over a module
-constexpr u32 kModBatch = 4;                     // most modules per warp ticket (small tickets: a short tail; 8 was 6 % slower, 16 17 %);
+constexpr u32 kModBatch = 8;                     // most modules per warp ticket (two units of four Run-3-like modules; tickets of 4: 3 % slower there, 1 % on the high pile-up batch);
                                                  // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
 constexpr u32 kNoKey = 0xFFFFFFFFu;
 constexpr u32 kNoRank = 0xFFFFu;
@@ -701,11 +701,11 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   }
   if (__any_sync(0xFFFFFFFFu, medBits != 0u)) medium_modules(base0, medBits);
 
-  // ---- phase 2: warp path.  A ticket is a batch of modBatch (1, 2 or 4) consecutive modules of one event.
-  // Tickets shrink towards the end of a large launch (modBatch 4): the first nEvA events are handed out four
+  // ---- phase 2: warp path.  A ticket is a batch of modBatch (1, 2 or kModBatch = 8) consecutive modules of one event.
+  // Tickets shrink towards the end of a large launch (modBatch 8): the first nEvA events are handed out eight
   // modules at a time, the next nEvB events two at a time, the rest one by one, so that the last tickets are short.
   const u32 bpe = (M + modBatch - 1) / modBatch, bpeB = (M + 1u) / 2u;
-  const u32 nEvA = modBatch == 4u ? nEv - nEv / 4u : nEv, nEvB = modBatch == 4u ? (nEv - nEvA + 1u) / 2u : 0u;
+  const u32 nEvA = modBatch == kModBatch ? nEv - nEv / 4u : nEv, nEvB = modBatch == kModBatch ? (nEv - nEvA + 1u) / 2u : 0u;
   const u32 tA = nEvA * bpe, tB = tA + nEvB * bpeB, nTickets = tB + (nEv - nEvA - nEvB) * M;
   for (;;) {
     u32 t = 0;
@@ -748,6 +748,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
       while (k2 < nm) {
         const u32 en = __shfl_sync(0xFFFFFFFFu, st, k2 + 1u);
         if (en < e2 || en > ev.cap || en - s > kWarpCap) break;
+        if (k2 - k >= 4u && en - s > 32u) break;              // at most four modules in a unit of the shared-memory path (eight: spills, 5 % slower)
         if (e2 - s <= lane) { mIdx = k2 - k; mStart = e2; }   // module k2 starts at e2 (what a pack of at most 32 digis needs)
         e2 = en; ++k2;
       }
