@@ -378,16 +378,19 @@ def _blob_module(rng, m, n, dup_frac=0.0, box=40):
     ([17, 100, 256, 250, 257, 600, 20, 20], 0.15),
     ([3] * 700, 0.0),                                    # hundreds of modules per 512-digi window
     ([3000, 5, 40, 300, 9000, 0, 700, 33, 8192, 8193], 0.1),   # large on average: the large ones go to k_dense (both of its tiers)
+    # both sides of the single-warp path's upper end (1024 digis) and of the dense path's shared-memory tier (2048), next to
+    # runs of small modules that share a unit (at most four) and a ticket
+    ([1023, 1024, 1025, 1500, 2048, 2049, 200, 100, 100, 100, 100] + [30] * 9 + [1, 0, 255, 2, 60, 60, 60, 60, 60, 7], 0.05),
 ])
 def test_module_size_boundaries(pr, sizes, dup):
-    """Modules on both sides of every path boundary of k_cluster (warp path up to 256 digis, dense
-    path beyond, two dense modules in one window, windows with hundreds of tiny modules)."""
+    """Modules on both sides of every path boundary of k_cluster (register packs up to 32 digis, units of up to four
+    modules and 256 digis, one warp with global arrays up to 1024, the CTA-wide dense path beyond and its tiers)."""
     rng = np.random.default_rng(len(sizes) * 1000 + int(dup * 100))
     M = len(sizes) + 3
     pix = []
     for m, n in enumerate(sizes):
         if n:
-            pix += _blob_module(rng, m + 1, n, dup, box=12 if n <= 64 else 40)
+            pix += _blob_module(rng, m + 1, n, dup, box=12 if n <= 64 else 40 if n <= 1500 else 64)
     ev = hand(pix, M)
     cal = wl.Calib(rng.uniform(60, 100, M).astype(np.float32), rng.normal(0, 200, M).astype(np.float32), 1000.0, 4000.0)
     out, got = run_device(pr, ev, cal)
