@@ -524,28 +524,41 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
   __syncthreads();
   // P4: unions with the backward neighbours (W, NW, N, NE), decision tree:
   //     N ? {N} : { NE?, W ? {W} : NW? }   — spans every 8-adjacency once all pixels did it.
-  for (u32 i = tid; i < nn; i += kT) {
-    if (parent[i] == kInvalid) continue;
-    const u32 prow = ev.row[s + i] + 1u, b = ev.col[s + i] + 1u;
-    const u32 wd = prow * stride + (b >> 5);
-    const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
-    const u32 owner = perm[r];
-    if (owner != i) { uf_union(parent, i, owner); continue; }
-    const u32 pos = b - 1u, w0 = pos >> 5, shf = pos & 31u;
-    const u32 rowAbove = (prow - 1u) * stride, rowSelf = prow * stride;
-    const u32 nb = __funnelshift_r(smBitmap[rowAbove + w0], smBitmap[rowAbove + w0 + 1], shf) & 7u;
-    const u32 cb = __funnelshift_r(smBitmap[rowSelf + w0], smBitmap[rowSelf + w0 + 1], shf) & 7u;
-    auto owner_at = [&](u32 rowBase, u32 bb) -> u32 {
-      const u32 ww = rowBase + (bb >> 5);
-      return perm[smPrefix[ww] + __popc(smBitmap[ww] & ((1u << (bb & 31)) - 1u))];
-    };
-    if (nb & 2u) {
-      uf_union(parent, i, owner_at(rowAbove, b));
-    } else {
-      if (nb & 4u) uf_union(parent, i, owner_at(rowAbove, b + 1u));
-      if (cb & 1u) uf_union(parent, i, owner_at(rowSelf, b - 1u));
-      else if (nb & 1u) uf_union(parent, i, owner_at(rowAbove, b - 1u));
+  // A thread first finds its (at most two) partners — where to look is a different place in every branch of the tree, what
+  // to do with them is not: the unions then run with all the threads that have one side by side.
+  for (u32 i0 = 0; i0 < nn; i0 += kT) {
+    const u32 i = i0 + tid;
+    u32 e1 = kInvalid, e2 = kInvalid;
+    if (i < nn && parent[i] != kInvalid) {
+      const u32 prow = ev.row[s + i] + 1u, b = ev.col[s + i] + 1u;
+      const u32 wd = prow * stride + (b >> 5);
+      const u32 r = smPrefix[wd] + __popc(smBitmap[wd] & ((1u << (b & 31)) - 1u));
+      const u32 owner = perm[r];
+      if (owner != i) e1 = owner;
+      else {
+        const u32 pos = b - 1u, w0 = pos >> 5, shf = pos & 31u;
+        const u32 rowAbove = (prow - 1u) * stride, rowSelf = prow * stride;
+        const u32 nb = __funnelshift_r(smBitmap[rowAbove + w0], smBitmap[rowAbove + w0 + 1], shf) & 7u;
+        const u32 cb = __funnelshift_r(smBitmap[rowSelf + w0], smBitmap[rowSelf + w0 + 1], shf) & 7u;
+        // pixel 1 (bit offset from b - 1 in the row above: 0 = NW, 1 = N, 2 = NE; in the own row: 0 = W) and pixel 2
+        u32 p1 = kInvalid, p2 = kInvalid;               // rowBase << 16 | padded column
+        if (nb & 2u) p1 = rowAbove << 16 | b;
+        else {
+          if (nb & 4u) p1 = rowAbove << 16 | (b + 1u);
+          if (cb & 1u) p2 = rowSelf << 16 | (b - 1u);
+          else if (nb & 1u) p2 = rowAbove << 16 | (b - 1u);
+        }
+        if (p1 == kInvalid) { p1 = p2; p2 = kInvalid; }
+        auto owner_at = [&](u32 p) -> u32 {
+          const u32 bb = p & 0xFFFFu, ww = (p >> 16) + (bb >> 5);
+          return perm[smPrefix[ww] + __popc(smBitmap[ww] & ((1u << (bb & 31)) - 1u))];
+        };
+        if (p1 != kInvalid) e1 = owner_at(p1);
+        if (p2 != kInvalid) e2 = owner_at(p2);
+      }
     }
+    if (e1 != kInvalid) uf_union(parent, i, e1);
+    if (e2 != kInvalid) uf_union(parent, i, e2);
   }
   __syncthreads();
   // P5: flatten (roots are stable now)
