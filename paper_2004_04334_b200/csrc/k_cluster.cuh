@@ -53,32 +53,51 @@ __host__ __device__ inline size_t cluster_smem_bytes(u32 bitmapWords) {
   return ((dense > warp ? dense : warp) + 15) & ~(size_t)15;
 }
 
+// The union-find forest of the dense path lives in shared memory (modules up to the shared tier) or in the global
+// workspace.  ParentRef names it with its address space known at compile time: volatile loads and stores of shared
+// memory proper (a generic volatile load goes through the global-memory path and waits on the long scoreboard).
+template <bool kShared> struct ParentRef {
+  u32* p;
+  __device__ __forceinline__ u32 ld(u32 i) const {
+    u32 v;
+    if (kShared) asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"((u32)__cvta_generic_to_shared(p + i)) : "memory");
+    else v = *reinterpret_cast<volatile u32*>(p + i);
+    return v;
+  }
+  __device__ __forceinline__ void st(u32 i, u32 v) const {
+    if (kShared) asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"((u32)__cvta_generic_to_shared(p + i)), "r"(v) : "memory");
+    else *reinterpret_cast<volatile u32*>(p + i) = v;
+  }
+};
 // Root of x, halving the path on the way (a node's parent only ever moves to another ancestor in its set, so
 // concurrent finds and hooks stay consistent).  Only while unions are running: see uf_root.
-__device__ __forceinline__ u32 uf_find(volatile u32* parent, u32 x) {
-  u32 p = parent[x];
+template <bool kShared>
+__device__ __forceinline__ u32 uf_find(ParentRef<kShared> parent, u32 x) {
+  u32 p = parent.ld(x);
   while (p != x) {
-    const u32 gp = parent[p];
-    if (gp != p) parent[x] = gp;
+    const u32 gp = parent.ld(p);
+    if (gp != p) parent.st(x, gp);
     x = p; p = gp;
   }
   return x;
 }
 // Root of x without touching the forest: for the flattening pass, where a late halving store could
 // overwrite another thread's final root.
-__device__ __forceinline__ u32 uf_root(const volatile u32* parent, u32 x) {
+template <bool kShared>
+__device__ __forceinline__ u32 uf_root(ParentRef<kShared> parent, u32 x) {
   u32 p;
-  while ((p = parent[x]) != x) x = p;
+  while ((p = parent.ld(x)) != x) x = p;
   return x;
 }
 // Hook the larger root under the smaller one (atomicMin), so the final root of every set is its
 // minimum digi index = the canonical label (A10).
-__device__ __forceinline__ void uf_union(u32* parent, u32 a, u32 b) {
+template <bool kShared>
+__device__ __forceinline__ void uf_union(ParentRef<kShared> parent, u32 a, u32 b) {
   for (;;) {
     a = uf_find(parent, a); b = uf_find(parent, b);
     if (a == b) return;
     if (a < b) { u32 t = a; a = b; b = t; }
-    const u32 old = atomicMin(parent + a, b);
+    const u32 old = atomicMin(parent.p + a, b);
     if (old == a) return;
     a = old;
   }
@@ -557,14 +576,19 @@ __device__ __forceinline__ void dense_count(const EvDesc& ev, const Geom& g, u32
         if (p2 != kInvalid) e2 = owner_at(p2);
       }
     }
-    if (e1 != kInvalid) uf_union(parent, i, e1);
-    if (e2 != kInvalid) uf_union(parent, i, e2);
+    if (digiInSmem) {
+      if (e1 != kInvalid) uf_union(ParentRef<true>{parent}, i, e1);
+      if (e2 != kInvalid) uf_union(ParentRef<true>{parent}, i, e2);
+    } else {
+      if (e1 != kInvalid) uf_union(ParentRef<false>{parent}, i, e1);
+      if (e2 != kInvalid) uf_union(ParentRef<false>{parent}, i, e2);
+    }
   }
   __syncthreads();
   // P5: flatten (roots are stable now)
   for (u32 i = tid; i < nn; i += kT) {
     if (parent[i] == kInvalid) continue;
-    const u32 rt = uf_root(parent, i);
+    const u32 rt = digiInSmem ? uf_root(ParentRef<true>{parent}, i) : uf_root(ParentRef<false>{parent}, i);
     if (rt != i) parent[i] = rt;
   }
   __syncthreads();
