@@ -191,15 +191,16 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
 //       the list of the column before (NW, W, SW).  Of these backward neighbours (column-major order) at most two
 //       edges are kept:  W ? {W} : { N ? N : NW,  SW }  — the dropped ones are adjacent to a kept one and are found from
 //       there, so the kept edges span every 8-adjacency.  A digi that shares its pixel with one of lower index keeps
-//       only the edge to that one.  Round 1 of the label equivalence is taken at once (labels = identity): the
-//       larger end of an edge is put under the smaller one.
-//   P3  label equivalence on the forest L[] (L[i] <= i, a digi of i's component; a root has L[i] == i): an edge
-//       whose ends have different roots hooks the larger root under the smaller one with a plain store (only while
-//       it still is a root: a tree is never split; of several lanes hooking one root in the same instruction one
-//       wins, the others find their edge unresolved in the next round) and stays on the list of unresolved edges; an
-//       edge whose ends share their root is resolved for good.  The first round looks at every edge, the following
-//       ones only at the list, until it is empty.  Roots only ever go under smaller roots: the final root of a
-//       component is its minimum digi index = the canonical label (A10).
+//       only the edge to that one.  Round 1 of the label equivalence is taken at once (labels = identity), in the
+//       digi's own slot: L[i] = min(i, its kept neighbours).
+//   P3  label equivalence on the forest L[] (L[i] <= i, a digi of i's component; a root has L[i] == i).  A kept edge
+//       that became its digi's link in P2 is resolved by construction; all the others go on the list of unresolved
+//       edges.  A round looks at the list: an edge whose ends have different roots hooks the larger root under the
+//       smaller one with a plain store (only while it still is a root: a tree is never split; of several lanes
+//       hooking one root in the same instruction one wins, the others find their edge unresolved in the next round)
+//       and stays on the list; an edge whose ends share their root is resolved for good and leaves it.  Until the list
+//       is empty.  Roots only ever go under smaller roots: the final root of a component is its minimum digi index =
+//       the canonical label (A10).
 //   P4  flatten; rank of every root in ascending index (= label) order.
 //   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory (exact: at most 256 terms below
 //       2^43), size and bounding box, kAccRoots clusters per pass: the lanes of a 32-digi chunk that share a cluster
@@ -321,26 +322,17 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
         if (e1 == kNoIdx) { e1 = SW != kNoIdx ? SW : i; }
         else if (SW != kNoIdx) e2 = SW;
       }
-      if (e1 != i) { const u32 hi = max(i, e1), lo = min(i, e1); if (wr.L[hi] > lo) wr.L[hi] = (idx_t)lo; }
-      if (e2 != i) { const u32 hi = max(i, e2), lo = min(i, e2); if (wr.L[hi] > lo) wr.L[hi] = (idx_t)lo; }
+      wr.L[i] = (idx_t)min(i, min(e1, e2));        // round 1 of the label equivalence (labels = identity), own slot only
     }
     if (!kMedium || i < n) wr.edge[i] = (pair_t)(e1 | e2 << kPairShift);
   }
   __syncwarp();
-  // P3: first every edge, then the unresolved ones
+  // P3: an edge that became its digi's link in P2 is resolved by construction; all the others start on the list
   u32 nAct = 0;
   for (u32 i = lane; i < nPad; i += 32u) {
     const u32 ed = (!kMedium || i < n) ? (u32)wr.edge[i] : (i | i << kPairShift), e1 = ed & kIdxMask, e2 = ed >> kPairShift;
-    bool u1 = false, u2 = false;
-    if (e1 != i) {
-      const u32 a = wm_find(wr.L, i), b = wm_find(wr.L, e1);
-      wr.L[i] = (idx_t)a;                   // (a root stays one; otherwise a shorter path for the finds to come)
-      if (a != b) { u1 = true; wm_hook(wr.L, a, b); }
-      if (e2 != i) {
-        const u32 b2 = wm_find(wr.L, e2);
-        if (a != b2) { u2 = true; wm_hook(wr.L, a, b2); }
-      }
-    }
+    const u32 li = wr.L[i];
+    const bool u1 = e1 != i && e1 != li, u2 = e2 != i && e2 != li;
     const u32 b1 = __ballot_sync(0xFFFFFFFFu, u1);
     if (u1) active[nAct + __popc(b1 & lt)] = (pair_t)(i | e1 << kPairShift);
     nAct += __popc(b1);
