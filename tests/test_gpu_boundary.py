@@ -349,3 +349,42 @@ def test_legacy_aos_consumer_of_the_transfer_stage(pr):
         assert np.array_equal(aos["row_min"], r.ht_rows & 0xFFFF) and np.array_equal(aos["row_max"], r.ht_rows >> 16)
         assert np.array_equal(aos["col_min"], r.ht_cols & 0xFFFF) and np.array_equal(aos["col_max"], r.ht_cols >> 16)
         slot.release()
+
+
+def test_a_slot_may_alternate_between_its_graph_and_plain_launches(pr):
+    """The slot's CUDA graph (device input, no mirrors) has no memset node: its kernels leave the control words zeroed
+    behind them.  An acquire outside the graph (mirrors wanted, a batch, a chained module) leaves its counters in the
+    control block; the next graph launch must not see them.  Every step is compared with the oracle."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, 30 + k) for k in range(4)]
+    refs = [oracle.run(e.words, e.adc, e.n_modules, cal.gain, cal.pedestal) for e in evs]
+    dev = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        stream = torch.cuda.Stream()
+
+        def check(out, r):
+            assert (out.n_digis, out.n_errors, out.n_kept_digis, out.n_clusters_all, out.n_clusters, out.status_bits) == \
+                (r.n_digis, r.n_errors, r.n_kept_digis, r.n_clusters_all, r.n_clusters, 0)
+            assert np.array_equal(out.to_numpy("clus"), r.clus) and np.array_equal(out.to_numpy("cl_label"), r.cl_label)
+        plan = ["graph", "graph", "mirrors", "graph", "batch", "graph", "chain", "graph", "graph"]
+        for step, kind in enumerate(plan):
+            k = step % 4
+            if kind == "batch":
+                slot.acquire_batch([dev[k], dev[(k + 1) % 4]], stream=stream)
+                wait(slot)
+                code, outs = slot.produce_batch(2)
+                assert code == 0
+                check(outs[0], refs[k]); check(outs[1], refs[(k + 1) % 4])
+            elif kind == "chain":
+                slot.digis_acquire(*dev[k], stream=stream)
+                wait(slot)
+                code, out = slot.produce()
+                assert code == 0 and out.n_digis == refs[k].n_digis
+            else:
+                slot.acquire(*dev[k], stream=stream, want=pr.PR_WANT_LABELS if kind == "mirrors" else 0)
+                wait(slot)
+                code, out = slot.produce()
+                assert code == 0
+                check(out, refs[k])
+            slot.release()
