@@ -448,3 +448,35 @@ def lib_code_of(pr, fn):
         return fn()
     except pr.PixRecoError as e:
         return e.code
+
+
+def test_a_module_beyond_the_exact_sum_limit_is_reported_not_truncated(pr):
+    """A9: the exact int64 sums are overflow-free up to 2^17 - 1 digis per module.  A module with 2^17 digis (every pixel
+    of the module twice, minus a few) must end with PR_ERR_CAPACITY / PR_STATUS_CAPACITY — never a silently wrong answer
+    (SURVEY 8(b) "Capacity") — the other modules of the event are clustered as usual, and the slot stays usable."""
+    M, R, C = 4, 160, 416
+    n_big = 1 << 17
+    rng = np.random.default_rng(17)
+    cells = np.concatenate([np.arange(R * C), rng.permutation(R * C)[: n_big - R * C]]).astype(np.uint32)
+    rng.shuffle(cells)
+    big = (np.uint32(2) << 20) | ((cells // C) << 12) | ((cells % C) << 3)
+    small_pix = [(1, 10, 10, 200), (1, 10, 11, 200), (1, 50, 50, 200), (3, 7, 7, 200)]
+    small = wl.event_from_pixels(small_pix, M)
+    m1 = small.words[(small.words >> 20) == 1]; m3 = small.words[(small.words >> 20) == 3]
+    words = np.concatenate([m1, big.astype(np.uint32), m3]).astype(np.uint32)
+    adc = np.full(words.shape[0], 200, np.uint16)
+    cal = wl.flat_calib(M)
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slot = p.slot()
+        slot.acquire(to_dev(words), to_dev(adc), stream=torch.cuda.Stream())
+        wait(slot)
+        code, out = slot.produce(raise_on_error=False)
+        assert code == pr.PR_ERR_CAPACITY
+        slot.release()
+        # the same slot, an ordinary event: the status does not stick
+        slot.acquire(to_dev(small.words), to_dev(small.adc), stream=torch.cuda.Stream())
+        wait(slot)
+        code, out = slot.produce()
+        assert code == 0
+        compare(out, oracle_of(small, cal), lambda f: out.to_numpy(f))
+        slot.release()
