@@ -257,9 +257,9 @@ __device__ __forceinline__ void wm_hook(idx_t* L, u32 a, u32 b) {
 }
 
 // A UNIT may hold up to four consecutive modules (digis [s, s + n); module j + 1 of the unit starts at digi s + bnd.b[j],
-// kNoBnd if the unit has no such module): their pixels are stacked along the row index with one empty row between two
-// modules (row' = row + j * (R + 1)), so that one pass clusters them all and no edge crosses a module border.  Kept
-// clusters are ranked per module; cntOut[j] receives module j's number of kept clusters.
+// kNoBnd if the unit has no such module): their pixels are stacked along the row index, 512 rows apart
+// (row' = row | j << 9: bits 18-19 of the info word are the module, and rows of two modules are never adjacent), so that
+// one pass clusters them all and no edge crosses a module border.  Kept clusters are ranked per module; cntOut[j] receives module j's number of kept clusters.
 constexpr u32 kNoBnd = 0xFFFFFFFFu;
 struct UnitBounds { u32 b[3]; };
 __device__ __forceinline__ u32 unit_module(const UnitBounds& bnd, u32 i) { return (i >= bnd.b[0] ? 1u : 0u) + (i >= bnd.b[1] ? 1u : 0u) + (i >= bnd.b[2] ? 1u : 0u); }
@@ -290,7 +290,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     wr.L[i] = (idx_t)i;
     u32 next = kNoIdx;
     if (kept) next = atomicExch(head + (rcc & 511u) + 1u, i) & kNoIdx;
-    if (!kMedium || i < n) wr.info[i] = kept ? ((rcc + (unit_module(bnd, i) * (g.R + 1u) << 9)) | next << 20) : kNoKey;   // (the global workspace ends at n)
+    if (!kMedium || i < n) wr.info[i] = kept ? (rcc | unit_module(bnd, i) << 18 | next << 20) : kNoKey;   // (the global workspace ends at n)
     nKept += __popc(__ballot_sync(0xFFFFFFFFu, kept));
     qc = qn; rcc = rcn;
   }
@@ -396,7 +396,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       double qf = 0.0, qx = 0.0, qy = 0.0;
       u32 bR = 0, bC = 0;
       if (in) {
-        const u32 row = ((x >> 9) & 0x7FFu) - unit_module(bnd, i) * (g.R + 1u), col = x & 511u;
+        const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
         qf = (double)((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
         qx = qf * (double)row; qy = qf * (double)col;
         bR = box_rows(row); bC = box_cols(col);
@@ -451,10 +451,11 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   // P7
   for (u32 i = lane; i < n; i += 32u) {
     u32 lab = kInvalid; int32_t cl = -1;
-    if (wr.info[i] != kNoKey) {
+    const u32 x = wr.info[i];
+    if (x != kNoKey) {
       const u32 r = wr.L[i], kr = krAt[r];
       lab = s + r;
-      if (kr != kNoRank) cl = (int32_t)clus_ranked(kr, mFirst + unit_module(bnd, i));
+      if (kr != kNoRank) cl = (int32_t)clus_ranked(kr, mFirst + ((x >> 18) & 3u));
     }
     ev.label[s + i] = lab; ev.clus[s + i] = cl;
   }
