@@ -148,7 +148,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     reinterpret_cast<u32*>(const_cast<EvDesc*>(batch))[tid] = reinterpret_cast<const u32*>(hostDesc)[tid];
   // control warp: tiles in flight, whether a draw came back empty, the ticket drawn in the previous iteration and its event
   u32 inflight = 0, tktP = kTileSkip, eP = 0;
-  bool ended = false;
+  bool ended = gridDim.x >= totalTiles;        // one ticket per CTA covers the launch: the draws of the prologues were the last ones
   if (ctl) {
     for (int j = 0; j < kDrawAhead; ++j) { inflight += tile_of(j) < totalTiles ? 1u : 0u; ended = ended || tile_of(j) == kTileEnd; }
   }
