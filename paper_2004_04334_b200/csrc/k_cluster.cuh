@@ -737,18 +737,26 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   const u32 bpe = (M + modBatch - 1) / modBatch, bpeB = (M + 1u) / 2u;
   const u32 nEvA = modBatch == kModBatch ? nEv - nEv / 4u : nEv, nEvB = modBatch == kModBatch ? (nEv - nEvA + 1u) / 2u : 0u;
   const u32 tA = nEvA * bpe, tB = tA + nEvB * bpeB, nTickets = tB + (nEv - nEvA - nEvB) * M;
-  for (;;) {
+  // (a launch with a warp for every ticket — a single event — needs no ticket counter: warp w takes ticket w, and the two
+  // trips to the counter, one of them after the work is done, are off the event's latency)
+  const bool oneEach = modBatch == 1u && nTickets <= nWarps;
+  for (u32 trip = 0;; ++trip) {
     u32 t = 0;
-    if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
-    t = __shfl_sync(0xFFFFFFFFu, t, 0);
+    if (oneEach) {
+      if (trip) break;
+      t = gw;
+    } else {
+      if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
+      t = __shfl_sync(0xFFFFFFFFu, t, 0);
+    }
     if (t >= nTickets) break;
     u32 e, m0, nm;
     if (t < tA) { e = t / bpe; m0 = (t - e * bpe) * modBatch; nm = min(modBatch, M - m0); }
     else if (t < tB) { const u32 u = t - tA; e = u / bpeB; m0 = (u - e * bpeB) * 2u; nm = min(2u, M - m0); e += nEvA; }
     else { const u32 u = t - tB; e = u / M; m0 = u - e * M; nm = 1u; e += nEvA + nEvB; }
     const EvDesc& ev = kSingle ? single : batch[e];
+    const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;      // (asked for together with the status: one round trip)
     if (ev.counters->status & 1u) continue;
-    const u32 st = lane <= nm ? ev.modDigiStart[m0 + lane] : 0u;
     u32 accK = 0, accA = 0, accG = 0;
     // The ticket's digis are contiguous.  The next unit's first chunk (32 digis) is loaded while the current unit
     // (a pack of small modules, or one module of 33..kWarpCap digis) is processed.

@@ -28,16 +28,20 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
   const EvDesc& ev = kSingle ? single : batch[e];
   const u32 nMods = kFinMods * groupsPerUnit;
   const u32 m0 = u * nMods, m1 = min(m0 + nMods, M), nm = m1 - m0;
+  // (the tables are read beside the status word, not after it: they are there whatever the status says)
+  u32 sum = 0, cLoad = 0, dLoad = 0;
+  for (u32 k = tid; k < u * groupsPerUnit; k += 256) sum += ev.grpCount[k];        // the groups before this unit
+  if (warp < groupsPerUnit && m0 + tid < m1) cLoad = ev.modCount[m0 + tid];
+  if (tid <= nMods) dLoad = ev.modDigiStart[min(m0 + tid, M)];
   if (!(ev.counters->status & 1u)) {
-    u32 sum = 0, base;
-    for (u32 k = tid; k < u * groupsPerUnit; k += 256) sum += ev.grpCount[k];      // the groups before this unit
+    u32 base;
     u32 c = 0, incl = 0;
     if (warp < groupsPerUnit) {                       // warp w scans the unit's group w
-      c = m0 + tid < m1 ? ev.modCount[m0 + tid] : 0u;
+      c = cLoad;
       incl = warp_incl_scan(c, lane);
       if (lane == 31) sTot[warp] = incl;
     }
-    if (tid <= nMods) sDigi[tid] = ev.modDigiStart[min(m0 + tid, M)];
+    if (tid <= nMods) sDigi[tid] = dLoad;
     block_excl_scan(sum, sScan, &base);               // (two barriers: sTot is visible after it)
     if (warp < groupsPerUnit) {
       u32 off = base;
