@@ -198,9 +198,10 @@ int pr_event_destroy(pr_event* ev);                  /* PR_ERR_BAD_STATE while w
  * `cuda_stream` (a cudaStream_t passed as void*, e.g. torch.cuda.Stream().cuda_stream; NULL is
  * the legacy default stream) and return at once.  Argument/state errors are returned here and
  * nothing is enqueued.  The slot must be idle (fresh or released).
- * A device-resident event without host mirrors is enqueued with ONE call: the slot keeps an instantiated CUDA graph of
- * its chain (clear control words, descriptor upload, the three kernels, completion event), everything that changes
- * from event to event travels in the descriptor; it is rebuilt only when the event size class changes.  The paper
+ * A device-resident event without host mirrors is enqueued with ONE launch: the slot keeps an instantiated CUDA graph of
+ * its chain (the three kernels and the completion event; the kernels leave the control words cleared behind them),
+ * everything that changes from event to event travels in the descriptor, which is set as a parameter of the three
+ * kernel nodes before the launch; the graph is rebuilt only when the event size class changes.  The paper
  * found CUDA graphs "too restrictive" for its modules in 2020; for one module's fixed chain they fit.     */
 int pr_acquire(pr_event* ev, const pr_input* in, void* cuda_stream);
 /* Same for a batch of n independent events processed by ONE chain of launches on one stream

@@ -105,6 +105,9 @@ struct pr_event {
   // the single-event chain as an instantiated CUDA graph: everything that changes between events travels in the
   // descriptor (gDescHost -> gDescDev by a copy node); rebuilt when the control block or the size class changes
   cudaGraphExec_t gExec = nullptr; cudaStream_t capStream = nullptr;
+  cudaGraph_t gGraph = nullptr; cudaGraphNode_t gNode[3] = {nullptr, nullptr, nullptr};   // the three kernel nodes: their parameters are set per launch
+  uint32_t gUnpackGrid = 0, gPro = 0, gClusterGrid = 0, gModBatch = 0, gUnits = 0;
+  LaunchCtl* gLc = nullptr; u64* gTileState = nullptr;
   EvDesc* gDescHost = nullptr; char* gDescDev = nullptr;      // [EvDesc][tile -> event map: zeros]
   void* gCtl = nullptr; uint32_t gTilesClass = 0; size_t gCtlZero = 0;
   uint64_t graphLaunches = 0, graphBuilds = 0;
@@ -214,6 +217,7 @@ void CUDART_CB trampoline(void* p) {
 void destroy_graph(pr_event* ev) {
   pr_handle* h = ev->h;
   if (ev->gExec) { cudaGraphExecDestroy(ev->gExec); ev->gExec = nullptr; }
+  if (ev->gGraph) { cudaGraphDestroy(ev->gGraph); ev->gGraph = nullptr; }
   if (ev->capStream) { cudaStreamDestroy(ev->capStream); ev->capStream = nullptr; }
   if (ev->gDescHost) { h->hostPool->free(ev->gDescHost, nullptr, true); ev->gDescHost = nullptr; }
   if (ev->gDescDev) { h->devPool->free(ev->gDescDev, nullptr, true); ev->gDescDev = nullptr; }
@@ -276,17 +280,11 @@ int fail_after_enqueue(pr_event* ev, int code) {
 // from device memory), record the completion event.  Grids are those of the size class; CTAs without a tile or a ticket
 // leave at once.  Only here may a slot's acquire allocate (first use of a size class).
 int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc, u64* tileState, cudaStream_t stream) {
+  (void)stream;
   pr_handle* h = ev->h;
   const uint32_t M = h->cfg.n_modules;
   if (ev->gExec) { cudaGraphExecDestroy(ev->gExec); ev->gExec = nullptr; }
-  const size_t descBytes = align_up(sizeof(EvDesc) + sizeof(u16) * 4096, 256);
-  if (!ev->gDescHost) {
-    ev->gDescHost = (EvDesc*)h->hostPool->alloc(sizeof(EvDesc), nullptr);
-    ev->gDescDev = (char*)h->devPool->alloc(descBytes, nullptr);
-    if (!ev->gDescHost || !ev->gDescDev) return PR_ERR_OOM;
-  }
-  const EvDesc* dd = (const EvDesc*)ev->gDescDev;
-  const u16* tileEvent = (const u16*)(ev->gDescDev + sizeof(EvDesc));
+  if (ev->gGraph) { cudaGraphDestroy(ev->gGraph); ev->gGraph = nullptr; }
   const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
   const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
   const uint32_t modBatch = (uint64_t)M >= 4 * warpsResident ? kModBatch : (uint64_t)M >= 2 * warpsResident ? 2u : 1u;
@@ -302,28 +300,62 @@ int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc
   const uint32_t finSplits = 1;                                  // (the class stays below 8192 words per module group on average)
   cudaStream_t cs = ev->capStream;
   cudaGraph_t graph = nullptr;
-  // the tile -> event map of a one-event launch is all zeros: cleared on the event's stream, ahead of the graph's first
-  // launch there (a later launch on another stream comes after this acquire was seen complete)
-  PR_CUDA(h, cudaMemsetAsync(ev->gDescDev, 0, descBytes, stream));
   cudaError_t e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
   if (e != cudaSuccess) return cuda_fail(h, e, "cudaStreamBeginCapture");
-  // no memset node: the kernels leave the control words zeroed behind them (k_unpack: tile ticket and look-back states;
-  // k_finalize with selfClean: module ticket, counters, group counts).  The descriptor travels by a copy node: reading it
-  // from the slot's mapped pinned block inside k_unpack (hostDesc) put two PCIe round trips at the head of the chain and
-  // was 2 us slower per event than the copy node
-  cudaMemcpyAsync(ev->gDescDev, ev->gDescHost, sizeof(EvDesc), cudaMemcpyHostToDevice, cs);
-  EvDesc none{};
-  k_unpack<false><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), cs>>>(none, dd, tileEvent, kTilesFromDesc, pro, lc, tileState, h->geom, nullptr);
-  k_cluster<false><<<clusterGrid, kClusterThreads, h->clusterSmem, cs>>>(none, dd, 1, lc, nullptr, modBatch, h->geom);
-  k_finalize<false><<<unitsPerEvent * finSplits, 256, 0, cs>>>(none, dd, 1, unitsPerEvent, finSplits, 1u, lc, h->geom, 1u);
+  // Three kernel nodes and the completion event, nothing else.  No memset node: the kernels leave the control words zeroed
+  // behind them (k_unpack: tile ticket and look-back states; k_finalize with selfClean: module ticket, counters, group
+  // counts).  No copy node: the event's descriptor is a kernel PARAMETER (the one-event form of the kernels), set on the
+  // three nodes before every launch (graph_set_event) — a copy node cost ~4 us at the head of every event's chain, reading
+  // the descriptor from mapped pinned memory inside k_unpack two PCIe round trips.
+  const EvDesc& d0 = ev->sub[0].desc;
+  k_unpack<true><<<unpackGrid, kUnpackThreads + 64, sizeof(UnpackShared), cs>>>(d0, nullptr, nullptr, d0.nTiles, pro, lc, tileState, h->geom, nullptr);
+  k_cluster<true><<<clusterGrid, kClusterThreads, h->clusterSmem, cs>>>(d0, nullptr, 1, lc, nullptr, modBatch, h->geom);
+  k_finalize<true><<<unitsPerEvent * finSplits, 256, 0, cs>>>(d0, nullptr, 1, unitsPerEvent, finSplits, 1u, lc, h->geom, 1u);
   cudaEventRecordWithFlags(ev->done, cs, cudaEventRecordExternal);   // an event-record NODE: ev->done stays an ordinary event the host can query
   e = cudaStreamEndCapture(cs, &graph);
   if (e != cudaSuccess || !graph) { cudaGetLastError(); return cuda_fail(h, e, "cudaStreamEndCapture"); }
+  // the kernel nodes, by the function they launch
+  cudaGraphNode_t nodes[8]; size_t nNodes = 8;
+  ev->gNode[0] = ev->gNode[1] = ev->gNode[2] = nullptr;
+  if (cudaGraphGetNodes(graph, nodes, &nNodes) == cudaSuccess) {
+    for (size_t k = 0; k < nNodes && k < 8; ++k) {
+      cudaGraphNodeType ty;
+      cudaKernelNodeParams kp{};
+      if (cudaGraphNodeGetType(nodes[k], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+      if (cudaGraphKernelNodeGetParams(nodes[k], &kp) != cudaSuccess) continue;
+      if (kp.func == (void*)k_unpack<true>) ev->gNode[0] = nodes[k];
+      else if (kp.func == (void*)k_cluster<true>) ev->gNode[1] = nodes[k];
+      else if (kp.func == (void*)k_finalize<true>) ev->gNode[2] = nodes[k];
+    }
+  }
+  if (!ev->gNode[0] || !ev->gNode[1] || !ev->gNode[2]) { cudaGetLastError(); cudaGraphDestroy(graph); return cuda_fail(h, cudaErrorUnknown, "graph kernel nodes"); }
   e = cudaGraphInstantiate(&ev->gExec, graph, 0);
-  cudaGraphDestroy(graph);
-  if (e != cudaSuccess) { ev->gExec = nullptr; return cuda_fail(h, e, "cudaGraphInstantiate"); }
+  if (e != cudaSuccess) { ev->gExec = nullptr; cudaGraphDestroy(graph); return cuda_fail(h, e, "cudaGraphInstantiate"); }
+  ev->gGraph = graph;                                        // (the nodes belong to it)
   ev->gCtl = ev->ctl; ev->gTilesClass = tilesClass; ev->gCtlZero = ctlZero;
+  ev->gUnpackGrid = unpackGrid; ev->gPro = pro; ev->gClusterGrid = clusterGrid; ev->gModBatch = modBatch; ev->gUnits = unitsPerEvent;
+  ev->gLc = lc; ev->gTileState = tileState;
   ++ev->graphBuilds;
+  return PR_OK;
+}
+
+// The event of this launch: its descriptor (and its tile count) into the parameters of the graph's three kernel nodes.
+int graph_set_event(pr_event* ev, const EvDesc& d0) {
+  pr_handle* h = ev->h;
+  const EvDesc* noBatch = nullptr; const u16* noMap = nullptr; u32* noList = nullptr; const EvDesc* noHost = nullptr;
+  u32 one = 1, nTiles = d0.nTiles, pro = ev->gPro, modBatch = ev->gModBatch, units = ev->gUnits, splits = 1, groups = 1, clean = 1;
+  LaunchCtl* lc = ev->gLc; u64* ts = ev->gTileState;
+  void* aU[] = {(void*)&d0, &noBatch, &noMap, &nTiles, &pro, &lc, &ts, &h->geom, &noHost};
+  void* aC[] = {(void*)&d0, &noBatch, &one, &lc, &noList, &modBatch, &h->geom};
+  void* aF[] = {(void*)&d0, &noBatch, &one, &units, &splits, &groups, &lc, &h->geom, &clean};
+  cudaKernelNodeParams kp{};
+  kp.extra = nullptr;
+  kp.func = (void*)k_unpack<true>; kp.gridDim = dim3(ev->gUnpackGrid); kp.blockDim = dim3(kUnpackThreads + 64); kp.sharedMemBytes = (unsigned)sizeof(UnpackShared); kp.kernelParams = aU;
+  PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[0], &kp));
+  kp.func = (void*)k_cluster<true>; kp.gridDim = dim3(ev->gClusterGrid); kp.blockDim = dim3(kClusterThreads); kp.sharedMemBytes = (unsigned)h->clusterSmem; kp.kernelParams = aC;
+  PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[1], &kp));
+  kp.func = (void*)k_finalize<true>; kp.gridDim = dim3(units * splits); kp.blockDim = dim3(256); kp.sharedMemBytes = 0; kp.kernelParams = aF;
+  PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[2], &kp));
   return PR_OK;
 }
 
@@ -499,10 +531,13 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       int rc = build_graph(ev, tilesClass, ctlZero, lc, tileState, stream);
       if (rc != PR_OK) return fail_after_enqueue(ev, rc);
     }
-    *ev->gDescHost = ev->sub[0].desc;
+    {
+      int rc = graph_set_event(ev, ev->sub[0].desc);
+      if (rc != PR_OK) return fail_after_enqueue(ev, rc);
+    }
     PR_CUDA_Q(ev, cudaGraphLaunch(ev->gExec, stream));
     ++ev->graphLaunches;
-    nLaunch = 3; nMemcpy = 1;
+    nLaunch = 3; nMemcpy = 0;
   } else {
   // tickets, counters, group counts: one small memset; the look-back states only when the block is new (k_unpack's last
   // CTA puts their zeros back, and those of its two ticket words, harmlessly cleared again here)
