@@ -229,16 +229,30 @@ __device__ __forceinline__ WmStore<false> wm_store_small(WarpRegion& r) {
   return st;
 }
 // Medium module = digis [s, s + n), n <= kMediumCap: the warp's region holds L (2 KB) and 4 KB of scratch.
-__device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const EvDesc& ev, u32 s) {
+// While six bytes per digi leave room for the column heads (up to 640 digis: the hot modules of a high pile-up event) the
+// info words sit beside L too: the neighbour walk of P2 then stays in shared memory, and what is left holds the accumulators.
+__device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const EvDesc& ev, u32 s, u32 n) {
   WmStore<true> st;
   unsigned char* base = reinterpret_cast<unsigned char*>(&r);
-  st.L = reinterpret_cast<u16*>(base); st.scratch = base + 2u * kMediumCap; st.accRoots = (sizeof(WarpRegion) - 2u * kMediumCap) / 36u;
-  st.info = ev.wsPerm + s; st.q = nullptr; st.edge = ev.wsParent + s;
-  st.rk = reinterpret_cast<u16*>(ev.wsRoot + s); st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
+  const u32 nCap = (n + 63u) & ~63u;
+  st.L = reinterpret_cast<u16*>(base);
+  st.rk = reinterpret_cast<u16*>(ev.wsRoot + s);
+  if (8u * nCap + 4u * (512u + 4u) <= sizeof(WarpRegion)) {                    // up to 448 digis: the cluster ranks too
+    st.info = reinterpret_cast<u32*>(base + 2u * nCap); st.rk = reinterpret_cast<u16*>(base + 6u * nCap);   // [L][info][rk][scratch]
+    st.scratch = base + 8u * nCap; st.accRoots = ((u32)sizeof(WarpRegion) - 8u * nCap) / 36u;
+  } else if (6u * nCap + 4u * (512u + 4u) <= sizeof(WarpRegion)) {
+    st.info = reinterpret_cast<u32*>(base + 2u * nCap);                        // [L][info][scratch]
+    st.scratch = base + 6u * nCap; st.accRoots = ((u32)sizeof(WarpRegion) - 6u * nCap) / 36u;
+  } else {
+    st.info = ev.wsPerm + s;
+    st.scratch = base + 2u * kMediumCap; st.accRoots = (sizeof(WarpRegion) - 2u * kMediumCap) / 36u;
+  }
+  st.q = nullptr; st.edge = ev.wsParent + s;
+  st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
   st.krAt = reinterpret_cast<u16*>(ev.wsKnum + s); st.active = reinterpret_cast<u32*>(ev.wsS + s);   // 2 n entries
   return st;
 }
-static_assert(sizeof(WarpRegion) - 2u * kMediumCap >= 4u * (512u + 2u), "the medium layout's scratch holds the column heads");
+static_assert(sizeof(WarpRegion) - 2u * kMediumCap >= 4u * (512u + 2u), "the medium layouts' scratch holds the column heads");
 
 template <typename idx_t>
 __device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
@@ -681,7 +695,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
         u32 nk, nr, cnts[4];
         const UnitBounds one = {{kNoBnd, kNoBnd, kNoBnd}};
-        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s), q0, rc0, m, one, &nk, &nr, cnts);
+        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s, nn), q0, rc0, m, one, &nk, &nr, cnts);
         const u32 cnt = cnts[0];
         if (lane == 0) {
           ev.modCount[m] = cnt;
