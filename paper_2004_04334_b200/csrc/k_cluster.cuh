@@ -25,24 +25,25 @@ namespace pixreco {
 // numbering (ascending label order, A12) and writes the cluster SoA.
 constexpr u32 kWarpCap = 256;                    // warp path: modules with at most this many digis
 constexpr u32 kMediumCap = 1024;                 // one warp with its large arrays in the global workspace: up to this many digis
-constexpr u32 kWarpScratch = 6144 - kWarpCap * (4 + 4 + 1 + 1 + 1 + 2);   // 2816 bytes
-constexpr u32 kAccRoots = kWarpScratch / 36;     // 78 clusters accumulated per pass over a module
+constexpr u32 kWarpRegion = 6784;                 // bytes of shared memory per warp: eight of them are what the CTA path needs anyway
+constexpr u32 kWarpScratch = kWarpRegion - kWarpCap * (4 + 4 + 4 + 1 + 1);   // 3200 bytes
+constexpr u32 kAccRoots = kWarpScratch / 36;     // 88 clusters accumulated per pass over a module
 constexpr u32 kModBatch = 8;                     // most modules per warp ticket (two units of four Run-3-like modules; tickets of 4: 3 % slower there, 1 % on the high pile-up batch);
                                                  // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
 constexpr u32 kNoKey = 0xFFFFFFFFu;
 constexpr u32 kNoRank = 0xFFFFu;
 
-struct WarpRegion {                 // 6 KB of shared memory per warp
+struct WarpRegion {                 // kWarpRegion bytes of shared memory per warp
   u32 info[kWarpCap];               // col | row' << 9 | next digi of the column << 20 (kNoIdx: none); kNoKey for a digi below the pixel threshold
   float q[kWarpCap];                // charge
-  unsigned char L[kWarpCap];        // label-equivalence forest, finally the root = minimum digi index of the cluster
+  u32 L[kWarpCap];                  // union-find forest (a word per digi: hooks are atomicMin), finally the root = minimum digi index of the
+                                    // cluster in the low half; at a root the high half then takes the rank among the module's kept clusters
   unsigned char rk[kWarpCap];       // at a root: rank of its cluster among the module's clusters (ascending label)
   unsigned char rootAt[kWarpCap];   // root of the cluster with that rank
-  u16 edge[kWarpCap];               // the (at most two) kept backward neighbours, e1 | e2 << 8, self = none; then the kept-cluster rank per root
-  __align__(16) unsigned char scratch[kWarpScratch];   // column heads, then the unresolved edges, then the accumulators
+  __align__(16) unsigned char scratch[kWarpScratch];   // column heads, then the accumulators
 };
-static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 4 * (512 + 2) && kWarpScratch >= 2 * 2 * kWarpCap, "scratch holds the accumulators, the column heads and the edge list");
-static_assert(sizeof(WarpRegion) == 6144, "6 KB per warp");
+static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 4 * (512 + 2), "scratch holds the accumulators and the column heads");
+static_assert(sizeof(WarpRegion) == kWarpRegion, "the warp's region");
 
 __host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords, u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
   size_t w = (bitmapWords + 3) & ~3u;
@@ -185,74 +186,67 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
 // ---- warp path: one module = digis [s, s+n), 32 < n <= kWarpCap, processed by the calling warp with only __syncwarp
 // between its passes.  Returns (kept digis, clusters, kept clusters) in all lanes.
 //   P1  load; kept flag (A8); every kept digi is pushed on the list of its COLUMN (head per column, `next` inside the
-//       digi's info word).  The push is a plain store that is read back: of the lanes that hit one column in the same
-//       instruction one store lands, that lane links to the previous head, the others try again (no atomics).
+//       digi's info word) with one atomicExch on the head.
 //   P2  neighbours: a walk over the digi's own column list (N = row - 1; a second digi on the same pixel, A6) and over
 //       the list of the column before (NW, W, SW).  Of these backward neighbours (column-major order) at most two
 //       edges are kept:  W ? {W} : { N ? N : NW,  SW }  — the dropped ones are adjacent to a kept one and are found from
 //       there, so the kept edges span every 8-adjacency.  A digi that shares its pixel with one of lower index keeps
-//       only the edge to that one.  Round 1 of the label equivalence is taken at once (labels = identity), in the
-//       digi's own slot: L[i] = min(i, its kept neighbours).
-//   P3  label equivalence on the forest L[] (L[i] <= i, a digi of i's component; a root has L[i] == i).  A kept edge
-//       that became its digi's link in P2 is resolved by construction; all the others go on the list of unresolved
-//       edges.  A round looks at the list: an edge whose ends have different roots hooks the larger root under the
-//       smaller one with a plain store (only while it still is a root: a tree is never split; of several lanes
-//       hooking one root in the same instruction one wins, the others find their edge unresolved in the next round)
-//       and stays on the list; an edge whose ends share their root is resolved for good and leaves it.  Until the list
-//       is empty.  Roots only ever go under smaller roots: the final root of a component is its minimum digi index =
-//       the canonical label (A10).
+//       only the edge to that one.
+//   P3  (inside P2's loop) union of the two ends of every kept edge on the forest L[] (one word per digi, L[i] <= i, a
+//       digi of i's component; a root has L[i] == i): both roots by plain loads, then atomicMin(L[larger root],
+//       smaller root).  If the larger one was a root it now hangs under the smaller one; if another lane had hooked it
+//       meanwhile, atomicMin left it under the smaller of the two candidates and the union goes on with the other pair
+//       (wm_union).  No edge list, no rounds: an edge is resolved when its lane leaves the loop.  Roots only ever go
+//       under smaller digis: the final root of a component is its minimum digi index = the canonical label (A10).
 //   P4  flatten; rank of every root in ascending index (= label) order.
-//   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory (exact: at most 256 terms below
-//       2^43), size and bounding box, kAccRoots clusters per pass: the lanes of a 32-digi chunk that share a cluster
+//   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory (exact: at most 1024 terms below
+//       2^43), size and bounding box, accRoots clusters per pass: the lanes of a 32-digi chunk that share a cluster
 //       are reduced with shuffles, their first lane owns the read-modify-write.
-//   P6  the roots apply the cluster threshold (A8), number the kept clusters and stage their sums.
+//   P6  the roots apply the cluster threshold (A8), number the kept clusters and stage their sums; the rank among the
+//       module's kept clusters goes into the free high half of the root's own word L[root].
 //   P7  per-digi outputs: label (final), cluster rank within the module.
-// Where warp_module keeps its arrays.  A module of at most kWarpCap digis lives in the warp's own 6 KB of shared memory
-// with one-byte digi indices; a module of up to kMediumCap digis (kMedium) keeps only the forest L[] (two-byte
-// indices), the column heads and the accumulators there, the rest lies in the event's global workspace at the
-// module's own digi range (cached in L1/L2; the module belongs to this warp alone).
+// Where warp_module keeps its arrays.  A module of at most kWarpCap digis lives in the warp's own region of shared
+// memory with one-byte digi indices; a module of up to kMediumCap digis (kMedium) keeps the forest L[], the column
+// heads and the accumulators there and, while they fit, the info words and the cluster ranks too (wm_store_medium);
+// the rest lies in the event's global workspace at the module's own digi range (cached in L1/L2; the module belongs
+// to this warp alone).
 template <bool kMedium> struct WmStore;
 template <> struct WmStore<false> {
-  typedef unsigned char idx_t; typedef u16 pair_t;
-  static constexpr u32 kNoIdx = 0x7FFu, kIdxMask = 0xFFu, kPairShift = 8;
-  u32* info; float* q; idx_t *L, *rk, *rootAt; pair_t *edge, *active; u16* krAt; unsigned char* scratch; u32 accRoots;
+  typedef unsigned char idx_t;
+  static constexpr u32 kNoIdx = 0x7FFu;
+  u32* info; float* q; u32* L; idx_t *rk, *rootAt; unsigned char* scratch; u32 accRoots;
 };
 template <> struct WmStore<true> {
-  typedef u16 idx_t; typedef u32 pair_t;
-  static constexpr u32 kNoIdx = 0x7FFu, kIdxMask = 0xFFFFu, kPairShift = 16;
-  u32* info; float* q; idx_t *L, *rk, *rootAt; pair_t *edge, *active; u16* krAt; unsigned char* scratch; u32 accRoots;
+  typedef u16 idx_t;
+  static constexpr u32 kNoIdx = 0x7FFu;
+  u32* info; float* q; u32* L; idx_t *rk, *rootAt; unsigned char* scratch; u32 accRoots;
 };
 __device__ __forceinline__ WmStore<false> wm_store_small(WarpRegion& r) {
   WmStore<false> st;
-  st.info = r.info; st.q = r.q; st.L = r.L; st.rk = r.rk; st.rootAt = r.rootAt; st.edge = r.edge;
-  st.active = reinterpret_cast<u16*>(r.scratch); st.krAt = r.edge; st.scratch = r.scratch; st.accRoots = kAccRoots;
+  st.info = r.info; st.q = r.q; st.L = r.L; st.rk = r.rk; st.rootAt = r.rootAt; st.scratch = r.scratch; st.accRoots = kAccRoots;
   return st;
 }
-// Medium module = digis [s, s + n), n <= kMediumCap: the warp's region holds L (2 KB) and 4 KB of scratch.
-// While six bytes per digi leave room for the column heads (up to 640 digis: the hot modules of a high pile-up event) the
-// info words sit beside L too: the neighbour walk of P2 then stays in shared memory, and what is left holds the accumulators.
-__device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const EvDesc& ev, u32 s, u32 n) {
+// Medium module = digis [s, s + n), 256 < n <= kMediumCap: the warp's region always holds the forest L (a word per digi),
+// the column heads and then the accumulators.  While eight bytes per digi leave room for the column heads (some 600
+// digis: the hot modules of a high pile-up event) the info words sit beside L too: the neighbour walk of P2 then stays
+// in shared memory; with ten bytes per digi (some 480 digis) the cluster ranks as well.  What does not fit lies in the
+// event's global workspace at the module's own digi range.
+__device__ __forceinline__ u32 wm_head_bytes(const Geom& g) { return ((g.C + 2u + 3u) & ~3u) * 4u; }
+__device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const EvDesc& ev, const Geom& g, u32 s, u32 n) {
   WmStore<true> st;
   unsigned char* base = reinterpret_cast<unsigned char*>(&r);
-  const u32 nCap = (n + 63u) & ~63u;
-  st.L = reinterpret_cast<u16*>(base);
-  st.rk = reinterpret_cast<u16*>(ev.wsRoot + s);
-  if (8u * nCap + 4u * (512u + 4u) <= sizeof(WarpRegion)) {                    // up to 448 digis: the cluster ranks too
-    st.info = reinterpret_cast<u32*>(base + 2u * nCap); st.rk = reinterpret_cast<u16*>(base + 6u * nCap);   // [L][info][rk][scratch]
-    st.scratch = base + 8u * nCap; st.accRoots = ((u32)sizeof(WarpRegion) - 8u * nCap) / 36u;
-  } else if (6u * nCap + 4u * (512u + 4u) <= sizeof(WarpRegion)) {
-    st.info = reinterpret_cast<u32*>(base + 2u * nCap);                        // [L][info][scratch]
-    st.scratch = base + 6u * nCap; st.accRoots = ((u32)sizeof(WarpRegion) - 6u * nCap) / 36u;
-  } else {
-    st.info = ev.wsPerm + s;
-    st.scratch = base + 2u * kMediumCap; st.accRoots = (sizeof(WarpRegion) - 2u * kMediumCap) / 36u;
-  }
-  st.q = nullptr; st.edge = ev.wsParent + s;
-  st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
-  st.krAt = reinterpret_cast<u16*>(ev.wsKnum + s); st.active = reinterpret_cast<u32*>(ev.wsS + s);   // 2 n entries
+  const u32 nCap = (n + 31u) & ~31u, room = kWarpRegion - wm_head_bytes(g);
+  st.L = reinterpret_cast<u32*>(base);
+  st.info = ev.wsPerm + s; st.rk = reinterpret_cast<u16*>(ev.wsRoot + s);
+  u32 used = 4u * nCap;
+  if (8u * nCap <= room) { st.info = reinterpret_cast<u32*>(base + used); used += 4u * nCap; }
+  if (10u * nCap <= room) { st.rk = reinterpret_cast<u16*>(base + used); used += 2u * nCap; }
+  used = (used + 15u) & ~15u;
+  st.scratch = base + used; st.accRoots = (kWarpRegion - used) / 36u;
+  st.q = nullptr; st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
   return st;
 }
-static_assert(sizeof(WarpRegion) - 2u * kMediumCap >= 4u * (512u + 2u), "the medium layouts' scratch holds the column heads");
+static_assert(kWarpRegion - 4u * kMediumCap >= 4u * (512u + 4u), "L of the largest medium module leaves room for the column heads");
 
 template <typename idx_t>
 __device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
@@ -263,11 +257,17 @@ __device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
     l = p;
   }
 }
-// Root a and root b are different: the larger one goes under the smaller one if it still is a root.
-template <typename idx_t>
-__device__ __forceinline__ void wm_hook(idx_t* L, u32 a, u32 b) {
-  const u32 hi = max(a, b), lo = min(a, b);
-  if (L[hi] == hi) L[hi] = (idx_t)lo;
+// Union of the sets of a and b on a forest of words (L[x] <= x): roots by plain loads, then the larger root goes under
+// the smaller one with atomicMin; if it was no root any more (another lane hooked it meanwhile) its former parent and the
+// smaller root are merged next.  Lanes of one warp may run this side by side on one forest.
+__device__ __forceinline__ void wm_union(u32* L, u32 a, u32 b) {
+  a = wm_find(L, a); b = wm_find(L, b);
+  while (a != b) {
+    const u32 hi = max(a, b), lo = min(a, b);
+    const u32 old = atomicMin(L + hi, lo);
+    if (old == hi) break;
+    a = old; b = lo;
+  }
 }
 
 // A UNIT may hold up to four consecutive modules (digis [s, s + n); module j + 1 of the unit starts at digi s + bnd.b[j],
@@ -282,14 +282,13 @@ template <bool kMedium>
 __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32 s, u32 n, const WmStore<kMedium>& wr, float q0, u32 rc0,
                                             u32 mFirst, const UnitBounds& bnd, u32* nKeptDigis, u32* nRootsOut, u32 (&cntOut)[4]) {
   typedef typename WmStore<kMedium>::idx_t idx_t;
-  typedef typename WmStore<kMedium>::pair_t pair_t;
-  constexpr u32 kNoIdx = WmStore<kMedium>::kNoIdx, kIdxMask = WmStore<kMedium>::kIdxMask, kPairShift = WmStore<kMedium>::kPairShift;
+  constexpr u32 kNoIdx = WmStore<kMedium>::kNoIdx;
   const u32 kAccRoots = wr.accRoots;
   const u32 lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
   const u32 nPad = (n + 31u) & ~31u;
   u32* head = reinterpret_cast<u32*>(wr.scratch);            // [C + 2]: head[c + 1] = last digi pushed on column c, head[0] stays empty
-  pair_t* active = wr.active;                               // after P2: unresolved edges, i | e << kPairShift
-  u16* krAt = wr.krAt;                                      // after P3: rank among the module's KEPT clusters of the cluster rooted at i
+  const u16* rootOf = reinterpret_cast<const u16*>(wr.L);   // after P4: low half of L[i] = root of i ...
+  u16* krAt = reinterpret_cast<u16*>(wr.L) + 1;             // ... after P6: high half of L[root] = rank among the module's KEPT clusters
 
   // P1
   for (u32 i = lane; i < g.C + 2u; i += 32u) head[i] = 0xFFFFFFFFu;
@@ -301,7 +300,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     if (i + 32u < n) { qn = ev.charge[s + i + 32u]; rcn = (u32)ev.row[s + i + 32u] << 9 | (u32)ev.col[s + i + 32u]; }
     const bool kept = i < n && qc >= g.pixThr;                                   // A8
     if (!kMedium) wr.q[i] = qc;
-    wr.L[i] = (idx_t)i;
+    wr.L[i] = i;
     u32 next = kNoIdx;
     if (kept) next = atomicExch(head + (rcc & 511u) + 1u, i) & kNoIdx;
     if (!kMedium || i < n) wr.info[i] = kept ? (rcc | unit_module(bnd, i) << 18 | next << 20) : kNoKey;   // (the global workspace ends at n)
@@ -336,50 +335,18 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
         if (e1 == kNoIdx) { e1 = SW != kNoIdx ? SW : i; }
         else if (SW != kNoIdx) e2 = SW;
       }
-      wr.L[i] = (idx_t)min(i, min(e1, e2));        // round 1 of the label equivalence (labels = identity), own slot only
     }
-    if (!kMedium || i < n) wr.edge[i] = (pair_t)(e1 | e2 << kPairShift);
+    // P3: the unions of the kept edges, at once
+    if (e1 != i) wm_union(wr.L, i, e1);
+    if (e2 != i) wm_union(wr.L, i, e2);
   }
   __syncwarp();
-  // P3: an edge that became its digi's link in P2 is resolved by construction; all the others start on the list
-  u32 nAct = 0;
-  for (u32 i = lane; i < nPad; i += 32u) {
-    const u32 ed = (!kMedium || i < n) ? (u32)wr.edge[i] : (i | i << kPairShift), e1 = ed & kIdxMask, e2 = ed >> kPairShift;
-    const u32 li = wr.L[i];
-    const bool u1 = e1 != i && e1 != li, u2 = e2 != i && e2 != li;
-    const u32 b1 = __ballot_sync(0xFFFFFFFFu, u1);
-    if (u1) active[nAct + __popc(b1 & lt)] = (pair_t)(i | e1 << kPairShift);
-    nAct += __popc(b1);
-    const u32 b2 = __ballot_sync(0xFFFFFFFFu, u2);
-    if (b2) {
-      if (u2) active[nAct + __popc(b2 & lt)] = (pair_t)(i | e2 << kPairShift);
-      nAct += __popc(b2);
-    }
-  }
-  __syncwarp();
-  while (nAct) {
-    u32 nNew = 0;
-    for (u32 k = lane; k < ((nAct + 31u) & ~31u); k += 32u) {
-      bool keep = false; u32 pr = 0;
-      if (k < nAct) {
-        pr = active[k];
-        const u32 a = wm_find(wr.L, pr & kIdxMask), b = wm_find(wr.L, pr >> kPairShift);
-        if (a != b) { keep = true; wm_hook(wr.L, a, b); }
-      }
-      __syncwarp();
-      const u32 kb = __ballot_sync(0xFFFFFFFFu, keep);
-      if (keep) active[nNew + __popc(kb & lt)] = (pair_t)pr;
-      nNew += __popc(kb);
-    }
-    __syncwarp();
-    nAct = nNew;
-  }
   // P4
   u32 nR = 0;
   for (u32 i = lane; i < nPad; i += 32u) {
     const bool kept = (!kMedium || i < n) && wr.info[i] != kNoKey;
     u32 l = i;
-    if (kept) { l = wm_find(wr.L, i); wr.L[i] = (idx_t)l; }
+    if (kept) { l = wm_find(wr.L, i); wr.L[i] = l; }
     const bool isRoot = kept && l == i;
     const u32 rb = __ballot_sync(0xFFFFFFFFu, isRoot);
     if (isRoot) { const u32 k = nR + __popc(rb & lt); wr.rk[i] = (idx_t)k; wr.rootAt[k] = (idx_t)i; }
@@ -400,7 +367,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       u32 rk = 0; bool in = false;
       u32 r = 0x10000u + lane;
       if (x != kNoKey) {
-        r = wr.L[i];
+        r = rootOf[2u * i];
         rk = (u32)wr.rk[r] - p0;
         in = rk < nAcc;
         if (!in) r = 0x10000u + lane;
@@ -457,7 +424,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
           ev.stLabel[o] = s + root; ev.stSize[o] = cb[k * 3u];
           ev.stBoxR[o] = cb[k * 3u + 1u]; ev.stBoxC[o] = cb[k * 3u + 2u];
         }
-        krAt[root] = (u16)kr;
+        krAt[2u * root] = (u16)kr;
       }
     }
     __syncwarp();
@@ -467,7 +434,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     u32 lab = kInvalid; int32_t cl = -1;
     const u32 x = wr.info[i];
     if (x != kNoKey) {
-      const u32 r = wr.L[i], kr = krAt[r];
+      const u32 r = rootOf[2u * i], kr = krAt[2u * r];
       lab = s + r;
       if (kr != kNoRank) cl = (int32_t)clus_ranked(kr, mFirst + ((x >> 18) & 3u));
     }
@@ -695,7 +662,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
         const float q0 = ev.charge[s + lane]; const u32 rc0 = (u32)ev.row[s + lane] << 9 | (u32)ev.col[s + lane];
         u32 nk, nr, cnts[4];
         const UnitBounds one = {{kNoBnd, kNoBnd, kNoBnd}};
-        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, s, nn), q0, rc0, m, one, &nk, &nr, cnts);
+        warp_module<true>(ev, g, s, nn, wm_store_medium(wr, ev, g, s, nn), q0, rc0, m, one, &nk, &nr, cnts);
         const u32 cnt = cnts[0];
         if (lane == 0) {
           ev.modCount[m] = cnt;

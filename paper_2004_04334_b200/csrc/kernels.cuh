@@ -5,8 +5,8 @@
 //              loads into a shared-memory ring, staged SoA output written by TMA bulk stores; tiles
 //              handed out by an atomic ticket.
 //   k_cluster  a3+a4 fused: a warp clusters a unit of up to four small modules (register packs up to 32 digis;
-//              column lists + reduced edge set + label equivalence on a byte forest up to 256; one warp with its
-//              large arrays in the global workspace up to 1024), exact cluster sums and bounding boxes, cluster
+//              column lists + reduced edge set + atomicMin union-find on a word forest in shared memory up to 1024,
+//              what does not fit the warp's region beyond some 600 digis in the global workspace), exact cluster sums and bounding boxes, cluster
 //              threshold, numbering inside the module; a whole CTA (bitmap + union-find) beyond.
 //   k_finalize event-wide numbering, cluster table, hit table, counters to the host.
 //   k_dense    the dense path for launches whose modules are large on average: one module per CTA,
