@@ -136,7 +136,7 @@ int pr_digis_acquire(pr_event* ev, const pr_input* in, void* cuda_stream) {
   // ---- enqueue: clear the control words, stage the input, unpack, close the product
   uint64_t nMemcpy = 0, nLaunch = 0;
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, fresh ? ev->ctlBytes : ctlZero, stream));
-  ev->ctlDirty = true;
+  ev->ctlDirty = true; ev->flagDone = false;
   if (stage && in->n_words) {
     PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stW[0], in->words, (size_t)in->n_words * 4, cudaMemcpyHostToDevice, stream));
     PR_CUDA_Q(ev, cudaMemcpyAsync(ev->stA[0], in->adc, (size_t)in->n_words * 2, cudaMemcpyHostToDevice, stream));
@@ -233,7 +233,7 @@ int pr_clusters_acquire(pr_event* ev, pr_product* p, uint32_t want, void* own_st
 
   uint64_t nMemcpy = 0, nLaunch = 0;
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, fresh ? ev->ctlBytes : ctlZero, stream));
-  ev->ctlDirty = true;
+  ev->ctlDirty = true; ev->flagDone = false;
   const uint32_t unitsPerEvent = (M + kFinMods - 1) / kFinMods;
   const uint64_t warpsResident = (uint64_t)h->smCount * h->clusterBlocksPerSM * (kClusterThreads / 32);
   const uint32_t modBatch = (uint64_t)M >= 4 * warpsResident ? kModBatch : (uint64_t)M >= 2 * warpsResident ? 2u : 1u;

@@ -270,6 +270,25 @@ __device__ __forceinline__ void wm_union(u32* L, u32 a, u32 b) {
   }
 }
 
+// Union of the sets of i, e1 and e2 (e2 == i: none): the three roots in one loop (independent loads), then the larger
+// roots under the smallest one; a root that another lane had hooked meanwhile takes the slow way (wm_union).
+__device__ __forceinline__ void wm_union3(u32* L, u32 i, u32 e1, u32 e2) {
+  u32 a = L[i], b = L[e1], c = L[e2];
+  for (;;) {
+    const u32 pa = L[a], pb = L[b], pc = L[c];
+    if (pa == a && pb == b && pc == c) break;
+    a = pa; b = pb; c = pc;
+  }
+  const u32 m = min(a, min(b, c));
+  u32 oa = a, ob = b, oc = c;
+  if (a != m) oa = atomicMin(L + a, m);
+  if (b != m) ob = atomicMin(L + b, m);
+  if (c != m && c != a && c != b) oc = atomicMin(L + c, m);
+  if (oa != a) wm_union(L, oa, m);
+  if (ob != b) wm_union(L, ob, m);
+  if (oc != c) wm_union(L, oc, m);
+}
+
 // A UNIT may hold up to four consecutive modules (digis [s, s + n); module j + 1 of the unit starts at digi s + bnd.b[j],
 // kNoBnd if the unit has no such module): their pixels are stacked along the row index, 512 rows apart
 // (row' = row | j << 9: bits 18-19 of the info word are the module, and rows of two modules are never adjacent), so that
@@ -337,8 +356,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       }
     }
     // P3: the unions of the kept edges, at once
-    if (e1 != i) wm_union(wr.L, i, e1);
-    if (e2 != i) wm_union(wr.L, i, e2);
+    if (e1 != i) wm_union3(wr.L, i, e1, e2);
   }
   __syncwarp();
   // P4
@@ -682,8 +700,8 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
     if (gi < total) {
       const u32 e = gi / M, m = gi - e * M;
       const EvDesc& ev = kSingle ? single : batch[e];
+      const u32 s = ev.modDigiStart[m], t = ev.modDigiStart[m + 1];   // (asked for beside the status word: one round trip)
       if (!(ev.counters->status & 1u)) {              // A5 violated: modDigiStart is undefined, no per-digi work
-        const u32 s = ev.modDigiStart[m], t = ev.modDigiStart[m + 1];
         const bool ok = t >= s && t <= ev.cap;
         big = ok && t - s > bigAbove;
         if (ok && !big && t - s > kWarpCap) medBits |= 1u << trip;
@@ -720,7 +738,7 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   const u32 tA = nEvA * bpe, tB = tA + nEvB * bpeB, nTickets = tB + (nEv - nEvA - nEvB) * M;
   // (a launch with a warp for every ticket — a single event — needs no ticket counter: warp w takes ticket w, and the two
   // trips to the counter, one of them after the work is done, are off the event's latency)
-  const bool oneEach = modBatch == 1u && nTickets <= nWarps;
+  const bool oneEach = nTickets <= nWarps;
   for (u32 trip = 0;; ++trip) {
     u32 t = 0;
     if (oneEach) {

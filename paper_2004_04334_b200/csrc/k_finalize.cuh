@@ -13,6 +13,26 @@ namespace pixreco {
 // clustering in the paper's Fig. 1; A26-A30: position from the same exact sums, bounding box, border flags, error
 // estimate), writes modClusStart[]; the CTA of an event's last module group publishes that event's counters to mapped
 // pinned host memory.
+// The event's counters to mapped pinned host memory and, for k_export, to their device copy.  With `flag` the host polls
+// seq instead of the completion event: the other fields and every earlier write of the launch are fenced before it.
+__device__ __forceinline__ void publish_counters(const EvDesc& ev, const LaunchCtl* lc, u32 nClusters, bool flag) {
+  const DevCounters* c = ev.counters;
+  const u32 status = __ldcg(&c->status);
+  HostCounters h;
+  h.nWords = __ldcg(&c->nWords); h.nDigis = __ldcg(&c->nDigis); h.nErrors = __ldcg(&c->nErrors); h.nKept = __ldcg(&c->nKept);
+  h.nClustersAll = __ldcg(&c->nClustersAll); h.nClusters = (status & 1u) ? 0u : nClusters; h.status = status; h.seq = flag ? 0u : 1u;
+  h.tStart = lc->tStart; h.tEnd = global_timer();
+  *ev.hostCounters = h;
+  DevCounters r;                                   // device copy of the final counters: k_export takes its sizes from it
+  r.nWords = h.nWords; r.nDigis = h.nDigis; r.nErrors = h.nErrors; r.nKept = h.nKept; r.nClustersAll = h.nClustersAll;
+  r.nClusters = h.nClusters; r.status = status; r.pad = 0;
+  *ev.result = r;
+  if (flag) {
+    __threadfence_system();
+    *reinterpret_cast<volatile u32*>(&ev.hostCounters->seq) = 1u;
+  }
+}
+
 constexpr u32 kFinMods = 32;                     // modules per group of grpCount[] (k_cluster adds whole tickets to one group)
 constexpr u32 kFinMaxGroups = 4;                 // a CTA takes 1, 2 or 4 consecutive groups (launches with many units: less set-up per digi)
 static_assert(kFinMods == 32 && 32 % kModBatch == 0, "grpCount groups are 32 modules and hold whole warp tickets");
@@ -103,22 +123,12 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
   }
   // The CTA of the event's last module group publishes the event's counters to mapped pinned host memory: all
   // the others were final when this kernel started, nClusters is this CTA's own result.
-  if (m1 == M && sp == 0 && tid == 0) {
-    const DevCounters* c = ev.counters;
-    const u32 status = c->status;
-    HostCounters h;
-    h.nWords = c->nWords; h.nDigis = c->nDigis; h.nErrors = c->nErrors; h.nKept = c->nKept;
-    h.nClustersAll = c->nClustersAll; h.nClusters = (status & 1u) ? 0u : sStart[nMods]; h.status = status; h.seq = 1;
-    h.tStart = lc->tStart; h.tEnd = global_timer();
-    *ev.hostCounters = h;
-    DevCounters r;                                   // device copy of the final counters: k_export takes its sizes from it
-    r.nWords = h.nWords; r.nDigis = h.nDigis; r.nErrors = h.nErrors; r.nKept = h.nKept; r.nClustersAll = h.nClustersAll;
-    r.nClusters = h.nClusters; r.status = status; r.pad = 0;
-    *ev.result = r;
-  }
-  // selfClean (a slot's graph, one event): the last CTA to leave puts the zeros back into the words that the next
-  // launch of the graph expects cleared — the module ticket, the event's counters and group counts — so that the graph
-  // needs no memset node (k_unpack does the same for its ticket and its look-back states).
+  if (!selfClean && m1 == M && sp == 0 && tid == 0) publish_counters(ev, lc, sStart[nMods], false);
+  // selfClean (a slot's graph, one event): the last CTA to leave publishes the counters instead — every other CTA's
+  // results are visible by then, so the host may take seq != 0 in the mapped counters as the completion of the whole
+  // acquire, without a driver call — and puts the zeros back into the words that the next launch of the graph expects
+  // cleared — the module ticket, the event's counters and group counts — so that the graph needs no memset node
+  // (k_unpack does the same for its ticket and its look-back states).
   if (selfClean) {
     __shared__ u32 sLast;
     __syncthreads();
@@ -126,6 +136,8 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
     __syncthreads();
     if (sLast) {
       __threadfence();
+      if (tid == 0) publish_counters(ev, lc, __ldcg(&ev.counters->nClusters), true);
+      __syncthreads();
       u32* c = reinterpret_cast<u32*>(ev.counters);
       if (tid < sizeof(DevCounters) / 4u) c[tid] = 0u;
       for (u32 k = tid; k < (M + kFinMods - 1u) / kFinMods; k += 256u) ev.grpCount[k] = 0u;

@@ -105,6 +105,9 @@ struct pr_event {
   // the single-event chain as an instantiated CUDA graph: everything that changes between events travels in the
   // descriptor (gDescHost -> gDescDev by a copy node); rebuilt when the control block or the size class changes
   cudaGraphExec_t gExec = nullptr; cudaStream_t capStream = nullptr;
+  EvDesc gDesc{}; bool gDescSet = false;   // the descriptor that the graph's k_cluster and k_finalize nodes hold
+  bool flagDone = false;                    // this acquire went through the slot's graph: k_finalize's last CTA raises seq in the mapped counters when
+                                            // everything is written, and poll() reads that word instead of asking the driver about `done`
   cudaGraph_t gGraph = nullptr; cudaGraphNode_t gNode[3] = {nullptr, nullptr, nullptr};   // the three kernel nodes: their parameters are set per launch
   uint32_t gUnpackGrid = 0, gPro = 0, gClusterGrid = 0, gModBatch = 0, gUnits = 0;
   LaunchCtl* gLc = nullptr; u64* gTileState = nullptr;
@@ -335,6 +338,7 @@ int build_graph(pr_event* ev, uint32_t tilesClass, size_t ctlZero, LaunchCtl* lc
   ev->gCtl = ev->ctl; ev->gTilesClass = tilesClass; ev->gCtlZero = ctlZero;
   ev->gUnpackGrid = unpackGrid; ev->gPro = pro; ev->gClusterGrid = clusterGrid; ev->gModBatch = modBatch; ev->gUnits = unitsPerEvent;
   ev->gLc = lc; ev->gTileState = tileState;
+  ev->gDescSet = false;
   ++ev->graphBuilds;
   return PR_OK;
 }
@@ -352,10 +356,15 @@ int graph_set_event(pr_event* ev, const EvDesc& d0) {
   kp.extra = nullptr;
   kp.func = (void*)k_unpack<true>; kp.gridDim = dim3(ev->gUnpackGrid); kp.blockDim = dim3(kUnpackThreads + 64); kp.sharedMemBytes = (unsigned)sizeof(UnpackShared); kp.kernelParams = aU;
   PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[0], &kp));
+  // k_cluster and k_finalize read nothing of the descriptor that names the input (words, adc, nWords, tileBase, nTiles:
+  // its first 28 bytes); the rest names the slot's own buffers, which the caching pool hands back event after event
+  constexpr size_t kInputPart = offsetof(EvDesc, cap);
+  if (ev->gDescSet && memcmp((const char*)&d0 + kInputPart, (const char*)&ev->gDesc + kInputPart, sizeof(EvDesc) - kInputPart) == 0) return PR_OK;
   kp.func = (void*)k_cluster<true>; kp.gridDim = dim3(ev->gClusterGrid); kp.blockDim = dim3(kClusterThreads); kp.sharedMemBytes = (unsigned)h->clusterSmem; kp.kernelParams = aC;
   PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[1], &kp));
   kp.func = (void*)k_finalize<true>; kp.gridDim = dim3(units * splits); kp.blockDim = dim3(256); kp.sharedMemBytes = 0; kp.kernelParams = aF;
   PR_CUDA(h, cudaGraphExecKernelNodeSetParams(ev->gExec, ev->gNode[2], &kp));
+  ev->gDesc = d0; ev->gDescSet = true;
   return PR_OK;
 }
 
@@ -536,6 +545,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
       if (rc != PR_OK) return fail_after_enqueue(ev, rc);
     }
     PR_CUDA_Q(ev, cudaGraphLaunch(ev->gExec, stream));
+    ev->flagDone = true;
     ++ev->graphLaunches;
     nLaunch = 3; nMemcpy = 0;
   } else {
@@ -543,6 +553,7 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
   // CTA puts their zeros back, and those of its two ticket words, harmlessly cleared again here)
   PR_CUDA_Q(ev, cudaMemsetAsync(ev->ctl, 0, ctlFresh ? ev->ctlBytes : ctlZero, stream));
   ev->ctlDirty = true;                             // (only the slot's graph leaves the control words zeroed behind it)
+  ev->flagDone = false;
   if (merged) {
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanW, (const void*)wLo, wHi - wLo, cudaMemcpyHostToDevice, stream));
     PR_CUDA_Q(ev, cudaMemcpyAsync(spanA, (const void*)aLo, aHi - aLo, cudaMemcpyHostToDevice, stream));
@@ -694,9 +705,14 @@ int acquire_impl(pr_event* ev, const pr_input* ins, uint32_t n, void* cuda_strea
 int poll(pr_event* ev) {
   if (ev->state == kDone) return PR_OK;
   if (ev->state != kInFlight) return PR_ERR_BAD_STATE;
-  cudaError_t r = cudaEventQuery(ev->done);
-  if (r == cudaErrorNotReady) { cudaGetLastError(); return PR_NOT_READY; }
-  if (r != cudaSuccess) return cuda_fail(ev->h, r, "cudaEventQuery");
+  if (ev->flagDone) {
+    if (*reinterpret_cast<const volatile uint32_t*>(&ev->hostCounters[0].seq) == 0u) return PR_NOT_READY;
+    std::atomic_thread_fence(std::memory_order_acquire);
+  } else {
+    cudaError_t r = cudaEventQuery(ev->done);
+    if (r == cudaErrorNotReady) { cudaGetLastError(); return PR_NOT_READY; }
+    if (r != cudaSuccess) return cuda_fail(ev->h, r, "cudaEventQuery");
+  }
   int worst = PR_OK; uint64_t dg = 0, cl = 0;
   for (uint32_t k = 0; k < ev->n; ++k) {
     const HostCounters& c = ev->hostCounters[k];
@@ -1061,6 +1077,7 @@ int pr_transfer(pr_event* ev, uint32_t want, void* cuda_stream, pr_done_fn done,
   ev->doneFn = done; ev->doneUser = user;
   ev->state = kInFlight;
   ev->transferStage = true;
+  ev->flagDone = false;                          // this stage ends with `done`, recorded above
   if (done) {
     ev->cbPending.store(1, std::memory_order_release);
     cudaError_t ce = cudaLaunchHostFunc(stream, trampoline, ev);
