@@ -162,7 +162,14 @@ k_export(const ExportItem* __restrict__ items, u32 nItems) {
     const size_t nVec = (bytes + 15) >> 4;                 // buffers are padded to 16 B
     const uint4* s = reinterpret_cast<const uint4*>(x.src);
     uint4* d = reinterpret_cast<uint4*>(x.dst);
-    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nVec; v += (size_t)gridDim.x * blockDim.x) d[v] = s[v];
+    const size_t step = (size_t)gridDim.x * blockDim.x;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < nVec; v += 4 * step) {     // four loads, then four stores
+      uint4 r[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) if (v + k * step < nVec) r[k] = s[v + k * step];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) if (v + k * step < nVec) d[v + k * step] = r[k];
+    }
   }
 }
 
