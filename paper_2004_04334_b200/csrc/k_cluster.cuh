@@ -736,16 +736,15 @@ k_cluster(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batc
   const u32 bpe = (M + modBatch - 1) / modBatch, bpeB = (M + 1u) / 2u;
   const u32 nEvA = modBatch == kModBatch ? nEv - nEv / 4u : nEv, nEvB = modBatch == kModBatch ? (nEv - nEvA + 1u) / 2u : 0u;
   const u32 tA = nEvA * bpe, tB = tA + nEvB * bpeB, nTickets = tB + (nEv - nEvA - nEvB) * M;
-  // (a launch with a warp for every ticket — a single event — needs no ticket counter: warp w takes ticket w, and the two
-  // trips to the counter, one of them after the work is done, are off the event's latency)
+  // Warp w's first ticket is ticket w, without a trip to the counter (all the warps of a launch would meet there at its
+  // start: some thousand atomics on one word); the counter hands out the tickets from nWarps on.  A launch with a warp
+  // for every ticket — a single event — never goes there: the trip after the work is done is off the event's latency too.
   const bool oneEach = nTickets <= nWarps;
   for (u32 trip = 0;; ++trip) {
-    u32 t = 0;
-    if (oneEach) {
-      if (trip) break;
-      t = gw;
-    } else {
-      if (lane == 0) t = atomicAdd(&lc->modTicket, 1u);
+    u32 t = gw;
+    if (trip) {
+      if (oneEach) break;
+      if (lane == 0) t = nWarps + atomicAdd(&lc->modTicket, 1u);
       t = __shfl_sync(0xFFFFFFFFu, t, 0);
     }
     if (t >= nTickets) break;
