@@ -541,7 +541,7 @@ def run_ours(args, rank, world):
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": t_e2e / n_e2e * bps * 1e3, "batches_timed": n_e2e, "batches_in_flight": n2,
-                    "what": "pinned host inputs (one block per batch from pr_host_alloc), want = CLUSTERS | HITS, same batch API; PCIe-bound: the H2D copies alone allow 44.8k events/s (54 GB/s), the mirrors leave through k_export's stores to mapped pinned memory (39 GB/s alone); fetching them by a pr_transfer stage (gather + one DMA copy) instead measured 22k"},
+                    "what": "pinned host inputs (one block per batch from pr_host_alloc), want = CLUSTERS | HITS, same batch API; PCIe-bound in both directions at once (0.31 GB in and 0.31 GB out per 256-event batch; a DMA copy in and kernel stores out measured 45 GB/s each way together on this box, 55 / 53 GB/s alone): the mirrors leave through k_export's stores to mapped pinned memory, 32 CTAs streaming item after item; fetching them by a pr_transfer stage (gather + one DMA copy) instead measured 22k events/s"},
             "steady_state_cudaMalloc": int(new_mallocs), "wall_s": t_wall}
 
     if rank == 0:

@@ -9,7 +9,7 @@
  *     known to be complete ("External Worker").  Here: pr_acquire / pr_produce.
  *   - Completion is signalled by a callback queued into the CUDA stream, able to carry an error
  *     (P:L35), never by a blocking wait (P:L31 fn.1 lists the banned calls).  Here: the
- *     optional `done` callback and/or polling pr_query (cudaEventQuery).
+ *     optional `done` callback and/or polling pr_query (cudaEventQuery, or a completion word in mapped memory).
  *   - Only asynchronous CUDA calls during event processing; work of one event is queued into ONE
  *     stream, different events' streams run concurrently.  The caller owns the stream.
  *   - Device and pinned-host memory come from a caching pool so that no runtime allocation API is
@@ -208,7 +208,10 @@ int pr_acquire(pr_event* ev, const pr_input* in, void* cuda_stream);
  * (B200-first: one Run-3 event is ~1000x too small to fill the GPU).  All inputs share mem_kind
  * and want; `done` of inputs[0] fires once for the batch.  n in 1..4096.                          */
 int pr_acquire_batch(pr_event* ev, const pr_input* inputs, uint32_t n, void* cuda_stream);
-/* PR_OK when the slot's work is complete, PR_NOT_READY if not (cudaEventQuery; never waits).     */
+/* PR_OK when the slot's work is complete, PR_NOT_READY if not (never waits): cudaEventQuery on the
+ * slot's event, or — for a one-event acquire replayed from the slot's CUDA graph — a load of the
+ * completion word that the last CTA of the last kernel raises in mapped pinned memory after a
+ * system-scope fence (every result of the acquire is visible to the host and to any stream then).  */
 int pr_query(pr_event* ev);
 /* produce: non-blocking.  PR_NOT_READY if called too early; otherwise fills *out and
  * returns PR_OK or the device-detected error (PR_ERR_INPUT_ORDER, PR_ERR_CAPACITY), in which case

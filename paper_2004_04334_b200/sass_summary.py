@@ -15,7 +15,7 @@ import subprocess
 import sys
 
 MNEMONICS = [("UBLKCP", r"\bUBLKCP"), ("SYNCS (mbarrier)", r"\bSYNCS"), ("ATOMS (all)", r"\bATOMS"), ("ATOMS.CAST.SPIN", r"\bATOMS\.CAST\.SPIN"),
-             ("ATOMS.EXCH", r"\bATOMS\.EXCH"), ("ATOMG/RED (global)", r"\b(ATOMG|RED)\b|\bATOMG\.|\bRED\."), ("REDUX", r"\bREDUX"),
+             ("ATOMS.EXCH", r"\bATOMS\.EXCH"), ("ATOMS.MIN", r"\bATOMS\.MIN"), ("ATOMG/RED (global)", r"\b(ATOMG|RED)\b|\bATOMG\.|\bRED\."), ("REDUX", r"\bREDUX"),
              ("MATCH", r"\bMATCH"), ("SHFL", r"\bSHFL"), ("VOTE", r"\bVOTE"), ("LDS", r"\bLDS"), ("STS", r"\bSTS"), ("DADD/DMUL/DFMA", r"\bD(ADD|MUL|FMA)\b"),
              ("BAR.SYNC", r"\bBAR\.SYNC"), ("HMMA/UTCMMA/tcgen05 (tensor cores)", r"\b(HMMA|IMMA|UTC[A-Z]*MMA|UTCMMA)"), ("LDTM/STTM (tensor memory)", r"\b(LDTM|STTM)")]
 
