@@ -388,3 +388,42 @@ def test_a_slot_may_alternate_between_its_graph_and_plain_launches(pr):
                 assert code == 0
                 check(out, refs[k])
             slot.release()
+
+
+def test_graph_acquire_is_complete_when_its_flag_is_up(pr):
+    """A one-event acquire replayed from the slot's graph completes on a word in mapped pinned memory that the last CTA
+    of k_finalize raises after a system-scope fence (no cudaEventQuery).  When pr_produce says PR_OK every output of
+    the acquire must be visible to ANY stream: 300 events back to back, each read at once on a side stream that is not
+    ordered with the slot's stream, and compared with the oracle (the next event is already queued behind it on the
+    slot's stream: the slot's buffers come back from the pool, so a stale or partial table would show)."""
+    cal = wl.make_calib(1)
+    evs = [wl.make_event(1, 60 + k) for k in range(6)]
+    refs = [oracle.run(e.words, e.adc, e.n_modules, cal.gain, cal.pedestal) for e in evs]
+    dev = [(to_dev(e.words), to_dev(e.adc)) for e in evs]
+    side = torch.cuda.Stream()
+    with pr.PixReco(cal.gain, cal.pedestal) as p:
+        slots = [p.slot(), p.slot()]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        st0 = p.stats()
+        slots[0].acquire(*dev[0], stream=streams[0])
+        for it in range(300):
+            cur, nxt = slots[it & 1], slots[(it + 1) & 1]
+            nxt.acquire(*dev[(it + 1) % 6], stream=streams[(it + 1) & 1])     # keeps the device busy beside the read-back
+            wait(cur)
+            code, out = cur.produce()
+            assert code == 0
+            r = refs[it % 6]
+            assert (out.n_digis, out.n_kept_digis, out.n_clusters_all, out.n_clusters) == \
+                (r.n_digis, r.n_kept_digis, r.n_clusters_all, r.n_clusters), it
+            with torch.cuda.stream(side):
+                clus = out._device_bytes("clus").clone()
+                lab = out._device_bytes("cl_label").clone()
+                x = out._device_bytes("ht_x").clone()
+            side.synchronize()
+            assert np.array_equal(clus.cpu().numpy().view(np.int32), r.clus), it
+            assert np.array_equal(lab.cpu().numpy().view(np.uint32), r.cl_label), it
+            assert np.array_equal(x.cpu().numpy().view(np.float32), r.ht_x), it
+            cur.release()
+        wait(slots[0]); slots[0].produce(); slots[0].release()
+        st = p.stats()
+        assert st["memcpy_calls"] == st0["memcpy_calls"]             # all 301 went through the graph (no copies, no mirrors)
