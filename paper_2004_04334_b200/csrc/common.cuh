@@ -51,6 +51,19 @@ __device__ __forceinline__ u64 global_timer() {
   return t;
 }
 
+// A kept cluster as the clustering kernels stage it for k_finalize: exact sums (A9), label, size, bounding box (A28:
+// max(255 - row) << 16 | max(row), max(511 - col) << 16 | max(col)).  ONE 48-byte record per cluster (three 16-byte
+// accesses): a module's kept clusters are one contiguous run in memory.  (Seven separate arrays, as until capture Q of
+// round 2, made seven sparse runs per module: k_finalize read 2.5 times the bytes it used.)
+struct __align__(16) StagedCluster { double S, Sx, Sy; u32 label, size, boxR, boxC, pad0, pad1; };
+static_assert(sizeof(StagedCluster) == 48, "three 16-byte vectors");
+__device__ __forceinline__ void stage_store(StagedCluster* p, double S, double Sx, double Sy, u32 label, u32 size, u32 boxR, u32 boxC) {
+  uint4* q = reinterpret_cast<uint4*>(p);
+  q[0] = make_uint4((u32)__double2loint(S), (u32)__double2hiint(S), (u32)__double2loint(Sx), (u32)__double2hiint(Sx));
+  q[1] = make_uint4((u32)__double2loint(Sy), (u32)__double2hiint(Sy), label, size);
+  q[2] = make_uint4(boxR, boxC, 0u, 0u);
+}
+
 // One event of a launch.  The first 128 bytes are all that k_unpack reads: in a batch, one warp-wide
 // load brings them into shared memory.
 struct EvDesc {
@@ -76,9 +89,7 @@ struct EvDesc {
   DevCounters* result;              // device copy of the event's final counters (per acquire; k_export reads its sizes there)
   u32* modCount;                    // [M+1] kept clusters per module (k_cluster -> k_finalize)
   u32* grpCount;                    // [ceil(M / 32)] the same summed over groups of kFinMods modules (zeroed per acquire)
-  // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
-  double *stS, *stSx, *stSy; u32 *stLabel, *stSize;
-  u32 *stBoxR, *stBoxC;             // bounding box (A28): max(255 - row) << 16 | max(row), max(511 - col) << 16 | max(col)
+  StagedCluster* staged;            // staged kept clusters: record k of the module with first digi s lives at index s + k [cap]
 };
 static_assert(offsetof(EvDesc, label) == 128, "k_unpack's part of the descriptor is one 128-byte line");
 

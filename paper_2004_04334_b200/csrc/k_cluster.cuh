@@ -171,9 +171,7 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
   const u32 kr = (u32)__popc(kb & lt & ~((1u << (mStart - s)) - 1u));           // rank among the module's kept clusters
   if (keptC) {
     const u32 o = mStart + kr;
-    ev.stS[o] = qf; ev.stSx[o] = qx; ev.stSy[o] = qy;
-    ev.stLabel[o] = s + lane; ev.stSize[o] = (u32)__popc(reach);
-    ev.stBoxR[o] = bR; ev.stBoxC[o] = bC;
+    stage_store(ev.staged + o, qf, qx, qy, s + lane, (u32)__popc(reach), bR, bC);
   }
   const u32 krRoot = __shfl_sync(0xFFFFFFFFu, keptC ? kr : kNoRank, root);
   if (lane < n) {
@@ -438,9 +436,7 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
           const u32 before = mr == 0u ? cntOut[0] : mr == 1u ? cntOut[1] : mr == 2u ? cntOut[2] : cntOut[3];
           kr = before - (u32)__popc(mine) + (u32)__popc(mine & lt);
           const u32 o = s + (mr ? bnd.b[mr - 1u] : 0u) + kr;
-          ev.stS[o] = S; ev.stSx[o] = acc[k * 3u + 1u]; ev.stSy[o] = acc[k * 3u + 2u];
-          ev.stLabel[o] = s + root; ev.stSize[o] = cb[k * 3u];
-          ev.stBoxR[o] = cb[k * 3u + 1u]; ev.stBoxC[o] = cb[k * 3u + 2u];
+          stage_store(ev.staged + o, S, acc[k * 3u + 1u], acc[k * 3u + 2u], s + root, cb[k * 3u], cb[k * 3u + 1u], cb[k * 3u + 2u]);
         }
         krAt[2u * root] = (u16)kr;
       }
@@ -634,9 +630,8 @@ __device__ __forceinline__ void dense_stage(const EvDesc& ev, u32 m, u32 s, u32 
     const int32_t kn = cx.knum[k];
     if (kn < 0) continue;
     const u32 o = s + (u32)kn;                       // kn <= k < nn: inside the module's own range
-    ev.stS[o] = __ll2double_rn((i64)cx.S[k]); ev.stSx[o] = __ll2double_rn((i64)cx.Sx[k]); ev.stSy[o] = __ll2double_rn((i64)cx.Sy[k]);
-    ev.stLabel[o] = s + cx.root[k]; ev.stSize[o] = cx.csize[k];
-    ev.stBoxR[o] = cx.box[4u * k] << 16 | cx.box[4u * k + 1u]; ev.stBoxC[o] = cx.box[4u * k + 2u] << 16 | cx.box[4u * k + 3u];
+    stage_store(ev.staged + o, __ll2double_rn((i64)cx.S[k]), __ll2double_rn((i64)cx.Sx[k]), __ll2double_rn((i64)cx.Sy[k]), s + cx.root[k], cx.csize[k],
+                cx.box[4u * k] << 16 | cx.box[4u * k + 1u], cx.box[4u * k + 2u] << 16 | cx.box[4u * k + 3u]);
   }
   for (u32 i = tid; i < nn; i += kT) {
     const u32 p = cx.parent[i];

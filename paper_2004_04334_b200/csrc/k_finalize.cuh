@@ -98,15 +98,17 @@ k_finalize(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ bat
           if (li + step < nMods + 1 && sStart[li + step] <= o) li += step;       // last module with start <= o and a cluster there
         const u32 src = sDigi[li] + (o - sStart[li]);
         if (o < ev.cap && src < ev.cap) {
-          const double S = ev.stS[src];
-          ev.clLabel[o] = ev.stLabel[src]; ev.clModule[o] = (u16)(m0 + li); ev.clSize[o] = ev.stSize[src];
+          const uint4* rec = reinterpret_cast<const uint4*>(ev.staged + src);                              // StagedCluster
+          const uint4 r0 = rec[0], r1 = rec[1], r2 = rec[2];
+          const double S = __hiloint2double((int)r0.y, (int)r0.x), Sx = __hiloint2double((int)r0.w, (int)r0.z), Sy = __hiloint2double((int)r1.y, (int)r1.x);
+          ev.clLabel[o] = r1.z; ev.clModule[o] = (u16)(m0 + li); ev.clSize[o] = r1.w;
           ev.clCharge[o] = __double2float_rn(S * (1.0 / 16384.0));
-          const double rc = __ddiv_rn(ev.stSx[src], S), cc = __ddiv_rn(ev.stSy[src], S);                   // A9
+          const double rc = __ddiv_rn(Sx, S), cc = __ddiv_rn(Sy, S);                                       // A9
           ev.clRow[o] = __double2float_rn(rc);
           ev.clCol[o] = __double2float_rn(cc);
           // the hit of this cluster.  A27: divide, add 0.5, subtract half the module, multiply by the pitch — binary64, in
           // this order, one cast; A28 box; A29 border flags; A30 error = pitch/sqrt(12) * {span at a border, 1 for span 1, else 0.5}
-          const u32 bR = ev.stBoxR[src], bC = ev.stBoxC[src];
+          const u32 bR = r2.x, bC = r2.y;
           const u32 rmin = 255u - (bR >> 16), rmax = bR & 0xFFFFu, cmin = 511u - (bC >> 16), cmax = bC & 0xFFFFu;
           const bool er = rmin == 0u || rmax == g.R - 1u, ec = cmin == 0u || cmax == g.C - 1u;
           const u32 sr = rmax - rmin + 1u, sc = cmax - cmin + 1u;

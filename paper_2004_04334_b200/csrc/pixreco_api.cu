@@ -162,8 +162,7 @@ void carve_clusters(Carver& c, EvDesc& d, uint32_t cap, uint32_t M) {
   d.htX = c.take<float>(cap); d.htY = c.take<float>(cap); d.htXerr = c.take<float>(cap); d.htYerr = c.take<float>(cap);
   d.htRows = c.take<u32>(cap); d.htCols = c.take<u32>(cap); d.htFlags = c.take<u16>(cap);
   d.modCount = c.take<u32>(M + 4);
-  d.stS = c.take<double>(cap); d.stSx = c.take<double>(cap); d.stSy = c.take<double>(cap);
-  d.stLabel = c.take<u32>(cap); d.stSize = c.take<u32>(cap); d.stBoxR = c.take<u32>(cap); d.stBoxC = c.take<u32>(cap);
+  d.staged = c.take<StagedCluster>(cap);
   // touched only by modules beyond the shared-memory tiers
   d.wsPerm = c.take<u32>(cap); d.wsParent = c.take<u32>(cap); d.wsRoot = c.take<u32>(cap);
   d.wsKnum = c.take<int32_t>(cap); d.wsSize = c.take<u32>(cap);
