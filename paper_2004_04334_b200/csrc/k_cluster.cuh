@@ -308,7 +308,12 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   u16* krAt = reinterpret_cast<u16*>(wr.L) + 1;             // ... after P6: high half of L[root] = rank among the module's KEPT clusters
 
   // P1
-  for (u32 i = lane; i < g.C + 2u; i += 32u) head[i] = 0xFFFFFFFFu;
+  // The lists are per (column, parity of the module within the unit): the odd modules' columns start `off` heads
+  // further on, in what the accumulators do not need yet (a unit's four modules would otherwise share every column's
+  // list, and a digi walks the whole list).  Where the two ranges overlap a list holds digis of two columns; the
+  // walks compare the whole (column, row') key.  A medium module is alone: one list per column.
+  const u32 nHead = kMedium ? g.C + 2u : kWarpScratch / 4u, off = kMedium ? 0u : nHead - (g.C + 2u);
+  for (u32 i = lane; i < nHead; i += 32u) head[i] = 0xFFFFFFFFu;
   __syncwarp();
   u32 nKept = 0;
   float qc = q0; u32 rcc = rc0;
@@ -319,8 +324,9 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     if (!kMedium) wr.q[i] = qc;
     wr.L[i] = i;
     u32 next = kNoIdx;
-    if (kept) next = atomicExch(head + (rcc & 511u) + 1u, i) & kNoIdx;
-    if (!kMedium || i < n) wr.info[i] = kept ? (rcc | unit_module(bnd, i) << 18 | next << 20) : kNoKey;   // (the global workspace ends at n)
+    const u32 mu = unit_module(bnd, i);
+    if (kept) next = atomicExch(head + (rcc & 511u) + 1u + (mu & 1u) * off, i) & kNoIdx;
+    if (!kMedium || i < n) wr.info[i] = kept ? (rcc | mu << 18 | next << 20) : kNoKey;   // (the global workspace ends at n)
     nKept += __popc(__ballot_sync(0xFFFFFFFFu, kept));
     qc = qn; rcc = rcn;
   }
@@ -330,19 +336,19 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
     u32 e1 = i, e2 = i;
     if (x != kNoKey) {
-      const u32 c = x & 511u, r = (x >> 9) & 0x7FFu;
+      const u32 key = x & 0xFFFFFu, c = x & 511u, hb = c + ((x >> 18) & 1u) * off;   // key = col | row' << 9 (row' holds the module)
       u32 W = kNoIdx, N = kNoIdx, NW = kNoIdx, SW = kNoIdx, own = i;
-      for (u32 j = head[c + 1u]; j < kNoIdx;) {    // the digi's own column (never empty): N, and the lowest digi on the same pixel
-        const u32 y = wr.info[j], rj = (y >> 9) & 0x7FFu;
-        if (rj == r) own = min(own, j);
-        if (rj + 1u == r) N = j;
+      for (u32 j = head[hb + 1u]; j < kNoIdx;) {   // the digi's own column (never empty): N, and the lowest digi on the same pixel
+        const u32 y = wr.info[j], ky = y & 0xFFFFFu;
+        if (ky == key) own = min(own, j);
+        if (ky + 512u == key) N = j;
         j = y >> 20;
       }
-      for (u32 j = head[c]; j < kNoIdx;) {         // the column before: NW, W, SW
-        const u32 y = wr.info[j], d = ((y >> 9) & 0x7FFu) - r;
+      for (u32 j = c ? head[hb] : kNoIdx; j < kNoIdx;) {   // the column before: NW, W, SW
+        const u32 y = wr.info[j], d = (y & 0xFFFFFu) - (key - 1u);
         if (d == 0u) W = j;
-        if (d == 0xFFFFFFFFu) NW = j;
-        if (d == 1u) SW = j;
+        if (d == 0u - 512u) NW = j;
+        if (d == 512u) SW = j;
         j = y >> 20;
       }
       if (own != i) e1 = own;
