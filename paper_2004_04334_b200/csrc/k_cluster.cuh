@@ -27,7 +27,7 @@ constexpr u32 kWarpCap = 256;                    // warp path: modules with at m
 constexpr u32 kMediumCap = 1024;                 // one warp with its large arrays in the global workspace: up to this many digis
 constexpr u32 kWarpRegion = 6784;                 // bytes of shared memory per warp: eight of them are what the CTA path needs anyway
 constexpr u32 kWarpScratch = kWarpRegion - kWarpCap * (4 + 4 + 4 + 1 + 1);   // 3200 bytes
-constexpr u32 kAccRoots = kWarpScratch / 36;     // 88 clusters accumulated per pass over a module
+constexpr u32 kAccRoots = kWarpScratch / 44;      // 72 clusters accumulated per pass over a module (kAccWords = 11 words each)
 constexpr u32 kModBatch = 8;                     // most modules per warp ticket (two units of four Run-3-like modules; tickets of 4: 3 % slower there, 1 % on the high pile-up batch);
                                                  // small launches use 2 or 1 so that every warp gets work (modBatch, a power of two)
 constexpr u32 kNoKey = 0xFFFFFFFFu;
@@ -42,7 +42,7 @@ struct WarpRegion {                 // kWarpRegion bytes of shared memory per wa
   unsigned char rootAt[kWarpCap];   // root of the cluster with that rank
   __align__(16) unsigned char scratch[kWarpScratch];   // column heads, then the accumulators
 };
-static_assert(kWarpScratch >= kAccRoots * 36 && kWarpScratch >= 4 * (512 + 2), "scratch holds the accumulators and the column heads");
+static_assert(kWarpScratch >= kAccRoots * 44 && kWarpScratch >= 4 * (512 + 2), "scratch holds the accumulators and the column heads");
 static_assert(sizeof(WarpRegion) == kWarpRegion, "the warp's region");
 
 __host__ __device__ inline size_t dense_smem_bytes(u32 bitmapWords, u32 capDigis = kSmemDigis, u32 capClusters = kSmemClusters) {
@@ -197,9 +197,10 @@ __device__ __forceinline__ void warp_pack(const EvDesc& ev, const Geom& g, u32 s
 //       (wm_union).  No edge list, no rounds: an edge is resolved when its lane leaves the loop.  Roots only ever go
 //       under smaller digis: the final root of a component is its minimum digi index = the canonical label (A10).
 //   P4  flatten; rank of every root in ascending index (= label) order.
-//   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as binary64 in shared memory (exact: at most 1024 terms below
-//       2^43), size and bounding box, accRoots clusters per pass: the lanes of a 32-digi chunk that share a cluster
-//       are reduced with shuffles, their first lane owns the read-modify-write.
+//   P5  per-cluster sums S, Sx, Sy of qf = q * 2^14 (A9) as 64-bit integers in shared memory, size and bounding box,
+//       accRoots clusters per pass: every digi adds to its cluster's eleven words with native 32-bit atomics (a 64-bit
+//       add is the add on the low word, whose return value tells this thread whether ITS add carried, and an add of
+//       high word + carry when that is not zero: acc_add64).
 //   P6  the roots apply the cluster threshold (A8), number the kept clusters and stage their sums; the rank among the
 //       module's kept clusters goes into the free high half of the root's own word L[root].
 //   P7  per-digi outputs: label (final), cluster rank within the module.
@@ -240,7 +241,7 @@ __device__ __forceinline__ WmStore<true> wm_store_medium(WarpRegion& r, const Ev
   if (8u * nCap <= room) { st.info = reinterpret_cast<u32*>(base + used); used += 4u * nCap; }
   if (10u * nCap <= room) { st.rk = reinterpret_cast<u16*>(base + used); used += 2u * nCap; }
   used = (used + 15u) & ~15u;
-  st.scratch = base + used; st.accRoots = (kWarpRegion - used) / 36u;
+  st.scratch = base + used; st.accRoots = (kWarpRegion - used) / 44u;
   st.q = nullptr; st.rootAt = reinterpret_cast<u16*>(ev.wsSize + s);
   return st;
 }
@@ -255,6 +256,17 @@ __device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
     l = p;
   }
 }
+// acc[0..1] += v as a 64-bit integer with native 32-bit shared-memory atomics: the add on the low word returns what was
+// there, so this thread knows whether ITS add carried, and takes the carry along with its high word.
+constexpr u32 kAccWords = 11;
+__device__ __forceinline__ void acc_add64(u32* a, u64 v) {
+  const u32 lo = (u32)v;
+  u32 hi = (u32)(v >> 32);
+  const u32 old = atomicAdd(a, lo);
+  hi += old > ~lo ? 1u : 0u;
+  if (hi) atomicAdd(a + 1, hi);
+}
+
 // Union of the sets of a and b on a forest of words (L[x] <= x): roots by plain loads, then the larger root goes under
 // the smaller one with atomicMin; if it was no root any more (another lane hooked it meanwhile) its former parent and the
 // smaller root are merged next.  Lanes of one warp may run this side by side on one forest.
@@ -376,57 +388,33 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
   }
   __syncwarp();
   // P5, P6
-  double* acc = reinterpret_cast<double*>(wr.scratch);
-  u32* cb = reinterpret_cast<u32*>(acc + kAccRoots * 3u);      // three words per cluster: size, box rows, box cols
+  u32* acc = reinterpret_cast<u32*>(wr.scratch);             // kAccWords per cluster: S, Sx, Sy as (low, high) words, size, four box maxima
   cntOut[0] = cntOut[1] = cntOut[2] = cntOut[3] = 0u;
   for (u32 p0 = 0; p0 < nR; p0 += kAccRoots) {
     const u32 nAcc = min(nR - p0, kAccRoots);
-    for (u32 i = lane; i < nAcc * 3u; i += 32u) acc[i] = 0.0;
-    for (u32 i = lane; i < nAcc * 3u; i += 32u) cb[i] = 0u;
+    for (u32 i = lane; i < nAcc * kAccWords; i += 32u) acc[i] = 0u;
     __syncwarp();
     for (u32 i = lane; i < nPad; i += 32u) {
       const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
-      u32 rk = 0; bool in = false;
-      u32 r = 0x10000u + lane;
       if (x != kNoKey) {
-        r = rootOf[2u * i];
-        rk = (u32)wr.rk[r] - p0;
-        in = rk < nAcc;
-        if (!in) r = 0x10000u + lane;
+        const u32 rk = (u32)wr.rk[rootOf[2u * i]] - p0;
+        if (rk < nAcc) {
+          const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
+          const u64 qf = (u64)__float2ll_rz((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
+          u32* a = acc + rk * kAccWords;
+          acc_add64(a, qf); acc_add64(a + 2, qf * row); acc_add64(a + 4, qf * col);
+          atomicAdd(a + 6, 1u);
+          atomicMax(a + 7, 255u - row); atomicMax(a + 8, row); atomicMax(a + 9, 511u - col); atomicMax(a + 10, col);
+        }
       }
-      const u32 peers = __match_any_sync(0xFFFFFFFFu, r);
-      const u32 most = __reduce_max_sync(0xFFFFFFFFu, in ? (u32)__popc(peers) : 0u);
-      double qf = 0.0, qx = 0.0, qy = 0.0;
-      u32 bR = 0, bC = 0;
-      if (in) {
-        const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
-        qf = (double)((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
-        qx = qf * (double)row; qy = qf * (double)col;
-        bR = box_rows(row); bC = box_cols(col);
-      }
-      // suffix sums along each cluster's lane list by pointer jumping: the first lane ends with the total
-      const u32 above = peers & (0xFFFFFFFEu << lane);
-      u32 nxt = above ? (u32)__ffs((int)above) - 1u : 32u;
-      for (u32 span = 1; span < most; span <<= 1) {
-        const u32 src = nxt & 31u;
-        const double a = __shfl_sync(0xFFFFFFFFu, qf, src), b = __shfl_sync(0xFFFFFFFFu, qx, src), c = __shfl_sync(0xFFFFFFFFu, qy, src);
-        const u32 nn = __shfl_sync(0xFFFFFFFFu, nxt, src);
-        const u32 r2 = __shfl_sync(0xFFFFFFFFu, bR, src), c2 = __shfl_sync(0xFFFFFFFFu, bC, src);
-        if (nxt < 32u) { qf += a; qx += b; qy += c; bR = __vmaxu2(bR, r2); bC = __vmaxu2(bC, c2); nxt = nn; }
-      }
-      if (in && (peers & lt) == 0u) {                 // one owner per cluster and chunk
-        double* a = acc + rk * 3u;
-        a[0] += qf; a[1] += qx; a[2] += qy;
-        u32* c = cb + rk * 3u;
-        c[0] += (u32)__popc(peers); c[1] = __vmaxu2(c[1], bR); c[2] = __vmaxu2(c[2], bC);
-      }
-      __syncwarp();
     }
+    __syncwarp();
     for (u32 k = lane; k < ((nAcc + 31u) & ~31u); k += 32u) {
-      double S = 0.0;
+      i64 S = 0;
       u32 root = 0, mr = 4u;
-      if (k < nAcc) { S = acc[k * 3u]; root = wr.rootAt[p0 + k]; mr = unit_module(bnd, root); }
-      const bool keptC = k < nAcc && __double2ll_rz(S) >= g.clusThrFixed;
+      const u32* a = acc + k * kAccWords;
+      if (k < nAcc) { S = (i64)((u64)a[0] | (u64)a[1] << 32); root = wr.rootAt[p0 + k]; mr = unit_module(bnd, root); }
+      const bool keptC = k < nAcc && S >= g.clusThrFixed;
       const u32 kb = __ballot_sync(0xFFFFFFFFu, keptC);
       u32 mine = 0;                                  // the kept roots of this chunk in my module; the roots come in ascending order
 #pragma unroll
@@ -442,7 +430,8 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
           const u32 before = mr == 0u ? cntOut[0] : mr == 1u ? cntOut[1] : mr == 2u ? cntOut[2] : cntOut[3];
           kr = before - (u32)__popc(mine) + (u32)__popc(mine & lt);
           const u32 o = s + (mr ? bnd.b[mr - 1u] : 0u) + kr;
-          stage_store(ev.staged + o, S, acc[k * 3u + 1u], acc[k * 3u + 2u], s + root, cb[k * 3u], cb[k * 3u + 1u], cb[k * 3u + 2u]);
+          stage_store(ev.staged + o, __ll2double_rn(S), __ll2double_rn((i64)((u64)a[2] | (u64)a[3] << 32)), __ll2double_rn((i64)((u64)a[4] | (u64)a[5] << 32)),
+                      s + root, a[6], a[7] << 16 | a[8], a[9] << 16 | a[10]);
         }
         krAt[2u * root] = (u16)kr;
       }
