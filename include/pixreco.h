@@ -280,6 +280,41 @@ int pr_occupancy_acquire(pr_event* ev, pr_product* digis, void* own_stream, void
 int pr_occupancy_produce(pr_event* ev, const uint32_t** d_count, const uint32_t** d_adc_sum,
                          const uint32_t** h_count, const uint32_t** h_adc_sum);
 
+/* ---- raw -> digis without any allocation (for callers that cannot reach cudaMalloc) --------------------------------
+ * The first step of the path — raw words -> digis + charge, the k_unpack of pr_acquire / pr_digis_acquire (the "raw to
+ * digi" step of the paper's Fig. 1; readings A1-A7) — as ONE call that allocates nothing, for code under CUDA
+ * graph capture, tight serving loops or harnesses that forbid cudaMalloc.  Inputs and outputs are the CALLER's device
+ * buffers on the handle's device; the kernel's scratch (launch control words, counters, one look-back state per
+ * 2048-word tile) is a file-scope __device__ array of pr_static_scratch_bytes() = 65792 bytes that every GPU holds from
+ * the moment it loads the library until exit, which bounds the input: n_words <= PR_STATIC_MAX_WORDS, beyond that
+ * PR_ERR_CAPACITY and nothing is enqueued.  The call enqueues one memset (what must start at zero is cleared on every
+ * call: the array keeps the last call's contents) and two kernels on `cuda_stream` and returns at once; it calls no
+ * cudaMalloc / cudaFree, no pool and no allocating library routine, and it waits for nothing.  Completion is the
+ * caller's business (its stream).  ALL calls on one device share the one array: two calls whose work overlaps on the
+ * GPU (different streams without an ordering between them) race on it — order them, or use pr_digis_acquire.
+ * Arguments: d_words [n_words] u32 and d_adc [n_words] u16 (device, 16-byte aligned, used in place; may be NULL when
+ * n_words == 0).  pr_digis_out: device buffers, every base 16-byte aligned, owned by the caller before and after:
+ * d_module, d_row, d_col, d_adc u16 [cap]; d_word_idx u32 [cap]; d_charge f32 [cap]; d_err_word, d_err_idx u32 [cap],
+ * cap = n_words rounded up to a multiple of 8 (at least 8); d_mod_digi_start u32 [n_modules + 1]; d_counters u32 [8]
+ * = {n_words, n_digis, n_errors, 0, 0, 0, status_bits, 0}.  Elements beyond n_digis / n_errors are not written.  The
+ * same values, bit for bit, as the digi part of pr_acquire (status bit 0 = PR_ERR_INPUT_ORDER: then
+ * d_mod_digi_start is undefined).  Returns PR_OK, PR_ERR_INVALID_ARG (NULL or misaligned pointer), PR_ERR_CAPACITY,
+ * PR_ERR_CUDA.  pr_static_setup looks the array's device address up (cudaGetSymbolAddress, once per device) ahead of
+ * the first call — pr_unpack_static does it itself otherwise; call it before a stream capture begins.              */
+#define PR_STATIC_MAX_WORDS (1u << 24)
+typedef struct pr_digis_out {
+  uint16_t *d_module, *d_row, *d_col, *d_adc;
+  uint32_t* d_word_idx;
+  float* d_charge;
+  uint32_t *d_err_word, *d_err_idx;
+  uint32_t* d_mod_digi_start;
+  uint32_t* d_counters;
+} pr_digis_out;
+size_t pr_static_scratch_bytes(void);
+int pr_static_setup(pr_handle* h);
+int pr_unpack_static(pr_handle* h, const uint32_t* d_words, const uint16_t* d_adc, uint32_t n_words, const pr_digis_out* out,
+                     void* cuda_stream);
+
 /* ---- pinned host memory from the handle's host pool, for inputs ---- */
 void* pr_host_alloc(pr_handle* h, size_t bytes);     /* NULL on failure */
 int   pr_host_free(pr_handle* h, void* p);

@@ -10,7 +10,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libpixreco.so")
 SOURCES = ["pixreco_api.cu", "pool.cpp"]
-DEPS = SOURCES + ["kernels.cuh", "common.cuh", "k_unpack.cuh", "k_cluster.cuh", "k_finalize.cuh", "k_chain.cuh", "k_bucket.cuh", "chain_api.cuh", "pool.hpp"]
+DEPS = SOURCES + ["kernels.cuh", "common.cuh", "k_unpack.cuh", "k_cluster.cuh", "k_finalize.cuh", "k_chain.cuh", "k_bucket.cuh", "chain_api.cuh", "static_api.cuh", "pool.hpp"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

@@ -1123,3 +1123,4 @@ int pr_get_stats(pr_handle* h, pr_stats* out) {
 }  // extern "C"
 
 #include "chain_api.cuh"
+#include "static_api.cuh"

@@ -89,6 +89,15 @@ class pr_stats(ctypes.Structure):
                  ("export_ms", ctypes.c_double)])
 
 
+PR_STATIC_MAX_WORDS = 1 << 24
+DIGIS_OUT_FIELDS = ("d_module", "d_row", "d_col", "d_adc", "d_word_idx", "d_charge", "d_err_word", "d_err_idx",
+                    "d_mod_digi_start", "d_counters")
+
+
+class pr_digis_out(ctypes.Structure):
+    _fields_ = [(n, c_void_p) for n in DIGIS_OUT_FIELDS]
+
+
 # every symbol include/pixreco.h declares: name -> (restype, argtypes)
 SIGNATURES = {
     "pr_create": (c_int, [POINTER(pr_config), POINTER(c_void_p)]),
@@ -117,6 +126,9 @@ SIGNATURES = {
     "pr_clusters_acquire": (c_int, [c_void_p, c_void_p, c_uint32, c_void_p, POINTER(c_void_p), pr_done_fn, c_void_p]),
     "pr_occupancy_acquire": (c_int, [c_void_p, c_void_p, c_void_p, POINTER(c_void_p), pr_done_fn, c_void_p]),
     "pr_occupancy_produce": (c_int, [c_void_p, POINTER(c_void_p), POINTER(c_void_p), POINTER(c_void_p), POINTER(c_void_p)]),
+    "pr_static_scratch_bytes": (c_size_t, []),
+    "pr_static_setup": (c_int, [c_void_p]),
+    "pr_unpack_static": (c_int, [c_void_p, c_void_p, c_void_p, c_uint32, POINTER(pr_digis_out), c_void_p]),
     "pr_pool_create": (c_int, [c_int, c_int, c_uint64, POINTER(c_void_p)]),
     "pr_pool_alloc": (c_void_p, [c_void_p, c_size_t, c_void_p]),
     "pr_pool_free": (c_int, [c_void_p, c_void_p, c_void_p, c_int]),
@@ -487,6 +499,15 @@ class PixReco:
     def host_free(self, arr_or_ptr):
         p = arr_or_ptr.ctypes.data if isinstance(arr_or_ptr, np.ndarray) else arr_or_ptr
         _check(lib().pr_host_free(self.handle, c_void_p(p)), "pr_host_free", self.handle)
+
+    def unpack_static(self, words, adc, out: dict, stream=0, n_words=None) -> int:
+        """pr_unpack_static: raw words -> digis into the caller's CUDA tensors ``out[name]`` (names: DIGIS_OUT_FIELDS),
+        no allocation anywhere; returns the C return code (PR_OK, or an error such as PR_ERR_CAPACITY) without raising."""
+        n = int(words.shape[0]) if n_words is None else int(n_words)
+        o = pr_digis_out(*[c_void_p(_ptr(out[k])) for k in DIGIS_OUT_FIELDS])
+        return lib().pr_unpack_static(self.handle, c_void_p(_ptr(words)) if words is not None and int(words.shape[0]) else None,
+                                      c_void_p(_ptr(adc)) if adc is not None and int(adc.shape[0]) else None, n, ctypes.byref(o),
+                                      c_void_p(getattr(stream, "cuda_stream", stream)))
 
     def stats(self) -> dict:
         st = pr_stats()
