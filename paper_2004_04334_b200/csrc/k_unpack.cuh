@@ -24,16 +24,20 @@ namespace pixreco {
 //           back, the aggregate has long been there: no CTA waits for the progress of another one
 //   scatter tile i: its event-global digi offset g0 is known (look-back resolved in iteration
 //           i - 1).  Warp w owns words [256w, 256w + 256) of the tile, lane l word 32j + l of row j:
-//           position = g0 + warp prefix + row prefix + popc(ballot below lane).  The digi is stored
-//           in FINAL form (module,row,col,adc u16; wordIdx u32; charge f32 = fmaf, A7) into six
-//           shared-memory arrays at index 8 + (g0 & 7) + position, i.e. with the 16-byte phase of
-//           its global destination; error words (rare) go straight to global memory
+//           position = g0 + warp prefix + row prefix + popc(ballot below lane).  The digi's four
+//           16-bit fields (module,row,col,adc) are stored in FINAL form into four shared-memory
+//           arrays at index 8 + (g0 & 7) + position, i.e. with the 16-byte phase of their global
+//           destination; its two 32-bit fields (wordIdx; charge = fmaf, A7) go straight to global
+//           memory — consecutive lanes hold consecutive digis, so a warp's row is one contiguous
+//           run of 4-byte stores — which keeps the CTA at 69 KB of shared memory and 64 registers:
+//           three CTAs per SM with the full four-slot ring; error words (rare) go straight to
+//           global memory too
 //   look-back (warp 0) for tile i + 1: loads issued before the scatter, resolved after it
-//   store   one thread issues six TMA bulk stores of the 16-byte-aligned middle of the staged
+//   store   one thread issues four TMA bulk stores of the 16-byte-aligned middle of the staged
 //           arrays; sixteen lanes store the up-to-7 head and tail elements; all threads scan the
 //           staged module array for module boundaries (modDigiStart) and order violations (A5)
 // Algorithmic HBM bytes per event: 6W read + 16D (digi SoA incl. charge) + 8E written.
-constexpr int kUnpackCtasPerSM = 2;
+constexpr int kUnpackCtasPerSM = 3;
 constexpr int kRawSlots = 4;                      // raw tiles in the shared-memory ring
 constexpr int kCountAhead = 2;                    // a tile is counted this many iterations before it is written
 constexpr int kDescRing = 8;                      // descriptor / tile-index ring, power of two >= kRawSlots + 4
@@ -48,8 +52,6 @@ struct __align__(128) UnpackShared {
   u32 words[kRawSlots][kTileWords];               // raw ring (TMA destination)
   u16 adc[kRawSlots][kTileWords];
   u16 sModule[kStageElems], sRow[kStageElems], sCol[kStageElems], sAdc[kStageElems];   // staging (TMA source)
-  u32 sWordIdx[kStageElems];
-  float sCharge[kStageElems];
   u64 full[kRawSlots];                            // mbarriers: raw slot filled
   u32 bal[kRawSlots][8][8];                       // [slot][warp][row] validity ballots
   u32 wcnt[kRawSlots][8], wmax[kRawSlots][8];     // per warp: digis, max(module)+1
@@ -245,8 +247,10 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
           const u32 mod = x >> 20;
           const float2 gp = __ldg(g.calib + mod);
           sh.sModule[el] = (u16)mod; sh.sRow[el] = (u16)((x >> 12) & 0xFFu); sh.sCol[el] = (u16)((x >> 3) & 0x1FFu);
-          sh.sAdc[el] = (u16)a; sh.sWordIdx[el] = wi0 + 32u * j;
-          sh.sCharge[el] = __fmaf_rn((float)a, gp.x, gp.y);
+          sh.sAdc[el] = (u16)a;
+          // (the two 4-byte arrays go straight to global memory: consecutive lanes hold consecutive digis)
+          const u32 p = g0 + (el - 8u - ph);
+          e.wordIdx[p] = wi0 + 32u * j; e.charge[p] = __fmaf_rn((float)a, gp.x, gp.y);
         } else if (256u * warp + 32u * j + lane < nIn) {
           // error word (A2-A4): errors before it = words before it - digis before it
           const u32 ei = (wi0 + 32u * j) - (g0 + (el - 8u - ph));
@@ -268,7 +272,6 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
             const u32 cnt = midHi - midLo, se = 8u + ph + (midLo - g0);
             bulk_store(e.module + midLo, sh.sModule + se, cnt * 2u); bulk_store(e.row + midLo, sh.sRow + se, cnt * 2u);
             bulk_store(e.col + midLo, sh.sCol + se, cnt * 2u); bulk_store(e.adcOut + midLo, sh.sAdc + se, cnt * 2u);
-            bulk_store(e.wordIdx + midLo, sh.sWordIdx + se, cnt * 4u); bulk_store(e.charge + midLo, sh.sCharge + se, cnt * 4u);
           }
           bulk_commit();
         }
@@ -278,7 +281,6 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
           if (k < n && (lane < 8u || k >= 8u) && !(p >= midLo && p < midHi)) {
             const u32 se = lo + k;
             e.module[p] = sh.sModule[se]; e.row[p] = sh.sRow[se]; e.col[p] = sh.sCol[se]; e.adcOut[p] = sh.sAdc[se];
-            e.wordIdx[p] = sh.sWordIdx[se]; e.charge[p] = sh.sCharge[se];
           }
         }
         --inflight;
