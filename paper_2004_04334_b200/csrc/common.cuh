@@ -31,14 +31,15 @@ constexpr u32 kMaxModuleDigis = (1u << 17) - 1u;   // A9: the exact sums are ove
 struct DevCounters {
   u32 nWords, nDigis, nErrors, nKept, nClustersAll, nClusters, status, pad;
 };
-// Per-launch control words.  The first two are put back to zero by the last CTA of k_unpack (with the look-back
-// states); the rest is zeroed per acquire together with the counters.
+// Per-launch control words.  The first two and unpackStarted are put back to zero by the last CTA of k_unpack (with the
+// look-back states); the rest is zeroed per acquire together with the counters.
 struct LaunchCtl {
   u32 tileTicket, unpackExited;     // k_unpack: next tile of the launch, CTAs that have left
   u32 modTicket, modDone;           // k_cluster: next warp ticket
   u64 tStart;                       // %globaltimer at the start of the acquire's first kernel
   u32 nBig, bigTicket;              // modules handed from k_cluster to k_dense, next one to take
-  u32 pad[8];
+  u32 unpackStarted;                // k_unpack: CTAs that have started (put back to zero with the ticket)
+  u32 pad[7];
 };
 // What the host reads after completion (mapped pinned memory, written by the CTA that finishes the event).
 struct HostCounters {

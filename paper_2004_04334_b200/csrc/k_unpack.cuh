@@ -43,6 +43,7 @@ constexpr int kCountAhead = 2;                    // a tile is counted this many
 constexpr int kDescRing = 8;                      // descriptor / tile-index ring, power of two >= kRawSlots + 4
 constexpr int kDrawAhead = 6;                     // a ticket drawn in iteration i becomes local tile i + kDrawAhead
 constexpr u32 kTilesFromDesc = 0xFFFFFFFDu;       // totalTiles argument of a graph launch: take nTiles of the (one) event
+constexpr u64 kStartWaitNs = 20000;               // upper bound of the wait for the rest of the grid at the start of a CTA
 constexpr u32 kTileSkip = 0xFFFFFFFEu, kTileEnd = 0xFFFFFFFFu;   // pipeline slot without a tile: a bubble / no more tiles
 constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
 static_assert(kCountAhead >= 1 && kCountAhead <= kRawSlots - 2, "a raw tile needs a full iteration to arrive before it is counted");
@@ -142,6 +143,15 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
 #pragma unroll
     for (u32 j = 0; j < (u32)kDescRing; ++j) sh.tile[j] = j == 0u ? (t0 < totalTiles ? t0 : kTileEnd) : (j < (u32)kDrawAhead && t0 < totalTiles ? kTileSkip : kTileEnd);
     sh.last = 0u;
+    // The CTAs of the launch start their pipelines together.  A CTA that starts alone — the grid arrives piecemeal when
+    // it follows another stream's kernel whose CTAs retire one by one — runs through its empty pipeline slots in no
+    // time and draws a BLOCK of consecutive tickets; its successors' first look-backs then wait for its later
+    // iterations, a chain through the whole grid (measured: 0.49-0.54 ms instead of 0.30 ms for the 256-event batch
+    // behind a k_cluster of the other stream).  The wait is bounded: nothing depends on it, and a grid that is not
+    // co-resident (beside other kernels, or oversubscribed on purpose) goes on after kStartWaitNs.
+    atomicAdd(&lc->unpackStarted, 1u);
+    const u64 tw = global_timer();
+    while (*reinterpret_cast<volatile u32*>(&lc->unpackStarted) < gridDim.x && global_timer() - tw < kStartWaitNs) {}
   }
   __syncthreads();
   if (!kSingle && (int)warp < kDrawAhead && tile_of((int)warp) < totalTiles)
@@ -387,7 +397,7 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
   if (sh.last) {
     __threadfence();
     for (u32 t = tid; t < totalTiles; t += kUnpackThreads + 64) tileStateAll[t] = 0ull;
-    if (tid == 0) { lc->tileTicket = 0u; lc->unpackExited = 0u; }
+    if (tid == 0) { lc->tileTicket = 0u; lc->unpackExited = 0u; lc->unpackStarted = 0u; }
   }
 }
 
