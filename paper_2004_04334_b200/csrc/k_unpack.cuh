@@ -43,6 +43,7 @@ constexpr int kCountAhead = 2;                    // a tile is counted this many
 constexpr int kDescRing = 8;                      // descriptor / tile-index ring, power of two >= kRawSlots + 4
 constexpr int kDrawAhead = 6;                     // a ticket drawn in iteration i becomes local tile i + kDrawAhead
 constexpr u32 kTilesFromDesc = 0xFFFFFFFDu;       // totalTiles argument of a graph launch: take nTiles of the (one) event
+constexpr u32 kStartWaitGrid = 128;               // launches with at least this many CTAs wait for one another at the start
 constexpr u64 kStartWaitNs = 20000;               // upper bound of the wait for the rest of the grid at the start of a CTA
 constexpr u32 kTileSkip = 0xFFFFFFFEu, kTileEnd = 0xFFFFFFFFu;   // pipeline slot without a tile: a bubble / no more tiles
 constexpr u32 kStageElems = kTileWords + 32;      // 8 front pad + phase (< 8) + tile, multiple of 8
@@ -149,9 +150,12 @@ k_unpack(const __grid_constant__ EvDesc single, const EvDesc* __restrict__ batch
     // iterations, a chain through the whole grid (measured: 0.49-0.54 ms instead of 0.30 ms for the 256-event batch
     // behind a k_cluster of the other stream).  The wait is bounded: nothing depends on it, and a grid that is not
     // co-resident (beside other kernels, or oversubscribed on purpose) goes on after kStartWaitNs.
-    atomicAdd(&lc->unpackStarted, 1u);
-    const u64 tw = global_timer();
-    while (*reinterpret_cast<volatile u32*>(&lc->unpackStarted) < gridDim.x && global_timer() - tw < kStartWaitNs) {}
+    // (a small launch — a single event — has no chain worth the wait)
+    if (gridDim.x >= kStartWaitGrid) {
+      atomicAdd(&lc->unpackStarted, 1u);
+      const u64 tw = global_timer();
+      while (*reinterpret_cast<volatile u32*>(&lc->unpackStarted) < gridDim.x && global_timer() - tw < kStartWaitNs) {}
+    }
   }
   __syncthreads();
   if (!kSingle && (int)warp < kDrawAhead && tile_of((int)warp) < totalTiles)
