@@ -181,6 +181,26 @@ def _oracle_worker(args):
             return n, d, dt
 
 
+_REF = {}     # the reference arm's events and calibration: set before the fork, inherited by the worker processes
+
+
+def _ref_worker(args):
+    """One step's share of one process of the reference arm: its own `per_proc` events (inherited through the fork, no
+    copy per step), the oracle's workspace kept across steps.  Returns (events, digis)."""
+    import oracle
+    i, per_proc = args
+    events, cal = _REF["pool"][i * per_proc:(i + 1) * per_proc], _REF["cal"]
+    ws = _REF.get("ws")
+    if ws is None:
+        ws = _REF["ws"] = oracle.Workspace(max(e.n_words for e in _REF["pool"]), cal.n_modules)
+    d = 0
+    for e in events:
+        oracle.run_raw(e.words, e.adc, e.n_modules, e.n_rows, e.n_cols, cal.gain, cal.pedestal,
+                       cal.pixel_threshold_e, cal.cluster_threshold_e, ws)
+        d += int(ws.counters[0])
+    return len(events), d
+
+
 def oracle_rates(pool, cal, budget_s, cores):
     """The oracle as it stands on 1 core and on `cores` cores (one independent process per core, each over its own
     slice of `pool`; if the pool has fewer events than cores the slices repeat, said in `sample`)."""
@@ -209,19 +229,20 @@ def run_reference(args, rank):
     import multiprocessing as mp
     cores = os.cpu_count() or 1
     cal = wl.make_calib(HEAD_CONFIG)
-    per_proc = 2
+    per_proc = 8
     pool = make_pool(wl, HEAD_CONFIG, cores * per_proc)
+    _REF["pool"], _REF["cal"] = pool, cal
     sample = len(pool)                                      # events per step: every process does `per_proc` events
     steps, warm = min(args.steps, 40), min(max(args.warmup, 1), 3)
     ctx = mp.get_context("fork")
     with ctx.Pool(cores) as p:
-        jobs = [(pool[i * per_proc:(i + 1) * per_proc], cal, 0.0, per_proc) for i in range(cores)]
+        jobs = [(i, per_proc) for i in range(cores)]
         for _ in range(warm):
-            p.map(_oracle_worker, jobs)
+            p.map(_ref_worker, jobs, chunksize=1)
         t0 = time.perf_counter()
         digis = 0
         for _ in range(steps):
-            digis += sum(o[1] for o in p.map(_oracle_worker, jobs))
+            digis += sum(o[1] for o in p.map(_ref_worker, jobs, chunksize=1))
         dt = time.perf_counter() - t0
     v = sample * steps / dt
     line = {"impl": "reference", "metric": "pixel-reco events/s", "value": v, "unit": "events/s", "n_gpus": args.gpus,
