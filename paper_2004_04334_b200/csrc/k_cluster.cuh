@@ -394,29 +394,25 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
     const u32 nAcc = min(nR - p0, kAccRoots);
     for (u32 i = lane; i < nAcc * kAccWords; i += 32u) acc[i] = 0u;
     __syncwarp();
-    for (u32 i = lane; i < nPad; i += 32u) {
+    // Lane l takes the digis [l c, (l + 1) c) (c = chunks of the unit), not every 32nd one: neighbouring digis mostly
+    // share their cluster, and 32 lanes that add to the same few words in one instruction are served one after the
+    // other.  The lanes start at different offsets inside their blocks (rotated by l / (32 / gcd(c, 32))), which
+    // puts the 32 loads of an instruction in 32 different banks.
+    const u32 cN = nPad >> 5, aN = min((u32)__ffs((int)cN) - 1u, 5u), offN = lane >> (5u - aN);
+    for (u32 kk = 0; kk < cN; ++kk) {
+      u32 t = kk + offN;
+      if (t >= cN) t -= cN;
+      const u32 i = lane * cN + t;
       const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
-      u32 rk = 0xFFFFFF00u + lane;                      // (no cluster of this pass: a key of its own)
       if (x != kNoKey) {
-        const u32 k = (u32)wr.rk[rootOf[2u * i]] - p0;
-        if (k < nAcc) rk = k;
-      }
-      // Neighbouring lanes hold neighbouring digis, which mostly share their cluster: of such a pair the even lane
-      // takes the size and the box for both (half of these atomics, which all meet on the cluster's words).
-      const u32 ork = __shfl_xor_sync(0xFFFFFFFFu, rk, 1), ox = __shfl_xor_sync(0xFFFFFFFFu, x, 1);
-      if (rk < nAcc) {
-        const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
-        const u64 qf = (u64)__float2ll_rz((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
-        u32* a = acc + rk * kAccWords;
-        acc_add64(a, qf); acc_add64(a + 2, qf * row); acc_add64(a + 4, qf * col);
-        if (ork != rk) {
+        const u32 rk = (u32)wr.rk[rootOf[2u * i]] - p0;
+        if (rk < nAcc) {
+          const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
+          const u64 qf = (u64)__float2ll_rz((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
+          u32* a = acc + rk * kAccWords;
+          acc_add64(a, qf); acc_add64(a + 2, qf * row); acc_add64(a + 4, qf * col);
           atomicAdd(a + 6, 1u);
           atomicMax(a + 7, 255u - row); atomicMax(a + 8, row); atomicMax(a + 9, 511u - col); atomicMax(a + 10, col);
-        } else if (!(lane & 1u)) {
-          const u32 orow = (ox >> 9) & 0x1FFu, ocol = ox & 511u;
-          atomicAdd(a + 6, 2u);
-          atomicMax(a + 7, 255u - min(row, orow)); atomicMax(a + 8, max(row, orow));
-          atomicMax(a + 9, 511u - min(col, ocol)); atomicMax(a + 10, max(col, ocol));
         }
       }
     }
