@@ -259,6 +259,7 @@ __device__ __forceinline__ u32 wm_find(const idx_t* L, u32 x) {
 // acc[0..1] += v as a 64-bit integer with native 32-bit shared-memory atomics: the add on the low word returns what was
 // there, so this thread knows whether ITS add carried, and takes the carry along with its high word.
 constexpr u32 kAccWords = 11;
+constexpr u32 kMomentOff = 8;                     // Sx, Sy are accumulated relative to (root row - 8, root col - 8)
 __device__ __forceinline__ void acc_add64(u32* a, u64 v) {
   const u32 lo = (u32)v;
   u32 hi = (u32)(v >> 32);
@@ -405,12 +406,17 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
       const u32 i = lane * cN + t;
       const u32 x = (!kMedium || i < n) ? wr.info[i] : kNoKey;
       if (x != kNoKey) {
-        const u32 rk = (u32)wr.rk[rootOf[2u * i]] - p0;
+        const u32 r = rootOf[2u * i], rk = (u32)wr.rk[r] - p0;
         if (rk < nAcc) {
           const u32 row = (x >> 9) & 0x1FFu, col = x & 511u;
-          const u64 qf = (u64)__float2ll_rz((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
+          const i64 qf = __float2ll_rz((kMedium ? ev.charge[s + i] : wr.q[i]) * 16384.0f);
+          // Sx and Sy are taken relative to the cluster's root pixel (kMomentOff rows / columns before it): the products
+          // then stay below 2^32 as a rule and their high words are zero, i.e. one atomic instead of two (any other
+          // value is still added exactly, as a 64-bit integer modulo 2^64; P6 adds the root's share back)
+          const u32 x0 = wr.info[r];
+          const int dr = (int)(row + kMomentOff) - (int)((x0 >> 9) & 0x1FFu), dc = (int)(col + kMomentOff) - (int)(x0 & 511u);
           u32* a = acc + rk * kAccWords;
-          acc_add64(a, qf); acc_add64(a + 2, qf * row); acc_add64(a + 4, qf * col);
+          acc_add64(a, (u64)qf); acc_add64(a + 2, (u64)(qf * dr)); acc_add64(a + 4, (u64)(qf * dc));
           atomicAdd(a + 6, 1u);
           atomicMax(a + 7, 255u - row); atomicMax(a + 8, row); atomicMax(a + 9, 511u - col); atomicMax(a + 10, col);
         }
@@ -438,8 +444,10 @@ __device__ __forceinline__ void warp_module(const EvDesc& ev, const Geom& g, u32
           const u32 before = mr == 0u ? cntOut[0] : mr == 1u ? cntOut[1] : mr == 2u ? cntOut[2] : cntOut[3];
           kr = before - (u32)__popc(mine) + (u32)__popc(mine & lt);
           const u32 o = s + (mr ? bnd.b[mr - 1u] : 0u) + kr;
-          stage_store(ev.staged + o, __ll2double_rn(S), __ll2double_rn((i64)((u64)a[2] | (u64)a[3] << 32)), __ll2double_rn((i64)((u64)a[4] | (u64)a[5] << 32)),
-                      s + root, a[6], a[7] << 16 | a[8], a[9] << 16 | a[10]);
+          const u32 x0 = wr.info[root];
+          const i64 Sx = (i64)((u64)a[2] | (u64)a[3] << 32) + ((i64)((x0 >> 9) & 0x1FFu) - (i64)kMomentOff) * S;
+          const i64 Sy = (i64)((u64)a[4] | (u64)a[5] << 32) + ((i64)(x0 & 511u) - (i64)kMomentOff) * S;
+          stage_store(ev.staged + o, __ll2double_rn(S), __ll2double_rn(Sx), __ll2double_rn(Sy), s + root, a[6], a[7] << 16 | a[8], a[9] << 16 | a[10]);
         }
         krAt[2u * root] = (u16)kr;
       }
