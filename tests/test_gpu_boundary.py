@@ -205,7 +205,7 @@ def test_consumer_on_another_stream_waits_on_the_product_event(pr):
         charge_ptr, n = out0.raw.d_charge, out0.n_digis
         slot.release()
         with torch.cuda.stream(prod):
-            torch.cuda._sleep(int(0.02 * 1.5e9))
+            torch.cuda._sleep(int(0.1 * 2.0e9))                   # ~0.1 s of queue ahead of the producer
         slot.acquire(w, a, stream=prod)
         assert slot.query() == pr.PR_NOT_READY
         assert slot.stream_wait(cons) == 0                      # cudaStreamWaitEvent, no host wait

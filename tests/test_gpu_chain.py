@@ -54,43 +54,51 @@ def test_two_branch_dag_without_a_host_wait(pr, config, event, over):
         prod, clus, occ = p.slot(), p.slot(), p.slot()
         w, a = to_dev(ev.words), to_dev(ev.adc)
         s0, s1, s2 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
-        torch.cuda.synchronize()
-        with torch.cuda.stream(s0):
-            torch.cuda._sleep(400_000_000)                                 # ~0.2 s of queue ahead of the producer
-        prod.digis_acquire(w, a, stream=s0, event_id=77)
-        product = prod.digis_product()
-        used1 = clus.clusters_acquire(product, want=pr.PR_WANT_ALL, own_stream=s1)
-        used2 = occ.occupancy_acquire(product, own_stream=s2)
-        assert prod.query() == pr.PR_NOT_READY, "the producer was complete before its consumers were enqueued: test proves nothing"
-        # ScopedContext rule: first consumer on the producer's stream, second on its own
-        assert used1 == s0.cuda_stream and used2 == s2.cuda_stream
-        dev, st, evt = ctypes.c_int32(), ctypes.c_void_p(), ctypes.c_void_p()
-        assert pr.lib().pr_product_info(ctypes.c_void_p(product), ctypes.byref(dev), ctypes.byref(st), ctypes.byref(evt)) == 0
-        assert dev.value == 0 and (st.value or 0) == s0.cuda_stream and evt.value == prod.cuda_event
-        # produce of a consumer is PR_NOT_READY while early, and the producer cannot be released under its consumers
-        assert clus.produce()[0] == pr.PR_NOT_READY and occ.occupancy_produce()[0] == pr.PR_NOT_READY
-        wait(prod); wait(clus); wait(occ)
-        assert prod.release() == pr.PR_NOT_READY
+        # Two passes: the first one fills the handle's pools (a fresh handle's first pinned and device allocations can
+        # take longer than any delay one would want to queue: on a cold box they used to outlast the 0.2 s below once in
+        # a while), the second one is the one that proves the point — it allocates nothing, so the host gets through
+        # its three acquires long before the delay ahead of the producer is over.
+        for delayed in (False, True):
+            torch.cuda.synchronize()
+            if delayed:
+                with torch.cuda.stream(s0):
+                    torch.cuda._sleep(1_000_000_000)                           # ~0.5 s of queue ahead of the producer
+            prod.digis_acquire(w, a, stream=s0, event_id=77)
+            product = prod.digis_product()
+            used1 = clus.clusters_acquire(product, want=pr.PR_WANT_ALL, own_stream=s1)
+            used2 = occ.occupancy_acquire(product, own_stream=s2)
+            if delayed:
+                assert prod.query() == pr.PR_NOT_READY, "the producer was complete before its consumers were enqueued: test proves nothing"
+            # ScopedContext rule: first consumer on the producer's stream, second on its own
+            assert used1 == s0.cuda_stream and used2 == s2.cuda_stream
+            dev, st, evt = ctypes.c_int32(), ctypes.c_void_p(), ctypes.c_void_p()
+            assert pr.lib().pr_product_info(ctypes.c_void_p(product), ctypes.byref(dev), ctypes.byref(st), ctypes.byref(evt)) == 0
+            assert dev.value == 0 and (st.value or 0) == s0.cuda_stream and evt.value == prod.cuda_event
+            # produce of a consumer is PR_NOT_READY while early, and the producer cannot be released under its consumers
+            if delayed:
+                assert clus.produce()[0] == pr.PR_NOT_READY and occ.occupancy_produce()[0] == pr.PR_NOT_READY
+            wait(prod); wait(clus); wait(occ)
+            assert prod.release() == pr.PR_NOT_READY
 
-        code, dout = prod.produce()
-        assert code == 0 and dout.event_id == 77 and dout.n_clusters == 0 and not dout.raw.d_cl_label
-        check_digis(dout, ref, dout.to_numpy)
-        code, cout = clus.produce()
-        assert code == 0 and cout.event_id == 77
-        compare(cout, ref, cout.host)                                      # pinned mirrors of every array
-        compare(cout, ref, cout.to_numpy)                                  # device views
-        code, cnt, tot = occ.occupancy_produce()
-        assert code == 0
-        ocnt, otot = oracle.occupancy(ref.module, ref.adc, ref.kept, ev.n_modules)
-        assert np.array_equal(cnt, ocnt) and np.array_equal(tot, otot)
-        assert int(cnt.sum()) == ref.n_kept_digis
+            code, dout = prod.produce()
+            assert code == 0 and dout.event_id == 77 and dout.n_clusters == 0 and not dout.raw.d_cl_label
+            check_digis(dout, ref, dout.to_numpy)
+            code, cout = clus.produce()
+            assert code == 0 and cout.event_id == 77
+            compare(cout, ref, cout.host)                                      # pinned mirrors of every array
+            compare(cout, ref, cout.to_numpy)                                  # device views
+            code, cnt, tot = occ.occupancy_produce()
+            assert code == 0
+            ocnt, otot = oracle.occupancy(ref.module, ref.adc, ref.kept, ev.n_modules)
+            assert np.array_equal(cnt, ocnt) and np.array_equal(tot, otot)
+            assert int(cnt.sum()) == ref.n_kept_digis
 
-        assert clus.release() == 0
-        assert prod.release() == pr.PR_NOT_READY                           # the occupancy consumer still holds it
-        assert occ.release() == 0
-        assert prod.release() == 0
+            assert clus.release() == 0
+            assert prod.release() == pr.PR_NOT_READY                           # the occupancy consumer still holds it
+            assert occ.release() == 0
+            assert prod.release() == 0
         st = p.stats()
-        assert st["events_acquired"] == 1 and st["events_produced"] == 1 and st["digis"] == ref.n_digis and st["clusters"] == ref.n_clusters
+        assert st["events_acquired"] == 2 and st["events_produced"] == 2 and st["digis"] == 2 * ref.n_digis and st["clusters"] == 2 * ref.n_clusters
 
 
 def test_first_come_takes_the_stream_whatever_the_module(pr):
