@@ -63,7 +63,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--slots", type=int, default=2, help="batches in flight, device-resident (two keep the GPU busy back to back; with three the "
-                                                         "kernels of different batches share the SMs and every batch takes 9 %% longer)")
+                                                         "third buys nothing: 1 %% slower)")
     ap.add_argument("--e2e-slots", type=int, default=3, help="batches in flight, end to end (the PCIe copies of one batch overlap the kernels of others)")
     ap.add_argument("--no-extra", action="store_true", help="skip roofline.by_config and the all-config CPU baseline")
     ap.add_argument("--only", default=None, choices=["configs1", "configs3", "configs4"],
